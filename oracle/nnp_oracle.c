@@ -1,0 +1,557 @@
+/*
+ * nnp_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU statement of what the ANI-2x energy/force/MD hot path computes
+ * (FeNNol paper, arxiv 2405.01491, /root/reference/PAPER.md; Fig. 2, SecII.A,
+ * SecII.B, SecV, Eq. (A9)/L443 for the angular symmetry function).  The paper never
+ * prints the ANI equations or constants, so the step-by-step definition followed here is
+ * SURVEY.md Sec.8(c) C1 (O1..O7) with the readings of Sec.8(c) C2 -- each function cites its item.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+ * load this file.  It shares no code, header, table or helper with the CUDA path under
+ * paper_2405_01491_b200/csrc/.  There is no blocking, fusion or reordering beyond what the
+ * definition states: neighbours by brute force (or an independent, separately tested uniform
+ * grid for large N), direct sums for the AEV, a textbook MLP, an analytic gradient that the
+ * tests pin with central finite differences.
+ *
+ * Parity pins (tests/test_oracle_*.py): AEV length closed form, hand-evaluated dimer/trimer
+ * values, MLP vs numpy matmul, finite differences, net force / net torque zero, translation,
+ * rotation, lattice-shift, wrap and same-species permutation invariance, cutoff continuity,
+ * box replication extensivity, ensemble and batch identities, velocity-Verlet reversibility
+ * and dt^2 energy error.  Absolute values against the paper: "parity unpinned" (the paper
+ * prints none for this path; SURVEY.md Sec.8(c) C3 last row).
+ *
+ * Build:  gcc -O2 -std=c99 -ffp-contract=off -fopenmp -shared -fPIC nnp_oracle.c -lm
+ * Units: kcal/mol, Angstrom, fs, amu (reading B6).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+typedef struct {
+    int n_species;          /* S = 7 for ANI-2x (H,C,N,O,S,F,Cl = 0..6, reading B2) */
+    double rcr, rca;        /* radial / angular cutoff (5.1 / 3.5 A, reading A1) */
+    double eta_r;           /* radial Gaussian width */
+    int n_shf_r;            /* 16 */
+    const double *shf_r;
+    double eta_a, zeta;     /* angular */
+    int n_shf_a;            /* 8 */
+    const double *shf_a;
+    int n_shf_z;            /* 4 */
+    const double *shf_z;
+    double celu_alpha;      /* 0.1 */
+    int n_nets;             /* 1 or 8 (reading B5: arithmetic mean) */
+    int n_layers;           /* affine layers per network (4) */
+    const int *widths;      /* [S][n_layers+1] */
+    const double *params;   /* flat: for net, for species, for layer: W[in][out] row-major, then b[out] */
+    const double *self_energy; /* [S] or NULL (reading B4) */
+} orc_model;
+
+/* ---- closed-form sizes (SURVEY 8(c) C3 "AEV length") ------------------------------------- */
+int orc_n_pairs(int S) { return S * (S + 1) / 2; }
+int orc_aev_len(const orc_model *m)
+{
+    return m->n_species * m->n_shf_r + orc_n_pairs(m->n_species) * m->n_shf_a * m->n_shf_z;
+}
+/* O3: p(s,t), s<=t, row-major upper triangle: row s starts at sum_{u<s}(S-u). */
+int orc_pair_index(int S, int s, int t)
+{
+    if (s > t) { int u = s; s = t; t = u; }
+    return s * (2 * S + 1 - s) / 2 + (t - s);
+}
+long orc_params_per_net(const orc_model *m)
+{
+    long tot = 0;
+    for (int s = 0; s < m->n_species; ++s)
+        for (int l = 0; l < m->n_layers; ++l) {
+            long in = m->widths[s * (m->n_layers + 1) + l], out = m->widths[s * (m->n_layers + 1) + l + 1];
+            tot += in * out + out;
+        }
+    return tot;
+}
+static const double *layer_ptr(const orc_model *m, int net, int s, int l)
+{
+    long off = net * orc_params_per_net(m);
+    for (int u = 0; u < m->n_species; ++u)
+        for (int k = 0; k < m->n_layers; ++k) {
+            if (u == s && k == l) return m->params + off;
+            long in = m->widths[u * (m->n_layers + 1) + k], out = m->widths[u * (m->n_layers + 1) + k + 1];
+            off += in * out + out;
+        }
+    return NULL;
+}
+
+/* ---- O1: neighbours ---------------------------------------------------------------------- */
+/* fp64 minimum-image displacement d = x_j - x_i (reading C1: cubic/orthorhombic box, min image). */
+static void disp(const double *xi, const double *xj, const double *box, double d[3])
+{
+    for (int c = 0; c < 3; ++c) {
+        d[c] = xj[c] - xi[c];
+        if (box && box[c] > 0.0) d[c] -= box[c] * round(d[c] / box[c]);
+    }
+}
+
+/* Reading A3: the DEFINED list-membership predicate is fp32 with a fixed operation order:
+ *   dx = xj - xi (rn); dx = dx - L*rintf(dx*invL) (separate rn mul, rn mul, rn sub; invL = 1.0f/L);
+ *   r2 = (dx*dx + dy*dy) + dz*dz (each op rn, no FMA); member iff r2 < rlist*rlist (rn product).
+ * This file is compiled with -ffp-contract=off so no operation below is fused. */
+static int within_f32(const float *xi, const float *xj, const float *L, const float *invL, float rl2)
+{
+    float d[3];
+    for (int c = 0; c < 3; ++c) {
+        float t = xj[c] - xi[c];
+        if (L[c] > 0.0f) {
+            float q = t * invL[c];
+            float k = rintf(q);
+            float s = L[c] * k;
+            t = t - s;
+        }
+        d[c] = t;
+    }
+    float a = d[0] * d[0];
+    float b = d[1] * d[1];
+    float c2 = d[2] * d[2];
+    float r2 = (a + b) + c2;
+    return r2 < rl2;
+}
+
+/* Brute force O(N^2): directed list (each pair twice); same molecule only.
+ * fp32_pred=0: fp64 r2 < rcut^2; fp32_pred=1: reading A3 with rlist = (float)rcut.
+ * Returns max row length, or -(needed) if some row exceeds cap (list then truncated). */
+int orc_neighbors_brute(int n, const double *xyz, const double *box, const int *mol_id, double rcut,
+                        int fp32_pred, int cap, int *counts, int *list)
+{
+    float Lf[3] = {0, 0, 0}, invL[3] = {0, 0, 0};
+    if (box) for (int c = 0; c < 3; ++c) { Lf[c] = (float)box[c]; invL[c] = Lf[c] > 0 ? 1.0f / Lf[c] : 0.0f; }
+    float rl = (float)rcut;
+    float rl2 = rl * rl;
+    int maxc = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(max : maxc)
+    for (int i = 0; i < n; ++i) {
+        int c = 0;
+        float xi[3] = {(float)xyz[3 * i], (float)xyz[3 * i + 1], (float)xyz[3 * i + 2]};
+        for (int j = 0; j < n; ++j) {
+            if (j == i) continue;
+            if (mol_id && mol_id[i] != mol_id[j]) continue;
+            int in;
+            if (fp32_pred) {
+                float xj[3] = {(float)xyz[3 * j], (float)xyz[3 * j + 1], (float)xyz[3 * j + 2]};
+                in = within_f32(xi, xj, Lf, invL, rl2);
+            } else {
+                double d[3];
+                disp(xyz + 3 * i, xyz + 3 * j, box, d);
+                in = (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]) < rcut * rcut;
+            }
+            if (in) { if (c < cap) list[(long)i * cap + c] = j; ++c; }
+        }
+        counts[i] = c;
+        if (c > maxc) maxc = c;
+    }
+    return maxc > cap ? -maxc : maxc;
+}
+
+/* Uniform grid for large periodic N (SURVEY 8(d) "Oracle timing"): bins of edge >= rcut, every atom
+ * tests the atoms of all DISTINCT bins within +-1 in each dimension with the same predicate as the
+ * brute force.  Independent of the CUDA cell list; pinned against orc_neighbors_brute in tests.
+ * Periodic boxes only (box[c] >= 2*rcut required for the minimum image to be unique). */
+int orc_neighbors_grid(int n, const double *xyz, const double *box, double rcut, int fp32_pred, int cap,
+                       int *counts, int *list)
+{
+    int nb[3];
+    for (int c = 0; c < 3; ++c) {
+        if (!(box[c] >= 2.0 * rcut)) return -1000000000;
+        nb[c] = (int)floor(box[c] / (rcut * 1.001));
+        if (nb[c] < 1) nb[c] = 1;
+    }
+    long nbin = (long)nb[0] * nb[1] * nb[2];
+    int *bin_of = (int *)malloc(sizeof(int) * n);
+    int *start = (int *)calloc(nbin + 1, sizeof(int));
+    int *items = (int *)malloc(sizeof(int) * n);
+    for (int i = 0; i < n; ++i) {
+        int b[3];
+        for (int c = 0; c < 3; ++c) {
+            double w = xyz[3 * i + c] - box[c] * floor(xyz[3 * i + c] / box[c]); /* wrap into [0,L) */
+            b[c] = (int)floor(w / box[c] * nb[c]);
+            if (b[c] >= nb[c]) b[c] = nb[c] - 1;
+            if (b[c] < 0) b[c] = 0;
+        }
+        bin_of[i] = (b[2] * nb[1] + b[1]) * nb[0] + b[0];
+        start[bin_of[i] + 1]++;
+    }
+    for (long k = 0; k < nbin; ++k) start[k + 1] += start[k];
+    int *fill = (int *)calloc(nbin, sizeof(int));
+    for (int i = 0; i < n; ++i) items[start[bin_of[i]] + fill[bin_of[i]]++] = i;
+    free(fill);
+
+    float Lf[3], invL[3];
+    for (int c = 0; c < 3; ++c) { Lf[c] = (float)box[c]; invL[c] = 1.0f / Lf[c]; }
+    float rl = (float)rcut;
+    float rl2 = rl * rl;
+    int maxc = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(max : maxc)
+    for (int i = 0; i < n; ++i) {
+        int bi = bin_of[i];
+        int b0 = bi % nb[0], b1 = (bi / nb[0]) % nb[1], b2 = bi / (nb[0] * nb[1]);
+        int bb[3] = {b0, b1, b2};
+        int cand[3][3], nc[3];
+        for (int c = 0; c < 3; ++c) { /* distinct bins among b-1, b, b+1 (mod nb) */
+            nc[c] = 0;
+            for (int o = -1; o <= 1; ++o) {
+                int v = ((bb[c] + o) % nb[c] + nb[c]) % nb[c];
+                int dup = 0;
+                for (int q = 0; q < nc[c]; ++q) if (cand[c][q] == v) dup = 1;
+                if (!dup) cand[c][nc[c]++] = v;
+            }
+        }
+        int cnt = 0;
+        float xi[3] = {(float)xyz[3 * i], (float)xyz[3 * i + 1], (float)xyz[3 * i + 2]};
+        for (int a2 = 0; a2 < nc[2]; ++a2)
+            for (int a1 = 0; a1 < nc[1]; ++a1)
+                for (int a0 = 0; a0 < nc[0]; ++a0) {
+                    long b = ((long)cand[2][a2] * nb[1] + cand[1][a1]) * nb[0] + cand[0][a0];
+                    for (int q = start[b]; q < start[b + 1]; ++q) {
+                        int j = items[q];
+                        if (j == i) continue;
+                        int in;
+                        if (fp32_pred) {
+                            float xj[3] = {(float)xyz[3 * j], (float)xyz[3 * j + 1], (float)xyz[3 * j + 2]};
+                            in = within_f32(xi, xj, Lf, invL, rl2);
+                        } else {
+                            double d[3];
+                            disp(xyz + 3 * i, xyz + 3 * j, box, d);
+                            in = (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]) < rcut * rcut;
+                        }
+                        if (in) { if (cnt < cap) list[(long)i * cap + cnt] = j; ++cnt; }
+                    }
+                }
+        counts[i] = cnt;
+        if (cnt > maxc) maxc = cnt;
+    }
+    free(bin_of); free(start); free(items);
+    return maxc > cap ? -maxc : maxc;
+}
+
+/* ---- O2/O3 pieces ------------------------------------------------------------------------ */
+/* Cosine switch ("cosine function as used in ANI"), reading A4: 0 for r >= R. */
+double orc_fc(double r, double R) { return r < R ? 0.5 * cos(M_PI * r / R) + 0.5 : 0.0; }
+static double dfc(double r, double R) { return r < R ? -0.5 * M_PI / R * sin(M_PI * r / R) : 0.0; }
+
+/* O4: CELU_alpha(x) = max(0,x) + min(0, alpha(exp(x/alpha)-1)) */
+double orc_celu(double x, double alpha) { return x > 0.0 ? x : alpha * (exp(x / alpha) - 1.0); }
+static double dcelu(double x, double alpha) { return x > 0.0 ? 1.0 : exp(x / alpha); }
+
+/* O4: one species network forward; optionally O6 backward to the input gradient.
+ * h0 = G (length widths[0]); z_l = W_l^T h_{l-1} + b_l; h_l = CELU(z_l) for l < n_layers; output = z_last. */
+static double mlp_eval(const orc_model *m, int net, int s, const double *G, double *grad /* or NULL */)
+{
+    const int nl = m->n_layers;
+    const int *w = m->widths + s * (nl + 1);
+    int maxw = 0;
+    for (int l = 0; l <= nl; ++l) if (w[l] > maxw) maxw = w[l];
+    double *h = (double *)malloc(sizeof(double) * (size_t)(nl + 1) * maxw); /* h[l] */
+    double *z = (double *)malloc(sizeof(double) * (size_t)(nl + 1) * maxw); /* z[l] */
+    memcpy(h, G, sizeof(double) * w[0]);
+    for (int l = 1; l <= nl; ++l) {
+        const double *W = layer_ptr(m, net, s, l - 1);
+        const double *b = W + (long)w[l - 1] * w[l];
+        const double *hin = h + (size_t)(l - 1) * maxw;
+        double *zl = z + (size_t)l * maxw, *hl = h + (size_t)l * maxw;
+        for (int o = 0; o < w[l]; ++o) zl[o] = b[o];
+        for (int i = 0; i < w[l - 1]; ++i) {
+            double hi = hin[i];
+            const double *Wi = W + (long)i * w[l];
+            for (int o = 0; o < w[l]; ++o) zl[o] += Wi[o] * hi;
+        }
+        for (int o = 0; o < w[l]; ++o) hl[o] = (l < nl) ? orc_celu(zl[o], m->celu_alpha) : zl[o];
+    }
+    double out = z[(size_t)nl * maxw]; /* widths[nl] == 1 */
+    if (grad) {
+        /* dE/dz_last = 1; dE/dh_{l-1} = W_l dE/dz_l; dE/dz_l = dE/dh_l * CELU'(z_l) */
+        double *dz = (double *)malloc(sizeof(double) * maxw);
+        double *dh = (double *)malloc(sizeof(double) * maxw);
+        dz[0] = 1.0;
+        for (int l = nl; l >= 1; --l) {
+            const double *W = layer_ptr(m, net, s, l - 1);
+            for (int i = 0; i < w[l - 1]; ++i) {
+                double acc = 0.0;
+                for (int o = 0; o < w[l]; ++o) acc += W[(long)i * w[l] + o] * dz[o];
+                dh[i] = acc;
+            }
+            if (l - 1 >= 1) {
+                const double *zl = z + (size_t)(l - 1) * maxw;
+                for (int i = 0; i < w[l - 1]; ++i) dz[i] = dh[i] * dcelu(zl[i], m->celu_alpha);
+            }
+        }
+        for (int i = 0; i < w[0]; ++i) grad[i] = dh[i];
+        free(dz); free(dh);
+    }
+    free(h); free(z);
+    return out;
+}
+
+/* Exposed for the MLP pins (vs numpy matmul). */
+double orc_mlp(const orc_model *m, int net, int species, const double *G, double *grad)
+{
+    return mlp_eval(m, net, species, G, grad);
+}
+
+/* O2 + O3: AEV of atom i from its radial list (ids with r < rcr); angular neighbours are the subset
+ * with r < rca (PAPER.md L51-55 GraphFilter / GraphAngularExtension). */
+static void aev_atom(const orc_model *m, int i, const int *species, const double *xyz, const double *box,
+                     int nn, const int *nbr, double *G)
+{
+    const int S = m->n_species, nr = m->n_shf_r, na = m->n_shf_a, nz = m->n_shf_z;
+    const int len = orc_aev_len(m), rad = S * nr;
+    for (int q = 0; q < len; ++q) G[q] = 0.0;
+    for (int a = 0; a < nn; ++a) {
+        int j = nbr[a];
+        double d[3]; disp(xyz + 3 * i, xyz + 3 * j, box, d);
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (!(r < m->rcr)) continue;
+        double f = orc_fc(r, m->rcr);
+        for (int k = 0; k < nr; ++k)
+            G[species[j] * nr + k] += 0.25 * exp(-m->eta_r * (r - m->shf_r[k]) * (r - m->shf_r[k])) * f;
+    }
+    for (int a = 0; a < nn; ++a) {
+        int j = nbr[a];
+        double dj[3]; disp(xyz + 3 * i, xyz + 3 * j, box, dj);
+        double rj = sqrt(dj[0] * dj[0] + dj[1] * dj[1] + dj[2] * dj[2]);
+        if (!(rj < m->rca)) continue;
+        for (int b = a + 1; b < nn; ++b) { /* unordered pairs {j,k} */
+            int k = nbr[b];
+            double dk[3]; disp(xyz + 3 * i, xyz + 3 * k, box, dk);
+            double rk = sqrt(dk[0] * dk[0] + dk[1] * dk[1] + dk[2] * dk[2]);
+            if (!(rk < m->rca)) continue;
+            double c = (dj[0] * dk[0] + dj[1] * dk[1] + dj[2] * dk[2]) / (rj * rk);
+            double th = acos(0.95 * c);
+            double rb = 0.5 * (rj + rk);
+            double ff = orc_fc(rj, m->rca) * orc_fc(rk, m->rca);
+            int p = orc_pair_index(S, species[j], species[k]);
+            for (int ia = 0; ia < na; ++ia) {
+                double R = exp(-m->eta_a * (rb - m->shf_a[ia]) * (rb - m->shf_a[ia]));
+                for (int iz = 0; iz < nz; ++iz) {
+                    double A = pow(0.5 * (1.0 + cos(th - m->shf_z[iz])), m->zeta);
+                    G[rad + (p * na + ia) * nz + iz] += 2.0 * A * R * ff;
+                }
+            }
+        }
+    }
+}
+
+/* O6: given g = dE/dG_i, add -dE/dx to F for atom i and its neighbours. */
+static void aev_atom_backward(const orc_model *m, int i, const int *species, const double *xyz, const double *box,
+                              int nn, const int *nbr, const double *g, double *F)
+{
+    const int S = m->n_species, nr = m->n_shf_r, na = m->n_shf_a, nz = m->n_shf_z;
+    const int rad = S * nr;
+    double Fi[3] = {0, 0, 0};
+    for (int a = 0; a < nn; ++a) {
+        int j = nbr[a];
+        double d[3]; disp(xyz + 3 * i, xyz + 3 * j, box, d);
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (!(r < m->rcr)) continue;
+        double f = orc_fc(r, m->rcr), fp = dfc(r, m->rcr);
+        double dEdr = 0.0;
+        for (int k = 0; k < nr; ++k) {
+            double u = r - m->shf_r[k];
+            double e = exp(-m->eta_r * u * u);
+            dEdr += g[species[j] * nr + k] * 0.25 * e * (-2.0 * m->eta_r * u * f + fp);
+        }
+        for (int c = 0; c < 3; ++c) {
+            double v = dEdr * d[c] / r; /* dE/dd_ij ; d_ij = x_j - x_i */
+#pragma omp atomic
+            F[3 * j + c] -= v;
+            Fi[c] += v;
+        }
+    }
+    for (int a = 0; a < nn; ++a) {
+        int j = nbr[a];
+        double dj[3]; disp(xyz + 3 * i, xyz + 3 * j, box, dj);
+        double rj = sqrt(dj[0] * dj[0] + dj[1] * dj[1] + dj[2] * dj[2]);
+        if (!(rj < m->rca)) continue;
+        for (int b = a + 1; b < nn; ++b) {
+            int k = nbr[b];
+            double dk[3]; disp(xyz + 3 * i, xyz + 3 * k, box, dk);
+            double rk = sqrt(dk[0] * dk[0] + dk[1] * dk[1] + dk[2] * dk[2]);
+            if (!(rk < m->rca)) continue;
+            double c = (dj[0] * dk[0] + dj[1] * dk[1] + dj[2] * dk[2]) / (rj * rk);
+            double th = acos(0.95 * c);
+            double dth_dc = -0.95 / sqrt(1.0 - 0.9025 * c * c);
+            double rb = 0.5 * (rj + rk);
+            double fj = orc_fc(rj, m->rca), fk = orc_fc(rk, m->rca);
+            double fjp = dfc(rj, m->rca), fkp = dfc(rk, m->rca);
+            int p = orc_pair_index(S, species[j], species[k]);
+            double dE_dth = 0.0, dE_drb = 0.0, dE_dff = 0.0; /* ff = fj*fk */
+            for (int ia = 0; ia < na; ++ia) {
+                double u = rb - m->shf_a[ia];
+                double R = exp(-m->eta_a * u * u);
+                double dR = -2.0 * m->eta_a * u * R;
+                for (int iz = 0; iz < nz; ++iz) {
+                    double w = g[rad + (p * na + ia) * nz + iz];
+                    double base = 0.5 * (1.0 + cos(th - m->shf_z[iz]));
+                    double A = pow(base, m->zeta);
+                    double dA = -0.5 * m->zeta * sin(th - m->shf_z[iz]) * pow(base, m->zeta - 1.0);
+                    dE_dth += w * 2.0 * dA * R * fj * fk;
+                    dE_drb += w * 2.0 * A * dR * fj * fk;
+                    dE_dff += w * 2.0 * A * R;
+                }
+            }
+            double dE_dc = dE_dth * dth_dc;
+            double dE_drj = 0.5 * dE_drb + dE_dff * fjp * fk;
+            double dE_drk = 0.5 * dE_drb + dE_dff * fj * fkp;
+            for (int q = 0; q < 3; ++q) {
+                double dc_ddj = dk[q] / (rj * rk) - c * dj[q] / (rj * rj);
+                double dc_ddk = dj[q] / (rj * rk) - c * dk[q] / (rk * rk);
+                double vj = dE_dc * dc_ddj + dE_drj * dj[q] / rj;
+                double vk = dE_dc * dc_ddk + dE_drk * dk[q] / rk;
+#pragma omp atomic
+                F[3 * j + q] -= vj;
+#pragma omp atomic
+                F[3 * k + q] -= vk;
+                Fi[q] += vj + vk;
+            }
+        }
+    }
+    for (int c = 0; c < 3; ++c) {
+#pragma omp atomic
+        F[3 * i + c] += Fi[c];
+    }
+}
+
+/* O1-O6.  nbr_method: 0 brute force, 1 grid (periodic only).  Lists are built at the exact radial
+ * cutoff in fp64.  Outputs (any may be NULL except E): E[n_mols] (O5), F[n][3] (O6), e_atom[n],
+ * aev[n][len], dEdG[n][len].  mol_offsets NULL => one structure.  Returns 0, or <0 on failure. */
+int orc_energy_forces(const orc_model *m, int n, const int *species, const double *xyz, const double *box,
+                      int n_mols, const int *mol_offsets, int nbr_method, double *E, double *F,
+                      double *e_atom, double *aev, double *dEdG)
+{
+    const int len = orc_aev_len(m);
+    const double *bx = NULL;
+    if (box && (box[0] > 0.0 || box[1] > 0.0 || box[2] > 0.0)) bx = box;
+    int *mol_id = (int *)malloc(sizeof(int) * (n > 0 ? n : 1));
+    if (mol_offsets) {
+        for (int q = 0; q < n_mols; ++q)
+            for (int i = mol_offsets[q]; i < mol_offsets[q + 1]; ++i) mol_id[i] = q;
+    } else {
+        n_mols = 1;
+        for (int i = 0; i < n; ++i) mol_id[i] = 0;
+    }
+    for (int q = 0; q < n_mols; ++q) E[q] = 0.0;
+    if (F) memset(F, 0, sizeof(double) * 3 * (size_t)n);
+    if (n == 0) { free(mol_id); return 0; }
+
+    int cap = 64, rc;
+    int *counts = (int *)malloc(sizeof(int) * n), *list = NULL;
+    for (;;) {
+        list = (int *)malloc(sizeof(int) * (size_t)n * cap);
+        if (nbr_method == 1 && bx) rc = orc_neighbors_grid(n, xyz, bx, m->rcr, 0, cap, counts, list);
+        else rc = orc_neighbors_brute(n, xyz, bx, mol_offsets ? mol_id : NULL, m->rcr, 0, cap, counts, list);
+        if (rc >= 0) break;
+        free(list);
+        if (rc <= -1000000000) { free(counts); free(mol_id); return -1; }
+        cap = -rc + 8;
+    }
+    int fail = 0;
+#pragma omp parallel
+    {
+        double *G = (double *)malloc(sizeof(double) * len);
+        double *g = (double *)malloc(sizeof(double) * len);
+        double *gn = (double *)malloc(sizeof(double) * len);
+#pragma omp for schedule(dynamic, 16)
+        for (int i = 0; i < n; ++i) {
+            int s = species[i];
+            if (s < 0 || s >= m->n_species) { fail = 1; continue; }
+            aev_atom(m, i, species, xyz, bx, counts[i], list + (size_t)i * cap, G);
+            double e = 0.0;
+            for (int q = 0; q < len; ++q) g[q] = 0.0;
+            for (int net = 0; net < m->n_nets; ++net) { /* reading B5: mean over the ensemble */
+                e += mlp_eval(m, net, s, G, (F || dEdG) ? gn : NULL);
+                if (F || dEdG) for (int q = 0; q < len; ++q) g[q] += gn[q];
+            }
+            e /= m->n_nets;
+            for (int q = 0; q < len; ++q) g[q] /= m->n_nets;
+            if (m->self_energy) e += m->self_energy[s];
+            if (e_atom) e_atom[i] = e;
+            if (aev) memcpy(aev + (size_t)i * len, G, sizeof(double) * len);
+            if (dEdG) memcpy(dEdG + (size_t)i * len, g, sizeof(double) * len);
+#pragma omp atomic
+            E[mol_id[i]] += e;
+            if (F) aev_atom_backward(m, i, species, xyz, bx, counts[i], list + (size_t)i * cap, g, F);
+        }
+        free(G); free(g); free(gn);
+    }
+    free(counts); free(list); free(mol_id);
+    return fail ? -2 : 0;
+}
+
+/* O7 rebuild rule (reading C2): max_i |x_i - xref_i| > skin/2 (strict). */
+int orc_needs_rebuild(int n, const double *xyz, const double *xref, double skin)
+{
+    double lim2 = 0.25 * skin * skin;
+    for (int i = 0; i < n; ++i) {
+        double d0 = xyz[3 * i] - xref[3 * i], d1 = xyz[3 * i + 1] - xref[3 * i + 1], d2 = xyz[3 * i + 2] - xref[3 * i + 2];
+        if (d0 * d0 + d1 * d1 + d2 * d2 > lim2) return 1;
+    }
+    return 0;
+}
+
+/* O7: velocity Verlet (NVE "reverts to the velocity Verlet integrator").
+ * a = accel_conv * F / m.  Per step: v += dt/2 a; x += dt v; [rebuild test]; F(x); v += dt/2 a.
+ * Coordinates are not wrapped.  Forces are evaluated with exact (fresh) lists every step -- in exact
+ * arithmetic a valid skinned list gives the same E,F -- but the rebuild rule is tracked so that
+ * n_rebuilds reports what an implementation using a Verlet skin must do (the initial build counts as 1).
+ * F_io: forces at the input positions if have_forces, else computed here; holds the final forces on return.
+ * epot/ekin: [n_steps+1] values at steps 0..n_steps (may be NULL). */
+int orc_md(const orc_model *m, int n, const int *species, double *xyz, double *vel, double *F_io, int have_forces,
+           const double *mass /*[S]*/, const double *box, double dt, double accel_conv, int n_steps, double skin,
+           int nbr_method, double *epot, double *ekin, int *n_rebuilds)
+{
+    double E;
+    int rc = 0, nreb = 1;
+    double *xref = (double *)malloc(sizeof(double) * 3 * (size_t)n);
+    memcpy(xref, xyz, sizeof(double) * 3 * (size_t)n);
+    if (!have_forces || epot) {
+        rc = orc_energy_forces(m, n, species, xyz, box, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL);
+        if (rc) { free(xref); return rc; }
+    }
+    for (int step = 0;; ++step) {
+        if (ekin) {
+            double k = 0.0;
+            for (int i = 0; i < n; ++i)
+                k += 0.5 * mass[species[i]] * (vel[3 * i] * vel[3 * i] + vel[3 * i + 1] * vel[3 * i + 1] + vel[3 * i + 2] * vel[3 * i + 2]);
+            ekin[step] = k / accel_conv;
+        }
+        if (epot) epot[step] = E;
+        if (step == n_steps) break;
+        for (int i = 0; i < n; ++i)
+            for (int c = 0; c < 3; ++c) {
+                vel[3 * i + c] += 0.5 * dt * accel_conv * F_io[3 * i + c] / mass[species[i]];
+                xyz[3 * i + c] += dt * vel[3 * i + c];
+            }
+        if (orc_needs_rebuild(n, xyz, xref, skin)) { memcpy(xref, xyz, sizeof(double) * 3 * (size_t)n); ++nreb; }
+        rc = orc_energy_forces(m, n, species, xyz, box, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL);
+        if (rc) break;
+        for (int i = 0; i < n; ++i)
+            for (int c = 0; c < 3; ++c) vel[3 * i + c] += 0.5 * dt * accel_conv * F_io[3 * i + c] / mass[species[i]];
+    }
+    if (n_rebuilds) *n_rebuilds = nreb;
+    free(xref);
+    return rc;
+}
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

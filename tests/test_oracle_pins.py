@@ -1,0 +1,484 @@
+"""Pins for oracle/ (CPU only).  Each test states which plausible mistake it would catch.
+
+Citations: SURVEY.md 8(c) C1 (O1-O7), C2 (readings), C3 (pins); PAPER.md L41 (directed lists, batching),
+L61 (cosine switch, continuity at the cutoff), L176 (Fig. 2 pipeline), L307 (velocity Verlet), L443 (angular form).
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.spatial import cKDTree
+
+from oracle import nnp_oracle as orc
+from paper_2405_01491_b200 import inputs
+
+
+def rot(seed):
+    return inputs._random_rotations(np.random.default_rng(seed), 1)[0]
+
+
+# ---------------------------------------------------------------- sizes / indexing
+def test_aev_length_closed_form(ani_model):
+    # BASELINE.json: 7x16 radial + 28x4x8 angular = 1008
+    assert ani_model.aev_len == 7 * 16 + 28 * 4 * 8 == 1008
+
+
+def test_pair_index_is_upper_triangle_bijection():
+    seen = {}
+    for s in range(7):
+        for t in range(s, 7):
+            p = orc.pair_index(7, s, t)
+            assert orc.pair_index(7, t, s) == p
+            seen[p] = (s, t)
+    assert sorted(seen) == list(range(28))
+    assert orc.pair_index(7, 6, 6) == 27 and orc.pair_index(7, 0, 0) == 0 and orc.pair_index(7, 1, 1) == 7
+    # row-major: p increases with t inside a row, rows in order of s
+    order = [seen[p] for p in range(28)]
+    assert order == sorted(order)
+
+
+# ---------------------------------------------------------------- scalar pieces: values known without the formula
+def test_cutoff_function_special_values():
+    R = 5.1
+    assert orc.fc(0.0, R) == 1.0
+    assert abs(orc.fc(R / 2, R) - 0.5) < 1e-15
+    assert abs(orc.fc(R / 3, R) - 0.75) < 1e-15          # cos(pi/3) = 1/2
+    assert orc.fc(R, R) == 0.0 and orc.fc(R * 1.0001, R) == 0.0 and orc.fc(2 * R, R) == 0.0   # reading A4
+    assert 0 < orc.fc(R * (1 - 1e-6), R) < 1e-11          # goes smoothly to zero
+
+
+def test_celu_special_values():
+    a = 0.1
+    assert orc.celu(0.0, a) == 0.0
+    assert orc.celu(2.5, a) == 2.5
+    assert abs(orc.celu(-50.0, a) + a) < 1e-15
+    assert abs(orc.celu(-a * math.log(2.0), a) + a / 2) < 1e-15      # alpha(e^{-ln2}-1) = -alpha/2
+
+
+# ---------------------------------------------------------------- radial block
+def test_isolated_atom_and_beyond_cutoff_zero(ani_model):
+    r = orc.energy_forces(ani_model, [3], [[0, 0, 0]], want_aev=True)
+    assert np.all(r["aev"] == 0)
+    r = orc.energy_forces(ani_model, [3, 0], [[0, 0, 0], [5.1, 0, 0]], want_aev=True)
+    assert np.all(r["aev"] == 0) and np.all(r["F"] == 0)
+
+
+def test_dimer_radial_hand_values(ani_model, consts):
+    # r = ShfR_k exactly => Gaussian = 1 => G[s_j*16+k] = fc(r)/4 ; and at r = R/2, fc = 1/2.
+    for k in (0, 5, 15):
+        r0 = float(consts["shf_r"][k])
+        res = orc.energy_forces(ani_model, [3, 1], [[0, 0, 0], [0, r0, 0]], want_aev=True)
+        G = res["aev"]
+        # atom 0 (O) sees a C (species 1): block 1; atom 1 sees an O (species 3): block 3
+        assert abs(G[0, 1 * 16 + k] - 0.25 * (0.5 * math.cos(math.pi * r0 / 5.1) + 0.5)) < 1e-15
+        assert abs(G[1, 3 * 16 + k] - G[0, 1 * 16 + k]) < 1e-16
+        nz = np.nonzero(G[0])[0]
+        assert nz.min() >= 16 and nz.max() < 32           # only the neighbour-species block, no angular terms
+        # neighbouring shifts: ratio exp(-eta*Delta^2) with Delta = 0.26875
+        if k < 15:
+            assert abs(G[0, 16 + k + 1] / G[0, 16 + k] - math.exp(-19.7 * 0.26875 ** 2)) < 1e-12
+    res = orc.energy_forces(ani_model, [0, 0], [[1, 1, 1], [1, 1, 1 + 2.55]], want_aev=True)
+    k = 7   # shf_r[7] = 2.68125
+    assert abs(res["aev"][0, k] - 0.125 * math.exp(-19.7 * (2.55 - 2.68125) ** 2)) < 1e-15
+
+
+def test_radial_additivity_over_neighbours(ani_model):
+    # two neighbours of the same species beyond the angular cutoff of each other's pairing: radial block adds
+    a = orc.energy_forces(ani_model, [0, 3], [[0, 0, 0], [4.0, 0, 0]], want_aev=True)["aev"][0]
+    b = orc.energy_forces(ani_model, [0, 3], [[0, 0, 0], [0, 4.5, 0]], want_aev=True)["aev"][0]
+    c = orc.energy_forces(ani_model, [0, 3, 3], [[0, 0, 0], [4.0, 0, 0], [0, 4.5, 0]], want_aev=True)["aev"][0]
+    assert np.allclose(c, a + b, atol=1e-16)
+    assert np.all(c[112:] == 0)       # both beyond 3.5 A: no angular term
+
+
+# ---------------------------------------------------------------- angular block
+def _trimer(r, theta, sj=0, sk=0, si=3):
+    xyz = [[0, 0, 0], [r, 0, 0], [r * math.cos(theta), r * math.sin(theta), 0]]
+    return [si, sj, sk], xyz
+
+
+def test_trimer_angular_hand_values(ani_model, consts):
+    # r_ij = r_ik = ShfA_a and 0.95 cos(theta) = cos(ShfZ_z)  =>  both factors are exactly 1
+    # => G[112 + p*32 + a*4 + z] = 2 fc(r)^2
+    for a in (0, 3, 7):
+        for z in (0, 1, 2, 3):
+            r = float(consts["shf_a"][a])
+            theta = math.acos(math.cos(float(consts["shf_z"][z])) / 0.95)
+            sp, xyz = _trimer(r, theta, 0, 0)
+            G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+            fcv = 0.5 * math.cos(math.pi * r / 3.5) + 0.5
+            p = 0   # (H,H)
+            assert abs(G[112 + p * 32 + a * 4 + z] - 2 * fcv * fcv) < 1e-13
+            assert np.all(G[112 + 32:] == 0)              # nothing outside block (H,H)
+
+
+def test_trimer_block_placement_and_swap(ani_model):
+    r, th = 1.7, 1.9
+    for sj, sk in ((0, 3), (1, 6), (6, 6), (2, 4)):
+        sp, xyz = _trimer(r, th, sj, sk)
+        G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+        p = orc.pair_index(7, sj, sk)
+        ang = G[112:].reshape(28, 32)
+        assert np.all(ang[p] > 0)
+        assert np.all(np.delete(ang, p, axis=0) == 0)
+        sp2, xyz2 = [sp[0], sp[2], sp[1]], [xyz[0], xyz[2], xyz[1]]      # swap j and k
+        G2 = orc.energy_forces(ani_model, sp2, xyz2, want_aev=True)["aev"][0]
+        assert np.allclose(G, G2, rtol=0, atol=1e-16)
+
+
+def test_trimer_collinear_angles_finite(ani_model):
+    for th in (0.0 + 1e-9, math.pi / 2, math.pi):
+        sp, xyz = _trimer(1.5, th)
+        xyz[2] = [1.2 * math.cos(th), 1.2 * math.sin(th), 0.0]
+        res = orc.energy_forces(ani_model, sp, xyz, want_aev=True)
+        assert np.all(np.isfinite(res["aev"])) and np.all(np.isfinite(res["F"]))
+
+
+def test_angular_uses_angular_cutoff_only(ani_model):
+    # k at 3.6 A (> 3.5): contributes radially, but no triplet
+    sp, xyz = [3, 0, 0], [[0, 0, 0], [1.0, 0, 0], [0, 3.6, 0]]
+    G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+    assert np.all(G[112:] == 0) and G[:16].sum() > 0
+    xyz[2] = [0, 3.4, 0]
+    G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+    assert G[112:144].sum() > 0
+
+
+# ---------------------------------------------------------------- MLP vs library routines
+def _numpy_mlp(widths_row, params_iter, G, alpha=0.1):
+    h = G
+    nl = len(widths_row) - 1
+    Ws = []
+    for l in range(nl):
+        fi, fo = widths_row[l], widths_row[l + 1]
+        W = next(params_iter)(fi * fo).reshape(fi, fo)
+        b = next(params_iter)(fo)
+        Ws.append((W, b))
+    zs = []
+    for l, (W, b) in enumerate(Ws):
+        z = h @ W + b
+        zs.append(z)
+        h = np.where(z > 0, z, alpha * np.expm1(z / alpha)) if l < nl - 1 else z
+    # reverse mode by hand with numpy
+    d = np.ones(1)
+    for l in range(nl - 1, -1, -1):
+        W, _ = Ws[l]
+        d = W @ d
+        if l > 0:
+            d = d * np.where(zs[l - 1] > 0, 1.0, np.exp(zs[l - 1] / alpha))
+    return h[0], d
+
+
+def test_mlp_matches_numpy_matmul_all_species(consts):
+    p = inputs.make_weights(7, 2, bias_std=0.3)
+    m = orc.OracleModel(consts, inputs.WIDTHS, p, 2)
+    rng = np.random.default_rng(0)
+    pos = [0]
+
+    def taker():
+        while True:
+            def take(n):
+                out = p[pos[0]:pos[0] + n]
+                pos[0] += n
+                return out
+            yield take
+    it = taker()
+    for net in range(2):
+        for s in range(7):
+            G = rng.normal(size=1008) * 0.5
+            e_ref, g_ref = _numpy_mlp(list(inputs.WIDTHS[s]), it, G)
+            e, g = m.mlp(net, s, G, want_grad=True)
+            assert abs(e - e_ref) < 1e-12 * max(1, abs(e_ref))
+            assert np.allclose(g, g_ref, rtol=1e-11, atol=1e-13)
+    assert pos[0] == p.size
+
+
+def test_mlp_zero_weights_gives_bias_chain_and_single_layer_dot(consts):
+    w = np.array([[1008, 1]] * 7, dtype=np.int32)
+    rng = np.random.default_rng(1)
+    p = rng.normal(size=7 * 1009)
+    m = orc.OracleModel(consts, w, p, 1)
+    G = rng.normal(size=1008)
+    for s in range(7):
+        W, b = p[s * 1009:s * 1009 + 1008], p[s * 1009 + 1008]
+        e, g = m.mlp(0, s, G, want_grad=True)
+        assert abs(e - (G @ W + b)) < 1e-12 and np.allclose(g, W)
+    w2 = np.array([[1008, 4, 1]] * 7, dtype=np.int32)
+    p2 = np.zeros(7 * (1008 * 4 + 4 + 4 + 1))
+    per = 1008 * 4 + 4 + 4 + 1
+    p2[1008 * 4:1008 * 4 + 4] = [-1.0, 0.5, 0.0, -0.05]       # b1
+    p2[1008 * 4 + 4:1008 * 4 + 8] = [1.0, 2.0, 3.0, 4.0]      # W2
+    p2[per - 1] = 0.25
+    m2 = orc.OracleModel(consts, w2, p2, 1)
+    expect = 0.1 * math.expm1(-10.0) * 1 + 0.5 * 2 + 0 + 0.1 * math.expm1(-0.5) * 4 + 0.25
+    assert abs(m2.mlp(0, 0, G) - expect) < 1e-14
+
+
+# ---------------------------------------------------------------- neighbours
+def _kdtree_sets(xyz, box, r, mol_id=None):
+    if box is not None:
+        t = cKDTree(np.mod(xyz, box), boxsize=box)
+        rows = t.query_ball_point(np.mod(xyz, box), r)
+    else:
+        t = cKDTree(xyz)
+        rows = t.query_ball_point(xyz, r)
+    out = []
+    for i, row in enumerate(rows):
+        out.append(sorted(j for j in row if j != i and (mol_id is None or mol_id[j] == mol_id[i])))
+    return out
+
+
+def test_brute_force_neighbours_vs_kdtree_periodic(water64):
+    sp, xyz, box = water64
+    for r in (3.5, 5.1, 5.6):
+        mine = orc.neighbors(xyz, box, r)
+        ref = _kdtree_sets(xyz, box, r * (1 - 1e-12))
+        assert all(list(a) == b for a, b in zip(mine, ref))
+        # directed list: j in N(i) <=> i in N(j)
+        S = [set(a.tolist()) for a in mine]
+        assert all(i in S[j] for i in range(len(S)) for j in S[i])
+
+
+def test_neighbour_counts_match_density(consts):
+    sp, xyz, box = inputs.water_box(512, seed=3)
+    rho = len(sp) / box[0] ** 3
+    for r, expect in ((5.1, 55.7), (3.5, 18.0)):
+        c = np.mean([len(a) for a in orc.neighbors(xyz, box, r, method="grid")])
+        assert abs(c - rho * 4 / 3 * math.pi * r ** 3) / c < 0.08
+        assert abs(c - expect) / expect < 0.08          # SURVEY 8(a) figures for water
+
+
+def test_grid_neighbours_equal_brute_force():
+    sp, xyz, box = inputs.water_box(300, seed=5)
+    xyz = xyz + np.random.default_rng(0).integers(-2, 3, size=xyz.shape) * box     # unwrapped coordinates too
+    for r in (3.5, 5.6):
+        for f32 in (False, True):
+            a = orc.neighbors(xyz, box, r, fp32_pred=f32, method="brute")
+            b = orc.neighbors(xyz, box, r, fp32_pred=f32, method="grid")
+            assert all(np.array_equal(x, y) for x, y in zip(a, b))
+
+
+def test_fp32_predicate_agrees_outside_guard_band(water64):
+    sp, xyz, box = water64
+    r = 5.6
+    a = orc.neighbors(xyz, box, r, fp32_pred=True)
+    lo = orc.neighbors(xyz, box, r - 1e-4)
+    hi = orc.neighbors(xyz, box, r + 1e-4)
+    for x, l, h in zip(a, lo, hi):
+        assert set(l.tolist()) <= set(x.tolist()) <= set(h.tolist())
+
+
+def test_molecule_batch_never_pairs_across_molecules():
+    sp, xyz, offs = inputs.molecule_batch(6, seed=2)
+    xyz = xyz.copy()
+    xyz[offs[1]:offs[2]] += xyz[0] - xyz[offs[1]]       # put molecule 1 on top of molecule 0
+    mol = np.repeat(np.arange(6), np.diff(offs)).astype(np.int32)
+    rows = orc.neighbors(xyz, None, 5.1, mol_id=mol)
+    assert all(mol[j] == mol[i] for i, row in enumerate(rows) for j in row)
+    assert [list(r) for r in rows] == _kdtree_sets(xyz, None, 5.1, mol)
+
+
+# ---------------------------------------------------------------- forces: finite differences and invariances
+def _fd_check(model, sp, xyz, box, idx, h=1e-4, mol_offsets=None):
+    base = orc.energy_forces(model, sp, xyz, box, mol_offsets)
+    err = 0.0
+    for (i, c) in idx:
+        xp, xm = np.array(xyz), np.array(xyz)
+        xp[i, c] += h
+        xm[i, c] -= h
+        ep = orc.energy_forces(model, sp, xp, box, mol_offsets, want_forces=False)["E"].sum()
+        em = orc.energy_forces(model, sp, xm, box, mol_offsets, want_forces=False)["E"].sum()
+        fd = -(ep - em) / (2 * h)
+        err = max(err, abs(fd - base["F"][i, c]))
+    return err, np.abs(base["F"]).max()
+
+
+def test_forces_equal_minus_gradient_periodic_water_small_model(small_model, water64):
+    sp, xyz, box = water64
+    rng = np.random.default_rng(0)
+    idx = [(int(rng.integers(192)), int(rng.integers(3))) for _ in range(40)]
+    err, fmax = _fd_check(small_model, sp, xyz, box, idx)
+    assert fmax > 1e-3 and err < 2e-7 * max(1.0, fmax)
+
+
+def test_forces_equal_minus_gradient_ani_widths(ani_model, water64):
+    sp, xyz, box = water64
+    idx = [(0, 0), (1, 2), (100, 1), (191, 0)]
+    err, fmax = _fd_check(ani_model, sp, xyz, box, idx)
+    assert fmax > 1e-3 and err < 2e-7 * max(1.0, fmax)
+
+
+def test_forces_equal_minus_gradient_all_species_molecule(small_model):
+    sp, xyz, offs = inputs.molecule_batch(3, nmin=12, nmax=14, seed=11)
+    sp = (np.arange(len(sp)) % 7).astype(np.int32)       # every species and every species pair present
+    idx = [(i, c) for i in range(0, len(sp), 3) for c in range(3)]
+    err, fmax = _fd_check(small_model, sp, xyz, None, idx, mol_offsets=offs)
+    assert fmax > 1e-3 and err < 2e-7 * max(1.0, fmax)
+
+
+def test_net_force_and_torque_vanish(small_model, water64):
+    sp, xyz, box = water64
+    F = orc.energy_forces(small_model, sp, xyz, box)["F"]
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).sum()
+    sp, xyz, offs = inputs.molecule_batch(2, seed=4)
+    r = orc.energy_forces(small_model, sp, xyz, None, offs)
+    for m in range(2):
+        sl = slice(offs[m], offs[m + 1])
+        assert np.abs(r["F"][sl].sum(0)).max() < 1e-11
+        assert np.abs(np.cross(xyz[sl], r["F"][sl]).sum(0)).max() < 1e-10
+
+
+def test_rotation_translation_invariance_nonperiodic(small_model):
+    sp, xyz, offs = inputs.molecule_batch(1, nmin=20, nmax=20, seed=9)
+    a = orc.energy_forces(small_model, sp, xyz)
+    R = rot(1)
+    b = orc.energy_forces(small_model, sp, xyz @ R.T + np.array([3.0, -2.0, 0.7]))
+    assert abs(a["E"][0] - b["E"][0]) < 1e-11 * max(1, abs(a["E"][0]))
+    assert np.allclose(a["F"] @ R.T, b["F"], atol=1e-10)
+
+
+def test_periodic_symmetries(small_model, water64):
+    sp, xyz, box = water64
+    a = orc.energy_forces(small_model, sp, xyz, box)
+    # cubic symmetry: x->y->z->x and a mirror
+    P = np.array([[0, 1, 0], [0, 0, 1], [1, 0, 0]], dtype=float)
+    b = orc.energy_forces(small_model, sp, xyz @ P.T, box)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-10 and np.allclose(a["F"] @ P.T, b["F"], atol=1e-10)
+    M = np.diag([1.0, -1.0, 1.0])
+    b = orc.energy_forces(small_model, sp, xyz @ M, box)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-10 and np.allclose(a["F"] @ M, b["F"], atol=1e-10)
+    # global translation, and wrapping individual atoms by lattice vectors
+    b = orc.energy_forces(small_model, sp, xyz + np.array([1.234, -7.0, 30.1]), box)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-9 and np.allclose(a["F"], b["F"], atol=1e-9)
+    sh = np.random.default_rng(0).integers(-2, 3, size=xyz.shape) * box
+    b = orc.energy_forces(small_model, sp, xyz + sh, box)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-9 and np.allclose(a["F"], b["F"], atol=1e-9)
+
+
+def test_same_species_permutation_invariance(small_model, water64):
+    sp, xyz, box = water64
+    a = orc.energy_forces(small_model, sp, xyz, box)
+    perm = np.random.default_rng(2).permutation(len(sp))
+    b = orc.energy_forces(small_model, sp[perm], xyz[perm], box)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-10
+    assert np.allclose(a["F"][perm], b["F"], atol=1e-11)
+    # swapping two atoms' species labels of different species must change the energy
+    sp2 = sp.copy()
+    sp2[0], sp2[1] = sp[1], sp[0]
+    assert abs(orc.energy_forces(small_model, sp2, xyz, box)["E"][0] - a["E"][0]) > 1e-6
+
+
+def test_energy_and_force_continuous_across_cutoffs(small_model):
+    # no discontinuity when atoms enter/leave the neighbourhood
+    base = [[0, 0, 0], [1.0, 0.2, 0], [-0.3, 1.1, 0.4]]
+    sp = [3, 0, 0, 1]
+    for R in (5.1, 3.5):
+        vals = []
+        for dr in (-1e-7, 1e-7):
+            xyz = base + [[0.0, 0.0, R + dr]]
+            r = orc.energy_forces(small_model, sp, xyz)
+            vals.append((r["E"][0], r["F"].copy()))
+        assert abs(vals[0][0] - vals[1][0]) < 1e-9
+        assert np.abs(vals[0][1] - vals[1][1]).max() < 1e-5
+
+
+def test_extensivity_under_box_replication(small_model, water64):
+    sp, xyz, box = water64
+    a = orc.energy_forces(small_model, sp, xyz, box)
+    sp2, xyz2, box2 = inputs.replicate(sp, xyz, box, 2)
+    b = orc.energy_forces(small_model, sp2, xyz2, box2, nbr_method=1)
+    assert abs(b["E"][0] - 8 * a["E"][0]) < 1e-9 * abs(a["E"][0]) * 8 + 1e-9
+    assert np.allclose(b["F"].reshape(8, -1, 3), a["F"][None], atol=1e-10)
+    c = orc.energy_forces(small_model, sp2, xyz2, box2, nbr_method=0)
+    assert np.allclose(b["F"], c["F"], atol=1e-12) and abs(b["E"][0] - c["E"][0]) < 1e-9
+
+
+def test_ensemble_identities(consts, small_widths, water64):
+    sp, xyz, box = water64
+    p = inputs.make_weights(21, 3, widths=small_widths, bias_std=0.2)
+    per = p.size // 3
+    singles = [orc.energy_forces(orc.OracleModel(consts, small_widths, p[k * per:(k + 1) * per], 1), sp, xyz, box)
+               for k in range(3)]
+    ens = orc.energy_forces(orc.OracleModel(consts, small_widths, p, 3), sp, xyz, box)
+    assert abs(ens["E"][0] - np.mean([s["E"][0] for s in singles])) < 1e-10           # reading B5: mean
+    assert np.allclose(ens["F"], np.mean([s["F"] for s in singles], axis=0), atol=1e-12)
+    same = orc.energy_forces(orc.OracleModel(consts, small_widths, np.tile(p[:per], 8), 8), sp, xyz, box)
+    assert abs(same["E"][0] - singles[0]["E"][0]) < 1e-10 and np.allclose(same["F"], singles[0]["F"], atol=1e-12)
+
+
+def test_batch_equals_each_molecule_alone(small_model):
+    sp, xyz, offs = inputs.molecule_batch(5, seed=6)
+    xyz = xyz.copy()
+    xyz[offs[2]:offs[3]] += xyz[offs[1]] - xyz[offs[2]]      # overlapping molecules must still not interact
+    b = orc.energy_forces(small_model, sp, xyz, None, offs)
+    for m in range(5):
+        sl = slice(offs[m], offs[m + 1])
+        a = orc.energy_forces(small_model, sp[sl], xyz[sl])
+        assert abs(a["E"][0] - b["E"][m]) < 1e-11 and np.allclose(a["F"], b["F"][sl], atol=1e-12)
+
+
+def test_self_energy_shifts_energy_only(consts, small_widths, water64):
+    sp, xyz, box = water64
+    p = inputs.make_weights(5, 1, widths=small_widths)
+    se = np.arange(7) * 1.5 - 2.0
+    a = orc.energy_forces(orc.OracleModel(consts, small_widths, p, 1), sp, xyz, box)
+    b = orc.energy_forces(orc.OracleModel(consts, small_widths, p, 1, self_energy=se), sp, xyz, box)
+    assert abs(b["E"][0] - a["E"][0] - se[sp].sum()) < 1e-9 and np.allclose(a["F"], b["F"], rtol=0, atol=1e-13)
+
+
+# ---------------------------------------------------------------- MD (O7)
+def _md_setup(small_model):
+    sp, xyz, box = inputs.water_box(27, seed=8)
+    v = inputs.maxwell_boltzmann(sp, 300.0, seed=1)
+    return sp, xyz, box, v
+
+
+def test_velocity_verlet_time_reversible(small_model):
+    sp, xyz, box, v = _md_setup(small_model)
+    a = orc.md(small_model, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 20)
+    b = orc.md(small_model, sp, a["xyz"], -a["vel"], inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 20)
+    assert np.abs(b["xyz"] - xyz).max() < 1e-10 and np.abs(b["vel"] + v).max() < 1e-11
+
+
+def test_velocity_verlet_energy_error_scales_dt2(small_model):
+    sp, xyz, box, v = _md_setup(small_model)
+    errs = []
+    for dt, n in ((0.5, 40), (0.25, 80)):
+        r = orc.md(small_model, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, n)
+        tot = r["epot"] + r["ekin"]
+        errs.append(np.abs(tot - tot[0]).max())
+    assert errs[0] > 0 and 2.5 < errs[0] / errs[1] < 6.0
+
+
+def test_velocity_verlet_first_step_by_hand(small_model):
+    sp, xyz, box, v = _md_setup(small_model)
+    dt = 0.5
+    F0 = orc.energy_forces(small_model, sp, xyz, box)["F"]
+    a0 = inputs.ACCEL_CONV * F0 / inputs.MASS[sp][:, None]
+    x1 = xyz + dt * v + 0.5 * dt * dt * a0                       # textbook velocity-Verlet position update
+    F1 = orc.energy_forces(small_model, sp, x1, box)["F"]
+    v1 = v + 0.5 * dt * (a0 + inputs.ACCEL_CONV * F1 / inputs.MASS[sp][:, None])
+    r = orc.md(small_model, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, 1)
+    assert np.abs(r["xyz"] - x1).max() < 1e-13 and np.abs(r["vel"] - v1).max() < 1e-14
+    ke = 0.5 * (inputs.MASS[sp][:, None] * v ** 2).sum() / inputs.ACCEL_CONV
+    assert abs(r["ekin"][0] - ke) < 1e-10
+    # kinetic temperature of the seeded Maxwell-Boltzmann draw is near 300 K (reading C3)
+    T = 2 * ke / (3 * len(sp) * inputs.KB)
+    assert 200 < T < 400
+
+
+def test_rebuild_rule_strict_half_skin():
+    x0 = np.zeros((4, 3))
+    x1 = x0.copy()
+    x1[2, 1] = 0.25
+    assert not orc.needs_rebuild(x1, x0, 0.5)          # == skin/2: strict (reading C2)
+    x1[2, 1] = 0.2500001
+    assert orc.needs_rebuild(x1, x0, 0.5)
+    x1[2] = [0.15, 0.15, 0.15]                          # |d| = 0.2598 > 0.25
+    assert orc.needs_rebuild(x1, x0, 0.5)
+
+
+def test_md_rebuild_count_reasonable(small_model):
+    sp, xyz, box, v = _md_setup(small_model)
+    r = orc.md(small_model, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 30, skin=0.5)
+    assert 2 <= r["n_rebuilds"] <= 12
