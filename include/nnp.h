@@ -1,0 +1,148 @@
+/*
+ * nnp.h -- C-ABI of the B200-native ANI-2x energy / force / MD hot path.
+ *
+ * What is computed (citations are /root/reference/PAPER.md lines + SURVEY.md 8(c) items, restated in
+ * DESIGN.md "The path"): one ANI-like evaluation as in Fig. 2 of the FeNNol paper:
+ *   stage 1  neighbour lists (GraphGenerator / GraphFilter, L41-55; cell list + Verlet skin, L49, L341)
+ *   stage 2  atomic environment vectors (ANI_AEV, L71, L79, cosine switch L61, angular form L443)
+ *   stage 3  species-specialised MLPs (ChemicalNet, L87) summed per structure (L176)
+ *   stage 4  forces = -dE/dx, the hand-written reverse pass of what the paper gets from jax.grad (L65, L176)
+ *   stage 5  velocity Verlet, GPU-resident (fennol_md NVE, L307)
+ *
+ * Conventions
+ *   - Every function returns NNP_OK (0) or a negative nnp_status; none throws or exits.  After a failure
+ *     nnp_last_error(ctx) returns a static / ctx-owned description.
+ *   - Pointer names say where the memory lives: d_* device memory owned by the caller (e.g. a torch
+ *     tensor) that must stay valid until the stream work that uses it has completed; h_* host memory
+ *     (pinned memory makes the copies asynchronous).  The library never frees caller memory.
+ *   - All work is enqueued on the CUDA stream given to nnp_create and the calls return without waiting,
+ *     except where "synchronises" is stated.  Conditions only visible on the device (neighbour capacity
+ *     overflow) are latched in a device flag and reported by the next synchronising call.
+ *   - Atom indices in and out are the caller's original order.  Internally atoms are kept sorted by
+ *     (species, cell); that order is never visible.
+ *   - Units: Angstrom, fs, amu, energy unit of the weights (kcal/mol in the tests); accelerations are
+ *     accel_conv * F / m.
+ *   - Arithmetic: fp32 throughout, energies accumulated in fp64.  The MLP contractions run in the mode
+ *     chosen by mm_mode and the mode is part of every reported number.
+ *
+ * Fixed shape of this build (nnp_create returns NNP_EINVAL otherwise): n_species <= 7, n_shf_r == 16,
+ * n_shf_a == 8, n_shf_z == 4, n_layers == 4 with widths[s] = {1008-compatible AEV length, h1, h2, h3, 1},
+ * hidden widths multiples of 32 and <= 256.
+ */
+#ifndef NNP_H
+#define NNP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nnp_ctx nnp_ctx; /* opaque; owned by the library; freed by nnp_destroy */
+
+typedef enum {
+    NNP_OK = 0,
+    NNP_EINVAL = -1,    /* bad argument / unsupported shape */
+    NNP_ENOMEM = -2,    /* device or host allocation failed */
+    NNP_ECUDA = -3,     /* CUDA runtime error (message in nnp_last_error) */
+    NNP_ECAPACITY = -4, /* a neighbour row exceeded cap_r / cap_a: recreate with larger caps */
+    NNP_ESTALE = -5,    /* energy/forces or MD requested without a neighbour list for the current system */
+    NNP_EBOX = -6       /* periodic box edge < 2*(cutoff+skin): minimum image not unique (reading C1) */
+} nnp_status;
+
+enum { NNP_MM_FP32_SIMT = 0, NNP_MM_3XTF32_TC = 1, NNP_MM_TF32_TC = 2 };
+
+typedef struct {
+    int n_species;            /* <= 7; ANI-2x: 7, index order H,C,N,O,S,F,Cl (reading B2) */
+    float rcr, rca;           /* radial / angular cutoffs, Angstrom (5.1 / 3.5; reading A1) */
+    float eta_r;              /* radial Gaussian exponent */
+    int n_shf_r;              /* 16 */
+    const float *shf_r;       /* host [n_shf_r] */
+    float eta_a, zeta;        /* angular Gaussian exponent, angular power */
+    int n_shf_a;              /* 8 */
+    const float *shf_a;       /* host [n_shf_a] */
+    int n_shf_z;              /* 4 */
+    const float *shf_z;       /* host [n_shf_z], radians */
+    float celu_alpha;         /* CELU alpha (0.1) */
+    int n_nets;               /* ensemble size; energies and forces are the arithmetic mean (reading B5) */
+    int n_layers;             /* 4 affine layers */
+    const int *widths;        /* host [n_species][n_layers+1], widths[s][0] = AEV length, widths[s][4] = 1 */
+    const float *params;      /* host, flat: for net, for species, for layer: W[in][out] row-major then b[out] */
+    const float *self_energy; /* host [n_species] or NULL (= 0); added per atom, no force (reading B4) */
+    const float *mass;        /* host [n_species], amu */
+    float accel_conv;         /* a = accel_conv * F / m  (4.184e-4 for kcal/mol, A, fs, amu; reading B6) */
+    int mm_mode;              /* NNP_MM_*: how the MLP contractions are computed */
+    int cap_r, cap_a;         /* neighbour-row capacities (radial / angular lists); 0 => 160 / 64; <= 255, multiple of 4 */
+} nnp_params;
+
+/* Copies all parameters to the device (the caller keeps its arrays) and allocates every scratch buffer
+ * for up to max_atoms atoms in up to max_mols structures.  cuda_stream is a cudaStream_t (NULL = legacy
+ * default stream).  Synchronises. */
+int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, int device, void *cuda_stream);
+void nnp_destroy(nnp_ctx *ctx);
+const char *nnp_last_error(const nnp_ctx *ctx); /* ctx may be NULL (create failures) */
+
+/* Loads a system: species index per atom (0..n_species-1) and coordinates [n][3] (fp32, Angstrom, need
+ * not be wrapped).  h_box: orthorhombic edge lengths; all zero => non-periodic.  Batches (PAPER.md L41,
+ * L176): d_mol_offsets[n_mols+1] gives each structure's atom range in the concatenated arrays, atoms of
+ * different structures never interact; NULL => one structure.  Periodic batches are not supported.
+ * Invalidates neighbour lists and MD state.  Synchronises (species counts are read back). */
+int nnp_set_system(nnp_ctx *ctx, int n_atoms, const int32_t *d_species, const float *d_xyz,
+                   const float h_box[3], int n_mols, const int32_t *d_mol_offsets);
+
+/* Replaces the coordinates of the loaded system ([n][3], original order); lists stay as they are (the
+ * caller asserts no atom moved more than skin/2 since nnp_build_neighbors). */
+int nnp_set_positions(nnp_ctx *ctx, const float *d_xyz);
+
+/* Stage 1.  Builds the directed radial list {j : r_ij < rcr+skin} and angular list {j : r_ij < rca+skin}
+ * (same structure only, minimum image) with an O(N) cell list; membership is the fp32 predicate of
+ * reading A3.  Re-sorts the internal atom order.  Returns NNP_EBOX if a periodic edge is
+ * shorter than 2*(rcr+skin). */
+int nnp_build_neighbors(nnp_ctx *ctx, float skin);
+
+/* Test hook: rows of list `which` (0 radial, 1 angular) with ORIGINAL atom indices, row i for original
+ * atom i, unsorted.  d_counts[n]; d_list[n][stride], entries beyond counts[i] untouched.  Synchronises;
+ * reports NNP_ECAPACITY. */
+int nnp_get_neighbors(nnp_ctx *ctx, int which, int32_t *d_counts, int32_t *d_list, int stride);
+
+/* Stages 2-4 with the current lists.  d_energy[n_mols] fp64 (mean over nets, + self energies);
+ * d_forces[n][3] fp32 in original order, may be NULL (energy only still runs the full path). */
+int nnp_energy_forces(nnp_ctx *ctx, double *d_energy, float *d_forces);
+
+/* Test hooks (valid after nnp_energy_forces): AEVs [n][aev_len] and per-atom energies [n], original order. */
+int nnp_get_aev(nnp_ctx *ctx, float *d_aev);
+int nnp_get_atomic_energies(nnp_ctx *ctx, float *d_e_atom);
+
+/* Stage 5.  nnp_md_init: velocities [n][3] (A/fs, original order), time step (fs), Verlet skin (A);
+ * builds the lists and evaluates the initial forces.  nnp_md_step: n_steps of velocity Verlet
+ * (v += dt/2 a; x += dt v; rebuild lists iff max_i |x_i - x_i(last build)| > skin/2, decided on the
+ * device; forces; v += dt/2 a), no host synchronisation inside (reading C2). */
+int nnp_md_init(nnp_ctx *ctx, const float *d_vel, float dt_fs, float skin);
+int nnp_md_step(nnp_ctx *ctx, int n_steps);
+
+/* Copies out the current state in original order; any pointer may be NULL.  d_epot/d_ekin: fp64 scalars
+ * (potential energy of the last force evaluation, kinetic energy after the last step, energy units);
+ * d_n_rebuilds: list builds since nnp_md_init (the initial one included).  Asynchronous. */
+int nnp_get_state(nnp_ctx *ctx, float *d_xyz, float *d_vel, double *d_epot, double *d_ekin, int32_t *d_n_rebuilds);
+
+/* Waits for the stream and reports latched device conditions (NNP_ECAPACITY, NNP_ECUDA). */
+int nnp_sync(nnp_ctx *ctx);
+
+/* Host-buffer entry points (the end-to-end path: H2D copies, the same kernels, D2H copies; synchronise).
+ * nnp_energy_forces_host = nnp_set_system + nnp_build_neighbors(skin) + nnp_energy_forces.
+ * nnp_md_step_host: uploads h_xyz/h_vel [n][3] into the running MD state (atoms as in nnp_set_system; lists
+ * are kept and rebuilt by the displacement rule), runs n_steps, downloads positions, velocities, epot, ekin. */
+int nnp_energy_forces_host(nnp_ctx *ctx, int n_atoms, const int32_t *h_species, const float *h_xyz,
+                           const float h_box[3], int n_mols, const int32_t *h_mol_offsets, float skin,
+                           double *h_energy, float *h_forces);
+int nnp_md_step_host(nnp_ctx *ctx, float *h_xyz, float *h_vel, int n_steps, double *h_epot, double *h_ekin);
+
+/* Introspection for the bench: number of kernel launches issued by this ctx so far. */
+int64_t nnp_launch_count(const nnp_ctx *ctx);
+int nnp_aev_len(const nnp_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NNP_H */

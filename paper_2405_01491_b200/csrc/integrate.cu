@@ -1,0 +1,137 @@
+// Stage 5: velocity Verlet with the Verlet-skin rebuild test on the device (fennol_md NVE, PAPER.md L307;
+// skin and rebuild policy L341, reading C2), the per-structure energy sum (L176, reading B5) and the
+// permutations between the caller's atom order and the internal (species, cell) order.
+#include "nnp_internal.cuh"
+
+namespace {
+
+constexpr int T = 256;
+
+// v += dt/2 a(F); x += dt v; request a list rebuild iff |x - xref|^2 > (skin/2)^2 for any atom.
+__global__ void k_kick_drift(int n, float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ frc,
+                             const float4 *__restrict__ xref, const int *__restrict__ spc,
+                             const float *__restrict__ inv_mass_conv, float dt, float half_skin2, int *__restrict__ flags)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < n) {
+        const float k = 0.5f * dt * inv_mass_conv[spc[i]];
+        float4 v = vel[i], x = pos[i];
+        const float4 f = frc[i], r = xref[i];
+        v.x = fmaf(k, f.x, v.x); v.y = fmaf(k, f.y, v.y); v.z = fmaf(k, f.z, v.z);
+        x.x = fmaf(dt, v.x, x.x); x.y = fmaf(dt, v.y, x.y); x.z = fmaf(dt, v.z, x.z);
+        vel[i] = v;
+        pos[i] = x;
+        const float dx = x.x - r.x, dy = x.y - r.y, dz = x.z - r.z;
+        moved = dx * dx + dy * dy + dz * dz > half_skin2;
+    }
+    if (__syncthreads_or(moved) && threadIdx.x == 0) flags[1] = 1;
+}
+
+// v += dt/2 a(F); kinetic energy sum_i m v^2 / (2 accel_conv) accumulated in fp64.
+__global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restrict__ frc, const int *__restrict__ spc,
+                          const float *__restrict__ inv_mass_conv, const float *__restrict__ mass, float dt,
+                          float inv_accel_conv, double *__restrict__ ekin)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float ke = 0.f;
+    if (i < n) {
+        const int s = spc[i];
+        const float k = 0.5f * dt * inv_mass_conv[s];
+        float4 v = vel[i];
+        const float4 f = frc[i];
+        v.x = fmaf(k, f.x, v.x); v.y = fmaf(k, f.y, v.y); v.z = fmaf(k, f.z, v.z);
+        vel[i] = v;
+        ke = 0.5f * mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z) * inv_accel_conv;
+    }
+    __shared__ double part[T / 32];
+    double d = (double)ke;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = d;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < T / 32; ++w) s += part[w];
+        atomicAdd(ekin, s);
+    }
+}
+
+// E_mol += e_atom * inv_nets + e_shift[species]   (fp64 accumulation; block-reduced when there is one structure)
+__global__ void k_energy_reduce(int n, const float *__restrict__ e_atom, const int *__restrict__ spc,
+                                const int *__restrict__ mol, const float *__restrict__ e_shift, float inv_nets,
+                                int single, double *__restrict__ e_mol)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (i < n) e = (double)e_atom[i] * (double)inv_nets + (double)e_shift[spc[i]];
+    if (!single) {
+        if (i < n) atomicAdd(&e_mol[mol[i]], e);
+        return;
+    }
+    __shared__ double part[T / 32];
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = e;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < T / 32; ++w) s += part[w];
+        atomicAdd(&e_mol[0], s);
+    }
+}
+
+__global__ void k_unpermute3(int n, const float4 *__restrict__ src, const int *__restrict__ orig, float *__restrict__ dst)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 v = src[i];
+    const int o = orig[i];
+    dst[3 * o] = v.x; dst[3 * o + 1] = v.y; dst[3 * o + 2] = v.z;
+}
+
+__global__ void k_permute_in3(int n, const float *__restrict__ src, const int *__restrict__ orig, float4 *__restrict__ dst)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int o = orig[i];
+    dst[i] = make_float4(src[3 * o], src[3 * o + 1], src[3 * o + 2], 0.f);
+}
+
+} // namespace
+
+void nnp_launch_kick_drift(nnp_ctx *c)
+{
+    const float hs = 0.5f * c->skin;
+    k_kick_drift<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->pos, c->vel, c->frc, c->xref, c->spc,
+                                                          c->d_inv_mass_conv, c->dt, hs * hs, c->flags);
+    c->launches += 1;
+}
+
+void nnp_launch_kick_ke(nnp_ctx *c)
+{
+    cudaMemsetAsync(c->ekin, 0, sizeof(double), c->stream);
+    k_kick_ke<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->vel, c->frc, c->spc, c->d_inv_mass_conv, c->d_mass,
+                                                       c->dt, 1.0f / c->accel_conv, c->ekin);
+    c->launches += 1;
+}
+
+void nnp_launch_energy_reduce(nnp_ctx *c)
+{
+    cudaMemsetAsync(c->e_mol, 0, sizeof(double) * c->n_mols, c->stream);
+    k_energy_reduce<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->e_atom, c->spc, c->mol, c->d_e_shift,
+                                                             1.0f / (float)c->n_nets, c->n_mols == 1, c->e_mol);
+    c->launches += 1;
+}
+
+void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst)
+{
+    k_unpermute3<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, src, c->orig, dst);
+    c->launches += 1;
+}
+
+void nnp_launch_permute_in3(nnp_ctx *c, const float *src, float4 *dst)
+{
+    k_permute_in3<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, src, c->orig, dst);
+    c->launches += 1;
+}

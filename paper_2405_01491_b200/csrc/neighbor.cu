@@ -1,0 +1,261 @@
+// Stage 1: O(N) cell-list neighbour build (PAPER.md L41-55 GraphGenerator/GraphFilter, L49 "future releases
+// will use cell lists", L341 Verlet skin).  Atoms are re-sorted species-major, cell-minor, so that
+//   * every species bucket is one contiguous row range for the grouped MLP GEMMs (stage 3), and
+//   * every neighbour row, filled species by species, is automatically grouped by neighbour species
+//     (stage 2 needs that: its angular accumulators are per species pair).
+// List membership is the fp32 predicate of reading A3: fixed order, round-to-nearest, no FMA.
+#include "nnp_internal.cuh"
+
+namespace {
+
+constexpr int kWarpsPerBlock = 8;
+
+__device__ __forceinline__ int cell_coord(float x, float L, float invL, float scale, int nc)
+{
+    float w = x - L * floorf(x * invL); // wrap into [0, L]; rounding can give exactly L
+    int c = (int)(w * scale);
+    return min(max(c, 0), nc - 1);
+}
+
+__device__ __forceinline__ int cell_of(const float4 p, const GridInfo &g, int mol)
+{
+    if (!g.periodic) return mol;
+    int cx = cell_coord(p.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
+    int cy = cell_coord(p.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
+    int cz = cell_coord(p.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
+    return (cz * g.nc[1] + cy) * g.nc[0] + cx;
+}
+
+__global__ void k_keys_hist(int n, const float4 *__restrict__ pos, const int *__restrict__ spc,
+                            const int *__restrict__ mol, GridInfo g, int *__restrict__ key,
+                            int *__restrict__ hist, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int k = spc[i] * g.ncell + cell_of(pos[i], g, mol[i]);
+    key[i] = k;
+    atomicAdd(&hist[k], 1);
+}
+
+// Single-block exclusive scan of hist[0..nk) into start[0..nk]; also clears hist for reuse as cursor.
+__global__ void k_scan(int nk, int *__restrict__ hist, int *__restrict__ start, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    __shared__ int warp_sums[32];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int base = 0; base < nk; base += blockDim.x) {
+        int i = base + threadIdx.x;
+        int v = i < nk ? hist[i] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sums[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            int w = lane < (blockDim.x >> 5) ? warp_sums[lane] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += y;
+            }
+            warp_sums[lane] = w; // inclusive
+        }
+        __syncthreads();
+        int prefix = carry + (wid > 0 ? warp_sums[wid - 1] : 0);
+        if (i < nk) { start[i] = prefix + x - v; hist[i] = 0; }
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = prefix + x;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) start[nk] = carry;
+}
+
+__global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ start,
+                          int *__restrict__ cursor, int *__restrict__ order, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int k = key[i];
+    order[start[k] + atomicAdd(&cursor[k], 1)] = i;
+}
+
+// Deterministic order inside each (species, cell) bucket: insertion sort by previous index.
+__global__ void k_sort_buckets(int nk, const int *__restrict__ start, int *__restrict__ order,
+                               int *__restrict__ cursor, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nk) return;
+    cursor[k] = 0; // leave the histogram / cursor array zeroed for the next build
+    int a = start[k], b = start[k + 1];
+    for (int i = a + 1; i < b; ++i) {
+        int v = order[i], j = i - 1;
+        while (j >= a && order[j] > v) { order[j + 1] = order[j]; --j; }
+        order[j + 1] = v;
+    }
+}
+
+__global__ void k_gather(int n, const int *__restrict__ order, const float4 *__restrict__ pos,
+                         const float4 *__restrict__ vel, const int *__restrict__ spc, const int *__restrict__ orig,
+                         const int *__restrict__ mol, float4 *__restrict__ pos_o, float4 *__restrict__ vel_o,
+                         int *__restrict__ spc_o, int *__restrict__ orig_o, int *__restrict__ mol_o, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int s = order[i];
+    pos_o[i] = pos[s];
+    vel_o[i] = vel[s];
+    spc_o[i] = spc[s];
+    orig_o[i] = orig[s];
+    mol_o[i] = mol[s];
+}
+
+__global__ void k_copyback(int n, const float4 *__restrict__ pos_t, const float4 *__restrict__ vel_t,
+                           const int *__restrict__ spc_t, const int *__restrict__ orig_t, const int *__restrict__ mol_t,
+                           float4 *__restrict__ pos, float4 *__restrict__ vel, float4 *__restrict__ xref,
+                           int *__restrict__ spc, int *__restrict__ orig, int *__restrict__ mol, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 p = pos_t[i];
+    pos[i] = p;
+    xref[i] = p;
+    vel[i] = vel_t[i];
+    spc[i] = spc_t[i];
+    orig[i] = orig_t[i];
+    mol[i] = mol_t[i];
+}
+
+// Reading A3: dx = xj - xi; dx -= L*rint(dx*invL); r2 = (dx*dx + dy*dy) + dz*dz; every op round-to-nearest,
+// never contracted into an FMA.
+__device__ __forceinline__ float r2_defined(const float4 a, const float4 b, const GridInfo &g)
+{
+    float dx = __fsub_rn(b.x, a.x), dy = __fsub_rn(b.y, a.y), dz = __fsub_rn(b.z, a.z);
+    if (g.periodic) {
+        dx = __fsub_rn(dx, __fmul_rn(g.box[0], rintf(__fmul_rn(dx, g.inv_box[0]))));
+        dy = __fsub_rn(dy, __fmul_rn(g.box[1], rintf(__fmul_rn(dy, g.inv_box[1]))));
+        dz = __fsub_rn(dz, __fmul_rn(g.box[2], rintf(__fmul_rn(dz, g.inv_box[2]))));
+    }
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+
+// One warp per atom.  For species s = 0..S-1, for the distinct cells within +-1 of the atom's cell
+// (x-adjacent cells are contiguous in the sorted order, so each (y,z) row is at most two ranges), test 32
+// candidates per step with coalesced float4 loads and append hits with ballot compaction.
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_build_lists(int n, int S, const float4 *__restrict__ pos, const int *__restrict__ mol,
+              const int *__restrict__ cell_start, GridInfo g, float rl2_r, float rl2_a, int cap_r, int cap_a,
+              int *__restrict__ nbr_r, int *__restrict__ nbr_a, uint16_t *__restrict__ seg_r,
+              uint16_t *__restrict__ seg_a, int *__restrict__ flags, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+    if (i >= n) return;
+    const float4 pi = pos[i];
+    int cx = 0, cy = 0, cz = 0;
+    int ys[3], zs[3], nys = 1, nzs = 1;
+    int xa[2], xb[2], nxs = 1; // x ranges [xa, xb]
+    if (g.periodic) {
+        cx = cell_coord(pi.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
+        cy = cell_coord(pi.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
+        cz = cell_coord(pi.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
+        // distinct cells among c-1, c, c+1 (mod nc)
+        if (g.nc[1] >= 3) { nys = 3; ys[0] = (cy + g.nc[1] - 1) % g.nc[1]; ys[1] = cy; ys[2] = (cy + 1) % g.nc[1]; }
+        else { nys = g.nc[1]; ys[0] = 0; ys[1] = 1; }
+        if (g.nc[2] >= 3) { nzs = 3; zs[0] = (cz + g.nc[2] - 1) % g.nc[2]; zs[1] = cz; zs[2] = (cz + 1) % g.nc[2]; }
+        else { nzs = g.nc[2]; zs[0] = 0; zs[1] = 1; }
+        if (g.nc[0] <= 3) { xa[0] = 0; xb[0] = g.nc[0] - 1; }
+        else if (cx == 0) { xa[0] = 0; xb[0] = 1; xa[1] = g.nc[0] - 1; xb[1] = g.nc[0] - 1; nxs = 2; }
+        else if (cx == g.nc[0] - 1) { xa[0] = cx - 1; xb[0] = cx; xa[1] = 0; xb[1] = 0; nxs = 2; }
+        else { xa[0] = cx - 1; xb[0] = cx + 1; }
+    } else {
+        ys[0] = 0; zs[0] = 0;
+        xa[0] = xb[0] = mol[i]; // the "cell" of a non-periodic structure is the structure itself
+    }
+    int cnt_r = 0, cnt_a = 0;
+    int *row_r = nbr_r + (size_t)i * cap_r;
+    int *row_a = nbr_a + (size_t)i * cap_a;
+    const unsigned lt = (1u << lane) - 1u;
+    for (int s = 0; s < S; ++s) {
+        if (lane == 0) {
+            seg_r[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_r, cap_r);
+            seg_a[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_a, cap_a);
+        }
+        const int base = s * g.ncell;
+        for (int iz = 0; iz < nzs; ++iz)
+            for (int iy = 0; iy < nys; ++iy) {
+                const int rowbase = base + (zs[iz] * g.nc[1] + ys[iy]) * g.nc[0];
+                for (int ix = 0; ix < nxs; ++ix) {
+                    const int beg = cell_start[rowbase + xa[ix]];
+                    const int end = cell_start[rowbase + xb[ix] + 1];
+                    for (int j0 = beg; j0 < end; j0 += 32) {
+                        const int j = j0 + lane;
+                        bool hr = false, ha = false;
+                        if (j < end && j != i) {
+                            float r2 = r2_defined(pi, pos[j], g);
+                            hr = r2 < rl2_r;
+                            ha = r2 < rl2_a;
+                        }
+                        unsigned mr = __ballot_sync(0xffffffffu, hr);
+                        unsigned ma = __ballot_sync(0xffffffffu, ha);
+                        if (hr) { int p = cnt_r + __popc(mr & lt); if (p < cap_r) row_r[p] = j; }
+                        if (ha) { int p = cnt_a + __popc(ma & lt); if (p < cap_a) row_a[p] = j; }
+                        cnt_r += __popc(mr);
+                        cnt_a += __popc(ma);
+                    }
+                }
+            }
+    }
+    if (lane == 0) {
+        for (int s = S; s < NNP_MAX_SPECIES; ++s) {
+            seg_r[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_r, cap_r);
+            seg_a[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_a, cap_a);
+        }
+        if (cnt_r > cap_r) atomicOr(&flags[0], NNP_FLAG_CAP_R);
+        if (cnt_a > cap_a) atomicOr(&flags[0], NNP_FLAG_CAP_A);
+    }
+}
+
+__global__ void k_finish_build(int *flags, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    flags[1] = 0;
+    flags[2] += 1;
+}
+
+} // namespace
+
+int nnp_launch_build(nnp_ctx *c, const int *cond)
+{
+    const int n = c->n, S = c->S;
+    const int nk = S * c->grid.ncell;
+    const int T = 256, nb = nnp_div_up(n, T);
+    cudaStream_t st = c->stream;
+    // c->cursor doubles as the histogram; it is zero on entry (cleared at create and by k_sort_buckets)
+    k_keys_hist<<<nb, T, 0, st>>>(n, c->pos, c->spc, c->mol, c->grid, c->key, c->cursor, cond);
+    k_scan<<<1, 1024, 0, st>>>(nk, c->cursor, c->cell_start, cond);
+    k_scatter<<<nb, T, 0, st>>>(n, c->key, c->cell_start, c->cursor, c->order, cond);
+    k_sort_buckets<<<nnp_div_up(nk, T), T, 0, st>>>(nk, c->cell_start, c->order, c->cursor, cond);
+    k_gather<<<nb, T, 0, st>>>(n, c->order, c->pos, c->vel, c->spc, c->orig, c->mol, c->pos_tmp, c->vel_tmp,
+                               c->spc_tmp, c->orig_tmp, c->mol_tmp, cond);
+    k_copyback<<<nb, T, 0, st>>>(n, c->pos_tmp, c->vel_tmp, c->spc_tmp, c->orig_tmp, c->mol_tmp, c->pos, c->vel,
+                                 c->xref, c->spc, c->orig, c->mol, cond);
+    const float rl_r = c->aev.rcr + c->skin, rl_a = c->aev.rca + c->skin;
+    k_build_lists<<<nnp_div_up(n, kWarpsPerBlock), kWarpsPerBlock * 32, 0, st>>>(
+        n, S, c->pos, c->mol, c->cell_start, c->grid, rl_r * rl_r, rl_a * rl_a, c->aev.cap_r, c->aev.cap_a,
+        c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->flags, cond);
+    k_finish_build<<<1, 1, 0, st>>>(c->flags, cond);
+    c->launches += 8;
+    return 0;
+}

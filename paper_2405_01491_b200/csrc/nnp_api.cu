@@ -1,0 +1,621 @@
+// C-ABI entry points (include/nnp.h): argument checking, device memory, and the order in which the stage
+// kernels are enqueued.  Every arithmetic step of the path runs in the kernels of neighbor.cu, aev.cu,
+// mlp_simt.cu / mlp_tc.cu and integrate.cu.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "nnp_internal.cuh"
+
+static std::string g_create_error;
+
+#define NNP_FAIL(ctx, code, ...)                              \
+    do {                                                      \
+        char _b[512];                                         \
+        snprintf(_b, sizeof(_b), __VA_ARGS__);                \
+        if (ctx) (ctx)->err = _b; else g_create_error = _b;   \
+        return (code);                                        \
+    } while (0)
+
+#define CU(ctx, call)                                                                              \
+    do {                                                                                           \
+        cudaError_t _e = (call);                                                                   \
+        if (_e != cudaSuccess)                                                                     \
+            NNP_FAIL(ctx, _e == cudaErrorMemoryAllocation ? NNP_ENOMEM : NNP_ECUDA, "%s: %s", #call, \
+                     cudaGetErrorString(_e));                                                      \
+    } while (0)
+
+namespace {
+
+constexpr int T = 256;
+
+__global__ void k_init_system(int n, const int *__restrict__ species, const float *__restrict__ xyz,
+                              const int *__restrict__ mol_offsets, int n_mols, float4 *__restrict__ pos,
+                              float4 *__restrict__ vel, int *__restrict__ spc, int *__restrict__ orig,
+                              int *__restrict__ mol, int *__restrict__ counts, int S, int *__restrict__ bad)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int s = species[i];
+    if (s < 0 || s >= S) { atomicOr(bad, 1); s = 0; }
+    pos[i] = make_float4(xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], 0.f);
+    vel[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    spc[i] = s;
+    orig[i] = i;
+    int m = 0;
+    if (mol_offsets) { // largest m with mol_offsets[m] <= i
+        int lo = 0, hi = n_mols;
+        while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (mol_offsets[mid] <= i) lo = mid; else hi = mid; }
+        m = lo;
+    }
+    mol[i] = m;
+    atomicAdd(&counts[s], 1);
+}
+
+__global__ void k_get_neighbors(int n, const int *__restrict__ nbr, const uint16_t *__restrict__ seg, int cap,
+                                const int *__restrict__ orig, int *__restrict__ counts, int *__restrict__ list, int stride)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int o = orig[i];
+    const int cnt = seg[(size_t)i * NNP_MAX_SPECIES + NNP_MAX_SPECIES - 1];
+    counts[o] = cnt;
+    for (int a = 0; a < cnt && a < stride; ++a) list[(size_t)o * stride + a] = orig[nbr[(size_t)i * cap + a]];
+}
+
+__global__ void k_get_aev(int n, int len, int kpad, const float *__restrict__ G, const int *__restrict__ orig,
+                          float *__restrict__ out)
+{
+    int i = blockIdx.x;
+    if (i >= n) return;
+    const int o = orig[i];
+    for (int q = threadIdx.x; q < len; q += blockDim.x) out[(size_t)o * len + q] = G[(size_t)i * kpad + q];
+}
+
+__global__ void k_get_e_atom(int n, const float *__restrict__ e_atom, const int *__restrict__ spc,
+                             const float *__restrict__ e_shift, float inv_nets, const int *__restrict__ orig,
+                             float *__restrict__ out)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    out[orig[i]] = e_atom[i] * inv_nets + e_shift[spc[i]];
+}
+
+template <typename Tp>
+int dev_alloc(nnp_ctx *c, Tp **p, size_t count)
+{
+    CU(c, cudaMalloc((void **)p, sizeof(Tp) * (count ? count : 1)));
+    return NNP_OK;
+}
+
+LayerW &layer(nnp_ctx *c, int net, int s, int l) { return c->layers[((size_t)net * c->S + s) * NNP_NLAYERS + l]; }
+
+int check_flags(nnp_ctx *c)
+{
+    int h[3];
+    CU(c, cudaMemcpyAsync(h, c->flags, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (h[0] & (NNP_FLAG_CAP_R | NNP_FLAG_CAP_A))
+        NNP_FAIL(c, NNP_ECAPACITY, "neighbour capacity exceeded (%s): recreate with larger cap_r/cap_a",
+                 (h[0] & NNP_FLAG_CAP_R) ? "radial" : "angular");
+    return NNP_OK;
+}
+
+// One GemmBatch per (net, op); op 0..2 forward layers, 3..5 reverse layers.
+void make_batch(nnp_ctx *c, int net, int op, GemmBatch &b)
+{
+    memset(&b, 0, sizeof(b));
+    b.alpha = c->alpha;
+    const int kpad = c->aev.kpad;
+    int ng = 0;
+    for (int s = 0; s < c->S; ++s) {
+        const int off = c->bucket_off[s], M = c->bucket_off[s + 1] - off;
+        if (M == 0) continue;
+        GemmGroup &g = b.g[ng++];
+        const int h1 = c->widths[s][1], h2 = c->widths[s][2], h3 = c->widths[s][3];
+        float *H0 = c->H[0] + (size_t)off * c->hmax[0];
+        float *H1 = c->H[1] + (size_t)off * c->hmax[1];
+        float *H2 = c->H[2] + (size_t)off * c->hmax[2];
+        g.M = M;
+        switch (op) {
+        case 0:
+            g.A = c->G + (size_t)off * kpad; g.lda = kpad; g.K = kpad; g.N = h1;
+            g.B = layer(c, net, s, 0).W; g.Bt = layer(c, net, s, 0).Wt; g.bias = layer(c, net, s, 0).b;
+            g.C = H0; g.ldc = c->hmax[0];
+            break;
+        case 1:
+            g.A = H0; g.lda = c->hmax[0]; g.K = h1; g.N = h2;
+            g.B = layer(c, net, s, 1).W; g.Bt = layer(c, net, s, 1).Wt; g.bias = layer(c, net, s, 1).b;
+            g.C = H1; g.ldc = c->hmax[1];
+            break;
+        case 2:
+            g.A = H1; g.lda = c->hmax[1]; g.K = h2; g.N = h3;
+            g.B = layer(c, net, s, 2).W; g.Bt = layer(c, net, s, 2).Wt; g.bias = layer(c, net, s, 2).b;
+            g.w4 = layer(c, net, s, 3).W; g.e_atom = c->e_atom + off;
+            g.C = H2; g.ldc = c->hmax[2];
+            break;
+        case 3: // delta2 = (delta3 W3^T) * celu'(h2), in place in H1
+            g.A = H2; g.lda = c->hmax[2]; g.K = h3; g.N = h2;
+            g.B = layer(c, net, s, 2).Wt; g.Bt = layer(c, net, s, 2).W;
+            g.C = H1; g.ldc = c->hmax[1];
+            break;
+        case 4: // delta1 = (delta2 W2^T) * celu'(h1), in place in H0
+            g.A = H1; g.lda = c->hmax[1]; g.K = h2; g.N = h1;
+            g.B = layer(c, net, s, 1).Wt; g.Bt = layer(c, net, s, 1).W;
+            g.C = H0; g.ldc = c->hmax[0];
+            break;
+        case 5: // dE/dG (+)= delta1 W1^T
+            g.A = H0; g.lda = c->hmax[0]; g.K = h1; g.N = kpad;
+            g.B = layer(c, net, s, 0).Wt; g.Bt = layer(c, net, s, 0).W;
+            g.C = c->dG + (size_t)off * kpad; g.ldc = kpad;
+            break;
+        }
+    }
+    b.n_groups = ng;
+}
+
+int run_gemm(nnp_ctx *c, const GemmBatch &b, int epi)
+{
+    if (c->mm_mode == NNP_MM_FP32_SIMT) { nnp_launch_gemm_simt(c, b, epi); return NNP_OK; }
+    return nnp_launch_gemm_tc(c, b, epi, c->mm_mode == NNP_MM_3XTF32_TC);
+}
+
+// Stages 2-4 on the current lists: frc, e_mol.
+int run_forces(nnp_ctx *c)
+{
+    CU(c, cudaMemsetAsync(c->frc, 0, sizeof(float4) * (size_t)c->n, c->stream));
+    CU(c, cudaMemsetAsync(c->e_atom, 0, sizeof(float) * (size_t)c->n, c->stream));
+    nnp_launch_aev_forward(c);
+    static const int epi_of[6] = {EPI_CELU, EPI_CELU, EPI_CELU_OUT, EPI_DCELU, EPI_DCELU, EPI_STORE};
+    GemmBatch b;
+    for (int net = 0; net < c->n_nets; ++net)
+        for (int op = 0; op < 6; ++op) {
+            make_batch(c, net, op, b);
+            int epi = epi_of[op];
+            if (op == 5 && net > 0) epi = EPI_ACCUM;
+            int rc = run_gemm(c, b, epi);
+            if (rc != NNP_OK) return rc;
+        }
+    nnp_launch_energy_reduce(c);
+    nnp_launch_aev_backward(c, 1.0f / (float)c->n_nets);
+    CU(c, cudaGetLastError());
+    c->have_forces = 1;
+    return NNP_OK;
+}
+
+int setup_grid(nnp_ctx *c, float skin)
+{
+    GridInfo &g = c->grid;
+    memset(&g, 0, sizeof(g));
+    const float rl = c->aev.rcr + skin;
+    g.periodic = c->periodic;
+    if (c->periodic) {
+        long ncell = 1;
+        for (int d = 0; d < 3; ++d) {
+            if (c->box[d] < 2.0f * rl)
+                NNP_FAIL(c, NNP_EBOX, "box edge %g < 2*(rcr+skin) = %g: minimum image not unique", c->box[d], 2.0f * rl);
+            int nc = (int)floorf(c->box[d] / (rl * 1.0001f));
+            if (nc < 1) nc = 1;
+            if (nc > 128) nc = 128;
+            g.nc[d] = nc;
+            g.box[d] = c->box[d];
+            g.inv_box[d] = 1.0f / c->box[d];
+            g.cell_scale[d] = (float)nc / c->box[d];
+            ncell *= nc;
+        }
+        g.ncell = (int)ncell;
+    } else {
+        g.nc[0] = c->n_mols; g.nc[1] = 1; g.nc[2] = 1;
+        g.ncell = c->n_mols;
+    }
+    const int nk = c->S * g.ncell + 1;
+    if (nk > c->nkeys_cap) {
+        if (c->cell_start) cudaFree(c->cell_start);
+        if (c->cursor) cudaFree(c->cursor);
+        c->cell_start = c->cursor = nullptr;
+        c->nkeys_cap = 0;
+        int rc;
+        if ((rc = dev_alloc(c, &c->cell_start, nk))) return rc;
+        if ((rc = dev_alloc(c, &c->cursor, nk))) return rc;
+        c->nkeys_cap = nk;
+    }
+    CU(c, cudaMemsetAsync(c->cursor, 0, sizeof(int) * nk, c->stream));
+    c->aev.periodic = c->periodic;
+    for (int d = 0; d < 3; ++d) { c->aev.box[d] = g.box[d]; c->aev.inv_box[d] = g.inv_box[d]; }
+    return NNP_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+const char *nnp_last_error(const nnp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int64_t nnp_launch_count(const nnp_ctx *ctx) { return ctx ? ctx->launches : 0; }
+int nnp_aev_len(const nnp_ctx *ctx) { return ctx ? ctx->aev.aev_len : 0; }
+
+void nnp_destroy(nnp_ctx *c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    void *ptrs[] = {c->d_params_blob, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
+                    c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
+                    c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
+                    c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags,
+                    c->io_xyz, c->io_vel, c->io_species};
+    for (void *p : ptrs) if (p) cudaFree(p);
+    delete[] c->layers;
+    delete c;
+}
+
+int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, int device, void *cuda_stream)
+{
+    nnp_ctx *none = nullptr;
+    if (!out || !p) NNP_FAIL(none, NNP_EINVAL, "null argument");
+    *out = nullptr;
+    if (p->n_species < 1 || p->n_species > 7) NNP_FAIL(none, NNP_EINVAL, "n_species must be 1..7");
+    if (p->n_shf_r != NNP_NSHF_R || p->n_shf_a != NNP_NSHF_A || p->n_shf_z != NNP_NSHF_Z || p->n_layers != NNP_NLAYERS)
+        NNP_FAIL(none, NNP_EINVAL, "this build is fixed to 16 radial shifts, 8x4 angular shifts, 4 layers");
+    if (!p->shf_r || !p->shf_a || !p->shf_z || !p->widths || !p->params || !p->mass)
+        NNP_FAIL(none, NNP_EINVAL, "null parameter array");
+    if (max_atoms < 1 || max_mols < 1 || p->n_nets < 1) NNP_FAIL(none, NNP_EINVAL, "max_atoms, max_mols, n_nets must be >= 1");
+    if (!(p->rcr > 0.f) || !(p->rca > 0.f) || p->rca > p->rcr) NNP_FAIL(none, NNP_EINVAL, "need 0 < rca <= rcr");
+    if (p->mm_mode < 0 || p->mm_mode > 2) NNP_FAIL(none, NNP_EINVAL, "bad mm_mode");
+    const int S = p->n_species;
+    const int aev_len = S * NNP_NSHF_R + S * (S + 1) / 2 * NNP_ANG_BLOCK;
+    for (int s = 0; s < S; ++s) {
+        const int *w = p->widths + s * (NNP_NLAYERS + 1);
+        if (w[0] != aev_len || w[4] != 1) NNP_FAIL(none, NNP_EINVAL, "widths[%d] must start with %d and end with 1", s, aev_len);
+        for (int l = 1; l <= 3; ++l)
+            if (w[l] < 32 || w[l] > 256 || w[l] % 32) NNP_FAIL(none, NNP_EINVAL, "hidden widths must be multiples of 32 in [32,256]");
+    }
+    int cap_r = p->cap_r ? p->cap_r : 160, cap_a = p->cap_a ? p->cap_a : 64;
+    if (cap_r < 4 || cap_r > 65532 || cap_r % 4 || cap_a < 4 || cap_a > 65532 || cap_a % 4)
+        NNP_FAIL(none, NNP_EINVAL, "cap_r / cap_a must be multiples of 4");
+
+    if (cudaSetDevice(device) != cudaSuccess) NNP_FAIL(none, NNP_ECUDA, "cudaSetDevice(%d) failed", device);
+    nnp_ctx *c = new nnp_ctx();
+    // new T() value-initialises: every POD member starts at zero
+    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode;
+    c->alpha = p->celu_alpha; c->accel_conv = p->accel_conv;
+    c->stream = (cudaStream_t)cuda_stream; c->device = device;
+    c->max_atoms = max_atoms; c->max_mols = max_mols;
+    c->hmax[0] = c->hmax[1] = c->hmax[2] = 0;
+    for (int s = 0; s < S; ++s)
+        for (int l = 0; l <= NNP_NLAYERS; ++l) {
+            c->widths[s][l] = p->widths[s * (NNP_NLAYERS + 1) + l];
+            if (l >= 1 && l <= 3 && c->widths[s][l] > c->hmax[l - 1]) c->hmax[l - 1] = c->widths[s][l];
+        }
+    AevParams &a = c->aev;
+    a.S = S; a.n_rad = S * NNP_NSHF_R; a.aev_len = aev_len; a.kpad = (aev_len + 31) / 32 * 32;
+    a.cap_r = cap_r; a.cap_a = cap_a;
+    a.rcr = p->rcr; a.rca = p->rca; a.rcr2 = p->rcr * p->rcr; a.rca2 = p->rca * p->rca;
+    a.pi_rcr = (float)(M_PI / (double)p->rcr); a.pi_rca = (float)(M_PI / (double)p->rca);
+    a.eta_r = p->eta_r; a.eta_a = p->eta_a; a.zeta = p->zeta;
+    a.neg_eta_r_log2e = (float)(-(double)p->eta_r * 1.4426950408889634);
+    a.neg_eta_a_log2e = (float)(-(double)p->eta_a * 1.4426950408889634);
+    for (int k = 0; k < NNP_NSHF_R; ++k) a.shf_r[k] = p->shf_r[k];
+    for (int k = 0; k < NNP_NSHF_A; ++k) a.shf_a[k] = p->shf_a[k];
+    for (int k = 0; k < NNP_NSHF_Z; ++k) { a.cos_z[k] = (float)cos((double)p->shf_z[k]); a.sin_z[k] = (float)sin((double)p->shf_z[k]); }
+
+    // ---- weights: W [in_pad][out], Wt [out][in_pad], b [out] for every (net, species, layer)
+    c->layers = new LayerW[(size_t)c->n_nets * S * NNP_NLAYERS];
+    size_t total = 0;
+    for (int net = 0; net < c->n_nets; ++net)
+        for (int s = 0; s < S; ++s)
+            for (int l = 0; l < NNP_NLAYERS; ++l) {
+                LayerW &L = layer(c, net, s, l);
+                L.in = c->widths[s][l]; L.out = c->widths[s][l + 1];
+                L.in_pad = l == 0 ? a.kpad : L.in;
+                total += 2 * (size_t)L.in_pad * L.out + (size_t)((L.out + 3) / 4 * 4);
+            }
+    std::vector<float> blob(total, 0.f);
+    std::vector<double> shift(S, 0.0);
+    {
+        size_t o = 0;
+        const float *src = p->params;
+        for (int net = 0; net < c->n_nets; ++net)
+            for (int s = 0; s < S; ++s)
+                for (int l = 0; l < NNP_NLAYERS; ++l) {
+                    LayerW &L = layer(c, net, s, l);
+                    float *W = &blob[o]; o += (size_t)L.in_pad * L.out;
+                    float *Wt = &blob[o]; o += (size_t)L.in_pad * L.out;
+                    float *b = &blob[o]; o += (size_t)((L.out + 3) / 4 * 4);
+                    for (int i = 0; i < L.in; ++i)
+                        for (int j = 0; j < L.out; ++j) {
+                            const float v = src[(size_t)i * L.out + j];
+                            W[(size_t)i * L.out + j] = v;
+                            Wt[(size_t)j * L.in_pad + i] = v;
+                        }
+                    src += (size_t)L.in * L.out;
+                    for (int j = 0; j < L.out; ++j) b[j] = src[j];
+                    src += L.out;
+                    if (l == NNP_NLAYERS - 1) shift[s] += (double)b[0] / c->n_nets;
+                    L.W = (float *)(W - blob.data()); L.Wt = (float *)(Wt - blob.data()); L.b = (float *)(b - blob.data());
+                }
+    }
+    int rc;
+#define TRY(x) do { if ((rc = (x)) != NNP_OK) { g_create_error = c->err; nnp_destroy(c); return rc; } } while (0)
+#define TRYCU(x) do { cudaError_t _e = (x); if (_e != cudaSuccess) { g_create_error = std::string(#x ": ") + cudaGetErrorString(_e); nnp_destroy(c); return _e == cudaErrorMemoryAllocation ? NNP_ENOMEM : NNP_ECUDA; } } while (0)
+    TRY(dev_alloc(c, &c->d_params_blob, total));
+    TRYCU(cudaMemcpy(c->d_params_blob, blob.data(), sizeof(float) * total, cudaMemcpyHostToDevice));
+    for (size_t q = 0; q < (size_t)c->n_nets * S * NNP_NLAYERS; ++q) { // offsets -> device pointers
+        LayerW &L = c->layers[q];
+        L.W = c->d_params_blob + (size_t)L.W; L.Wt = c->d_params_blob + (size_t)L.Wt; L.b = c->d_params_blob + (size_t)L.b;
+    }
+    float imc[NNP_MAX_SPECIES] = {0}, ms[NNP_MAX_SPECIES] = {0}, es[NNP_MAX_SPECIES] = {0};
+    for (int s = 0; s < S; ++s) {
+        if (!(p->mass[s] > 0.f)) { g_create_error = "mass must be > 0"; nnp_destroy(c); return NNP_EINVAL; }
+        c->mass[s] = ms[s] = p->mass[s];
+        imc[s] = p->accel_conv / p->mass[s];
+        c->e_shift[s] = es[s] = (float)(shift[s] + (p->self_energy ? (double)p->self_energy[s] : 0.0));
+    }
+    TRY(dev_alloc(c, &c->d_inv_mass_conv, NNP_MAX_SPECIES));
+    TRY(dev_alloc(c, &c->d_mass, NNP_MAX_SPECIES));
+    TRY(dev_alloc(c, &c->d_e_shift, NNP_MAX_SPECIES));
+    TRYCU(cudaMemcpy(c->d_inv_mass_conv, imc, sizeof(imc), cudaMemcpyHostToDevice));
+    TRYCU(cudaMemcpy(c->d_mass, ms, sizeof(ms), cudaMemcpyHostToDevice));
+    TRYCU(cudaMemcpy(c->d_e_shift, es, sizeof(es), cudaMemcpyHostToDevice));
+
+    const size_t N = (size_t)max_atoms;
+    TRY(dev_alloc(c, &c->pos, N)); TRY(dev_alloc(c, &c->pos_tmp, N));
+    TRY(dev_alloc(c, &c->vel, N)); TRY(dev_alloc(c, &c->vel_tmp, N));
+    TRY(dev_alloc(c, &c->frc, N)); TRY(dev_alloc(c, &c->xref, N));
+    TRY(dev_alloc(c, &c->spc, N)); TRY(dev_alloc(c, &c->spc_tmp, N));
+    TRY(dev_alloc(c, &c->orig, N)); TRY(dev_alloc(c, &c->orig_tmp, N));
+    TRY(dev_alloc(c, &c->mol, N)); TRY(dev_alloc(c, &c->mol_tmp, N));
+    TRY(dev_alloc(c, &c->mol_offsets, (size_t)max_mols + 1));
+    TRY(dev_alloc(c, &c->key, N)); TRY(dev_alloc(c, &c->order, N));
+    TRY(dev_alloc(c, &c->nbr_r, N * cap_r)); TRY(dev_alloc(c, &c->nbr_a, N * cap_a));
+    TRY(dev_alloc(c, &c->seg_r, N * NNP_MAX_SPECIES)); TRY(dev_alloc(c, &c->seg_a, N * NNP_MAX_SPECIES));
+    TRY(dev_alloc(c, &c->G, N * a.kpad));
+    if (c->n_nets == 1) c->dG = c->G; // dE/dG overwrites G once layer 1 has consumed it
+    else TRY(dev_alloc(c, &c->dG, N * a.kpad));
+    for (int l = 0; l < 3; ++l) TRY(dev_alloc(c, &c->H[l], N * c->hmax[l]));
+    TRY(dev_alloc(c, &c->e_atom, N));
+    TRY(dev_alloc(c, &c->e_mol, (size_t)max_mols));
+    TRY(dev_alloc(c, &c->ekin, 1));
+    TRY(dev_alloc(c, &c->flags, 16));
+    TRY(dev_alloc(c, &c->io_xyz, 3 * N)); TRY(dev_alloc(c, &c->io_vel, 3 * N)); TRY(dev_alloc(c, &c->io_species, N));
+    TRYCU(cudaMemset(c->flags, 0, sizeof(int) * 16));
+    TRYCU(cudaMemset(c->ekin, 0, sizeof(double)));
+    TRYCU(cudaDeviceSynchronize());
+#undef TRY
+#undef TRYCU
+    *out = c;
+    return NNP_OK;
+}
+
+int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const float *d_xyz, const float h_box[3],
+                   int n_mols, const int32_t *d_mol_offsets)
+{
+    if (!c) return NNP_EINVAL;
+    if (!d_species || !d_xyz || !h_box) NNP_FAIL(c, NNP_EINVAL, "null argument");
+    if (n_atoms < 0 || n_atoms > c->max_atoms) NNP_FAIL(c, NNP_EINVAL, "n_atoms %d outside [0, max_atoms=%d]", n_atoms, c->max_atoms);
+    if (!d_mol_offsets) n_mols = 1;
+    if (n_mols < 1 || n_mols > c->max_mols) NNP_FAIL(c, NNP_EINVAL, "n_mols %d outside [1, max_mols=%d]", n_mols, c->max_mols);
+    const int nper = (h_box[0] > 0.f) + (h_box[1] > 0.f) + (h_box[2] > 0.f);
+    if (nper != 0 && nper != 3) NNP_FAIL(c, NNP_EINVAL, "box must be all zero (non-periodic) or all positive");
+    if (nper == 3 && n_mols > 1) NNP_FAIL(c, NNP_EINVAL, "periodic batches are not supported");
+    CU(c, cudaSetDevice(c->device));
+    c->n = n_atoms; c->n_mols = n_mols; c->periodic = nper == 3;
+    for (int d = 0; d < 3; ++d) c->box[d] = h_box[d];
+    c->have_system = 1; c->have_lists = 0; c->have_forces = 0; c->md_ready = 0;
+    int *bins = c->flags + 8; // [8..15] species histogram, [3] bad-species marker
+    CU(c, cudaMemsetAsync(c->flags, 0, sizeof(int) * 16, c->stream));
+    int h_counts[NNP_MAX_SPECIES] = {0};
+    if (n_atoms > 0) {
+        if (d_mol_offsets)
+            CU(c, cudaMemcpyAsync(c->mol_offsets, d_mol_offsets, sizeof(int) * (n_mols + 1), cudaMemcpyDeviceToDevice, c->stream));
+        k_init_system<<<nnp_div_up(n_atoms, T), T, 0, c->stream>>>(n_atoms, d_species, d_xyz, d_mol_offsets ? c->mol_offsets : nullptr,
+                                                                   n_mols, c->pos, c->vel, c->spc, c->orig, c->mol, bins, c->S,
+                                                                   c->flags + 3);
+        c->launches += 1;
+        int bad = 0;
+        CU(c, cudaMemcpyAsync(h_counts, bins, sizeof(int) * NNP_MAX_SPECIES, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaMemcpyAsync(&bad, c->flags + 3, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        if (bad) { c->have_system = 0; NNP_FAIL(c, NNP_EINVAL, "species index outside [0, n_species)"); }
+    }
+    c->bucket_off[0] = 0;
+    for (int s = 0; s < NNP_MAX_SPECIES; ++s) c->bucket_off[s + 1] = c->bucket_off[s] + (s < c->S ? h_counts[s] : 0);
+    return NNP_OK;
+}
+
+int nnp_set_positions(nnp_ctx *c, const float *d_xyz)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_system || !d_xyz) NNP_FAIL(c, NNP_EINVAL, "no system loaded / null argument");
+    if (c->n == 0) return NNP_OK;
+    nnp_launch_permute_in3(c, d_xyz, c->pos);
+    c->have_forces = 0;
+    return NNP_OK;
+}
+
+int nnp_build_neighbors(nnp_ctx *c, float skin)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "nnp_set_system first");
+    if (!(skin >= 0.f)) NNP_FAIL(c, NNP_EINVAL, "skin must be >= 0");
+    CU(c, cudaSetDevice(c->device));
+    c->skin = skin;
+    int rc = setup_grid(c, skin);
+    if (rc) return rc;
+    if (c->n > 0) nnp_launch_build(c, nullptr);
+    CU(c, cudaGetLastError());
+    c->have_lists = 1;
+    c->have_forces = 0;
+    return NNP_OK;
+}
+
+int nnp_get_neighbors(nnp_ctx *c, int which, int32_t *d_counts, int32_t *d_list, int stride)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_lists) NNP_FAIL(c, NNP_ESTALE, "no neighbour list");
+    if (!d_counts || !d_list || stride < 1 || (which != 0 && which != 1)) NNP_FAIL(c, NNP_EINVAL, "bad argument");
+    if (c->n > 0) {
+        k_get_neighbors<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, which ? c->nbr_a : c->nbr_r, which ? c->seg_a : c->seg_r,
+                                                                 which ? c->aev.cap_a : c->aev.cap_r, c->orig, d_counts, d_list, stride);
+        c->launches += 1;
+    }
+    return check_flags(c);
+}
+
+static int energy_forces_impl(nnp_ctx *c, double *d_energy /* nullptr: leave in e_mol */, float *d_forces)
+{
+    if (!c->have_lists) NNP_FAIL(c, NNP_ESTALE, "nnp_build_neighbors first");
+    CU(c, cudaSetDevice(c->device));
+    if (c->n == 0) {
+        CU(c, cudaMemsetAsync(c->e_mol, 0, sizeof(double) * c->n_mols, c->stream));
+    } else {
+        int rc = run_forces(c);
+        if (rc) return rc;
+        if (d_forces) nnp_launch_unpermute3(c, c->frc, d_forces);
+    }
+    if (d_energy) CU(c, cudaMemcpyAsync(d_energy, c->e_mol, sizeof(double) * c->n_mols, cudaMemcpyDeviceToDevice, c->stream));
+    return NNP_OK;
+}
+
+int nnp_energy_forces(nnp_ctx *c, double *d_energy, float *d_forces)
+{
+    if (!c) return NNP_EINVAL;
+    if (!d_energy) NNP_FAIL(c, NNP_EINVAL, "null energy pointer");
+    return energy_forces_impl(c, d_energy, d_forces);
+}
+
+int nnp_get_aev(nnp_ctx *c, float *d_aev)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_lists || !d_aev) NNP_FAIL(c, NNP_ESTALE, "no neighbour list / null argument");
+    if (c->n == 0) return NNP_OK;
+    nnp_launch_aev_forward(c); // G may have been overwritten by dE/dG: recompute
+    k_get_aev<<<c->n, 128, 0, c->stream>>>(c->n, c->aev.aev_len, c->aev.kpad, c->G, c->orig, d_aev);
+    c->launches += 1;
+    c->have_forces = 0;
+    CU(c, cudaGetLastError());
+    return NNP_OK;
+}
+
+int nnp_get_atomic_energies(nnp_ctx *c, float *d_e_atom)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_forces || !d_e_atom) NNP_FAIL(c, NNP_ESTALE, "nnp_energy_forces first / null argument");
+    k_get_e_atom<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->e_atom, c->spc, c->d_e_shift, 1.0f / c->n_nets, c->orig, d_e_atom);
+    c->launches += 1;
+    return NNP_OK;
+}
+
+int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "nnp_set_system first");
+    if (!d_vel || !(dt_fs > 0.f) || !(skin > 0.f)) NNP_FAIL(c, NNP_EINVAL, "need velocities, dt > 0, skin > 0");
+    if (c->n_mols != 1) NNP_FAIL(c, NNP_EINVAL, "MD runs on one structure");
+    if (c->n == 0) NNP_FAIL(c, NNP_EINVAL, "empty system");
+    CU(c, cudaSetDevice(c->device));
+    nnp_launch_permute_in3(c, d_vel, c->vel);
+    c->dt = dt_fs;
+    CU(c, cudaMemsetAsync(c->flags + 1, 0, sizeof(int) * 2, c->stream)); // rebuild request and counter
+    int rc = nnp_build_neighbors(c, skin);
+    if (rc) return rc;
+    // the initial build counts as rebuild 1 (k_finish_build)
+    rc = run_forces(c);
+    if (rc) return rc;
+    const float dt = c->dt;
+    c->dt = 0.f;
+    nnp_launch_kick_ke(c); // kinetic energy of the initial velocities
+    c->dt = dt;
+    c->md_ready = 1;
+    return NNP_OK;
+}
+
+int nnp_md_step(nnp_ctx *c, int n_steps)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->md_ready) NNP_FAIL(c, NNP_ESTALE, "nnp_md_init first");
+    if (n_steps < 0) NNP_FAIL(c, NNP_EINVAL, "n_steps < 0");
+    CU(c, cudaSetDevice(c->device));
+    for (int step = 0; step < n_steps; ++step) {
+        nnp_launch_kick_drift(c);
+        nnp_launch_build(c, c->flags + 1); // every kernel returns at once unless the drift requested a rebuild
+        int rc = run_forces(c);
+        if (rc) return rc;
+        nnp_launch_kick_ke(c);
+    }
+    return NNP_OK;
+}
+
+int nnp_get_state(nnp_ctx *c, float *d_xyz, float *d_vel, double *d_epot, double *d_ekin, int32_t *d_n_rebuilds)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "no system");
+    if (c->n > 0) {
+        if (d_xyz) nnp_launch_unpermute3(c, c->pos, d_xyz);
+        if (d_vel) nnp_launch_unpermute3(c, c->vel, d_vel);
+    }
+    if (d_epot) CU(c, cudaMemcpyAsync(d_epot, c->e_mol, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    if (d_ekin) CU(c, cudaMemcpyAsync(d_ekin, c->ekin, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    if (d_n_rebuilds) CU(c, cudaMemcpyAsync(d_n_rebuilds, c->flags + 2, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
+    return NNP_OK;
+}
+
+int nnp_sync(nnp_ctx *c)
+{
+    if (!c) return NNP_EINVAL;
+    CU(c, cudaSetDevice(c->device));
+    return check_flags(c);
+}
+
+int nnp_energy_forces_host(nnp_ctx *c, int n_atoms, const int32_t *h_species, const float *h_xyz, const float h_box[3],
+                           int n_mols, const int32_t *h_mol_offsets, float skin, double *h_energy, float *h_forces)
+{
+    if (!c) return NNP_EINVAL;
+    if (!h_species || !h_xyz || !h_box || !h_energy) NNP_FAIL(c, NNP_EINVAL, "null argument");
+    if (n_atoms < 0 || n_atoms > c->max_atoms) NNP_FAIL(c, NNP_EINVAL, "n_atoms outside [0, max_atoms]");
+    if (h_mol_offsets && (n_mols < 1 || n_mols > c->max_mols)) NNP_FAIL(c, NNP_EINVAL, "n_mols outside [1, max_mols]");
+    CU(c, cudaSetDevice(c->device));
+    CU(c, cudaMemcpyAsync(c->io_species, h_species, sizeof(int) * (size_t)n_atoms, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->io_xyz, h_xyz, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, c->stream));
+    int *d_off = nullptr;
+    if (h_mol_offsets) {
+        d_off = c->key; // scratch until the build; set_system copies it into mol_offsets
+        if (n_mols + 1 > c->max_atoms) NNP_FAIL(c, NNP_EINVAL, "n_mols + 1 > max_atoms");
+        CU(c, cudaMemcpyAsync(d_off, h_mol_offsets, sizeof(int) * (n_mols + 1), cudaMemcpyHostToDevice, c->stream));
+    }
+    int rc = nnp_set_system(c, n_atoms, c->io_species, c->io_xyz, h_box, n_mols, d_off);
+    if (rc) return rc;
+    if ((rc = nnp_build_neighbors(c, skin))) return rc;
+    // energies stay in e_mol; forces go through io_vel as staging
+    if ((rc = energy_forces_impl(c, nullptr, h_forces ? c->io_vel : nullptr))) return rc;
+    CU(c, cudaMemcpyAsync(h_energy, c->e_mol, sizeof(double) * c->n_mols, cudaMemcpyDeviceToHost, c->stream));
+    if (h_forces && n_atoms > 0)
+        CU(c, cudaMemcpyAsync(h_forces, c->io_vel, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyDeviceToHost, c->stream));
+    return check_flags(c);
+}
+
+int nnp_md_step_host(nnp_ctx *c, float *h_xyz, float *h_vel, int n_steps, double *h_epot, double *h_ekin)
+{
+    if (!c) return NNP_EINVAL;
+    if (!c->md_ready) NNP_FAIL(c, NNP_ESTALE, "nnp_md_init first");
+    if (!h_xyz || !h_vel) NNP_FAIL(c, NNP_EINVAL, "null argument");
+    CU(c, cudaSetDevice(c->device));
+    const size_t bytes = sizeof(float) * 3 * (size_t)c->n;
+    CU(c, cudaMemcpyAsync(c->io_xyz, h_xyz, bytes, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->io_vel, h_vel, bytes, cudaMemcpyHostToDevice, c->stream));
+    nnp_launch_permute_in3(c, c->io_xyz, c->pos);
+    nnp_launch_permute_in3(c, c->io_vel, c->vel);
+    int rc = nnp_md_step(c, n_steps);
+    if (rc) return rc;
+    nnp_launch_unpermute3(c, c->pos, c->io_xyz);
+    nnp_launch_unpermute3(c, c->vel, c->io_vel);
+    CU(c, cudaMemcpyAsync(h_xyz, c->io_xyz, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaMemcpyAsync(h_vel, c->io_vel, bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (h_epot) CU(c, cudaMemcpyAsync(h_epot, c->e_mol, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (h_ekin) CU(c, cudaMemcpyAsync(h_ekin, c->ekin, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    return check_flags(c);
+}
+
+} // extern "C"

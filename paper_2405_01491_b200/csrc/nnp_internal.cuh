@@ -1,0 +1,155 @@
+// Internal declarations of the CUDA path (sm_100a).  Not part of the C-ABI (include/nnp.h).
+// Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "../../include/nnp.h"
+
+#define NNP_MAX_SPECIES 8
+#define NNP_NSHF_R 16
+#define NNP_NSHF_A 8
+#define NNP_NSHF_Z 4
+#define NNP_ANG_BLOCK (NNP_NSHF_A * NNP_NSHF_Z) /* 32 features per species pair */
+#define NNP_NLAYERS 4
+
+// Device error flags latched by kernels, reported by synchronising calls.
+enum { NNP_FLAG_CAP_R = 1, NNP_FLAG_CAP_A = 2 };
+
+// ---- periodic cell grid / molecule bins (stage 1) ------------------------------------------------
+struct GridInfo {
+    int nc[3];        // cells per dimension (periodic) or {n_mols,1,1} (batched molecules)
+    int ncell;        // nc[0]*nc[1]*nc[2]
+    int periodic;     // 1: orthorhombic minimum image; 0: bins are molecules
+    float box[3];
+    float inv_box[3]; // 1.0f / box (IEEE division on the host)
+    float cell_scale[3]; // nc / box
+};
+
+// ---- AEV constants (stage 2/4), passed to kernels by value --------------------------------------
+struct AevParams {
+    int S;           // species
+    int n_rad;       // S*16
+    int aev_len;     // n_rad + S(S+1)/2*32
+    int kpad;        // row stride of G / dG in floats (aev_len rounded up to 32 -> 1024)
+    int cap_r, cap_a;
+    float rcr, rca;
+    float rcr2, rca2;
+    float pi_rcr, pi_rca;      // pi / cutoff
+    float neg_eta_r_log2e;     // -eta_r * log2(e)
+    float neg_eta_a_log2e;
+    float eta_r, eta_a, zeta;
+    float shf_r[NNP_NSHF_R];
+    float shf_a[NNP_NSHF_A];
+    float cos_z[NNP_NSHF_Z], sin_z[NNP_NSHF_Z];
+    int periodic;
+    float box[3], inv_box[3];
+};
+
+// ---- grouped GEMM description (stage 3/4) --------------------------------------------------------
+enum GemmEpilogue {
+    EPI_CELU = 0,     // C = celu(acc + bias)
+    EPI_CELU_OUT = 1, // h = celu(acc + bias); e_atom[m] += sum_n h*w4[n]; C = w4[n] * celu'(h)
+    EPI_DCELU = 2,    // C = acc * celu'(H) with H read from C (in place)
+    EPI_STORE = 3,    // C = acc
+    EPI_ACCUM = 4     // C += acc
+};
+
+struct GemmGroup {
+    const float *A;   // [M][lda]   K-contiguous rows
+    const float *B;   // [K][N]     row-major (SIMT path)
+    const float *Bt;  // [N][K]     K-contiguous rows (tensor-core path)
+    float *C;         // [M][ldc]
+    const float *bias; // [N] or nullptr
+    const float *w4;  // [N] last-layer weights (EPI_CELU_OUT)
+    float *e_atom;    // [M] (EPI_CELU_OUT)
+    int M, N, K, lda, ldc;
+};
+
+struct GemmBatch {
+    GemmGroup g[NNP_MAX_SPECIES];
+    int n_groups;
+    int tile_off[NNP_MAX_SPECIES + 1]; // prefix sum of M tiles per group (tile height given at launch)
+    float alpha;                       // CELU alpha
+};
+
+// ---- context -----------------------------------------------------------------------------------
+struct LayerW {
+    float *W;  // device [in_pad][out]
+    float *Wt; // device [out][in_pad]
+    float *b;  // device [out]
+    int in, in_pad, out;
+};
+
+struct nnp_ctx {
+    // model
+    int S, n_nets, mm_mode;
+    int widths[NNP_MAX_SPECIES][NNP_NLAYERS + 1];
+    int hmax[3]; // max hidden widths over species (strides of the activation buffers)
+    AevParams aev;
+    float alpha, accel_conv;
+    float mass[NNP_MAX_SPECIES];
+    float e_shift[NNP_MAX_SPECIES]; // mean over nets of last-layer bias + self energy
+    LayerW *layers;                 // host array [n_nets][S][4]
+    float *d_params_blob;           // all device weights in one allocation
+    float *d_inv_mass_conv;         // [S] accel_conv / mass
+    float *d_mass;                  // [S]
+    float *d_e_shift;               // [S]
+
+    cudaStream_t stream;
+    int device, max_atoms, max_mols;
+    int64_t launches;
+    std::string err;
+
+    // system
+    int n, n_mols, periodic, have_system, have_lists, have_forces, md_ready;
+    float box[3];
+    int bucket_off[NNP_MAX_SPECIES + 1]; // species-major internal order: atoms of species s are [off[s], off[s+1])
+    GridInfo grid;
+    float skin, dt;
+
+    // per-atom state, internal order
+    float4 *pos, *pos_tmp; // xyz, w unused
+    float4 *vel, *vel_tmp;
+    float4 *frc;           // forces (fp32 atomics)
+    float4 *xref;          // positions at the last list build
+    int *spc, *spc_tmp;    // species
+    int *orig, *orig_tmp;  // internal -> original index
+    int *mol, *mol_tmp;    // structure id
+    int *mol_offsets;      // [n_mols+1] device copy
+    // sort scratch
+    int *key, *order, *cell_start, *cursor; // cell_start/cursor: [S*ncell+1]
+    int nkeys_cap;
+    // lists
+    int *nbr_r, *nbr_a;      // [n][cap]
+    uint16_t *seg_r, *seg_a; // [n][8] species-segment start offsets; entries S..7 = row length (S <= 7)
+    // features and network
+    float *G, *dG;           // [n][kpad]
+    float *H[3];             // activations / deltas [n][hmax[l]]
+    float *e_atom;           // [n]
+    double *e_mol;           // [max_mols]
+    double *ekin;            // scalar
+    int *flags;              // [0] error flags, [1] rebuild request, [2] rebuild count
+    // staging for the host entry points
+    float *io_xyz, *io_vel;  // [n][3]
+    int *io_species;
+};
+
+// ---- launches implemented across the .cu files --------------------------------------------------
+// neighbor.cu
+int nnp_launch_build(nnp_ctx *c, const int *cond_flag); // sort + lists; cond_flag != nullptr: only if *cond_flag != 0
+// aev.cu
+void nnp_launch_aev_forward(nnp_ctx *c);
+void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets);
+// mlp_simt.cu / mlp_tc.cu
+void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi);
+int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3);
+// integrate.cu
+void nnp_launch_kick_drift(nnp_ctx *c);
+void nnp_launch_kick_ke(nnp_ctx *c);
+void nnp_launch_energy_reduce(nnp_ctx *c);
+void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst);
+void nnp_launch_permute_in3(nnp_ctx *c, const float *src, float4 *dst); // dst[i] = src[orig[i]]
+
+static inline int nnp_div_up(int a, int b) { return (a + b - 1) / b; }

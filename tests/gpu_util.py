@@ -1,0 +1,64 @@
+"""Helpers for the -m gpu parity tests: run the CUDA path through the C-ABI binding and the oracle on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): neighbour lists exactly as sets, |dE|/|E| <= 1e-5,
+max |dF| <= 1e-3 energy units / Angstrom."""
+import numpy as np
+import torch
+
+from oracle import nnp_oracle as orc
+from paper_2405_01491_b200 import inputs, nnp
+
+E_RTOL = 1e-5
+F_ATOL = 1e-3
+# reading B7: last-layer scale that brings the random-weight RMS force on water to ~20 kcal/mol/A
+# (oracle RMS force at scale 1 is 0.30; tests/golden/force_scale.md)
+FORCE_SCALE = 66.0
+
+
+def make_model(n_nets=1, seed=inputs.SEED0, widths=inputs.WIDTHS, scale=FORCE_SCALE, bias_std=0.05, self_energy=None):
+    consts = inputs.ani2x_constants()
+    params = inputs.make_weights(seed, n_nets, widths=widths, last_layer_scale=scale, bias_std=bias_std)
+    omodel = orc.OracleModel(consts, widths, params, n_nets, self_energy=self_energy)
+    return consts, widths, params, omodel
+
+
+def gpu_create(consts, widths, params, n_nets, max_atoms, max_mols=1, mm_mode=0, cap_r=0, cap_a=0, self_energy=None):
+    p, keep = nnp.make_params(consts, widths, params, inputs.MASS, inputs.ACCEL_CONV, n_nets=n_nets,
+                              self_energy=self_energy, mm_mode=mm_mode, cap_r=cap_r, cap_a=cap_a)
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = nnp.nnp_create(p, max_atoms, max_mols, 0, stream)
+    return ctx
+
+
+def gpu_energy_forces(ctx, species, xyz, box, mol_offsets=None, skin=0.0):
+    dev = torch.device("cuda:0")
+    n = len(species)
+    d_sp = torch.as_tensor(np.asarray(species, dtype=np.int32), device=dev)
+    d_x = torch.as_tensor(np.asarray(xyz, dtype=np.float32), device=dev).contiguous()
+    n_mols = 1 if mol_offsets is None else len(mol_offsets) - 1
+    d_mo = None if mol_offsets is None else torch.as_tensor(np.asarray(mol_offsets, dtype=np.int32), device=dev)
+    nnp.nnp_set_system(ctx, n, d_sp, d_x, box, n_mols, d_mo)
+    nnp.nnp_build_neighbors(ctx, skin)
+    d_E = torch.zeros(n_mols, dtype=torch.float64, device=dev)
+    d_F = torch.zeros((max(n, 1), 3), dtype=torch.float32, device=dev)
+    nnp.nnp_energy_forces(ctx, d_E, d_F)
+    nnp.nnp_sync(ctx)
+    return d_E.cpu().numpy(), d_F.cpu().numpy()[:n].astype(np.float64)
+
+
+def gpu_neighbors(ctx, which, n, stride=256):
+    dev = torch.device("cuda:0")
+    d_c = torch.zeros(max(n, 1), dtype=torch.int32, device=dev)
+    d_l = torch.full((max(n, 1), stride), -1, dtype=torch.int32, device=dev)
+    nnp.nnp_get_neighbors(ctx, which, d_c, d_l, stride)
+    c = d_c.cpu().numpy()
+    l = d_l.cpu().numpy()
+    return [np.sort(l[i, :c[i]]) for i in range(n)]
+
+
+def assert_parity(Eg, Fg, ref, e_rtol=E_RTOL, f_atol=F_ATOL):
+    Eo, Fo = ref["E"], ref["F"]
+    for m in range(len(Eo)):
+        assert abs(Eg[m] - Eo[m]) <= e_rtol * abs(Eo[m]), ("energy", m, Eg[m], Eo[m], abs(Eg[m] - Eo[m]) / abs(Eo[m]))
+    err = np.abs(Fg - Fo).max() if len(Fo) else 0.0
+    assert err <= f_atol, ("force max abs err", err, "rms force", np.sqrt((Fo ** 2).sum(1).mean()))
+    return err

@@ -1,0 +1,258 @@
+"""-m gpu parity tests: the CUDA path (through the C-ABI binding) against the fp64 oracle on the same seeded
+inputs.  Bars (BASELINE.json): neighbour lists exactly as sets; |dE|/|E| <= 1e-5; max |dF| <= 1e-3."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import nnp_oracle as orc          # noqa: E402
+from paper_2405_01491_b200 import inputs, nnp  # noqa: E402
+from tests import gpu_util as U               # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def model1():
+    return U.make_model(1)
+
+
+def _rlist(rc, skin):
+    return float(np.float32(rc) + np.float32(skin))
+
+
+def _check_lists(ctx, xyz, box, n, skin, mol_id=None, method="brute"):
+    for which, rc in ((0, 5.1), (1, 3.5)):
+        got = U.gpu_neighbors(ctx, which, n)
+        ref = orc.neighbors(xyz, box, _rlist(rc, skin), mol_id=mol_id, fp32_pred=True, method=method)
+        bad = [i for i in range(n) if not np.array_equal(got[i], ref[i])]
+        assert not bad, (which, len(bad), bad[:5])
+
+
+# ---------------------------------------------------------------- config 1: 64 waters, tiny box (2 cells / side)
+def test_config1_water64(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(64, 12.42)
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp))
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        _check_lists(ctx, xyz, box, len(sp), 0.0)
+        ref = orc.energy_forces(om, sp, xyz, box)
+        U.assert_parity(Eg, Fg, ref)
+        # AEV hook, element by element
+        d_aev = torch.zeros((len(sp), 1008), dtype=torch.float32, device="cuda")
+        nnp.nnp_get_aev(ctx, d_aev)
+        nnp.nnp_sync(ctx)
+        aev_ref = orc.energy_forces(om, sp, xyz, box, want_forces=False, want_aev=True)["aev"]
+        assert np.abs(d_aev.cpu().numpy() - aev_ref).max() < 2e-5 * max(1.0, np.abs(aev_ref).max())
+        # with a skin: same energies and forces from the longer lists (reading A4)
+        Eg2, Fg2 = U.gpu_energy_forces(ctx, sp, xyz, box, skin=0.5)
+        _check_lists(ctx, xyz, box, len(sp), 0.5)
+        U.assert_parity(Eg2, Fg2, ref)
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_unwrapped_coordinates_and_box_error(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(64, 12.42, seed=7)
+    xyz = (xyz + np.random.default_rng(0).integers(-3, 4, size=xyz.shape) * box).astype(np.float32).astype(np.float64)
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp))
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        _check_lists(ctx, xyz, box, len(sp), 0.0)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box))
+        with pytest.raises(nnp.NnpError) as e:      # 12.42 < 2*(5.1+1.2)
+            U.gpu_energy_forces(ctx, sp, xyz, box, skin=1.2)
+        assert e.value.status == nnp.NNP_EBOX
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- medium water box: several cells, ragged GEMM tiles
+def test_water_1000_cells_and_tails(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(1000, seed=3)           # 3000 atoms, L = 31.04 A -> 6 cells / side at 5.1 A
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp))
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        _check_lists(ctx, xyz, box, len(sp), 0.0, method="grid")
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, nbr_method=1))
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- config 2 shape: 8-net ensemble (reduced size)
+def test_ensemble_8_nets_water():
+    consts, widths, params, om = U.make_model(8, seed=inputs.SEED0 + 2)
+    sp, xyz, box = inputs.water_box(343, seed=4)
+    ctx = U.gpu_create(consts, widths, params, 8, len(sp))
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, nbr_method=1))
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- config 4 shape: all 7 species, uneven buckets
+def test_mixed_species_solvated_chain(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.solvated_chain(n_solute=600, L=24.0, seed=5)
+    assert len(np.unique(sp)) == 7
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp))
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        _check_lists(ctx, xyz, box, len(sp), 0.0, method="grid")
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, nbr_method=1))
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- config 5 shape: batched non-periodic molecules
+def test_molecule_batch(model1):
+    consts, widths, params, om = U.make_model(2, seed=inputs.SEED0 + 5)
+    sp, xyz, offs = inputs.molecule_batch(300, seed=12)
+    mol = np.repeat(np.arange(300), np.diff(offs)).astype(np.int32)
+    ctx = U.gpu_create(consts, widths, params, 2, len(sp), max_mols=300)
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, None, mol_offsets=offs)
+        _check_lists(ctx, xyz, None, len(sp), 0.0, mol_id=mol)
+        ref = orc.energy_forces(om, sp, xyz, None, offs)
+        U.assert_parity(Eg, Fg, ref)
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- degenerate inputs
+def test_edge_cases(model1):
+    consts, widths, params, om = model1
+    ctx = U.gpu_create(consts, widths, params, 1, 64, max_mols=4)
+    try:
+        # empty system
+        Eg, Fg = U.gpu_energy_forces(ctx, np.zeros(0, np.int32), np.zeros((0, 3)), None)
+        assert Eg[0] == 0.0
+        # single isolated atom: energy = network(0) = bias chain
+        Eg, Fg = U.gpu_energy_forces(ctx, [3], [[0.0, 0.0, 0.0]], None)
+        ref = orc.energy_forces(om, [3], [[0.0, 0.0, 0.0]])
+        assert abs(Eg[0] - ref["E"][0]) <= 1e-5 * abs(ref["E"][0]) and np.all(Fg == 0)
+        # dimer and collinear trimer
+        for sp, xyz in (([0, 0], [[0, 0, 0], [0.74, 0, 0]]), ([3, 0, 0], [[0, 0, 0], [0.96, 0, 0], [-0.96, 0, 0]])):
+            Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, None)
+            U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz))
+        # batch containing 1-atom molecules
+        sp = [0, 3, 0, 0, 1]
+        xyz = [[0, 0, 0], [5, 5, 5], [5.9, 5, 5], [5, 5.9, 5], [9, 9, 9]]
+        offs = [0, 1, 4, 5]
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, None, mol_offsets=offs)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, None, offs))
+        # bad species index is rejected
+        with pytest.raises(nnp.NnpError):
+            U.gpu_energy_forces(ctx, [9], [[0, 0, 0]], None)
+        # energy_forces without lists
+        d = torch.zeros((1, 3), device="cuda")
+        nnp.nnp_set_system(ctx, 1, torch.zeros(1, dtype=torch.int32, device="cuda"), d, None)
+        with pytest.raises(nnp.NnpError) as e:
+            nnp.nnp_energy_forces(ctx, torch.zeros(1, dtype=torch.float64, device="cuda"), d)
+        assert e.value.status == nnp.NNP_ESTALE
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_capacity_overflow_is_reported(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(64, 12.42)
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp), cap_r=32, cap_a=64)
+    try:
+        with pytest.raises(nnp.NnpError) as e:
+            U.gpu_energy_forces(ctx, sp, xyz, box)
+        assert e.value.status == nnp.NNP_ECAPACITY
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- MD (stage 5)
+def test_md_steps_against_oracle(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(216, seed=9)
+    v = inputs.maxwell_boltzmann(sp, 300.0, seed=2)
+    n = len(sp)
+    dev = torch.device("cuda:0")
+    ctx = U.gpu_create(consts, widths, params, 1, n)
+    try:
+        d_sp = torch.as_tensor(sp, device=dev)
+        d_x = torch.as_tensor(xyz.astype(np.float32), device=dev)
+        d_v = torch.as_tensor(v.astype(np.float32), device=dev)
+        nnp.nnp_set_system(ctx, n, d_sp, d_x, box)
+        nnp.nnp_md_init(ctx, d_v, 0.5, 0.5)
+        o_x, o_v = torch.zeros_like(d_x), torch.zeros_like(d_v)
+        o_ep = torch.zeros(1, dtype=torch.float64, device=dev)
+        o_ek = torch.zeros(1, dtype=torch.float64, device=dev)
+        o_nr = torch.zeros(1, dtype=torch.int32, device=dev)
+
+        def state():
+            nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, o_nr)
+            nnp.nnp_sync(ctx)
+            return (o_x.cpu().numpy().astype(np.float64), o_v.cpu().numpy().astype(np.float64),
+                    float(o_ep.item()), float(o_ek.item()), int(o_nr.item()))
+
+        x0, v0, ep0, ek0, nr0 = state()
+        assert nr0 == 1 and np.array_equal(x0, xyz) and np.array_equal(v0, v)
+        ref0 = orc.energy_forces(om, sp, xyz, box)
+        assert abs(ep0 - ref0["E"][0]) <= U.E_RTOL * abs(ref0["E"][0])
+        ke0 = 0.5 * (inputs.MASS[sp][:, None] * v ** 2).sum() / inputs.ACCEL_CONV
+        assert abs(ek0 - ke0) <= 1e-5 * ke0
+
+        # one step against the oracle integrator started from the same state
+        nnp.nnp_md_step(ctx, 1)
+        x1, v1, ep1, ek1, nr1 = state()
+        o1 = orc.md(om, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 1)
+        assert np.abs(x1 - o1["xyz"]).max() < 2e-6 and np.abs(v1 - o1["vel"]).max() < 2e-6
+        assert abs(ep1 - o1["epot"][1]) <= 2e-5 * abs(o1["epot"][1])
+
+        # 60 more steps: the lists must have been rebuilt by the displacement rule and must still be valid:
+        # E and F of the GPU state, recomputed by the oracle at the GPU's positions, agree
+        tot = [ep1 + ek1]
+        for _ in range(6):
+            nnp.nnp_md_step(ctx, 10)
+            xs, vs, ep, ek, nr = state()
+            tot.append(ep + ek)
+        assert nr >= 3
+        ref = orc.energy_forces(om, sp, xs, box)
+        assert abs(ep - ref["E"][0]) <= U.E_RTOL * abs(ref["E"][0])
+        # forces at the final state through a fresh evaluation of the same positions
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xs, box, skin=0.5)
+        U.assert_parity(Eg, Fg, ref)
+        # NVE: total energy conserved to integrator accuracy (< 0.1 % criterion)
+        tot = np.array(tot)
+        assert np.abs(tot - tot[0]).max() < 1e-3 * abs(ek0) + 1e-3 * abs(tot[0])
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_host_entry_points_roundtrip(model1):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(125, seed=10)
+    n = len(sp)
+    ctx = U.gpu_create(consts, widths, params, 1, n)
+    try:
+        h_sp = np.ascontiguousarray(sp, dtype=np.int32)
+        h_x = np.ascontiguousarray(xyz, dtype=np.float32)
+        h_E = np.zeros(1)
+        h_F = np.zeros((n, 3), dtype=np.float32)
+        nnp.nnp_energy_forces_host(ctx, n, h_sp, h_x, box, 1, None, 0.0, h_E, h_F)
+        ref = orc.energy_forces(om, sp, xyz, box)
+        U.assert_parity(h_E, h_F.astype(np.float64), ref)
+        # MD through host buffers equals MD through device buffers
+        v = inputs.maxwell_boltzmann(sp, 300.0, seed=3).astype(np.float32)
+        dev = torch.device("cuda:0")
+        nnp.nnp_set_system(ctx, n, torch.as_tensor(h_sp, device=dev), torch.as_tensor(h_x, device=dev), box)
+        nnp.nnp_md_init(ctx, torch.as_tensor(v, device=dev), 0.5, 0.5)
+        hx, hv = h_x.copy(), v.copy()
+        ep, ek = np.zeros(1), np.zeros(1)
+        for _ in range(5):
+            nnp.nnp_md_step_host(ctx, hx, hv, 1, ep, ek)
+        o = orc.md(om, sp, xyz, v.astype(np.float64), inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 5)
+        assert np.abs(hx - o["xyz"]).max() < 1e-5 and np.abs(hv - o["vel"]).max() < 1e-5
+        assert abs(ep[0] - o["epot"][5]) <= 5e-5 * abs(o["epot"][5])
+    finally:
+        nnp.nnp_destroy(ctx)
