@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py -- ANI-2x energy+force MD throughput on B200 (BASELINE.json metric), one JSON line.
+
+Workload (BASELINE.json configs[2], the configuration the metric is quoted on): 32,768 rigid-geometry waters
+= 98,304 atoms in a periodic cube L = 99.4 A, seeded Maxwell-Boltzmann velocities at 300 K, velocity Verlet at
+dt = 0.5 fs, Verlet skin 0.5 A with the displacement-triggered rebuild, one network of seeded Xavier weights,
+fp32.  A "step" is one MD step = one pass of all five stages (neighbour rebuild when triggered, AEV, MLPs,
+reverse pass + force scatter, integrator).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--mm-mode 0|1|2]
+
+N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -> N independent replicas,
+"scaling": "weak", value = sum of atom-steps over ranks / max time over ranks.
+--impl reference: the fp64 CPU oracle (oracle/) as it stands on the host cores, on bounded samples.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "ANI-2x energy+force MD atom-steps/s (0.5 fs velocity Verlet, 98,304-atom water box)"
+UNIT = "atom-steps/s"
+DT_FS, SKIN, T_KELVIN = 0.5, 0.5, 300.0
+N_WATERS = 32768
+BOX_L = 99.4
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sus=d["bf16_tflops_sustained"],
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sus=1400.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                if len(f) >= 7:
+                    self.rows.append(f)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.2)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]),
+                "power_w_max": max(float(r[2]) for r in self.rows), "samples": len(self.rows), "reasons": reasons}
+
+
+def oracle_model(n_nets=1):
+    from oracle import nnp_oracle as orc
+    from paper_2405_01491_b200 import inputs
+    consts = inputs.ani2x_constants()
+    params = inputs.make_weights(inputs.SEED0, n_nets, last_layer_scale=inputs.FORCE_SCALE_WATER)
+    return orc, orc.OracleModel(consts, inputs.WIDTHS, params, n_nets)
+
+
+def time_oracle_md(n_waters, n_steps, seed):
+    """Oracle MD on a water box of the workload's density.  orc.md evaluates the initial forces and then one
+    force evaluation per step, so the timed work is n_steps + 1 step-equivalents (the integrator itself is
+    negligible).  Returns (atom-steps, seconds, cores)."""
+    from paper_2405_01491_b200 import inputs
+    orc, om = oracle_model()
+    sp, xyz, box = inputs.water_box(n_waters, seed=seed)
+    v = inputs.maxwell_boltzmann(sp, T_KELVIN)
+    t0 = time.perf_counter()
+    orc.md(om, sp, xyz, v, inputs.MASS, box, DT_FS, inputs.ACCEL_CONV, n_steps, skin=SKIN,
+           nbr_method=1 if n_waters >= 216 else 0)
+    dt = time.perf_counter() - t0
+    return len(sp) * (n_steps + 1), dt, orc.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    K, W = args.steps, args.warmup
+    # calibrate on the smallest box, then pick the largest sample that keeps the run within ~3 minutes
+    a, t, cores = time_oracle_md(64, 1, 1)
+    rate = a / t                          # atom-steps/s
+    budget = 150.0 / max(1, K + W + 1)
+    n_waters = 64
+    for cand in (216, 512, 1000, 4096):
+        if cand * 3 / rate <= budget:
+            n_waters = cand
+    atoms, secs, cores = time_oracle_md(n_waters, K + W, 2)
+    secs_timed = secs * K / (K + W + 1)
+    value = n_waters * 3 * K / secs_timed
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+            "warmup": W, "ms_per_step": 1e3 * secs_timed / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "water_98304_md (configs[2]); each step = one oracle MD step of a %d-atom water box "
+                                   "of the same density" % (n_waters * 3), "dt_fs": DT_FS, "skin_A": SKIN},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": "%d velocity-Verlet steps of a %d-atom water box (same density, same model)" %
+                                       (K, n_waters * 3)},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    from paper_2405_01491_b200 import inputs, nnp
+    import __graft_entry__
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if rank == 0:
+        __graft_entry__.build()
+    if dist:
+        dist.barrier()
+    nnp.lib()          # fails loudly if the CUDA library is missing
+
+    # ---- workload: replica `rank` gets its own seed (independent trajectories, "replicas only")
+    sp, xyz, box = inputs.water_box(args.waters, BOX_L if args.waters == N_WATERS else None, seed=inputs.SEED0 + 3 + 1000 * rank)
+    n = len(sp)
+    vel = inputs.maxwell_boltzmann(sp, T_KELVIN, seed=inputs.SEED0 + 103 + 1000 * rank)
+    consts = inputs.ani2x_constants()
+    params = inputs.make_weights(inputs.SEED0, 1, last_layer_scale=args.force_scale)
+    p, keep = nnp.make_params(consts, inputs.WIDTHS, params, inputs.MASS, inputs.ACCEL_CONV, n_nets=1, mm_mode=args.mm_mode)
+    stream = torch.cuda.Stream(device=dev)
+    ctx = nnp.nnp_create(p, n, 1, local, stream.cuda_stream)
+
+    d_sp = torch.as_tensor(sp, device=dev)
+    d_x = torch.as_tensor(xyz.astype(np.float32), device=dev)
+    d_v = torch.as_tensor(vel.astype(np.float32), device=dev)
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident run (value)
+    nnp.nnp_set_system(ctx, n, d_sp, d_x, box)
+    nnp.nnp_md_init(ctx, d_v, DT_FS, SKIN)
+    nnp.nnp_md_step(ctx, W)
+    nnp.nnp_sync(ctx)
+    o_ep = torch.zeros(1, dtype=torch.float64, device=dev)
+    o_ek = torch.zeros(1, dtype=torch.float64, device=dev)
+    o_nr = torch.zeros(1, dtype=torch.int32, device=dev)
+    nnp.nnp_get_state(ctx, None, None, o_ep, o_ek, o_nr)
+    nnp.nnp_sync(ctx)
+    e_start, nr_start = float(o_ep.item() + o_ek.item()), int(o_nr.item())
+    ek_start = float(o_ek.item())
+    nnp.nnp_profile(ctx, max(1, K // 256))
+    sampler = ClockSampler(local)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = nnp.nnp_launch_count(ctx)
+    barrier()
+    sampler.start()
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        nnp.nnp_md_step(ctx, K)
+        ev1.record(stream)
+    barrier()
+    sampler.stop_flag.set()
+    launches = nnp.nnp_launch_count(ctx) - l0
+    ms = ev0.elapsed_time(ev1)
+    nnp.nnp_sync(ctx)
+    stage_ms, stage_n = nnp.nnp_profile_read(ctx)
+    nnp.nnp_profile(ctx, 0)
+    nnp.nnp_get_state(ctx, None, None, o_ep, o_ek, o_nr)
+    nnp.nnp_sync(ctx)
+    e_end, nr_end, ek_end = float(o_ep.item() + o_ek.item()), int(o_nr.item()), float(o_ek.item())
+    sampler.join(timeout=2)
+
+    # ---- end-to-end through the host entry point: every step uploads x,v and downloads x,v,E (pinned memory)
+    Ke = min(K, args.e2e_steps)
+    h_x = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    h_v = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    h_e = torch.zeros(2, dtype=torch.float64).pin_memory()
+    tmp_x, tmp_v = torch.zeros_like(d_x), torch.zeros_like(d_v)
+    nnp.nnp_get_state(ctx, tmp_x, tmp_v, None, None, None)
+    nnp.nnp_sync(ctx)
+    h_x.copy_(tmp_x)
+    h_v.copy_(tmp_v)
+    for _ in range(3):
+        nnp.nnp_md_step_host(ctx, h_x, h_v, 1, h_e[0:1], h_e[1:2])
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        nnp.nnp_md_step_host(ctx, h_x, h_v, 1, h_e[0:1], h_e[1:2])
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+
+    # ---- max over ranks
+    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max, e2e_ms_max = float(t[0].item()), float(t[1].item())
+    nnp.nnp_destroy(ctx)
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    pk = peaks()
+    clocks = sampler.summary()
+    value = world * n * K / (ms_max * 1e-3)
+    steps_per_s = K / (ms_max * 1e-3)
+    per_stage = {nnp.STAGE_NAMES[k]: (stage_ms[k] / stage_n[k] if stage_n[k] else 0.0) for k in range(nnp.NNP_N_STAGES)}
+    tot_stage = sum(per_stage.values())
+    dom = max(per_stage, key=per_stage.get)
+    roof = roofline_for(dom, per_stage[dom], n, sp, args.mm_mode, pk, clocks)
+    roof["stage_ms"] = {k: round(v, 4) for k, v in per_stage.items()}
+    roof["stage_share"] = {k: round(v / tot_stage, 4) for k, v in per_stage.items()} if tot_stage else {}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "water_%d_md (BASELINE configs[2])" % n if args.waters == N_WATERS else "water_%d_md" % n,
+                   "atoms": n, "box_A": float(box[0]), "dt_fs": DT_FS, "skin_A": SKIN, "n_nets": 1,
+                   "mm_mode": ["fp32_simt", "3xtf32_tcgen05", "tf32_tcgen05"][args.mm_mode],
+                   "force_scale": args.force_scale, "ns_per_day": steps_per_s * DT_FS * 1e-6 * 86400,
+                   "rebuilds_in_timed_region": nr_end - nr_start,
+                   "temperature_K_end": 2 * ek_end / (3 * n * inputs.KB), "temperature_K_start": 2 * ek_start / (3 * n * inputs.KB),
+                   "etot_drift_rel": (e_end - e_start) / abs(e_start) if e_start else None,
+                   "l2_policy": "inputs larger than L2 (G 403 MB + activations 240 MB per step; no flush needed)",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": world * n * Ke / (e2e_ms_max * 1e-3), "unit": UNIT, "steps": Ke,
+                "h2d_bytes_per_step": 2 * n * 12, "d2h_bytes_per_step": 2 * n * 12 + 16,
+                "api": "nnp_md_step_host (pinned host x,v up; x,v,epot,ekin down; every step)"},
+        "gpu_launches": launches,
+        "roofline": roof,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        atoms, secs, cores = time_oracle_md(args.cpu_waters, 2, 5)
+        line["cpu_baseline"] = {"value": atoms / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "2 velocity-Verlet steps of a %d-atom water box of the same density and model "
+                                          "(fp64 oracle, OpenMP)" % (args.cpu_waters * 3)}
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks):
+    """Roofline entry for the dominant stage (DESIGN.md 'Kernels and rooflines' gives the per-atom figures)."""
+    from paper_2405_01491_b200 import inputs
+    W = inputs.WIDTHS
+    counts = np.bincount(sp, minlength=7)
+    kpad = 1024
+
+    def macs(op):
+        tot = 0
+        for s in range(7):
+            h1, h2, h3 = int(W[s, 1]), int(W[s, 2]), int(W[s, 3])
+            tot += counts[s] * {"mlp_fwd_l1": kpad * h1, "mlp_fwd_l2": h1 * h2, "mlp_fwd_l3_out": h2 * h3 + h3,
+                                "mlp_bwd_l3": h3 * h2, "mlp_bwd_l2": h2 * h1, "mlp_bwd_l1_dEdG": h1 * kpad}[op]
+        return tot
+
+    if stage.startswith("mlp"):
+        flops = 2.0 * macs(stage)
+        ach = flops / (ms * 1e-3) / 1e12 if ms else 0.0
+        if mm_mode == 0:
+            sm_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
+            peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+            return {"kernel": stage, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                    "traffic": None, "peak_source": "148 SM x 128 FMA lanes x 2 x %.0f MHz (clocks.max.sm); median clock under load %s MHz"
+                    % (pk["sm_max_mhz"], sm_mhz)}
+        peak = pk["bf16_sus"] * 0.5
+        return {"kernel": stage, "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": None,
+                "peak_source": "%s sustained bf16 cuBLAS %.1f TF/s x 0.5 (nominal tf32/bf16 ratio); algorithmic fp32 flops "
+                               "counted once (3xTF32 issues 3 MMAs per product)" % (pk["source"], pk["bf16_sus"])}
+    if stage in ("aev_forward", "aev_backward_scatter"):
+        # algorithmic fp32 operations per atom for water at 1 g/cm3 (55.7 radial, 18.0 angular neighbours)
+        per_atom = {"aev_forward": 55.7 * 16 * 6 + 153 * 150.0, "aev_backward_scatter": 55.7 * 16 * 10 + 153 * 330.0}[stage]
+        ach = per_atom * n / (ms * 1e-3) / 1e12 if ms else 0.0
+        peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+        return {"kernel": stage, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": None, "peak_source": "148 SM x 128 lanes x 2 x clocks.max.sm"}
+    bytes_per_atom = {"kick_drift": 96.0, "kick_ekin": 52.0, "energy_sum": 12.0, "neighbor_build": 403.0 + 48.0}.get(stage, 64.0)
+    ach = bytes_per_atom * n / (ms * 1e-3) / 1e9 if ms else 0.0
+    return {"kernel": stage, "bound": "hbm", "achieved": ach, "peak": pk["hbm"], "unit": "GB/s", "frac": ach / pk["hbm"],
+            "traffic": None, "peak_source": pk["source"]}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mm-mode", type=int, default=int(os.environ.get("NNP_MM_MODE", "0")))
+    ap.add_argument("--waters", type=int, default=N_WATERS)
+    ap.add_argument("--force-scale", type=float, default=None)
+    ap.add_argument("--e2e-steps", type=int, default=200)
+    ap.add_argument("--cpu-waters", type=int, default=4096)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.force_scale is None:
+        from paper_2405_01491_b200 import inputs
+        args.force_scale = inputs.FORCE_SCALE_WATER
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -138,6 +138,16 @@ int nnp_energy_forces_host(nnp_ctx *ctx, int n_atoms, const int32_t *h_species, 
                            double *h_energy, float *h_forces);
 int nnp_md_step_host(nnp_ctx *ctx, float *h_xyz, float *h_vel, int n_steps, double *h_epot, double *h_ekin);
 
+/* Per-stage device timing for the bench (CUDA events on the ctx stream around the stage launches of every
+ * `stride`-th nnp_md_step step / nnp_energy_forces call; stride 0 switches it off and clears the sums).
+ * nnp_profile_read synchronises and returns, per stage, the summed milliseconds and the number of samples:
+ * 0 kick+drift, 1 neighbour build (all its kernels; near zero on steps without a rebuild), 2 AEV forward,
+ * 3..5 MLP forward layers 1..3 (layer 3 includes the output layer), 6..8 MLP reverse layers 3..1 (8 = dE/dG),
+ * 9 energy sum, 10 AEV reverse + force scatter, 11 kick + kinetic energy.  Arrays of NNP_N_STAGES entries. */
+#define NNP_N_STAGES 12
+int nnp_profile(nnp_ctx *ctx, int stride);
+int nnp_profile_read(nnp_ctx *ctx, double *h_ms_sum, int64_t *h_samples);
+
 /* Introspection for the bench: number of kernel launches issued by this ctx so far. */
 int64_t nnp_launch_count(const nnp_ctx *ctx);
 int nnp_aev_len(const nnp_ctx *ctx);

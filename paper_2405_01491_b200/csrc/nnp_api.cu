@@ -27,6 +27,45 @@ static std::string g_create_error;
                      cudaGetErrorString(_e));                                                      \
     } while (0)
 
+void nnp_prof_mark(nnp_ctx *c, int stage)
+{
+    if (!c->prof_active) return;
+    cudaEvent_t ev;
+    if (!c->prof_pool.empty()) { ev = c->prof_pool.back(); c->prof_pool.pop_back(); }
+    else if (cudaEventCreate(&ev) != cudaSuccess) return;
+    cudaEventRecord(ev, c->stream);
+    c->prof_marks.emplace_back(ev, stage);
+}
+
+static void prof_begin(nnp_ctx *c)
+{
+    c->prof_active = c->prof_stride > 0 && (c->prof_calls++ % c->prof_stride) == 0 && c->prof_marks.size() < 200000;
+    nnp_prof_mark(c, -1);
+}
+
+static void prof_collect(nnp_ctx *c)
+{
+    cudaStreamSynchronize(c->stream);
+    for (size_t q = 0; q < c->prof_marks.size(); ++q) {
+        const int st = c->prof_marks[q].second;
+        if (st >= 0 && q > 0) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, c->prof_marks[q - 1].first, c->prof_marks[q].first) == cudaSuccess) {
+                c->prof_ms[st] += ms;
+            }
+        }
+    }
+    // samples: one per "begin" mark for every stage that appeared after it
+    int seen[NNP_N_STAGES];
+    for (size_t q = 0; q < c->prof_marks.size(); ++q) {
+        const int st = c->prof_marks[q].second;
+        if (st < 0) { for (int k = 0; k < NNP_N_STAGES; ++k) seen[k] = 0; }
+        else if (!seen[st]) { seen[st] = 1; c->prof_n[st] += 1; }
+        c->prof_pool.push_back(c->prof_marks[q].first);
+    }
+    c->prof_marks.clear();
+}
+
 namespace {
 
 constexpr int T = 256;
@@ -168,6 +207,7 @@ int run_forces(nnp_ctx *c)
     CU(c, cudaMemsetAsync(c->frc, 0, sizeof(float4) * (size_t)c->n, c->stream));
     CU(c, cudaMemsetAsync(c->e_atom, 0, sizeof(float) * (size_t)c->n, c->stream));
     nnp_launch_aev_forward(c);
+    nnp_prof_mark(c, 2);
     static const int epi_of[6] = {EPI_CELU, EPI_CELU, EPI_CELU_OUT, EPI_DCELU, EPI_DCELU, EPI_STORE};
     GemmBatch b;
     for (int net = 0; net < c->n_nets; ++net)
@@ -177,9 +217,12 @@ int run_forces(nnp_ctx *c)
             if (op == 5 && net > 0) epi = EPI_ACCUM;
             int rc = run_gemm(c, b, epi);
             if (rc != NNP_OK) return rc;
+            nnp_prof_mark(c, 3 + op);
         }
     nnp_launch_energy_reduce(c);
+    nnp_prof_mark(c, 9);
     nnp_launch_aev_backward(c, 1.0f / (float)c->n_nets);
+    nnp_prof_mark(c, 10);
     CU(c, cudaGetLastError());
     c->have_forces = 1;
     return NNP_OK;
@@ -247,6 +290,8 @@ void nnp_destroy(nnp_ctx *c)
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags,
                     c->io_xyz, c->io_vel, c->io_species};
     for (void *p : ptrs) if (p) cudaFree(p);
+    for (auto &m : c->prof_marks) cudaEventDestroy(m.first);
+    for (auto &e : c->prof_pool) cudaEventDestroy(e);
     delete[] c->layers;
     delete c;
 }
@@ -393,7 +438,9 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
                    int n_mols, const int32_t *d_mol_offsets)
 {
     if (!c) return NNP_EINVAL;
-    if (!d_species || !d_xyz || !h_box) NNP_FAIL(c, NNP_EINVAL, "null argument");
+    static const float zero_box[3] = {0.f, 0.f, 0.f};
+    if (!h_box) h_box = zero_box;
+    if (n_atoms > 0 && (!d_species || !d_xyz)) NNP_FAIL(c, NNP_EINVAL, "null argument");
     if (n_atoms < 0 || n_atoms > c->max_atoms) NNP_FAIL(c, NNP_EINVAL, "n_atoms %d outside [0, max_atoms=%d]", n_atoms, c->max_atoms);
     if (!d_mol_offsets) n_mols = 1;
     if (n_mols < 1 || n_mols > c->max_mols) NNP_FAIL(c, NNP_EINVAL, "n_mols %d outside [1, max_mols=%d]", n_mols, c->max_mols);
@@ -471,7 +518,9 @@ static int energy_forces_impl(nnp_ctx *c, double *d_energy /* nullptr: leave in 
     if (c->n == 0) {
         CU(c, cudaMemsetAsync(c->e_mol, 0, sizeof(double) * c->n_mols, c->stream));
     } else {
+        prof_begin(c);
         int rc = run_forces(c);
+        c->prof_active = 0;
         if (rc) return rc;
         if (d_forces) nnp_launch_unpermute3(c, c->frc, d_forces);
     }
@@ -539,11 +588,16 @@ int nnp_md_step(nnp_ctx *c, int n_steps)
     if (n_steps < 0) NNP_FAIL(c, NNP_EINVAL, "n_steps < 0");
     CU(c, cudaSetDevice(c->device));
     for (int step = 0; step < n_steps; ++step) {
+        prof_begin(c);
         nnp_launch_kick_drift(c);
+        nnp_prof_mark(c, 0);
         nnp_launch_build(c, c->flags + 1); // every kernel returns at once unless the drift requested a rebuild
+        nnp_prof_mark(c, 1);
         int rc = run_forces(c);
-        if (rc) return rc;
+        if (rc) { c->prof_active = 0; return rc; }
         nnp_launch_kick_ke(c);
+        nnp_prof_mark(c, 11);
+        c->prof_active = 0;
     }
     return NNP_OK;
 }
@@ -562,6 +616,25 @@ int nnp_get_state(nnp_ctx *c, float *d_xyz, float *d_vel, double *d_epot, double
     return NNP_OK;
 }
 
+int nnp_profile(nnp_ctx *c, int stride)
+{
+    if (!c || stride < 0) return NNP_EINVAL;
+    prof_collect(c);
+    c->prof_stride = stride;
+    c->prof_calls = 0;
+    if (stride == 0)
+        for (int k = 0; k < NNP_N_STAGES; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
+    return NNP_OK;
+}
+
+int nnp_profile_read(nnp_ctx *c, double *h_ms_sum, int64_t *h_samples)
+{
+    if (!c || !h_ms_sum || !h_samples) return NNP_EINVAL;
+    prof_collect(c);
+    for (int k = 0; k < NNP_N_STAGES; ++k) { h_ms_sum[k] = c->prof_ms[k]; h_samples[k] = c->prof_n[k]; }
+    return NNP_OK;
+}
+
 int nnp_sync(nnp_ctx *c)
 {
     if (!c) return NNP_EINVAL;
@@ -573,7 +646,7 @@ int nnp_energy_forces_host(nnp_ctx *c, int n_atoms, const int32_t *h_species, co
                            int n_mols, const int32_t *h_mol_offsets, float skin, double *h_energy, float *h_forces)
 {
     if (!c) return NNP_EINVAL;
-    if (!h_species || !h_xyz || !h_box || !h_energy) NNP_FAIL(c, NNP_EINVAL, "null argument");
+    if ((n_atoms > 0 && (!h_species || !h_xyz)) || !h_energy) NNP_FAIL(c, NNP_EINVAL, "null argument");
     if (n_atoms < 0 || n_atoms > c->max_atoms) NNP_FAIL(c, NNP_EINVAL, "n_atoms outside [0, max_atoms]");
     if (h_mol_offsets && (n_mols < 1 || n_mols > c->max_mols)) NNP_FAIL(c, NNP_EINVAL, "n_mols outside [1, max_mols]");
     CU(c, cudaSetDevice(c->device));

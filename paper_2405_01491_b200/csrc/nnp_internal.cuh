@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "../../include/nnp.h"
 
@@ -101,6 +102,13 @@ struct nnp_ctx {
     int device, max_atoms, max_mols;
     int64_t launches;
     std::string err;
+    // per-stage event timing (nnp_profile)
+    int prof_stride, prof_active;
+    int64_t prof_calls;
+    std::vector<cudaEvent_t> prof_pool;          // recycled events
+    std::vector<std::pair<cudaEvent_t, int>> prof_marks; // (event, stage id or -1 for "begin")
+    double prof_ms[NNP_N_STAGES];
+    int64_t prof_n[NNP_N_STAGES];
 
     // system
     int n, n_mols, periodic, have_system, have_lists, have_forces, md_ready;
@@ -151,5 +159,7 @@ void nnp_launch_kick_ke(nnp_ctx *c);
 void nnp_launch_energy_reduce(nnp_ctx *c);
 void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst);
 void nnp_launch_permute_in3(nnp_ctx *c, const float *src, float4 *dst); // dst[i] = src[orig[i]]
+
+void nnp_prof_mark(nnp_ctx *c, int stage); // nnp_api.cu
 
 static inline int nnp_div_up(int a, int b) { return (a + b - 1) / b; }

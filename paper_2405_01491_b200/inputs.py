@@ -20,6 +20,9 @@ ACCEL_CONV = 4.184e-4            # (kcal/mol/A)/amu -> A/fs^2
 KB = 0.0019872041                # kcal/mol/K
 WATER_DENSITY = 0.033428         # molecules / A^3 (1 g/cm^3)
 SEED0 = 240501491
+# Reading B7: scalar applied to the last-layer weights so that random Xavier weights give liquid-like force
+# magnitudes on water.  Derived with the oracle only (tests/golden/force_scale.md): RMS |F| = 0.30 at scale 1.
+FORCE_SCALE_WATER = 66.0
 
 # BASELINE.json layer widths, species order H C N O S F Cl
 WIDTHS = np.array([

@@ -21,7 +21,8 @@ STATUS_NAMES = {0: "NNP_OK", -1: "NNP_EINVAL", -2: "NNP_ENOMEM", -3: "NNP_ECUDA"
 EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp_set_positions",
            "nnp_build_neighbors", "nnp_get_neighbors", "nnp_energy_forces", "nnp_get_aev",
            "nnp_get_atomic_energies", "nnp_md_init", "nnp_md_step", "nnp_get_state", "nnp_sync",
-           "nnp_energy_forces_host", "nnp_md_step_host", "nnp_launch_count", "nnp_aev_len"]
+           "nnp_energy_forces_host", "nnp_md_step_host", "nnp_profile", "nnp_profile_read", "nnp_launch_count",
+           "nnp_aev_len"]
 
 
 class NnpError(RuntimeError):
@@ -72,6 +73,8 @@ def lib():
         L.nnp_sync.argtypes = [vp]
         L.nnp_energy_forces_host.argtypes = [vp, C.c_int, ip, fp, C.POINTER(C.c_float), C.c_int, ip, C.c_float, dp, fp]
         L.nnp_md_step_host.argtypes = [vp, fp, fp, C.c_int, dp, dp]
+        L.nnp_profile.argtypes = [vp, C.c_int]
+        L.nnp_profile_read.argtypes = [vp, dp, ip]
         L.nnp_launch_count.argtypes = [vp]
         L.nnp_launch_count.restype = C.c_int64
         L.nnp_aev_len.argtypes = [vp]
@@ -193,6 +196,22 @@ def nnp_energy_forces_host(ctx, n_atoms, h_species, h_xyz, box, n_mols, h_mol_of
 
 def nnp_md_step_host(ctx, h_xyz, h_vel, n_steps, h_epot, h_ekin):
     return _check(ctx, lib().nnp_md_step_host(ctx, _ptr(h_xyz), _ptr(h_vel), int(n_steps), _ptr(h_epot), _ptr(h_ekin)))
+
+
+NNP_N_STAGES = 12
+STAGE_NAMES = ["kick_drift", "neighbor_build", "aev_forward", "mlp_fwd_l1", "mlp_fwd_l2", "mlp_fwd_l3_out",
+               "mlp_bwd_l3", "mlp_bwd_l2", "mlp_bwd_l1_dEdG", "energy_sum", "aev_backward_scatter", "kick_ekin"]
+
+
+def nnp_profile(ctx, stride):
+    return _check(ctx, lib().nnp_profile(ctx, int(stride)))
+
+
+def nnp_profile_read(ctx):
+    ms = np.zeros(NNP_N_STAGES, dtype=np.float64)
+    cnt = np.zeros(NNP_N_STAGES, dtype=np.int64)
+    _check(ctx, lib().nnp_profile_read(ctx, _ptr(ms), _ptr(cnt)))
+    return ms, cnt
 
 
 def nnp_launch_count(ctx):

@@ -9,9 +9,7 @@ from paper_2405_01491_b200 import inputs, nnp
 
 E_RTOL = 1e-5
 F_ATOL = 1e-3
-# reading B7: last-layer scale that brings the random-weight RMS force on water to ~20 kcal/mol/A
-# (oracle RMS force at scale 1 is 0.30; tests/golden/force_scale.md)
-FORCE_SCALE = 66.0
+FORCE_SCALE = inputs.FORCE_SCALE_WATER   # reading B7
 
 
 def make_model(n_nets=1, seed=inputs.SEED0, widths=inputs.WIDTHS, scale=FORCE_SCALE, bias_std=0.05, self_energy=None):
@@ -55,10 +53,19 @@ def gpu_neighbors(ctx, which, n, stride=256):
     return [np.sort(l[i, :c[i]]) for i in range(n)]
 
 
-def assert_parity(Eg, Fg, ref, e_rtol=E_RTOL, f_atol=F_ATOL):
+E_CANCEL = 2e-6   # DESIGN.md "Tolerances" (reading B8): fp32 floor when atomic energies cancel in E_m
+
+
+def assert_parity(Eg, Fg, ref, e_rtol=E_RTOL, f_atol=F_ATOL, mol_offsets=None):
+    """|dE|/|E| <= 1e-5 per structure.  Only where a structure's atomic energies cancel (|E_m| tiny against
+    sum_i |e_i|, reading B8) the bar is the fp32 floor 2e-6 * sum_i |e_i| instead; needs ref["e_atom"]."""
     Eo, Fo = ref["E"], ref["F"]
     for m in range(len(Eo)):
-        assert abs(Eg[m] - Eo[m]) <= e_rtol * abs(Eo[m]), ("energy", m, Eg[m], Eo[m], abs(Eg[m] - Eo[m]) / abs(Eo[m]))
+        tol = e_rtol * abs(Eo[m])
+        if ref.get("e_atom") is not None:
+            ea = ref["e_atom"] if mol_offsets is None else ref["e_atom"][mol_offsets[m]:mol_offsets[m + 1]]
+            tol = max(tol, E_CANCEL * np.abs(ea).sum())
+        assert abs(Eg[m] - Eo[m]) <= tol, ("energy", m, Eg[m], Eo[m], abs(Eg[m] - Eo[m]) / abs(Eo[m]))
     err = np.abs(Fg - Fo).max() if len(Fo) else 0.0
     assert err <= f_atol, ("force max abs err", err, "rms force", np.sqrt((Fo ** 2).sum(1).mean()))
     return err
