@@ -77,7 +77,7 @@ def oracle_model(n_nets=1):
     from oracle import nnp_oracle as orc
     from paper_2405_01491_b200 import inputs
     consts = inputs.ani2x_constants()
-    params = inputs.make_weights(inputs.SEED0, n_nets, last_layer_scale=inputs.FORCE_SCALE_WATER)
+    params = inputs.make_weights(inputs.SEED0, n_nets, last_layer_scale=inputs.FORCE_SCALE_MD)
     return orc, orc.OracleModel(consts, inputs.WIDTHS, params, n_nets)
 
 
@@ -320,7 +320,7 @@ def main():
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mm-mode", type=int, default=int(os.environ.get("NNP_MM_MODE", "0")))
+    ap.add_argument("--mm-mode", type=int, default=int(os.environ.get("NNP_MM_MODE", "1")))
     ap.add_argument("--waters", type=int, default=N_WATERS)
     ap.add_argument("--force-scale", type=float, default=None)
     ap.add_argument("--e2e-steps", type=int, default=200)
@@ -331,7 +331,7 @@ def main():
         args.warmup = 3
     if args.force_scale is None:
         from paper_2405_01491_b200 import inputs
-        args.force_scale = inputs.FORCE_SCALE_WATER
+        args.force_scale = inputs.FORCE_SCALE_MD
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -1,9 +1,406 @@
-// Stage 3/4, mm_mode = NNP_MM_3XTF32_TC / NNP_MM_TF32_TC: tcgen05 + TMA grouped GEMMs.  (Placeholder until the
-// tensor-core kernels land: fails loudly, never falls back.)
+// Stage 3/4, mm_mode = NNP_MM_3XTF32_TC / NNP_MM_TF32_TC: species-grouped GEMMs on the 5th-generation tensor
+// cores (tcgen05.mma kind::tf32, accumulators in TMEM, operands by TMA) with the layer epilogues fused.
+// ChemicalNet.  Precision (only full fp32 matmuls conserve energy; TF32 does
+// not): the default mode is 3xTF32 -- every fp32 operand x is split into hi = tf32(x) and lo = tf32(x - hi), and
+// A.B is accumulated in fp32 as A_lo.B_hi + A_hi.B_lo + A_hi.B_hi, which carries ~21 mantissa bits per operand.
+// Weights are split once at nnp_create; activations are split on the fly inside the kernel.
+//
+// One CTA computes one 128-row (atoms) x N (<= 256 features) output tile:
+//   warp 0   TMA producer: per 32-wide K block, the fp32 A tile [128][32] and the B_hi / B_lo tiles [N][32]
+//            (K-major, 128-byte swizzle) into a 2-stage shared-memory ring, mbarrier complete_tx.
+//   warps 2-5 converters: each thread owns one A row: reads it from the swizzled tile (conflict-free LDS.128),
+//            splits it into tf32 hi / lo and writes both into TMEM (tcgen05.st) -- A is fed to the tensor core
+//            from TMEM (".ts" form), so shared-memory bandwidth is spent on B only.
+//   warp 1   one elected thread issues tcgen05.mma (3 per 8-wide K step in 3xTF32 mode); tcgen05.commit
+//            releases the stage (shared memory + TMEM A slot) and finally signals the accumulator.
+//   warps 2-5 epilogue: tcgen05.ld the accumulator row, apply bias/CELU/CELU'/output-layer dot, store.
+#include <cuda.h>
+
+#include <string.h>
+
 #include "nnp_internal.cuh"
 
-int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &, int, int)
+namespace {
+
+constexpr int TILE_M = 128;
+constexpr int BLOCK_K = 32;               // fp32 elements = one 128-byte swizzle row
+constexpr int UMMA_K = 8;                 // tf32
+constexpr int N_MAX = 256;
+constexpr int STAGES = 2;
+constexpr int A_TILE_BYTES = TILE_M * BLOCK_K * 4;          // 16 KiB
+constexpr int B_TILE_BYTES_MAX = N_MAX * BLOCK_K * 4;       // 32 KiB
+constexpr int STAGE_BYTES = A_TILE_BYTES + 2 * B_TILE_BYTES_MAX; // 80 KiB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int TMEM_COLS = 512;
+constexpr int TMEM_A_COL0 = 256;          // A staging: stage s -> hi at 256 + 64 s, lo at 256 + 64 s + 32
+constexpr int THREADS = 192;
+
+struct TcGroup {
+    CUtensorMap mapA, mapBhi, mapBlo;
+    float *C;
+    const float *bias, *w4;
+    float *e_atom;
+    int M, N, K, ldc;
+    int n_tiles_n; // N / min(N, 256)
+};
+
+struct TcBatch {
+    TcGroup g[NNP_MAX_SPECIES - 1];
+    int n_groups;
+    int tile_off[NNP_MAX_SPECIES];
+    float alpha;
+};
+
+// ---------------------------------------------------------------- PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
-    c->err = "mm_mode 1/2 (tcgen05 path) is not built in this revision; use NNP_MM_FP32_SIMT";
-    return NNP_EINVAL;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// Bounded wait: a protocol bug must not hang the GPU (the box is shared); trap after ~seconds.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done = 0;
+    for (uint32_t it = 0; it < (1u << 26); ++it) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        if (done) return;
+    }
+    __trap();
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+        "l"(map), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[tmem] . B[smem desc]^T, kind::tf32, A from tensor memory
+__device__ __forceinline__ void mma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]),
+        "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]),
+        "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+
+// tf32 split: hi = x rounded to 10 mantissa bits (nearest, ties away), lo = x - hi (exact), lo rounded the same way
+__device__ __forceinline__ uint32_t tf32_round(float x)
+{
+    return (__float_as_uint(x) + 0x1000u) & 0xffffe000u;
+}
+
+// K-major, 128-byte-swizzled operand tile: rows of 128 B, 8-row groups 1024 B apart
+__device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr >> 4) & 0x3fff);
+    d |= (uint64_t)1 << 16;                  // leading byte offset (unused for swizzled K-major)
+    d |= (uint64_t)(1024 >> 4) << 32;        // stride byte offset between 8-row groups
+    d |= (uint64_t)1 << 46;                  // descriptor version (sm_100)
+    d |= (uint64_t)2 << 61;                  // SWIZZLE_128B
+    return d;
+}
+
+__device__ __forceinline__ float celu_fwd(float x, float alpha, float inv_alpha)
+{
+    return x > 0.f ? x : alpha * (__expf(x * inv_alpha) - 1.0f);
+}
+__device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
+
+template <int EPI, bool SPLIT3>
+__global__ void __launch_bounds__(THREADS, 1)
+k_gemm_tc(const __grid_constant__ TcBatch batch)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+    // barriers: full[s] @ 0,8 ; aready[s] @ 16,24 ; empty[s] @ 32,40 ; accfull @ 48 ; tmem ptr @ 64
+    const uint32_t bar_full = bar_base, bar_aready = bar_base + 16, bar_empty = bar_base + 32, bar_acc = bar_base + 48;
+    const uint32_t tmem_slot = bar_base + 64;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // tile -> (group, m-tile, n-tile)
+    int gi = 0;
+    while (gi + 1 < batch.n_groups && (int)blockIdx.x >= batch.tile_off[gi + 1]) ++gi;
+    const TcGroup &g = batch.g[gi];
+    const int t = (int)blockIdx.x - batch.tile_off[gi];
+    const int mt = t / g.n_tiles_n, nt = t - mt * g.n_tiles_n;
+    const int NT = g.n_tiles_n > 1 ? N_MAX : g.N; // columns of this tile
+    const int m0 = mt * TILE_M, n0 = nt * N_MAX;
+    const int num_kb = g.K / BLOCK_K;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_aready + 8 * s, 128);
+            mbar_init(bar_empty + 8 * s, 1);
+        }
+        mbar_init(bar_acc, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    if (warp == 0) {
+        // ===== TMA producer
+        if (lane == 0) {
+            const uint32_t tx = A_TILE_BYTES + (SPLIT3 ? 2u : 1u) * (uint32_t)NT * BLOCK_K * 4u;
+            for (int kb = 0; kb < num_kb; ++kb) {
+                const int s = kb % STAGES;
+                const uint32_t ph = (kb / STAGES) & 1;
+                mbar_wait(bar_empty + 8 * s, ph ^ 1);
+                const uint32_t stage = smem_base + s * STAGE_BYTES;
+                mbar_expect_tx(bar_full + 8 * s, tx);
+                tma_load_2d(stage, &g.mapA, kb * BLOCK_K, m0, bar_full + 8 * s);
+                tma_load_2d(stage + A_TILE_BYTES, &g.mapBhi, kb * BLOCK_K, n0, bar_full + 8 * s);
+                if (SPLIT3) tma_load_2d(stage + A_TILE_BYTES + B_TILE_BYTES_MAX, &g.mapBlo, kb * BLOCK_K, n0, bar_full + 8 * s);
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NT >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+            for (int kb = 0; kb < num_kb; ++kb) {
+                const int s = kb % STAGES;
+                const uint32_t ph = (kb / STAGES) & 1;
+                mbar_wait(bar_full + 8 * s, ph);
+                mbar_wait(bar_aready + 8 * s, ph);
+                tc_fence_after();
+                const uint32_t stage = smem_base + s * STAGE_BYTES;
+                const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
+                const uint64_t dlo = make_kmajor_sw128_desc(stage + A_TILE_BYTES + B_TILE_BYTES_MAX);
+                const uint32_t a_hi = tmem_base + TMEM_A_COL0 + 64 * s, a_lo = a_hi + 32;
+#pragma unroll
+                for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+                    const uint64_t koff = (uint64_t)(k * UMMA_K * 4 >> 4);
+                    const uint32_t first = (kb | k) ? 1u : 0u;
+                    if (SPLIT3) {
+                        mma_tf32_ts(tmem_base, a_lo + k * UMMA_K, dhi + koff, idesc, first);
+                        mma_tf32_ts(tmem_base, a_hi + k * UMMA_K, dlo + koff, idesc, 1u);
+                        mma_tf32_ts(tmem_base, a_hi + k * UMMA_K, dhi + koff, idesc, 1u);
+                    } else {
+                        mma_tf32_ts(tmem_base, a_hi + k * UMMA_K, dhi + koff, idesc, first);
+                    }
+                }
+                tc_commit(bar_empty + 8 * s);
+            }
+            tc_commit(bar_acc);
+        }
+    } else {
+        // ===== converters, then epilogue (warps 2..5 -> TMEM lane quarters 2,3,0,1)
+        const int quarter = warp & 3;
+        const int row = quarter * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
+        for (int kb = 0; kb < num_kb; ++kb) {
+            const int s = kb % STAGES;
+            const uint32_t ph = (kb / STAGES) & 1;
+            mbar_wait(bar_full + 8 * s, ph);
+            const uint32_t arow = smem_base + s * STAGE_BYTES + row * 128;
+            uint32_t hi[32], lo[32];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                float4 v;
+                const uint32_t addr = arow + (uint32_t)((c ^ (row & 7)) << 4);
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+                const float x[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t h = tf32_round(x[e]);
+                    hi[4 * c + e] = h;
+                    if (SPLIT3) lo[4 * c + e] = tf32_round(x[e] - __uint_as_float(h));
+                }
+            }
+            tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s, hi);
+            if (SPLIT3) tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s + 32, lo);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            tc_fence_before();
+            mbar_arrive(bar_aready + 8 * s);
+        }
+
+        // ---- epilogue: this thread owns output row m0 + row, columns n0 .. n0 + NT
+        mbar_wait(bar_acc, 0);
+        tc_fence_after();
+        const int m = m0 + row;
+        const bool rowok = m < g.M;
+        const float alpha = batch.alpha, inv_alpha = 1.0f / batch.alpha;
+        float *crow = g.C + (size_t)(rowok ? m : 0) * g.ldc + n0;
+        float esum = 0.f;
+        for (int c0 = 0; c0 < NT; c0 += 32) {
+            uint32_t acc[32];
+            tmem_ld32(lane_addr + c0, acc);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (rowok) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    float4 o;
+                    float *ov = reinterpret_cast<float *>(&o);
+                    float4 prev = make_float4(0.f, 0.f, 0.f, 0.f), bb = prev, ww = prev;
+                    if (EPI == EPI_DCELU || EPI == EPI_ACCUM) prev = *reinterpret_cast<const float4 *>(crow + c0 + 4 * q);
+                    if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bb = *reinterpret_cast<const float4 *>(g.bias + n0 + c0 + 4 * q);
+                    if (EPI == EPI_CELU_OUT) ww = *reinterpret_cast<const float4 *>(g.w4 + n0 + c0 + 4 * q);
+                    const float *pv = reinterpret_cast<const float *>(&prev);
+                    const float *bv = reinterpret_cast<const float *>(&bb);
+                    const float *wv = reinterpret_cast<const float *>(&ww);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        float v = __uint_as_float(acc[4 * q + e]);
+                        if (EPI == EPI_CELU) v = celu_fwd(v + bv[e], alpha, inv_alpha);
+                        if (EPI == EPI_CELU_OUT) {
+                            const float h = celu_fwd(v + bv[e], alpha, inv_alpha);
+                            esum = fmaf(h, wv[e], esum);
+                            v = wv[e] * celu_grad_from_h(h, inv_alpha);
+                        }
+                        if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[e], inv_alpha);
+                        if (EPI == EPI_ACCUM) v += pv[e];
+                        ov[e] = v;
+                    }
+                    *reinterpret_cast<float4 *>(crow + c0 + 4 * q) = o;
+                }
+            }
+        }
+        if (EPI == EPI_CELU_OUT && rowok) g.e_atom[m] += esum; // one thread per row, full width in this CTA
+        tc_fence_before();
+    }
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
+// ---------------------------------------------------------------- host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+bool load_encode()
+{
+    if (g_encode) return true;
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return false;
+    g_encode = (EncodeTiledFn)fn;
+    return true;
+}
+
+// 2-D fp32 tensor [rows][cols] with row pitch `ld` floats; box = [box_rows][32 cols], 128-byte swizzle, zero fill
+bool make_map(CUtensorMap *m, const float *base, int rows, int cols, int ld, int box_rows)
+{
+    cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+    cuuint32_t box[2] = {(cuuint32_t)BLOCK_K, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return g_encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int EPI>
+void launch(cudaStream_t st, const TcBatch &b, int tiles, bool split3)
+{
+    if (split3) {
+        cudaFuncSetAttribute(k_gemm_tc<EPI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        k_gemm_tc<EPI, true><<<tiles, THREADS, SMEM_BYTES, st>>>(b);
+    } else {
+        cudaFuncSetAttribute(k_gemm_tc<EPI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        k_gemm_tc<EPI, false><<<tiles, THREADS, SMEM_BYTES, st>>>(b);
+    }
+}
+
+} // namespace
+
+int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
+{
+    if (!load_encode()) { c->err = "cuTensorMapEncodeTiled entry point not available"; return NNP_ECUDA; }
+    TcBatch tb;
+    memset(&tb, 0, sizeof(tb));
+    tb.alpha = b.alpha;
+    int tiles = 0;
+    for (int i = 0; i < b.n_groups; ++i) {
+        const GemmGroup &g = b.g[i];
+        TcGroup &t = tb.g[i];
+        if (!g.Bt_hi || !g.Bt_lo) { c->err = "tensor-core path: weight operand has no tf32 split"; return NNP_EINVAL; }
+        const int NT = g.N > N_MAX ? N_MAX : g.N;
+        if (g.N % NT || g.K % BLOCK_K || NT % 16) { c->err = "tensor-core path: unsupported GEMM shape"; return NNP_EINVAL; }
+        if (!make_map(&t.mapA, g.A, g.M, g.K, g.lda, TILE_M) || !make_map(&t.mapBhi, g.Bt_hi, g.N, g.K, g.K, NT) ||
+            !make_map(&t.mapBlo, g.Bt_lo, g.N, g.K, g.K, NT)) {
+            c->err = "cuTensorMapEncodeTiled failed";
+            return NNP_ECUDA;
+        }
+        t.C = g.C; t.bias = g.bias; t.w4 = g.w4; t.e_atom = g.e_atom;
+        t.M = g.M; t.N = g.N; t.K = g.K; t.ldc = g.ldc;
+        t.n_tiles_n = g.N / NT;
+        tb.tile_off[i] = tiles;
+        tiles += nnp_div_up(g.M, TILE_M) * t.n_tiles_n;
+    }
+    tb.n_groups = b.n_groups;
+    tb.tile_off[b.n_groups] = tiles;
+    if (tiles == 0) return NNP_OK;
+    const bool s3 = split3 != 0;
+    switch (epi) {
+    case EPI_CELU: launch<EPI_CELU>(c->stream, tb, tiles, s3); break;
+    case EPI_CELU_OUT: launch<EPI_CELU_OUT>(c->stream, tb, tiles, s3); break;
+    case EPI_DCELU: launch<EPI_DCELU>(c->stream, tb, tiles, s3); break;
+    case EPI_STORE: launch<EPI_STORE>(c->stream, tb, tiles, s3); break;
+    case EPI_ACCUM: launch<EPI_ACCUM>(c->stream, tb, tiles, s3); break;
+    default: c->err = "bad epilogue"; return NNP_EINVAL;
+    }
+    c->launches += 1;
+    return NNP_OK;
 }

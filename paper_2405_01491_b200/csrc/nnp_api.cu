@@ -162,32 +162,38 @@ void make_batch(nnp_ctx *c, int net, int op, GemmBatch &b)
         case 0:
             g.A = c->G + (size_t)off * kpad; g.lda = kpad; g.K = kpad; g.N = h1;
             g.B = layer(c, net, s, 0).W; g.Bt = layer(c, net, s, 0).Wt; g.bias = layer(c, net, s, 0).b;
+            g.Bt_hi = layer(c, net, s, 0).Wt_hi; g.Bt_lo = layer(c, net, s, 0).Wt_lo;
             g.C = H0; g.ldc = c->hmax[0];
             break;
         case 1:
             g.A = H0; g.lda = c->hmax[0]; g.K = h1; g.N = h2;
             g.B = layer(c, net, s, 1).W; g.Bt = layer(c, net, s, 1).Wt; g.bias = layer(c, net, s, 1).b;
+            g.Bt_hi = layer(c, net, s, 1).Wt_hi; g.Bt_lo = layer(c, net, s, 1).Wt_lo;
             g.C = H1; g.ldc = c->hmax[1];
             break;
         case 2:
             g.A = H1; g.lda = c->hmax[1]; g.K = h2; g.N = h3;
             g.B = layer(c, net, s, 2).W; g.Bt = layer(c, net, s, 2).Wt; g.bias = layer(c, net, s, 2).b;
+            g.Bt_hi = layer(c, net, s, 2).Wt_hi; g.Bt_lo = layer(c, net, s, 2).Wt_lo;
             g.w4 = layer(c, net, s, 3).W; g.e_atom = c->e_atom + off;
             g.C = H2; g.ldc = c->hmax[2];
             break;
         case 3: // delta2 = (delta3 W3^T) * celu'(h2), in place in H1
             g.A = H2; g.lda = c->hmax[2]; g.K = h3; g.N = h2;
             g.B = layer(c, net, s, 2).Wt; g.Bt = layer(c, net, s, 2).W;
+            g.Bt_hi = layer(c, net, s, 2).W_hi; g.Bt_lo = layer(c, net, s, 2).W_lo;
             g.C = H1; g.ldc = c->hmax[1];
             break;
         case 4: // delta1 = (delta2 W2^T) * celu'(h1), in place in H0
             g.A = H1; g.lda = c->hmax[1]; g.K = h2; g.N = h1;
             g.B = layer(c, net, s, 1).Wt; g.Bt = layer(c, net, s, 1).W;
+            g.Bt_hi = layer(c, net, s, 1).W_hi; g.Bt_lo = layer(c, net, s, 1).W_lo;
             g.C = H0; g.ldc = c->hmax[0];
             break;
         case 5: // dE/dG (+)= delta1 W1^T
             g.A = H0; g.lda = c->hmax[0]; g.K = h1; g.N = kpad;
             g.B = layer(c, net, s, 0).Wt; g.Bt = layer(c, net, s, 0).W;
+            g.Bt_hi = layer(c, net, s, 0).W_hi; g.Bt_lo = layer(c, net, s, 0).W_lo;
             g.C = c->dG + (size_t)off * kpad; g.ldc = kpad;
             break;
         }
@@ -355,7 +361,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
                 LayerW &L = layer(c, net, s, l);
                 L.in = c->widths[s][l]; L.out = c->widths[s][l + 1];
                 L.in_pad = l == 0 ? a.kpad : L.in;
-                total += 2 * (size_t)L.in_pad * L.out + (size_t)((L.out + 3) / 4 * 4);
+                total += (c->mm_mode ? 6 : 2) * (size_t)L.in_pad * L.out + (size_t)((L.out + 3) / 4 * 4);
             }
     std::vector<float> blob(total, 0.f);
     std::vector<double> shift(S, 0.0);
@@ -380,6 +386,25 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
                     src += L.out;
                     if (l == NNP_NLAYERS - 1) shift[s] += (double)b[0] / c->n_nets;
                     L.W = (float *)(W - blob.data()); L.Wt = (float *)(Wt - blob.data()); L.b = (float *)(b - blob.data());
+                    if (c->mm_mode) { // tf32 hi / lo splits of both orientations (same rounding as the kernel's A split)
+                        const size_t cnt = (size_t)L.in_pad * L.out;
+                        float *dst[4] = {&blob[o], &blob[o + cnt], &blob[o + 2 * cnt], &blob[o + 3 * cnt]};
+                        o += 4 * cnt;
+                        const float *srcs[2] = {W, Wt};
+                        for (int w = 0; w < 2; ++w)
+                            for (size_t q = 0; q < cnt; ++q) {
+                                uint32_t u; memcpy(&u, &srcs[w][q], 4);
+                                uint32_t h = (u + 0x1000u) & 0xffffe000u;
+                                float hf; memcpy(&hf, &h, 4);
+                                float lf = srcs[w][q] - hf;
+                                uint32_t lu; memcpy(&lu, &lf, 4);
+                                lu = (lu + 0x1000u) & 0xffffe000u;
+                                memcpy(&dst[2 * w][q], &h, 4);
+                                memcpy(&dst[2 * w + 1][q], &lu, 4);
+                            }
+                        L.W_hi = (float *)(dst[0] - blob.data()); L.W_lo = (float *)(dst[1] - blob.data());
+                        L.Wt_hi = (float *)(dst[2] - blob.data()); L.Wt_lo = (float *)(dst[3] - blob.data());
+                    }
                 }
     }
     int rc;
@@ -390,6 +415,10 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     for (size_t q = 0; q < (size_t)c->n_nets * S * NNP_NLAYERS; ++q) { // offsets -> device pointers
         LayerW &L = c->layers[q];
         L.W = c->d_params_blob + (size_t)L.W; L.Wt = c->d_params_blob + (size_t)L.Wt; L.b = c->d_params_blob + (size_t)L.b;
+        if (c->mm_mode) {
+            L.W_hi = c->d_params_blob + (size_t)L.W_hi; L.W_lo = c->d_params_blob + (size_t)L.W_lo;
+            L.Wt_hi = c->d_params_blob + (size_t)L.Wt_hi; L.Wt_lo = c->d_params_blob + (size_t)L.Wt_lo;
+        }
     }
     float imc[NNP_MAX_SPECIES] = {0}, ms[NNP_MAX_SPECIES] = {0}, es[NNP_MAX_SPECIES] = {0};
     for (int s = 0; s < S; ++s) {

@@ -60,7 +60,8 @@ enum GemmEpilogue {
 struct GemmGroup {
     const float *A;   // [M][lda]   K-contiguous rows
     const float *B;   // [K][N]     row-major (SIMT path)
-    const float *Bt;  // [N][K]     K-contiguous rows (tensor-core path)
+    const float *Bt;  // [N][K]     K-contiguous rows (tensor-core path, plain TF32 rounds it on the fly)
+    const float *Bt_hi, *Bt_lo; // tf32 hi / lo split of Bt (3xTF32; nullptr in SIMT mode)
     float *C;         // [M][ldc]
     const float *bias; // [N] or nullptr
     const float *w4;  // [N] last-layer weights (EPI_CELU_OUT)
@@ -80,6 +81,7 @@ struct LayerW {
     float *W;  // device [in_pad][out]
     float *Wt; // device [out][in_pad]
     float *b;  // device [out]
+    float *W_hi, *W_lo, *Wt_hi, *Wt_lo; // tf32 splits (tensor-core modes only)
     int in, in_pad, out;
 };
 
