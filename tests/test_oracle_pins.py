@@ -482,3 +482,24 @@ def test_md_rebuild_count_reasonable(small_model):
     sp, xyz, box, v = _md_setup(small_model)
     r = orc.md(small_model, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 30, skin=0.5)
     assert 2 <= r["n_rebuilds"] <= 12
+
+
+# ---------------------------------------------------------------- regression pin (values written by tests/golden/make_oracle_golden.py)
+def test_oracle_matches_stored_golden(consts):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_water64.txt")
+    params = inputs.make_weights(inputs.SEED0, 1, last_layer_scale=inputs.FORCE_SCALE_WATER, bias_std=0.05)
+    om = orc.OracleModel(consts, inputs.WIDTHS, params, 1)
+    sp, xyz, box = inputs.water_box(64, 12.42)
+    r = orc.energy_forces(om, sp, xyz, box, want_aev=True)
+    for line in open(path):
+        t = line.split()
+        if t[0] == "E":
+            assert abs(r["E"][0] - float(t[1])) < 1e-9 * abs(float(t[1]))
+        elif t[0] == "F":
+            assert np.allclose(r["F"][int(t[1])], [float(x) for x in t[2:5]], rtol=1e-9, atol=1e-9)
+        elif t[0] == "AEVSUM":
+            assert abs(r["aev"].sum() - float(t[1])) < 1e-9 * float(t[1])
+        elif t[0] == "AEVNNZ":
+            # water: only H,O radial blocks and the (H,H),(H,O),(O,O) angular blocks can be non-zero
+            assert int((r["aev"] != 0).sum()) == int(t[1]) <= 192 * 128
