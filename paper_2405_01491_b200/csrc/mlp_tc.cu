@@ -25,15 +25,18 @@ namespace {
 constexpr int TILE_M = 128;
 constexpr int BLOCK_K = 32;               // fp32 elements = one 128-byte swizzle row
 constexpr int UMMA_K = 8;                 // tf32
-constexpr int N_MAX = 256;
-constexpr int STAGES = 2;
+constexpr int NT_MAX = 128;               // columns per output tile (wider layers are split in two halves)
+constexpr int STAGES = 4;
 constexpr int A_TILE_BYTES = TILE_M * BLOCK_K * 4;          // 16 KiB
-constexpr int B_TILE_BYTES_MAX = N_MAX * BLOCK_K * 4;       // 32 KiB
-constexpr int STAGE_BYTES = A_TILE_BYTES + 2 * B_TILE_BYTES_MAX; // 80 KiB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int B_TILE_BYTES_MAX = NT_MAX * BLOCK_K * 4;      // 16 KiB
+constexpr int STAGE_BYTES = A_TILE_BYTES + 2 * B_TILE_BYTES_MAX; // 48 KiB
+constexpr int EPI_STG_LD = 36;                                   // floats per staged row (16-byte aligned, conflict-free)
+constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;               // per epilogue warp: one 32 x 32 chunk
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 4 * EPI_STG_BYTES;
 constexpr int TMEM_COLS = 512;
+constexpr int TMEM_ACC_STRIDE = 128;      // two accumulator buffers at columns 0 and 128
 constexpr int TMEM_A_COL0 = 256;          // A staging: stage s -> hi at 256 + 64 s, lo at 256 + 64 s + 32
-constexpr int THREADS = 192;
+constexpr int THREADS = 448;              // warp 0 TMA, warp 1 MMA, warps 2-9 converters (two groups), warps 10-13 epilogue
 
 struct TcGroup {
     CUtensorMap mapA, mapBhi, mapBlo;
@@ -41,13 +44,15 @@ struct TcGroup {
     const float *bias, *w4;
     float *e_atom;
     int M, N, K, ldc;
-    int n_tiles_n; // N / min(N, 256)
+    int NT;        // columns per tile
+    int n_tiles_n; // N / NT
 };
 
 struct TcBatch {
     TcGroup g[NNP_MAX_SPECIES - 1];
     int n_groups;
-    int tile_off[NNP_MAX_SPECIES];
+    int tile_off[NNP_MAX_SPECIES]; // prefix sum of (m tiles x n tiles) per group
+    int n_tiles;
     float alpha;
 };
 
@@ -131,6 +136,17 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
         : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+}
+
 // tf32 split: hi = x rounded to 10 mantissa bits (nearest, ties away), lo = x - hi (exact), lo rounded the same way
 __device__ __forceinline__ uint32_t tf32_round(float x)
 {
@@ -155,6 +171,21 @@ __device__ __forceinline__ float celu_fwd(float x, float alpha, float inv_alpha)
 }
 __device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
 
+// tile index -> (group, m0, n0)
+struct TileCoord { int gi, m0, n0; };
+__device__ __forceinline__ TileCoord tile_coord(const TcBatch &batch, int t)
+{
+    int gi = 0;
+    while (gi + 1 < batch.n_groups && t >= batch.tile_off[gi + 1]) ++gi;
+    const int r = t - batch.tile_off[gi];
+    const int ntn = batch.g[gi].n_tiles_n;
+    const int mt = r / ntn, nt = r - mt * ntn;
+    return TileCoord{gi, mt * TILE_M, nt * batch.g[gi].NT};
+}
+
+// Persistent: CTA c processes the contiguous tile range [c T / G, (c+1) T / G); the two n-halves of an m-tile are
+// adjacent, so the second read of the A tile hits L2.  The smem/TMEM-A ring (4 stages) and the two accumulator
+// buffers run across tile boundaries: the epilogue of tile i overlaps the conversion + MMAs of tile i+1.
 template <int EPI, bool SPLIT3>
 __global__ void __launch_bounds__(THREADS, 1)
 k_gemm_tc(const __grid_constant__ TcBatch batch)
@@ -162,21 +193,14 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
-    // barriers: full[s] @ 0,8 ; aready[s] @ 16,24 ; empty[s] @ 32,40 ; accfull @ 48 ; tmem ptr @ 64
-    const uint32_t bar_full = bar_base, bar_aready = bar_base + 16, bar_empty = bar_base + 32, bar_acc = bar_base + 48;
-    const uint32_t tmem_slot = bar_base + 64;
+    // barriers (8 B each): full[4] @0, aready[4] @32, empty[4] @64, acc_full[2] @96, acc_empty[2] @112; tmem ptr @128
+    const uint32_t bar_full = bar_base, bar_aready = bar_base + 32, bar_empty = bar_base + 64;
+    const uint32_t bar_accf = bar_base + 96, bar_acce = bar_base + 112;
+    const uint32_t tmem_slot = bar_base + 128;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-    // tile -> (group, m-tile, n-tile)
-    int gi = 0;
-    while (gi + 1 < batch.n_groups && (int)blockIdx.x >= batch.tile_off[gi + 1]) ++gi;
-    const TcGroup &g = batch.g[gi];
-    const int t = (int)blockIdx.x - batch.tile_off[gi];
-    const int mt = t / g.n_tiles_n, nt = t - mt * g.n_tiles_n;
-    const int NT = g.n_tiles_n > 1 ? N_MAX : g.N; // columns of this tile
-    const int m0 = mt * TILE_M, n0 = nt * N_MAX;
-    const int num_kb = g.K / BLOCK_K;
+    const int t_beg = (int)(((long long)blockIdx.x * batch.n_tiles) / gridDim.x);
+    const int t_end = (int)(((long long)(blockIdx.x + 1) * batch.n_tiles) / gridDim.x);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -184,7 +208,10 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             mbar_init(bar_aready + 8 * s, 128);
             mbar_init(bar_empty + 8 * s, 1);
         }
-        mbar_init(bar_acc, 1);
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_accf + 8 * b, 1);
+            mbar_init(bar_acce + 8 * b, 128);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -200,122 +227,190 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
     if (warp == 0) {
         // ===== TMA producer
         if (lane == 0) {
-            const uint32_t tx = A_TILE_BYTES + (SPLIT3 ? 2u : 1u) * (uint32_t)NT * BLOCK_K * 4u;
-            for (int kb = 0; kb < num_kb; ++kb) {
-                const int s = kb % STAGES;
-                const uint32_t ph = (kb / STAGES) & 1;
-                mbar_wait(bar_empty + 8 * s, ph ^ 1);
-                const uint32_t stage = smem_base + s * STAGE_BYTES;
-                mbar_expect_tx(bar_full + 8 * s, tx);
-                tma_load_2d(stage, &g.mapA, kb * BLOCK_K, m0, bar_full + 8 * s);
-                tma_load_2d(stage + A_TILE_BYTES, &g.mapBhi, kb * BLOCK_K, n0, bar_full + 8 * s);
-                if (SPLIT3) tma_load_2d(stage + A_TILE_BYTES + B_TILE_BYTES_MAX, &g.mapBlo, kb * BLOCK_K, n0, bar_full + 8 * s);
+            uint32_t it = 0; // k-block counter across tiles
+            for (int t = t_beg; t < t_end; ++t) {
+                const TileCoord tc = tile_coord(batch, t);
+                const TcGroup &g = batch.g[tc.gi];
+                const uint32_t tx = A_TILE_BYTES + (SPLIT3 ? 2u : 1u) * (uint32_t)g.NT * BLOCK_K * 4u;
+                const int num_kb = g.K / BLOCK_K;
+                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                    const int s = it % STAGES;
+                    const uint32_t ph = (it / STAGES) & 1;
+                    mbar_wait(bar_empty + 8 * s, ph ^ 1);
+                    const uint32_t stage = smem_base + s * STAGE_BYTES;
+                    mbar_expect_tx(bar_full + 8 * s, tx);
+                    tma_load_2d(stage, &g.mapA, kb * BLOCK_K, tc.m0, bar_full + 8 * s);
+                    tma_load_2d(stage + A_TILE_BYTES, &g.mapBhi, kb * BLOCK_K, tc.n0, bar_full + 8 * s);
+                    if (SPLIT3) tma_load_2d(stage + A_TILE_BYTES + B_TILE_BYTES_MAX, &g.mapBlo, kb * BLOCK_K, tc.n0, bar_full + 8 * s);
+                }
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer
         if (lane == 0) {
-            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NT >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
-            for (int kb = 0; kb < num_kb; ++kb) {
-                const int s = kb % STAGES;
-                const uint32_t ph = (kb / STAGES) & 1;
-                mbar_wait(bar_full + 8 * s, ph);
-                mbar_wait(bar_aready + 8 * s, ph);
+            uint32_t it = 0;
+            int lt = 0; // local tile counter
+            for (int t = t_beg; t < t_end; ++t, ++lt) {
+                const TileCoord tc = tile_coord(batch, t);
+                const TcGroup &g = batch.g[tc.gi];
+                const int num_kb = g.K / BLOCK_K;
+                const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(g.NT >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+                const int b = lt & 1;
+                const uint32_t acc = tmem_base + b * TMEM_ACC_STRIDE;
+                mbar_wait(bar_acce + 8 * b, ((lt >> 1) & 1) ^ 1); // epilogue has drained this accumulator buffer
                 tc_fence_after();
-                const uint32_t stage = smem_base + s * STAGE_BYTES;
-                const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
-                const uint64_t dlo = make_kmajor_sw128_desc(stage + A_TILE_BYTES + B_TILE_BYTES_MAX);
-                const uint32_t a_hi = tmem_base + TMEM_A_COL0 + 64 * s, a_lo = a_hi + 32;
+                for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                    const int s = it % STAGES;
+                    const uint32_t ph = (it / STAGES) & 1;
+                    mbar_wait(bar_full + 8 * s, ph);
+                    mbar_wait(bar_aready + 8 * s, ph);
+                    tc_fence_after();
+                    const uint32_t stage = smem_base + s * STAGE_BYTES;
+                    const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
+                    const uint64_t dlo = make_kmajor_sw128_desc(stage + A_TILE_BYTES + B_TILE_BYTES_MAX);
+                    const uint32_t a_hi = tmem_base + TMEM_A_COL0 + 64 * s, a_lo = a_hi + 32;
 #pragma unroll
-                for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
-                    const uint64_t koff = (uint64_t)(k * UMMA_K * 4 >> 4);
-                    const uint32_t first = (kb | k) ? 1u : 0u;
-                    if (SPLIT3) {
-                        mma_tf32_ts(tmem_base, a_lo + k * UMMA_K, dhi + koff, idesc, first);
-                        mma_tf32_ts(tmem_base, a_hi + k * UMMA_K, dlo + koff, idesc, 1u);
-                        mma_tf32_ts(tmem_base, a_hi + k * UMMA_K, dhi + koff, idesc, 1u);
-                    } else {
-                        mma_tf32_ts(tmem_base, a_hi + k * UMMA_K, dhi + koff, idesc, first);
+                    for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+                        const uint64_t koff = (uint64_t)(k * UMMA_K * 4 >> 4);
+                        const uint32_t first = (kb | k) ? 1u : 0u;
+                        if (SPLIT3) {
+                            mma_tf32_ts(acc, a_lo + k * UMMA_K, dhi + koff, idesc, first);
+                            mma_tf32_ts(acc, a_hi + k * UMMA_K, dlo + koff, idesc, 1u);
+                            mma_tf32_ts(acc, a_hi + k * UMMA_K, dhi + koff, idesc, 1u);
+                        } else {
+                            mma_tf32_ts(acc, a_hi + k * UMMA_K, dhi + koff, idesc, first);
+                        }
+                    }
+                    tc_commit(bar_empty + 8 * s);
+                }
+                tc_commit(bar_accf + 8 * b);
+            }
+        }
+    } else if (warp < 10) {
+        // ===== converters: fp32 A row -> tf32 hi/lo in TMEM.  Two groups of four warps (lane quarters warp & 3)
+        // take alternate K blocks, so one block's LDS -> split -> tcgen05.st -> wait latency hides behind the other's.
+        const int quarter = warp & 3;
+        const int cgroup = (warp - 2) >> 2;
+        const int row = quarter * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
+        uint32_t it = 0;
+        for (int t = t_beg; t < t_end; ++t) {
+            const TileCoord tc = tile_coord(batch, t);
+            const int num_kb = batch.g[tc.gi].K / BLOCK_K;
+            for (int kb = 0; kb < num_kb; ++kb, ++it) {
+                if ((int)(it & 1) != cgroup) continue;
+                const int s = it % STAGES;
+                const uint32_t ph = (it / STAGES) & 1;
+                mbar_wait(bar_full + 8 * s, ph);
+                const uint32_t arow = smem_base + s * STAGE_BYTES + row * 128;
+                uint32_t hi[32], lo[32];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    float4 v;
+                    const uint32_t addr = arow + (uint32_t)((c ^ (row & 7)) << 4);
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+                    const float x[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const uint32_t h = tf32_round(x[e]);
+                        hi[4 * c + e] = h;
+                        if (SPLIT3) lo[4 * c + e] = tf32_round(x[e] - __uint_as_float(h));
                     }
                 }
-                tc_commit(bar_empty + 8 * s);
+                tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s, hi);
+                if (SPLIT3) tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s + 32, lo);
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                tc_fence_before();
+                mbar_arrive(bar_aready + 8 * s);
             }
-            tc_commit(bar_acc);
         }
     } else {
-        // ===== converters, then epilogue (warps 2..5 -> TMEM lane quarters 2,3,0,1)
+        // ===== epilogue (warps 10..13 -> lane quarters 2,3,0,1): this thread owns accumulator row `row`.
+        // Global traffic goes through a per-warp 32 x 32 staging chunk so that every LDG/STG covers full 128-byte lines.
         const int quarter = warp & 3;
         const int row = quarter * 32 + lane;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
-        for (int kb = 0; kb < num_kb; ++kb) {
-            const int s = kb % STAGES;
-            const uint32_t ph = (kb / STAGES) & 1;
-            mbar_wait(bar_full + 8 * s, ph);
-            const uint32_t arow = smem_base + s * STAGE_BYTES + row * 128;
-            uint32_t hi[32], lo[32];
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                float4 v;
-                const uint32_t addr = arow + (uint32_t)((c ^ (row & 7)) << 4);
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-                const float x[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const uint32_t h = tf32_round(x[e]);
-                    hi[4 * c + e] = h;
-                    if (SPLIT3) lo[4 * c + e] = tf32_round(x[e] - __uint_as_float(h));
-                }
-            }
-            tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s, hi);
-            if (SPLIT3) tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s + 32, lo);
-            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-            tc_fence_before();
-            mbar_arrive(bar_aready + 8 * s);
-        }
-
-        // ---- epilogue: this thread owns output row m0 + row, columns n0 .. n0 + NT
-        mbar_wait(bar_acc, 0);
-        tc_fence_after();
-        const int m = m0 + row;
-        const bool rowok = m < g.M;
+        const uint32_t stg = bar_base + 256 + (uint32_t)(warp - 10) * EPI_STG_BYTES;
+        const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
+        const int sub_r = lane >> 3, sub_c = (lane & 7) * 4; // cooperative access: 4 rows x 8 x 16 B per instruction
         const float alpha = batch.alpha, inv_alpha = 1.0f / batch.alpha;
-        float *crow = g.C + (size_t)(rowok ? m : 0) * g.ldc + n0;
-        float esum = 0.f;
-        for (int c0 = 0; c0 < NT; c0 += 32) {
-            uint32_t acc[32];
-            tmem_ld32(lane_addr + c0, acc);
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (rowok) {
+        int lt = 0;
+        for (int t = t_beg; t < t_end; ++t, ++lt) {
+            const TileCoord tc = tile_coord(batch, t);
+            const TcGroup &g = batch.g[tc.gi];
+            const int b = lt & 1;
+            mbar_wait(bar_accf + 8 * b, (lt >> 1) & 1);
+            tc_fence_after();
+            const int mrow0 = tc.m0 + quarter * 32; // first global row of this warp's 32 rows
+            const int m = mrow0 + lane;
+            const bool rowok = m < g.M;
+            float esum = 0.f;
+            for (int c0 = 0; c0 < g.NT; c0 += 32) {
+                const int w = min(32, g.NT - c0); // 32 or 16 (warp-uniform)
+                float *cbase = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
+                if (EPI == EPI_DCELU || EPI == EPI_ACCUM) { // previous contents, coalesced -> staging
 #pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    float4 o;
-                    float *ov = reinterpret_cast<float *>(&o);
-                    float4 prev = make_float4(0.f, 0.f, 0.f, 0.f), bb = prev, ww = prev;
-                    if (EPI == EPI_DCELU || EPI == EPI_ACCUM) prev = *reinterpret_cast<const float4 *>(crow + c0 + 4 * q);
-                    if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bb = *reinterpret_cast<const float4 *>(g.bias + n0 + c0 + 4 * q);
-                    if (EPI == EPI_CELU_OUT) ww = *reinterpret_cast<const float4 *>(g.w4 + n0 + c0 + 4 * q);
-                    const float *pv = reinterpret_cast<const float *>(&prev);
-                    const float *bv = reinterpret_cast<const float *>(&bb);
-                    const float *wv = reinterpret_cast<const float *>(&ww);
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        float v = __uint_as_float(acc[4 * q + e]);
-                        if (EPI == EPI_CELU) v = celu_fwd(v + bv[e], alpha, inv_alpha);
-                        if (EPI == EPI_CELU_OUT) {
-                            const float h = celu_fwd(v + bv[e], alpha, inv_alpha);
-                            esum = fmaf(h, wv[e], esum);
-                            v = wv[e] * celu_grad_from_h(h, inv_alpha);
-                        }
-                        if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[e], inv_alpha);
-                        if (EPI == EPI_ACCUM) v += pv[e];
-                        ov[e] = v;
+                    for (int i = 0; i < 8; ++i) {
+                        const int r = i * 4 + sub_r;
+                        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (mrow0 + r < g.M && sub_c < w) v = *reinterpret_cast<const float4 *>(cbase + (size_t)r * g.ldc + sub_c);
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
                     }
-                    *reinterpret_cast<float4 *>(crow + c0 + 4 * q) = o;
+                    __syncwarp();
                 }
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    if (h * 16 >= w) break;
+                    uint32_t acc[16];
+                    tmem_ld16(lane_addr + b * TMEM_ACC_STRIDE + c0 + h * 16, acc);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int col = h * 16 + 4 * q;
+                        float4 o;
+                        float *ov = reinterpret_cast<float *>(&o);
+                        float4 prev = make_float4(0.f, 0.f, 0.f, 0.f), bb = prev, ww = prev;
+                        if (EPI == EPI_DCELU || EPI == EPI_ACCUM)
+                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(prev.x), "=f"(prev.y), "=f"(prev.z), "=f"(prev.w) : "r"(my_row + col * 4));
+                        if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bb = *reinterpret_cast<const float4 *>(g.bias + tc.n0 + c0 + col);
+                        if (EPI == EPI_CELU_OUT) ww = *reinterpret_cast<const float4 *>(g.w4 + tc.n0 + c0 + col);
+                        const float *pv = reinterpret_cast<const float *>(&prev);
+                        const float *bv = reinterpret_cast<const float *>(&bb);
+                        const float *wv = reinterpret_cast<const float *>(&ww);
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            float v = __uint_as_float(acc[4 * q + e]);
+                            if (EPI == EPI_CELU) v = celu_fwd(v + bv[e], alpha, inv_alpha);
+                            if (EPI == EPI_CELU_OUT) {
+                                const float hh = celu_fwd(v + bv[e], alpha, inv_alpha);
+                                esum = fmaf(hh, wv[e], esum);
+                                v = wv[e] * celu_grad_from_h(hh, inv_alpha);
+                            }
+                            if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[e], inv_alpha);
+                            if (EPI == EPI_ACCUM) v += pv[e];
+                            ov[e] = v;
+                        }
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + col * 4), "f"(o.x), "f"(o.y), "f"(o.z), "f"(o.w) : "memory");
+                    }
+                }
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < 8; ++i) { // staging -> global, full 128-byte lines
+                    const int r = i * 4 + sub_r;
+                    if (mrow0 + r < g.M && sub_c < w) {
+                        float4 v;
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
+                        *reinterpret_cast<float4 *>(cbase + (size_t)r * g.ldc + sub_c) = v;
+                    }
+                }
+                __syncwarp();
             }
+            // the accumulator buffer may be overwritten by the MMAs of tile lt + 2
+            tc_fence_before();
+            mbar_arrive(bar_acce + 8 * b);
+            // a layer wider than one tile contributes its share of the output-layer dot from each half
+            if (EPI == EPI_CELU_OUT && rowok) atomicAdd(g.e_atom + m, esum);
         }
-        if (EPI == EPI_CELU_OUT && rowok) g.e_atom[m] += esum; // one thread per row, full width in this CTA
-        tc_fence_before();
     }
     __syncthreads();
     if (warp == 1) {
@@ -351,15 +446,24 @@ bool make_map(CUtensorMap *m, const float *base, int rows, int cols, int ld, int
                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+int g_num_sms = 0;
+
 template <int EPI>
 void launch(cudaStream_t st, const TcBatch &b, int tiles, bool split3)
 {
+    if (!g_num_sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (g_num_sms <= 0) g_num_sms = 148;
+    }
+    const int grid = tiles < g_num_sms ? tiles : g_num_sms; // persistent: one CTA per SM
     if (split3) {
         cudaFuncSetAttribute(k_gemm_tc<EPI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        k_gemm_tc<EPI, true><<<tiles, THREADS, SMEM_BYTES, st>>>(b);
+        k_gemm_tc<EPI, true><<<grid, THREADS, SMEM_BYTES, st>>>(b);
     } else {
         cudaFuncSetAttribute(k_gemm_tc<EPI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        k_gemm_tc<EPI, false><<<tiles, THREADS, SMEM_BYTES, st>>>(b);
+        k_gemm_tc<EPI, false><<<grid, THREADS, SMEM_BYTES, st>>>(b);
     }
 }
 
@@ -376,8 +480,14 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
         const GemmGroup &g = b.g[i];
         TcGroup &t = tb.g[i];
         if (!g.Bt_hi || !g.Bt_lo) { c->err = "tensor-core path: weight operand has no tf32 split"; return NNP_EINVAL; }
-        const int NT = g.N > N_MAX ? N_MAX : g.N;
-        if (g.N % NT || g.K % BLOCK_K || NT % 16) { c->err = "tensor-core path: unsupported GEMM shape"; return NNP_EINVAL; }
+        int NT = g.N;                       // <= 128 columns per tile; wider layers in equal parts that are multiples of 16
+        int parts = 1;
+        while (NT > NT_MAX || (g.N % parts) || (NT % 16)) {
+            ++parts;
+            if (parts > 64) { c->err = "tensor-core path: unsupported GEMM width"; return NNP_EINVAL; }
+            NT = g.N / parts;
+        }
+        if (g.K % BLOCK_K) { c->err = "tensor-core path: K must be a multiple of 32"; return NNP_EINVAL; }
         if (!make_map(&t.mapA, g.A, g.M, g.K, g.lda, TILE_M) || !make_map(&t.mapBhi, g.Bt_hi, g.N, g.K, g.K, NT) ||
             !make_map(&t.mapBlo, g.Bt_lo, g.N, g.K, g.K, NT)) {
             c->err = "cuTensorMapEncodeTiled failed";
@@ -385,12 +495,14 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
         }
         t.C = g.C; t.bias = g.bias; t.w4 = g.w4; t.e_atom = g.e_atom;
         t.M = g.M; t.N = g.N; t.K = g.K; t.ldc = g.ldc;
+        t.NT = NT;
         t.n_tiles_n = g.N / NT;
         tb.tile_off[i] = tiles;
         tiles += nnp_div_up(g.M, TILE_M) * t.n_tiles_n;
     }
     tb.n_groups = b.n_groups;
     tb.tile_off[b.n_groups] = tiles;
+    tb.n_tiles = tiles;
     if (tiles == 0) return NNP_OK;
     const bool s3 = split3 != 0;
     switch (epi) {
