@@ -9,12 +9,16 @@ namespace {
 constexpr int BM = 128, BN = 64, BK = 16, THREADS = 256;
 constexpr int TM = 8, TN = 4; // per-thread micro-tile: 16 x 16 threads
 
+// Branch-free CELU: max(x,0) + alpha (2^(min(x,0) log2e / alpha) - 1).  (A conditional form makes the compiler
+// emit one divergent branch per element, which serialised the tensor-core epilogue.)
 __device__ __forceinline__ float celu_fwd(float x, float alpha, float inv_alpha)
 {
-    return x > 0.f ? x : alpha * (__expf(x * inv_alpha) - 1.0f);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fminf(x, 0.f) * (inv_alpha * 1.4426950408889634f)));
+    return fmaxf(x, 0.f) + alpha * (e - 1.0f);
 }
 // CELU'(z) expressed with h = CELU(z): 1 for h > 0, else exp(z/alpha) = 1 + h/alpha
-__device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
+__device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return fmaf(fminf(h, 0.f), inv_alpha, 1.0f); }
 
 template <int EPI>
 __global__ void __launch_bounds__(THREADS)

@@ -16,6 +16,7 @@
 //   warps 2-5 epilogue: tcgen05.ld the accumulator row, apply bias/CELU/CELU'/output-layer dot, store.
 #include <cuda.h>
 
+#include <stdio.h>
 #include <string.h>
 
 #include "nnp_internal.cuh"
@@ -54,7 +55,16 @@ struct TcBatch {
     int tile_off[NNP_MAX_SPECIES]; // prefix sum of (m tiles x n tiles) per group
     int n_tiles;
     float alpha;
+#ifdef NNP_TC_TRACE
+    long long *trace; // [it][8] clock64 stamps of CTA 0
+#endif
 };
+
+#ifdef NNP_TC_TRACE
+#define TRACE(slot) do { if (blockIdx.x == 0 && batch.trace && it < 256) batch.trace[it * 8 + (slot)] = clock64(); } while (0)
+#else
+#define TRACE(slot) do { } while (0)
+#endif
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -165,11 +175,16 @@ __device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr)
     return d;
 }
 
+// Branch-free CELU: max(x,0) + alpha (2^(min(x,0) log2e / alpha) - 1).  (A conditional form makes the compiler
+// emit one divergent branch per element, which serialised the tensor-core epilogue.)
 __device__ __forceinline__ float celu_fwd(float x, float alpha, float inv_alpha)
 {
-    return x > 0.f ? x : alpha * (__expf(x * inv_alpha) - 1.0f);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(fminf(x, 0.f) * (inv_alpha * 1.4426950408889634f)));
+    return fmaxf(x, 0.f) + alpha * (e - 1.0f);
 }
-__device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
+// CELU'(z) expressed with h = CELU(z): 1 for h > 0, else exp(z/alpha) = 1 + h/alpha
+__device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return fmaf(fminf(h, 0.f), inv_alpha, 1.0f); }
 
 // tile index -> (group, m0, n0)
 struct TileCoord { int gi, m0, n0; };
@@ -205,7 +220,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_aready + 8 * s, 128);
+            mbar_init(bar_aready + 8 * s, 129); // 128 converter threads + the producer's expect_tx for the B tiles
             mbar_init(bar_empty + 8 * s, 1);
         }
         for (int b = 0; b < 2; ++b) {
@@ -231,17 +246,20 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             for (int t = t_beg; t < t_end; ++t) {
                 const TileCoord tc = tile_coord(batch, t);
                 const TcGroup &g = batch.g[tc.gi];
-                const uint32_t tx = A_TILE_BYTES + (SPLIT3 ? 2u : 1u) * (uint32_t)g.NT * BLOCK_K * 4u;
+                const uint32_t tx_b = (SPLIT3 ? 2u : 1u) * (uint32_t)g.NT * BLOCK_K * 4u;
                 const int num_kb = g.K / BLOCK_K;
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const int s = it % STAGES;
                     const uint32_t ph = (it / STAGES) & 1;
                     mbar_wait(bar_empty + 8 * s, ph ^ 1);
+                    TRACE(0);
                     const uint32_t stage = smem_base + s * STAGE_BYTES;
-                    mbar_expect_tx(bar_full + 8 * s, tx);
+                    // A -> full[s] (wakes the converters); B -> aready[s], the one barrier the MMA thread waits on
+                    mbar_expect_tx(bar_full + 8 * s, A_TILE_BYTES);
                     tma_load_2d(stage, &g.mapA, kb * BLOCK_K, tc.m0, bar_full + 8 * s);
-                    tma_load_2d(stage + A_TILE_BYTES, &g.mapBhi, kb * BLOCK_K, tc.n0, bar_full + 8 * s);
-                    if (SPLIT3) tma_load_2d(stage + A_TILE_BYTES + B_TILE_BYTES_MAX, &g.mapBlo, kb * BLOCK_K, tc.n0, bar_full + 8 * s);
+                    mbar_expect_tx(bar_aready + 8 * s, tx_b);
+                    tma_load_2d(stage + A_TILE_BYTES, &g.mapBhi, kb * BLOCK_K, tc.n0, bar_aready + 8 * s);
+                    if (SPLIT3) tma_load_2d(stage + A_TILE_BYTES + B_TILE_BYTES_MAX, &g.mapBlo, kb * BLOCK_K, tc.n0, bar_aready + 8 * s);
                 }
             }
         }
@@ -258,12 +276,14 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 const int b = lt & 1;
                 const uint32_t acc = tmem_base + b * TMEM_ACC_STRIDE;
                 mbar_wait(bar_acce + 8 * b, ((lt >> 1) & 1) ^ 1); // epilogue has drained this accumulator buffer
+                TRACE(6);
                 tc_fence_after();
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const int s = it % STAGES;
                     const uint32_t ph = (it / STAGES) & 1;
-                    mbar_wait(bar_full + 8 * s, ph);
-                    mbar_wait(bar_aready + 8 * s, ph);
+                    TRACE(3);
+                    mbar_wait(bar_aready + 8 * s, ph); // B tiles landed and A converted into TMEM
+                    TRACE(4);
                     tc_fence_after();
                     const uint32_t stage = smem_base + s * STAGE_BYTES;
                     const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
@@ -282,6 +302,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                         }
                     }
                     tc_commit(bar_empty + 8 * s);
+                    TRACE(5);
                 }
                 tc_commit(bar_accf + 8 * b);
             }
@@ -302,6 +323,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 const int s = it % STAGES;
                 const uint32_t ph = (it / STAGES) & 1;
                 mbar_wait(bar_full + 8 * s, ph);
+                if (threadIdx.x == 64 || threadIdx.x == 192) TRACE(1);
                 const uint32_t arow = smem_base + s * STAGE_BYTES + row * 128;
                 uint32_t hi[32], lo[32];
 #pragma unroll
@@ -322,6 +344,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 mbar_arrive(bar_aready + 8 * s);
+                if (threadIdx.x == 64 || threadIdx.x == 192) TRACE(2);
             }
         }
     } else {
@@ -340,51 +363,76 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             const TcGroup &g = batch.g[tc.gi];
             const int b = lt & 1;
             mbar_wait(bar_accf + 8 * b, (lt >> 1) & 1);
+#ifdef NNP_TC_TRACE
+            if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K) + 1; TRACE(7); }
+#endif
             tc_fence_after();
             const int mrow0 = tc.m0 + quarter * 32; // first global row of this warp's 32 rows
             const int m = mrow0 + lane;
             const bool rowok = m < g.M;
             float esum = 0.f;
-            for (int c0 = 0; c0 < g.NT; c0 += 32) {
-                const int w = min(32, g.NT - c0); // 32 or 16 (warp-uniform)
-                float *cbase = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
-                if (EPI == EPI_DCELU || EPI == EPI_ACCUM) { // previous contents, coalesced -> staging
+            // Operands from global memory are fetched one chunk ahead (the L1 is only ~12 KB next to 216 KB of
+            // shared memory, so every one of these loads is an L2 round trip): bias / w4 one column per lane
+            // (redistributed with shuffles), previous contents 8 x 16 B per lane, coalesced.
+            float bias_l = 0.f, w4_l = 0.f;
+            float4 pre[8];
+            auto prefetch = [&](int c0) {
+                const int w = min(32, g.NT - c0);
+                if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bias_l = lane < w ? g.bias[tc.n0 + c0 + lane] : 0.f;
+                if (EPI == EPI_CELU_OUT) w4_l = lane < w ? g.w4[tc.n0 + c0 + lane] : 0.f;
+                if (EPI == EPI_DCELU || EPI == EPI_ACCUM) {
+                    const float *cb = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const int r = i * 4 + sub_r;
-                        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (mrow0 + r < g.M && sub_c < w) v = *reinterpret_cast<const float4 *>(cbase + (size_t)r * g.ldc + sub_c);
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+                        pre[i] = (mrow0 + r < g.M && sub_c < w) ? *reinterpret_cast<const float4 *>(cb + (size_t)r * g.ldc + sub_c)
+                                                               : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                }
+            };
+            prefetch(0);
+            for (int c0 = 0; c0 < g.NT; c0 += 32) {
+                const int w = min(32, g.NT - c0); // 32 or 16 (warp-uniform)
+                float *cbase = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
+                const float bias_c = bias_l, w4_c = w4_l;
+                if (EPI == EPI_DCELU || EPI == EPI_ACCUM) { // previous contents -> staging
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int r = i * 4 + sub_r;
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(pre[i].x), "f"(pre[i].y), "f"(pre[i].z), "f"(pre[i].w) : "memory");
                     }
                     __syncwarp();
                 }
+                if (c0 + 32 < g.NT) prefetch(c0 + 32);
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     if (h * 16 >= w) break;
                     uint32_t acc[16];
                     tmem_ld16(lane_addr + b * TMEM_ACC_STRIDE + c0 + h * 16, acc);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#ifdef NNP_TC_TRACE
+                    if (threadIdx.x == 320 && c0 == 0 && h == 0) { const int it = lt * (g.K / BLOCK_K) + 2; TRACE(7); }
+#endif
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         const int col = h * 16 + 4 * q;
                         float4 o;
                         float *ov = reinterpret_cast<float *>(&o);
-                        float4 prev = make_float4(0.f, 0.f, 0.f, 0.f), bb = prev, ww = prev;
+                        float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (EPI == EPI_DCELU || EPI == EPI_ACCUM)
                             asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(prev.x), "=f"(prev.y), "=f"(prev.z), "=f"(prev.w) : "r"(my_row + col * 4));
-                        if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bb = *reinterpret_cast<const float4 *>(g.bias + tc.n0 + c0 + col);
-                        if (EPI == EPI_CELU_OUT) ww = *reinterpret_cast<const float4 *>(g.w4 + tc.n0 + c0 + col);
                         const float *pv = reinterpret_cast<const float *>(&prev);
-                        const float *bv = reinterpret_cast<const float *>(&bb);
-                        const float *wv = reinterpret_cast<const float *>(&ww);
 #pragma unroll
                         for (int e = 0; e < 4; ++e) {
                             float v = __uint_as_float(acc[4 * q + e]);
-                            if (EPI == EPI_CELU) v = celu_fwd(v + bv[e], alpha, inv_alpha);
+                            float bv = 0.f, wv = 0.f;
+                            if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bv = __shfl_sync(0xffffffffu, bias_c, col + e);
+                            if (EPI == EPI_CELU_OUT) wv = __shfl_sync(0xffffffffu, w4_c, col + e);
+                            if (EPI == EPI_CELU) v = celu_fwd(v + bv, alpha, inv_alpha);
                             if (EPI == EPI_CELU_OUT) {
-                                const float hh = celu_fwd(v + bv[e], alpha, inv_alpha);
-                                esum = fmaf(hh, wv[e], esum);
-                                v = wv[e] * celu_grad_from_h(hh, inv_alpha);
+                                const float hh = celu_fwd(v + bv, alpha, inv_alpha);
+                                esum = fmaf(hh, wv, esum);
+                                v = wv * celu_grad_from_h(hh, inv_alpha);
                             }
                             if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[e], inv_alpha);
                             if (EPI == EPI_ACCUM) v += pv[e];
@@ -393,6 +441,9 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                         asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + col * 4), "f"(o.x), "f"(o.y), "f"(o.z), "f"(o.w) : "memory");
                     }
                 }
+#ifdef NNP_TC_TRACE
+                if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 3; TRACE(7); }
+#endif
                 __syncwarp();
 #pragma unroll
                 for (int i = 0; i < 8; ++i) { // staging -> global, full 128-byte lines
@@ -404,10 +455,16 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     }
                 }
                 __syncwarp();
+#ifdef NNP_TC_TRACE
+                if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 4; TRACE(7); }
+#endif
             }
             // the accumulator buffer may be overwritten by the MMAs of tile lt + 2
             tc_fence_before();
             mbar_arrive(bar_acce + 8 * b);
+#ifdef NNP_TC_TRACE
+            if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K); TRACE(7); }
+#endif
             // a layer wider than one tile contributes its share of the output-layer dot from each half
             if (EPI == EPI_CELU_OUT && rowok) atomicAdd(g.e_atom + m, esum);
         }
@@ -504,6 +561,13 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     tb.tile_off[b.n_groups] = tiles;
     tb.n_tiles = tiles;
     if (tiles == 0) return NNP_OK;
+#ifdef NNP_TC_TRACE
+    static long long *d_trace = nullptr;
+    static int traced = 0;
+    if (!d_trace) { cudaMalloc(&d_trace, 256 * 8 * 8); }
+    tb.trace = (traced < 6) ? d_trace : nullptr;
+    if (tb.trace) cudaMemsetAsync(d_trace, 0, 256 * 8 * 8, c->stream);
+#endif
     const bool s3 = split3 != 0;
     switch (epi) {
     case EPI_CELU: launch<EPI_CELU>(c->stream, tb, tiles, s3); break;
@@ -514,5 +578,19 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     default: c->err = "bad epilogue"; return NNP_EINVAL;
     }
     c->launches += 1;
+#ifdef NNP_TC_TRACE
+    if (tb.trace) {
+        static long long h[256 * 8];
+        cudaStreamSynchronize(c->stream);
+        cudaMemcpy(h, d_trace, sizeof(h), cudaMemcpyDeviceToHost);
+        fprintf(stderr, "TRACE launch %d epi %d tiles %d (cycles rel. to first TMA issue): it | P0 tma-issue | C1 full-seen | C2 aready | M3 pre-wait | M4 aready | M5 committed | M6 acc-free | E7 epi-done\n", traced, epi, tiles);
+        for (int it = 0; it < 40; ++it) {
+            if (!h[it * 8]) break;
+            fprintf(stderr, "  %3d | %7lld | %7lld | %7lld | %7lld | %7lld | %7lld | %7lld | %7lld\n", it, h[it * 8] - h[0], h[it * 8 + 1] - h[0], h[it * 8 + 2] - h[0],
+                    h[it * 8 + 3] - h[0], h[it * 8 + 4] - h[0], h[it * 8 + 5] - h[0], h[it * 8 + 6] ? h[it * 8 + 6] - h[0] : 0, h[it * 8 + 7] ? h[it * 8 + 7] - h[0] : 0);
+        }
+        ++traced;
+    }
+#endif
     return NNP_OK;
 }
