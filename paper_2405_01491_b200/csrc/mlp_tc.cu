@@ -157,6 +157,17 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
         : "memory");
 }
 
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 // tf32 split: hi = x rounded to 10 mantissa bits (nearest, ties away), lo = x - hi (exact), lo rounded the same way
 __device__ __forceinline__ uint32_t tf32_round(float x)
 {
@@ -264,8 +275,9 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer
-        if (lane == 0) {
+        // ===== MMA issuer: the whole warp runs the loop with warp-uniform values (descriptors stay in uniform
+        // registers); one elected lane issues tcgen05.mma / tcgen05.commit.
+        {
             uint32_t it = 0;
             int lt = 0; // local tile counter
             for (int t = t_beg; t < t_end; ++t, ++lt) {
@@ -289,22 +301,25 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
                     const uint64_t dlo = make_kmajor_sw128_desc(stage + A_TILE_BYTES + B_TILE_BYTES_MAX);
                     const uint32_t a_hi = tmem_base + TMEM_A_COL0 + 64 * s, a_lo = a_hi + 32;
+                    if (elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
-                        const uint64_t koff = (uint64_t)(k * UMMA_K * 4 >> 4);
-                        const uint32_t first = (kb | k) ? 1u : 0u;
-                        if (SPLIT3) {
-                            mma_tf32_ts(acc, a_lo + k * UMMA_K, dhi + koff, idesc, first);
-                            mma_tf32_ts(acc, a_hi + k * UMMA_K, dlo + koff, idesc, 1u);
-                            mma_tf32_ts(acc, a_hi + k * UMMA_K, dhi + koff, idesc, 1u);
-                        } else {
-                            mma_tf32_ts(acc, a_hi + k * UMMA_K, dhi + koff, idesc, first);
+                        for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+                            const uint64_t koff = (uint64_t)(k * UMMA_K * 4 >> 4);
+                            const uint32_t first = (kb | k) ? 1u : 0u;
+                            if (SPLIT3) {
+                                mma_tf32_ts(acc, a_lo + k * UMMA_K, dhi + koff, idesc, first);
+                                mma_tf32_ts(acc, a_hi + k * UMMA_K, dlo + koff, idesc, 1u);
+                                mma_tf32_ts(acc, a_hi + k * UMMA_K, dhi + koff, idesc, 1u);
+                            } else {
+                                mma_tf32_ts(acc, a_hi + k * UMMA_K, dhi + koff, idesc, first);
+                            }
                         }
+                        tc_commit(bar_empty + 8 * s);
+                        if (kb + 1 == num_kb) tc_commit(bar_accf + 8 * b);
                     }
-                    tc_commit(bar_empty + 8 * s);
+                    __syncwarp();
                     TRACE(5);
                 }
-                tc_commit(bar_accf + 8 * b);
             }
         }
     } else if (warp < 10) {
