@@ -74,6 +74,10 @@ typedef struct {
     float accel_conv;         /* a = accel_conv * F / m  (4.184e-4 for kcal/mol, A, fs, amu; reading B6) */
     int mm_mode;              /* NNP_MM_*: how the MLP contractions are computed */
     int cap_r, cap_a;         /* neighbour-row capacities (radial / angular lists); 0 => 160 / 64; <= 255, multiple of 4 */
+    int dense_aev;            /* 0 (default): AEV columns of species absent from the loaded system -- identically zero
+                                 for every atom -- are neither stored nor multiplied (the layer-1 weights are gathered
+                                 to the active columns at nnp_set_system; results are unchanged).  1: always keep all
+                                 aev_len columns (e.g. 1008), as a plain implementation would. */
 } nnp_params;
 
 /* Copies all parameters to the device (the caller keeps its arrays) and allocates every scratch buffer
@@ -150,7 +154,8 @@ int nnp_profile_read(nnp_ctx *ctx, double *h_ms_sum, int64_t *h_samples);
 
 /* Introspection for the bench: number of kernel launches issued by this ctx so far. */
 int64_t nnp_launch_count(const nnp_ctx *ctx);
-int nnp_aev_len(const nnp_ctx *ctx);
+int nnp_aev_len(const nnp_ctx *ctx);            /* full AEV length of the model (1008 for 7 species) */
+int nnp_aev_active_columns(const nnp_ctx *ctx); /* columns stored for the loaded system (see nnp_params.dense_aev) */
 
 #ifdef __cplusplus
 }

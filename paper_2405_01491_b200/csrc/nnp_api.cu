@@ -104,13 +104,37 @@ __global__ void k_get_neighbors(int n, const int *__restrict__ nbr, const uint16
     for (int a = 0; a < cnt && a < stride; ++a) list[(size_t)o * stride + a] = orig[nbr[(size_t)i * cap + a]];
 }
 
-__global__ void k_get_aev(int n, int len, int kpad, const float *__restrict__ G, const int *__restrict__ orig,
-                          float *__restrict__ out)
+// Test hook: active columns of G -> the full aev_len layout (columns of absent species are zero).
+__global__ void k_get_aev(int n, int len_full, int len_c, int kpad, const float *__restrict__ G, const int *__restrict__ fmap,
+                          const int *__restrict__ orig, float *__restrict__ out)
 {
     int i = blockIdx.x;
     if (i >= n) return;
     const int o = orig[i];
-    for (int q = threadIdx.x; q < len; q += blockDim.x) out[(size_t)o * len + q] = G[(size_t)i * kpad + q];
+    for (int q = threadIdx.x; q < len_full; q += blockDim.x) out[(size_t)o * len_full + q] = 0.f;
+    __syncthreads();
+    for (int q = threadIdx.x; q < len_c; q += blockDim.x) out[(size_t)o * len_full + fmap[q]] = G[(size_t)i * kpad + q];
+}
+
+// Layer-1 weights restricted to the active AEV columns: row c of the compact matrix is row fmap[c] of the full one
+// (zero for padding), in both orientations and, for the tensor-core modes, as tf32 hi / lo splits.
+__global__ void k_gather_l1(int kpad, int out, const int *__restrict__ fmap, const float *__restrict__ W_full,
+                            float *__restrict__ W, float *__restrict__ Wt, float *__restrict__ W_hi, float *__restrict__ W_lo,
+                            float *__restrict__ Wt_hi, float *__restrict__ Wt_lo)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= kpad * out) return;
+    const int c = idx / out, j = idx - c * out;
+    const int f = fmap[c];
+    const float v = f >= 0 ? W_full[(size_t)f * out + j] : 0.f;
+    W[idx] = v;
+    Wt[(size_t)j * kpad + c] = v;
+    if (W_hi) {
+        const uint32_t h = (__float_as_uint(v) + 0x1000u) & 0xffffe000u;
+        const uint32_t l = (__float_as_uint(v - __uint_as_float(h)) + 0x1000u) & 0xffffe000u;
+        W_hi[idx] = __uint_as_float(h); W_lo[idx] = __uint_as_float(l);
+        Wt_hi[(size_t)j * kpad + c] = __uint_as_float(h); Wt_lo[(size_t)j * kpad + c] = __uint_as_float(l);
+    }
 }
 
 __global__ void k_get_e_atom(int n, const float *__restrict__ e_atom, const int *__restrict__ spc,
@@ -130,6 +154,56 @@ int dev_alloc(nnp_ctx *c, Tp **p, size_t count)
 }
 
 LayerW &layer(nnp_ctx *c, int net, int s, int l) { return c->layers[((size_t)net * c->S + s) * NNP_NLAYERS + l]; }
+Layer1C &l1c(nnp_ctx *c, int net, int s) { return c->l1c[(size_t)net * c->S + s]; }
+
+// Active-column layout for the species in `mask`; rebuilds the compact layer-1 copies when the mask changed.
+int set_layout(nnp_ctx *c, unsigned mask)
+{
+    AevParams &a = c->aev;
+    const int S = c->S;
+    int np = 0;
+    for (int s = 0; s < NNP_MAX_SPECIES; ++s) { a.cmap[s] = -1; a.plist[s] = 0; }
+    for (int s = 0; s < S; ++s)
+        if (mask >> s & 1u) { a.cmap[s] = np; a.plist[np] = s; ++np; }
+    a.np = np;
+    a.n_rad = np * NNP_NSHF_R;
+    a.aev_len = a.n_rad + np * (np + 1) / 2 * NNP_ANG_BLOCK;
+    a.kpad = (a.aev_len + 31) / 32 * 32;
+    if (mask == c->present_mask) return NNP_OK;
+    // compact column -> full column
+    std::vector<int> fmap(c->kpad_full, -1);
+    for (int cs = 0; cs < np; ++cs)
+        for (int k = 0; k < NNP_NSHF_R; ++k) fmap[cs * NNP_NSHF_R + k] = a.plist[cs] * NNP_NSHF_R + k;
+    int pc = 0;
+    for (int cs = 0; cs < np; ++cs)
+        for (int ct = cs; ct < np; ++ct, ++pc) {
+            const int s = a.plist[cs], t = a.plist[ct];
+            const int pf = s * (2 * S + 1 - s) / 2 + (t - s);
+            for (int q = 0; q < NNP_ANG_BLOCK; ++q) fmap[a.n_rad + pc * NNP_ANG_BLOCK + q] = S * NNP_NSHF_R + pf * NNP_ANG_BLOCK + q;
+        }
+    CU(c, cudaMemcpyAsync(c->d_fmap, fmap.data(), sizeof(int) * c->kpad_full, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream)); // fmap is a stack-lifetime host buffer
+    float *base = c->d_l1c_blob;
+    const int narr = c->mm_mode ? 6 : 2;
+    for (int net = 0; net < c->n_nets; ++net)
+        for (int s = 0; s < S; ++s) {
+            const int out = c->widths[s][1];
+            const size_t cnt = (size_t)a.kpad * out;
+            Layer1C &L = l1c(c, net, s);
+            L.W = base; L.Wt = base + cnt;
+            L.W_hi = L.W_lo = L.Wt_hi = L.Wt_lo = nullptr;
+            if (c->mm_mode) { L.W_hi = base + 2 * cnt; L.W_lo = base + 3 * cnt; L.Wt_hi = base + 4 * cnt; L.Wt_lo = base + 5 * cnt; }
+            base += (size_t)narr * c->kpad_full * out;
+            k_gather_l1<<<nnp_div_up((int)cnt, T), T, 0, c->stream>>>(a.kpad, out, c->d_fmap, layer(c, net, s, 0).W, L.W, L.Wt,
+                                                                      L.W_hi, L.W_lo, L.Wt_hi, L.Wt_lo);
+            c->launches += 1;
+        }
+    // G / dG: columns beyond aev_len must be zero (layer 1 multiplies all kpad columns)
+    CU(c, cudaMemsetAsync(c->G, 0, sizeof(float) * (size_t)c->max_atoms * c->kpad_full, c->stream));
+    CU(c, cudaGetLastError());
+    c->present_mask = mask;
+    return NNP_OK;
+}
 
 int check_flags(nnp_ctx *c)
 {
@@ -161,8 +235,8 @@ void make_batch(nnp_ctx *c, int net, int op, GemmBatch &b)
         switch (op) {
         case 0:
             g.A = c->G + (size_t)off * kpad; g.lda = kpad; g.K = kpad; g.N = h1;
-            g.B = layer(c, net, s, 0).W; g.Bt = layer(c, net, s, 0).Wt; g.bias = layer(c, net, s, 0).b;
-            g.Bt_hi = layer(c, net, s, 0).Wt_hi; g.Bt_lo = layer(c, net, s, 0).Wt_lo;
+            g.B = l1c(c, net, s).W; g.Bt = l1c(c, net, s).Wt; g.bias = layer(c, net, s, 0).b;
+            g.Bt_hi = l1c(c, net, s).Wt_hi; g.Bt_lo = l1c(c, net, s).Wt_lo;
             g.C = H0; g.ldc = c->hmax[0];
             break;
         case 1:
@@ -192,8 +266,8 @@ void make_batch(nnp_ctx *c, int net, int op, GemmBatch &b)
             break;
         case 5: // dE/dG (+)= delta1 W1^T
             g.A = H0; g.lda = c->hmax[0]; g.K = h1; g.N = kpad;
-            g.B = layer(c, net, s, 0).Wt; g.Bt = layer(c, net, s, 0).W;
-            g.Bt_hi = layer(c, net, s, 0).W_hi; g.Bt_lo = layer(c, net, s, 0).W_lo;
+            g.B = l1c(c, net, s).Wt; g.Bt = l1c(c, net, s).W;
+            g.Bt_hi = l1c(c, net, s).W_hi; g.Bt_lo = l1c(c, net, s).W_lo;
             g.C = c->dG + (size_t)off * kpad; g.ldc = kpad;
             break;
         }
@@ -283,14 +357,15 @@ extern "C" {
 const char *nnp_last_error(const nnp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
 int64_t nnp_launch_count(const nnp_ctx *ctx) { return ctx ? ctx->launches : 0; }
-int nnp_aev_len(const nnp_ctx *ctx) { return ctx ? ctx->aev.aev_len : 0; }
+int nnp_aev_len(const nnp_ctx *ctx) { return ctx ? ctx->aev_len_full : 0; }
+int nnp_aev_active_columns(const nnp_ctx *ctx) { return ctx ? ctx->aev.aev_len : 0; }
 
 void nnp_destroy(nnp_ctx *c)
 {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    void *ptrs[] = {c->d_params_blob, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
+    void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags,
@@ -299,6 +374,7 @@ void nnp_destroy(nnp_ctx *c)
     for (auto &m : c->prof_marks) cudaEventDestroy(m.first);
     for (auto &e : c->prof_pool) cudaEventDestroy(e);
     delete[] c->layers;
+    delete[] c->l1c;
     delete c;
 }
 
@@ -330,7 +406,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     if (cudaSetDevice(device) != cudaSuccess) NNP_FAIL(none, NNP_ECUDA, "cudaSetDevice(%d) failed", device);
     nnp_ctx *c = new nnp_ctx();
     // new T() value-initialises: every POD member starts at zero
-    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode;
+    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode; c->dense_aev = p->dense_aev != 0;
     c->alpha = p->celu_alpha; c->accel_conv = p->accel_conv;
     c->stream = (cudaStream_t)cuda_stream; c->device = device;
     c->max_atoms = max_atoms; c->max_mols = max_mols;
@@ -342,19 +418,28 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
         }
     AevParams &a = c->aev;
     a.S = S; a.n_rad = S * NNP_NSHF_R; a.aev_len = aev_len; a.kpad = (aev_len + 31) / 32 * 32;
+    a.np = S;
+    for (int s = 0; s < NNP_MAX_SPECIES; ++s) { a.cmap[s] = s < S ? s : -1; a.plist[s] = s < S ? s : 0; }
+    c->aev_len_full = aev_len; c->kpad_full = a.kpad;
     a.cap_r = cap_r; a.cap_a = cap_a;
     a.rcr = p->rcr; a.rca = p->rca; a.rcr2 = p->rcr * p->rcr; a.rca2 = p->rca * p->rca;
     a.pi_rcr = (float)(M_PI / (double)p->rcr); a.pi_rca = (float)(M_PI / (double)p->rca);
     a.eta_r = p->eta_r; a.eta_a = p->eta_a; a.zeta = p->zeta;
     a.neg_eta_r_log2e = (float)(-(double)p->eta_r * 1.4426950408889634);
     a.neg_eta_a_log2e = (float)(-(double)p->eta_a * 1.4426950408889634);
+    a.ka = (float)sqrt((double)p->eta_a * 1.4426950408889634);
+    a.kr = (float)sqrt((double)p->eta_r * 1.4426950408889634);
+    for (int k = 0; k < NNP_NSHF_R; ++k) a.kr_shf[k] = (float)(sqrt((double)p->eta_r * 1.4426950408889634) * (double)p->shf_r[k]);
+    for (int k = 0; k < NNP_NSHF_A; ++k) a.ka_shf[k] = (float)(sqrt((double)p->eta_a * 1.4426950408889634) * (double)p->shf_a[k]);
     for (int k = 0; k < NNP_NSHF_R; ++k) a.shf_r[k] = p->shf_r[k];
     for (int k = 0; k < NNP_NSHF_A; ++k) a.shf_a[k] = p->shf_a[k];
     for (int k = 0; k < NNP_NSHF_Z; ++k) { a.cos_z[k] = (float)cos((double)p->shf_z[k]); a.sin_z[k] = (float)sin((double)p->shf_z[k]); }
 
     // ---- weights: W [in_pad][out], Wt [out][in_pad], b [out] for every (net, species, layer)
     c->layers = new LayerW[(size_t)c->n_nets * S * NNP_NLAYERS];
-    size_t total = 0;
+    c->l1c = new Layer1C[(size_t)c->n_nets * S]();
+    size_t total = 0, total_l1c = 0;
+    for (int s = 0; s < S; ++s) total_l1c += (size_t)c->n_nets * (c->mm_mode ? 6 : 2) * a.kpad * c->widths[s][1];
     for (int net = 0; net < c->n_nets; ++net)
         for (int s = 0; s < S; ++s)
             for (int l = 0; l < NNP_NLAYERS; ++l) {
@@ -411,6 +496,14 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
 #define TRY(x) do { if ((rc = (x)) != NNP_OK) { g_create_error = c->err; nnp_destroy(c); return rc; } } while (0)
 #define TRYCU(x) do { cudaError_t _e = (x); if (_e != cudaSuccess) { g_create_error = std::string(#x ": ") + cudaGetErrorString(_e); nnp_destroy(c); return _e == cudaErrorMemoryAllocation ? NNP_ENOMEM : NNP_ECUDA; } } while (0)
     TRY(dev_alloc(c, &c->d_params_blob, total));
+    TRY(dev_alloc(c, &c->d_l1c_blob, total_l1c));
+    TRY(dev_alloc(c, &c->d_fmap, (size_t)a.kpad));
+    TRY(dev_alloc(c, &c->d_tri, (size_t)NNP_TRI_LEN));
+    {
+        std::vector<uint16_t> tri(NNP_TRI_LEN);
+        nnp_aev_tri_table(tri.data());
+        TRYCU(cudaMemcpy(c->d_tri, tri.data(), sizeof(uint16_t) * NNP_TRI_LEN, cudaMemcpyHostToDevice));
+    }
     TRYCU(cudaMemcpy(c->d_params_blob, blob.data(), sizeof(float) * total, cudaMemcpyHostToDevice));
     for (size_t q = 0; q < (size_t)c->n_nets * S * NNP_NLAYERS; ++q) { // offsets -> device pointers
         LayerW &L = c->layers[q];
@@ -498,7 +591,11 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
     }
     c->bucket_off[0] = 0;
     for (int s = 0; s < NNP_MAX_SPECIES; ++s) c->bucket_off[s + 1] = c->bucket_off[s] + (s < c->S ? h_counts[s] : 0);
-    return NNP_OK;
+    unsigned mask = 0;
+    for (int s = 0; s < c->S; ++s)
+        if (h_counts[s] > 0) mask |= 1u << s;
+    if (c->dense_aev || mask == 0) mask = (1u << c->S) - 1u;
+    return set_layout(c, mask);
 }
 
 int nnp_set_positions(nnp_ctx *c, const float *d_xyz)
@@ -570,7 +667,7 @@ int nnp_get_aev(nnp_ctx *c, float *d_aev)
     if (!c->have_lists || !d_aev) NNP_FAIL(c, NNP_ESTALE, "no neighbour list / null argument");
     if (c->n == 0) return NNP_OK;
     nnp_launch_aev_forward(c); // G may have been overwritten by dE/dG: recompute
-    k_get_aev<<<c->n, 128, 0, c->stream>>>(c->n, c->aev.aev_len, c->aev.kpad, c->G, c->orig, d_aev);
+    k_get_aev<<<c->n, 128, 0, c->stream>>>(c->n, c->aev_len_full, c->aev.aev_len, c->aev.kpad, c->G, c->d_fmap, c->orig, d_aev);
     c->launches += 1;
     c->have_forces = 0;
     CU(c, cudaGetLastError());

@@ -14,6 +14,7 @@
 #define NNP_NSHF_Z 4
 #define NNP_ANG_BLOCK (NNP_NSHF_A * NNP_NSHF_Z) /* 32 features per species pair */
 #define NNP_NLAYERS 4
+#define NNP_TRI_LEN 2016 /* pairs (lo < hi) with hi < 64: decode table of the AEV kernels */
 
 // Device error flags latched by kernels, reported by synchronising calls.
 enum { NNP_FLAG_CAP_R = 1, NNP_FLAG_CAP_A = 2 };
@@ -29,11 +30,18 @@ struct GridInfo {
 };
 
 // ---- AEV constants (stage 2/4), passed to kernels by value --------------------------------------
+// Columns of G: only the feature blocks of species PRESENT in the loaded system are stored ("active columns":
+// np*16 radial + np(np+1)/2*32 angular); blocks of absent species are identically zero for every atom, so
+// dropping them (and the matching rows of the layer-1 weights) changes no result.  cmap/plist translate between
+// model species and the compact index; with dense_aev (or all species present) the layout is the full one.
 struct AevParams {
-    int S;           // species
-    int n_rad;       // S*16
-    int aev_len;     // n_rad + S(S+1)/2*32
-    int kpad;        // row stride of G / dG in floats (aev_len rounded up to 32 -> 1024)
+    int S;           // species of the model
+    int np;          // species present in the loaded system (compact index 0..np-1, ascending species)
+    int cmap[NNP_MAX_SPECIES];  // species -> compact index, -1 if absent
+    int plist[NNP_MAX_SPECIES]; // compact index -> species
+    int n_rad;       // np*16
+    int aev_len;     // n_rad + np(np+1)/2*32 (active columns)
+    int kpad;        // row stride of G / dG in floats (aev_len rounded up to 32)
     int cap_r, cap_a;
     float rcr, rca;
     float rcr2, rca2;
@@ -44,6 +52,10 @@ struct AevParams {
     float shf_r[NNP_NSHF_R];
     float shf_a[NNP_NSHF_A];
     float cos_z[NNP_NSHF_Z], sin_z[NNP_NSHF_Z];
+    float ka;                   // sqrt(eta_a log2 e): exp(-eta_a u^2) = 2^-(ka u)^2
+    float ka_shf[NNP_NSHF_A];   // ka * shf_a
+    float kr;                   // sqrt(eta_r log2 e)
+    float kr_shf[NNP_NSHF_R];   // kr * shf_r
     int periodic;
     float box[3], inv_box[3];
 };
@@ -84,10 +96,20 @@ struct LayerW {
     float *W_hi, *W_lo, *Wt_hi, *Wt_lo; // tf32 splits (tensor-core modes only)
     int in, in_pad, out;
 };
+// layer 1 restricted to the active columns of the loaded system (built by nnp_set_system)
+struct Layer1C {
+    float *W, *Wt, *W_hi, *W_lo, *Wt_hi, *Wt_lo; // [kpad][out] / [out][kpad]
+};
 
 struct nnp_ctx {
     // model
-    int S, n_nets, mm_mode;
+    int S, n_nets, mm_mode, dense_aev;
+    int aev_len_full, kpad_full;    // 1008 / 1024 for 7 species
+    unsigned present_mask;          // species mask the compact layer-1 copies were built for (0: none yet)
+    Layer1C *l1c;                   // host array [n_nets][S]
+    float *d_l1c_blob;              // device storage of the compact layer-1 copies (sized for the full layout)
+    int *d_fmap;                    // [kpad_full] compact column -> full column (-1: zero padding)
+    uint16_t *d_tri;                // [NNP_TRI_LEN] pair decode table (aev.cu)
     int widths[NNP_MAX_SPECIES][NNP_NLAYERS + 1];
     int hmax[3]; // max hidden widths over species (strides of the activation buffers)
     AevParams aev;
@@ -152,6 +174,7 @@ int nnp_launch_build(nnp_ctx *c, const int *cond_flag); // sort + lists; cond_fl
 // aev.cu
 void nnp_launch_aev_forward(nnp_ctx *c);
 void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets);
+void nnp_aev_tri_table(uint16_t *h_tri /* [NNP_TRI_LEN] */);
 // mlp_simt.cu / mlp_tc.cu
 void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi);
 int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3);

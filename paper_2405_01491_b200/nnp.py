@@ -22,7 +22,7 @@ EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp
            "nnp_build_neighbors", "nnp_get_neighbors", "nnp_energy_forces", "nnp_get_aev",
            "nnp_get_atomic_energies", "nnp_md_init", "nnp_md_step", "nnp_get_state", "nnp_sync",
            "nnp_energy_forces_host", "nnp_md_step_host", "nnp_profile", "nnp_profile_read", "nnp_launch_count",
-           "nnp_aev_len"]
+           "nnp_aev_len", "nnp_aev_active_columns"]
 
 
 class NnpError(RuntimeError):
@@ -41,6 +41,7 @@ class nnp_params(C.Structure):
         ("widths", C.POINTER(C.c_int)), ("params", C.POINTER(C.c_float)),
         ("self_energy", C.POINTER(C.c_float)), ("mass", C.POINTER(C.c_float)),
         ("accel_conv", C.c_float), ("mm_mode", C.c_int), ("cap_r", C.c_int), ("cap_a", C.c_int),
+        ("dense_aev", C.c_int),
     ]
 
 
@@ -78,6 +79,7 @@ def lib():
         L.nnp_launch_count.argtypes = [vp]
         L.nnp_launch_count.restype = C.c_int64
         L.nnp_aev_len.argtypes = [vp]
+        L.nnp_aev_active_columns.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -100,7 +102,7 @@ def _check(ctx, rc):
 
 
 def make_params(consts, widths, params, mass, accel_conv, n_nets=1, self_energy=None, mm_mode=NNP_MM_FP32_SIMT,
-                cap_r=0, cap_a=0):
+                cap_r=0, cap_a=0, dense_aev=0):
     """Fills an nnp_params from numpy arrays; returns (struct, keepalive list)."""
     f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
     keep = dict(shf_r=f32(consts["shf_r"]), shf_a=f32(consts["shf_a"]), shf_z=f32(consts["shf_z"]),
@@ -121,6 +123,7 @@ def make_params(consts, widths, params, mass, accel_conv, n_nets=1, self_energy=
     p.self_energy = fp(keep["self_energy"]) if keep["self_energy"] is not None else None
     p.mass = fp(keep["mass"])
     p.accel_conv, p.mm_mode, p.cap_r, p.cap_a = float(accel_conv), int(mm_mode), int(cap_r), int(cap_a)
+    p.dense_aev = int(dense_aev)
     return p, keep
 
 
@@ -220,3 +223,7 @@ def nnp_launch_count(ctx):
 
 def nnp_aev_len(ctx):
     return int(lib().nnp_aev_len(ctx))
+
+
+def nnp_aev_active_columns(ctx):
+    return int(lib().nnp_aev_active_columns(ctx))
