@@ -3,17 +3,23 @@
 // (0.5+0.5cos(theta-theta_n))^zeta, L55 pairs of edges with a common centre, L65/L176 forces by reverse mode).
 //
 // Persistent warps, one centre atom per warp at a time.  Neighbour rows are grouped by neighbour species (stage 1).
-//   radial:  lane = neighbour, 16 Gaussians in registers per species segment, butterfly reduction over lanes.
+//   loads:   the species-segment table of the NEXT centre is fetched one centre ahead; for the current centre all
+//            neighbour indices (radial trips + angular chunks) are loaded first, then all their positions, so one
+//            centre costs one index->position latency chain instead of one per loop trip.
+//   radial:  the 32 lanes are split among the species segments of the radial row in proportion to their lengths
+//            (every lane serves one species, so its 16 Gaussian accumulators belong to one species); the lanes'
+//            accumulators are transposed through shared memory and summed per species.
 //   angular: the in-cutoff neighbours are compacted into shared memory (dx,dy,dz,r | fc,1/r | fc'), still grouped
-//            by species.  The pairs (j,k) of ALL species-pair blocks are then processed in one loop: the 32 lanes
-//            are split among the non-empty blocks in proportion to their pair counts (every lane serves one
-//            block, so its 8x4 accumulators belong to one block), which takes ceil(pairs/32)+~0 trips instead of
-//            one ragged loop per block.  The lanes' accumulators are transposed through shared memory and the
-//            rows of each block summed by lane = feature -> one coalesced 128 B store per block.  Triplets are
-//            enumerated on the fly and never stored (the paper's GraphAngularExtension stores them, L55).
+//            by species.  The pairs (j,k) of ALL species-pair blocks are processed in one loop: the lanes are split
+//            among the non-empty blocks in proportion to their pair counts (one block per lane: its 8x4
+//            accumulators belong to one block), which takes ~ceil(pairs/32) trips instead of one ragged loop per
+//            block.  Accumulators go through the same shared-memory transpose; lane = feature sums the rows of
+//            each block -> one coalesced 128 B store per block.  Triplets are enumerated on the fly and never
+//            stored (the paper's GraphAngularExtension stores them, L55).
 //   reverse: per pair only three scalars (alpha_j, alpha_k, beta with dE/dd_ij = alpha_j d_ij + beta d_ik) are
-//            parked in a per-warp shared-memory arena; a second pass with lane = neighbour sums them into the
-//            neighbour forces without atomics; one 16-byte vector reduction per neighbour goes to global.
+//            parked in two per-warp na x na shared-memory matrices; a second pass with lane = neighbour sums its
+//            row into the neighbour force without atomics; one 16-byte vector reduction per neighbour goes to
+//            global memory.
 // cos(theta' - ShfZ) with theta' = acos(0.95 cos theta) is expanded as c' cos ShfZ + sqrt(1-c'^2) sin ShfZ: no acos;
 // |c'| <= 0.95 keeps sqrt(1-c'^2) >= 0.31 and (1+cos(theta'-ShfZ))/2 >= 0.1, so neither needs a clamp.
 // Columns of G are the active ones of the loaded system (AevParams::cmap / plist, nnp_internal.cuh).
@@ -21,10 +27,19 @@
 
 namespace {
 
+#ifndef AEV_FWD_MINB
+#define AEV_FWD_MINB 6
+#endif
+#ifndef AEV_BWD_MINB
+#define AEV_BWD_MINB 5
+#endif
 constexpr int kWarps = 4;
 constexpr int kCapA = 64;        // shared-memory slots for in-cutoff angular neighbours per centre
-constexpr int kArena = 528;      // pair records per warp: covers n <= 33 in-cutoff neighbours (528 pairs)
+constexpr int kMat = 32;         // reverse pass: pair matrices cover na <= 32 in-cutoff neighbours, beyond: atomics
+constexpr int kMatLd = 33;
 constexpr int kRedLd = 36;       // row stride of the transpose buffer (conflict-free 16-byte rows / 4-byte columns)
+constexpr int KR = 3;            // radial trips whose loads are issued up front (3 x 32 lanes >= typical row)
+constexpr int KA = 2;            // angular chunks of 32 loaded up front (cap_a = 64)
 constexpr unsigned kFull = 0xffffffffu;
 static_assert(kCapA * (kCapA - 1) / 2 == NNP_TRI_LEN, "pair decode table length");
 
@@ -42,8 +57,9 @@ struct WarpSmemBwd {
     int j[kCapA];
     int seg[NNP_MAX_SPECIES + 1];
     int own[32];
-    float alo[kArena], ahi[kArena], bet[kArena]; // pair (a<b): alpha of a, alpha of b, beta
-};                                               // fallback path (more pairs than kArena): f[kCapA][3] aliases alo
+    float alp[kMat * kMatLd]; // alp[a][b]: alpha of a in pair (a,b); fallback path: f[kCapA][3] aliases it
+    float bet[kMat * kMatLd]; // bet[a][b] = bet[b][a]
+};
 
 __device__ __forceinline__ float ex2(float x)
 {
@@ -75,79 +91,6 @@ __device__ __forceinline__ float3 min_image(const float4 a, const float4 b, cons
     return make_float3(dx, dy, dz);
 }
 
-// Sum v[0..16) over the 32 lanes; afterwards lane l holds in v[0] the total of element (l >> 1).
-__device__ __forceinline__ void butterfly_reduce16(float (&v)[16], int lane)
-{
-    int w = 16;
-#pragma unroll
-    for (int m = 8; m >= 1; m >>= 1, w >>= 1) {
-        const bool upper = lane & w;
-#pragma unroll
-        for (int q = 0; q < m; ++q) {
-            float send = upper ? v[q] : v[q + m];
-            float keep = upper ? v[q + m] : v[q];
-            v[q] = keep + __shfl_xor_sync(kFull, send, w);
-        }
-    }
-    v[0] += __shfl_xor_sync(kFull, v[0], 1);
-}
-
-// Compacts the angular neighbours with r < rca into shared memory, keeping the species grouping (compact species
-// index).  Returns the count.
-template <bool BWD, class SM>
-__device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, int i, int lane, const float4 pi,
-                                             const float4 *__restrict__ pos, const int *__restrict__ nbr_a,
-                                             const uint16_t *__restrict__ seg_a, int *__restrict__ flags)
-{
-    const uint16_t *sg = seg_a + (size_t)i * NNP_MAX_SPECIES;
-    const int *row = nbr_a + (size_t)i * P.cap_a;
-    const unsigned lt = (1u << lane) - 1u;
-    int na = 0;
-    for (int cs = 0; cs < P.np; ++cs) {
-        const int s = P.plist[cs];
-        if (lane == 0) sm.seg[cs] = na;
-        const int a_beg = sg[s], a_end = sg[s + 1];
-        for (int a0 = a_beg; a0 < a_end; a0 += 32) {
-            const int a = a0 + lane;
-            bool hit = false;
-            float3 d = make_float3(0.f, 0.f, 0.f);
-            float r2 = 0.f;
-            int j = 0;
-            if (a < a_end) {
-                j = row[a];
-                d = min_image(pi, pos[j], P);
-                r2 = d.x * d.x + d.y * d.y + d.z * d.z;
-                hit = r2 < P.rca2;
-            }
-            const unsigned m = __ballot_sync(kFull, hit);
-            if (hit) {
-                const int p = na + __popc(m & lt);
-                if (p < kCapA) {
-                    const float rinv = rsq(r2);
-                    const float r = r2 * rinv;
-                    float sn, cs_;
-                    __sincosf(P.pi_rca * r, &sn, &cs_);
-                    sm.d[p] = make_float4(d.x, d.y, d.z, r);
-                    sm.fr[p] = make_float2(0.5f * cs_ + 0.5f, rinv);
-                    if constexpr (BWD) {
-                        sm.dfc[p] = -0.5f * P.pi_rca * sn;
-                        sm.j[p] = j;
-                    }
-                }
-            }
-            na += __popc(m);
-            if (na > kCapA) { // more in-cutoff angular neighbours than shared-memory slots
-                if (lane == 0) atomicOr(&flags[0], NNP_FLAG_CAP_A);
-                na = kCapA;
-            }
-        }
-    }
-    if (lane == 0)
-        for (int cs = P.np; cs <= NNP_MAX_SPECIES; ++cs) sm.seg[cs] = na;
-    __syncwarp();
-    return na;
-}
-
 // Species-pair block (compact indices cs <= ct) served by lane b < np(np+1)/2 when it acts as "block lane".
 __device__ __forceinline__ void block_of_lane(int np, int lane, int &bcs, int &bct)
 {
@@ -159,24 +102,20 @@ __device__ __forceinline__ void block_of_lane(int np, int lane, int &bcs, int &b
     }
 }
 
-// Lane partition for one centre: block lane b holds n_b pairs; finds the smallest trip count I with
-// sum_b ceil(n_b / I) <= 32, gives block b the lanes [beg_b, beg_b + L_b), L_b = ceil(n_b / I).
+// Lane partition: "block lane" b holds a work list of n_b items (0 for lanes that own no block) and a tag.
+// Finds the smallest trip count I with sum_b ceil(n_b / I) <= 32 and gives block b the worker lanes
+// [beg_b, beg_b + L_b), L_b = ceil(n_b / I).  Worker r of a block takes items r, r + L, r + 2L, ...
 struct LanePart {
-    int I;          // trips (warp-uniform); 0: no pairs at all
+    int I;          // trips (warp-uniform); 0: nothing to do
     int beg_b, L_b; // as block lane
-    int cs, ct;     // block served by this lane as worker
-    int r, L;       // rank inside the block's lane group and its size; active iff r < L
+    int tag;        // as worker: tag of the block served
+    int r, L;       // as worker: rank inside the block's lane group and its size; active iff r < L
 };
-__device__ __forceinline__ LanePart partition(const int *seg, int *own, int np, int lane, int bcs, int bct)
+__device__ __forceinline__ LanePart partition(int n_b, int tag_b, int *own, int lane)
 {
     LanePart pt;
-    int n_b = 0;
-    if (lane < np * (np + 1) / 2) {
-        const int ns = seg[bcs + 1] - seg[bcs], nt = seg[bct + 1] - seg[bct];
-        n_b = bcs == bct ? ns * (ns - 1) / 2 : ns * nt;
-    }
+    pt.I = 0; pt.beg_b = 0; pt.L_b = 0; pt.tag = 0; pt.r = 0; pt.L = 0;
     const int N = __reduce_add_sync(kFull, n_b);
-    pt.I = 0; pt.beg_b = 0; pt.L_b = 0; pt.cs = 0; pt.ct = 0; pt.r = 0; pt.L = 0;
     if (N == 0) return pt;
     int I = (N + 31) >> 5, L_b;
     for (;;) {
@@ -193,14 +132,14 @@ __device__ __forceinline__ LanePart partition(const int *seg, int *own, int np, 
     }
     const int beg_b = x - L_b;
     const unsigned starts = __reduce_or_sync(kFull, L_b > 0 ? (1u << beg_b) : 0u);
-    if (L_b > 0) own[beg_b] = bcs | (bct << 3) | (L_b << 6) | (beg_b << 12);
+    if (L_b > 0) own[beg_b] = tag_b | (L_b << 8) | (beg_b << 16);
     __syncwarp();
     const int p = 31 - __clz(starts & (kFull >> (31 - lane))); // first lane of this lane's group (bit 0 is always set)
     const int w = own[p];
     __syncwarp();
     pt.I = I; pt.beg_b = beg_b; pt.L_b = L_b;
-    pt.cs = w & 7; pt.ct = (w >> 3) & 7; pt.L = (w >> 6) & 63;
-    pt.r = lane - ((w >> 12) & 31);
+    pt.tag = w & 0xff; pt.L = (w >> 8) & 0xff;
+    pt.r = lane - (w >> 16);
     return pt;
 }
 
@@ -218,7 +157,108 @@ __device__ __forceinline__ void decode_pair(int q, bool same, int nt, float inv_
     }
 }
 
-__global__ void __launch_bounds__(kWarps * 32)
+// Everything both kernels do before their arithmetic: lane roles, the segment tables (one centre ahead), the
+// radial lane partition, and the batched index / position loads of the current centre.
+struct Centre {
+    float4 pi;
+    LanePart pr;          // radial partition (tag = compact species of this worker lane)
+    int wa_beg, wa_end;   // this worker's species segment in the radial row
+    int jr[KR];           // radial neighbours of the first KR trips (-1: none)
+    float4 xr[KR];
+    int ja[KA];           // angular row entries lane + 32 k (-1: none)
+    float4 xa[KA];
+    int len_a;            // angular row length
+    int ab_beg;           // as block lane cs < np: start of the species segment in the angular row
+};
+
+__device__ __forceinline__ void load_centre(Centre &c, const AevParams &P, int i, int lane, int my_s, int sgr_l, int sga_l,
+                                            const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
+                                            const int *__restrict__ nbr_a, int *own)
+{
+    c.pi = pos[i];
+    const int rb_beg = __shfl_sync(kFull, sgr_l, my_s), rb_end = __shfl_sync(kFull, sgr_l, my_s + 1);
+    c.ab_beg = __shfl_sync(kFull, sga_l, my_s);
+    c.len_a = __shfl_sync(kFull, sga_l, NNP_MAX_SPECIES - 1);
+    c.pr = partition(lane < P.np ? rb_end - rb_beg : 0, lane, own, lane);
+    c.wa_beg = __shfl_sync(kFull, rb_beg, c.pr.tag);
+    c.wa_end = __shfl_sync(kFull, rb_end, c.pr.tag);
+    const int *row_r = nbr_r + (size_t)i * P.cap_r;
+    const int *row_a = nbr_a + (size_t)i * P.cap_a;
+#pragma unroll
+    for (int t = 0; t < KR; ++t) {
+        const int a = c.wa_beg + c.pr.r + t * c.pr.L;
+        c.jr[t] = (c.pr.r < c.pr.L && a < c.wa_end) ? row_r[a] : -1;
+    }
+#pragma unroll
+    for (int k = 0; k < KA; ++k) {
+        const int a = lane + 32 * k;
+        c.ja[k] = a < c.len_a ? row_a[a] : -1;
+    }
+#pragma unroll
+    for (int t = 0; t < KR; ++t) c.xr[t] = c.jr[t] >= 0 ? pos[c.jr[t]] : c.pi;
+#pragma unroll
+    for (int k = 0; k < KA; ++k) c.xa[k] = c.ja[k] >= 0 ? pos[c.ja[k]] : c.pi;
+}
+
+// Compacts the angular row entries with r < rca into shared memory in row order (= grouped by species); block lane
+// cs < np counts the hits in front of its species segment -> seg[].  Returns the count.
+template <bool BWD, class SM>
+__device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const Centre &c, int i, int lane,
+                                             const float4 *__restrict__ pos, const int *__restrict__ nbr_a,
+                                             int *__restrict__ flags)
+{
+    const unsigned lt = (1u << lane) - 1u;
+    int na = 0, segc = 0;
+    auto chunk = [&](int k, int j, const float4 xj) {
+        bool hit = false;
+        float3 d = make_float3(0.f, 0.f, 0.f);
+        float r2 = 1.f;
+        if (j >= 0) {
+            d = min_image(c.pi, xj, P);
+            r2 = d.x * d.x + d.y * d.y + d.z * d.z;
+            hit = r2 < P.rca2;
+        }
+        const unsigned m = __ballot_sync(kFull, hit);
+        if (hit) {
+            const int p = na + __popc(m & lt);
+            if (p < kCapA) {
+                const float rinv = rsq(r2);
+                const float r = r2 * rinv;
+                float sn, cs_;
+                __sincosf(P.pi_rca * r, &sn, &cs_);
+                sm.d[p] = make_float4(d.x, d.y, d.z, r);
+                sm.fr[p] = make_float2(0.5f * cs_ + 0.5f, rinv);
+                if constexpr (BWD) {
+                    sm.dfc[p] = -0.5f * P.pi_rca * sn;
+                    sm.j[p] = j;
+                }
+            }
+        }
+        const int bound = c.ab_beg - 32 * k; // entries of this chunk in front of my species segment
+        const unsigned below = bound >= 32 ? kFull : (bound <= 0 ? 0u : ((1u << bound) - 1u));
+        segc += __popc(m & below);
+        na += __popc(m);
+    };
+#pragma unroll
+    for (int k = 0; k < KA; ++k) chunk(k, c.ja[k], c.xa[k]);
+    if (c.len_a > 32 * KA) { // rows longer than the prefetched chunks (cap_a > 64)
+        const int *row = nbr_a + (size_t)i * P.cap_a;
+        for (int k = KA; 32 * k < c.len_a; ++k) {
+            const int a = lane + 32 * k;
+            const int j = a < c.len_a ? row[a] : -1;
+            chunk(k, j, j >= 0 ? pos[j] : c.pi);
+        }
+    }
+    if (na > kCapA) { // more in-cutoff angular neighbours than shared-memory slots
+        if (lane == 0) atomicOr(&flags[0], NNP_FLAG_CAP_A);
+        na = kCapA;
+    }
+    if (lane <= NNP_MAX_SPECIES) sm.seg[lane] = lane < P.np ? min(segc, kCapA) : na;
+    __syncwarp();
+    return na;
+}
+
+__global__ void __launch_bounds__(kWarps * 32, AEV_FWD_MINB)
 k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
               const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
               const uint16_t *__restrict__ seg_a, const uint16_t *__restrict__ tri, float *__restrict__ G,
@@ -230,61 +270,100 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
     int bcs, bct;
     block_of_lane(P.np, lane, bcs, bct);
     const int nb_tot = P.np * (P.np + 1) / 2;
+    int my_s = 0;
+#pragma unroll
+    for (int q = 0; q < NNP_MAX_SPECIES - 1; ++q)
+        if (lane == q && q < P.np) my_s = P.plist[q];
     float hcz[NNP_NSHF_Z], hsz[NNP_NSHF_Z];
 #pragma unroll
     for (int z = 0; z < NNP_NSHF_Z; ++z) { hcz[z] = 0.5f * P.cos_z[z]; hsz[z] = 0.5f * P.sin_z[z]; }
 
-    for (int i = blockIdx.x * kWarps + wid; i < n; i += gridDim.x * kWarps) {
-        const float4 pi = pos[i];
+    const int stride = gridDim.x * kWarps;
+    int i = blockIdx.x * kWarps + wid;
+    int sgr_l = 0, sga_l = 0;
+    if (i < n && lane < NNP_MAX_SPECIES) {
+        sgr_l = seg_r[(size_t)i * NNP_MAX_SPECIES + lane];
+        sga_l = seg_a[(size_t)i * NNP_MAX_SPECIES + lane];
+    }
+    for (; i < n; i += stride) {
+        int sgr_n = 0, sga_n = 0; // segment tables of the next centre
+        if (i + stride < n && lane < NNP_MAX_SPECIES) {
+            sgr_n = seg_r[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
+            sga_n = seg_a[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
+        }
+        Centre c;
+        load_centre(c, P, i, lane, my_s, sgr_l, sga_l, pos, nbr_r, nbr_a, sm.own);
         float *Grow = G + (size_t)i * P.kpad;
 
         // ---- radial block: G[cs*16+k] = 1/4 sum_j exp(-eta_r (r-ShfR_k)^2) fc(r)
         {
-            const uint16_t *sg = seg_r + (size_t)i * NNP_MAX_SPECIES; // sg[S..7] = row length (S <= 7)
-            const int *row = nbr_r + (size_t)i * P.cap_r;
-            for (int cs = 0; cs < P.np; ++cs) {
-                const int s = P.plist[cs];
-                const int a_beg = sg[s], a_end = sg[s + 1];
-                if (a_end == a_beg) {
-                    if (lane < NNP_NSHF_R) Grow[cs * NNP_NSHF_R + lane] = 0.f;
-                    continue;
-                }
-                float acc[NNP_NSHF_R];
+            float acc[NNP_NSHF_R];
 #pragma unroll
-                for (int k = 0; k < NNP_NSHF_R; ++k) acc[k] = 0.f;
-                for (int a = a_beg + lane; a < a_end; a += 32) {
-                    const float3 d = min_image(pi, pos[row[a]], P);
-                    const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
-                    if (r2 < P.rcr2) {
-                        const float r = r2 * rsq(r2);
-                        const float fc = 0.125f * __cosf(P.pi_rcr * r) + 0.125f; // (1/4) fc
-                        const float kr_r = P.kr * r;
+            for (int k = 0; k < NNP_NSHF_R; ++k) acc[k] = 0.f;
+            auto term = [&](const float4 xj) {
+                const float3 d = min_image(c.pi, xj, P);
+                const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
+                if (r2 < P.rcr2) {
+                    const float r = r2 * rsq(r2);
+                    const float fc = 0.125f * __cosf(P.pi_rcr * r) + 0.125f; // (1/4) fc
 #pragma unroll
-                        for (int k = 0; k < NNP_NSHF_R; ++k) {
-                            const float w = kr_r - P.kr_shf[k];
-                            acc[k] = fmaf(fc, ex2(-w * w), acc[k]);
-                        }
+                    for (int k = 0; k < NNP_NSHF_R; ++k) {
+                        const float w = fmaf(P.kr, r, -P.kr_shf[k]);
+                        acc[k] = fmaf(fc, ex2(-w * w), acc[k]);
                     }
                 }
-                butterfly_reduce16(acc, lane);
-                if ((lane & 1) == 0) Grow[cs * NNP_NSHF_R + (lane >> 1)] = acc[0];
+            };
+#pragma unroll
+            for (int t = 0; t < KR; ++t)
+                if (c.jr[t] >= 0) term(c.xr[t]);
+            if (c.pr.I > KR) {
+                const int *row = nbr_r + (size_t)i * P.cap_r;
+                for (int t = KR; t < c.pr.I; ++t) {
+                    const int a = c.wa_beg + c.pr.r + t * c.pr.L;
+                    if (c.pr.r < c.pr.L && a < c.wa_end) term(pos[row[a]]);
+                }
+            }
+            if (c.pr.I > 0) {
+                float *myrow = sm.red + lane * kRedLd;
+#pragma unroll
+                for (int q4 = 0; q4 < NNP_NSHF_R / 4; ++q4)
+                    *reinterpret_cast<float4 *>(myrow + 4 * q4) = make_float4(acc[4 * q4], acc[4 * q4 + 1], acc[4 * q4 + 2], acc[4 * q4 + 3]);
+                __syncwarp();
+            }
+            // rows [beg_b, beg_b + L_b) belong to species b; a half warp sums the 16 columns of one species
+            for (int p0 = 0; p0 < P.np; p0 += 2) {
+                const int cs = p0 + (lane >> 4);
+                const int csc = min(cs, P.np - 1);
+                const int beg = __shfl_sync(kFull, c.pr.beg_b, csc);
+                int L = __shfl_sync(kFull, c.pr.L_b, csc);
+                if (cs >= P.np) L = 0;
+                float sum = 0.f;
+                for (int rr = beg; rr < beg + L; ++rr) sum += sm.red[rr * kRedLd + (lane & 15)];
+                if (cs < P.np) Grow[cs * NNP_NSHF_R + (lane & 15)] = sum;
             }
             for (int q = P.aev_len + lane; q < P.kpad; q += 32) Grow[q] = 0.f; // zero padding columns
+            __syncwarp();
         }
 
         // ---- angular block
-        stage_angular<false>(sm, P, i, lane, pi, pos, nbr_a, seg_a, flags);
-        const LanePart pt = partition(sm.seg, sm.own, P.np, lane, bcs, bct);
-        float acc[NNP_ANG_BLOCK];
-#pragma unroll
-        for (int q = 0; q < NNP_ANG_BLOCK; ++q) acc[q] = 0.f;
+        stage_angular<false>(sm, P, c, i, lane, pos, nbr_a, flags);
+        int n_b = 0;
+        if (lane < nb_tot) {
+            const int ns = sm.seg[bcs + 1] - sm.seg[bcs], nt = sm.seg[bct + 1] - sm.seg[bct];
+            n_b = bcs == bct ? ns * (ns - 1) / 2 : ns * nt;
+        }
+        const LanePart pt = partition(n_b, bcs | (bct << 3), sm.own, lane);
         if (pt.I > 0) {
-            const int a0 = sm.seg[pt.cs], b0 = sm.seg[pt.ct];
-            const int nt = sm.seg[pt.ct + 1] - b0;
-            const bool same = pt.cs == pt.ct;
+            float acc[NNP_ANG_BLOCK];
+#pragma unroll
+            for (int q = 0; q < NNP_ANG_BLOCK; ++q) acc[q] = 0.f;
+            const int wcs = pt.tag & 7, wct = pt.tag >> 3;
+            const int a0 = sm.seg[wcs], b0 = sm.seg[wct];
+            const int nt = sm.seg[wct + 1] - b0;
+            const bool same = wcs == wct;
             int npairs = 0;
             if (pt.r < pt.L) {
-                const int ns = sm.seg[pt.cs + 1] - a0;
+                const int ns = sm.seg[wcs + 1] - a0;
                 npairs = same ? ns * (ns - 1) / 2 : ns * nt;
             }
             const float inv_nt = __frcp_rn((float)max(nt, 1));
@@ -295,19 +374,19 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 const float4 dj = sm.d[ia], dk = sm.d[ib];
                 const float2 fj = sm.fr[ia], fk = sm.fr[ib];
                 const float ff = 2.0f * fj.x * fk.x;
-                const float c = (0.95f * fj.y * fk.y) * (dj.x * dk.x + dj.y * dk.y + dj.z * dk.z);
-                const float s2 = fmaf(-c, c, 1.0f);
+                const float cc = (0.95f * fj.y * fk.y) * (dj.x * dk.x + dj.y * dk.y + dj.z * dk.z);
+                const float s2 = fmaf(-cc, cc, 1.0f);
                 const float sn = s2 * rsq(s2);
-                const float krb = (0.5f * P.ka) * (dj.w + dk.w);
+                const float rjk = dj.w + dk.w;
                 float fz[NNP_NSHF_Z];
 #pragma unroll
                 for (int z = 0; z < NNP_NSHF_Z; ++z) {
-                    const float base = fmaf(c, hcz[z], fmaf(sn, hsz[z], 0.5f));
+                    const float base = fmaf(cc, hcz[z], fmaf(sn, hsz[z], 0.5f));
                     fz[z] = ff * ex2(P.zeta * lg2(base));
                 }
 #pragma unroll
                 for (int a = 0; a < NNP_NSHF_A; ++a) {
-                    const float w = krb - P.ka_shf[a];
+                    const float w = fmaf(0.5f * P.ka, rjk, -P.ka_shf[a]);
                     const float ra = ex2(-w * w);
 #pragma unroll
                     for (int z = 0; z < NNP_NSHF_Z; ++z) acc[a * NNP_NSHF_Z + z] = fmaf(ra, fz[z], acc[a * NNP_NSHF_Z + z]);
@@ -322,16 +401,22 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
         // rows [beg_b, beg_b + L_b) of the transpose buffer belong to block b; lane = feature inside the block
         for (int p = 0; p < nb_tot; ++p) {
             const int beg = __shfl_sync(kFull, pt.beg_b, p), L = __shfl_sync(kFull, pt.L_b, p);
-            float sum = 0.f;
-            for (int rr = beg; rr < beg + L; ++rr) sum += sm.red[rr * kRedLd + lane];
-            Grow[P.n_rad + p * NNP_ANG_BLOCK + lane] = sum;
+            float s0 = 0.f, s1 = 0.f;
+            int rr = beg;
+            for (; rr + 1 < beg + L; rr += 2) {
+                s0 += sm.red[rr * kRedLd + lane];
+                s1 += sm.red[(rr + 1) * kRedLd + lane];
+            }
+            if (rr < beg + L) s0 += sm.red[rr * kRedLd + lane];
+            Grow[P.n_rad + p * NNP_ANG_BLOCK + lane] = s0 + s1;
         }
         __syncwarp();
+        sgr_l = sgr_n; sga_l = sga_n;
     }
 }
 
 // Reverse pass: g = dE/dG_i (row of dG, times inv_nets).  Adds -dE/dx to frc for the centre and its neighbours.
-__global__ void __launch_bounds__(kWarps * 32)
+__global__ void __launch_bounds__(kWarps * 32, AEV_BWD_MINB)
 k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
                const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
                const uint16_t *__restrict__ seg_a, const uint16_t *__restrict__ tri, const float *__restrict__ dG,
@@ -343,6 +428,11 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     WarpSmemBwd &sm = smem[wid];
     int bcs, bct;
     block_of_lane(P.np, lane, bcs, bct);
+    const int nb_tot = P.np * (P.np + 1) / 2;
+    int my_s = 0;
+#pragma unroll
+    for (int q = 0; q < NNP_MAX_SPECIES - 1; ++q)
+        if (lane == q && q < P.np) my_s = P.plist[q];
     float hcz[NNP_NSHF_Z], hsz[NNP_NSHF_Z];
 #pragma unroll
     for (int z = 0; z < NNP_NSHF_Z; ++z) { hcz[z] = 0.5f * P.cos_z[z]; hsz[z] = 0.5f * P.sin_z[z]; }
@@ -351,78 +441,101 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     // d/drb exp(-eta (rb - s)^2) = -2 eta (rb - s) ra = (-2 eta / ka) w ra with w = ka (rb - s)
     const float drb_scale = -2.0f * P.eta_a / P.ka;
     const float dr_scale = -2.0f * P.eta_r / P.kr;
-    float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.alo);
+    float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.alp);
 
-    for (int i = blockIdx.x * kWarps + wid; i < n; i += gridDim.x * kWarps) {
-        const float4 pi = pos[i];
+    const int stride = gridDim.x * kWarps;
+    int i = blockIdx.x * kWarps + wid;
+    int sgr_l = 0, sga_l = 0;
+    if (i < n && lane < NNP_MAX_SPECIES) {
+        sgr_l = seg_r[(size_t)i * NNP_MAX_SPECIES + lane];
+        sga_l = seg_a[(size_t)i * NNP_MAX_SPECIES + lane];
+    }
+    for (; i < n; i += stride) {
+        int sgr_n = 0, sga_n = 0;
+        if (i + stride < n && lane < NNP_MAX_SPECIES) {
+            sgr_n = seg_r[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
+            sga_n = seg_a[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
+        }
+        Centre c;
+        load_centre(c, P, i, lane, my_s, sgr_l, sga_l, pos, nbr_r, nbr_a, sm.own);
         const float *grow = dG + (size_t)i * P.kpad;
         float fi[3] = {0.f, 0.f, 0.f}; // dE/dd summed over this lane's terms (force on i = +sum)
 
         // ---- radial: dE/dr_ij = sum_k g[s_j*16+k] * 1/4 e_k (-2 eta (r-ShfR_k) fc + fc')
-        {
-            const uint16_t *sg = seg_r + (size_t)i * NNP_MAX_SPECIES;
-            const int *row = nbr_r + (size_t)i * P.cap_r;
-            for (int cs = 0; cs < P.np; ++cs) {
-                const int s = P.plist[cs];
-                const int a_beg = sg[s], a_end = sg[s + 1];
-                if (a_end == a_beg) continue;
-                float gr[NNP_NSHF_R];
-                const float sc0 = 0.25f * inv_nets;
+        if (c.pr.I > 0) {
+            float gr[NNP_NSHF_R];
+            const float sc0 = 0.25f * inv_nets;
 #pragma unroll
-                for (int k4 = 0; k4 < NNP_NSHF_R / 4; ++k4) {
-                    const float4 v = *reinterpret_cast<const float4 *>(grow + cs * NNP_NSHF_R + 4 * k4);
-                    gr[4 * k4] = v.x * sc0; gr[4 * k4 + 1] = v.y * sc0;
-                    gr[4 * k4 + 2] = v.z * sc0; gr[4 * k4 + 3] = v.w * sc0;
-                }
-                for (int a = a_beg + lane; a < a_end; a += 32) {
-                    const int j = row[a];
-                    const float3 d = min_image(pi, pos[j], P);
-                    const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
-                    if (r2 < P.rcr2) {
-                        const float rinv = rsq(r2);
-                        const float r = r2 * rinv;
-                        float sn, cs_;
-                        __sincosf(P.pi_rcr * r, &sn, &cs_);
-                        const float fc = (0.5f * cs_ + 0.5f) * dr_scale;
-                        const float dfc = -0.5f * P.pi_rcr * sn;
-                        const float kr_r = P.kr * r;
-                        float dEdr = 0.f;
+            for (int k4 = 0; k4 < NNP_NSHF_R / 4; ++k4) {
+                float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (c.pr.r < c.pr.L) v = *reinterpret_cast<const float4 *>(grow + c.pr.tag * NNP_NSHF_R + 4 * k4);
+                gr[4 * k4] = v.x * sc0; gr[4 * k4 + 1] = v.y * sc0;
+                gr[4 * k4 + 2] = v.z * sc0; gr[4 * k4 + 3] = v.w * sc0;
+            }
+            auto term = [&](int j, const float4 xj) {
+                const float3 d = min_image(c.pi, xj, P);
+                const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
+                if (r2 < P.rcr2) {
+                    const float rinv = rsq(r2);
+                    const float r = r2 * rinv;
+                    float sn, cs_;
+                    __sincosf(P.pi_rcr * r, &sn, &cs_);
+                    const float fc = (0.5f * cs_ + 0.5f) * dr_scale;
+                    const float dfc = -0.5f * P.pi_rcr * sn;
+                    float dEdr = 0.f;
 #pragma unroll
-                        for (int k = 0; k < NNP_NSHF_R; ++k) {
-                            const float w = kr_r - P.kr_shf[k];
-                            const float e = ex2(-w * w);
-                            dEdr = fmaf(gr[k] * e, fmaf(w, fc, dfc), dEdr);
-                        }
-                        const float sc = dEdr * rinv;
-                        const float vx = sc * d.x, vy = sc * d.y, vz = sc * d.z;
-                        atomicAdd(&frc[j], make_float4(-vx, -vy, -vz, 0.f));
-                        fi[0] += vx; fi[1] += vy; fi[2] += vz;
+                    for (int k = 0; k < NNP_NSHF_R; ++k) {
+                        const float w = fmaf(P.kr, r, -P.kr_shf[k]);
+                        const float e = ex2(-w * w);
+                        dEdr = fmaf(gr[k] * e, fmaf(w, fc, dfc), dEdr);
                     }
+                    const float sc = dEdr * rinv;
+                    const float vx = sc * d.x, vy = sc * d.y, vz = sc * d.z;
+                    atomicAdd(&frc[j], make_float4(-vx, -vy, -vz, 0.f));
+                    fi[0] += vx; fi[1] += vy; fi[2] += vz;
+                }
+            };
+#pragma unroll
+            for (int t = 0; t < KR; ++t)
+                if (c.jr[t] >= 0) term(c.jr[t], c.xr[t]);
+            if (c.pr.I > KR) {
+                const int *row = nbr_r + (size_t)i * P.cap_r;
+                for (int t = KR; t < c.pr.I; ++t) {
+                    const int a = c.wa_beg + c.pr.r + t * c.pr.L;
+                    if (c.pr.r < c.pr.L && a < c.wa_end) { const int j = row[a]; term(j, pos[j]); }
                 }
             }
         }
 
         // ---- angular
-        const int na = stage_angular<true>(sm, P, i, lane, pi, pos, nbr_a, seg_a, flags);
-        const bool arena = na * (na - 1) / 2 <= kArena; // warp-uniform
-        if (!arena) {
+        const int na = stage_angular<true>(sm, P, c, i, lane, pos, nbr_a, flags);
+        const bool arena = na <= kMat; // warp-uniform
+        if (arena) {
+            if (lane < na) { sm.alp[lane * kMatLd + lane] = 0.f; sm.bet[lane * kMatLd + lane] = 0.f; }
+        } else {
             for (int a = lane; a < na; a += 32) { fsm[a][0] = 0.f; fsm[a][1] = 0.f; fsm[a][2] = 0.f; }
-            __syncwarp();
         }
-        const LanePart pt = partition(sm.seg, sm.own, P.np, lane, bcs, bct);
+        __syncwarp();
+        int n_b = 0;
+        if (lane < nb_tot) {
+            const int ns = sm.seg[bcs + 1] - sm.seg[bcs], nt = sm.seg[bct + 1] - sm.seg[bct];
+            n_b = bcs == bct ? ns * (ns - 1) / 2 : ns * nt;
+        }
+        const LanePart pt = partition(n_b, bcs | (bct << 3), sm.own, lane);
         if (pt.I > 0) {
-            const int a0 = sm.seg[pt.cs], b0 = sm.seg[pt.ct];
-            const int nt = sm.seg[pt.ct + 1] - b0;
-            const bool same = pt.cs == pt.ct;
+            const int wcs = pt.tag & 7, wct = pt.tag >> 3;
+            const int a0 = sm.seg[wcs], b0 = sm.seg[wct];
+            const int nt = sm.seg[wct + 1] - b0;
+            const bool same = wcs == wct;
             int npairs = 0;
             if (pt.r < pt.L) {
-                const int ns = sm.seg[pt.cs + 1] - a0;
+                const int ns = sm.seg[wcs + 1] - a0;
                 npairs = same ? ns * (ns - 1) / 2 : ns * nt;
             }
             const float inv_nt = __frcp_rn((float)max(nt, 1));
             float gw[NNP_ANG_BLOCK];
             {
-                const int pb = pt.cs * (2 * P.np + 1 - pt.cs) / 2 + (pt.ct - pt.cs);
+                const int pb = wcs * (2 * P.np + 1 - wcs) / 2 + (wct - wcs);
                 const float *gp = grow + P.n_rad + pb * NNP_ANG_BLOCK;
                 const float sc0 = 2.0f * inv_nets; // the prefactor 2 of the angular term
 #pragma unroll
@@ -441,25 +554,25 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float2 fj = sm.fr[ia], fk = sm.fr[ib];
                 const float rjk_inv = fj.y * fk.y;
                 const float cs_ = (dj.x * dk.x + dj.y * dk.y + dj.z * dk.z) * rjk_inv; // cos(theta)
-                const float c = 0.95f * cs_;
-                const float s2 = fmaf(-c, c, 1.0f);
+                const float cc = 0.95f * cs_;
+                const float s2 = fmaf(-cc, cc, 1.0f);
                 const float sn_inv = rsq(s2);
                 const float sn = s2 * sn_inv;
-                const float krb = (0.5f * P.ka) * (dj.w + dk.w);
+                const float rjk = dj.w + dk.w;
                 float fz[NNP_NSHF_Z], dfz[NNP_NSHF_Z]; // F_z and (dF_z/dcos(theta)) / k_ang
 #pragma unroll
                 for (int z = 0; z < NNP_NSHF_Z; ++z) {
-                    const float base = fmaf(c, hcz[z], fmaf(sn, hsz[z], 0.5f));
+                    const float base = fmaf(cc, hcz[z], fmaf(sn, hsz[z], 0.5f));
                     const float pw = ex2(zm1 * lg2(base)); // base^(zeta-1)
                     fz[z] = pw * base;
                     // dF/dtheta' = -(zeta/2) sin(theta'-phi) base^(zeta-1); dtheta'/dcos = -0.95/sn
-                    dfz[z] = fmaf(sn, hcz[z], -c * hsz[z]) * pw;
+                    dfz[z] = fmaf(sn, hcz[z], -cc * hsz[z]) * pw;
                 }
                 float Az[NNP_NSHF_Z] = {0.f, 0.f, 0.f, 0.f};
                 float dE_drb = 0.f;
 #pragma unroll
                 for (int a = 0; a < NNP_NSHF_A; ++a) {
-                    const float w = krb - P.ka_shf[a];
+                    const float w = fmaf(0.5f * P.ka, rjk, -P.ka_shf[a]);
                     const float ra = ex2(-w * w);
                     float Ba = 0.f;
 #pragma unroll
@@ -485,8 +598,9 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float alj = (dE_drj - dE_dcs * cs_ * fj.y) * fj.y;
                 const float alk = (dE_drk - dE_dcs * cs_ * fk.y) * fk.y;
                 if (arena) {
-                    const int slot = ib * (ib - 1) / 2 + ia; // ia < ib
-                    sm.alo[slot] = alj; sm.ahi[slot] = alk; sm.bet[slot] = beta;
+                    const int sab = ia * kMatLd + ib, sba = ib * kMatLd + ia;
+                    sm.alp[sab] = alj; sm.alp[sba] = alk;
+                    sm.bet[sab] = beta; sm.bet[sba] = beta;
                 } else {
                     atomicAdd(&fsm[ia][0], alj * dj.x + beta * dk.x);
                     atomicAdd(&fsm[ia][1], alj * dj.y + beta * dk.y);
@@ -505,18 +619,11 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float4 da = sm.d[a];
                 float asum = 0.f;
                 fx = 0.f; fy = 0.f; fz = 0.f;
-                for (int b = 0; b < a; ++b) {
-                    const int slot = a * (a - 1) / 2 + b;
-                    const float be = sm.bet[slot];
+                const float *ra = sm.alp + a * kMatLd, *rb = sm.bet + a * kMatLd;
+                for (int b = 0; b < na; ++b) {
+                    const float be = rb[b];
                     const float4 db = sm.d[b];
-                    asum += sm.ahi[slot];
-                    fx = fmaf(be, db.x, fx); fy = fmaf(be, db.y, fy); fz = fmaf(be, db.z, fz);
-                }
-                for (int b = a + 1; b < na; ++b) {
-                    const int slot = b * (b - 1) / 2 + a;
-                    const float be = sm.bet[slot];
-                    const float4 db = sm.d[b];
-                    asum += sm.alo[slot];
+                    asum += ra[b];
                     fx = fmaf(be, db.x, fx); fy = fmaf(be, db.y, fy); fz = fmaf(be, db.z, fz);
                 }
                 fx = fmaf(asum, da.x, fx); fy = fmaf(asum, da.y, fy); fz = fmaf(asum, da.z, fz);
@@ -527,12 +634,13 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
             fi[0] += fx; fi[1] += fy; fi[2] += fz;
         }
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
+        for (int q = 0; q < 3; ++q) {
 #pragma unroll
-            for (int o = 16; o >= 1; o >>= 1) fi[c] += __shfl_xor_sync(kFull, fi[c], o);
+            for (int o = 16; o >= 1; o >>= 1) fi[q] += __shfl_xor_sync(kFull, fi[q], o);
         }
         if (lane == 0) atomicAdd(&frc[i], make_float4(fi[0], fi[1], fi[2], 0.f));
         __syncwarp();
+        sgr_l = sgr_n; sga_l = sga_n;
     }
 }
 
