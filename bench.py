@@ -190,7 +190,8 @@ def run_ours(args):
         ev1.record(stream)
     barrier()
     sampler.stop_flag.set()
-    launches = nnp.nnp_launch_count(ctx) - l0
+    launches = nnp.nnp_launch_count(ctx) - l0   # kernels outside the conditional rebuild; + 8 per rebuild below
+    kact = nnp.nnp_aev_active_columns(ctx)
     ms = ev0.elapsed_time(ev1)
     nnp.nnp_sync(ctx)
     stage_ms, stage_n = nnp.nnp_profile_read(ctx)
@@ -237,7 +238,8 @@ def run_ours(args):
     per_stage = {nnp.STAGE_NAMES[k]: (stage_ms[k] / stage_n[k] if stage_n[k] else 0.0) for k in range(nnp.NNP_N_STAGES)}
     tot_stage = sum(per_stage.values())
     dom = max(per_stage, key=per_stage.get)
-    roof = roofline_for(dom, per_stage[dom], n, sp, args.mm_mode, pk, clocks)
+    kpad = (kact + 31) // 32 * 32
+    roof = roofline_for(dom, per_stage[dom], n, sp, args.mm_mode, pk, clocks, kpad)
     roof["stage_ms"] = {k: round(v, 4) for k, v in per_stage.items()}
     roof["stage_share"] = {k: round(v / tot_stage, 4) for k, v in per_stage.items()} if tot_stage else {}
 
@@ -252,13 +254,16 @@ def run_ours(args):
                    "rebuilds_in_timed_region": nr_end - nr_start,
                    "temperature_K_end": 2 * ek_end / (3 * n * inputs.KB), "temperature_K_start": 2 * ek_start / (3 * n * inputs.KB),
                    "etot_drift_rel": (e_end - e_start) / abs(e_start) if e_start else None,
-                   "l2_policy": "inputs larger than L2 (G 403 MB + activations 240 MB per step; no flush needed)",
+                   "aev_active_columns": kact,
+                   "l2_policy": "inputs larger than L2: per step the kernels stream G (%d MB), the activations (%d MB) and "
+                                "the neighbour rows (%d MB); no flush needed" % (n * kpad * 4 // 2**20, n * 608 * 4 // 2**20,
+                                                                                   n * 224 * 4 // 2**20),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": world * n * Ke / (e2e_ms_max * 1e-3), "unit": UNIT, "steps": Ke,
                 "h2d_bytes_per_step": 2 * n * 12, "d2h_bytes_per_step": 2 * n * 12 + 16,
                 "api": "nnp_md_step_host (pinned host x,v up; x,v,epot,ekin down; every step)"},
-        "gpu_launches": launches,
+        "gpu_launches": launches + 8 * (nr_end - nr_start),
         "roofline": roof,
     }
     if world == 1 and not args.no_cpu_baseline:
@@ -272,12 +277,11 @@ def run_ours(args):
     return 0
 
 
-def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks):
+def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
     """Roofline entry for the dominant stage (DESIGN.md 'Kernels and rooflines' gives the per-atom figures)."""
     from paper_2405_01491_b200 import inputs
     W = inputs.WIDTHS
     counts = np.bincount(sp, minlength=7)
-    kpad = 1024
 
     def macs(op):
         tot = 0

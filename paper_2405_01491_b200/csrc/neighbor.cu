@@ -39,42 +39,43 @@ __global__ void k_keys_hist(int n, const float4 *__restrict__ pos, const int *__
 }
 
 // Single-block exclusive scan of hist[0..nk) into start[0..nk]; also clears hist for reuse as cursor.
-__global__ void k_scan(int nk, int *__restrict__ hist, int *__restrict__ start, const int *cond)
+// Each of the 1024 threads owns one contiguous chunk (serial sum, one block-wide scan, serial write-back), so the
+// whole scan costs two passes over the keys and three block barriers.
+__global__ void __launch_bounds__(1024) k_scan(int nk, int *__restrict__ hist, int *__restrict__ start, const int *cond)
 {
     if (cond && *cond == 0) return;
     __shared__ int warp_sums[32];
-    __shared__ int carry;
-    if (threadIdx.x == 0) carry = 0;
-    __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int base = 0; base < nk; base += blockDim.x) {
-        int i = base + threadIdx.x;
-        int v = i < nk ? hist[i] : 0;
-        int x = v;
+    const int chunk = (nk + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int beg = min(nk, (int)threadIdx.x * chunk), end = min(nk, beg + chunk);
+    int sum = 0;
+    for (int i = beg; i < end; ++i) sum += hist[i];
+    int x = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_sums[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        int w = lane < ((int)blockDim.x >> 5) ? warp_sums[lane] : 0;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            int y = __shfl_up_sync(0xffffffffu, x, o);
-            if (lane >= o) x += y;
+            int y = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += y;
         }
-        if (lane == 31) warp_sums[wid] = x;
-        __syncthreads();
-        if (wid == 0) {
-            int w = lane < (blockDim.x >> 5) ? warp_sums[lane] : 0;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int y = __shfl_up_sync(0xffffffffu, w, o);
-                if (lane >= o) w += y;
-            }
-            warp_sums[lane] = w; // inclusive
-        }
-        __syncthreads();
-        int prefix = carry + (wid > 0 ? warp_sums[wid - 1] : 0);
-        if (i < nk) { start[i] = prefix + x - v; hist[i] = 0; }
-        __syncthreads();
-        if (threadIdx.x == blockDim.x - 1) carry = prefix + x;
-        __syncthreads();
+        warp_sums[lane] = w; // inclusive
     }
-    if (threadIdx.x == 0) start[nk] = carry;
+    __syncthreads();
+    int run = (wid > 0 ? warp_sums[wid - 1] : 0) + x - sum;
+    for (int i = beg; i < end; ++i) {
+        const int v = hist[i];
+        start[i] = run;
+        hist[i] = 0;
+        run += v;
+    }
+    if (threadIdx.x == blockDim.x - 1) start[nk] = run;
 }
 
 __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ start,
@@ -149,39 +150,46 @@ __device__ __forceinline__ float r2_defined(const float4 a, const float4 b, cons
     return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
 }
 
-// One warp per atom.  For species s = 0..S-1, for the distinct cells within +-1 of the atom's cell
-// (x-adjacent cells are contiguous in the sorted order, so each (y,z) row is at most two ranges), test 32
-// candidates per step with coalesced float4 loads and append hits with ballot compaction.
+// One warp per atom.  Per species (rows must stay grouped by neighbour species, stage 2), the candidate cells
+// are <= 18 contiguous index ranges of the sorted order: the 3 x 3 (y,z) rows of the stencil, each one or two
+// x-ranges (x-adjacent cells are adjacent in the sort).  Lane r fetches the bounds of range r (one load round per
+// species instead of a dependent chain per row), a warp scan turns the lengths into one flat candidate list, and
+// the lanes walk that list 32 candidates at a time (coalesced float4 loads, ballot compaction into the two rows),
+// so a trip is full even where single ranges hold 10-40 atoms.
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_build_lists(int n, int S, const float4 *__restrict__ pos, const int *__restrict__ mol,
+k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, const int *__restrict__ mol,
               const int *__restrict__ cell_start, GridInfo g, float rl2_r, float rl2_a, int cap_r, int cap_a,
               int *__restrict__ nbr_r, int *__restrict__ nbr_a, uint16_t *__restrict__ seg_r,
               uint16_t *__restrict__ seg_a, int *__restrict__ flags, const int *cond)
 {
     if (cond && *cond == 0) return;
+    const unsigned kFull = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int i = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
     if (i >= n) return;
     const float4 pi = pos[i];
-    int cx = 0, cy = 0, cz = 0;
-    int ys[3], zs[3], nys = 1, nzs = 1;
-    int xa[2], xb[2], nxs = 1; // x ranges [xa, xb]
+    // range `lane` of the stencil: first / last cell (inside one species block) and whether it exists
+    int c_first = 0, c_last = 0, nranges = 1;
     if (g.periodic) {
-        cx = cell_coord(pi.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
-        cy = cell_coord(pi.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
-        cz = cell_coord(pi.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
-        // distinct cells among c-1, c, c+1 (mod nc)
-        if (g.nc[1] >= 3) { nys = 3; ys[0] = (cy + g.nc[1] - 1) % g.nc[1]; ys[1] = cy; ys[2] = (cy + 1) % g.nc[1]; }
-        else { nys = g.nc[1]; ys[0] = 0; ys[1] = 1; }
-        if (g.nc[2] >= 3) { nzs = 3; zs[0] = (cz + g.nc[2] - 1) % g.nc[2]; zs[1] = cz; zs[2] = (cz + 1) % g.nc[2]; }
-        else { nzs = g.nc[2]; zs[0] = 0; zs[1] = 1; }
-        if (g.nc[0] <= 3) { xa[0] = 0; xb[0] = g.nc[0] - 1; }
-        else if (cx == 0) { xa[0] = 0; xb[0] = 1; xa[1] = g.nc[0] - 1; xb[1] = g.nc[0] - 1; nxs = 2; }
-        else if (cx == g.nc[0] - 1) { xa[0] = cx - 1; xb[0] = cx; xa[1] = 0; xb[1] = 0; nxs = 2; }
-        else { xa[0] = cx - 1; xb[0] = cx + 1; }
+        const int cx = cell_coord(pi.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
+        const int cy = cell_coord(pi.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
+        const int cz = cell_coord(pi.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
+        const int nys = g.nc[1] >= 3 ? 3 : g.nc[1], nzs = g.nc[2] >= 3 ? 3 : g.nc[2]; // distinct cells among c-1, c, c+1
+        const int nxs = (g.nc[0] > 3 && (cx == 0 || cx == g.nc[0] - 1)) ? 2 : 1;     // the x range wraps
+        nranges = nzs * nys * nxs;
+        const int ix = lane % nxs, t = lane / nxs, iy = t % nys, iz = t / nys;
+        const int y = nys == 3 ? (cy + iy + g.nc[1] - 1) % g.nc[1] : iy;
+        const int z = nzs == 3 ? (cz + iz + g.nc[2] - 1) % g.nc[2] : iz;
+        int xa, xb;
+        if (g.nc[0] <= 3) { xa = 0; xb = g.nc[0] - 1; }
+        else if (cx == 0) { xa = ix ? g.nc[0] - 1 : 0; xb = ix ? g.nc[0] - 1 : 1; }
+        else if (cx == g.nc[0] - 1) { xa = ix ? 0 : cx - 1; xb = ix ? 0 : cx; }
+        else { xa = cx - 1; xb = cx + 1; }
+        const int rowbase = (z * g.nc[1] + y) * g.nc[0];
+        c_first = rowbase + xa;
+        c_last = rowbase + xb;
     } else {
-        ys[0] = 0; zs[0] = 0;
-        xa[0] = xb[0] = mol[i]; // the "cell" of a non-periodic structure is the structure itself
+        c_first = c_last = mol[i]; // the "cell" of a non-periodic structure is the structure itself
     }
     int cnt_r = 0, cnt_a = 0;
     int *row_r = nbr_r + (size_t)i * cap_r;
@@ -192,30 +200,44 @@ k_build_lists(int n, int S, const float4 *__restrict__ pos, const int *__restric
             seg_r[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_r, cap_r);
             seg_a[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_a, cap_a);
         }
-        const int base = s * g.ncell;
-        for (int iz = 0; iz < nzs; ++iz)
-            for (int iy = 0; iy < nys; ++iy) {
-                const int rowbase = base + (zs[iz] * g.nc[1] + ys[iy]) * g.nc[0];
-                for (int ix = 0; ix < nxs; ++ix) {
-                    const int beg = cell_start[rowbase + xa[ix]];
-                    const int end = cell_start[rowbase + xb[ix] + 1];
-                    for (int j0 = beg; j0 < end; j0 += 32) {
-                        const int j = j0 + lane;
-                        bool hr = false, ha = false;
-                        if (j < end && j != i) {
-                            float r2 = r2_defined(pi, pos[j], g);
-                            hr = r2 < rl2_r;
-                            ha = r2 < rl2_a;
-                        }
-                        unsigned mr = __ballot_sync(0xffffffffu, hr);
-                        unsigned ma = __ballot_sync(0xffffffffu, ha);
-                        if (hr) { int p = cnt_r + __popc(mr & lt); if (p < cap_r) row_r[p] = j; }
-                        if (ha) { int p = cnt_a + __popc(ma & lt); if (p < cap_a) row_a[p] = j; }
-                        cnt_r += __popc(mr);
-                        cnt_a += __popc(ma);
-                    }
-                }
+        if (!(present >> s & 1u)) continue;
+        int beg = 0, len = 0;
+        if (lane < nranges) {
+            beg = cell_start[s * g.ncell + c_first];
+            len = cell_start[s * g.ncell + c_last + 1] - beg;
+        }
+        int incl = len; // inclusive prefix of the range lengths
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += y;
+        }
+        const int total = __shfl_sync(kFull, incl, 31);
+        const int off = beg - (incl - len); // flat index v of range r is atom v + off_r
+        int r = 0;                          // range this lane's flat index currently falls into
+        for (int t0 = 0; t0 < total; t0 += 32) {
+            const int v = t0 + lane;
+            const bool act = v < total;
+            for (;;) { // advance past finished (and empty) ranges; v grows monotonically, so r never goes back
+                const int r_end = __shfl_sync(kFull, incl, r); // every lane takes part (no short-circuit around it)
+                const bool adv = act && v >= r_end;
+                if (!__any_sync(kFull, adv)) break;
+                if (adv) ++r;
             }
+            const int j = v + __shfl_sync(kFull, off, r);
+            bool hr = false, ha = false;
+            if (act && j != i) {
+                const float r2 = r2_defined(pi, pos[j], g);
+                hr = r2 < rl2_r;
+                ha = r2 < rl2_a;
+            }
+            const unsigned mr = __ballot_sync(kFull, hr);
+            const unsigned ma = __ballot_sync(kFull, ha);
+            if (hr) { const int p = cnt_r + __popc(mr & lt); if (p < cap_r) row_r[p] = j; }
+            if (ha) { const int p = cnt_a + __popc(ma & lt); if (p < cap_a) row_a[p] = j; }
+            cnt_r += __popc(mr);
+            cnt_a += __popc(ma);
+        }
     }
     if (lane == 0) {
         for (int s = S; s < NNP_MAX_SPECIES; ++s) {
@@ -253,9 +275,9 @@ int nnp_launch_build(nnp_ctx *c, const int *cond)
                                  c->xref, c->spc, c->orig, c->mol, cond);
     const float rl_r = c->aev.rcr + c->skin, rl_a = c->aev.rca + c->skin;
     k_build_lists<<<nnp_div_up(n, kWarpsPerBlock), kWarpsPerBlock * 32, 0, st>>>(
-        n, S, c->pos, c->mol, c->cell_start, c->grid, rl_r * rl_r, rl_a * rl_a, c->aev.cap_r, c->aev.cap_a,
+        n, S, c->present_mask, c->pos, c->mol, c->cell_start, c->grid, rl_r * rl_r, rl_a * rl_a, c->aev.cap_r, c->aev.cap_a,
         c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->flags, cond);
     k_finish_build<<<1, 1, 0, st>>>(c->flags, cond);
-    c->launches += 8;
+    if (!cond) c->launches += 8; // conditional builds are counted from the device-side rebuild counter (flags[2])
     return 0;
 }

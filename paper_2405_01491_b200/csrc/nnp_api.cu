@@ -3,6 +3,7 @@
 // mlp_simt.cu / mlp_tc.cu and integrate.cu.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -144,6 +145,12 @@ __global__ void k_get_e_atom(int n, const float *__restrict__ e_atom, const int 
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     out[orig[i]] = e_atom[i] * inv_nets + e_shift[spc[i]];
+}
+
+// Sets the IF node of the MD-step graph from the rebuild request the drift kernel left in flags[1].
+__global__ void k_set_rebuild_cond(cudaGraphConditionalHandle h, const int *__restrict__ flag)
+{
+    cudaGraphSetConditional(h, *flag != 0 ? 1u : 0u);
 }
 
 template <typename Tp>
@@ -350,6 +357,72 @@ int setup_grid(nnp_ctx *c, float skin)
     return NNP_OK;
 }
 
+void drop_md_graph(nnp_ctx *c)
+{
+    if (c->md_exec) { cudaGraphExecDestroy(c->md_exec); c->md_exec = nullptr; }
+    if (c->md_graph) { cudaGraphDestroy(c->md_graph); c->md_graph = nullptr; }
+}
+
+// Captures one MD step into a graph.  The neighbour rebuild (8 kernels) sits in the body of a conditional IF node
+// whose value a one-thread kernel copies from the device-side rebuild request, so a step without a rebuild
+// launches none of them (the kernel-by-kernel path launches all 8 and lets each return at once).
+int build_md_graph(nnp_ctx *c)
+{
+    drop_md_graph(c);
+    if (!c->aux_stream) CU(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+    cudaGraph_t g = nullptr;
+    CU(c, cudaGraphCreate(&g, 0));
+    c->md_graph = g;
+    cudaGraphConditionalHandle h;
+    CU(c, cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault));
+    const int64_t launches0 = c->launches;
+    int rc = NNP_OK;
+    cudaStream_t main_stream = c->stream;
+    CU(c, cudaStreamBeginCaptureToGraph(main_stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+    bool capturing = true;
+    do {
+        nnp_launch_kick_drift(c);
+        k_set_rebuild_cond<<<1, 1, 0, main_stream>>>(h, c->flags + 1);
+        c->launches += 1;
+        cudaStreamCaptureStatus st;
+        const cudaGraphNode_t *deps = nullptr;
+        size_t ndeps = 0;
+        if (cudaStreamGetCaptureInfo_v2(main_stream, &st, nullptr, nullptr, &deps, &ndeps) != cudaSuccess) { rc = NNP_ECUDA; break; }
+        cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+        np.conditional.handle = h;
+        np.conditional.type = cudaGraphCondTypeIf;
+        np.conditional.size = 1;
+        cudaGraphNode_t cnode;
+        if (cudaGraphAddNode(&cnode, g, deps, ndeps, &np) != cudaSuccess) { rc = NNP_ECUDA; break; }
+        cudaGraph_t body = np.conditional.phGraph_out[0];
+        const int64_t l1 = c->launches;
+        if (cudaStreamBeginCaptureToGraph(c->aux_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { rc = NNP_ECUDA; break; }
+        c->stream = c->aux_stream;
+        nnp_launch_build(c, nullptr);
+        c->stream = main_stream;
+        cudaGraph_t body_out = nullptr;
+        if (cudaStreamEndCapture(c->aux_stream, &body_out) != cudaSuccess) { rc = NNP_ECUDA; break; }
+        c->launches = l1; // the body's kernels run only on a rebuild: counted from the device-side rebuild counter
+        if (cudaStreamUpdateCaptureDependencies(main_stream, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) { rc = NNP_ECUDA; break; }
+        rc = run_forces(c);
+        if (rc) break;
+        nnp_launch_kick_ke(c);
+    } while (0);
+    cudaGraph_t out = nullptr;
+    cudaError_t e = capturing ? cudaStreamEndCapture(main_stream, &out) : cudaSuccess;
+    c->stream = main_stream;
+    c->md_graph_launches = c->launches - launches0;
+    c->launches = launches0;
+    if (rc == NNP_OK && e != cudaSuccess) rc = NNP_ECUDA;
+    if (rc == NNP_OK && cudaGraphInstantiate(&c->md_exec, g, 0) != cudaSuccess) rc = NNP_ECUDA;
+    if (rc != NNP_OK) {
+        const cudaError_t last = cudaGetLastError();
+        drop_md_graph(c);
+        if (c->err.empty() || rc == NNP_ECUDA) c->err = std::string("MD-step graph capture failed: ") + cudaGetErrorString(last != cudaSuccess ? last : e);
+    }
+    return rc;
+}
+
 } // namespace
 
 extern "C" {
@@ -365,6 +438,8 @@ void nnp_destroy(nnp_ctx *c)
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
+    drop_md_graph(c);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
@@ -409,6 +484,10 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode; c->dense_aev = p->dense_aev != 0;
     c->alpha = p->celu_alpha; c->accel_conv = p->accel_conv;
     c->stream = (cudaStream_t)cuda_stream; c->device = device;
+    { // the legacy / per-thread default streams cannot be captured: steps are then enqueued kernel by kernel
+        const char *e = getenv("NNP_NO_GRAPH");
+        c->no_graph = (e && e[0] == '1') || c->stream == nullptr || c->stream == cudaStreamLegacy || c->stream == cudaStreamPerThread;
+    }
     c->max_atoms = max_atoms; c->max_mols = max_mols;
     c->hmax[0] = c->hmax[1] = c->hmax[2] = 0;
     for (int s = 0; s < S; ++s)
@@ -573,6 +652,7 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
     c->n = n_atoms; c->n_mols = n_mols; c->periodic = nper == 3;
     for (int d = 0; d < 3; ++d) c->box[d] = h_box[d];
     c->have_system = 1; c->have_lists = 0; c->have_forces = 0; c->md_ready = 0;
+    drop_md_graph(c);
     int *bins = c->flags + 8; // [8..15] species histogram, [3] bad-species marker
     CU(c, cudaMemsetAsync(c->flags, 0, sizeof(int) * 16, c->stream));
     int h_counts[NNP_MAX_SPECIES] = {0};
@@ -693,6 +773,7 @@ int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
     CU(c, cudaSetDevice(c->device));
     nnp_launch_permute_in3(c, d_vel, c->vel);
     c->dt = dt_fs;
+    drop_md_graph(c);
     CU(c, cudaMemsetAsync(c->flags + 1, 0, sizeof(int) * 2, c->stream)); // rebuild request and counter
     int rc = nnp_build_neighbors(c, skin);
     if (rc) return rc;
@@ -713,8 +794,17 @@ int nnp_md_step(nnp_ctx *c, int n_steps)
     if (!c->md_ready) NNP_FAIL(c, NNP_ESTALE, "nnp_md_init first");
     if (n_steps < 0) NNP_FAIL(c, NNP_EINVAL, "n_steps < 0");
     CU(c, cudaSetDevice(c->device));
+    if (!c->no_graph && !c->md_exec && n_steps > 0) {
+        int rc = build_md_graph(c);
+        if (rc) return rc;
+    }
     for (int step = 0; step < n_steps; ++step) {
         prof_begin(c);
+        if (c->md_exec && !c->prof_active) { // the per-stage event marks need the kernel-by-kernel path
+            CU(c, cudaGraphLaunch(c->md_exec, c->stream));
+            c->launches += c->md_graph_launches;
+            continue;
+        }
         nnp_launch_kick_drift(c);
         nnp_prof_mark(c, 0);
         nnp_launch_build(c, c->flags + 1); // every kernel returns at once unless the drift requested a rebuild

@@ -166,6 +166,12 @@ struct nnp_ctx {
     // staging for the host entry points
     float *io_xyz, *io_vel;  // [n][3]
     int *io_species;
+    // one MD step as a CUDA graph: kick+drift -> IF(rebuild requested){stage 1} -> stages 2-4 -> kick (nnp_api.cu)
+    cudaGraph_t md_graph;
+    cudaGraphExec_t md_exec;
+    cudaStream_t aux_stream;     // capture stream of the conditional body
+    int64_t md_graph_launches;   // kernels per graph launch outside the conditional body
+    int no_graph;                // NNP_NO_GRAPH=1: enqueue every step kernel by kernel
 };
 
 // ---- launches implemented across the .cu files --------------------------------------------------

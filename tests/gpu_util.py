@@ -24,13 +24,16 @@ def make_model(n_nets=1, seed=inputs.SEED0, widths=inputs.WIDTHS, scale=FORCE_SC
 MM_MODE = int(os.environ.get("NNP_MM_MODE", "1"))   # default: 3xTF32 tcgen05 (the mode bench.py reports)
 
 
-def gpu_create(consts, widths, params, n_nets, max_atoms, max_mols=1, mm_mode=None, cap_r=0, cap_a=0, self_energy=None):
+def gpu_create(consts, widths, params, n_nets, max_atoms, max_mols=1, mm_mode=None, cap_r=0, cap_a=0, self_energy=None,
+               stream=None):
+    """stream: a torch.cuda.Stream (the MD step then runs as a CUDA graph) or None = the current (default) stream,
+    which cannot be captured, so steps are enqueued kernel by kernel."""
     if mm_mode is None:
         mm_mode = MM_MODE
     p, keep = nnp.make_params(consts, widths, params, inputs.MASS, inputs.ACCEL_CONV, n_nets=n_nets,
                               self_energy=self_energy, mm_mode=mm_mode, cap_r=cap_r, cap_a=cap_a)
-    stream = torch.cuda.current_stream().cuda_stream
-    ctx = nnp.nnp_create(p, max_atoms, max_mols, 0, stream)
+    handle = torch.cuda.current_stream().cuda_stream if stream is None else stream.cuda_stream
+    ctx = nnp.nnp_create(p, max_atoms, max_mols, 0, handle)
     return ctx
 
 
@@ -41,10 +44,11 @@ def gpu_energy_forces(ctx, species, xyz, box, mol_offsets=None, skin=0.0):
     d_x = torch.as_tensor(np.asarray(xyz, dtype=np.float32), device=dev).contiguous()
     n_mols = 1 if mol_offsets is None else len(mol_offsets) - 1
     d_mo = None if mol_offsets is None else torch.as_tensor(np.asarray(mol_offsets, dtype=np.int32), device=dev)
-    nnp.nnp_set_system(ctx, n, d_sp, d_x, box, n_mols, d_mo)
-    nnp.nnp_build_neighbors(ctx, skin)
     d_E = torch.zeros(n_mols, dtype=torch.float64, device=dev)
     d_F = torch.zeros((max(n, 1), 3), dtype=torch.float32, device=dev)
+    torch.cuda.synchronize()   # the context may run on a side stream
+    nnp.nnp_set_system(ctx, n, d_sp, d_x, box, n_mols, d_mo)
+    nnp.nnp_build_neighbors(ctx, skin)
     nnp.nnp_energy_forces(ctx, d_E, d_F)
     nnp.nnp_sync(ctx)
     return d_E.cpu().numpy(), d_F.cpu().numpy()[:n].astype(np.float64)

@@ -177,23 +177,28 @@ def test_capacity_overflow_is_reported(model1):
 
 
 # ---------------------------------------------------------------- MD (stage 5)
-def test_md_steps_against_oracle(model1):
+@pytest.mark.parametrize("graph", [False, True], ids=["kernel_by_kernel", "cuda_graph"])
+def test_md_steps_against_oracle(model1, graph):
+    """graph=True: the context runs on a side stream, so nnp_md_step launches the captured step graph (rebuild inside
+    a conditional node); graph=False: default stream, every kernel enqueued separately."""
     consts, widths, params, om = model1
     sp, xyz, box = inputs.water_box(216, seed=9)
     v = inputs.maxwell_boltzmann(sp, 300.0, seed=2)
     n = len(sp)
     dev = torch.device("cuda:0")
-    ctx = U.gpu_create(consts, widths, params, 1, n)
+    ctx = U.gpu_create(consts, widths, params, 1, n, stream=torch.cuda.Stream(device=dev) if graph else None)
     try:
         d_sp = torch.as_tensor(sp, device=dev)
         d_x = torch.as_tensor(xyz.astype(np.float32), device=dev)
         d_v = torch.as_tensor(v.astype(np.float32), device=dev)
+        torch.cuda.synchronize()
         nnp.nnp_set_system(ctx, n, d_sp, d_x, box)
         nnp.nnp_md_init(ctx, d_v, 0.5, 0.5)
         o_x, o_v = torch.zeros_like(d_x), torch.zeros_like(d_v)
         o_ep = torch.zeros(1, dtype=torch.float64, device=dev)
         o_ek = torch.zeros(1, dtype=torch.float64, device=dev)
         o_nr = torch.zeros(1, dtype=torch.int32, device=dev)
+        torch.cuda.synchronize()
 
         def state():
             nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, o_nr)
