@@ -80,13 +80,45 @@ __device__ __forceinline__ float rsq(float x)
     return y;
 }
 
+// Packed fp32 pairs (FFMA2 / FMUL2 / FADD2 on sm_100): one issue slot for two lanes of arithmetic.  A float2 built as
+// (s, s) from one scalar compiles to the scalar-broadcast operand form, no extra moves.
+__device__ __forceinline__ float2 fma2(const float2 a, const float2 b, const float2 c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<const unsigned long long *>(&a)), "l"(*reinterpret_cast<const unsigned long long *>(&b)),
+          "l"(*reinterpret_cast<const unsigned long long *>(&c)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 mul2(const float2 a, const float2 b)
+{
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<const unsigned long long *>(&a)), "l"(*reinterpret_cast<const unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 add2(const float2 a, const float2 b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<const unsigned long long *>(&a)), "l"(*reinterpret_cast<const unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 bc2(const float s) { return make_float2(s, s); }
+
 __device__ __forceinline__ float3 min_image(const float4 a, const float4 b, const AevParams &P)
 {
     float dx = b.x - a.x, dy = b.y - a.y, dz = b.z - a.z;
     if (P.periodic) {
-        dx -= P.box[0] * rintf(dx * P.inv_box[0]);
-        dy -= P.box[1] * rintf(dy * P.inv_box[1]);
-        dz -= P.box[2] * rintf(dz * P.inv_box[2]);
+        // round-to-nearest by the 1.5 * 2^23 trick: two FADDs on the FMA pipe instead of an FRND on the XU pipe
+        // (|d / L| < 2^22 always); any consistent choice of image is fine here, list membership is decided in stage 1
+        const float M = 12582912.0f;
+        dx -= P.box[0] * ((dx * P.inv_box[0] + M) - M);
+        dy -= P.box[1] * ((dy * P.inv_box[1] + M) - M);
+        dz -= P.box[2] * ((dz * P.inv_box[2] + M) - M);
     }
     return make_float3(dx, dy, dz);
 }
@@ -110,11 +142,12 @@ struct LanePart {
     int beg_b, L_b; // as block lane
     int tag;        // as worker: tag of the block served
     int r, L;       // as worker: rank inside the block's lane group and its size; active iff r < L
+    unsigned starts; // bit l set: a lane group starts at lane l (warp-uniform)
 };
 __device__ __forceinline__ LanePart partition(int n_b, int tag_b, int *own, int lane)
 {
     LanePart pt;
-    pt.I = 0; pt.beg_b = 0; pt.L_b = 0; pt.tag = 0; pt.r = 0; pt.L = 0;
+    pt.I = 0; pt.beg_b = 0; pt.L_b = 0; pt.tag = 0; pt.r = 0; pt.L = 0; pt.starts = 0u;
     const int N = __reduce_add_sync(kFull, n_b);
     if (N == 0) return pt;
     int I = (N + 31) >> 5, L_b;
@@ -132,14 +165,14 @@ __device__ __forceinline__ LanePart partition(int n_b, int tag_b, int *own, int 
     }
     const int beg_b = x - L_b;
     const unsigned starts = __reduce_or_sync(kFull, L_b > 0 ? (1u << beg_b) : 0u);
-    if (L_b > 0) own[beg_b] = tag_b | (L_b << 8) | (beg_b << 16);
+    if (L_b > 0) own[beg_b] = tag_b | (L_b << 8) | (beg_b << 16) | (lane << 24); // bits 24+: block lane index
     __syncwarp();
     const int p = 31 - __clz(starts & (kFull >> (31 - lane))); // first lane of this lane's group (bit 0 is always set)
     const int w = own[p];
     __syncwarp();
-    pt.I = I; pt.beg_b = beg_b; pt.L_b = L_b;
+    pt.I = I; pt.beg_b = beg_b; pt.L_b = L_b; pt.starts = starts;
     pt.tag = w & 0xff; pt.L = (w >> 8) & 0xff;
-    pt.r = lane - (w >> 16);
+    pt.r = lane - ((w >> 16) & 0xff);
     return pt;
 }
 
@@ -156,6 +189,83 @@ __device__ __forceinline__ void decode_pair(int q, bool same, int nt, float inv_
         b = q - a * nt;
     }
 }
+
+// Which centre a warp takes next.  MODE 0: static (warp w takes w, w + W, ...).  MODE 1: one global ticket counter.
+// MODE 2: the centres are cut into one contiguous range per SM and the warps of SM s take tickets of range s, so the
+// warps that run on one SM at the same time work on ~20 consecutive (cell-sorted) atoms: their neighbour rows and
+// positions share L1 lines, and the force reductions that hit the same atom come from one SM instead of queueing
+// from many.  A warp whose range is used up moves to any range with centres left, so every centre is processed
+// wherever the blocks were placed.  sched[0]: warps that have left (the last one zeroes all counters, so every
+// launch starts clean without a memset); sched[32 + s]: tickets taken from range s (MODE 1: s = 0).
+#ifndef AEV_FWD_SCHED
+#define AEV_FWD_SCHED 1
+#endif
+#ifndef AEV_BWD_SCHED
+#define AEV_BWD_SCHED 0
+#endif
+template <int MODE>
+struct CentreQueue {
+    int *sched;
+    int n, nsm, s, lane;
+    int beg, end;  // current range
+    int pending;   // lane 0: ticket requested and not yet read
+
+    __device__ __forceinline__ void set_range(int r)
+    {
+        s = r;
+        beg = (int)((long long)r * n / nsm);
+        end = (int)((long long)(r + 1) * n / nsm);
+    }
+    __device__ __forceinline__ void init(int *sched_, int n_, int nsm_, int lane_)
+    {
+        sched = sched_; n = n_; lane = lane_; pending = 0;
+        nsm = MODE == 2 ? nsm_ : 1;
+        unsigned smid = 0;
+        if (MODE == 2) asm("mov.u32 %0, %%smid;" : "=r"(smid));
+        set_range((int)(smid % (unsigned)nsm));
+    }
+    __device__ __forceinline__ void request()
+    {
+        if (MODE != 0 && lane == 0) pending = atomicAdd(sched + 32 + s, 1);
+    }
+    // cur: the centre being processed (MODE 0 only)
+    __device__ __forceinline__ int receive(int cur)
+    {
+        if (MODE == 0) return cur < 0 ? (int)(blockIdx.x * kWarps + (threadIdx.x >> 5)) : cur + (int)(gridDim.x * kWarps);
+        for (;;) {
+            const int t = beg + __shfl_sync(kFull, pending, 0);
+            if (t < end) return t;
+            if (MODE == 1) return n;
+            // range used up: take any range that still has centres (counters only grow, so this terminates)
+            int found = -1;
+            for (int r0 = 1; r0 < nsm && found < 0; r0 += 32) {
+                const int off = r0 + lane;
+                int cand = s + off;
+                if (cand >= nsm) cand -= nsm;
+                bool has = false;
+                if (off < nsm) {
+                    const int cb = (int)((long long)cand * n / nsm), ce = (int)((long long)(cand + 1) * n / nsm);
+                    has = *(volatile int *)(sched + 32 + cand) < ce - cb;
+                }
+                const unsigned m = __ballot_sync(kFull, has);
+                if (m) found = __shfl_sync(kFull, cand, __ffs(m) - 1);
+            }
+            if (found < 0) return n;
+            set_range(found);
+            request();
+        }
+    }
+    __device__ __forceinline__ void release()
+    {
+        if (MODE == 0) return;
+        int last = 0;
+        if (lane == 0) last = atomicAdd(sched, 1) == (int)(gridDim.x * kWarps) - 1;
+        if (__shfl_sync(kFull, last, 0)) {
+            for (int r = lane; r < nsm; r += 32) atomicExch(sched + 32 + r, 0);
+            if (lane == 0) atomicExch(sched, 0);
+        }
+    }
+};
 
 // Everything both kernels do before their arithmetic: lane roles, the segment tables (one centre ahead), the
 // radial lane partition, and the batched index / position loads of the current centre.
@@ -227,7 +337,10 @@ __device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const C
                 float sn, cs_;
                 __sincosf(P.pi_rca * r, &sn, &cs_);
                 sm.d[p] = make_float4(d.x, d.y, d.z, r);
-                sm.fr[p] = make_float2(0.5f * cs_ + 0.5f, rinv);
+                // forward: lg2(fc) + 1/2, so that lfc_j + lfc_k = lg2(2 fc_j fc_k) folds the pair prefactor into the
+                // exponent of the zeta power; reverse: fc itself
+                const float fc = 0.5f * cs_ + 0.5f;
+                sm.fr[p] = make_float2(BWD ? fc : lg2(fc) + 0.5f, rinv);
                 if constexpr (BWD) {
                     sm.dfc[p] = -0.5f * P.pi_rca * sn;
                     sm.j[p] = j;
@@ -262,7 +375,7 @@ __global__ void __launch_bounds__(kWarps * 32, AEV_FWD_MINB)
 k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
               const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
               const uint16_t *__restrict__ seg_a, const uint16_t *__restrict__ tri, float *__restrict__ G,
-              int *__restrict__ flags)
+              int *__restrict__ flags, int *__restrict__ sched, int nsm)
 {
     __shared__ WarpSmem smem[kWarps];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -278,38 +391,38 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 #pragma unroll
     for (int z = 0; z < NNP_NSHF_Z; ++z) { hcz[z] = 0.5f * P.cos_z[z]; hsz[z] = 0.5f * P.sin_z[z]; }
 
-    const int stride = gridDim.x * kWarps;
-    int i = blockIdx.x * kWarps + wid;
+    CentreQueue<AEV_FWD_SCHED> queue;
+    queue.init(sched, n, nsm, lane);
+    queue.request();
+    int i = queue.receive(-1);
     int sgr_l = 0, sga_l = 0;
     if (i < n && lane < NNP_MAX_SPECIES) {
         sgr_l = seg_r[(size_t)i * NNP_MAX_SPECIES + lane];
         sga_l = seg_a[(size_t)i * NNP_MAX_SPECIES + lane];
     }
-    for (; i < n; i += stride) {
-        int sgr_n = 0, sga_n = 0; // segment tables of the next centre
-        if (i + stride < n && lane < NNP_MAX_SPECIES) {
-            sgr_n = seg_r[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
-            sga_n = seg_a[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
-        }
+    while (i < n) {
+        queue.request(); // read after the radial phase
         Centre c;
         load_centre(c, P, i, lane, my_s, sgr_l, sga_l, pos, nbr_r, nbr_a, sm.own);
         float *Grow = G + (size_t)i * P.kpad;
 
         // ---- radial block: G[cs*16+k] = 1/4 sum_j exp(-eta_r (r-ShfR_k)^2) fc(r)
         {
-            float acc[NNP_NSHF_R];
+            float2 acc[NNP_NSHF_R / 2];
 #pragma unroll
-            for (int k = 0; k < NNP_NSHF_R; ++k) acc[k] = 0.f;
+            for (int k = 0; k < NNP_NSHF_R / 2; ++k) acc[k] = make_float2(0.f, 0.f);
             auto term = [&](const float4 xj) {
                 const float3 d = min_image(c.pi, xj, P);
                 const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
                 if (r2 < P.rcr2) {
                     const float r = r2 * rsq(r2);
-                    const float fc = 0.125f * __cosf(P.pi_rcr * r) + 0.125f; // (1/4) fc
+                    const float2 fc = bc2(0.125f * __cosf(P.pi_rcr * r) + 0.125f); // (1/4) fc
+                    const float2 u = bc2(P.kr * r);
 #pragma unroll
-                    for (int k = 0; k < NNP_NSHF_R; ++k) {
-                        const float w = fmaf(P.kr, r, -P.kr_shf[k]);
-                        acc[k] = fmaf(fc, ex2(-w * w), acc[k]);
+                    for (int k = 0; k < NNP_NSHF_R / 2; ++k) {
+                        const float2 w = add2(u, make_float2(-P.kr_shf[2 * k], -P.kr_shf[2 * k + 1]));
+                        const float2 ww = mul2(w, w);
+                        acc[k] = fma2(fc, make_float2(ex2(-ww.x), ex2(-ww.y)), acc[k]);
                     }
                 }
             };
@@ -327,7 +440,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 float *myrow = sm.red + lane * kRedLd;
 #pragma unroll
                 for (int q4 = 0; q4 < NNP_NSHF_R / 4; ++q4)
-                    *reinterpret_cast<float4 *>(myrow + 4 * q4) = make_float4(acc[4 * q4], acc[4 * q4 + 1], acc[4 * q4 + 2], acc[4 * q4 + 3]);
+                    *reinterpret_cast<float4 *>(myrow + 4 * q4) = make_float4(acc[2 * q4].x, acc[2 * q4].y, acc[2 * q4 + 1].x, acc[2 * q4 + 1].y);
                 __syncwarp();
             }
             // rows [beg_b, beg_b + L_b) belong to species b; a half warp sums the 16 columns of one species
@@ -346,6 +459,12 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
         }
 
         // ---- angular block
+        const int i_next = queue.receive(i);
+        int sgr_n = 0, sga_n = 0; // segment tables of the next centre
+        if (i_next < n && lane < NNP_MAX_SPECIES) {
+            sgr_n = seg_r[(size_t)i_next * NNP_MAX_SPECIES + lane];
+            sga_n = seg_a[(size_t)i_next * NNP_MAX_SPECIES + lane];
+        }
         stage_angular<false>(sm, P, c, i, lane, pos, nbr_a, flags);
         int n_b = 0;
         if (lane < nb_tot) {
@@ -353,10 +472,13 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
             n_b = bcs == bct ? ns * (ns - 1) / 2 : ns * nt;
         }
         const LanePart pt = partition(n_b, bcs | (bct << 3), sm.own, lane);
+        // blocks without a pair are zero rows of G
+        for (unsigned zm = __ballot_sync(kFull, lane < nb_tot && n_b == 0); zm; zm &= zm - 1)
+            Grow[P.n_rad + (__ffs(zm) - 1) * NNP_ANG_BLOCK + lane] = 0.f;
         if (pt.I > 0) {
-            float acc[NNP_ANG_BLOCK];
+            float2 acc[NNP_ANG_BLOCK / 2]; // [a][z pair]
 #pragma unroll
-            for (int q = 0; q < NNP_ANG_BLOCK; ++q) acc[q] = 0.f;
+            for (int q = 0; q < NNP_ANG_BLOCK / 2; ++q) acc[q] = make_float2(0.f, 0.f);
             const int wcs = pt.tag & 7, wct = pt.tag >> 3;
             const int a0 = sm.seg[wcs], b0 = sm.seg[wct];
             const int nt = sm.seg[wct + 1] - b0;
@@ -367,52 +489,65 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 npairs = same ? ns * (ns - 1) / 2 : ns * nt;
             }
             const float inv_nt = __frcp_rn((float)max(nt, 1));
+            const float2 zeta2 = bc2(P.zeta), half2 = bc2(0.5f);
             for (int q = pt.r; q < npairs; q += pt.L) {
                 int ia, ib;
                 decode_pair(q, same, nt, inv_nt, tri, ia, ib);
                 ia += a0; ib += same ? a0 : b0;
                 const float4 dj = sm.d[ia], dk = sm.d[ib];
-                const float2 fj = sm.fr[ia], fk = sm.fr[ib];
-                const float ff = 2.0f * fj.x * fk.x;
+                const float2 fj = sm.fr[ia], fk = sm.fr[ib]; // (lg2 fc + 1/2, 1/r)
+                const float lff = fj.x + fk.x;               // lg2(2 fc_j fc_k)
                 const float cc = (0.95f * fj.y * fk.y) * (dj.x * dk.x + dj.y * dk.y + dj.z * dk.z);
                 const float s2 = fmaf(-cc, cc, 1.0f);
                 const float sn = s2 * rsq(s2);
-                const float rjk = dj.w + dk.w;
-                float fz[NNP_NSHF_Z];
+                const float2 cc2 = bc2(cc), sn2 = bc2(sn), lff2 = bc2(lff);
+                // F_z = 2 fc_j fc_k ((1 + cos(theta' - ShfZ_z)) / 2)^zeta = 2^(zeta lg2(base_z) + lff)
+                float2 fz[NNP_NSHF_Z / 2];
 #pragma unroll
-                for (int z = 0; z < NNP_NSHF_Z; ++z) {
-                    const float base = fmaf(cc, hcz[z], fmaf(sn, hsz[z], 0.5f));
-                    fz[z] = ff * ex2(P.zeta * lg2(base));
+                for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
+                    const float2 base = fma2(cc2, make_float2(hcz[2 * zp], hcz[2 * zp + 1]),
+                                             fma2(sn2, make_float2(hsz[2 * zp], hsz[2 * zp + 1]), half2));
+                    const float2 e = fma2(zeta2, make_float2(lg2(base.x), lg2(base.y)), lff2);
+                    fz[zp] = make_float2(ex2(e.x), ex2(e.y));
                 }
+                const float2 u = bc2(0.5f * P.ka * (dj.w + dk.w));
 #pragma unroll
-                for (int a = 0; a < NNP_NSHF_A; ++a) {
-                    const float w = fmaf(0.5f * P.ka, rjk, -P.ka_shf[a]);
-                    const float ra = ex2(-w * w);
+                for (int ap = 0; ap < NNP_NSHF_A / 2; ++ap) {
+                    const float2 w = add2(u, make_float2(-P.ka_shf[2 * ap], -P.ka_shf[2 * ap + 1]));
+                    const float2 ww = mul2(w, w);
+                    const float2 ra0 = bc2(ex2(-ww.x)), ra1 = bc2(ex2(-ww.y));
 #pragma unroll
-                    for (int z = 0; z < NNP_NSHF_Z; ++z) acc[a * NNP_NSHF_Z + z] = fmaf(ra, fz[z], acc[a * NNP_NSHF_Z + z]);
+                    for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
+                        acc[(2 * ap) * 2 + zp] = fma2(ra0, fz[zp], acc[(2 * ap) * 2 + zp]);
+                        acc[(2 * ap + 1) * 2 + zp] = fma2(ra1, fz[zp], acc[(2 * ap + 1) * 2 + zp]);
+                    }
                 }
             }
             float *myrow = sm.red + lane * kRedLd;
 #pragma unroll
             for (int q4 = 0; q4 < NNP_ANG_BLOCK / 4; ++q4)
-                *reinterpret_cast<float4 *>(myrow + 4 * q4) = make_float4(acc[4 * q4], acc[4 * q4 + 1], acc[4 * q4 + 2], acc[4 * q4 + 3]);
+                *reinterpret_cast<float4 *>(myrow + 4 * q4) = make_float4(acc[2 * q4].x, acc[2 * q4].y, acc[2 * q4 + 1].x, acc[2 * q4 + 1].y);
             __syncwarp();
-        }
-        // rows [beg_b, beg_b + L_b) of the transpose buffer belong to block b; lane = feature inside the block
-        for (int p = 0; p < nb_tot; ++p) {
-            const int beg = __shfl_sync(kFull, pt.beg_b, p), L = __shfl_sync(kFull, pt.L_b, p);
-            float s0 = 0.f, s1 = 0.f;
-            int rr = beg;
-            for (; rr + 1 < beg + L; rr += 2) {
-                s0 += sm.red[rr * kRedLd + lane];
-                s1 += sm.red[(rr + 1) * kRedLd + lane];
+            // Rows of the transpose buffer are grouped by block (lane groups of the partition; lanes past the last
+            // group hold zeros).  lane = feature inside the block: one running sum over the 32 rows, flushed as one
+            // coalesced 128 B store wherever the next row starts a new group (warp-uniform branches).
+            float sum = 0.f;
+            float *gp = Grow + P.n_rad + lane + (sm.own[0] >> 24) * NNP_ANG_BLOCK; // block lane index = block index p
+#pragma unroll
+            for (int rr = 0; rr < 32; ++rr) {
+                sum += sm.red[rr * kRedLd + lane];
+                if (rr == 31 || (pt.starts >> (rr + 1) & 1u)) {
+                    *gp = sum;
+                    sum = 0.f;
+                    if (rr < 31) gp = Grow + P.n_rad + lane + (sm.own[rr + 1] >> 24) * NNP_ANG_BLOCK;
+                }
             }
-            if (rr < beg + L) s0 += sm.red[rr * kRedLd + lane];
-            Grow[P.n_rad + p * NNP_ANG_BLOCK + lane] = s0 + s1;
         }
         __syncwarp();
         sgr_l = sgr_n; sga_l = sga_n;
+        i = i_next;
     }
+    queue.release();
 }
 
 // Reverse pass: g = dE/dG_i (row of dG, times inv_nets).  Adds -dE/dx to frc for the centre and its neighbours.
@@ -420,7 +555,7 @@ __global__ void __launch_bounds__(kWarps * 32, AEV_BWD_MINB)
 k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
                const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
                const uint16_t *__restrict__ seg_a, const uint16_t *__restrict__ tri, const float *__restrict__ dG,
-               float inv_nets, float4 *__restrict__ frc, int *__restrict__ flags)
+               float inv_nets, float4 *__restrict__ frc, int *__restrict__ flags, int *__restrict__ sched, int nsm)
 {
     extern __shared__ __align__(16) uint8_t smem_dyn[];
     WarpSmemBwd *smem = reinterpret_cast<WarpSmemBwd *>(smem_dyn);
@@ -443,19 +578,19 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     const float dr_scale = -2.0f * P.eta_r / P.kr;
     float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.alp);
 
-    const int stride = gridDim.x * kWarps;
-    int i = blockIdx.x * kWarps + wid;
+    // Centres are handed out dynamically (one ticket per centre): the cost of a centre varies with its pair count,
+    // and with a static split the slowest warp of a persistent grid ends ~20 % after the average one.
+    CentreQueue<AEV_BWD_SCHED> queue;
+    queue.init(sched, n, nsm, lane);
+    queue.request();
+    int i = queue.receive(-1);
     int sgr_l = 0, sga_l = 0;
     if (i < n && lane < NNP_MAX_SPECIES) {
         sgr_l = seg_r[(size_t)i * NNP_MAX_SPECIES + lane];
         sga_l = seg_a[(size_t)i * NNP_MAX_SPECIES + lane];
     }
-    for (; i < n; i += stride) {
-        int sgr_n = 0, sga_n = 0;
-        if (i + stride < n && lane < NNP_MAX_SPECIES) {
-            sgr_n = seg_r[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
-            sga_n = seg_a[(size_t)(i + stride) * NNP_MAX_SPECIES + lane];
-        }
+    while (i < n) {
+        queue.request(); // read after the radial phase
         Centre c;
         load_centre(c, P, i, lane, my_s, sgr_l, sga_l, pos, nbr_r, nbr_a, sm.own);
         const float *grow = dG + (size_t)i * P.kpad;
@@ -508,6 +643,12 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
         }
 
         // ---- angular
+        const int i_next = queue.receive(i);
+        int sgr_n = 0, sga_n = 0; // segment tables of the next centre
+        if (i_next < n && lane < NNP_MAX_SPECIES) {
+            sgr_n = seg_r[(size_t)i_next * NNP_MAX_SPECIES + lane];
+            sga_n = seg_a[(size_t)i_next * NNP_MAX_SPECIES + lane];
+        }
         const int na = stage_angular<true>(sm, P, c, i, lane, pos, nbr_a, flags);
         const bool arena = na <= kMat; // warp-uniform
         if (arena) {
@@ -641,7 +782,9 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
         if (lane == 0) atomicAdd(&frc[i], make_float4(fi[0], fi[1], fi[2], 0.f));
         __syncwarp();
         sgr_l = sgr_n; sga_l = sga_n;
+        i = i_next;
     }
+    queue.release();
 }
 
 int g_blocks_fwd = 0, g_blocks_bwd = 0, g_sms = 0;
@@ -661,6 +804,7 @@ static int persistent_grid(nnp_ctx *c, int blocks_per_sm)
     if (!g_sms) {
         cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, c->device);
         if (g_sms <= 0) g_sms = 148;
+        if (g_sms > 1024) g_sms = 1024;
     }
     const int want = nnp_div_up(c->n, kWarps);
     const int cap = g_sms * (blocks_per_sm > 0 ? blocks_per_sm : 1);
@@ -670,8 +814,9 @@ static int persistent_grid(nnp_ctx *c, int blocks_per_sm)
 void nnp_launch_aev_forward(nnp_ctx *c)
 {
     if (!g_blocks_fwd) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_fwd, k_aev_forward, kWarps * 32, 0);
-    k_aev_forward<<<persistent_grid(c, g_blocks_fwd), kWarps * 32, 0, c->stream>>>(c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a,
-                                                                                  c->seg_a, c->d_tri, c->G, c->flags);
+    const int grid = persistent_grid(c, g_blocks_fwd);
+    k_aev_forward<<<grid, kWarps * 32, 0, c->stream>>>(c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a,
+                                                                                  c->seg_a, c->d_tri, c->G, c->flags, c->aev_sched, g_sms);
     c->launches += 1;
 }
 
@@ -682,7 +827,8 @@ void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets)
         cudaFuncSetAttribute(k_aev_backward, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_bwd, k_aev_backward, kWarps * 32, smem);
     }
-    k_aev_backward<<<persistent_grid(c, g_blocks_bwd), kWarps * 32, smem, c->stream>>>(
-        c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a, c->seg_a, c->d_tri, c->dG, inv_nets, c->frc, c->flags);
+    const int grid = persistent_grid(c, g_blocks_bwd);
+    k_aev_backward<<<grid, kWarps * 32, smem, c->stream>>>(
+        c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a, c->seg_a, c->d_tri, c->dG, inv_nets, c->frc, c->flags, c->aev_sched + NNP_AEV_SCHED_LEN, g_sms);
     c->launches += 1;
 }

@@ -443,7 +443,7 @@ void nnp_destroy(nnp_ctx *c)
     void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
-                    c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags,
+                    c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags, c->aev_sched,
                     c->io_xyz, c->io_vel, c->io_species};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (auto &m : c->prof_marks) cudaEventDestroy(m.first);
@@ -627,6 +627,8 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     TRY(dev_alloc(c, &c->flags, 16));
     TRY(dev_alloc(c, &c->io_xyz, 3 * N)); TRY(dev_alloc(c, &c->io_vel, 3 * N)); TRY(dev_alloc(c, &c->io_species, N));
     TRYCU(cudaMemset(c->flags, 0, sizeof(int) * 16));
+    TRY(dev_alloc(c, &c->aev_sched, 2 * NNP_AEV_SCHED_LEN));
+    TRYCU(cudaMemset(c->aev_sched, 0, sizeof(int) * 2 * NNP_AEV_SCHED_LEN));
     TRYCU(cudaMemset(c->ekin, 0, sizeof(double)));
     TRYCU(cudaDeviceSynchronize());
 #undef TRY

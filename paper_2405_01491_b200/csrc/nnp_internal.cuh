@@ -14,6 +14,7 @@
 #define NNP_NSHF_Z 4
 #define NNP_ANG_BLOCK (NNP_NSHF_A * NNP_NSHF_Z) /* 32 features per species pair */
 #define NNP_NLAYERS 4
+#define NNP_AEV_SCHED_LEN 1056 /* per AEV kernel: [0] exit counter, [32 + s] tickets of SM range s (s < 1024) */
 #define NNP_TRI_LEN 2016 /* pairs (lo < hi) with hi < 64: decode table of the AEV kernels */
 
 // Device error flags latched by kernels, reported by synchronising calls.
@@ -163,6 +164,7 @@ struct nnp_ctx {
     double *e_mol;           // [max_mols]
     double *ekin;            // scalar
     int *flags;              // [0] error flags, [1] rebuild request, [2] rebuild count
+    int *aev_sched;          // [2][NNP_AEV_SCHED_LEN] centre queues of the two AEV kernels (aev.cu), zero between launches
     // staging for the host entry points
     float *io_xyz, *io_vel;  // [n][3]
     int *io_species;
