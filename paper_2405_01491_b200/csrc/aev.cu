@@ -598,14 +598,14 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
 
         // ---- radial: dE/dr_ij = sum_k g[s_j*16+k] * 1/4 e_k (-2 eta (r-ShfR_k) fc + fc')
         if (c.pr.I > 0) {
-            float gr[NNP_NSHF_R];
+            float2 gr[NNP_NSHF_R / 2];
             const float sc0 = 0.25f * inv_nets;
 #pragma unroll
             for (int k4 = 0; k4 < NNP_NSHF_R / 4; ++k4) {
                 float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (c.pr.r < c.pr.L) v = *reinterpret_cast<const float4 *>(grow + c.pr.tag * NNP_NSHF_R + 4 * k4);
-                gr[4 * k4] = v.x * sc0; gr[4 * k4 + 1] = v.y * sc0;
-                gr[4 * k4 + 2] = v.z * sc0; gr[4 * k4 + 3] = v.w * sc0;
+                gr[2 * k4] = make_float2(v.x * sc0, v.y * sc0);
+                gr[2 * k4 + 1] = make_float2(v.z * sc0, v.w * sc0);
             }
             auto term = [&](int j, const float4 xj) {
                 const float3 d = min_image(c.pi, xj, P);
@@ -615,15 +615,18 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                     const float r = r2 * rinv;
                     float sn, cs_;
                     __sincosf(P.pi_rcr * r, &sn, &cs_);
-                    const float fc = (0.5f * cs_ + 0.5f) * dr_scale;
-                    const float dfc = -0.5f * P.pi_rcr * sn;
-                    float dEdr = 0.f;
+                    const float2 fc = bc2((0.5f * cs_ + 0.5f) * dr_scale);
+                    const float2 dfc = bc2(-0.5f * P.pi_rcr * sn);
+                    const float2 u = bc2(P.kr * r);
+                    float2 acc = make_float2(0.f, 0.f);
 #pragma unroll
-                    for (int k = 0; k < NNP_NSHF_R; ++k) {
-                        const float w = fmaf(P.kr, r, -P.kr_shf[k]);
-                        const float e = ex2(-w * w);
-                        dEdr = fmaf(gr[k] * e, fmaf(w, fc, dfc), dEdr);
+                    for (int k = 0; k < NNP_NSHF_R / 2; ++k) {
+                        const float2 w = add2(u, make_float2(-P.kr_shf[2 * k], -P.kr_shf[2 * k + 1]));
+                        const float2 ww = mul2(w, w);
+                        const float2 e = make_float2(ex2(-ww.x), ex2(-ww.y));
+                        acc = fma2(mul2(gr[k], e), fma2(w, fc, dfc), acc);
                     }
+                    const float dEdr = acc.x + acc.y;
                     const float sc = dEdr * rinv;
                     const float vx = sc * d.x, vy = sc * d.y, vz = sc * d.z;
                     atomicAdd(&frc[j], make_float4(-vx, -vy, -vz, 0.f));
@@ -674,7 +677,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 npairs = same ? ns * (ns - 1) / 2 : ns * nt;
             }
             const float inv_nt = __frcp_rn((float)max(nt, 1));
-            float gw[NNP_ANG_BLOCK];
+            float2 gw[NNP_ANG_BLOCK / 2]; // [a][z pair]
             {
                 const int pb = wcs * (2 * P.np + 1 - wcs) / 2 + (wct - wcs);
                 const float *gp = grow + P.n_rad + pb * NNP_ANG_BLOCK;
@@ -683,10 +686,11 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 for (int q4 = 0; q4 < NNP_ANG_BLOCK / 4; ++q4) {
                     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (npairs > 0) v = *reinterpret_cast<const float4 *>(gp + 4 * q4);
-                    gw[4 * q4] = v.x * sc0; gw[4 * q4 + 1] = v.y * sc0;
-                    gw[4 * q4 + 2] = v.z * sc0; gw[4 * q4 + 3] = v.w * sc0;
+                    gw[2 * q4] = make_float2(v.x * sc0, v.y * sc0);
+                    gw[2 * q4 + 1] = make_float2(v.z * sc0, v.w * sc0);
                 }
             }
+            const float2 zm12 = bc2(zm1), half2 = bc2(0.5f);
             for (int q = pt.r; q < npairs; q += pt.L) {
                 int ia, ib;
                 decode_pair(q, same, nt, inv_nt, tri, ia, ib);
@@ -699,37 +703,43 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float s2 = fmaf(-cc, cc, 1.0f);
                 const float sn_inv = rsq(s2);
                 const float sn = s2 * sn_inv;
-                const float rjk = dj.w + dk.w;
-                float fz[NNP_NSHF_Z], dfz[NNP_NSHF_Z]; // F_z and (dF_z/dcos(theta)) / k_ang
+                const float2 cc2 = bc2(cc), sn2 = bc2(sn);
+                float2 fz[NNP_NSHF_Z / 2], dfz[NNP_NSHF_Z / 2]; // F_z and (dF_z/dcos(theta)) / k_ang
 #pragma unroll
-                for (int z = 0; z < NNP_NSHF_Z; ++z) {
-                    const float base = fmaf(cc, hcz[z], fmaf(sn, hsz[z], 0.5f));
-                    const float pw = ex2(zm1 * lg2(base)); // base^(zeta-1)
-                    fz[z] = pw * base;
+                for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
+                    const float2 hc = make_float2(hcz[2 * zp], hcz[2 * zp + 1]), hs = make_float2(hsz[2 * zp], hsz[2 * zp + 1]);
+                    const float2 base = fma2(cc2, hc, fma2(sn2, hs, half2));
+                    const float2 e = mul2(zm12, make_float2(lg2(base.x), lg2(base.y)));
+                    const float2 pw = make_float2(ex2(e.x), ex2(e.y)); // base^(zeta-1)
+                    fz[zp] = mul2(pw, base);
                     // dF/dtheta' = -(zeta/2) sin(theta'-phi) base^(zeta-1); dtheta'/dcos = -0.95/sn
-                    dfz[z] = fmaf(sn, hcz[z], -cc * hsz[z]) * pw;
+                    dfz[zp] = mul2(fma2(sn2, hc, mul2(cc2, make_float2(-hs.x, -hs.y))), pw);
                 }
-                float Az[NNP_NSHF_Z] = {0.f, 0.f, 0.f, 0.f};
-                float dE_drb = 0.f;
+                // A_z = sum_a g[a][z] ra_a (value and angular derivative), C_z = sum_a g[a][z] ra_a w_a (radial derivative)
+                float2 Az[NNP_NSHF_Z / 2], Cz[NNP_NSHF_Z / 2];
 #pragma unroll
-                for (int a = 0; a < NNP_NSHF_A; ++a) {
-                    const float w = fmaf(0.5f * P.ka, rjk, -P.ka_shf[a]);
-                    const float ra = ex2(-w * w);
-                    float Ba = 0.f;
+                for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) { Az[zp] = make_float2(0.f, 0.f); Cz[zp] = make_float2(0.f, 0.f); }
+                const float2 u = bc2(0.5f * P.ka * (dj.w + dk.w));
 #pragma unroll
-                    for (int z = 0; z < NNP_NSHF_Z; ++z) {
-                        const float g = gw[a * NNP_NSHF_Z + z];
-                        Az[z] = fmaf(g, ra, Az[z]);
-                        Ba = fmaf(g, fz[z], Ba);
+                for (int ap = 0; ap < NNP_NSHF_A / 2; ++ap) {
+                    const float2 w = add2(u, make_float2(-P.ka_shf[2 * ap], -P.ka_shf[2 * ap + 1]));
+                    const float2 ww = mul2(w, w);
+                    const float2 ra = make_float2(ex2(-ww.x), ex2(-ww.y));
+                    const float2 rw = mul2(ra, w);
+#pragma unroll
+                    for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
+                        Az[zp] = fma2(gw[(2 * ap) * 2 + zp], bc2(ra.x), Az[zp]);
+                        Cz[zp] = fma2(gw[(2 * ap) * 2 + zp], bc2(rw.x), Cz[zp]);
+                        Az[zp] = fma2(gw[(2 * ap + 1) * 2 + zp], bc2(ra.y), Az[zp]);
+                        Cz[zp] = fma2(gw[(2 * ap + 1) * 2 + zp], bc2(rw.y), Cz[zp]);
                     }
-                    dE_drb = fmaf(Ba, ra * w, dE_drb);
                 }
-                float T = 0.f, dE_dcs = 0.f;
-#pragma unroll
-                for (int z = 0; z < NNP_NSHF_Z; ++z) {
-                    T = fmaf(Az[z], fz[z], T);
-                    dE_dcs = fmaf(Az[z], dfz[z], dE_dcs);
-                }
+                const float2 T2 = fma2(Az[0], fz[0], mul2(Az[1], fz[1]));
+                const float2 D2 = fma2(Az[0], dfz[0], mul2(Az[1], dfz[1]));
+                const float2 R2 = fma2(Cz[0], fz[0], mul2(Cz[1], fz[1]));
+                const float T = T2.x + T2.y;
+                float dE_dcs = D2.x + D2.y;
+                const float dE_drb = R2.x + R2.y;
                 const float ff = fj.x * fk.x;
                 dE_dcs *= ff * (k_ang0 * sn_inv);
                 const float half_drb = (0.5f * drb_scale) * dE_drb * ff;
