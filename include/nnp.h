@@ -156,6 +156,10 @@ int nnp_profile_read(nnp_ctx *ctx, double *h_ms_sum, int64_t *h_samples);
 int64_t nnp_launch_count(const nnp_ctx *ctx);
 int nnp_aev_len(const nnp_ctx *ctx);            /* full AEV length of the model (1008 for 7 species) */
 int nnp_aev_active_columns(const nnp_ctx *ctx); /* columns stored for the loaded system (see nnp_params.dense_aev) */
+/* 1 if the AEV kernels evaluate the Gaussian shift sets by the ladder recurrence (uniformly spaced ShfR / ShfA whose
+ * powers stay in fp32 range), 0 if every exponential is evaluated directly (any shift set; NNP_NO_LADDER=1 in the
+ * environment at nnp_create forces this).  Same results within the parity tolerances either way. */
+int nnp_aev_ladder(const nnp_ctx *ctx);
 
 #ifdef __cplusplus
 }

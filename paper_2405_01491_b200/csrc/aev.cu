@@ -371,6 +371,7 @@ __device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const C
     return na;
 }
 
+template <bool LAD>
 __global__ void __launch_bounds__(kWarps * 32, AEV_FWD_MINB)
 k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
               const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
@@ -390,6 +391,8 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
     float hcz[NNP_NSHF_Z], hsz[NNP_NSHF_Z];
 #pragma unroll
     for (int z = 0; z < NNP_NSHF_Z; ++z) { hcz[z] = 0.5f * P.cos_z[z]; hsz[z] = 0.5f * P.sin_z[z]; }
+    // constant factors of the ladder, applied once per feature where lane = feature (1 without ladder)
+    const float lad_r = LAD ? P.lad_r[lane & 15] : 1.0f, lad_a = LAD ? P.lad_a[lane >> 2] : 1.0f;
 
     CentreQueue<AEV_FWD_SCHED> queue;
     queue.init(sched, n, nsm, lane);
@@ -418,11 +421,32 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                     const float r = r2 * rsq(r2);
                     const float2 fc = bc2(0.125f * __cosf(P.pi_rcr * r) + 0.125f); // (1/4) fc
                     const float2 u = bc2(P.kr * r);
+                    if constexpr (LAD) {
+                        // anchors k = 1, 5, 9, 13; acc[2m] = shifts (4m, 4m+1), acc[2m+1] = (4m+2, 4m+3), unscaled
+                        float2 t[NNP_NSHF_R / 8];
 #pragma unroll
-                    for (int k = 0; k < NNP_NSHF_R / 2; ++k) {
-                        const float2 w = add2(u, make_float2(-P.kr_shf[2 * k], -P.kr_shf[2 * k + 1]));
-                        const float2 ww = mul2(w, w);
-                        acc[k] = fma2(fc, make_float2(ex2(-ww.x), ex2(-ww.y)), acc[k]);
+                        for (int mp = 0; mp < NNP_NSHF_R / 8; ++mp) {
+                            const float2 w = add2(u, make_float2(-P.kr_shf[8 * mp + 1], -P.kr_shf[8 * mp + 5]));
+                            const float2 ww = mul2(w, w);
+                            t[mp] = mul2(fc, make_float2(ex2(-ww.x), ex2(-ww.y)));
+                        }
+                        const float x = (2.0f * P.dlt_r) * (u.x - P.kr_shf[1]);
+                        const float q = ex2(x);
+                        const float2 pq0 = make_float2(ex2(-x), 1.0f), pq1 = make_float2(q, q * q);
+#pragma unroll
+                        for (int mp = 0; mp < NNP_NSHF_R / 8; ++mp) {
+                            acc[4 * mp] = fma2(bc2(t[mp].x), pq0, acc[4 * mp]);
+                            acc[4 * mp + 1] = fma2(bc2(t[mp].x), pq1, acc[4 * mp + 1]);
+                            acc[4 * mp + 2] = fma2(bc2(t[mp].y), pq0, acc[4 * mp + 2]);
+                            acc[4 * mp + 3] = fma2(bc2(t[mp].y), pq1, acc[4 * mp + 3]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < NNP_NSHF_R / 2; ++k) {
+                            const float2 w = add2(u, make_float2(-P.kr_shf[2 * k], -P.kr_shf[2 * k + 1]));
+                            const float2 ww = mul2(w, w);
+                            acc[k] = fma2(fc, make_float2(ex2(-ww.x), ex2(-ww.y)), acc[k]);
+                        }
                     }
                 }
             };
@@ -452,7 +476,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 if (cs >= P.np) L = 0;
                 float sum = 0.f;
                 for (int rr = beg; rr < beg + L; ++rr) sum += sm.red[rr * kRedLd + (lane & 15)];
-                if (cs < P.np) Grow[cs * NNP_NSHF_R + (lane & 15)] = sum;
+                if (cs < P.np) Grow[cs * NNP_NSHF_R + (lane & 15)] = sum * lad_r;
             }
             for (int q = P.aev_len + lane; q < P.kpad; q += 32) Grow[q] = 0.f; // zero padding columns
             __syncwarp();
@@ -511,15 +535,30 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                     fz[zp] = make_float2(ex2(e.x), ex2(e.y));
                 }
                 const float2 u = bc2(0.5f * P.ka * (dj.w + dk.w));
+                float2 ra[NNP_NSHF_A / 2]; // radial factors (a, a+1); with the ladder: without their constant factors
+                if constexpr (LAD) {
+                    const float2 w = add2(u, make_float2(-P.ka_shf[1], -P.ka_shf[5])); // anchors a = 1, 5
+                    const float2 ww = mul2(w, w);
+                    const float x = (2.0f * P.dlt_a) * w.x;
+                    const float q = ex2(x);
+                    const float2 pq0 = make_float2(ex2(-x), 1.0f), pq1 = make_float2(q, q * q);
+                    const float e0 = ex2(-ww.x), e1 = ex2(-ww.y);
+                    ra[0] = mul2(bc2(e0), pq0); ra[1] = mul2(bc2(e0), pq1);
+                    ra[2] = mul2(bc2(e1), pq0); ra[3] = mul2(bc2(e1), pq1);
+                } else {
+#pragma unroll
+                    for (int ap = 0; ap < NNP_NSHF_A / 2; ++ap) {
+                        const float2 w = add2(u, make_float2(-P.ka_shf[2 * ap], -P.ka_shf[2 * ap + 1]));
+                        const float2 ww = mul2(w, w);
+                        ra[ap] = make_float2(ex2(-ww.x), ex2(-ww.y));
+                    }
+                }
 #pragma unroll
                 for (int ap = 0; ap < NNP_NSHF_A / 2; ++ap) {
-                    const float2 w = add2(u, make_float2(-P.ka_shf[2 * ap], -P.ka_shf[2 * ap + 1]));
-                    const float2 ww = mul2(w, w);
-                    const float2 ra0 = bc2(ex2(-ww.x)), ra1 = bc2(ex2(-ww.y));
 #pragma unroll
                     for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
-                        acc[(2 * ap) * 2 + zp] = fma2(ra0, fz[zp], acc[(2 * ap) * 2 + zp]);
-                        acc[(2 * ap + 1) * 2 + zp] = fma2(ra1, fz[zp], acc[(2 * ap + 1) * 2 + zp]);
+                        acc[(2 * ap) * 2 + zp] = fma2(bc2(ra[ap].x), fz[zp], acc[(2 * ap) * 2 + zp]);
+                        acc[(2 * ap + 1) * 2 + zp] = fma2(bc2(ra[ap].y), fz[zp], acc[(2 * ap + 1) * 2 + zp]);
                     }
                 }
             }
@@ -537,7 +576,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
             for (int rr = 0; rr < 32; ++rr) {
                 sum += sm.red[rr * kRedLd + lane];
                 if (rr == 31 || (pt.starts >> (rr + 1) & 1u)) {
-                    *gp = sum;
+                    *gp = sum * lad_a;
                     sum = 0.f;
                     if (rr < 31) gp = Grow + P.n_rad + lane + (sm.own[rr + 1] >> 24) * NNP_ANG_BLOCK;
                 }
@@ -551,6 +590,8 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 }
 
 // Reverse pass: g = dE/dG_i (row of dG, times inv_nets).  Adds -dE/dx to frc for the centre and its neighbours.
+// (The Gaussian ladder of the forward kernel is not used here: the reverse pass needs every w_k as well, the
+// recurrence then costs more issue slots than the exponentials it saves -- measured 0.355 vs 0.346 ms.)
 __global__ void __launch_bounds__(kWarps * 32, AEV_BWD_MINB)
 k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
                const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
@@ -823,9 +864,10 @@ static int persistent_grid(nnp_ctx *c, int blocks_per_sm)
 
 void nnp_launch_aev_forward(nnp_ctx *c)
 {
-    if (!g_blocks_fwd) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_fwd, k_aev_forward, kWarps * 32, 0);
+    if (!g_blocks_fwd) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_fwd, k_aev_forward<true>, kWarps * 32, 0);
     const int grid = persistent_grid(c, g_blocks_fwd);
-    k_aev_forward<<<grid, kWarps * 32, 0, c->stream>>>(c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a,
+    auto kern = c->aev.ladder ? k_aev_forward<true> : k_aev_forward<false>;
+    kern<<<grid, kWarps * 32, 0, c->stream>>>(c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a,
                                                                                   c->seg_a, c->d_tri, c->G, c->flags, c->aev_sched, g_sms);
     c->launches += 1;
 }

@@ -212,6 +212,44 @@ int set_layout(nnp_ctx *c, unsigned mask)
     return NNP_OK;
 }
 
+// Gaussian ladder constants (AevParams::ladder).  Shift k = 4m + J of group m relative to the anchor a = 4m + 1:
+//   2^-(w_a - (k-a) d)^2 = 2^-(w_a^2) * 2^(2 (k-a) d w_0) * 2^(-(k-a) d^2 (2 (a-1) + (k-a))),  w_a = w_0 - (a-1) d,
+// the last factor is lad[k].  Used only if the shifts are uniform to fp32 accuracy and every intermediate power
+// stays well inside the fp32 exponent range for r up to the cutoff; NNP_NO_LADDER=1 forces the direct evaluation.
+void setup_ladder(AevParams &a, const nnp_params *p)
+{
+    auto uniform = [](const float *shf, int n, double &step) {
+        step = ((double)shf[n - 1] - (double)shf[0]) / (n - 1);
+        if (!(step > 0.0)) return false;
+        for (int k = 0; k < n; ++k)
+            if (fabs((double)shf[k] - ((double)shf[0] + k * step)) > 2.5e-7 * fabs((double)shf[n - 1])) return false;
+        return true;
+    };
+    double step_r = 0.0, step_a = 0.0;
+    bool ok = uniform(p->shf_r, NNP_NSHF_R, step_r) && uniform(p->shf_a, NNP_NSHF_A, step_a);
+    const double kr = sqrt((double)p->eta_r * 1.4426950408889634), ka = sqrt((double)p->eta_a * 1.4426950408889634);
+    const double dr = kr * step_r, da = ka * step_a;
+    if (ok) {
+        // largest exponents met: Q^2 = 2^(4 d w_0max), raw sums 2^((4 + 16 m_max) d^2); smallest: 2^(-2 d w_0max - ...)
+        const double w0r = kr * ((double)p->rcr - (double)p->shf_r[1]), w0a = ka * ((double)p->rca - (double)p->shf_a[1]);
+        const double lim = 125.0; // fp32 overflows at 2^128
+        ok = 4.0 * dr * w0r < lim && 4.0 * da * w0a < lim && (4.0 + 16.0 * (NNP_NSHF_R / 4 - 1)) * dr * dr < lim - 8.0 &&
+             (4.0 + 16.0 * (NNP_NSHF_A / 4 - 1)) * da * da < lim - 8.0 && p->shf_r[1] > 0.f && p->shf_a[1] > 0.f;
+    }
+    const char *env = getenv("NNP_NO_LADDER");
+    if (env && env[0] == '1') ok = false;
+    a.ladder = ok ? 1 : 0;
+    a.dlt_r = (float)dr; a.dlt_a = (float)da;
+    for (int k = 0; k < NNP_NSHF_R; ++k) {
+        const int an = 4 * (k / 4) + 1, j = k - an;
+        a.lad_r[k] = ok ? (float)exp2(-(double)j * dr * dr * (2.0 * (an - 1) + j)) : 1.0f;
+    }
+    for (int k = 0; k < NNP_NSHF_A; ++k) {
+        const int an = 4 * (k / 4) + 1, j = k - an;
+        a.lad_a[k] = ok ? (float)exp2(-(double)j * da * da * (2.0 * (an - 1) + j)) : 1.0f;
+    }
+}
+
 int check_flags(nnp_ctx *c)
 {
     int h[3];
@@ -432,6 +470,7 @@ const char *nnp_last_error(const nnp_ctx *ctx) { return ctx ? ctx->err.c_str() :
 int64_t nnp_launch_count(const nnp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 int nnp_aev_len(const nnp_ctx *ctx) { return ctx ? ctx->aev_len_full : 0; }
 int nnp_aev_active_columns(const nnp_ctx *ctx) { return ctx ? ctx->aev.aev_len : 0; }
+int nnp_aev_ladder(const nnp_ctx *ctx) { return ctx ? ctx->aev.ladder : 0; }
 
 void nnp_destroy(nnp_ctx *c)
 {
@@ -513,6 +552,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     for (int k = 0; k < NNP_NSHF_R; ++k) a.shf_r[k] = p->shf_r[k];
     for (int k = 0; k < NNP_NSHF_A; ++k) a.shf_a[k] = p->shf_a[k];
     for (int k = 0; k < NNP_NSHF_Z; ++k) { a.cos_z[k] = (float)cos((double)p->shf_z[k]); a.sin_z[k] = (float)sin((double)p->shf_z[k]); }
+    setup_ladder(a, p);
 
     // ---- weights: W [in_pad][out], Wt [out][in_pad], b [out] for every (net, species, layer)
     c->layers = new LayerW[(size_t)c->n_nets * S * NNP_NLAYERS];

@@ -57,6 +57,13 @@ struct AevParams {
     float ka_shf[NNP_NSHF_A];   // ka * shf_a
     float kr;                   // sqrt(eta_r log2 e)
     float kr_shf[NNP_NSHF_R];   // kr * shf_r
+    // Gaussian ladder (aev.cu): with uniformly spaced shifts, exp(-eta (r - Shf_k)^2) for the four shifts k = 4m + J
+    // of a group follows from the anchor k = 4m + 1 by powers of Q = 2^(2 delta w_0): e_k = lad_c[k] e_anchor Q^(J-1),
+    // w_0 = k_ (r - Shf_1), delta = k_ (Shf_1 - Shf_0).  6 (radial) / 4 (angular) exponentials instead of 16 / 8.
+    int ladder;                 // 1: both shift sets are uniform and the powers stay inside fp32 range
+    float dlt_r, dlt_a;         // delta (scaled shift spacing)
+    float lad_r[NNP_NSHF_R];    // constant factors of the deferred scaling, 1 without ladder
+    float lad_a[NNP_NSHF_A];
     int periodic;
     float box[3], inv_box[3];
 };

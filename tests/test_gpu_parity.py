@@ -392,3 +392,37 @@ def test_dense_aev_layout_gives_the_same_result(model1):
         U.assert_parity(E2, F2, ref)
     finally:
         nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- Gaussian ladder vs direct evaluation of the shift sets
+@pytest.mark.parametrize("shifts", ["ani2x_direct", "nonuniform"])
+def test_direct_shift_evaluation(model1, shifts, monkeypatch):
+    """The default path evaluates the uniformly spaced ANI-2x shifts by the ladder recurrence (all other tests);
+    here the direct evaluation: forced for the same constants, and chosen automatically for a non-uniform shift set."""
+    consts, widths, params, om = model1
+    if shifts == "ani2x_direct":
+        monkeypatch.setenv("NNP_NO_LADDER", "1")
+    else:
+        rng = np.random.default_rng(77)
+        consts = dict(consts)
+        consts["shf_r"] = np.float32(consts["shf_r"] + rng.uniform(-0.05, 0.05, 16)).astype(np.float64)
+        consts["shf_a"] = np.float32(consts["shf_a"] + rng.uniform(-0.05, 0.05, 8)).astype(np.float64)
+        om = orc.OracleModel(consts, widths, params, 1)
+    sp, xyz, box = inputs.solvated_chain(n_solute=300, L=22.0, seed=9)
+    sp = sp.copy(); sp[:14] = np.arange(14) % 7
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp))
+    try:
+        assert nnp.nnp_aev_ladder(ctx) == 0
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, nbr_method=1))
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_ladder_is_the_default_for_ani2x_constants(model1):
+    consts, widths, params, om = model1
+    ctx = U.gpu_create(consts, widths, params, 1, 64)
+    try:
+        assert nnp.nnp_aev_ladder(ctx) == 1
+    finally:
+        nnp.nnp_destroy(ctx)
