@@ -277,7 +277,20 @@ def run_ours(args):
     return 0
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch [bytes] of each stage's kernel on the 98,304-atom workload,
+# from the one `ncu --set full` capture summarised in profiles/r01_ncu_full_3xtf32.md (3xTF32 mode).
+TRAFFIC_NCU = {"aev_forward": 68.3e6, "aev_backward_scatter": 110.6e6, "mlp_fwd_l1": 91.2e6, "mlp_fwd_l2": 135.2e6,
+               "mlp_fwd_l3_out": 100.0e6, "mlp_bwd_l3": 163.9e6, "mlp_bwd_l2": 220.3e6, "mlp_bwd_l1_dEdG": 107.3e6}
+
+
 def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
+    r = _roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad)
+    if n == 3 * N_WATERS and mm_mode == 1:
+        r["traffic"] = TRAFFIC_NCU.get(stage)
+    return r
+
+
+def _roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
     """Roofline entry for the dominant stage (DESIGN.md 'Kernels and rooflines' gives the per-atom figures)."""
     from paper_2405_01491_b200 import inputs
     W = inputs.WIDTHS
