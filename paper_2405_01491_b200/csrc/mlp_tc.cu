@@ -17,6 +17,7 @@
 #include <cuda.h>
 
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "nnp_internal.cuh"
@@ -54,6 +55,8 @@ struct TcBatch {
     int n_groups;
     int tile_off[NNP_MAX_SPECIES]; // prefix sum of (m tiles x n tiles) per group
     int n_tiles;
+    int tile_cost[NNP_MAX_SPECIES - 1]; // bytes moved per tile of the group, in units of 128 B
+    long long cost_total;
     float alpha;
 #ifdef NNP_TC_TRACE
     long long *trace; // [it][8] clock64 stamps of CTA 0
@@ -209,6 +212,17 @@ __device__ __forceinline__ TileCoord tile_coord(const TcBatch &batch, int t)
     return TileCoord{gi, mt * TILE_M, nt * batch.g[gi].NT};
 }
 
+// first tile whose cumulative cost reaches x
+__device__ __forceinline__ int tile_at_cost(const TcBatch &batch, long long x)
+{
+    for (int gi = 0; gi < batch.n_groups; ++gi) {
+        const long long w = batch.tile_cost[gi], n = batch.tile_off[gi + 1] - batch.tile_off[gi];
+        if (x < w * n) return batch.tile_off[gi] + (int)((x + w - 1) / w);
+        x -= w * n;
+    }
+    return batch.n_tiles;
+}
+
 // Persistent: CTA c processes the contiguous tile range [c T / G, (c+1) T / G); the two n-halves of an m-tile are
 // adjacent, so the second read of the A tile hits L2.  The smem/TMEM-A ring (4 stages) and the two accumulator
 // buffers run across tile boundaries: the epilogue of tile i overlaps the conversion + MMAs of tile i+1.
@@ -225,8 +239,9 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
     const uint32_t tmem_slot = bar_base + 128;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int t_beg = (int)(((long long)blockIdx.x * batch.n_tiles) / gridDim.x);
-    const int t_end = (int)(((long long)(blockIdx.x + 1) * batch.n_tiles) / gridDim.x);
+    // contiguous tile ranges of equal COST, not equal count: a hydrogen tile (K = 256) is 1/3 dearer than an oxygen tile
+    const int t_beg = tile_at_cost(batch, ((long long)blockIdx.x * batch.cost_total) / gridDim.x);
+    const int t_end = blockIdx.x + 1 == gridDim.x ? batch.n_tiles : tile_at_cost(batch, ((long long)(blockIdx.x + 1) * batch.cost_total) / gridDim.x);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -571,6 +586,11 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
         t.n_tiles_n = g.N / NT;
         tb.tile_off[i] = tiles;
         tiles += nnp_div_up(g.M, TILE_M) * t.n_tiles_n;
+        // bytes through the SM in units of 128 B (the kernel is bound by L2 -> SM traffic): per K block the A tile and the
+        // hi/lo weight tiles, plus the output tile (read and written by the in-place epilogues)
+        // ... plus a fixed 1000 per tile for the pipeline fill / accumulator hand-over (swept 0..8000 on the 98k water box)
+        tb.tile_cost[i] = g.K / BLOCK_K * (TILE_M + 2 * NT) + ((epi == EPI_DCELU || epi == EPI_ACCUM) ? 8 : 4) * NT + 1000;
+        tb.cost_total += (long long)tb.tile_cost[i] * (tiles - tb.tile_off[i]);
     }
     tb.n_groups = b.n_groups;
     tb.tile_off[b.n_groups] = tiles;
