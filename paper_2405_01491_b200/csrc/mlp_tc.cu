@@ -27,17 +27,16 @@ namespace {
 constexpr int TILE_M = 128;
 constexpr int BLOCK_K = 32;               // fp32 elements = one 128-byte swizzle row
 constexpr int UMMA_K = 8;                 // tf32
-constexpr int NT_MAX = 128;               // columns per output tile (wider layers are split in two halves)
-constexpr int STAGES = 4;
+constexpr int NT_MAX = 192;               // columns per output tile = the layer width up to 192; wider layers in equal parts
+constexpr int STAGES_MAX = 4;             // shared-memory ring: 4 stages of 48 KiB (NT <= 128) or 3 of up to 64 KiB
 constexpr int A_TILE_BYTES = TILE_M * BLOCK_K * 4;          // 16 KiB
-constexpr int B_TILE_BYTES_MAX = NT_MAX * BLOCK_K * 4;      // 16 KiB
-constexpr int STAGE_BYTES = A_TILE_BYTES + 2 * B_TILE_BYTES_MAX; // 48 KiB
 constexpr int EPI_STG_LD = 36;                                   // floats per staged row (16-byte aligned, conflict-free)
 constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;               // per epilogue warp: one 32 x 32 chunk
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 4 * EPI_STG_BYTES;
+constexpr int SMEM_FIXED = 1024 /*align*/ + 256 /*barriers*/ + 4 * EPI_STG_BYTES;
+constexpr int SMEM_LIMIT = 227 * 1024;
 constexpr int TMEM_COLS = 512;
-constexpr int TMEM_ACC_STRIDE = 128;      // two accumulator buffers at columns 0 and 128
-constexpr int TMEM_A_COL0 = 256;          // A staging: stage s -> hi at 256 + 64 s, lo at 256 + 64 s + 32
+// TMEM: two accumulator buffers at columns 0 and acc_stride (128 / 160 / 192), behind them a_slots = 4 / 3 / 2 A slots
+// (hi 32 + lo 32 columns); K block `it` uses slot it % a_slots and shared-memory stage it % stages (a_slots <= stages).
 constexpr int THREADS = 448;              // warp 0 TMA, warp 1 MMA, warps 2-9 converters (two groups), warps 10-13 epilogue
 
 struct TcGroup {
@@ -57,6 +56,8 @@ struct TcBatch {
     int n_tiles;
     int tile_cost[NNP_MAX_SPECIES - 1]; // bytes moved per tile of the group, in units of 128 B
     long long cost_total;
+    int stages, stage_bytes, b_tile_bytes; // ring depth; 16 KiB + 2 * b_tile_bytes; nt_max * 128
+    int acc_stride, a_slots;
     float alpha;
 #ifdef NNP_TC_TRACE
     long long *trace; // [it][8] clock64 stamps of CTA 0
@@ -232,7 +233,10 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
 {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+    const int S = batch.stages, T = batch.a_slots;
+    const uint32_t stage_bytes = (uint32_t)batch.stage_bytes, blo_off = A_TILE_BYTES + (uint32_t)batch.b_tile_bytes;
+    const uint32_t a_col0 = 2u * (uint32_t)batch.acc_stride;
+    const uint32_t bar_base = smem_base + S * stage_bytes;
     // barriers (8 B each): full[4] @0, aready[4] @32, empty[4] @64, acc_full[2] @96, acc_empty[2] @112; tmem ptr @128
     const uint32_t bar_full = bar_base, bar_aready = bar_base + 32, bar_empty = bar_base + 64;
     const uint32_t bar_accf = bar_base + 96, bar_acce = bar_base + 112;
@@ -244,7 +248,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
     const int t_end = blockIdx.x + 1 == gridDim.x ? batch.n_tiles : tile_at_cost(batch, ((long long)(blockIdx.x + 1) * batch.cost_total) / gridDim.x);
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) {
+        for (int s = 0; s < S; ++s) {
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_aready + 8 * s, 129); // 128 converter threads + the producer's expect_tx for the B tiles
             mbar_init(bar_empty + 8 * s, 1);
@@ -275,17 +279,17 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 const uint32_t tx_b = (SPLIT3 ? 2u : 1u) * (uint32_t)g.NT * BLOCK_K * 4u;
                 const int num_kb = g.K / BLOCK_K;
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
-                    const int s = it % STAGES;
-                    const uint32_t ph = (it / STAGES) & 1;
+                    const int s = it % S;
+                    const uint32_t ph = (it / S) & 1;
                     mbar_wait(bar_empty + 8 * s, ph ^ 1);
                     TRACE(0);
-                    const uint32_t stage = smem_base + s * STAGE_BYTES;
+                    const uint32_t stage = smem_base + s * stage_bytes;
                     // A -> full[s] (wakes the converters); B -> aready[s], the one barrier the MMA thread waits on
                     mbar_expect_tx(bar_full + 8 * s, A_TILE_BYTES);
                     tma_load_2d(stage, &g.mapA, kb * BLOCK_K, tc.m0, bar_full + 8 * s);
                     mbar_expect_tx(bar_aready + 8 * s, tx_b);
                     tma_load_2d(stage + A_TILE_BYTES, &g.mapBhi, kb * BLOCK_K, tc.n0, bar_aready + 8 * s);
-                    if (SPLIT3) tma_load_2d(stage + A_TILE_BYTES + B_TILE_BYTES_MAX, &g.mapBlo, kb * BLOCK_K, tc.n0, bar_aready + 8 * s);
+                    if (SPLIT3) tma_load_2d(stage + blo_off, &g.mapBlo, kb * BLOCK_K, tc.n0, bar_aready + 8 * s);
                 }
             }
         }
@@ -301,21 +305,21 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 const int num_kb = g.K / BLOCK_K;
                 const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(g.NT >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
                 const int b = lt & 1;
-                const uint32_t acc = tmem_base + b * TMEM_ACC_STRIDE;
+                const uint32_t acc = tmem_base + (uint32_t)(b * batch.acc_stride);
                 mbar_wait(bar_acce + 8 * b, ((lt >> 1) & 1) ^ 1); // epilogue has drained this accumulator buffer
                 TRACE(6);
                 tc_fence_after();
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
-                    const int s = it % STAGES;
-                    const uint32_t ph = (it / STAGES) & 1;
+                    const int s = it % S;
+                    const uint32_t ph = (it / S) & 1;
                     TRACE(3);
                     mbar_wait(bar_aready + 8 * s, ph); // B tiles landed and A converted into TMEM
                     TRACE(4);
                     tc_fence_after();
-                    const uint32_t stage = smem_base + s * STAGE_BYTES;
+                    const uint32_t stage = smem_base + s * stage_bytes;
                     const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
-                    const uint64_t dlo = make_kmajor_sw128_desc(stage + A_TILE_BYTES + B_TILE_BYTES_MAX);
-                    const uint32_t a_hi = tmem_base + TMEM_A_COL0 + 64 * s, a_lo = a_hi + 32;
+                    const uint64_t dlo = make_kmajor_sw128_desc(stage + blo_off);
+                    const uint32_t a_hi = tmem_base + a_col0 + 64u * (it % (uint32_t)T), a_lo = a_hi + 32;
                     if (elect_one()) {
 #pragma unroll
                         for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
@@ -350,11 +354,16 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             const int num_kb = batch.g[tc.gi].K / BLOCK_K;
             for (int kb = 0; kb < num_kb; ++kb, ++it) {
                 if ((int)(it & 1) != cgroup) continue;
-                const int s = it % STAGES;
-                const uint32_t ph = (it / STAGES) & 1;
+                const int s = it % S;
+                const uint32_t ph = (it / S) & 1;
+                if (T < S && it >= (uint32_t)T) { // fewer TMEM slots than stages: the slot is free once the MMAs of K block it - T are done
+                    const uint32_t jt = it - (uint32_t)T;
+                    mbar_wait(bar_empty + 8 * (jt % S), (jt / S) & 1);
+                    tc_fence_after();
+                }
                 mbar_wait(bar_full + 8 * s, ph);
                 if (threadIdx.x == 64 || threadIdx.x == 192) TRACE(1);
-                const uint32_t arow = smem_base + s * STAGE_BYTES + row * 128;
+                const uint32_t arow = smem_base + s * stage_bytes + row * 128;
                 uint32_t hi[32], lo[32];
 #pragma unroll
                 for (int c = 0; c < 8; ++c) {
@@ -369,8 +378,9 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                         if (SPLIT3) lo[4 * c + e] = tf32_round(x[e] - __uint_as_float(h));
                     }
                 }
-                tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s, hi);
-                if (SPLIT3) tmem_st32(lane_addr + TMEM_A_COL0 + 64 * s + 32, lo);
+                const uint32_t slot = lane_addr + a_col0 + 64u * (it % (uint32_t)T);
+                tmem_st32(slot, hi);
+                if (SPLIT3) tmem_st32(slot + 32, lo);
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 mbar_arrive(bar_aready + 8 * s);
@@ -438,7 +448,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 for (int h = 0; h < 2; ++h) {
                     if (h * 16 >= w) break;
                     uint32_t acc[16];
-                    tmem_ld16(lane_addr + b * TMEM_ACC_STRIDE + c0 + h * 16, acc);
+                    tmem_ld16(lane_addr + (uint32_t)(b * batch.acc_stride) + c0 + h * 16, acc);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #ifdef NNP_TC_TRACE
                     if (threadIdx.x == 320 && c0 == 0 && h == 0) { const int it = lt * (g.K / BLOCK_K) + 2; TRACE(7); }
@@ -545,12 +555,13 @@ void launch(cudaStream_t st, const TcBatch &b, int tiles, bool split3)
         if (g_num_sms <= 0) g_num_sms = 148;
     }
     const int grid = tiles < g_num_sms ? tiles : g_num_sms; // persistent: one CTA per SM
+    const int smem = b.stages * b.stage_bytes + SMEM_FIXED;
     if (split3) {
-        cudaFuncSetAttribute(k_gemm_tc<EPI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        k_gemm_tc<EPI, true><<<grid, THREADS, SMEM_BYTES, st>>>(b);
+        cudaFuncSetAttribute(k_gemm_tc<EPI, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_LIMIT);
+        k_gemm_tc<EPI, true><<<grid, THREADS, smem, st>>>(b);
     } else {
-        cudaFuncSetAttribute(k_gemm_tc<EPI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        k_gemm_tc<EPI, false><<<grid, THREADS, SMEM_BYTES, st>>>(b);
+        cudaFuncSetAttribute(k_gemm_tc<EPI, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_LIMIT);
+        k_gemm_tc<EPI, false><<<grid, THREADS, smem, st>>>(b);
     }
 }
 
@@ -562,14 +573,20 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     TcBatch tb;
     memset(&tb, 0, sizeof(tb));
     tb.alpha = b.alpha;
-    int tiles = 0;
+    int tiles = 0, nt_max = 16;
+    // Full-width tiles (one A load and conversion per 128 rows) where every group of the launch fits in 192 columns;
+    // a launch with a wider layer splits it into <= 128-column parts, and then the 48 KiB stages / 4-deep ring serve
+    // all its groups better than 64 KiB stages / 3-deep (measured on the 98k water box: 0.363 -> 0.344 ms over the six GEMMs)
+    int nt_cap = NT_MAX;
+    for (int i = 0; i < b.n_groups; ++i)
+        if (b.g[i].N > NT_MAX) nt_cap = 128;
     for (int i = 0; i < b.n_groups; ++i) {
         const GemmGroup &g = b.g[i];
         TcGroup &t = tb.g[i];
         if (!g.Bt_hi || !g.Bt_lo) { c->err = "tensor-core path: weight operand has no tf32 split"; return NNP_EINVAL; }
-        int NT = g.N;                       // <= 128 columns per tile; wider layers in equal parts that are multiples of 16
+        int NT = g.N;                       // <= 192 columns per tile; wider layers in equal parts that are multiples of 16
         int parts = 1;
-        while (NT > NT_MAX || (g.N % parts) || (NT % 16)) {
+        while (NT > nt_cap || (g.N % parts) || (NT % 16)) {
             ++parts;
             if (parts > 64) { c->err = "tensor-core path: unsupported GEMM width"; return NNP_EINVAL; }
             NT = g.N / parts;
@@ -584,6 +601,7 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
         t.M = g.M; t.N = g.N; t.K = g.K; t.ldc = g.ldc;
         t.NT = NT;
         t.n_tiles_n = g.N / NT;
+        if (NT > nt_max) nt_max = NT;
         tb.tile_off[i] = tiles;
         tiles += nnp_div_up(g.M, TILE_M) * t.n_tiles_n;
         // bytes through the SM in units of 128 B (the kernel is bound by L2 -> SM traffic): per K block the A tile and the
@@ -596,6 +614,13 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     tb.tile_off[b.n_groups] = tiles;
     tb.n_tiles = tiles;
     if (tiles == 0) return NNP_OK;
+    tb.b_tile_bytes = nt_max * BLOCK_K * 4;
+    tb.stage_bytes = A_TILE_BYTES + 2 * tb.b_tile_bytes;       // multiples of 1 KiB: swizzle atoms stay aligned
+    tb.stages = (SMEM_LIMIT - SMEM_FIXED) / tb.stage_bytes;
+    if (tb.stages > STAGES_MAX) tb.stages = STAGES_MAX;
+    tb.acc_stride = nt_max <= 128 ? 128 : 192;
+    tb.a_slots = (TMEM_COLS - 2 * tb.acc_stride) / 64;
+    if (tb.a_slots > tb.stages) tb.a_slots = tb.stages;
 #ifdef NNP_TC_TRACE
     static long long *d_trace = nullptr;
     static int traced = 0;
