@@ -169,6 +169,8 @@ def run_ours(args):
     # ---- device-resident run (value)
     nnp.nnp_set_system(ctx, n, d_sp, d_x, box)
     nnp.nnp_md_init(ctx, d_v, DT_FS, SKIN)
+    if args.langevin > 0:      # the paper's benchmarks run Langevin 300 K; not the default workload
+        nnp.nnp_md_set_langevin(ctx, args.langevin, inputs.KB * T_KELVIN, inputs.SEED0 + 7 + rank)
     nnp.nnp_md_step(ctx, W)
     nnp.nnp_sync(ctx)
     o_ep = torch.zeros(1, dtype=torch.float64, device=dev)
@@ -343,6 +345,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--cpu-waters", type=int, default=4096)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--langevin", type=float, default=0.0, help="friction in 1/fs: BAOAB Langevin at 300 K instead of velocity Verlet")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

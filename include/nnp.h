@@ -125,6 +125,15 @@ int nnp_get_atomic_energies(nnp_ctx *ctx, float *d_e_atom);
 int nnp_md_init(nnp_ctx *ctx, const float *d_vel, float dt_fs, float skin);
 int nnp_md_step(nnp_ctx *ctx, int n_steps);
 
+/* Langevin dynamics with the BAOAB splitting ("Langevin dynamics (using the BAOAB scheme)", the
+ * setting of the paper's benchmarks, L323).  After nnp_md_init; from then on nnp_md_step does
+ *   v += dt/2 a;  x += dt/2 v;  v = c1 v + c2_s xi;  x += dt/2 v;  [rebuild test]  forces;  v += dt/2 a
+ * with c1 = exp(-gamma dt), c2_s = sqrt((1 - c1^2) kT accel_conv / m_s), xi three standard normals per atom and step
+ * from Philox4x32-10 with counter (original atom index, step since nnp_md_init, 0, 0) and key = seed (uniforms
+ * ((r >> 9) + 1/2) 2^-23, Box-Muller), so a trajectory does not depend on how the steps are split over calls.
+ * gamma [1/fs] = 0 switches back to velocity Verlet.  kT in energy units.  nnp_md_init resets to velocity Verlet. */
+int nnp_md_set_langevin(nnp_ctx *ctx, float gamma, float kT, uint64_t seed);
+
 /* Copies out the current state in original order; any pointer may be NULL.  d_epot/d_ekin: fp64 scalars
  * (potential energy of the last force evaluation, kinetic energy after the last step, energy units);
  * d_n_rebuilds: list builds since nnp_md_init (the initial one included).  Asynchronous. */

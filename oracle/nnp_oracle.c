@@ -547,6 +547,89 @@ int orc_md(const orc_model *m, int n, const int *species, double *xyz, double *v
     return rc;
 }
 
+/* ---- NEXT-1: Langevin dynamics, BAOAB splitting.  PAPER.md L307: the MD engine offers
+ * "Langevin dynamics (using the BAOAB scheme)"; L323: every benchmark of the paper runs "Langevin 300 K".
+ * Per step (Leimkuhler & Matthews 2013, the scheme the paper names):
+ *   B: v += dt/2 a(F)      A: x += dt/2 v      O: v = c1 v + c2_s xi,  c1 = exp(-gamma dt),
+ *   A: x += dt/2 v         [rebuild test]      F(x)     B: v += dt/2 a(F)      c2_s = sqrt((1 - c1^2) kT accel_conv / m_s)
+ * xi: three independent standard normals per atom and step from a counter-based generator, so that the CUDA path can
+ * draw the same numbers: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11) with counter (atom index, step, 0, 0) and
+ * key (seed low, seed high); uniforms u = ((r >> 9) + 1/2) 2^-23 (exact in fp32 and fp64), Box-Muller
+ * xi_0 = sqrt(-2 ln u_0) cos(2 pi u_1), xi_1 = sqrt(-2 ln u_0) sin(2 pi u_1), xi_2 = sqrt(-2 ln u_2) cos(2 pi u_3).
+ * gamma = 0 gives c1 = 1, c2 = 0: velocity Verlet (pinned against orc_md). */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        if (round) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+void orc_langevin_normals(uint32_t atom, uint32_t step, uint64_t seed, double xi[3])
+{
+    const uint32_t ctr[4] = {atom, step, 0u, 0u}, key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t r[4];
+    double u[4];
+    orc_philox4x32_10(ctr, key, r);
+    for (int q = 0; q < 4; ++q) u[q] = ((double)(r[q] >> 9) + 0.5) / 8388608.0;
+    const double a = sqrt(-2.0 * log(u[0])), b = sqrt(-2.0 * log(u[2]));
+    xi[0] = a * cos(2.0 * M_PI * u[1]);
+    xi[1] = a * sin(2.0 * M_PI * u[1]);
+    xi[2] = b * cos(2.0 * M_PI * u[3]);
+}
+
+/* Same arguments as orc_md plus gamma [1/time], kT [energy], seed, step0 (counter of the first step). */
+int orc_md_langevin(const orc_model *m, int n, const int *species, double *xyz, double *vel, double *F_io, int have_forces,
+                    const double *mass /*[S]*/, const double *box, double dt, double accel_conv, int n_steps, double skin,
+                    int nbr_method, double gamma, double kT, uint64_t seed, uint32_t step0, double *epot, double *ekin,
+                    int *n_rebuilds)
+{
+    double E;
+    int rc = 0, nreb = 1;
+    const double c1 = exp(-gamma * dt);
+    double *xref = (double *)malloc(sizeof(double) * 3 * (size_t)n);
+    memcpy(xref, xyz, sizeof(double) * 3 * (size_t)n);
+    if (!have_forces || epot) {
+        rc = orc_energy_forces(m, n, species, xyz, box, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL);
+        if (rc) { free(xref); return rc; }
+    }
+    for (int step = 0;; ++step) {
+        if (ekin) {
+            double k = 0.0;
+            for (int i = 0; i < n; ++i)
+                k += 0.5 * mass[species[i]] * (vel[3 * i] * vel[3 * i] + vel[3 * i + 1] * vel[3 * i + 1] + vel[3 * i + 2] * vel[3 * i + 2]);
+            ekin[step] = k / accel_conv;
+        }
+        if (epot) epot[step] = E;
+        if (step == n_steps) break;
+        for (int i = 0; i < n; ++i) {
+            const double ms = mass[species[i]];
+            const double c2 = sqrt((1.0 - c1 * c1) * kT * accel_conv / ms);
+            double xi[3];
+            orc_langevin_normals((uint32_t)i, step0 + (uint32_t)step, seed, xi);
+            for (int c = 0; c < 3; ++c) {
+                vel[3 * i + c] += 0.5 * dt * accel_conv * F_io[3 * i + c] / ms; /* B */
+                xyz[3 * i + c] += 0.5 * dt * vel[3 * i + c];                    /* A */
+                vel[3 * i + c] = c1 * vel[3 * i + c] + c2 * xi[c];              /* O */
+                xyz[3 * i + c] += 0.5 * dt * vel[3 * i + c];                    /* A */
+            }
+        }
+        if (orc_needs_rebuild(n, xyz, xref, skin)) { memcpy(xref, xyz, sizeof(double) * 3 * (size_t)n); ++nreb; }
+        rc = orc_energy_forces(m, n, species, xyz, box, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL);
+        if (rc) break;
+        for (int i = 0; i < n; ++i)
+            for (int c = 0; c < 3; ++c) vel[3 * i + c] += 0.5 * dt * accel_conv * F_io[3 * i + c] / mass[species[i]]; /* B */
+    }
+    if (n_rebuilds) *n_rebuilds = nreb;
+    free(xref);
+    return rc;
+}
+
 int orc_num_threads(void)
 {
 #ifdef _OPENMP

@@ -194,3 +194,44 @@ def md(model, species, xyz, vel, mass, box, dt, accel_conv, n_steps, skin=0.5, n
     if rc != 0:
         raise RuntimeError("orc_md failed: %d" % rc)
     return {"xyz": x, "vel": v, "F": F, "epot": epot, "ekin": ekin, "n_rebuilds": nreb.value}
+
+
+def philox4x32_10(ctr, key):
+    """Philox4x32-10 block (4 x uint32) for counter ctr[4] and key[2]; test hook of the Langevin generator."""
+    c = (C.c_uint32 * 4)(*[int(x) & 0xffffffff for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) & 0xffffffff for x in key])
+    out = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, out)
+    return [int(x) for x in out]
+
+
+def langevin_normals(atom, step, seed):
+    xi = (C.c_double * 3)()
+    lib().orc_langevin_normals(C.c_uint32(atom), C.c_uint32(step), C.c_uint64(seed), xi)
+    return np.array(list(xi))
+
+
+def md_langevin(model, species, xyz, vel, mass, box, dt, accel_conv, n_steps, gamma, kT, seed, step0=0, skin=0.5,
+                nbr_method=0, forces=None):
+    """NEXT-1: BAOAB Langevin dynamics.  Returns the same dict as md()."""
+    species = np.ascontiguousarray(species, dtype=np.int32)
+    x = np.array(xyz, dtype=np.float64, order="C")
+    v = np.array(vel, dtype=np.float64, order="C")
+    n = x.shape[0]
+    F = np.zeros((n, 3)) if forces is None else np.array(forces, dtype=np.float64, order="C")
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    boxa = None if box is None else np.ascontiguousarray(box, dtype=np.float64)
+    epot = np.zeros(n_steps + 1)
+    ekin = np.zeros(n_steps + 1)
+    nreb = C.c_int(0)
+    f = lib().orc_md_langevin
+    f.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
+                  C.c_double, C.c_double, C.c_int, C.c_double, C.c_int, C.c_double, C.c_double, C.c_uint64, C.c_uint32,
+                  C.c_void_p, C.c_void_p, C.c_void_p]
+    rc = f(C.cast(C.byref(model.c), C.c_void_p), n, species.ctypes.data, x.ctypes.data, v.ctypes.data, F.ctypes.data,
+           int(forces is not None), mass.ctypes.data, None if boxa is None else boxa.ctypes.data, float(dt),
+           float(accel_conv), int(n_steps), float(skin), int(nbr_method), float(gamma), float(kT), int(seed), int(step0),
+           epot.ctypes.data, ekin.ctypes.data, C.cast(C.byref(nreb), C.c_void_p))
+    if rc != 0:
+        raise RuntimeError("orc_md_langevin failed: %d" % rc)
+    return {"xyz": x, "vel": v, "F": F, "epot": epot, "ekin": ekin, "n_rebuilds": nreb.value}

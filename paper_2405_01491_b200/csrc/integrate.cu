@@ -28,11 +28,65 @@ __global__ void k_kick_drift(int n, float4 *__restrict__ pos, float4 *__restrict
     if (__syncthreads_or(moved) && threadIdx.x == 0) flags[1] = 1;
 }
 
+// Philox4x32-10 (Salmon et al., SC'11): counter (atom, step, 0, 0), key = seed.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        if (round) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Langevin dynamics, BAOAB ("Langevin dynamics (using the BAOAB scheme)", L323):
+// B: v += dt/2 a(F); A: x += dt/2 v; O: v = c1 v + c2[species] xi; A: x += dt/2 v; then the rebuild test.
+// xi: three standard normals per atom and step, keyed by the ORIGINAL atom index and the device-side step counter
+// flags[4] (so the numbers do not depend on the internal atom order or on how many steps one call enqueues):
+// u = ((r >> 9) + 1/2) 2^-23 (exact in fp32), Box-Muller.  gamma = 0 never comes here (velocity Verlet kernel above).
+__global__ void k_kick_drift_langevin(int n, float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ frc,
+                                      const float4 *__restrict__ xref, const int *__restrict__ spc, const int *__restrict__ orig,
+                                      const float *__restrict__ inv_mass_conv, const float *__restrict__ c2_s, float c1, float dt,
+                                      float half_skin2, uint32_t seed_lo, uint32_t seed_hi, int *__restrict__ flags)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < n) {
+        const int s = spc[i];
+        const float k = 0.5f * dt * inv_mass_conv[s], hdt = 0.5f * dt, c2 = c2_s[s];
+        float4 v = vel[i], x = pos[i];
+        const float4 f = frc[i], r = xref[i];
+        v.x = fmaf(k, f.x, v.x); v.y = fmaf(k, f.y, v.y); v.z = fmaf(k, f.z, v.z);
+        x.x = fmaf(hdt, v.x, x.x); x.y = fmaf(hdt, v.y, x.y); x.z = fmaf(hdt, v.z, x.z);
+        uint32_t rn[4];
+        philox4x32_10((uint32_t)orig[i], (uint32_t)flags[4], 0u, 0u, seed_lo, seed_hi, rn);
+        float u[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) u[q] = ((float)(rn[q] >> 9) + 0.5f) * 1.1920928955078125e-07f; // 2^-23
+        const float a = sqrtf(-2.0f * logf(u[0])), b = sqrtf(-2.0f * logf(u[2]));
+        float sn, cs, cs2;
+        sincospif(2.0f * u[1], &sn, &cs);
+        cs2 = cospif(2.0f * u[3]);
+        v.x = fmaf(c1, v.x, c2 * (a * cs)); v.y = fmaf(c1, v.y, c2 * (a * sn)); v.z = fmaf(c1, v.z, c2 * (b * cs2));
+        x.x = fmaf(hdt, v.x, x.x); x.y = fmaf(hdt, v.y, x.y); x.z = fmaf(hdt, v.z, x.z);
+        vel[i] = v;
+        pos[i] = x;
+        const float dx = x.x - r.x, dy = x.y - r.y, dz = x.z - r.z;
+        moved = dx * dx + dy * dy + dz * dz > half_skin2;
+    }
+    if (__syncthreads_or(moved) && threadIdx.x == 0) flags[1] = 1;
+}
+
 // v += dt/2 a(F); kinetic energy sum_i m v^2 / (2 accel_conv) accumulated in fp64.
 __global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restrict__ frc, const int *__restrict__ spc,
                           const float *__restrict__ inv_mass_conv, const float *__restrict__ mass, float dt,
-                          float inv_accel_conv, double *__restrict__ ekin)
+                          float inv_accel_conv, double *__restrict__ ekin, int *__restrict__ step_ctr)
 {
+    if (step_ctr && blockIdx.x == 0 && threadIdx.x == 0) *step_ctr += 1; // Langevin step counter (read by the next drift kernel)
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     float ke = 0.f;
     if (i < n) {
@@ -103,16 +157,23 @@ __global__ void k_permute_in3(int n, const float *__restrict__ src, const int *_
 void nnp_launch_kick_drift(nnp_ctx *c)
 {
     const float hs = 0.5f * c->skin;
+    if (c->lgv_gamma > 0.f) {
+        k_kick_drift_langevin<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(
+            c->n, c->pos, c->vel, c->frc, c->xref, c->spc, c->orig, c->d_inv_mass_conv, c->d_lgv_c2, c->lgv_c1, c->dt, hs * hs,
+            (uint32_t)c->lgv_seed, (uint32_t)(c->lgv_seed >> 32), c->flags);
+        c->launches += 1;
+        return;
+    }
     k_kick_drift<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->pos, c->vel, c->frc, c->xref, c->spc,
                                                           c->d_inv_mass_conv, c->dt, hs * hs, c->flags);
     c->launches += 1;
 }
 
-void nnp_launch_kick_ke(nnp_ctx *c)
+void nnp_launch_kick_ke(nnp_ctx *c, int count_step)
 {
     cudaMemsetAsync(c->ekin, 0, sizeof(double), c->stream);
     k_kick_ke<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->vel, c->frc, c->spc, c->d_inv_mass_conv, c->d_mass,
-                                                       c->dt, 1.0f / c->accel_conv, c->ekin);
+                                                       c->dt, 1.0f / c->accel_conv, c->ekin, count_step ? c->flags + 4 : nullptr);
     c->launches += 1;
 }
 

@@ -444,7 +444,7 @@ int build_md_graph(nnp_ctx *c)
         if (cudaStreamUpdateCaptureDependencies(main_stream, &cnode, 1, cudaStreamSetCaptureDependencies) != cudaSuccess) { rc = NNP_ECUDA; break; }
         rc = run_forces(c);
         if (rc) break;
-        nnp_launch_kick_ke(c);
+        nnp_launch_kick_ke(c, 1);
     } while (0);
     cudaGraph_t out = nullptr;
     cudaError_t e = capturing ? cudaStreamEndCapture(main_stream, &out) : cudaSuccess;
@@ -479,7 +479,7 @@ void nnp_destroy(nnp_ctx *c)
     cudaStreamSynchronize(c->stream);
     drop_md_graph(c);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
-    void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
+    void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->d_lgv_c2, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags, c->aev_sched,
@@ -642,6 +642,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     TRY(dev_alloc(c, &c->d_inv_mass_conv, NNP_MAX_SPECIES));
     TRY(dev_alloc(c, &c->d_mass, NNP_MAX_SPECIES));
     TRY(dev_alloc(c, &c->d_e_shift, NNP_MAX_SPECIES));
+    TRY(dev_alloc(c, &c->d_lgv_c2, NNP_MAX_SPECIES));
     TRYCU(cudaMemcpy(c->d_inv_mass_conv, imc, sizeof(imc), cudaMemcpyHostToDevice));
     TRYCU(cudaMemcpy(c->d_mass, ms, sizeof(ms), cudaMemcpyHostToDevice));
     TRYCU(cudaMemcpy(c->d_e_shift, es, sizeof(es), cudaMemcpyHostToDevice));
@@ -815,8 +816,9 @@ int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
     CU(c, cudaSetDevice(c->device));
     nnp_launch_permute_in3(c, d_vel, c->vel);
     c->dt = dt_fs;
+    c->lgv_gamma = 0.f; // velocity Verlet until nnp_md_set_langevin
     drop_md_graph(c);
-    CU(c, cudaMemsetAsync(c->flags + 1, 0, sizeof(int) * 2, c->stream)); // rebuild request and counter
+    CU(c, cudaMemsetAsync(c->flags + 1, 0, sizeof(int) * 4, c->stream)); // rebuild request and counter, Langevin step counter
     int rc = nnp_build_neighbors(c, skin);
     if (rc) return rc;
     // the initial build counts as rebuild 1 (k_finish_build)
@@ -824,9 +826,26 @@ int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
     if (rc) return rc;
     const float dt = c->dt;
     c->dt = 0.f;
-    nnp_launch_kick_ke(c); // kinetic energy of the initial velocities
+    nnp_launch_kick_ke(c, 0); // kinetic energy of the initial velocities
     c->dt = dt;
     c->md_ready = 1;
+    return NNP_OK;
+}
+
+int nnp_md_set_langevin(nnp_ctx *c, float gamma, float kT, uint64_t seed)
+{
+    if (!c) return NNP_EINVAL;
+    if (!(gamma >= 0.f) || !(kT >= 0.f)) NNP_FAIL(c, NNP_EINVAL, "gamma and kT must be >= 0");
+    if (!c->md_ready) NNP_FAIL(c, NNP_ESTALE, "nnp_md_init first");
+    CU(c, cudaSetDevice(c->device));
+    c->lgv_gamma = gamma; c->lgv_kT = kT; c->lgv_seed = seed;
+    const double c1 = exp(-(double)gamma * (double)c->dt);
+    c->lgv_c1 = (float)c1;
+    float c2[NNP_MAX_SPECIES] = {0};
+    for (int s = 0; s < c->S; ++s) c2[s] = (float)sqrt((1.0 - c1 * c1) * (double)kT * (double)c->accel_conv / (double)c->mass[s]);
+    CU(c, cudaMemcpyAsync(c->d_lgv_c2, c2, sizeof(c2), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream)); // c2 is a stack array
+    drop_md_graph(c);                        // the drift kernel and its constants are baked into the graph
     return NNP_OK;
 }
 
@@ -853,7 +872,7 @@ int nnp_md_step(nnp_ctx *c, int n_steps)
         nnp_prof_mark(c, 1);
         int rc = run_forces(c);
         if (rc) { c->prof_active = 0; return rc; }
-        nnp_launch_kick_ke(c);
+        nnp_launch_kick_ke(c, 1);
         nnp_prof_mark(c, 11);
         c->prof_active = 0;
     }

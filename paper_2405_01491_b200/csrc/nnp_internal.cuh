@@ -148,6 +148,10 @@ struct nnp_ctx {
     int bucket_off[NNP_MAX_SPECIES + 1]; // species-major internal order: atoms of species s are [off[s], off[s+1])
     GridInfo grid;
     float skin, dt;
+    // Langevin BAOAB (nnp_md_set_langevin); gamma = 0: velocity Verlet
+    float lgv_gamma, lgv_kT, lgv_c1;
+    uint64_t lgv_seed;
+    float *d_lgv_c2;                // [S] sqrt((1 - c1^2) kT accel_conv / m_s)
 
     // per-atom state, internal order
     float4 *pos, *pos_tmp; // xyz, w unused
@@ -170,7 +174,7 @@ struct nnp_ctx {
     float *e_atom;           // [n]
     double *e_mol;           // [max_mols]
     double *ekin;            // scalar
-    int *flags;              // [0] error flags, [1] rebuild request, [2] rebuild count
+    int *flags;              // [0] error flags, [1] rebuild request, [2] rebuild count, [4] Langevin step counter
     int *aev_sched;          // [2][NNP_AEV_SCHED_LEN] centre queues of the two AEV kernels (aev.cu), zero between launches
     // staging for the host entry points
     float *io_xyz, *io_vel;  // [n][3]
@@ -195,7 +199,7 @@ void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi);
 int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3);
 // integrate.cu
 void nnp_launch_kick_drift(nnp_ctx *c);
-void nnp_launch_kick_ke(nnp_ctx *c);
+void nnp_launch_kick_ke(nnp_ctx *c, int count_step); // count_step: also advance the Langevin step counter flags[4]
 void nnp_launch_energy_reduce(nnp_ctx *c);
 void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst);
 void nnp_launch_permute_in3(nnp_ctx *c, const float *src, float4 *dst); // dst[i] = src[orig[i]]

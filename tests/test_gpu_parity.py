@@ -426,3 +426,83 @@ def test_ladder_is_the_default_for_ani2x_constants(model1):
         assert nnp.nnp_aev_ladder(ctx) == 1
     finally:
         nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- NEXT-1: Langevin BAOAB
+@pytest.mark.parametrize("graph", [False, True], ids=["kernel_by_kernel", "cuda_graph"])
+def test_langevin_baoab_against_oracle(model1, graph):
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(216, seed=19)
+    v = inputs.maxwell_boltzmann(sp, 300.0, seed=4)
+    n = len(sp)
+    dt, gamma, kT, seed = 0.5, 0.02, inputs.KB * 300.0, 987654321012345
+    dev = torch.device("cuda:0")
+    ctx = U.gpu_create(consts, widths, params, 1, n, stream=torch.cuda.Stream(device=dev) if graph else None)
+    try:
+        d_sp = torch.as_tensor(sp, device=dev)
+        d_x = torch.as_tensor(xyz.astype(np.float32), device=dev)
+        d_v = torch.as_tensor(v.astype(np.float32), device=dev)
+        o_x, o_v = torch.zeros_like(d_x), torch.zeros_like(d_v)
+        o_ek = torch.zeros(1, dtype=torch.float64, device=dev)
+        torch.cuda.synchronize()
+        nnp.nnp_set_system(ctx, n, d_sp, d_x, box)
+        with pytest.raises(nnp.NnpError):
+            nnp.nnp_md_set_langevin(ctx, gamma, kT, seed)        # before nnp_md_init
+        nnp.nnp_md_init(ctx, d_v, dt, 0.5)
+        nnp.nnp_md_set_langevin(ctx, gamma, kT, seed)
+
+        def state():
+            nnp.nnp_get_state(ctx, o_x, o_v, None, o_ek, None)
+            nnp.nnp_sync(ctx)
+            return o_x.cpu().numpy().astype(np.float64), o_v.cpu().numpy().astype(np.float64), float(o_ek.item())
+
+        # one step, then five more in one call (the device-side step counter feeds the generator)
+        nnp.nnp_md_step(ctx, 1)
+        x1, v1, _ = state()
+        o1 = orc.md_langevin(om, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, 1, gamma, kT, seed)
+        assert np.abs(x1 - o1["xyz"]).max() < 2e-6 and np.abs(v1 - o1["vel"]).max() < 2e-6
+        kick = orc.md(om, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, 1)
+        assert np.abs(v1 - kick["vel"]).max() > 1e-4             # the noise is in
+        nnp.nnp_md_step(ctx, 5)
+        x6, v6, ek6 = state()
+        o6 = orc.md_langevin(om, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, 6, gamma, kT, seed)
+        assert np.abs(x6 - o6["xyz"]).max() < 2e-5 and np.abs(v6 - o6["vel"]).max() < 2e-5
+        assert abs(ek6 - o6["ekin"][6]) < 1e-4 * o6["ekin"][6]
+        # gamma = 0 switches back to velocity Verlet: one step from the current state equals the oracle's VV step
+        nnp.nnp_md_set_langevin(ctx, 0.0, kT, seed)
+        nnp.nnp_md_step(ctx, 1)
+        x7, v7, _ = state()
+        o7 = orc.md(om, sp, x6, v6, inputs.MASS, box, dt, inputs.ACCEL_CONV, 1)
+        assert np.abs(x7 - o7["xyz"]).max() < 2e-6 and np.abs(v7 - o7["vel"]).max() < 2e-6
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_langevin_thermostat_holds_temperature(model1):
+    """648 atoms started at rest under random-weight forces (scale FORCE_SCALE_MD): friction 0.05/fs pulls the kinetic
+    temperature to the bath's 300 K and holds it there."""
+    consts, widths, _, _ = model1
+    params = inputs.make_weights(inputs.SEED0, 1, last_layer_scale=inputs.FORCE_SCALE_MD)
+    sp, xyz, box = inputs.water_box(216, seed=23)
+    n = len(sp)
+    dev = torch.device("cuda:0")
+    ctx = U.gpu_create(consts, widths, params, 1, n, stream=torch.cuda.Stream(device=dev))
+    try:
+        d_sp = torch.as_tensor(sp, device=dev)
+        d_x = torch.as_tensor(xyz.astype(np.float32), device=dev)
+        d_v = torch.zeros_like(d_x)
+        o_ek = torch.zeros(1, dtype=torch.float64, device=dev)
+        torch.cuda.synchronize()
+        nnp.nnp_set_system(ctx, n, d_sp, d_x, box)
+        nnp.nnp_md_init(ctx, d_v, 0.5, 0.5)
+        nnp.nnp_md_set_langevin(ctx, 0.05, inputs.KB * 300.0, 42)
+        nnp.nnp_md_step(ctx, 400)
+        temps = []
+        for _ in range(40):
+            nnp.nnp_md_step(ctx, 25)
+            nnp.nnp_get_state(ctx, None, None, None, o_ek, None)
+            nnp.nnp_sync(ctx)
+            temps.append(2 * float(o_ek.item()) / (3 * n * inputs.KB))
+        assert abs(np.mean(temps) - 300.0) < 20.0, np.mean(temps)
+    finally:
+        nnp.nnp_destroy(ctx)

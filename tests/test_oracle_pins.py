@@ -503,3 +503,72 @@ def test_oracle_matches_stored_golden(consts):
         elif t[0] == "AEVNNZ":
             # water: only H,O radial blocks and the (H,H),(H,O),(O,O) angular blocks can be non-zero
             assert int((r["aev"] != 0).sum()) == int(t[1]) <= 192 * 128
+
+
+# ---------------------------------------------------------------- NEXT-1: Langevin BAOAB
+def test_philox4x32_10_known_answers():
+    """Known-answer vectors of Philox4x32-10 from the reference distribution of Salmon et al. (SC'11), kat_vectors:
+    zero counter/key, all-ones counter/key, and the digits-of-pi counter/key."""
+    assert orc.philox4x32_10([0, 0, 0, 0], [0, 0]) == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+    assert orc.philox4x32_10([0xffffffff] * 4, [0xffffffff] * 2) == [0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd]
+    assert orc.philox4x32_10([0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344], [0xa4093822, 0x299f31d0]) == \
+        [0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1]
+
+
+def test_langevin_normals_are_standard_normal():
+    from scipy import stats
+    xi = np.array([orc.langevin_normals(a, s, 20240501) for a in range(400) for s in range(25)])
+    assert xi.shape == (10000, 3)
+    for c in range(3):
+        assert stats.kstest(xi[:, c], "norm").pvalue > 1e-3
+    assert np.abs(xi.mean(0)).max() < 0.04 and np.abs(xi.var(0) - 1).max() < 0.05
+    assert np.abs(np.corrcoef(xi.T) - np.eye(3)).max() < 0.04
+    # different atoms, steps and seeds give different numbers; the same triple repeats
+    assert np.array_equal(orc.langevin_normals(5, 9, 1), orc.langevin_normals(5, 9, 1))
+    assert not np.array_equal(orc.langevin_normals(5, 9, 1), orc.langevin_normals(5, 9, 2))
+    assert not np.array_equal(orc.langevin_normals(5, 9, 1), orc.langevin_normals(6, 9, 1))
+    assert not np.array_equal(orc.langevin_normals(5, 9, 1), orc.langevin_normals(5, 10, 1))
+
+
+def test_langevin_zero_friction_is_velocity_verlet(small_model):
+    sp, xyz, box, v = _md_setup(small_model)
+    a = orc.md(small_model, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 12)
+    b = orc.md_langevin(small_model, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 12, gamma=0.0,
+                        kT=inputs.KB * 300.0, seed=3)
+    assert np.abs(a["xyz"] - b["xyz"]).max() < 1e-12 and np.abs(a["vel"] - b["vel"]).max() < 1e-13
+    assert np.abs(a["epot"] - b["epot"]).max() < 1e-9 * np.abs(a["epot"]).max()
+
+
+def test_langevin_first_step_by_hand(small_model):
+    """B A O A (forces) B written out with numpy, the normals taken from the generator."""
+    sp, xyz, box, v = _md_setup(small_model)
+    dt, gamma, kT, seed, step0 = 0.5, 0.05, inputs.KB * 300.0, 77, 5
+    m = inputs.MASS[sp][:, None]
+    a0 = inputs.ACCEL_CONV * orc.energy_forces(small_model, sp, xyz, box)["F"] / m
+    xi = np.array([orc.langevin_normals(i, step0, seed) for i in range(len(sp))])
+    c1 = math.exp(-gamma * dt)
+    vb = v + 0.5 * dt * a0
+    xa = xyz + 0.5 * dt * vb
+    vo = c1 * vb + np.sqrt((1 - c1 * c1) * kT * inputs.ACCEL_CONV / m) * xi
+    x1 = xa + 0.5 * dt * vo
+    v1 = vo + 0.5 * dt * inputs.ACCEL_CONV * orc.energy_forces(small_model, sp, x1, box)["F"] / m
+    r = orc.md_langevin(small_model, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, 1, gamma, kT, seed, step0=step0)
+    assert np.abs(r["xyz"] - x1).max() < 1e-13 and np.abs(r["vel"] - v1).max() < 1e-13
+    # the noise really entered: the result differs from the frictionless step by about c2 * |xi|
+    r0 = orc.md(small_model, sp, xyz, v, inputs.MASS, box, dt, inputs.ACCEL_CONV, 1)
+    assert np.abs(r["vel"] - r0["vel"]).max() > 1e-4
+
+
+def test_langevin_equipartition_free_particles(small_model):
+    """Atoms far apart (no neighbours, zero forces): the O step alone must hold <m v^2> = kT per degree of freedom,
+    whatever the start (here: at rest)."""
+    n = 64
+    sp = (np.arange(n) % 2 * 3).astype(np.int32)                 # H and O
+    xyz = 50.0 * np.stack(np.meshgrid(np.arange(4), np.arange(4), np.arange(4), indexing="ij"), -1).reshape(-1, 3).astype(float)
+    v = np.zeros((n, 3))
+    T = 300.0
+    r = orc.md_langevin(small_model, sp, xyz, v, inputs.MASS, None, 0.5, inputs.ACCEL_CONV, 3000, gamma=0.02,
+                        kT=inputs.KB * T, seed=11)
+    temp = 2 * r["ekin"][500:] / (3 * n * inputs.KB)             # after 5 relaxation times
+    assert abs(temp.mean() - T) < 0.06 * T
+    assert r["ekin"][0] == 0.0 and np.abs(r["epot"] - r["epot"][0]).max() < 1e-9
