@@ -251,6 +251,7 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "water_%d_md (BASELINE configs[2])" % n if args.waters == N_WATERS else "water_%d_md" % n,
                    "atoms": n, "box_A": float(box[0]), "dt_fs": DT_FS, "skin_A": SKIN, "n_nets": 1,
+                   "integrator": "langevin_baoab gamma=%g/fs" % args.langevin if args.langevin > 0 else "velocity_verlet",
                    "mm_mode": ["fp32_simt", "3xtf32_tcgen05", "tf32_tcgen05"][args.mm_mode],
                    "force_scale": args.force_scale, "ns_per_day": steps_per_s * DT_FS * 1e-6 * 86400,
                    "rebuilds_in_timed_region": nr_end - nr_start,
