@@ -592,6 +592,11 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 // Reverse pass: g = dE/dG_i (row of dG, times inv_nets).  Adds -dE/dx to frc for the centre and its neighbours.
 // (The Gaussian ladder of the forward kernel is not used here: the reverse pass needs every w_k as well, the
 // recurrence then costs more issue slots than the exponentials it saves -- measured 0.355 vs 0.346 ms.)
+// GS: the centre's gradient row (kpad <= kGsMax floats) is copied into shared memory with cp.async at the top of the
+// iteration, behind the index -> position load chain, instead of being loaded from global memory where it is first
+// needed (those loads were 10 % of the stall samples).
+constexpr int kGsMax = 128;  // water: 128 active columns; 2 KiB per block keeps five blocks per SM
+template <bool GS>
 __global__ void __launch_bounds__(kWarps * 32, AEV_BWD_MINB)
 k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
                const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
@@ -600,6 +605,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
 {
     extern __shared__ __align__(16) uint8_t smem_dyn[];
     WarpSmemBwd *smem = reinterpret_cast<WarpSmemBwd *>(smem_dyn);
+    float *gs = reinterpret_cast<float *>(smem_dyn + kWarps * sizeof(WarpSmemBwd)) + (threadIdx.x >> 5) * kGsMax; // GS only
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     WarpSmemBwd &sm = smem[wid];
     int bcs, bct;
@@ -632,9 +638,23 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     }
     while (i < n) {
         queue.request(); // read after the radial phase
+        if constexpr (GS) {
+            const float *src = dG + (size_t)i * P.kpad;
+            for (int q = 4 * lane; q < P.kpad; q += 128)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(gs + q)), "l"(src + q) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
         Centre c;
         load_centre(c, P, i, lane, my_s, sgr_l, sga_l, pos, nbr_r, nbr_a, sm.own);
         const float *grow = dG + (size_t)i * P.kpad;
+        auto g4 = [&](int off) -> float4 { // four gradient values of this centre (off: multiple of 4)
+            if constexpr (GS) return *reinterpret_cast<const float4 *>(gs + off);
+            else return *reinterpret_cast<const float4 *>(grow + off);
+        };
+        if constexpr (GS) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            __syncwarp();
+        }
         float fi[3] = {0.f, 0.f, 0.f}; // dE/dd summed over this lane's terms (force on i = +sum)
 
         // ---- radial: dE/dr_ij = sum_k g[s_j*16+k] * 1/4 e_k (-2 eta (r-ShfR_k) fc + fc')
@@ -644,7 +664,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
 #pragma unroll
             for (int k4 = 0; k4 < NNP_NSHF_R / 4; ++k4) {
                 float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (c.pr.r < c.pr.L) v = *reinterpret_cast<const float4 *>(grow + c.pr.tag * NNP_NSHF_R + 4 * k4);
+                if (c.pr.r < c.pr.L) v = g4(c.pr.tag * NNP_NSHF_R + 4 * k4);
                 gr[2 * k4] = make_float2(v.x * sc0, v.y * sc0);
                 gr[2 * k4 + 1] = make_float2(v.z * sc0, v.w * sc0);
             }
@@ -721,12 +741,12 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
             float2 gw[NNP_ANG_BLOCK / 2]; // [a][z pair]
             {
                 const int pb = wcs * (2 * P.np + 1 - wcs) / 2 + (wct - wcs);
-                const float *gp = grow + P.n_rad + pb * NNP_ANG_BLOCK;
+                const int gp = P.n_rad + pb * NNP_ANG_BLOCK;
                 const float sc0 = 2.0f * inv_nets; // the prefactor 2 of the angular term
 #pragma unroll
                 for (int q4 = 0; q4 < NNP_ANG_BLOCK / 4; ++q4) {
                     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (npairs > 0) v = *reinterpret_cast<const float4 *>(gp + 4 * q4);
+                    if (npairs > 0) v = g4(gp + 4 * q4);
                     gw[2 * q4] = make_float2(v.x * sc0, v.y * sc0);
                     gw[2 * q4 + 1] = make_float2(v.z * sc0, v.w * sc0);
                 }
@@ -838,7 +858,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     queue.release();
 }
 
-int g_blocks_fwd = 0, g_blocks_bwd = 0, g_sms = 0;
+int g_blocks_fwd = 0, g_sms = 0;
 
 } // namespace
 
@@ -874,13 +894,16 @@ void nnp_launch_aev_forward(nnp_ctx *c)
 
 void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets)
 {
-    const int smem = (int)sizeof(WarpSmemBwd) * kWarps;
-    if (!g_blocks_bwd) {
-        cudaFuncSetAttribute(k_aev_backward, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_bwd, k_aev_backward, kWarps * 32, smem);
+    const bool gs = c->aev.kpad <= kGsMax;
+    const int smem = (int)sizeof(WarpSmemBwd) * kWarps + (gs ? kWarps * kGsMax * 4 : 0);
+    static int blocks[2] = {0, 0};
+    auto kern = gs ? k_aev_backward<true> : k_aev_backward<false>;
+    if (!blocks[gs]) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks[gs], kern, kWarps * 32, smem);
     }
-    const int grid = persistent_grid(c, g_blocks_bwd);
-    k_aev_backward<<<grid, kWarps * 32, smem, c->stream>>>(
+    const int grid = persistent_grid(c, blocks[gs]);
+    kern<<<grid, kWarps * 32, smem, c->stream>>>(
         c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a, c->seg_a, c->d_tri, c->dG, inv_nets, c->frc, c->flags, c->aev_sched + NNP_AEV_SCHED_LEN, g_sms);
     c->launches += 1;
 }
