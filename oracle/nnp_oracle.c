@@ -348,7 +348,7 @@ static void aev_atom(const orc_model *m, int i, const int *species, const double
 
 /* O6: given g = dE/dG_i, add -dE/dx to F for atom i and its neighbours. */
 static void aev_atom_backward(const orc_model *m, int i, const int *species, const double *xyz, const double *box,
-                              int nn, const int *nbr, const double *g, double *F)
+                              int nn, const int *nbr, const double *g, double *F, double *W /* NULL or [10]: strain derivative sum d_a dE/dd_b (9) and sum |d_a dE/dd_b| */)
 {
     const int S = m->n_species, nr = m->n_shf_r, na = m->n_shf_a, nz = m->n_shf_z;
     const int rad = S * nr;
@@ -370,6 +370,7 @@ static void aev_atom_backward(const orc_model *m, int i, const int *species, con
 #pragma omp atomic
             F[3 * j + c] -= v;
             Fi[c] += v;
+            if (W) for (int a2 = 0; a2 < 3; ++a2) { W[3 * a2 + c] += d[a2] * v; W[9] += fabs(d[a2] * v); }
         }
     }
     for (int a = 0; a < nn; ++a) {
@@ -417,6 +418,10 @@ static void aev_atom_backward(const orc_model *m, int i, const int *species, con
 #pragma omp atomic
                 F[3 * k + q] -= vk;
                 Fi[q] += vj + vk;
+                if (W) for (int a2 = 0; a2 < 3; ++a2) {
+                    W[3 * a2 + q] += dj[a2] * vj + dk[a2] * vk;
+                    W[9] += fabs(dj[a2] * vj) + fabs(dk[a2] * vk);
+                }
             }
         }
     }
@@ -429,9 +434,9 @@ static void aev_atom_backward(const orc_model *m, int i, const int *species, con
 /* O1-O6.  nbr_method: 0 brute force, 1 grid (periodic only).  Lists are built at the exact radial
  * cutoff in fp64.  Outputs (any may be NULL except E): E[n_mols] (O5), F[n][3] (O6), e_atom[n],
  * aev[n][len], dEdG[n][len].  mol_offsets NULL => one structure.  Returns 0, or <0 on failure. */
-int orc_energy_forces(const orc_model *m, int n, const int *species, const double *xyz, const double *box,
-                      int n_mols, const int *mol_offsets, int nbr_method, double *E, double *F,
-                      double *e_atom, double *aev, double *dEdG)
+static int energy_forces_impl(const orc_model *m, int n, const int *species, const double *xyz, const double *box,
+                              int n_mols, const int *mol_offsets, int nbr_method, double *E, double *F,
+                              double *e_atom, double *aev, double *dEdG, double *virial)
 {
     const int len = orc_aev_len(m);
     const double *bx = NULL;
@@ -465,6 +470,7 @@ int orc_energy_forces(const orc_model *m, int n, const int *species, const doubl
         double *G = (double *)malloc(sizeof(double) * len);
         double *g = (double *)malloc(sizeof(double) * len);
         double *gn = (double *)malloc(sizeof(double) * len);
+        double Wt[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 #pragma omp for schedule(dynamic, 16)
         for (int i = 0; i < n; ++i) {
             int s = species[i];
@@ -484,12 +490,38 @@ int orc_energy_forces(const orc_model *m, int n, const int *species, const doubl
             if (dEdG) memcpy(dEdG + (size_t)i * len, g, sizeof(double) * len);
 #pragma omp atomic
             E[mol_id[i]] += e;
-            if (F) aev_atom_backward(m, i, species, xyz, bx, counts[i], list + (size_t)i * cap, g, F);
+            if (F) aev_atom_backward(m, i, species, xyz, bx, counts[i], list + (size_t)i * cap, g, F, virial ? Wt : NULL);
         }
+        if (virial)
+            for (int q = 0; q < 10; ++q) {
+#pragma omp atomic
+                virial[q] += Wt[q];
+            }
         free(G); free(g); free(gn);
     }
     free(counts); free(list); free(mol_id);
     return fail ? -2 : 0;
+}
+
+int orc_energy_forces(const orc_model *m, int n, const int *species, const double *xyz, const double *box,
+                      int n_mols, const int *mol_offsets, int nbr_method, double *E, double *F,
+                      double *e_atom, double *aev, double *dEdG)
+{
+    return energy_forces_impl(m, n, species, xyz, box, n_mols, mol_offsets, nbr_method, E, F, e_atom, aev, dEdG, NULL);
+}
+
+/* NEXT-2 (first part; "energy_and_forces_and_virial"): the energy depends on
+ * the coordinates (and, under PBC, the cell) only through the displacement vectors d it is built from -- d_ij of every
+ * radial term and d_ij, d_ik of every angular term -- so under a homogeneous deformation x -> (1 + eps) x,
+ * cell -> (1 + eps) cell every d -> (1 + eps) d and
+ *     V_ab = dE/d eps_ab = sum over those d of d_a (dE/dd)_b          (the virial; stress = V / volume).
+ * One structure only.  virial[0..8] = V (row-major, symmetric up to rounding because E is rotation invariant),
+ * virial[9] = sum |d_a (dE/dd)_b|, the scale against which rounding errors of an fp32 evaluation are judged. */
+int orc_energy_forces_virial(const orc_model *m, int n, const int *species, const double *xyz, const double *box,
+                             int nbr_method, double *E, double *F, double *virial /*[10]*/)
+{
+    for (int q = 0; q < 10; ++q) virial[q] = 0.0;
+    return energy_forces_impl(m, n, species, xyz, box, 1, NULL, nbr_method, E, F, NULL, NULL, NULL, virial);
 }
 
 /* O7 rebuild rule (reading C2): max_i |x_i - xref_i| > skin/2 (strict). */

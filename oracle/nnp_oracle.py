@@ -235,3 +235,22 @@ def md_langevin(model, species, xyz, vel, mass, box, dt, accel_conv, n_steps, ga
     if rc != 0:
         raise RuntimeError("orc_md_langevin failed: %d" % rc)
     return {"xyz": x, "vel": v, "F": F, "epot": epot, "ekin": ekin, "n_rebuilds": nreb.value}
+
+
+def energy_forces_virial(model, species, xyz, box, nbr_method=0):
+    """NEXT-2: E, F and the virial V_ab = dE/d eps_ab = sum_d d_a (dE/dd)_b of ONE structure.
+    Returns dict(E, F, virial[3][3], virial_abs)."""
+    species = np.ascontiguousarray(species, dtype=np.int32)
+    x = np.ascontiguousarray(xyz, dtype=np.float64)
+    n = x.shape[0]
+    boxa = None if box is None else np.ascontiguousarray(box, dtype=np.float64)
+    E = np.zeros(1)
+    F = np.zeros((n, 3))
+    W = np.zeros(10)
+    f = lib().orc_energy_forces_virial
+    f.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    rc = f(C.cast(C.byref(model.c), C.c_void_p), n, species.ctypes.data, x.ctypes.data,
+           None if boxa is None else boxa.ctypes.data, int(nbr_method), E.ctypes.data, F.ctypes.data, W.ctypes.data)
+    if rc != 0:
+        raise RuntimeError("orc_energy_forces_virial failed: %d" % rc)
+    return {"E": E, "F": F, "virial": W[:9].reshape(3, 3).copy(), "virial_abs": float(W[9])}

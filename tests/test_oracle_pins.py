@@ -572,3 +572,52 @@ def test_langevin_equipartition_free_particles(small_model):
     temp = 2 * r["ekin"][500:] / (3 * n * inputs.KB)             # after 5 relaxation times
     assert abs(temp.mean() - T) < 0.06 * T
     assert r["ekin"][0] == 0.0 and np.abs(r["epot"] - r["epot"][0]).max() < 1e-9
+
+
+# ---------------------------------------------------------------- NEXT-2: virial (PAPER.md L262 energy_and_forces_and_virial)
+def test_virial_is_the_strain_derivative_periodic(small_model, water64):
+    """V_aa = dE/d eps_aa by central differences of the energy under a homogeneous stretch of coordinates AND box."""
+    sp, xyz, box = water64
+    r = orc.energy_forces_virial(small_model, sp, xyz, box)
+    V, h = r["virial"], 2e-5
+    for a in range(3):
+        s = np.ones(3)
+        s[a] += h
+        ep = orc.energy_forces(small_model, sp, xyz * s, np.asarray(box) * s)["E"][0]
+        s[a] -= 2 * h
+        em = orc.energy_forces(small_model, sp, xyz * s, np.asarray(box) * s)["E"][0]
+        assert abs((ep - em) / (2 * h) - V[a, a]) < 2e-7 * r["virial_abs"]
+    assert np.abs(V - V.T).max() < 1e-12 * r["virial_abs"]          # rotation invariance => symmetric
+    assert np.allclose(r["F"], orc.energy_forces(small_model, sp, xyz, box)["F"], rtol=0, atol=1e-14)
+    assert r["virial_abs"] >= np.abs(V).max()
+
+
+def test_virial_full_tensor_and_clausius_form_nonperiodic(small_model):
+    """Without a box every component follows from x -> (1 + eps) x, shear included, and V_ab = -sum_i x_ia F_ib."""
+    sp, xyz, offs = inputs.molecule_batch(1, nmin=24, nmax=24, seed=31)
+    r = orc.energy_forces_virial(small_model, sp, xyz, None)
+    V, h = r["virial"], 2e-5
+    for a in range(3):
+        for b in range(3):
+            eps = np.zeros((3, 3))
+            eps[a, b] = h
+            ep = orc.energy_forces(small_model, sp, xyz @ (np.eye(3) + eps), None)["E"][0]   # x'_b = x_b + eps_ab x_a
+            em = orc.energy_forces(small_model, sp, xyz @ (np.eye(3) - eps), None)["E"][0]
+            assert abs((ep - em) / (2 * h) - V[a, b]) < 2e-7 * r["virial_abs"], (a, b)
+    assert np.abs(V + xyz.T @ r["F"]).max() < 1e-11 * r["virial_abs"]
+    # a rigid translation changes nothing (net force is zero)
+    r2 = orc.energy_forces_virial(small_model, sp, xyz + np.array([3.0, -2.0, 5.0]), None)
+    assert np.abs(r2["virial"] - V).max() < 1e-10 * r["virial_abs"]
+
+
+def test_virial_of_a_dimer_by_hand(small_model, consts):
+    """Two atoms on the x axis: only V_xx = r dE/dr is non-zero, and dE/dr follows from the forces."""
+    rr = 1.3
+    sp = np.array([0, 3], dtype=np.int32)
+    xyz = np.array([[0.0, 0.0, 0.0], [rr, 0.0, 0.0]])
+    r = orc.energy_forces_virial(small_model, sp, xyz, None)
+    dEdr = -r["F"][1, 0]
+    assert abs(r["virial"][0, 0] - rr * dEdr) < 1e-12 * max(1.0, abs(rr * dEdr))
+    V = r["virial"].copy()
+    V[0, 0] = 0.0
+    assert np.abs(V).max() < 1e-14
