@@ -114,6 +114,14 @@ int nnp_get_neighbors(nnp_ctx *ctx, int which, int32_t *d_counts, int32_t *d_lis
  * d_forces[n][3] fp32 in original order, may be NULL (energy only still runs the full path). */
 int nnp_energy_forces(nnp_ctx *ctx, double *d_energy, float *d_forces);
 
+/* Energy, forces and the virial of ONE structure (n_mols = 1; PAPER.md L262 energy_and_forces_and_virial, SURVEY.md
+ * 8(f) item 2, orthorhombic cells): d_virial[9] fp64, row-major V_ab = dE/d eps_ab = sum over every displacement
+ * vector d the energy is built from of d_a (dE/dd)_b -- the derivative of the energy under the homogeneous
+ * deformation x -> (1 + eps) x, cell -> (1 + eps) cell; symmetric; stress = V / volume; without a cell
+ * V_ab = -sum_i x_ia F_ib.  Accumulated in fp32 per lane and in fp64 across warps by the reverse AEV kernel.
+ * NNP_EINVAL for batched structures.  Otherwise as nnp_energy_forces. */
+int nnp_energy_forces_virial(nnp_ctx *ctx, double *d_energy, float *d_forces, double *d_virial);
+
 /* Test hooks (valid after nnp_energy_forces): AEVs [n][aev_len] and per-atom energies [n], original order. */
 int nnp_get_aev(nnp_ctx *ctx, float *d_aev);
 int nnp_get_atomic_energies(nnp_ctx *ctx, float *d_e_atom);

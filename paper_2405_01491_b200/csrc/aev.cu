@@ -596,12 +596,15 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 // iteration, behind the index -> position load chain, instead of being loaded from global memory where it is first
 // needed (those loads were 10 % of the stall samples).
 constexpr int kGsMax = 128;  // water: 128 active columns; 2 KiB per block keeps five blocks per SM
-template <bool GS>
+// VIR: also accumulate the virial V_ab = sum_d d_a (dE/dd)_b over every displacement vector the energy is built from
+// (PAPER.md L262): six per-lane sums over all centres of the warp, reduced once at the end.
+template <bool GS, bool VIR>
 __global__ void __launch_bounds__(kWarps * 32, AEV_BWD_MINB)
 k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
                const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
                const uint16_t *__restrict__ seg_a, const uint16_t *__restrict__ tri, const float *__restrict__ dG,
-               float inv_nets, float4 *__restrict__ frc, int *__restrict__ flags, int *__restrict__ sched, int nsm)
+               float inv_nets, float4 *__restrict__ frc, int *__restrict__ flags, int *__restrict__ sched, int nsm,
+               double *__restrict__ virial /* [6] xx yy zz xy xz yz, VIR only */)
 {
     extern __shared__ __align__(16) uint8_t smem_dyn[];
     WarpSmemBwd *smem = reinterpret_cast<WarpSmemBwd *>(smem_dyn);
@@ -627,6 +630,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
 
     // Centres are handed out dynamically (one ticket per centre): the cost of a centre varies with its pair count,
     // and with a static split the slowest warp of a persistent grid ends ~20 % after the average one.
+    float vir[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     CentreQueue<AEV_BWD_SCHED> queue;
     queue.init(sched, n, nsm, lane);
     queue.request();
@@ -692,6 +696,10 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                     const float vx = sc * d.x, vy = sc * d.y, vz = sc * d.z;
                     atomicAdd(&frc[j], make_float4(-vx, -vy, -vz, 0.f));
                     fi[0] += vx; fi[1] += vy; fi[2] += vz;
+                    if constexpr (VIR) {
+                        vir[0] = fmaf(d.x, vx, vir[0]); vir[1] = fmaf(d.y, vy, vir[1]); vir[2] = fmaf(d.z, vz, vir[2]);
+                        vir[3] = fmaf(d.x, vy, vir[3]); vir[4] = fmaf(d.x, vz, vir[4]); vir[5] = fmaf(d.y, vz, vir[5]);
+                    }
                 }
             };
 #pragma unroll
@@ -844,6 +852,11 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
             }
             atomicAdd(&frc[sm.j[a]], make_float4(-fx, -fy, -fz, 0.f));
             fi[0] += fx; fi[1] += fy; fi[2] += fz;
+            if constexpr (VIR) {
+                const float4 dv = sm.d[a];
+                vir[0] = fmaf(dv.x, fx, vir[0]); vir[1] = fmaf(dv.y, fy, vir[1]); vir[2] = fmaf(dv.z, fz, vir[2]);
+                vir[3] = fmaf(dv.x, fy, vir[3]); vir[4] = fmaf(dv.x, fz, vir[4]); vir[5] = fmaf(dv.y, fz, vir[5]);
+            }
         }
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
@@ -856,6 +869,15 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
         i = i_next;
     }
     queue.release();
+    if constexpr (VIR) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            double v = (double)vir[q];
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+            if (lane == 0) atomicAdd(virial + q, v);
+        }
+    }
 }
 
 int g_blocks_fwd = 0, g_sms = 0;
@@ -892,18 +914,20 @@ void nnp_launch_aev_forward(nnp_ctx *c)
     c->launches += 1;
 }
 
-void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets)
+void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets, double *d_virial)
 {
-    const bool gs = c->aev.kpad <= kGsMax;
+    const int gs = c->aev.kpad <= kGsMax ? 1 : 0, vir = d_virial ? 1 : 0;
     const int smem = (int)sizeof(WarpSmemBwd) * kWarps + (gs ? kWarps * kGsMax * 4 : 0);
-    static int blocks[2] = {0, 0};
-    auto kern = gs ? k_aev_backward<true> : k_aev_backward<false>;
-    if (!blocks[gs]) {
+    static int blocks[2][2] = {{0, 0}, {0, 0}};
+    auto kern = gs ? (vir ? k_aev_backward<true, true> : k_aev_backward<true, false>)
+                   : (vir ? k_aev_backward<false, true> : k_aev_backward<false, false>);
+    if (!blocks[gs][vir]) {
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks[gs], kern, kWarps * 32, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks[gs][vir], kern, kWarps * 32, smem);
     }
-    const int grid = persistent_grid(c, blocks[gs]);
+    const int grid = persistent_grid(c, blocks[gs][vir]);
     kern<<<grid, kWarps * 32, smem, c->stream>>>(
-        c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a, c->seg_a, c->d_tri, c->dG, inv_nets, c->frc, c->flags, c->aev_sched + NNP_AEV_SCHED_LEN, g_sms);
+        c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a, c->seg_a, c->d_tri, c->dG, inv_nets, c->frc, c->flags, c->aev_sched + NNP_AEV_SCHED_LEN, g_sms,
+        d_virial);
     c->launches += 1;
 }

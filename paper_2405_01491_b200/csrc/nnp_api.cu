@@ -346,7 +346,7 @@ int run_forces(nnp_ctx *c)
         }
     nnp_launch_energy_reduce(c);
     nnp_prof_mark(c, 9);
-    nnp_launch_aev_backward(c, 1.0f / (float)c->n_nets);
+    nnp_launch_aev_backward(c, 1.0f / (float)c->n_nets, c->want_virial ? c->d_virial : nullptr);
     nnp_prof_mark(c, 10);
     CU(c, cudaGetLastError());
     c->have_forces = 1;
@@ -479,7 +479,7 @@ void nnp_destroy(nnp_ctx *c)
     cudaStreamSynchronize(c->stream);
     drop_md_graph(c);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
-    void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->d_lgv_c2, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
+    void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->d_lgv_c2, c->d_virial, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags, c->aev_sched,
@@ -643,6 +643,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     TRY(dev_alloc(c, &c->d_mass, NNP_MAX_SPECIES));
     TRY(dev_alloc(c, &c->d_e_shift, NNP_MAX_SPECIES));
     TRY(dev_alloc(c, &c->d_lgv_c2, NNP_MAX_SPECIES));
+    TRY(dev_alloc(c, &c->d_virial, 6));
     TRYCU(cudaMemcpy(c->d_inv_mass_conv, imc, sizeof(imc), cudaMemcpyHostToDevice));
     TRYCU(cudaMemcpy(c->d_mass, ms, sizeof(ms), cudaMemcpyHostToDevice));
     TRYCU(cudaMemcpy(c->d_e_shift, es, sizeof(es), cudaMemcpyHostToDevice));
@@ -782,6 +783,30 @@ int nnp_energy_forces(nnp_ctx *c, double *d_energy, float *d_forces)
     if (!c) return NNP_EINVAL;
     if (!d_energy) NNP_FAIL(c, NNP_EINVAL, "null energy pointer");
     return energy_forces_impl(c, d_energy, d_forces);
+}
+
+// symmetric 3x3 from the six sums xx yy zz xy xz yz of the reverse AEV kernel
+__global__ void k_expand_virial(const double *__restrict__ v6, double *__restrict__ v9)
+{
+    const int map[9] = {0, 3, 4, 3, 1, 5, 4, 5, 2};
+    if (threadIdx.x < 9) v9[threadIdx.x] = v6[map[threadIdx.x]];
+}
+
+int nnp_energy_forces_virial(nnp_ctx *c, double *d_energy, float *d_forces, double *d_virial)
+{
+    if (!c) return NNP_EINVAL;
+    if (!d_energy || !d_virial) NNP_FAIL(c, NNP_EINVAL, "null energy / virial pointer");
+    if (c->n_mols != 1) NNP_FAIL(c, NNP_EINVAL, "the virial is defined for one structure (n_mols = 1)");
+    CU(c, cudaSetDevice(c->device));
+    CU(c, cudaMemsetAsync(c->d_virial, 0, sizeof(double) * 6, c->stream));
+    c->want_virial = 1;
+    const int rc = energy_forces_impl(c, d_energy, d_forces);
+    c->want_virial = 0;
+    if (rc) return rc;
+    k_expand_virial<<<1, 32, 0, c->stream>>>(c->d_virial, d_virial);
+    c->launches += 1;
+    CU(c, cudaGetLastError());
+    return NNP_OK;
 }
 
 int nnp_get_aev(nnp_ctx *c, float *d_aev)

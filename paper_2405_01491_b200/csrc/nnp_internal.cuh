@@ -152,6 +152,8 @@ struct nnp_ctx {
     float lgv_gamma, lgv_kT, lgv_c1;
     uint64_t lgv_seed;
     float *d_lgv_c2;                // [S] sqrt((1 - c1^2) kT accel_conv / m_s)
+    double *d_virial;               // [6] xx yy zz xy xz yz (nnp_energy_forces_virial)
+    int want_virial;
 
     // per-atom state, internal order
     float4 *pos, *pos_tmp; // xyz, w unused
@@ -192,7 +194,7 @@ struct nnp_ctx {
 int nnp_launch_build(nnp_ctx *c, const int *cond_flag); // sort + lists; cond_flag != nullptr: only if *cond_flag != 0
 // aev.cu
 void nnp_launch_aev_forward(nnp_ctx *c);
-void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets);
+void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets, double *d_virial /* [6] or nullptr */);
 void nnp_aev_tri_table(uint16_t *h_tri /* [NNP_TRI_LEN] */);
 // mlp_simt.cu / mlp_tc.cu
 void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi);

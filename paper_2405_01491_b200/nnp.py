@@ -22,7 +22,7 @@ EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp
            "nnp_build_neighbors", "nnp_get_neighbors", "nnp_energy_forces", "nnp_get_aev",
            "nnp_get_atomic_energies", "nnp_md_init", "nnp_md_step", "nnp_get_state", "nnp_sync",
            "nnp_energy_forces_host", "nnp_md_step_host", "nnp_profile", "nnp_profile_read", "nnp_launch_count",
-           "nnp_aev_len", "nnp_aev_active_columns", "nnp_aev_ladder", "nnp_md_set_langevin"]
+           "nnp_aev_len", "nnp_aev_active_columns", "nnp_aev_ladder", "nnp_md_set_langevin", "nnp_energy_forces_virial"]
 
 
 class NnpError(RuntimeError):
@@ -82,6 +82,7 @@ def lib():
         L.nnp_aev_active_columns.argtypes = [vp]
         L.nnp_aev_ladder.argtypes = [vp]
         L.nnp_md_set_langevin.argtypes = [vp, C.c_float, C.c_float, C.c_uint64]
+        L.nnp_energy_forces_virial.argtypes = [vp, dp, fp, dp]
         _lib = L
     return _lib
 
@@ -237,3 +238,7 @@ def nnp_aev_ladder(ctx):
 
 def nnp_md_set_langevin(ctx, gamma, kT, seed):
     return _check(ctx, lib().nnp_md_set_langevin(ctx, float(gamma), float(kT), int(seed)))
+
+
+def nnp_energy_forces_virial(ctx, d_energy, d_forces, d_virial):
+    return _check(ctx, lib().nnp_energy_forces_virial(ctx, _ptr(d_energy), _ptr(d_forces), _ptr(d_virial)))

@@ -506,3 +506,65 @@ def test_langevin_thermostat_holds_temperature(model1):
         assert abs(np.mean(temps) - 300.0) < 20.0, np.mean(temps)
     finally:
         nnp.nnp_destroy(ctx)
+
+
+# ---------------------------------------------------------------- NEXT-2: virial
+VIRIAL_RTOL = 1e-5   # of sum |d_a (dE/dd)_b|, the scale the fp32 sums work at (the tensor itself is their cancelling sum)
+
+
+def _gpu_virial(ctx, sp, xyz, box, skin=0.0, mol_offsets=None):
+    dev = torch.device("cuda:0")
+    n = len(sp)
+    d_sp = torch.as_tensor(np.asarray(sp, dtype=np.int32), device=dev)
+    d_x = torch.as_tensor(np.asarray(xyz, dtype=np.float32), device=dev).contiguous()
+    n_mols = 1 if mol_offsets is None else len(mol_offsets) - 1
+    d_mo = None if mol_offsets is None else torch.as_tensor(np.asarray(mol_offsets, dtype=np.int32), device=dev)
+    d_E = torch.zeros(n_mols, dtype=torch.float64, device=dev)
+    d_F = torch.zeros((n, 3), dtype=torch.float32, device=dev)
+    d_V = torch.zeros(9, dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+    nnp.nnp_set_system(ctx, n, d_sp, d_x, box, n_mols, d_mo)
+    nnp.nnp_build_neighbors(ctx, skin)
+    nnp.nnp_energy_forces_virial(ctx, d_E, d_F, d_V)
+    nnp.nnp_sync(ctx)
+    return d_E.cpu().numpy(), d_F.cpu().numpy().astype(np.float64), d_V.cpu().numpy().reshape(3, 3)
+
+
+@pytest.mark.parametrize("system", ["water_periodic_skin", "mixed_periodic", "molecule"])
+def test_virial_against_oracle(model1, system):
+    consts, widths, params, om = model1
+    skin = 0.0
+    if system == "water_periodic_skin":
+        sp, xyz, box = inputs.water_box(1000, seed=41)
+        skin = 0.5                                         # entries beyond the cutoff must contribute nothing
+    elif system == "mixed_periodic":
+        sp, xyz, box = inputs.solvated_chain(n_solute=300, L=22.0, seed=43)
+        sp = sp.copy(); sp[:14] = np.arange(14) % 7
+    else:
+        sp, xyz, _ = inputs.molecule_batch(1, nmin=30, nmax=30, seed=45)
+        box = None
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp))
+    try:
+        Eg, Fg, Vg = _gpu_virial(ctx, sp, xyz, box, skin)
+        ref = orc.energy_forces_virial(om, sp, xyz, box, nbr_method=1 if box is not None else 0)
+        U.assert_parity(Eg, Fg, ref)
+        assert np.abs(Vg - ref["virial"]).max() <= VIRIAL_RTOL * ref["virial_abs"], (Vg, ref["virial"])
+        assert np.array_equal(Vg, Vg.T)
+        if box is None:                                    # Clausius form from the GPU's own forces
+            assert np.abs(Vg + xyz.T @ Fg).max() <= 3 * VIRIAL_RTOL * ref["virial_abs"]
+        # the plain entry point still gives the same energy and forces
+        E2, F2 = U.gpu_energy_forces(ctx, sp, xyz, box, skin=skin)
+        assert abs(E2[0] - Eg[0]) <= 1e-6 * abs(Eg[0]) and np.abs(F2 - Fg).max() < 1e-4
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_virial_needs_a_single_structure(model1):
+    consts, widths, params, om = model1
+    sp, xyz, offs = inputs.molecule_batch(3, seed=46)
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp), max_mols=3)
+    try:
+        with pytest.raises(nnp.NnpError):
+            _gpu_virial(ctx, sp, xyz, None, mol_offsets=offs)
+    finally:
+        nnp.nnp_destroy(ctx)
