@@ -127,6 +127,27 @@ def run_reference(args):
     return 0
 
 
+# ---- the N > 1 path ("replicas only": independent trajectories, no data-path collective).  The three pieces of host
+# logic it consists of are functions of their own so that tests/test_multi_rank.py can run them under gloo on CPU.
+def replica_seed(base, rank):
+    """Every rank simulates its own seeded system."""
+    return base + 1000 * rank
+
+
+def max_over_ranks(values, dist, device):
+    """Timings are combined as the MAX over ranks (the job is as slow as its slowest replica)."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.tolist()]
+
+
+def whole_job_rate(world, atoms_per_rank, steps, ms_max):
+    """Aggregate atom-steps/s of all replicas over the slowest replica's time (weak scaling)."""
+    return world * atoms_per_rank * steps / (ms_max * 1e-3)
+
+
 def run_ours(args):
     import torch
     from paper_2405_01491_b200 import inputs, nnp
@@ -147,7 +168,7 @@ def run_ours(args):
     nnp.lib()          # fails loudly if the CUDA library is missing
 
     # ---- workload: replica `rank` gets its own seed (independent trajectories, "replicas only")
-    sp, xyz, box = inputs.water_box(args.waters, BOX_L if args.waters == N_WATERS else None, seed=inputs.SEED0 + 3 + 1000 * rank)
+    sp, xyz, box = inputs.water_box(args.waters, BOX_L if args.waters == N_WATERS else None, seed=replica_seed(inputs.SEED0 + 3, rank))
     n = len(sp)
     vel = inputs.maxwell_boltzmann(sp, T_KELVIN, seed=inputs.SEED0 + 103 + 1000 * rank)
     consts = inputs.ani2x_constants()
@@ -223,10 +244,7 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
 
     # ---- max over ranks
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    if dist:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max, e2e_ms_max = float(t[0].item()), float(t[1].item())
+    ms_max, e2e_ms_max = max_over_ranks([ms, e2e_s * 1e3], dist, dev)
     nnp.nnp_destroy(ctx)
     if rank != 0:
         if dist:
@@ -235,7 +253,7 @@ def run_ours(args):
 
     pk = peaks()
     clocks = sampler.summary()
-    value = world * n * K / (ms_max * 1e-3)
+    value = whole_job_rate(world, n, K, ms_max)
     steps_per_s = K / (ms_max * 1e-3)
     per_stage = {nnp.STAGE_NAMES[k]: (stage_ms[k] / stage_n[k] if stage_n[k] else 0.0) for k in range(nnp.NNP_N_STAGES)}
     tot_stage = sum(per_stage.values())
