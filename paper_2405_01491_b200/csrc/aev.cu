@@ -2,7 +2,10 @@
 // Definition: SURVEY.md 8(c) O2/O3/O6 (PAPER.md L61 cosine switch, L79 Gaussian radial basis, L443 angular form
 // (0.5+0.5cos(theta-theta_n))^zeta, L55 pairs of edges with a common centre, L65/L176 forces by reverse mode).
 //
-// Persistent warps, one centre atom per warp at a time.  Neighbour rows are grouped by neighbour species (stage 1).
+// Persistent warps, one centre atom per warp at a time (forward: handed out by a ticket counter, reverse: static
+// stride - CentreQueue below).  Neighbour rows are grouped by neighbour species (stage 1).  Arithmetic of the inner
+// loops is packed f32x2 (FFMA2 / FMUL2 / FADD2, one issue slot for two lanes of math); the forward kernel evaluates
+// uniformly spaced shift sets by a Gaussian ladder (AevParams::ladder).
 //   loads:   the species-segment table of the NEXT centre is fetched one centre ahead; for the current centre all
 //            neighbour indices (radial trips + angular chunks) are loaded first, then all their positions, so one
 //            centre costs one index->position latency chain instead of one per loop trip.
