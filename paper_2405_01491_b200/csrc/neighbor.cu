@@ -39,43 +39,42 @@ __global__ void k_keys_hist(int n, const float4 *__restrict__ pos, const int *__
 }
 
 // Single-block exclusive scan of hist[0..nk) into start[0..nk]; also clears hist for reuse as cursor.
-// Each of the 1024 threads owns one contiguous chunk (serial sum, one block-wide scan, serial write-back), so the
-// whole scan costs two passes over the keys and three block barriers.
+// The block walks the keys in tiles of 1024 with coalesced loads (thread t owns element tile + t), scans each tile
+// with warp shuffles and carries the running total: one pass over the keys, two block barriers per tile.
 __global__ void __launch_bounds__(1024) k_scan(int nk, int *__restrict__ hist, int *__restrict__ start, const int *cond)
 {
     if (cond && *cond == 0) return;
     __shared__ int warp_sums[32];
+    __shared__ int carry_s;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int chunk = (nk + (int)blockDim.x - 1) / (int)blockDim.x;
-    const int beg = min(nk, (int)threadIdx.x * chunk), end = min(nk, beg + chunk);
-    int sum = 0;
-    for (int i = beg; i < end; ++i) sum += hist[i];
-    int x = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int y = __shfl_up_sync(0xffffffffu, x, o);
-        if (lane >= o) x += y;
-    }
-    if (lane == 31) warp_sums[wid] = x;
+    if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
-    if (wid == 0) {
-        int w = lane < ((int)blockDim.x >> 5) ? warp_sums[lane] : 0;
+    for (int base = 0; base < nk; base += 1024) {
+        const int i = base + (int)threadIdx.x;
+        const int v = i < nk ? hist[i] : 0;
+        if (i < nk) hist[i] = 0;
+        int x = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            int y = __shfl_up_sync(0xffffffffu, w, o);
+            const int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sums[wid] = x;
+        __syncthreads();
+        const int carry = carry_s;
+        int w = warp_sums[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, w, o);
             if (lane >= o) w += y;
         }
-        warp_sums[lane] = w; // inclusive
+        const int before = __shfl_sync(0xffffffffu, w, wid) - warp_sums[wid]; // sum of the warps in front of this one
+        if (i < nk) start[i] = carry + before + x - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = carry + before + x; // inclusive total of the tile
     }
     __syncthreads();
-    int run = (wid > 0 ? warp_sums[wid - 1] : 0) + x - sum;
-    for (int i = beg; i < end; ++i) {
-        const int v = hist[i];
-        start[i] = run;
-        hist[i] = 0;
-        run += v;
-    }
-    if (threadIdx.x == blockDim.x - 1) start[nk] = run;
+    if (threadIdx.x == 0) start[nk] = carry_s;
 }
 
 __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ start,
