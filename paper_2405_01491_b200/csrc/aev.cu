@@ -76,6 +76,12 @@ __device__ __forceinline__ float lg2(float x)
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float rcp(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ float rsq(float x)
 {
     float y;
@@ -155,8 +161,8 @@ __device__ __forceinline__ LanePart partition(int n_b, int tag_b, int *own, int 
     if (N == 0) return pt;
     int I = (N + 31) >> 5, L_b;
     for (;;) {
-        // ceil(n_b / I): the fractional part of n_b / I is 0 or >= 1/I >= 1/80, far above the rounding error
-        L_b = (int)((float)n_b * __frcp_rn((float)I) + 0.999f);
+        // ceil(n_b / I): the fractional part of n_b / I is 0 or >= 1/I >= 1/80, far above the error of the approximate reciprocal
+        L_b = (int)((float)n_b * rcp((float)I) + 0.999f);
         if (__reduce_add_sync(kFull, L_b) <= 32) break;
         ++I;
     }
@@ -345,7 +351,7 @@ __device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const C
                 const float fc = 0.5f * cs_ + 0.5f;
                 sm.fr[p] = make_float2(BWD ? fc : lg2(fc) + 0.5f, rinv);
                 if constexpr (BWD) {
-                    sm.dfc[p] = -0.5f * P.pi_rca * sn;
+                    sm.dfc[p] = P.nh_pi_rca * sn;
                     sm.j[p] = j;
                 }
             }
@@ -391,9 +397,6 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 #pragma unroll
     for (int q = 0; q < NNP_MAX_SPECIES - 1; ++q)
         if (lane == q && q < P.np) my_s = P.plist[q];
-    float hcz[NNP_NSHF_Z], hsz[NNP_NSHF_Z];
-#pragma unroll
-    for (int z = 0; z < NNP_NSHF_Z; ++z) { hcz[z] = 0.5f * P.cos_z[z]; hsz[z] = 0.5f * P.sin_z[z]; }
     // constant factors of the ladder, applied once per feature where lane = feature (1 without ladder)
     const float lad_r = LAD ? P.lad_r[lane & 15] : 1.0f, lad_a = LAD ? P.lad_a[lane >> 2] : 1.0f;
 
@@ -429,11 +432,11 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                         float2 t[NNP_NSHF_R / 8];
 #pragma unroll
                         for (int mp = 0; mp < NNP_NSHF_R / 8; ++mp) {
-                            const float2 w = add2(u, make_float2(-P.kr_shf[8 * mp + 1], -P.kr_shf[8 * mp + 5]));
+                            const float2 w = add2(u, P.nkr_anc2[mp]);
                             const float2 ww = mul2(w, w);
                             t[mp] = mul2(fc, make_float2(ex2(-ww.x), ex2(-ww.y)));
                         }
-                        const float x = (2.0f * P.dlt_r) * (u.x - P.kr_shf[1]);
+                        const float x = P.two_dlt_r * (u.x - P.kr_shf[1]);
                         const float q = ex2(x);
                         const float2 pq0 = make_float2(ex2(-x), 1.0f), pq1 = make_float2(q, q * q);
 #pragma unroll
@@ -446,7 +449,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                     } else {
 #pragma unroll
                         for (int k = 0; k < NNP_NSHF_R / 2; ++k) {
-                            const float2 w = add2(u, make_float2(-P.kr_shf[2 * k], -P.kr_shf[2 * k + 1]));
+                            const float2 w = add2(u, P.nkr_shf2[k]);
                             const float2 ww = mul2(w, w);
                             acc[k] = fma2(fc, make_float2(ex2(-ww.x), ex2(-ww.y)), acc[k]);
                         }
@@ -515,7 +518,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 const int ns = sm.seg[wcs + 1] - a0;
                 npairs = same ? ns * (ns - 1) / 2 : ns * nt;
             }
-            const float inv_nt = __frcp_rn((float)max(nt, 1));
+            const float inv_nt = rcp((float)max(nt, 1));
             const float2 zeta2 = bc2(P.zeta), half2 = bc2(0.5f);
             for (int q = pt.r; q < npairs; q += pt.L) {
                 int ia, ib;
@@ -532,17 +535,16 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 float2 fz[NNP_NSHF_Z / 2];
 #pragma unroll
                 for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
-                    const float2 base = fma2(cc2, make_float2(hcz[2 * zp], hcz[2 * zp + 1]),
-                                             fma2(sn2, make_float2(hsz[2 * zp], hsz[2 * zp + 1]), half2));
+                    const float2 base = fma2(cc2, P.hcz2[zp], fma2(sn2, P.hsz2[zp], half2));
                     const float2 e = fma2(zeta2, make_float2(lg2(base.x), lg2(base.y)), lff2);
                     fz[zp] = make_float2(ex2(e.x), ex2(e.y));
                 }
-                const float2 u = bc2(0.5f * P.ka * (dj.w + dk.w));
+                const float2 u = bc2(P.half_ka * (dj.w + dk.w));
                 float2 ra[NNP_NSHF_A / 2]; // radial factors (a, a+1); with the ladder: without their constant factors
                 if constexpr (LAD) {
-                    const float2 w = add2(u, make_float2(-P.ka_shf[1], -P.ka_shf[5])); // anchors a = 1, 5
+                    const float2 w = add2(u, P.nka_anc2); // anchors a = 1, 5
                     const float2 ww = mul2(w, w);
-                    const float x = (2.0f * P.dlt_a) * w.x;
+                    const float x = P.two_dlt_a * w.x;
                     const float q = ex2(x);
                     const float2 pq0 = make_float2(ex2(-x), 1.0f), pq1 = make_float2(q, q * q);
                     const float e0 = ex2(-ww.x), e1 = ex2(-ww.y);
@@ -551,7 +553,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
                 } else {
 #pragma unroll
                     for (int ap = 0; ap < NNP_NSHF_A / 2; ++ap) {
-                        const float2 w = add2(u, make_float2(-P.ka_shf[2 * ap], -P.ka_shf[2 * ap + 1]));
+                        const float2 w = add2(u, P.nka_shf2[ap]);
                         const float2 ww = mul2(w, w);
                         ra[ap] = make_float2(ex2(-ww.x), ex2(-ww.y));
                     }
@@ -610,10 +612,13 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                double *__restrict__ virial /* [6] xx yy zz xy xz yz, VIR only */)
 {
     extern __shared__ __align__(16) uint8_t smem_dyn[];
-    WarpSmemBwd *smem = reinterpret_cast<WarpSmemBwd *>(smem_dyn);
-    float *gs = reinterpret_cast<float *>(smem_dyn + kWarps * sizeof(WarpSmemBwd)) + (threadIdx.x >> 5) * kGsMax; // GS only
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    WarpSmemBwd &sm = smem[wid];
+    // The warp's shared-memory base is made opaque to the compiler: left alone it re-derives the address from
+    // %tid / the shared window (two S2R + four ALU instructions) inside every trip of the pair loop.
+    uint32_t sm_addr = (uint32_t)__cvta_generic_to_shared(smem_dyn) + (uint32_t)wid * (uint32_t)sizeof(WarpSmemBwd);
+    asm volatile("mov.b32 %0, %0;" : "+r"(sm_addr));
+    WarpSmemBwd &sm = *reinterpret_cast<WarpSmemBwd *>(__cvta_shared_to_generic(sm_addr));
+    float *gs = reinterpret_cast<float *>(smem_dyn + kWarps * sizeof(WarpSmemBwd)) + wid * kGsMax; // GS only
     int bcs, bct;
     block_of_lane(P.np, lane, bcs, bct);
     const int nb_tot = P.np * (P.np + 1) / 2;
@@ -621,14 +626,8 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
 #pragma unroll
     for (int q = 0; q < NNP_MAX_SPECIES - 1; ++q)
         if (lane == q && q < P.np) my_s = P.plist[q];
-    float hcz[NNP_NSHF_Z], hsz[NNP_NSHF_Z];
-#pragma unroll
-    for (int z = 0; z < NNP_NSHF_Z; ++z) { hcz[z] = 0.5f * P.cos_z[z]; hsz[z] = 0.5f * P.sin_z[z]; }
-    const float k_ang0 = 0.5f * P.zeta * 0.95f * 2.0f; // x2: hcz/hsz carry the 1/2 of the base
-    const float zm1 = P.zeta - 1.0f;
-    // d/drb exp(-eta (rb - s)^2) = -2 eta (rb - s) ra = (-2 eta / ka) w ra with w = ka (rb - s)
-    const float drb_scale = -2.0f * P.eta_a / P.ka;
-    const float dr_scale = -2.0f * P.eta_r / P.kr;
+    // P.k_ang0 = zeta 0.95 (hcz2 / hsz2 carry the 1/2 of the base); d/drb exp(-eta (rb - s)^2) = -2 eta (rb - s) ra =
+    // (-2 eta / ka) w ra with w = ka (rb - s): P.half_drb_scale, P.dr_scale (AevParams, nnp_aev_derive)
     float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.alp);
 
     // Centres are handed out dynamically (one ticket per centre): the cost of a centre varies with its pair count,
@@ -683,13 +682,13 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                     const float r = r2 * rinv;
                     float sn, cs_;
                     __sincosf(P.pi_rcr * r, &sn, &cs_);
-                    const float2 fc = bc2((0.5f * cs_ + 0.5f) * dr_scale);
-                    const float2 dfc = bc2(-0.5f * P.pi_rcr * sn);
+                    const float2 fc = bc2((0.5f * cs_ + 0.5f) * P.dr_scale);
+                    const float2 dfc = bc2(P.nh_pi_rcr * sn);
                     const float2 u = bc2(P.kr * r);
                     float2 acc = make_float2(0.f, 0.f);
 #pragma unroll
                     for (int k = 0; k < NNP_NSHF_R / 2; ++k) {
-                        const float2 w = add2(u, make_float2(-P.kr_shf[2 * k], -P.kr_shf[2 * k + 1]));
+                        const float2 w = add2(u, P.nkr_shf2[k]);
                         const float2 ww = mul2(w, w);
                         const float2 e = make_float2(ex2(-ww.x), ex2(-ww.y));
                         acc = fma2(mul2(gr[k], e), fma2(w, fc, dfc), acc);
@@ -748,7 +747,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const int ns = sm.seg[wcs + 1] - a0;
                 npairs = same ? ns * (ns - 1) / 2 : ns * nt;
             }
-            const float inv_nt = __frcp_rn((float)max(nt, 1));
+            const float inv_nt = rcp((float)max(nt, 1));
             float2 gw[NNP_ANG_BLOCK / 2]; // [a][z pair]
             {
                 const int pb = wcs * (2 * P.np + 1 - wcs) / 2 + (wct - wcs);
@@ -762,7 +761,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                     gw[2 * q4 + 1] = make_float2(v.z * sc0, v.w * sc0);
                 }
             }
-            const float2 zm12 = bc2(zm1), half2 = bc2(0.5f);
+            const float2 zm12 = bc2(P.zm1), half2 = bc2(0.5f);
             for (int q = pt.r; q < npairs; q += pt.L) {
                 int ia, ib;
                 decode_pair(q, same, nt, inv_nt, tri, ia, ib);
@@ -779,22 +778,22 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 float2 fz[NNP_NSHF_Z / 2], dfz[NNP_NSHF_Z / 2]; // F_z and (dF_z/dcos(theta)) / k_ang
 #pragma unroll
                 for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) {
-                    const float2 hc = make_float2(hcz[2 * zp], hcz[2 * zp + 1]), hs = make_float2(hsz[2 * zp], hsz[2 * zp + 1]);
-                    const float2 base = fma2(cc2, hc, fma2(sn2, hs, half2));
+                    const float2 hc = P.hcz2[zp];
+                    const float2 base = fma2(cc2, hc, fma2(sn2, P.hsz2[zp], half2));
                     const float2 e = mul2(zm12, make_float2(lg2(base.x), lg2(base.y)));
                     const float2 pw = make_float2(ex2(e.x), ex2(e.y)); // base^(zeta-1)
                     fz[zp] = mul2(pw, base);
                     // dF/dtheta' = -(zeta/2) sin(theta'-phi) base^(zeta-1); dtheta'/dcos = -0.95/sn
-                    dfz[zp] = mul2(fma2(sn2, hc, mul2(cc2, make_float2(-hs.x, -hs.y))), pw);
+                    dfz[zp] = mul2(fma2(sn2, hc, mul2(cc2, P.nhsz2[zp])), pw);
                 }
                 // A_z = sum_a g[a][z] ra_a (value and angular derivative), C_z = sum_a g[a][z] ra_a w_a (radial derivative)
                 float2 Az[NNP_NSHF_Z / 2], Cz[NNP_NSHF_Z / 2];
 #pragma unroll
                 for (int zp = 0; zp < NNP_NSHF_Z / 2; ++zp) { Az[zp] = make_float2(0.f, 0.f); Cz[zp] = make_float2(0.f, 0.f); }
-                const float2 u = bc2(0.5f * P.ka * (dj.w + dk.w));
+                const float2 u = bc2(P.half_ka * (dj.w + dk.w));
 #pragma unroll
                 for (int ap = 0; ap < NNP_NSHF_A / 2; ++ap) {
-                    const float2 w = add2(u, make_float2(-P.ka_shf[2 * ap], -P.ka_shf[2 * ap + 1]));
+                    const float2 w = add2(u, P.nka_shf2[ap]);
                     const float2 ww = mul2(w, w);
                     const float2 ra = make_float2(ex2(-ww.x), ex2(-ww.y));
                     const float2 rw = mul2(ra, w);
@@ -813,8 +812,8 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 float dE_dcs = D2.x + D2.y;
                 const float dE_drb = R2.x + R2.y;
                 const float ff = fj.x * fk.x;
-                dE_dcs *= ff * (k_ang0 * sn_inv);
-                const float half_drb = (0.5f * drb_scale) * dE_drb * ff;
+                dE_dcs *= ff * (P.k_ang0 * sn_inv);
+                const float half_drb = P.half_drb_scale * dE_drb * ff;
                 const float dE_drj = fmaf(T * sm.dfc[ia], fk.x, half_drb);
                 const float dE_drk = fmaf(T * fj.x, sm.dfc[ib], half_drb);
                 const float beta = dE_dcs * rjk_inv;

@@ -250,6 +250,32 @@ void setup_ladder(AevParams &a, const nnp_params *p)
     }
 }
 
+} // namespace
+
+void nnp_aev_derive(AevParams &a)
+{
+    for (int z = 0; z < NNP_NSHF_Z / 2; ++z) {
+        a.hcz2[z] = make_float2(0.5f * a.cos_z[2 * z], 0.5f * a.cos_z[2 * z + 1]);
+        a.hsz2[z] = make_float2(0.5f * a.sin_z[2 * z], 0.5f * a.sin_z[2 * z + 1]);
+        a.nhsz2[z] = make_float2(-0.5f * a.sin_z[2 * z], -0.5f * a.sin_z[2 * z + 1]);
+    }
+    for (int k = 0; k < NNP_NSHF_A / 2; ++k) a.nka_shf2[k] = make_float2(-a.ka_shf[2 * k], -a.ka_shf[2 * k + 1]);
+    for (int k = 0; k < NNP_NSHF_R / 2; ++k) a.nkr_shf2[k] = make_float2(-a.kr_shf[2 * k], -a.kr_shf[2 * k + 1]);
+    for (int m = 0; m < NNP_NSHF_R / 8; ++m) a.nkr_anc2[m] = make_float2(-a.kr_shf[8 * m + 1], -a.kr_shf[8 * m + 5]);
+    a.nka_anc2 = make_float2(-a.ka_shf[1], -a.ka_shf[5]);
+    a.half_ka = 0.5f * a.ka;
+    a.k_ang0 = 0.5f * a.zeta * 0.95f * 2.0f;
+    a.zm1 = a.zeta - 1.0f;
+    a.half_drb_scale = 0.5f * (-2.0f * a.eta_a / a.ka);
+    a.dr_scale = -2.0f * a.eta_r / a.kr;
+    a.nh_pi_rcr = -0.5f * a.pi_rcr;
+    a.nh_pi_rca = -0.5f * a.pi_rca;
+    a.two_dlt_r = 2.0f * a.dlt_r;
+    a.two_dlt_a = 2.0f * a.dlt_a;
+}
+
+namespace {
+
 int check_flags(nnp_ctx *c)
 {
     int h[3];
@@ -553,6 +579,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     for (int k = 0; k < NNP_NSHF_A; ++k) a.shf_a[k] = p->shf_a[k];
     for (int k = 0; k < NNP_NSHF_Z; ++k) { a.cos_z[k] = (float)cos((double)p->shf_z[k]); a.sin_z[k] = (float)sin((double)p->shf_z[k]); }
     setup_ladder(a, p);
+    nnp_aev_derive(a);
 
     // ---- weights: W [in_pad][out], Wt [out][in_pad], b [out] for every (net, species, layer)
     c->layers = new LayerW[(size_t)c->n_nets * S * NNP_NLAYERS];

@@ -66,7 +66,23 @@ struct AevParams {
     float lad_a[NNP_NSHF_A];
     int periodic;
     float box[3], inv_box[3];
+    // Derived constants of the inner loops, computed once on the host (nnp_aev_derive): the kernels take them straight
+    // from the parameter bank (the pairs as one 64-bit uniform-register operand of the packed f32x2 instructions)
+    // instead of re-deriving them per loop trip under register pressure.
+    float2 hcz2[NNP_NSHF_Z / 2], hsz2[NNP_NSHF_Z / 2], nhsz2[NNP_NSHF_Z / 2]; // 1/2 cos ShfZ, 1/2 sin ShfZ, -1/2 sin ShfZ
+    float2 nka_shf2[NNP_NSHF_A / 2];  // -ka_shf, pairs (2a, 2a+1)
+    float2 nkr_shf2[NNP_NSHF_R / 2];  // -kr_shf, pairs (2k, 2k+1)
+    float2 nkr_anc2[NNP_NSHF_R / 8];  // ladder anchors (-kr_shf[8m+1], -kr_shf[8m+5])
+    float2 nka_anc2;                  // (-ka_shf[1], -ka_shf[5])
+    float half_ka;                    // ka / 2: ka (r_ij + r_ik) / 2
+    float k_ang0;                     // zeta * 0.95 (d base^zeta / d cos theta, with the 1/2 of the base folded in)
+    float zm1;                        // zeta - 1
+    float half_drb_scale;             // (1/2) (-2 eta_a / ka)
+    float dr_scale;                   // -2 eta_r / kr
+    float nh_pi_rcr, nh_pi_rca;       // -(1/2) pi / cutoff: fc' = nh_pi_rc sin(pi r / rc)
+    float two_dlt_r, two_dlt_a;
 };
+void nnp_aev_derive(AevParams &a);
 
 // ---- grouped GEMM description (stage 3/4) --------------------------------------------------------
 enum GemmEpilogue {
