@@ -397,17 +397,27 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
         const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
         const int sub_r = lane >> 3, sub_c = (lane & 7) * 4; // cooperative access: 4 rows x 8 x 16 B per instruction
         const float alpha = batch.alpha, inv_alpha = 1.0f / batch.alpha;
+        // In-place epilogues read the previous contents of C, written by the forward pass ~200 MB of traffic ago: the row
+        // of the NEXT tile this thread owns is pulled into L2 one tile ahead, so that the chunk loads below see an L2
+        // round trip instead of a DRAM one (they run only one 32-column chunk ahead of their use).
+        auto l2_prefetch_tile = [&](int t2) {
+            if (!(EPI == EPI_DCELU || EPI == EPI_ACCUM) || t2 >= t_end) return;
+            const TileCoord c2 = tile_coord(batch, t2);
+            const TcGroup &g2 = batch.g[c2.gi];
+            const int m2 = c2.m0 + row;
+            if (m2 < g2.M) {
+                const char *p2 = reinterpret_cast<const char *>(g2.C + (size_t)m2 * g2.ldc + c2.n0);
+                for (int off = 0; off < g2.NT * 4; off += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(p2 + off));
+            }
+        };
+        l2_prefetch_tile(t_beg);
         int lt = 0;
         for (int t = t_beg; t < t_end; ++t, ++lt) {
             const TileCoord tc = tile_coord(batch, t);
             const TcGroup &g = batch.g[tc.gi];
             const int b = lt & 1;
-            mbar_wait(bar_accf + 8 * b, (lt >> 1) & 1);
-#ifdef NNP_TC_TRACE
-            if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K) + 1; TRACE(7); }
-#endif
-            tc_fence_after();
             const int mrow0 = tc.m0 + quarter * 32; // first global row of this warp's 32 rows
+            l2_prefetch_tile(t + 1);
             const int m = mrow0 + lane;
             const bool rowok = m < g.M;
             float esum = 0.f;
@@ -430,7 +440,12 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     }
                 }
             };
-            prefetch(0);
+            prefetch(0); // issued before the wait for the accumulator: its latency hides behind the MMAs of this tile
+            mbar_wait(bar_accf + 8 * b, (lt >> 1) & 1);
+#ifdef NNP_TC_TRACE
+            if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K) + 1; TRACE(7); }
+#endif
+            tc_fence_after();
             for (int c0 = 0; c0 < g.NT; c0 += 32) {
                 const int w = min(32, g.NT - c0); // 32 or 16 (warp-uniform)
                 float *cbase = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
