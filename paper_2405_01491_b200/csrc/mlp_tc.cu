@@ -30,14 +30,16 @@ constexpr int UMMA_K = 8;                 // tf32
 constexpr int NT_MAX = 192;               // columns per output tile = the layer width up to 192; wider layers in equal parts
 constexpr int STAGES_MAX = 4;             // shared-memory ring: 4 stages of 48 KiB (NT <= 128) or 3 of up to 64 KiB
 constexpr int A_TILE_BYTES = TILE_M * BLOCK_K * 4;          // 16 KiB
-constexpr int EPI_STG_LD = 36;                                   // floats per staged row (16-byte aligned, conflict-free)
-constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;               // per epilogue warp: one 32 x 32 chunk
-constexpr int SMEM_FIXED = 1024 /*align*/ + 256 /*barriers*/ + 4 * EPI_STG_BYTES;
+constexpr int EPI_WARPS = 8;                                     // two per TMEM lane quarter, on alternate column chunks
+constexpr int EPI_CW = 16;                                       // columns per epilogue chunk
+constexpr int EPI_STG_LD = 20;                                   // floats per staged row (16-byte aligned, conflict-free)
+constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;               // per epilogue warp: one 32 x 16 chunk
+constexpr int SMEM_FIXED = 1024 /*align*/ + 256 /*barriers*/ + EPI_WARPS * EPI_STG_BYTES;
 constexpr int SMEM_LIMIT = 227 * 1024;
 constexpr int TMEM_COLS = 512;
 // TMEM: two accumulator buffers at columns 0 and acc_stride (128 / 160 / 192), behind them a_slots = 4 / 3 / 2 A slots
 // (hi 32 + lo 32 columns); K block `it` uses slot it % a_slots and shared-memory stage it % stages (a_slots <= stages).
-constexpr int THREADS = 448;              // warp 0 TMA, warp 1 MMA, warps 2-9 converters (two groups), warps 10-13 epilogue
+constexpr int THREADS = 576;              // warp 0 TMA, warp 1 MMA, warps 2-9 converters (two groups), warps 10-17 epilogue
 
 struct TcGroup {
     CUtensorMap mapA, mapBhi, mapBlo;
@@ -255,7 +257,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar_accf + 8 * b, 1);
-            mbar_init(bar_acce + 8 * b, 128);
+            mbar_init(bar_acce + 8 * b, EPI_WARPS * 32);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -388,18 +390,25 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             }
         }
     } else {
-        // ===== epilogue (warps 10..13 -> lane quarters 2,3,0,1): this thread owns accumulator row `row`.
-        // Global traffic goes through a per-warp 32 x 32 staging chunk so that every LDG/STG covers full 128-byte lines.
+        // ===== epilogue: warps 10..17 -> lane quarters 2,3,0,1,2,3,0,1; this thread owns accumulator row `row`.
+        // The accumulator is drained in 16-column chunks; the two warps of a lane quarter take alternate chunks (one warp
+        // per quarter could not keep up with the MMAs of a short-K tile: the reverse layers ran at 32 % tensor activity).
+        // Global traffic goes through a per-warp 32 x 16 staging chunk so that every LDG/STG covers whole 64-byte row
+        // segments (8 rows per instruction).
+        const int ew = warp - 10;
         const int quarter = warp & 3;
+        const int half = ew >> 2; // parity of the chunks this warp serves
         const int row = quarter * 32 + lane;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
-        const uint32_t stg = bar_base + 256 + (uint32_t)(warp - 10) * EPI_STG_BYTES;
+        const uint32_t stg = bar_base + 256 + (uint32_t)ew * EPI_STG_BYTES;
         const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
-        const int sub_r = lane >> 3, sub_c = (lane & 7) * 4; // cooperative access: 4 rows x 8 x 16 B per instruction
+        // cooperative access: 8 rows x 4 x 16 B per instruction; a quarter-warp covers rows q and q + 4, whose staged
+        // copies are 80 words apart (bank offset 16): conflict-free with the 20-word row stride
+        const int sub_r = (lane >> 3) + 4 * ((lane >> 2) & 1), sub_c = (lane & 3) * 4;
         const float alpha = batch.alpha, inv_alpha = 1.0f / batch.alpha;
         // In-place epilogues read the previous contents of C, written by the forward pass ~200 MB of traffic ago: the row
-        // of the NEXT tile this thread owns is pulled into L2 one tile ahead, so that the chunk loads below see an L2
-        // round trip instead of a DRAM one (they run only one 32-column chunk ahead of their use).
+        // of the NEXT tile this thread owns is pulled into L2 one tile ahead (the two warps of a quarter take alternate
+        // lines), so that the chunk loads below see an L2 round trip instead of a DRAM one.
         auto l2_prefetch_tile = [&](int t2) {
             if (!(EPI == EPI_DCELU || EPI == EPI_ACCUM) || t2 >= t_end) return;
             const TileCoord c2 = tile_coord(batch, t2);
@@ -407,7 +416,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             const int m2 = c2.m0 + row;
             if (m2 < g2.M) {
                 const char *p2 = reinterpret_cast<const char *>(g2.C + (size_t)m2 * g2.ldc + c2.n0);
-                for (int off = 0; off < g2.NT * 4; off += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(p2 + off));
+                for (int off = half * 128; off < g2.NT * 4; off += 256) asm volatile("prefetch.global.L2 [%0];" ::"l"(p2 + off));
             }
         };
         l2_prefetch_tile(t_beg);
@@ -423,87 +432,83 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             float esum = 0.f;
             // Operands from global memory are fetched one chunk ahead (the L1 is only ~12 KB next to 216 KB of
             // shared memory, so every one of these loads is an L2 round trip): bias / w4 one column per lane
-            // (redistributed with shuffles), previous contents 8 x 16 B per lane, coalesced.
+            // (redistributed with shuffles), previous contents 4 x 16 B per lane, coalesced.
             float bias_l = 0.f, w4_l = 0.f;
-            float4 pre[8];
+            float4 pre[4];
             auto prefetch = [&](int c0) {
-                const int w = min(32, g.NT - c0);
-                if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bias_l = lane < w ? g.bias[tc.n0 + c0 + lane] : 0.f;
-                if (EPI == EPI_CELU_OUT) w4_l = lane < w ? g.w4[tc.n0 + c0 + lane] : 0.f;
+                if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bias_l = lane < EPI_CW ? g.bias[tc.n0 + c0 + lane] : 0.f;
+                if (EPI == EPI_CELU_OUT) w4_l = lane < EPI_CW ? g.w4[tc.n0 + c0 + lane] : 0.f;
                 if (EPI == EPI_DCELU || EPI == EPI_ACCUM) {
                     const float *cb = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int r = i * 4 + sub_r;
-                        pre[i] = (mrow0 + r < g.M && sub_c < w) ? *reinterpret_cast<const float4 *>(cb + (size_t)r * g.ldc + sub_c)
-                                                               : make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int i = 0; i < 4; ++i) {
+                        const int r = i * 8 + sub_r;
+                        pre[i] = mrow0 + r < g.M ? *reinterpret_cast<const float4 *>(cb + (size_t)r * g.ldc + sub_c)
+                                                 : make_float4(0.f, 0.f, 0.f, 0.f);
                     }
                 }
             };
-            prefetch(0); // issued before the wait for the accumulator: its latency hides behind the MMAs of this tile
+            const int c_first = half * EPI_CW;
+            if (c_first < g.NT) prefetch(c_first); // before the wait for the accumulator: hides behind the MMAs of this tile
             mbar_wait(bar_accf + 8 * b, (lt >> 1) & 1);
 #ifdef NNP_TC_TRACE
             if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K) + 1; TRACE(7); }
 #endif
             tc_fence_after();
-            for (int c0 = 0; c0 < g.NT; c0 += 32) {
-                const int w = min(32, g.NT - c0); // 32 or 16 (warp-uniform)
+
+            for (int c0 = c_first; c0 < g.NT; c0 += 2 * EPI_CW) {
                 float *cbase = g.C + (size_t)mrow0 * g.ldc + tc.n0 + c0;
                 const float bias_c = bias_l, w4_c = w4_l;
                 if (EPI == EPI_DCELU || EPI == EPI_ACCUM) { // previous contents -> staging
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int r = i * 4 + sub_r;
+                    for (int i = 0; i < 4; ++i) {
+                        const int r = i * 8 + sub_r;
                         asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(pre[i].x), "f"(pre[i].y), "f"(pre[i].z), "f"(pre[i].w) : "memory");
                     }
                     __syncwarp();
                 }
-                if (c0 + 32 < g.NT) prefetch(c0 + 32);
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    if (h * 16 >= w) break;
-                    uint32_t acc[16];
-                    tmem_ld16(lane_addr + (uint32_t)(b * batch.acc_stride) + c0 + h * 16, acc);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (c0 + 2 * EPI_CW < g.NT) prefetch(c0 + 2 * EPI_CW);
+                uint32_t acc[16];
+                tmem_ld16(lane_addr + (uint32_t)(b * batch.acc_stride) + c0, acc);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #ifdef NNP_TC_TRACE
-                    if (threadIdx.x == 320 && c0 == 0 && h == 0) { const int it = lt * (g.K / BLOCK_K) + 2; TRACE(7); }
+                if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 2; TRACE(7); }
 #endif
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const int col = h * 16 + 4 * q;
-                        float4 o;
-                        float *ov = reinterpret_cast<float *>(&o);
-                        float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (EPI == EPI_DCELU || EPI == EPI_ACCUM)
-                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(prev.x), "=f"(prev.y), "=f"(prev.z), "=f"(prev.w) : "r"(my_row + col * 4));
-                        const float *pv = reinterpret_cast<const float *>(&prev);
+                for (int q = 0; q < 4; ++q) {
+                    const int col = 4 * q;
+                    float4 o;
+                    float *ov = reinterpret_cast<float *>(&o);
+                    float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (EPI == EPI_DCELU || EPI == EPI_ACCUM)
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(prev.x), "=f"(prev.y), "=f"(prev.z), "=f"(prev.w) : "r"(my_row + col * 4));
+                    const float *pv = reinterpret_cast<const float *>(&prev);
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            float v = __uint_as_float(acc[4 * q + e]);
-                            float bv = 0.f, wv = 0.f;
-                            if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bv = __shfl_sync(0xffffffffu, bias_c, col + e);
-                            if (EPI == EPI_CELU_OUT) wv = __shfl_sync(0xffffffffu, w4_c, col + e);
-                            if (EPI == EPI_CELU) v = celu_fwd(v + bv, alpha, inv_alpha);
-                            if (EPI == EPI_CELU_OUT) {
-                                const float hh = celu_fwd(v + bv, alpha, inv_alpha);
-                                esum = fmaf(hh, wv, esum);
-                                v = wv * celu_grad_from_h(hh, inv_alpha);
-                            }
-                            if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[e], inv_alpha);
-                            if (EPI == EPI_ACCUM) v += pv[e];
-                            ov[e] = v;
+                    for (int e = 0; e < 4; ++e) {
+                        float v = __uint_as_float(acc[4 * q + e]);
+                        float bv = 0.f, wv = 0.f;
+                        if (EPI == EPI_CELU || EPI == EPI_CELU_OUT) bv = __shfl_sync(0xffffffffu, bias_c, col + e);
+                        if (EPI == EPI_CELU_OUT) wv = __shfl_sync(0xffffffffu, w4_c, col + e);
+                        if (EPI == EPI_CELU) v = celu_fwd(v + bv, alpha, inv_alpha);
+                        if (EPI == EPI_CELU_OUT) {
+                            const float hh = celu_fwd(v + bv, alpha, inv_alpha);
+                            esum = fmaf(hh, wv, esum);
+                            v = wv * celu_grad_from_h(hh, inv_alpha);
                         }
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + col * 4), "f"(o.x), "f"(o.y), "f"(o.z), "f"(o.w) : "memory");
+                        if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[e], inv_alpha);
+                        if (EPI == EPI_ACCUM) v += pv[e];
+                        ov[e] = v;
                     }
+                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + col * 4), "f"(o.x), "f"(o.y), "f"(o.z), "f"(o.w) : "memory");
                 }
 #ifdef NNP_TC_TRACE
                 if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 3; TRACE(7); }
 #endif
                 __syncwarp();
 #pragma unroll
-                for (int i = 0; i < 8; ++i) { // staging -> global, full 128-byte lines
-                    const int r = i * 4 + sub_r;
-                    if (mrow0 + r < g.M && sub_c < w) {
+                for (int i = 0; i < 4; ++i) { // staging -> global, whole 64-byte row segments
+                    const int r = i * 8 + sub_r;
+                    if (mrow0 + r < g.M) {
                         float4 v;
                         asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
                         *reinterpret_cast<float4 *>(cbase + (size_t)r * g.ldc + sub_c) = v;
@@ -520,7 +525,7 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
 #ifdef NNP_TC_TRACE
             if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K); TRACE(7); }
 #endif
-            // a layer wider than one tile contributes its share of the output-layer dot from each half
+            // every epilogue warp (both chunk parities, each n-part of a wide layer) adds its share of the output-layer dot
             if (EPI == EPI_CELU_OUT && rowok) atomicAdd(g.e_atom + m, esum);
         }
     }

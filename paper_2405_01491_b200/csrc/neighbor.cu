@@ -39,42 +39,81 @@ __global__ void k_keys_hist(int n, const float4 *__restrict__ pos, const int *__
 }
 
 // Single-block exclusive scan of hist[0..nk) into start[0..nk]; also clears hist for reuse as cursor.
-// The block walks the keys in tiles of 1024 with coalesced loads (thread t owns element tile + t), scans each tile
-// with warp shuffles and carries the running total: one pass over the keys, two block barriers per tile.
+// A pass covers kScanTiles tiles of 1024 keys (thread t owns key tile * 1024 + t, coalesced): all loads of a pass are
+// issued before the first use (one global-memory latency per pass, not one per tile), each tile is scanned inside its
+// warps with shuffles, and three block barriers per PASS (warp totals -> per-tile offsets -> tile bases) replace the two
+// per tile of a tile-serial scan.  The 98k water box (7 x 17^3 = 34,391 keys) is one pass.
+constexpr int kScanTiles = 40;
 __global__ void __launch_bounds__(1024) k_scan(int nk, int *__restrict__ hist, int *__restrict__ start, const int *cond)
 {
     if (cond && *cond == 0) return;
-    __shared__ int warp_sums[32];
+    __shared__ int ws[kScanTiles][33];   // [tile][warp]: warp totals, then exclusive offsets of the warps inside the tile
+    __shared__ int tile_tot[2 * 32];     // tile totals, then exclusive tile bases (carry included)
     __shared__ int carry_s;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < nk; base += 1024) {
-        const int i = base + (int)threadIdx.x;
-        const int v = i < nk ? hist[i] : 0;
-        if (i < nk) hist[i] = 0;
-        int x = v;
+    const unsigned kFull = 0xffffffffu;
+    const int tid = (int)threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    static_assert(kScanTiles <= 64, "tile totals are scanned by one warp, two per lane");
+    if (tid == 0) carry_s = 0;
+    for (int base = 0; base < nk; base += kScanTiles * 1024) {
+        int x[kScanTiles]; // own value, then exclusive prefix inside the warp
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(0xffffffffu, x, o);
-            if (lane >= o) x += y;
+        for (int k = 0; k < kScanTiles; ++k) {
+            const int i = base + k * 1024 + tid;
+            x[k] = i < nk ? hist[i] : 0;
         }
-        if (lane == 31) warp_sums[wid] = x;
-        __syncthreads();
-        const int carry = carry_s;
-        int w = warp_sums[lane];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(0xffffffffu, w, o);
-            if (lane >= o) w += y;
+        for (int k = 0; k < kScanTiles; ++k) {
+            if (base + k * 1024 >= nk) { // block-uniform: a tile past the end counts as zeros
+                if (lane == 31) ws[k][wid] = 0;
+                continue;
+            }
+            const int i = base + k * 1024 + tid;
+            if (i < nk) hist[i] = 0;
+            const int v = x[k];
+            int sc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(kFull, sc, o);
+                if (lane >= o) sc += y;
+            }
+            if (lane == 31) ws[k][wid] = sc;
+            x[k] = sc - v;
         }
-        const int before = __shfl_sync(0xffffffffu, w, wid) - warp_sums[wid]; // sum of the warps in front of this one
-        if (i < nk) start[i] = carry + before + x - v;
+        __syncthreads(); // also orders the carry_s of the previous pass / the initial zero
+        for (int k = wid; k < kScanTiles; k += 32) { // warp w: offsets of the 32 warps inside tiles w, w + 32
+            const int v = ws[k][lane];
+            int sc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(kFull, sc, o);
+                if (lane >= o) sc += y;
+            }
+            ws[k][lane] = sc - v;
+            if (lane == 31) tile_tot[k] = sc;
+        }
         __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + before + x; // inclusive total of the tile
+        if (wid == 0) { // tile bases
+            const int v0 = lane < kScanTiles ? tile_tot[lane] : 0, v1 = lane + 32 < kScanTiles ? tile_tot[lane + 32] : 0;
+            int s0 = v0, s1 = v1;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y0 = __shfl_up_sync(kFull, s0, o), y1 = __shfl_up_sync(kFull, s1, o);
+                if (lane >= o) { s0 += y0; s1 += y1; }
+            }
+            const int carry = carry_s, tot0 = __shfl_sync(kFull, s0, 31), tot1 = __shfl_sync(kFull, s1, 31);
+            tile_tot[lane] = carry + s0 - v0;
+            tile_tot[lane + 32] = carry + tot0 + s1 - v1;
+            if (lane == 0) carry_s = carry + tot0 + tot1;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kScanTiles; ++k) {
+            const int i = base + k * 1024 + tid;
+            if (i < nk) start[i] = tile_tot[k] + ws[k][wid] + x[k];
+        }
+        __syncthreads(); // ws / tile_tot are rewritten by the next pass
     }
-    __syncthreads();
-    if (threadIdx.x == 0) start[nk] = carry_s;
+    if (tid == 0) start[nk] = carry_s;
 }
 
 __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ start,
