@@ -31,7 +31,7 @@
 namespace {
 
 #ifndef AEV_FWD_MINB
-#define AEV_FWD_MINB 6
+#define AEV_FWD_MINB 8
 #endif
 #ifndef AEV_BWD_MINB
 #define AEV_BWD_MINB 5

@@ -193,7 +193,9 @@ __device__ __forceinline__ float r2_defined(const float4 a, const float4 b, cons
 // x-ranges (x-adjacent cells are adjacent in the sort).  Lane r fetches the bounds of range r (one load round per
 // species instead of a dependent chain per row), a warp scan turns the lengths into one flat candidate list, and
 // the lanes walk that list 32 candidates at a time (coalesced float4 loads, ballot compaction into the two rows),
-// so a trip is full even where single ranges hold 10-40 atoms.
+// so a trip is full even where single ranges hold 10-40 atoms.  The non-empty ranges are compacted to the low lanes
+// (through shared memory); per trip one REDUX.OR builds the bit mask of the range ends that fall into the trip, and a
+// lane's range is (ends before the trip) + popc(mask up to its own bit): no search loop.
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, const int *__restrict__ mol,
               const int *__restrict__ cell_start, GridInfo g, float rl2_r, float rl2_a, int cap_r, int cap_a,
@@ -201,9 +203,10 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
               uint16_t *__restrict__ seg_a, int *__restrict__ flags, const int *cond)
 {
     if (cond && *cond == 0) return;
+    __shared__ int2 cr[kWarpsPerBlock][32]; // compacted non-empty ranges: (inclusive end in the flat list, index offset)
     const unsigned kFull = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    const int i = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int i = blockIdx.x * kWarpsPerBlock + wib;
     if (i >= n) return;
     const float4 pi = pos[i];
     // range `lane` of the stencil: first / last cell (inside one species block) and whether it exists
@@ -233,11 +236,9 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
     int *row_r = nbr_r + (size_t)i * cap_r;
     int *row_a = nbr_a + (size_t)i * cap_a;
     const unsigned lt = (1u << lane) - 1u;
+    int seg_r_l = 0, seg_a_l = 0; // lane s: where the segment of species s starts in the two rows
     for (int s = 0; s < S; ++s) {
-        if (lane == 0) {
-            seg_r[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_r, cap_r);
-            seg_a[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_a, cap_a);
-        }
+        if (lane == s) { seg_r_l = min(cnt_r, cap_r); seg_a_l = min(cnt_a, cap_a); }
         if (!(present >> s & 1u)) continue;
         int beg = 0, len = 0;
         if (lane < nranges) {
@@ -252,17 +253,20 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
         }
         const int total = __shfl_sync(kFull, incl, 31);
         const int off = beg - (incl - len); // flat index v of range r is atom v + off_r
-        int r = 0;                          // range this lane's flat index currently falls into
+        const unsigned nonempty = __ballot_sync(kFull, len > 0);
+        if (len > 0) cr[wib][__popc(nonempty & lt)] = make_int2(incl, off);
+        __syncwarp();
+        const int2 ce = lane < __popc(nonempty) ? cr[wib][lane] : make_int2(0x7fffffff, 0); // lane k: k-th non-empty range
+        __syncwarp();
+        int r0 = 0; // non-empty ranges that end before this trip
         for (int t0 = 0; t0 < total; t0 += 32) {
             const int v = t0 + lane;
             const bool act = v < total;
-            for (;;) { // advance past finished (and empty) ranges; v grows monotonically, so r never goes back
-                const int r_end = __shfl_sync(kFull, incl, r); // every lane takes part (no short-circuit around it)
-                const bool adv = act && v >= r_end;
-                if (!__any_sync(kFull, adv)) break;
-                if (adv) ++r;
-            }
-            const int j = v + __shfl_sync(kFull, off, r);
+            const unsigned d = (unsigned)(ce.x - t0); // the ends are distinct: one bit per range that ends inside the trip
+            const unsigned ends = __reduce_or_sync(kFull, d < 32u ? 1u << d : 0u);
+            const int r = r0 + __popc(ends & ((2u << lane) - 1u)); // ranges with end <= v
+            r0 += __popc(ends);
+            const int j = v + __shfl_sync(kFull, ce.y, r & 31);
             bool hr = false, ha = false;
             if (act && j != i) {
                 const float r2 = r2_defined(pi, pos[j], g);
@@ -271,17 +275,19 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
             }
             const unsigned mr = __ballot_sync(kFull, hr);
             const unsigned ma = __ballot_sync(kFull, ha);
-            if (hr) { const int p = cnt_r + __popc(mr & lt); if (p < cap_r) row_r[p] = j; }
-            if (ha) { const int p = cnt_a + __popc(ma & lt); if (p < cap_a) row_a[p] = j; }
+            const int p_r = cnt_r + __popc(mr & lt), p_a = cnt_a + __popc(ma & lt);
+            if (hr && p_r < cap_r) row_r[p_r] = j;
+            if (ha && p_a < cap_a) row_a[p_a] = j;
             cnt_r += __popc(mr);
             cnt_a += __popc(ma);
         }
     }
+    if (lane >= S) { seg_r_l = min(cnt_r, cap_r); seg_a_l = min(cnt_a, cap_a); } // entries S..7: the row length
+    if (lane < NNP_MAX_SPECIES) {
+        seg_r[(size_t)i * NNP_MAX_SPECIES + lane] = (uint16_t)seg_r_l;
+        seg_a[(size_t)i * NNP_MAX_SPECIES + lane] = (uint16_t)seg_a_l;
+    }
     if (lane == 0) {
-        for (int s = S; s < NNP_MAX_SPECIES; ++s) {
-            seg_r[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_r, cap_r);
-            seg_a[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cnt_a, cap_a);
-        }
         if (cnt_r > cap_r) atomicOr(&flags[0], NNP_FLAG_CAP_R);
         if (cnt_a > cap_a) atomicOr(&flags[0], NNP_FLAG_CAP_A);
     }
