@@ -22,7 +22,8 @@ EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp
            "nnp_build_neighbors", "nnp_get_neighbors", "nnp_energy_forces", "nnp_get_aev",
            "nnp_get_atomic_energies", "nnp_md_init", "nnp_md_step", "nnp_get_state", "nnp_sync",
            "nnp_energy_forces_host", "nnp_md_step_host", "nnp_profile", "nnp_profile_read", "nnp_launch_count",
-           "nnp_aev_len", "nnp_aev_active_columns", "nnp_aev_ladder", "nnp_md_set_langevin", "nnp_energy_forces_virial"]
+           "nnp_aev_len", "nnp_aev_active_columns", "nnp_aev_ladder", "nnp_md_set_langevin", "nnp_energy_forces_virial",
+           "nnp_measure_peaks"]
 
 
 class NnpError(RuntimeError):
@@ -83,6 +84,7 @@ def lib():
         L.nnp_aev_ladder.argtypes = [vp]
         L.nnp_md_set_langevin.argtypes = [vp, C.c_float, C.c_float, C.c_uint64]
         L.nnp_energy_forces_virial.argtypes = [vp, dp, fp, dp]
+        L.nnp_measure_peaks.argtypes = [C.c_int, dp]
         _lib = L
     return _lib
 
@@ -242,3 +244,17 @@ def nnp_md_set_langevin(ctx, gamma, kT, seed):
 
 def nnp_energy_forces_virial(ctx, d_energy, d_forces, d_virial):
     return _check(ctx, lib().nnp_energy_forces_virial(ctx, _ptr(d_energy), _ptr(d_forces), _ptr(d_virial)))
+
+
+NNP_N_PEAKS = 6
+PEAK_NAMES = ["fp32_fma_tflops", "mufu_ex2_gops", "tf32_tcgen05_ss_tflops", "tf32_tcgen05_ts_tflops",
+              "cycles_per_mma_m128n256k8_ss", "cycles_per_mma_m128n256k8_ts"]
+
+
+def nnp_measure_peaks(device=0):
+    """Measured roofline denominators of `device` (include/nnp.h), as a dict."""
+    out = np.zeros(NNP_N_PEAKS, dtype=np.float64)
+    rc = lib().nnp_measure_peaks(int(device), _ptr(out))
+    if rc != NNP_OK:
+        raise RuntimeError("nnp_measure_peaks failed with status %d" % rc)
+    return dict(zip(PEAK_NAMES, (float(v) for v in out)))

@@ -568,3 +568,15 @@ def test_virial_needs_a_single_structure(model1):
             _gpu_virial(ctx, sp, xyz, None, mol_offsets=offs)
     finally:
         nnp.nnp_destroy(ctx)
+
+
+def test_measured_peaks_are_plausible():
+    """nnp_measure_peaks: the micro-benchmarks run and land in the range the hardware allows.
+    B200: 148 SMs x 128 FMA lanes x 2 x 1.965 GHz = 74.4 TFLOP/s fp32, 148 x 16 x 1.965 GHz = 4.65 T MUFU ops/s, dense
+    TF32 tcgen05 nominally half of bf16 (2.25 PFLOP/s)."""
+    pk = nnp.nnp_measure_peaks(0)
+    assert 30.0 < pk["fp32_fma_tflops"] < 80.0, pk
+    assert 1500.0 < pk["mufu_ex2_gops"] < 5000.0, pk
+    for form in ("ss", "ts"):
+        assert 300.0 < pk["tf32_tcgen05_%s_tflops" % form] < 1300.0, pk
+        assert 16.0 <= pk["cycles_per_mma_m128n256k8_%s" % form] < 400.0, pk
