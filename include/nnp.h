@@ -183,9 +183,10 @@ int nnp_aev_ladder(const nnp_ctx *ctx);
  * launches each, synchronously on the default stream, and fills h_out (host, NNP_N_PEAKS doubles):
  *   0 fp32 FMA TFLOP/s (2 flops per FMA), 1 MUFU ex2 G ops/s, 2 dense TF32 tcgen05.mma TFLOP/s with both operands in
  *   shared memory, 3 the same with A in tensor memory (the operand form of the MLP GEMMs), 4 / 5 SM cycles per
- *   M128 N256 K8 MMA instruction for the two forms.  Needs no ctx; allocates and frees a few KB.  Diagnostic only:
+ *   M128 N256 K8 MMA instruction for the two forms, 6..12 SM cycles per M128 N K8 instruction (A in tensor memory) for
+ *   N = 64, 96, 128, 160, 192, 224, 256.  Needs no ctx; allocates and frees a few KB.  Diagnostic only:
  * nothing on the energy/force/MD path calls it.  Returns NNP_OK, NNP_EINVAL (null), NNP_ECUDA, NNP_ENOMEM. */
-#define NNP_N_PEAKS 6
+#define NNP_N_PEAKS 13
 int nnp_measure_peaks(int device, double *h_out);
 
 #ifdef __cplusplus

@@ -71,7 +71,7 @@ __device__ __forceinline__ uint64_t kmajor_sw128_desc(uint32_t smem_addr)
 
 // TS = false: D[tmem] += A[smem] . B[smem]^T;  TS = true: A from tensor memory (columns 256..287)
 template <bool TS>
-__global__ void __launch_bounds__(128, 1) k_peak_tf32(int n_groups, long long *cycles)
+__global__ void __launch_bounds__(128, 1) k_peak_tf32(int n_groups, int mma_n, long long *cycles)
 {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(128, 1) k_peak_tf32(int n_groups, long long *c
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }
     if (threadIdx.x == 0) {
-        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(PK_N >> 3) << 17) | ((uint32_t)(PK_M >> 4) << 24);
+        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(mma_n >> 3) << 17) | ((uint32_t)(PK_M >> 4) << 24);
         const uint64_t da = kmajor_sw128_desc(a_smem), db = kmajor_sw128_desc(b_smem);
         const long long t0 = clock64();
         for (int g = 0; g < n_groups; ++g) {
@@ -185,14 +185,22 @@ extern "C" int nnp_measure_peaks(int device, double *h_out /* [NNP_N_PEAKS] */)
     cudaFuncSetAttribute(k_peak_tf32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PK_SMEM);
     cudaFuncSetAttribute(k_peak_tf32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PK_SMEM);
     long long cyc[2] = {0, 0};
-    const float ms_ss = best_ms([&] { k_peak_tf32<false><<<sms, 128, PK_SMEM>>>(n_groups, d_cyc); }, 4);
+    const float ms_ss = best_ms([&] { k_peak_tf32<false><<<sms, 128, PK_SMEM>>>(n_groups, PK_N, d_cyc); }, 4);
     cudaMemcpy(&cyc[0], d_cyc, sizeof(long long), cudaMemcpyDeviceToHost);
-    const float ms_ts = best_ms([&] { k_peak_tf32<true><<<sms, 128, PK_SMEM>>>(n_groups, d_cyc); }, 4);
+    const float ms_ts = best_ms([&] { k_peak_tf32<true><<<sms, 128, PK_SMEM>>>(n_groups, PK_N, d_cyc); }, 4);
     cudaMemcpy(&cyc[1], d_cyc, sizeof(long long), cudaMemcpyDeviceToHost);
     h_out[2] = mma_flops / (ms_ss * 1e-3) * 1e-12;
     h_out[3] = mma_flops / (ms_ts * 1e-3) * 1e-12;
     h_out[4] = cyc[0] > 0 ? (double)cyc[0] / (4.0 * n_groups) : -1.0; // SM cycles per MMA instruction (M128 N256 K8)
     h_out[5] = cyc[1] > 0 ? (double)cyc[1] / (4.0 * n_groups) : -1.0;
+    // cycles per MMA instruction (A in tensor memory) against the N extent: NNP_PEAK_N_LIST columns 64, 96, ..., 256
+    for (int q = 0; q < 7; ++q) {
+        const int mma_n = 64 + 32 * q;
+        k_peak_tf32<true><<<sms, 128, PK_SMEM>>>(n_groups / 4, mma_n, d_cyc);
+        long long c = 0;
+        cudaMemcpy(&c, d_cyc, sizeof(long long), cudaMemcpyDeviceToHost);
+        h_out[6 + q] = c > 0 ? (double)c / (double)n_groups : -1.0;
+    }
     cudaFree(d_out);
     cudaFree(d_cyc);
     return cudaGetLastError() == cudaSuccess ? NNP_OK : NNP_ECUDA;

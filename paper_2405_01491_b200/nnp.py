@@ -246,9 +246,10 @@ def nnp_energy_forces_virial(ctx, d_energy, d_forces, d_virial):
     return _check(ctx, lib().nnp_energy_forces_virial(ctx, _ptr(d_energy), _ptr(d_forces), _ptr(d_virial)))
 
 
-NNP_N_PEAKS = 6
+NNP_N_PEAKS = 13
 PEAK_NAMES = ["fp32_fma_tflops", "mufu_ex2_gops", "tf32_tcgen05_ss_tflops", "tf32_tcgen05_ts_tflops",
-              "cycles_per_mma_m128n256k8_ss", "cycles_per_mma_m128n256k8_ts"]
+              "cycles_per_mma_m128n256k8_ss", "cycles_per_mma_m128n256k8_ts"] + \
+             ["cycles_per_mma_m128n%dk8_ts_sweep" % n for n in range(64, 257, 32)]
 
 
 def nnp_measure_peaks(device=0):
