@@ -90,7 +90,9 @@ const char *nnp_last_error(const nnp_ctx *ctx); /* ctx may be NULL (create failu
 /* Loads a system: species index per atom (0..n_species-1) and coordinates [n][3] (fp32, Angstrom, need
  * not be wrapped).  h_box: orthorhombic edge lengths; all zero => non-periodic.  Batches (PAPER.md L41,
  * L176): d_mol_offsets[n_mols+1] gives each structure's atom range in the concatenated arrays, atoms of
- * different structures never interact; NULL => one structure.  Periodic batches are not supported.
+ * different structures never interact; NULL => one structure.  With a box, a batch is a set of replicas of ONE
+ * periodic cell (same edge lengths for all, e.g. the beads of a ring polymer): every structure gets
+ * its own set of cell-list bins; energies come back per structure.  (MD and the virial take one structure.)
  * Invalidates neighbour lists and MD state.  Synchronises (species counts are read back). */
 int nnp_set_system(nnp_ctx *ctx, int n_atoms, const int32_t *d_species, const float *d_xyz,
                    const float h_box[3], int n_mols, const int32_t *d_mol_offsets);

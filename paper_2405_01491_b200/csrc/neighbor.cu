@@ -23,7 +23,7 @@ __device__ __forceinline__ int cell_of(const float4 p, const GridInfo &g, int mo
     int cx = cell_coord(p.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
     int cy = cell_coord(p.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
     int cz = cell_coord(p.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
-    return (cz * g.nc[1] + cy) * g.nc[0] + cx;
+    return mol * g.ncell_box + (cz * g.nc[1] + cy) * g.nc[0] + cx; // replicas of a periodic batch never share a bin
 }
 
 __global__ void k_keys_hist(int n, const float4 *__restrict__ pos, const int *__restrict__ spc,
@@ -226,7 +226,7 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
         else if (cx == 0) { xa = ix ? g.nc[0] - 1 : 0; xb = ix ? g.nc[0] - 1 : 1; }
         else if (cx == g.nc[0] - 1) { xa = ix ? 0 : cx - 1; xb = ix ? 0 : cx; }
         else { xa = cx - 1; xb = cx + 1; }
-        const int rowbase = (z * g.nc[1] + y) * g.nc[0];
+        const int rowbase = mol[i] * g.ncell_box + (z * g.nc[1] + y) * g.nc[0];
         c_first = rowbase + xa;
         c_last = rowbase + xb;
     } else {

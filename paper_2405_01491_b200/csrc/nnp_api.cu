@@ -399,7 +399,11 @@ int setup_grid(nnp_ctx *c, float skin)
             g.cell_scale[d] = (float)nc / c->box[d];
             ncell *= nc;
         }
-        g.ncell = (int)ncell;
+        // a periodic batch (replicas of one cell, e.g. the beads of a ring polymer): one bin set per replica
+        if (ncell * c->n_mols * c->S > (1L << 27))
+            NNP_FAIL(c, NNP_EINVAL, "%ld cells x %d structures x %d species: too many bins", ncell, c->n_mols, c->S);
+        g.ncell_box = (int)ncell;
+        g.ncell = (int)ncell * c->n_mols;
     } else {
         g.nc[0] = c->n_mols; g.nc[1] = 1; g.nc[2] = 1;
         g.ncell = c->n_mols;
@@ -718,7 +722,6 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
     if (n_mols < 1 || n_mols > c->max_mols) NNP_FAIL(c, NNP_EINVAL, "n_mols %d outside [1, max_mols=%d]", n_mols, c->max_mols);
     const int nper = (h_box[0] > 0.f) + (h_box[1] > 0.f) + (h_box[2] > 0.f);
     if (nper != 0 && nper != 3) NNP_FAIL(c, NNP_EINVAL, "box must be all zero (non-periodic) or all positive");
-    if (nper == 3 && n_mols > 1) NNP_FAIL(c, NNP_EINVAL, "periodic batches are not supported");
     CU(c, cudaSetDevice(c->device));
     c->n = n_atoms; c->n_mols = n_mols; c->periodic = nper == 3;
     for (int d = 0; d < 3; ++d) c->box[d] = h_box[d];

@@ -23,7 +23,8 @@ enum { NNP_FLAG_CAP_R = 1, NNP_FLAG_CAP_A = 2 };
 // ---- periodic cell grid / molecule bins (stage 1) ------------------------------------------------
 struct GridInfo {
     int nc[3];        // cells per dimension (periodic) or {n_mols,1,1} (batched molecules)
-    int ncell;        // nc[0]*nc[1]*nc[2]
+    int ncell;        // bins in all: nc[0]*nc[1]*nc[2] x (structures sharing the box), or n_mols
+    int ncell_box;    // periodic: nc[0]*nc[1]*nc[2], the bins of ONE structure (replica r owns bins [r, r+1) * ncell_box)
     int periodic;     // 1: orthorhombic minimum image; 0: bins are molecules
     float box[3];
     float inv_box[3]; // 1.0f / box (IEEE division on the host)

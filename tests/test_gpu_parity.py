@@ -129,6 +129,35 @@ def test_molecule_batch(model1):
         nnp.nnp_destroy(ctx)
 
 
+# ---------------------------------------------------------------- replicas of one periodic cell in one batch
+@pytest.mark.parametrize("n_waters, L, n_rep", [(64, 12.42, 5), (1000, None, 3)], ids=["tiny_box_x5", "water1000_x3"])
+def test_periodic_replica_batch(model1, n_waters, L, n_rep):
+    """RPMD-style replica batching: n_rep perturbed copies of one periodic water box in one call; lists
+    exactly those of the oracle (never across replicas), per-replica energies and all forces against the oracle."""
+    consts, widths, params, om = model1
+    sp1, x1, box = inputs.water_box(n_waters, L, seed=inputs.SEED0 + 9)
+    rng = np.random.default_rng(5)
+    reps = [(x1 + 0.04 * rng.standard_normal(x1.shape) * (r > 0)).astype(np.float32).astype(np.float64) for r in range(n_rep)]
+    sp = np.tile(sp1, n_rep)
+    xyz = np.concatenate(reps)
+    offs = (np.arange(n_rep + 1) * len(sp1)).astype(np.int32)
+    mol = np.repeat(np.arange(n_rep), len(sp1)).astype(np.int32)
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp), max_mols=n_rep)
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box, mol_offsets=offs)
+        _check_lists(ctx, xyz, box, len(sp), 0.0, mol_id=mol)
+        ref = orc.energy_forces(om, sp, xyz, box, offs, want_e_atom=True)
+        U.assert_parity(Eg, Fg, ref, mol_offsets=offs)
+        assert (np.abs(Eg - ref["E"]) <= U.E_RTOL * np.abs(ref["E"])).all()
+        # with a skin, and the same replicas one at a time through the single-structure path
+        Es, Fs = U.gpu_energy_forces(ctx, sp, xyz, box, mol_offsets=offs, skin=0.4)
+        U.assert_parity(Es, Fs, ref, mol_offsets=offs)
+        E1, F1 = U.gpu_energy_forces(ctx, sp1, reps[1], box)
+        assert abs(E1[0] - Eg[1]) <= 2e-6 * abs(Eg[1]) and np.abs(F1 - Fg[offs[1]:offs[2]]).max() < 2e-4
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
 # ---------------------------------------------------------------- degenerate inputs
 def test_edge_cases(model1):
     consts, widths, params, om = model1

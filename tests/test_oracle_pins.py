@@ -417,6 +417,22 @@ def test_batch_equals_each_molecule_alone(small_model):
         assert abs(a["E"][0] - b["E"][m]) < 1e-11 and np.allclose(a["F"], b["F"][sl], atol=1e-12)
 
 
+def test_periodic_replica_batch_equals_each_replica_alone(small_model, water64):
+    """Replicas of one periodic cell (the beads of a ring polymer; L41: same batch index => edge): the
+    batched energies and forces are those of each replica run alone in the same box."""
+    sp1, x1, box = water64
+    rng = np.random.default_rng(77)
+    reps = [x1 + 0.05 * rng.standard_normal(x1.shape) * (r > 0) for r in range(3)]
+    sp = np.tile(sp1, 3)
+    xyz = np.concatenate(reps)
+    offs = np.arange(4, dtype=np.int32) * len(sp1)
+    b = orc.energy_forces(small_model, sp, xyz, box, offs)
+    for r in range(3):
+        a = orc.energy_forces(small_model, sp1, reps[r], box)
+        assert abs(a["E"][0] - b["E"][r]) < 1e-10 and np.allclose(a["F"], b["F"][offs[r]:offs[r + 1]], atol=1e-11)
+    assert abs(b["E"][1] - b["E"][0]) > 1e-6   # the replicas do differ
+
+
 def test_self_energy_shifts_energy_only(consts, small_widths, water64):
     sp, xyz, box = water64
     p = inputs.make_weights(5, 1, widths=small_widths)
