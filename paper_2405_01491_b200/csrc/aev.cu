@@ -60,8 +60,7 @@ struct WarpSmemBwd {
     int j[kCapA];
     int seg[NNP_MAX_SPECIES + 1];
     int own[32];
-    float alp[kMat * kMatLd]; // alp[a][b]: alpha of a in pair (a,b); fallback path: f[kCapA][3] aliases it
-    float bet[kMat * kMatLd]; // bet[a][b] = bet[b][a]
+    float2 ab[kMat * kMatLd]; // ab[a][b] = (alpha of a in pair (a,b), beta(a,b) = beta(b,a)); fallback path: f[kCapA][3] aliases it
 };
 
 __device__ __forceinline__ float ex2(float x)
@@ -628,7 +627,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
         if (lane == q && q < P.np) my_s = P.plist[q];
     // P.k_ang0 = zeta 0.95 (hcz2 / hsz2 carry the 1/2 of the base); d/drb exp(-eta (rb - s)^2) = -2 eta (rb - s) ra =
     // (-2 eta / ka) w ra with w = ka (rb - s): P.half_drb_scale, P.dr_scale (AevParams, nnp_aev_derive)
-    float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.alp);
+    float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.ab);
 
     // Centres are handed out dynamically (one ticket per centre): the cost of a centre varies with its pair count,
     // and with a static split the slowest warp of a persistent grid ends ~20 % after the average one.
@@ -726,7 +725,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
         const int na = stage_angular<true>(sm, P, c, i, lane, pos, nbr_a, flags);
         const bool arena = na <= kMat; // warp-uniform
         if (arena) {
-            if (lane < na) { sm.alp[lane * kMatLd + lane] = 0.f; sm.bet[lane * kMatLd + lane] = 0.f; }
+            if (lane < na) sm.ab[lane * kMatLd + lane] = make_float2(0.f, 0.f);
         } else {
             for (int a = lane; a < na; a += 32) { fsm[a][0] = 0.f; fsm[a][1] = 0.f; fsm[a][2] = 0.f; }
         }
@@ -821,8 +820,8 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float alk = (dE_drk - dE_dcs * cs_ * fk.y) * fk.y;
                 if (arena) {
                     const int sab = ia * kMatLd + ib, sba = ib * kMatLd + ia;
-                    sm.alp[sab] = alj; sm.alp[sba] = alk;
-                    sm.bet[sab] = beta; sm.bet[sba] = beta;
+                    sm.ab[sab] = make_float2(alj, beta);
+                    sm.ab[sba] = make_float2(alk, beta);
                 } else {
                     atomicAdd(&fsm[ia][0], alj * dj.x + beta * dk.x);
                     atomicAdd(&fsm[ia][1], alj * dj.y + beta * dk.y);
@@ -841,12 +840,12 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float4 da = sm.d[a];
                 float asum = 0.f;
                 fx = 0.f; fy = 0.f; fz = 0.f;
-                const float *ra = sm.alp + a * kMatLd, *rb = sm.bet + a * kMatLd;
+                const float2 *rab = sm.ab + a * kMatLd;
                 for (int b = 0; b < na; ++b) {
-                    const float be = rb[b];
+                    const float2 w = rab[b];
                     const float4 db = sm.d[b];
-                    asum += ra[b];
-                    fx = fmaf(be, db.x, fx); fy = fmaf(be, db.y, fy); fz = fmaf(be, db.z, fz);
+                    asum += w.x;
+                    fx = fmaf(w.y, db.x, fx); fy = fmaf(w.y, db.y, fy); fz = fmaf(w.y, db.z, fz);
                 }
                 fx = fmaf(asum, da.x, fx); fy = fmaf(asum, da.y, fy); fz = fmaf(asum, da.z, fz);
             } else {
