@@ -17,6 +17,16 @@ __device__ __forceinline__ int cell_coord(float x, float L, float invL, float sc
     return min(max(c, 0), nc - 1);
 }
 
+// cell index and fractional position inside the cell (clamped to [0, 1])
+__device__ __forceinline__ int cell_coord_frac(float x, float L, float invL, float scale, int nc, float &f)
+{
+    const float w = x - L * floorf(x * invL);
+    const float cw = w * scale;
+    const int c = min(max((int)cw, 0), nc - 1);
+    f = fminf(fmaxf(cw - (float)c, 0.f), 1.f);
+    return c;
+}
+
 __device__ __forceinline__ int cell_of(const float4 p, const GridInfo &g, int mol)
 {
     if (!g.periodic) return mol;
@@ -198,7 +208,7 @@ __device__ __forceinline__ float r2_defined(const float4 a, const float4 b, cons
 // lane's range is (ends before the trip) + popc(mask up to its own bit): no search loop.
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, const int *__restrict__ mol,
-              const int *__restrict__ cell_start, GridInfo g, float rl2_r, float rl2_a, int cap_r, int cap_a,
+              const int *__restrict__ cell_start, GridInfo g, float rl2_r, float rl2_a, float rlm2, int cap_r, int cap_a,
               int *__restrict__ nbr_r, int *__restrict__ nbr_a, uint16_t *__restrict__ seg_r,
               uint16_t *__restrict__ seg_a, int *__restrict__ flags, const int *cond)
 {
@@ -211,21 +221,33 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
     const float4 pi = pos[i];
     // range `lane` of the stencil: first / last cell (inside one species block) and whether it exists
     int c_first = 0, c_last = 0, nranges = 1;
+    bool rng_ok = true; // false: no atom of this range can be inside the list radius
     if (g.periodic) {
-        const int cx = cell_coord(pi.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
-        const int cy = cell_coord(pi.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
-        const int cz = cell_coord(pi.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
+        float fx, fy, fz;
+        const int cx = cell_coord_frac(pi.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0], fx);
+        const int cy = cell_coord_frac(pi.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1], fy);
+        const int cz = cell_coord_frac(pi.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2], fz);
         const int nys = g.nc[1] >= 3 ? 3 : g.nc[1], nzs = g.nc[2] >= 3 ? 3 : g.nc[2]; // distinct cells among c-1, c, c+1
         const int nxs = (g.nc[0] > 3 && (cx == 0 || cx == g.nc[0] - 1)) ? 2 : 1;     // the x range wraps
         nranges = nzs * nys * nxs;
         const int ix = lane % nxs, t = lane / nxs, iy = t % nys, iz = t / nys;
         const int y = nys == 3 ? (cy + iy + g.nc[1] - 1) % g.nc[1] : iy;
         const int z = nzs == 3 ? (cz + iz + g.nc[2] - 1) % g.nc[2] : iz;
+        // Trim the stencil with the atom's position inside its cell: a (y,z) row whose nearest point is farther than the
+        // list radius (+ 0.01 A for the rounding of the binning) holds no neighbour, and of the three x cells of a row
+        // only those within sqrt(rl^2 - d_yz^2) of the atom are needed: ~27 % fewer candidates at cell edge ~ rl.
+        // (Only where c-1, c, c+1 are three distinct cells, so that the nearest image lies on the side looked at.)
+        float d2 = 0.f;
+        if (nys == 3 && iy != 1) { const float dd = (iy == 0 ? fy : 1.0f - fy) * g.box[1] / (float)g.nc[1]; d2 += dd * dd; }
+        if (nzs == 3 && iz != 1) { const float dd = (iz == 0 ? fz : 1.0f - fz) * g.box[2] / (float)g.nc[2]; d2 += dd * dd; }
+        rng_ok = d2 <= rlm2;
+        const float reach2 = rlm2 - d2, lenx = g.box[0] / (float)g.nc[0];
+        const bool need_m = (fx * lenx) * (fx * lenx) <= reach2, need_p = ((1.0f - fx) * lenx) * ((1.0f - fx) * lenx) <= reach2;
         int xa, xb;
         if (g.nc[0] <= 3) { xa = 0; xb = g.nc[0] - 1; }
-        else if (cx == 0) { xa = ix ? g.nc[0] - 1 : 0; xb = ix ? g.nc[0] - 1 : 1; }
-        else if (cx == g.nc[0] - 1) { xa = ix ? 0 : cx - 1; xb = ix ? 0 : cx; }
-        else { xa = cx - 1; xb = cx + 1; }
+        else if (cx == 0) { xa = ix ? g.nc[0] - 1 : 0; xb = ix ? g.nc[0] - 1 : (need_p ? 1 : 0); if (ix && !need_m) rng_ok = false; }
+        else if (cx == g.nc[0] - 1) { xa = ix ? 0 : (need_m ? cx - 1 : cx); xb = ix ? 0 : cx; if (ix && !need_p) rng_ok = false; }
+        else { xa = need_m ? cx - 1 : cx; xb = need_p ? cx + 1 : cx; }
         const int rowbase = mol[i] * g.ncell_box + (z * g.nc[1] + y) * g.nc[0];
         c_first = rowbase + xa;
         c_last = rowbase + xb;
@@ -241,7 +263,7 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
         if (lane == s) { seg_r_l = min(cnt_r, cap_r); seg_a_l = min(cnt_a, cap_a); }
         if (!(present >> s & 1u)) continue;
         int beg = 0, len = 0;
-        if (lane < nranges) {
+        if (lane < nranges && rng_ok) {
             beg = cell_start[s * g.ncell + c_first];
             len = cell_start[s * g.ncell + c_last + 1] - beg;
         }
@@ -319,7 +341,8 @@ int nnp_launch_build(nnp_ctx *c, const int *cond)
                                  c->xref, c->spc, c->orig, c->mol, cond);
     const float rl_r = c->aev.rcr + c->skin, rl_a = c->aev.rca + c->skin;
     k_build_lists<<<nnp_div_up(n, kWarpsPerBlock), kWarpsPerBlock * 32, 0, st>>>(
-        n, S, c->present_mask, c->pos, c->mol, c->cell_start, c->grid, rl_r * rl_r, rl_a * rl_a, c->aev.cap_r, c->aev.cap_a,
+        n, S, c->present_mask, c->pos, c->mol, c->cell_start, c->grid, rl_r * rl_r, rl_a * rl_a, (rl_r + 0.01f) * (rl_r + 0.01f),
+        c->aev.cap_r, c->aev.cap_a,
         c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->flags, cond);
     k_finish_build<<<1, 1, 0, st>>>(c->flags, cond);
     if (!cond) c->launches += 8; // conditional builds are counted from the device-side rebuild counter (flags[2])
