@@ -282,7 +282,7 @@ def run_ours(args):
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": world * n * Ke / (e2e_ms_max * 1e-3), "unit": UNIT, "steps": Ke,
-                "h2d_bytes_per_step": 2 * n * 12, "d2h_bytes_per_step": 2 * n * 12 + 16,
+                "h2d_bytes_per_step": 2 * n * 12, "d2h_bytes_per_step": 2 * n * 12 + 40,  # x, v and one packed (epot, ekin, 3 flag words) record
                 "api": "nnp_md_step_host (pinned host x,v up; x,v,epot,ekin down; every step)"},
         "gpu_launches": launches + 8 * (nr_end - nr_start),
         "roofline": roof,

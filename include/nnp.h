@@ -155,7 +155,8 @@ int nnp_sync(nnp_ctx *ctx);
 /* Host-buffer entry points (the end-to-end path: H2D copies, the same kernels, D2H copies; synchronise).
  * nnp_energy_forces_host = nnp_set_system + nnp_build_neighbors(skin) + nnp_energy_forces.
  * nnp_md_step_host: uploads h_xyz/h_vel [n][3] into the running MD state (atoms as in nnp_set_system; lists
- * are kept and rebuilt by the displacement rule), runs n_steps, downloads positions, velocities, epot, ekin. */
+ * are kept and rebuilt by the displacement rule), runs n_steps, downloads positions, velocities, epot, ekin (the two
+ * scalars and the device-side error flags travel in one 40-byte pinned copy).  Synchronises before returning. */
 int nnp_energy_forces_host(nnp_ctx *ctx, int n_atoms, const int32_t *h_species, const float *h_xyz,
                            const float h_box[3], int n_mols, const int32_t *h_mol_offsets, float skin,
                            double *h_energy, float *h_forces);

@@ -152,7 +152,55 @@ __global__ void k_permute_in3(int n, const float *__restrict__ src, const int *_
     dst[i] = make_float4(src[3 * o], src[3 * o + 1], src[3 * o + 2], 0.f);
 }
 
+__global__ void k_unpermute3x2(int n, const float4 *__restrict__ srcA, const float4 *__restrict__ srcB,
+                               const int *__restrict__ orig, float *__restrict__ dstA, float *__restrict__ dstB)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 a = srcA[i], b = srcB[i];
+    const int o = orig[i];
+    dstA[3 * o] = a.x; dstA[3 * o + 1] = a.y; dstA[3 * o + 2] = a.z;
+    dstB[3 * o] = b.x; dstB[3 * o + 1] = b.y; dstB[3 * o + 2] = b.z;
+}
+
+__global__ void k_permute_in3x2(int n, const float *__restrict__ srcA, const float *__restrict__ srcB,
+                                const int *__restrict__ orig, float4 *__restrict__ dstA, float4 *__restrict__ dstB)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int o = orig[i];
+    dstA[i] = make_float4(srcA[3 * o], srcA[3 * o + 1], srcA[3 * o + 2], 0.f);
+    dstB[i] = make_float4(srcB[3 * o], srcB[3 * o + 1], srcB[3 * o + 2], 0.f);
+}
+
+__global__ void k_pack_result(const double *__restrict__ e_mol, const double *__restrict__ ekin,
+                              const int *__restrict__ flags, double *__restrict__ res)
+{
+    if (threadIdx.x == 0) {
+        res[0] = e_mol[0]; res[1] = ekin[0];
+        res[2] = (double)flags[0]; res[3] = (double)flags[1]; res[4] = (double)flags[2];
+    }
+}
+
 } // namespace
+
+void nnp_launch_unpermute3x2(nnp_ctx *c, const float4 *srcA, float *dstA, const float4 *srcB, float *dstB)
+{
+    k_unpermute3x2<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, srcA, srcB, c->orig, dstA, dstB);
+    c->launches += 1;
+}
+
+void nnp_launch_permute_in3x2(nnp_ctx *c, const float *srcA, float4 *dstA, const float *srcB, float4 *dstB)
+{
+    k_permute_in3x2<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, srcA, srcB, c->orig, dstA, dstB);
+    c->launches += 1;
+}
+
+void nnp_launch_pack_result(nnp_ctx *c)
+{
+    k_pack_result<<<1, 32, 0, c->stream>>>(c->e_mol, c->ekin, c->flags, c->d_res);
+    c->launches += 1;
+}
 
 void nnp_launch_kick_drift(nnp_ctx *c)
 {

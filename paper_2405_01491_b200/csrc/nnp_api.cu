@@ -513,8 +513,9 @@ void nnp_destroy(nnp_ctx *c)
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags, c->aev_sched,
-                    c->io_xyz, c->io_vel, c->io_species};
+                    c->io_xyz, c->io_vel, c->io_species, c->d_res};
     for (void *p : ptrs) if (p) cudaFree(p);
+    if (c->h_res) cudaFreeHost(c->h_res);
     for (auto &m : c->prof_marks) cudaEventDestroy(m.first);
     for (auto &e : c->prof_pool) cudaEventDestroy(e);
     delete[] c->layers;
@@ -699,6 +700,8 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     TRY(dev_alloc(c, &c->ekin, 1));
     TRY(dev_alloc(c, &c->flags, 16));
     TRY(dev_alloc(c, &c->io_xyz, 3 * N)); TRY(dev_alloc(c, &c->io_vel, 3 * N)); TRY(dev_alloc(c, &c->io_species, N));
+    TRY(dev_alloc(c, &c->d_res, 8));
+    if (cudaHostAlloc((void **)&c->h_res, 8 * sizeof(double), cudaHostAllocDefault) != cudaSuccess) { c->h_res = nullptr; cudaGetLastError(); }
     TRYCU(cudaMemset(c->flags, 0, sizeof(int) * 16));
     TRY(dev_alloc(c, &c->aev_sched, 2 * NNP_AEV_SCHED_LEN));
     TRYCU(cudaMemset(c->aev_sched, 0, sizeof(int) * 2 * NNP_AEV_SCHED_LEN));
@@ -1010,17 +1013,28 @@ int nnp_md_step_host(nnp_ctx *c, float *h_xyz, float *h_vel, int n_steps, double
     const size_t bytes = sizeof(float) * 3 * (size_t)c->n;
     CU(c, cudaMemcpyAsync(c->io_xyz, h_xyz, bytes, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->io_vel, h_vel, bytes, cudaMemcpyHostToDevice, c->stream));
-    nnp_launch_permute_in3(c, c->io_xyz, c->pos);
-    nnp_launch_permute_in3(c, c->io_vel, c->vel);
+    nnp_launch_permute_in3x2(c, c->io_xyz, c->pos, c->io_vel, c->vel);
     int rc = nnp_md_step(c, n_steps);
     if (rc) return rc;
-    nnp_launch_unpermute3(c, c->pos, c->io_xyz);
-    nnp_launch_unpermute3(c, c->vel, c->io_vel);
+    nnp_launch_unpermute3x2(c, c->pos, c->io_xyz, c->vel, c->io_vel);
     CU(c, cudaMemcpyAsync(h_xyz, c->io_xyz, bytes, cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaMemcpyAsync(h_vel, c->io_vel, bytes, cudaMemcpyDeviceToHost, c->stream));
-    if (h_epot) CU(c, cudaMemcpyAsync(h_epot, c->e_mol, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    if (h_ekin) CU(c, cudaMemcpyAsync(h_ekin, c->ekin, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    return check_flags(c);
+    if (!c->h_res) { // no pinned staging: one copy per scalar
+        if (h_epot) CU(c, cudaMemcpyAsync(h_epot, c->e_mol, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        if (h_ekin) CU(c, cudaMemcpyAsync(h_ekin, c->ekin, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        return check_flags(c);
+    }
+    // energies and the device-side error flags come back in ONE pinned copy (three pageable 8-12 byte copies before)
+    nnp_launch_pack_result(c);
+    CU(c, cudaMemcpyAsync(c->h_res, c->d_res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (h_epot) *h_epot = c->h_res[0];
+    if (h_ekin) *h_ekin = c->h_res[1];
+    const int f0 = (int)c->h_res[2];
+    if (f0 & (NNP_FLAG_CAP_R | NNP_FLAG_CAP_A))
+        NNP_FAIL(c, NNP_ECAPACITY, "neighbour capacity exceeded (%s): recreate with larger cap_r/cap_a",
+                 (f0 & NNP_FLAG_CAP_R) ? "radial" : "angular");
+    return NNP_OK;
 }
 
 } // extern "C"

@@ -197,6 +197,7 @@ struct nnp_ctx {
     int *aev_sched;          // [2][NNP_AEV_SCHED_LEN] centre queues of the two AEV kernels (aev.cu), zero between launches
     // staging for the host entry points
     float *io_xyz, *io_vel;  // [n][3]
+    double *d_res, *h_res;   // nnp_md_step_host: (epot, ekin, flags[0..2]) packed on the device, read back in one pinned copy
     int *io_species;
     // one MD step as a CUDA graph: kick+drift -> IF(rebuild requested){stage 1} -> stages 2-4 -> kick (nnp_api.cu)
     cudaGraph_t md_graph;
@@ -221,6 +222,9 @@ void nnp_launch_kick_drift(nnp_ctx *c);
 void nnp_launch_kick_ke(nnp_ctx *c, int count_step); // count_step: also advance the Langevin step counter flags[4]
 void nnp_launch_energy_reduce(nnp_ctx *c);
 void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst);
+void nnp_launch_unpermute3x2(nnp_ctx *c, const float4 *srcA, float *dstA, const float4 *srcB, float *dstB); // both arrays, one launch
+void nnp_launch_permute_in3x2(nnp_ctx *c, const float *srcA, float4 *dstA, const float *srcB, float4 *dstB);
+void nnp_launch_pack_result(nnp_ctx *c); // d_res = (e_mol[0], ekin, flags[0], flags[1], flags[2])
 void nnp_launch_permute_in3(nnp_ctx *c, const float *src, float4 *dst); // dst[i] = src[orig[i]]
 
 void nnp_prof_mark(nnp_ctx *c, int stage); // nnp_api.cu
