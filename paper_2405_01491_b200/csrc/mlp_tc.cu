@@ -52,11 +52,11 @@ struct TcGroup {
 };
 
 struct TcBatch {
-    TcGroup g[NNP_MAX_SPECIES - 1];
+    TcGroup g[NNP_MAX_GROUPS];
     int n_groups;
-    int tile_off[NNP_MAX_SPECIES]; // prefix sum of (m tiles x n tiles) per group
+    int tile_off[NNP_MAX_GROUPS + 1]; // prefix sum of (m tiles x n tiles) per group
     int n_tiles;
-    int tile_cost[NNP_MAX_SPECIES - 1]; // bytes moved per tile of the group, in units of 128 B
+    int tile_cost[NNP_MAX_GROUPS]; // bytes moved per tile of the group, in units of 128 B
     long long cost_total;
     int stages, stage_bytes, b_tile_bytes; // ring depth; 16 KiB + 2 * b_tile_bytes; nt_max * 128
     int acc_stride, a_slots;

@@ -287,21 +287,24 @@ int check_flags(nnp_ctx *c)
     return NNP_OK;
 }
 
-// One GemmBatch per (net, op); op 0..2 forward layers, 3..5 reverse layers.
-void make_batch(nnp_ctx *c, int net, int op, GemmBatch &b)
+// One GemmBatch per op and range of networks [net0, net0 + n_batch): one group per (network, species present); op 0..2
+// forward layers, 3..5 reverse layers.  Every network of an ensemble has its own activation buffers, so the layers of
+// several networks run as ONE grouped launch (a 12k-atom ensemble call is otherwise 48 launches of ~100 tiles).
+void make_batch(nnp_ctx *c, int net0, int n_batch, int op, GemmBatch &b)
 {
     memset(&b, 0, sizeof(b));
     b.alpha = c->alpha;
     const int kpad = c->aev.kpad;
     int ng = 0;
+    for (int net = net0; net < net0 + n_batch; ++net)
     for (int s = 0; s < c->S; ++s) {
         const int off = c->bucket_off[s], M = c->bucket_off[s + 1] - off;
         if (M == 0) continue;
         GemmGroup &g = b.g[ng++];
         const int h1 = c->widths[s][1], h2 = c->widths[s][2], h3 = c->widths[s][3];
-        float *H0 = c->H[0] + (size_t)off * c->hmax[0];
-        float *H1 = c->H[1] + (size_t)off * c->hmax[1];
-        float *H2 = c->H[2] + (size_t)off * c->hmax[2];
+        float *H0 = c->H[0] + ((size_t)net * c->max_atoms + off) * c->hmax[0];
+        float *H1 = c->H[1] + ((size_t)net * c->max_atoms + off) * c->hmax[1];
+        float *H2 = c->H[2] + ((size_t)net * c->max_atoms + off) * c->hmax[2];
         g.M = M;
         switch (op) {
         case 0:
@@ -361,15 +364,24 @@ int run_forces(nnp_ctx *c)
     nnp_prof_mark(c, 2);
     static const int epi_of[6] = {EPI_CELU, EPI_CELU, EPI_CELU_OUT, EPI_DCELU, EPI_DCELU, EPI_STORE};
     GemmBatch b;
-    for (int net = 0; net < c->n_nets; ++net)
-        for (int op = 0; op < 6; ++op) {
-            make_batch(c, net, op, b);
-            int epi = epi_of[op];
-            if (op == 5 && net > 0) epi = EPI_ACCUM;
-            int rc = run_gemm(c, b, epi);
+    // networks per grouped launch (tensor-core modes): as many as the group table holds
+    const int np = c->aev.np > 0 ? c->aev.np : 1;
+    int nb = (c->mm_mode == NNP_MM_FP32_SIMT || c->n_nets == 1) ? 1 : NNP_MAX_GROUPS / np;
+    if (nb < 1) nb = 1;
+    if (nb > c->n_nets) nb = c->n_nets;
+    for (int net0 = 0; net0 < c->n_nets; net0 += nb)
+        for (int op = 0; op < 5; ++op) {
+            make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, op, b);
+            int rc = run_gemm(c, b, epi_of[op]);
             if (rc != NNP_OK) return rc;
             nnp_prof_mark(c, 3 + op);
         }
+    for (int net = 0; net < c->n_nets; ++net) { // dE/dG accumulates over the networks: one network per launch, in order
+        make_batch(c, net, 1, 5, b);
+        int rc = run_gemm(c, b, net > 0 ? EPI_ACCUM : EPI_STORE);
+        if (rc != NNP_OK) return rc;
+        nnp_prof_mark(c, 8);
+    }
     nnp_launch_energy_reduce(c);
     nnp_prof_mark(c, 9);
     nnp_launch_aev_backward(c, 1.0f / (float)c->n_nets, c->want_virial ? c->d_virial : nullptr);
@@ -694,7 +706,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     TRY(dev_alloc(c, &c->G, N * a.kpad));
     if (c->n_nets == 1) c->dG = c->G; // dE/dG overwrites G once layer 1 has consumed it
     else TRY(dev_alloc(c, &c->dG, N * a.kpad));
-    for (int l = 0; l < 3; ++l) TRY(dev_alloc(c, &c->H[l], N * c->hmax[l]));
+    for (int l = 0; l < 3; ++l) TRY(dev_alloc(c, &c->H[l], N * c->hmax[l] * (size_t)c->n_nets));
     TRY(dev_alloc(c, &c->e_atom, N));
     TRY(dev_alloc(c, &c->e_mol, (size_t)max_mols));
     TRY(dev_alloc(c, &c->ekin, 1));

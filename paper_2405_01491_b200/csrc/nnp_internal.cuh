@@ -9,6 +9,7 @@
 #include "../../include/nnp.h"
 
 #define NNP_MAX_SPECIES 8
+#define NNP_MAX_GROUPS 16  // (network, species) groups of one grouped GEMM launch: ensembles batch their networks per layer
 #define NNP_NSHF_R 16
 #define NNP_NSHF_A 8
 #define NNP_NSHF_Z 4
@@ -107,9 +108,9 @@ struct GemmGroup {
 };
 
 struct GemmBatch {
-    GemmGroup g[NNP_MAX_SPECIES];
+    GemmGroup g[NNP_MAX_GROUPS];
     int n_groups;
-    int tile_off[NNP_MAX_SPECIES + 1]; // prefix sum of M tiles per group (tile height given at launch)
+    int tile_off[NNP_MAX_GROUPS + 1]; // prefix sum of M tiles per group (tile height given at launch)
     float alpha;                       // CELU alpha
 };
 
@@ -189,7 +190,7 @@ struct nnp_ctx {
     uint16_t *seg_r, *seg_a; // [n][8] species-segment start offsets; entries S..7 = row length (S <= 7)
     // features and network
     float *G, *dG;           // [n][kpad]
-    float *H[3];             // activations / deltas [n][hmax[l]]
+    float *H[3];             // activations / deltas [n_nets][max_atoms][hmax[l]] (one set per network of an ensemble)
     float *e_atom;           // [n]
     double *e_mol;           // [max_mols]
     double *ekin;            // scalar
