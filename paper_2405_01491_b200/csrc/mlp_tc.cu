@@ -511,7 +511,8 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     if (mrow0 + r < g.M) {
                         float4 v;
                         asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
-                        *reinterpret_cast<float4 *>(cbase + (size_t)r * g.ldc + sub_c) = v;
+                        if (EPI == EPI_RED) atomicAdd(reinterpret_cast<float4 *>(cbase + (size_t)r * g.ldc + sub_c), v); // RED.ADD.F32x4
+                        else *reinterpret_cast<float4 *>(cbase + (size_t)r * g.ldc + sub_c) = v;
                     }
                 }
                 __syncwarp();
@@ -655,6 +656,7 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     case EPI_DCELU: launch<EPI_DCELU>(c->stream, tb, tiles, s3); break;
     case EPI_STORE: launch<EPI_STORE>(c->stream, tb, tiles, s3); break;
     case EPI_ACCUM: launch<EPI_ACCUM>(c->stream, tb, tiles, s3); break;
+    case EPI_RED: launch<EPI_RED>(c->stream, tb, tiles, s3); break;
     default: c->err = "bad epilogue"; return NNP_EINVAL;
     }
     c->launches += 1;

@@ -376,11 +376,23 @@ int run_forces(nnp_ctx *c)
             if (rc != NNP_OK) return rc;
             nnp_prof_mark(c, 3 + op);
         }
-    for (int net = 0; net < c->n_nets; ++net) { // dE/dG accumulates over the networks: one network per launch, in order
-        make_batch(c, net, 1, 5, b);
-        int rc = run_gemm(c, b, net > 0 ? EPI_ACCUM : EPI_STORE);
-        if (rc != NNP_OK) return rc;
-        nnp_prof_mark(c, 8);
+    if (nb > 1) {
+        // dE/dG sums over the networks: the groups of all batched networks add into the same rows with vector
+        // reductions in memory (the summation order over the networks is then not fixed, like the force scatter's)
+        CU(c, cudaMemsetAsync(c->dG, 0, sizeof(float) * (size_t)c->n * c->aev.kpad, c->stream));
+        for (int net0 = 0; net0 < c->n_nets; net0 += nb) {
+            make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, 5, b);
+            int rc = run_gemm(c, b, EPI_RED);
+            if (rc != NNP_OK) return rc;
+            nnp_prof_mark(c, 8);
+        }
+    } else {
+        for (int net = 0; net < c->n_nets; ++net) { // one network per launch, accumulated in place in network order
+            make_batch(c, net, 1, 5, b);
+            int rc = run_gemm(c, b, net > 0 ? EPI_ACCUM : EPI_STORE);
+            if (rc != NNP_OK) return rc;
+            nnp_prof_mark(c, 8);
+        }
     }
     nnp_launch_energy_reduce(c);
     nnp_prof_mark(c, 9);

@@ -92,7 +92,9 @@ enum GemmEpilogue {
     EPI_CELU_OUT = 1, // h = celu(acc + bias); e_atom[m] += sum_n h*w4[n]; C = w4[n] * celu'(h)
     EPI_DCELU = 2,    // C = acc * celu'(H) with H read from C (in place)
     EPI_STORE = 3,    // C = acc
-    EPI_ACCUM = 4     // C += acc
+    EPI_ACCUM = 4,    // C += acc
+    EPI_RED = 5       // C += acc with vector reductions in memory (several groups of one launch add into the same rows;
+                      // tensor-core path only)
 };
 
 struct GemmGroup {
