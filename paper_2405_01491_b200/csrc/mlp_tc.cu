@@ -599,6 +599,9 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     // a launch with a wider layer splits it into <= 128-column parts, and then the 48 KiB stages / 4-deep ring serve
     // all its groups better than 64 KiB stages / 3-deep (measured on the 98k water box: 0.363 -> 0.344 ms over the six GEMMs)
     int nt_cap = NT_MAX;
+    // fixed cost of a tile in the balance below, in 128-byte units (NNP_TC_FIXED overrides it for sweeps)
+    static int env_fixed = -1;
+    if (env_fixed < 0) { const char *e = getenv("NNP_TC_FIXED"); env_fixed = e ? atoi(e) : 3000; }
     for (int i = 0; i < b.n_groups; ++i)
         if (b.g[i].N > NT_MAX) nt_cap = 128;
     for (int i = 0; i < b.n_groups; ++i) {
@@ -627,8 +630,10 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
         tiles += nnp_div_up(g.M, TILE_M) * t.n_tiles_n;
         // bytes through the SM in units of 128 B (the kernel is bound by L2 -> SM traffic): per K block the A tile and the
         // hi/lo weight tiles, plus the output tile (read and written by the in-place epilogues)
-        // ... plus a fixed 1000 per tile for the pipeline fill / accumulator hand-over (swept 0..8000 on the 98k water box)
-        tb.tile_cost[i] = g.K / BLOCK_K * (TILE_M + 2 * NT) + ((epi == EPI_DCELU || epi == EPI_ACCUM) ? 8 : 4) * NT + 1000;
+        // ... plus a fixed 3000 per tile for the pipeline fill / accumulator hand-over (swept 0..20000 on the 98k water box with the
+        // eight-warp epilogue: the six GEMMs take 0.323 ms at 1000, 0.314 at 3000, 0.313 at 4000, 0.329 at 8000; the layers
+        // move in steps of ~4 us as the slowest CTA gains or loses a tile, which a dynamic tile queue would even out)
+        tb.tile_cost[i] = g.K / BLOCK_K * (TILE_M + 2 * NT) + ((epi == EPI_DCELU || epi == EPI_ACCUM) ? 8 : 4) * NT + env_fixed;
         tb.cost_total += (long long)tb.tile_cost[i] * (tiles - tb.tile_off[i]);
     }
     tb.n_groups = b.n_groups;
