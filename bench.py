@@ -333,8 +333,8 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch [bytes] of each stage's kernel on the 98,304-atom workload,
 # from the one `ncu --set full` capture summarised in profiles/r01_ncu_full_3xtf32.md (3xTF32 mode).
-TRAFFIC_NCU = {"aev_forward": 67.9e6, "aev_backward_scatter": 110.7e6, "mlp_fwd_l1": 94.4e6, "mlp_fwd_l2": 122.6e6,
-               "mlp_fwd_l3_out": 93.9e6, "mlp_bwd_l3": 156.5e6, "mlp_bwd_l2": 222.3e6, "mlp_bwd_l1_dEdG": 108.1e6}
+TRAFFIC_NCU = {"aev_forward": 67.7e6, "aev_backward_scatter": 110.8e6, "mlp_fwd_l1": 94.7e6, "mlp_fwd_l2": 122.3e6,
+               "mlp_fwd_l3_out": 94.3e6, "mlp_bwd_l3": 156.3e6, "mlp_bwd_l2": 225.5e6, "mlp_bwd_l1_dEdG": 108.6e6}
 
 
 def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
