@@ -158,6 +158,21 @@ def test_periodic_replica_batch(model1, n_waters, L, n_rep):
         nnp.nnp_destroy(ctx)
 
 
+# ---------------------------------------------------------------- the other matmul modes on an ensemble
+@pytest.mark.parametrize("mm_mode", [nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC], ids=["fp32_simt", "3xtf32_tc"])
+def test_ensemble_in_both_fp32_grade_modes(mm_mode):
+    """Three networks on a 216-water box: the fp32 SIMT path runs the networks one after the other, the tensor-core path
+    batches them into one grouped launch per layer (dE/dG summed by reductions in memory); both meet the bars."""
+    consts, widths, params, om = U.make_model(3, seed=inputs.SEED0 + 21)
+    sp, xyz, box = inputs.water_box(216, seed=inputs.SEED0 + 22)
+    ctx = U.gpu_create(consts, widths, params, 3, len(sp), mm_mode=mm_mode)
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, want_e_atom=True))   # reading B8: E is a cancelling sum here
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
 # ---------------------------------------------------------------- degenerate inputs
 def test_edge_cases(model1):
     consts, widths, params, om = model1
