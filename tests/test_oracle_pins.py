@@ -112,6 +112,55 @@ def test_trimer_angular_hand_values(ani_model, consts):
             assert np.all(G[112 + 32:] == 0)              # nothing outside block (H,H)
 
 
+def test_trimer_angular_off_peak_values(ani_model, consts):
+    """The angular term AWAY from its peaks (the form ((1+cos(theta'-ShfZ))/2)^zeta is PAPER.md L443).
+    Each case makes all but one factor exactly 1, so the remaining factor has a value known without the formula:
+    (i) pins the zeta power, (ii) pins eta_A and that r-bar is the ARITHMETIC mean, (iii) pins the ShfA spacing."""
+    eta_a, zeta = float(consts["eta_a"]), float(consts["zeta"])
+    shf_a, shf_z = np.asarray(consts["shf_a"], float), np.asarray(consts["shf_z"], float)
+    fc = lambda r: 0.5 * math.cos(math.pi * r / 3.5) + 0.5          # noqa: E731  pinned by test_cutoff_function_special_values
+    # (i) theta' = ShfZ_z +- pi/2  =>  (1 + cos(+-pi/2))/2 = 1/2  =>  G = 2 * 2^-zeta * fc^2  at r_ij = r_ik = ShfA_a
+    for z, sign in ((0, +1), (1, +1), (2, -1), (3, -1)):
+        thp = shf_z[z] + sign * math.pi / 2                          # inside [acos(.95), acos(-.95)] for these four
+        theta = math.acos(math.cos(thp) / 0.95)
+        for a in (1, 4):
+            r = float(shf_a[a])
+            sp, xyz = _trimer(r, theta)
+            G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+            want = 2.0 * 2.0 ** (-zeta) * fc(r) ** 2
+            assert abs(G[112 + a * 4 + z] / want - 1.0) < 1e-11, (z, a, G[112 + a * 4 + z], want)
+    # (ii) on-peak angle, r_ik = ShfA_a, r_ij = ShfA_a + 2 delta  =>  r-bar = ShfA_a + delta (arithmetic mean; the geometric
+    #      mean sqrt(s (s + 2 delta)) differs in the 2nd digit of the exponent)  =>  G = 2 exp(-eta_A delta^2) fc(r_ij) fc(r_ik)
+    for a, delta in ((2, 0.11), (5, -0.17), (0, 0.3)):
+        for z in (0, 2):
+            s = float(shf_a[a])
+            theta = math.acos(math.cos(shf_z[z]) / 0.95)
+            rj, rk = s + 2 * delta, s
+            xyz = [[0, 0, 0], [rj, 0, 0], [rk * math.cos(theta), rk * math.sin(theta), 0]]
+            G = orc.energy_forces(ani_model, [3, 0, 0], xyz, want_aev=True)["aev"][0]
+            want = 2.0 * math.exp(-eta_a * delta * delta) * fc(rj) * fc(rk)
+            assert abs(G[112 + a * 4 + z] / want - 1.0) < 1e-11, (a, z, G[112 + a * 4 + z], want)
+            geo = 2.0 * math.exp(-eta_a * (math.sqrt(rj * rk) - s) ** 2) * fc(rj) * fc(rk)
+            assert abs(geo / want - 1.0) > 1e-4                       # the case does tell the two means apart
+    # (iii) r_ij = r_ik = ShfA_a at the on-peak angle: feature a+1 / feature a = exp(-eta_A Delta^2), Delta = 0.3375;
+    #       two shifts on: exp(-4 eta_A Delta^2)
+    dlt = 0.3375
+    for a in (0, 3, 5):
+        theta = math.acos(math.cos(shf_z[1]) / 0.95)
+        sp, xyz = _trimer(float(shf_a[a]), theta)
+        G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+        assert abs(G[112 + (a + 1) * 4 + 1] / G[112 + a * 4 + 1] / math.exp(-eta_a * dlt ** 2) - 1.0) < 1e-11
+        assert abs(G[112 + (a + 2) * 4 + 1] / G[112 + a * 4 + 1] / math.exp(-4 * eta_a * dlt ** 2) - 1.0) < 1e-11
+    # and between neighbouring ShfZ at theta' = (ShfZ_0 + ShfZ_1)/2: equal bases => equal features (symmetric about the midpoint)
+    thp = 0.5 * (shf_z[0] + shf_z[1])
+    sp, xyz = _trimer(1.9, math.acos(math.cos(thp) / 0.95))
+    G = orc.energy_forces(ani_model, sp, xyz, want_aev=True)["aev"][0]
+    assert abs(G[112 + 3 * 4 + 0] / G[112 + 3 * 4 + 1] - 1.0) < 1e-11
+    # value there: base = (1 + cos(pi/8))/2 = cos^2(pi/16)
+    want = 2.0 * math.cos(math.pi / 16) ** (2 * zeta) * math.exp(-eta_a * (1.9 - shf_a[3]) ** 2) * fc(1.9) ** 2
+    assert abs(G[112 + 3 * 4 + 0] / want - 1.0) < 1e-11
+
+
 def test_trimer_block_placement_and_swap(ani_model):
     r, th = 1.7, 1.9
     for sj, sk in ((0, 3), (1, 6), (6, 6), (2, 4)):
