@@ -82,13 +82,13 @@ def oracle_model(n_nets=1):
     return orc, orc.OracleModel(consts, inputs.WIDTHS, params, n_nets)
 
 
-def time_oracle_md(n_waters, n_steps, seed):
+def time_oracle_md(n_waters, n_steps, seed, L=None):
     """Oracle MD on a water box of the workload's density.  orc.md evaluates the initial forces and then one
     force evaluation per step, so the timed work is n_steps + 1 step-equivalents (the integrator itself is
     negligible).  Returns (atom-steps, seconds, cores)."""
     from paper_2405_01491_b200 import inputs
     orc, om = oracle_model()
-    sp, xyz, box = inputs.water_box(n_waters, seed=seed)
+    sp, xyz, box = inputs.water_box(n_waters, L, seed=seed)
     v = inputs.maxwell_boltzmann(sp, T_KELVIN)
     t0 = time.perf_counter()
     orc.md(om, sp, xyz, v, inputs.MASS, box, DT_FS, inputs.ACCEL_CONV, n_steps, skin=SKIN,
@@ -108,10 +108,10 @@ def run_reference(args):
     rate = a / t                          # atom-steps/s
     budget = 150.0 / max(1, K + W + 1)
     n_waters = 64
-    for cand in (216, 512, 1000, 4096):
+    for cand in (216, 512, 1000, 4096, N_WATERS):
         if cand * 3 / rate <= budget:
             n_waters = cand
-    atoms, secs, cores = time_oracle_md(n_waters, K + W, 2)
+    atoms, secs, cores = time_oracle_md(n_waters, K + W, 2, BOX_L if n_waters == N_WATERS else None)
     secs_timed = secs * K / (K + W + 1)
     value = n_waters * 3 * K / secs_timed
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
@@ -124,6 +124,161 @@ def run_reference(args):
                                        (K, n_waters * 3)},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_eval_config(args):
+    """--config 1|2|4|5: the other BASELINE.json workloads.  A step = nnp_build_neighbors(skin 0) + nnp_energy_forces on
+    inputs resident in HBM; same JSON line as the headline, roofline entry for the dominant stage."""
+    import torch
+    from paper_2405_01491_b200 import eval_timing, inputs, nnp
+    import __graft_entry__
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:          # these lines are single-GPU measurements
+        return 0
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    __graft_entry__.build()
+    nnp.lib()
+    name, n_nets, sp, xyz, box, offs = eval_timing._workload(args.config)
+    n = len(sp)
+    n_mols = 1 if offs is None else len(offs) - 1
+    consts = inputs.ani2x_constants()
+    params = inputs.make_weights(inputs.SEED0 + args.config, n_nets, last_layer_scale=args.force_scale)
+    p, keep = nnp.make_params(consts, inputs.WIDTHS, params, inputs.MASS, inputs.ACCEL_CONV, n_nets=n_nets, mm_mode=args.mm_mode)
+    stream = torch.cuda.Stream(device=dev)
+    ctx = nnp.nnp_create(p, n, n_mols, 0, stream.cuda_stream)
+    K, W = args.steps, args.warmup
+    d_sp = torch.as_tensor(np.asarray(sp, dtype=np.int32), device=dev)
+    d_x = torch.as_tensor(np.asarray(xyz, dtype=np.float32), device=dev).contiguous()
+    d_mo = None if offs is None else torch.as_tensor(np.asarray(offs, dtype=np.int32), device=dev)
+    d_E = torch.zeros(n_mols, dtype=torch.float64, device=dev)
+    d_F = torch.zeros((n, 3), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 * 2**20, dtype=torch.uint8, device=dev)      # > the 126 MB L2
+    torch.cuda.synchronize()
+    nnp.nnp_set_system(ctx, n, d_sp, d_x, box, n_mols, d_mo)
+
+    def step():
+        nnp.nnp_build_neighbors(ctx, 0.0)
+        nnp.nnp_energy_forces(ctx, d_E, d_F)
+
+    with torch.cuda.stream(stream):
+        for _ in range(W):
+            step()
+        nnp.nnp_sync(ctx)
+        sampler = ClockSampler(0)
+        sampler.start()
+        l0 = nnp.nnp_launch_count(ctx)
+        evs = []
+        for _ in range(K):                      # L2 flushed between the timed iterations (outside the event pairs)
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            step()
+            b.record(stream)
+            evs.append((a, b))
+        nnp.nnp_sync(ctx)
+        launches = nnp.nnp_launch_count(ctx) - l0
+        sampler.stop_flag.set()
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+        # counts of the method's own work, from the lists (skin 0: the rows are the in-cutoff neighbours)
+        d_c = torch.zeros(n, dtype=torch.int32, device=dev)
+        d_l = torch.zeros((n, 4), dtype=torch.int32, device=dev)
+        nnp.nnp_get_neighbors(ctx, 0, d_c, d_l, 4)
+        n_rad = int(d_c.sum().item())
+        nnp.nnp_get_neighbors(ctx, 1, d_c, d_l, 4)
+        ca = d_c.to(torch.int64)
+        n_tri = int((ca * (ca - 1) // 2).sum().item())
+        # per-stage pass (untimed)
+        P = min(args.profile_steps, 20)
+        nnp.nnp_profile(ctx, 1)
+        for _ in range(P):
+            flush.fill_(1)
+            step()
+        stage_ms, stage_n = nnp.nnp_profile_read(ctx)
+        nnp.nnp_profile(ctx, 0)
+    kact = nnp.nnp_aev_active_columns(ctx)
+    sampler.join(timeout=2)
+    # ---- end to end: host species / coordinates / offsets in, energies and forces out, every step (pinned buffers)
+    h_sp = torch.as_tensor(np.asarray(sp, dtype=np.int32)).pin_memory()
+    h_x = torch.as_tensor(np.asarray(xyz, dtype=np.float32)).contiguous().pin_memory()
+    h_mo = None if offs is None else torch.as_tensor(np.asarray(offs, dtype=np.int32)).pin_memory()
+    h_E = torch.zeros(n_mols, dtype=torch.float64).pin_memory()
+    h_F = torch.zeros((n, 3), dtype=torch.float32).pin_memory()
+    Ke = min(K, args.e2e_steps)
+    for _ in range(3):
+        nnp.nnp_energy_forces_host(ctx, n, h_sp, h_x, box, n_mols, h_mo, 0.0, h_E, h_F)
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        nnp.nnp_energy_forces_host(ctx, n, h_sp, h_x, box, n_mols, h_mo, 0.0, h_E, h_F)
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    nnp.nnp_destroy(ctx)
+
+    pk, clocks = peaks(), sampler.summary()
+    build_ms = stage_ms[1] / max(1, stage_n[1])
+    per_stage = {nnp.STAGE_NAMES[k]: (stage_ms[k] / stage_n[k] if stage_n[k] else 0.0) for k in range(nnp.NNP_N_STAGES)}
+    per_stage = {k: v for k, v in per_stage.items() if k not in ("kick_drift", "kick_ekin")}
+    per_stage["neighbor_build"] = (ms / K) - sum(v for k, v in per_stage.items() if k != "neighbor_build")   # events cover E+F only
+    del build_ms
+    tot = sum(per_stage.values())
+    mlp_ms = sum(v for k, v in per_stage.items() if k.startswith("mlp"))
+    groups = {"mlp_all_layers": mlp_ms, **{k: v for k, v in per_stage.items() if not k.startswith("mlp")}}
+    dom = max(groups, key=groups.get)
+    kpad = (kact + 31) // 32 * 32
+    fp32_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    if dom == "mlp_all_layers":
+        counts = np.bincount(sp, minlength=7)
+        Wd = inputs.WIDTHS
+        macs = sum(int(counts[s]) * (kpad * int(Wd[s, 1]) + int(Wd[s, 1]) * int(Wd[s, 2]) + int(Wd[s, 2]) * int(Wd[s, 3]) + int(Wd[s, 3]))
+                   for s in range(7))
+        ach = 2.0 * 2.0 * macs * n_nets / (mlp_ms * 1e-3) / 1e12           # forward + input gradient
+        peak = pk["bf16_sus"] * 0.5 if args.mm_mode in (1, 2) else fp32_peak
+        roof = {"kernel": "mlp_all_layers (6 grouped GEMM launches per network batch)", "bound": "tensor" if args.mm_mode in (1, 2) else "alu",
+                "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                "peak_source": "%s sustained bf16 cuBLAS x 0.5; fp32-equivalent flops counted once" % pk["source"]}
+    elif dom in ("aev_forward", "aev_backward_scatter"):
+        flop = {"aev_forward": n_rad * 16 * 6 + n_tri * 150.0, "aev_backward_scatter": n_rad * 16 * 10 + n_tri * 330.0}[dom]
+        ach = flop / (groups[dom] * 1e-3) / 1e12
+        roof = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach / fp32_peak,
+                "traffic": None, "peak_source": "148 SM x 128 lanes x 2 x clocks.max.sm; work counted from the lists: %d radial terms, "
+                "%d triplets" % (n_rad, n_tri)}
+    else:
+        byts = {"neighbor_build": (n_rad + int(ca.sum().item())) * 4.0 + n * 48.0, "energy_sum": n * 12.0}.get(dom, n * 64.0)
+        ach = byts / (groups[dom] * 1e-3) / 1e9
+        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": pk["hbm"], "unit": "GB/s", "frac": ach / pk["hbm"],
+                "traffic": None, "peak_source": pk["source"]}
+    roof["traffic"] = traffic_from_profiles(dom, "config%d_mm%d" % (args.config, args.mm_mode))
+    roof["stage_ms"] = {k: round(v, 4) for k, v in per_stage.items()}
+    roof["stage_share"] = {k: round(v / tot, 4) for k, v in per_stage.items()} if tot else {}
+    roof["stage_ms_source"] = "separate untimed pass of %d steps with CUDA events around every stage; neighbor_build = step - rest" % P
+    line = {"metric": "ANI-2x energy+force atom-steps/s (one list build + one energy/force evaluation per step, %s)" % name,
+            "value": n * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": name, "atoms": n, "structures": n_mols, "n_nets": n_nets, "aev_active_columns": kact,
+                       "mm_mode": ["fp32_simt", "3xtf32_tcgen05", "tf32_tcgen05", "fp64_simt"][args.mm_mode],
+                       "us_per_evaluation": 1e3 * ms / K, "force_scale": args.force_scale,
+                       "radial_terms": n_rad, "triplets": n_tri,
+                       "launch_path": "kernel_by_kernel (nnp_build_neighbors + nnp_energy_forces per step)",
+                       "l2_policy": "L2 flushed (256 MB write) between timed iterations, outside the event pairs",
+                       "parallelism": "single GPU"},
+            "clocks": clocks,
+            "e2e": {"value": n * Ke / e2e_s, "unit": UNIT, "steps": Ke,
+                    "h2d_bytes_per_step": n * 16 + (4 * (n_mols + 1) if offs is not None else 0),
+                    "d2h_bytes_per_step": n * 12 + 8 * n_mols + 12,
+                    "api": "nnp_energy_forces_host (pinned host species, xyz[, offsets] up; energies, forces down; every step)"},
+            "gpu_launches": launches, "roofline": roof}
+    if not args.no_cpu_baseline:
+        orc, om = oracle_model(1)
+        om = orc.OracleModel(consts, inputs.WIDTHS, inputs.make_weights(inputs.SEED0 + args.config, 1, last_layer_scale=args.force_scale), 1)
+        t0 = time.perf_counter()
+        orc.energy_forces(om, sp, xyz, box, offs, nbr_method=1 if (box is not None and n >= 600) else 0)
+        secs = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": n / secs, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                                "sample": "one energy+force evaluation of the whole workload with ONE network (fp64 oracle, OpenMP; "
+                                          "the workload's ensemble has %d)" % n_nets}
     print(json.dumps(line))
     return 0
 
@@ -230,7 +385,7 @@ def run_ours(args):
     nnp.nnp_sync(ctx)
     st["e0"], st["nr0"], st["ek0"] = read_state()
     st["rebuilds"], st["restarts"] = 0, 0
-    nnp.nnp_profile(ctx, max(1, K // 256))
+    nnp.nnp_profile(ctx, 0)          # no instrumentation inside the timed region: every timed step is one CUDA-graph launch
     sampler = ClockSampler(local)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = nnp.nnp_launch_count(ctx)
@@ -246,12 +401,22 @@ def run_ours(args):
     kact = nnp.nnp_aev_active_columns(ctx)
     ms = ev0.elapsed_time(ev1)
     nnp.nnp_sync(ctx)
-    stage_ms, stage_n = nnp.nnp_profile_read(ctx)
-    nnp.nnp_profile(ctx, 0)
     e_end, nr_end, ek_end = read_state()
     e_start, ek_start = st["e0"], st["ek0"]          # energy drift and temperatures: over the last trajectory segment
     n_rebuilds, n_restarts = st["rebuilds"] + nr_end - st["nr0"], st["restarts"]
     sampler.join(timeout=2)
+
+    # ---- per-stage timings: a SEPARATE, untimed pass (CUDA events around every stage need the kernel-by-kernel launch
+    # path; the timed region above ran the graph path only).  Same trajectory, restarted so it stays on its healthy stretch.
+    P = args.profile_steps
+    restart()
+    nnp.nnp_md_step(ctx, 20)
+    nnp.nnp_sync(ctx)
+    nnp.nnp_profile(ctx, 1)
+    nnp.nnp_md_step(ctx, P)
+    stage_ms, stage_n = nnp.nnp_profile_read(ctx)
+    nnp.nnp_profile(ctx, 0)
+    st["since"] = 20 + P
 
     # ---- end-to-end through the host entry point: every step uploads x,v and downloads x,v,E (pinned memory)
     Ke = min(K, args.e2e_steps, TRAJ_MAX // 2)
@@ -293,6 +458,7 @@ def run_ours(args):
     dom = max(per_stage, key=per_stage.get)
     kpad = (kact + 31) // 32 * 32
     roof = roofline_for(dom, per_stage[dom], n, sp, args.mm_mode, pk, clocks, kpad)
+    roof["stage_ms_source"] = "separate untimed pass of %d kernel-by-kernel steps with CUDA events around every stage" % P
     roof["stage_ms"] = {k: round(v, 4) for k, v in per_stage.items()}
     roof["stage_share"] = {k: round(v / tot_stage, 4) for k, v in per_stage.items()} if tot_stage else {}
 
@@ -309,6 +475,8 @@ def run_ours(args):
                    "temperature_K_end": 2 * ek_end / (3 * n * inputs.KB), "temperature_K_start": 2 * ek_start / (3 * n * inputs.KB),
                    "etot_drift_rel": (e_end - e_start) / abs(e_start) if e_start else None,
                    "aev_active_columns": kact,
+                   "launch_path": "kernel_by_kernel" if os.environ.get("NNP_NO_GRAPH") == "1" else
+                                  "cuda_graph (one graph launch per step, rebuild inside a conditional node)",
                    "l2_policy": "inputs larger than L2: per step the kernels stream G (%d MB), the activations (%d MB) and "
                                 "the neighbour rows (%d MB); no flush needed" % (n * kpad * 4 // 2**20, n * 608 * 4 // 2**20,
                                                                                    n * 224 * 4 // 2**20),
@@ -321,26 +489,61 @@ def run_ours(args):
         "roofline": roof,
     }
     if world == 1 and not args.no_cpu_baseline:
-        atoms, secs, cores = time_oracle_md(args.cpu_waters, 2, 5)
+        atoms, secs, cores = time_oracle_md(args.cpu_waters, args.cpu_steps, inputs.SEED0 + 3,
+                                            BOX_L if args.cpu_waters == N_WATERS else None)
         line["cpu_baseline"] = {"value": atoms / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": "2 velocity-Verlet steps of a %d-atom water box of the same density and model "
-                                          "(fp64 oracle, OpenMP)" % (args.cpu_waters * 3)}
+                                "sample": "%d velocity-Verlet steps (%d force evaluations) of %s (fp64 oracle, OpenMP)" %
+                                          (args.cpu_steps, args.cpu_steps + 1,
+                                           "the workload itself: the same seeded 98,304-atom water box" if args.cpu_waters == N_WATERS
+                                           else "a %d-atom water box of the same density and model" % (args.cpu_waters * 3))}
     print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch [bytes] of each stage's kernel on the 98,304-atom workload,
-# from the one `ncu --set full` capture summarised in profiles/r01_ncu_full_3xtf32.md (3xTF32 mode).
-TRAFFIC_NCU = {"aev_forward": 67.7e6, "aev_backward_scatter": 110.8e6, "mlp_fwd_l1": 94.7e6, "mlp_fwd_l2": 122.3e6,
-               "mlp_fwd_l3_out": 94.3e6, "mlp_bwd_l3": 156.3e6, "mlp_bwd_l2": 225.5e6, "mlp_bwd_l1_dEdG": 108.6e6}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic_ncu.csv")
 
 
-def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
+def kernel_source_hash():
+    """sha256 over the CUDA sources: the stamp that ties an ncu capture to the kernels it was taken from (the GPU box has
+    no .git, so the commit id itself cannot be checked there)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2405_01491_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def traffic_from_profiles(stage, workload_key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch [bytes] of the stage's kernel from the committed `ncu --set
+    full` capture (profiles/traffic_ncu.csv: '# source=<hash>' header, rows workload,stage,read_bytes,write_bytes).
+    None when there is no capture of this workload or the kernels have changed since it was taken."""
+    if not os.path.exists(TRAFFIC_FILE):
+        return None
+    stamp, rows = None, {}
+    for ln in open(TRAFFIC_FILE):
+        ln = ln.strip()
+        if ln.startswith("#"):
+            if "source=" in ln:
+                stamp = ln.split("source=")[1].split()[0]
+            continue
+        f = ln.split(",")
+        if len(f) >= 4 and f[0] != "workload":
+            rows[(f[0], f[1])] = float(f[2]) + float(f[3])
+    if stamp != kernel_source_hash():
+        return None
+    return rows.get((workload_key, stage))
+
+
+def roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad, workload_key=None):
     r = _roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad)
-    if n == 3 * N_WATERS and mm_mode == 1:
-        r["traffic"] = TRAFFIC_NCU.get(stage)
+    if workload_key is None and n == 3 * N_WATERS:
+        workload_key = "config3"
+    r["traffic"] = traffic_from_profiles(stage, "%s_mm%d" % (workload_key, mm_mode)) if workload_key else None
     return r
 
 
@@ -395,7 +598,12 @@ def main():
     ap.add_argument("--waters", type=int, default=N_WATERS)
     ap.add_argument("--force-scale", type=float, default=None)
     ap.add_argument("--e2e-steps", type=int, default=200)
-    ap.add_argument("--cpu-waters", type=int, default=4096)
+    ap.add_argument("--cpu-waters", type=int, default=N_WATERS, help="cpu_baseline: waters in the oracle's box (default: the workload)")
+    ap.add_argument("--cpu-steps", type=int, default=2)
+    ap.add_argument("--profile-steps", type=int, default=48, help="steps of the separate per-stage timing pass")
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json configuration (1-based): 3 = the headline MD workload; 1, 2, 4, 5 = one list build + one "
+                         "energy/force evaluation per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--langevin", type=float, default=0.0, help="friction in 1/fs: BAOAB Langevin at 300 K instead of velocity Verlet")
     args = ap.parse_args()
@@ -406,6 +614,10 @@ def main():
         args.force_scale = inputs.FORCE_SCALE_MD
     if args.impl == "reference":
         return run_reference(args)
+    if args.config != 3:
+        if args.steps == 1000 and args.warmup == 50:      # the MD defaults: an evaluation workload needs far fewer
+            args.steps, args.warmup = 50, 5
+        return run_eval_config(args)
     return run_ours(args)
 
 

@@ -51,7 +51,11 @@ typedef enum {
     NNP_EBOX = -6       /* periodic box edge < 2*(cutoff+skin): minimum image not unique (reading C1) */
 } nnp_status;
 
-enum { NNP_MM_FP32_SIMT = 0, NNP_MM_3XTF32_TC = 1, NNP_MM_TF32_TC = 2 };
+/* How the MLP contractions are computed (Fig. 3: matmul precision decides energy conservation):
+ * 0 fp32 FMA on the CUDA cores; 1 (default of the tests and the bench) 3xTF32 on tcgen05, fp32-grade; 2 plain TF32 on
+ * tcgen05 (fails the parity bars, kept for the precision study); 3 fp32 operands with every product and sum in fp64
+ * (DFMA on the CUDA cores) -- the fp64 leg of the precision study, slow. */
+enum { NNP_MM_FP32_SIMT = 0, NNP_MM_3XTF32_TC = 1, NNP_MM_TF32_TC = 2, NNP_MM_FP64_SIMT = 3 };
 
 typedef struct {
     int n_species;            /* <= 7; ANI-2x: 7, index order H,C,N,O,S,F,Cl (reading B2) */
@@ -73,15 +77,26 @@ typedef struct {
     const float *mass;        /* host [n_species], amu */
     float accel_conv;         /* a = accel_conv * F / m  (4.184e-4 for kcal/mol, A, fs, amu; reading B6) */
     int mm_mode;              /* NNP_MM_*: how the MLP contractions are computed */
-    int cap_r, cap_a;         /* neighbour-row capacities (radial / angular lists); 0 => 160 / 64; <= 255, multiple of 4 */
+    int cap_r, cap_a;         /* capacities of the radial / angular neighbour ROWS (entries with r < cutoff + skin); 0 =>
+                                 160 / 64; multiples of 4 in [4, 65532].  Independently of cap_a, a centre may have at most
+                                 64 angular neighbours INSIDE the cutoff rca (the AEV kernels keep them in shared memory);
+                                 any overflow is reported as NNP_ECAPACITY, never truncated silently. */
     int dense_aev;            /* 0 (default): AEV columns of species absent from the loaded system -- identically zero
                                  for every atom -- are neither stored nor multiplied (the layer-1 weights are gathered
                                  to the active columns at nnp_set_system; results are unchanged).  1: always keep all
                                  aev_len columns (e.g. 1008), as a plain implementation would. */
+    /* Device-memory hooks (north_star: PyTorch supplies device memory): every device buffer the library
+     * owns is obtained from alloc(bytes, alloc_user) -- which returns a device pointer aligned to >= 256 bytes on the
+     * device given to nnp_create, or NULL on failure (-> NNP_ENOMEM) -- and returned with dealloc(ptr, alloc_user), at
+     * nnp_destroy at the latest.  E.g. torch.cuda.caching_allocator_alloc / _delete.  Both NULL: cudaMalloc / cudaFree. */
+    void *(*alloc)(size_t bytes, void *alloc_user);
+    void (*dealloc)(void *ptr, void *alloc_user);
+    void *alloc_user;
 } nnp_params;
 
-/* Copies all parameters to the device (the caller keeps its arrays) and allocates every scratch buffer
- * for up to max_atoms atoms in up to max_mols structures.  cuda_stream is a cudaStream_t (NULL = legacy
+/* The model of PAPER.md L176 (Fig. 2: AEV embedding, species-specialised networks, sum) with the constants of
+ * DESIGN.md section 2 as parameters.  Copies all parameters to the device (the caller keeps its arrays) and allocates
+ * every scratch buffer (through nnp_params.alloc if given) for up to max_atoms atoms in up to max_mols structures.  cuda_stream is a cudaStream_t (NULL = legacy
  * default stream).  Synchronises. */
 int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, int device, void *cuda_stream);
 void nnp_destroy(nnp_ctx *ctx);
@@ -156,7 +171,10 @@ int nnp_sync(nnp_ctx *ctx);
  * nnp_energy_forces_host = nnp_set_system + nnp_build_neighbors(skin) + nnp_energy_forces.
  * nnp_md_step_host: uploads h_xyz/h_vel [n][3] into the running MD state (atoms as in nnp_set_system; lists
  * are kept and rebuilt by the displacement rule), runs n_steps, downloads positions, velocities, epot, ekin (the two
- * scalars and the device-side error flags travel in one 40-byte pinned copy).  Synchronises before returning. */
+ * scalars and the device-side error flags travel in one 40-byte pinned copy).  Synchronises before returning.
+ * h_xyz / h_vel must be the state returned by the previous call (or the state given to nnp_md_init), possibly with atoms
+ * shifted by whole cell vectors: the first half kick uses the forces of the previous evaluation, which are NOT recomputed
+ * from the uploaded positions. */
 int nnp_energy_forces_host(nnp_ctx *ctx, int n_atoms, const int32_t *h_species, const float *h_xyz,
                            const float h_box[3], int n_mols, const int32_t *h_mol_offsets, float skin,
                            double *h_energy, float *h_forces);

@@ -629,8 +629,8 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     // (-2 eta / ka) w ra with w = ka (rb - s): P.half_drb_scale, P.dr_scale (AevParams, nnp_aev_derive)
     float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.ab);
 
-    // Centres are handed out dynamically (one ticket per centre): the cost of a centre varies with its pair count,
-    // and with a static split the slowest warp of a persistent grid ends ~20 % after the average one.
+    // Centres are assigned statically (AEV_BWD_SCHED 0: warp w takes w, w + W, ...): for this kernel the ticket queues
+    // measured slower (0.335 / 0.339 ms against 0.300 ms), see DESIGN.md section 6.
     float vir[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     CentreQueue<AEV_BWD_SCHED> queue;
     queue.init(sched, n, nsm, lane);

@@ -1,7 +1,9 @@
-// Stage 3/4, mm_mode = NNP_MM_FP32_SIMT: species-grouped fp32 GEMMs on the CUDA cores with the layer
+// Stage 3/4, mm_mode = NNP_MM_FP32_SIMT / NNP_MM_FP64_SIMT: species-grouped GEMMs on the CUDA cores with the layer
 // epilogues fused (bias + CELU; last hidden layer folded with the 1-wide output layer and CELU'; reverse-mode
 // delta chain with CELU').  ChemicalNet; "highest" fp32 precision, L315-321.
-// This is the full-fp32 reference path on the device; the tensor-core path is mlp_tc.cu.
+// ACC = float: the full-fp32 path on the device.  ACC = double: the fp64 leg of the precision study (Fig. 3
+// compares bf16 / TF32 / fp32 / fp64 matmuls): fp32 operands, every product and sum of the contraction, the bias, CELU and
+// CELU' in fp64 (DFMA), the result rounded once to the fp32 activation buffers.  The tensor-core path is mlp_tc.cu.
 #include "nnp_internal.cuh"
 
 namespace {
@@ -20,7 +22,13 @@ __device__ __forceinline__ float celu_fwd(float x, float alpha, float inv_alpha)
 // CELU'(z) expressed with h = CELU(z): 1 for h > 0, else exp(z/alpha) = 1 + h/alpha
 __device__ __forceinline__ float celu_grad_from_h(float h, float inv_alpha) { return fmaf(fminf(h, 0.f), inv_alpha, 1.0f); }
 
-template <int EPI>
+__device__ __forceinline__ double celu_fwd(double x, double alpha, double inv_alpha)
+{
+    return fmax(x, 0.0) + alpha * expm1(fmin(x, 0.0) * inv_alpha);
+}
+__device__ __forceinline__ double celu_grad_from_h(double h, double inv_alpha) { return fma(fmin(h, 0.0), inv_alpha, 1.0); }
+
+template <int EPI, typename ACC>
 __global__ void __launch_bounds__(THREADS)
 k_gemm_simt(GemmBatch batch)
 {
@@ -41,11 +49,11 @@ k_gemm_simt(GemmBatch batch)
     const int a_row = tid / 4, a_k4 = (tid % 4) * 4;
     const int b_k = tid / 16, b_n4 = (tid % 16) * 4;
 
-    float acc[TM][TN];
+    ACC acc[TM][TN];
 #pragma unroll
     for (int i = 0; i < TM; ++i)
 #pragma unroll
-        for (int j = 0; j < TN; ++j) acc[i][j] = 0.f;
+        for (int j = 0; j < TN; ++j) acc[i][j] = (ACC)0;
 
     float4 ra[2], rb;
     auto gload = [&](int k0) {
@@ -88,7 +96,7 @@ k_gemm_simt(GemmBatch batch)
 #pragma unroll
             for (int i = 0; i < TM; ++i)
 #pragma unroll
-                for (int j = 0; j < TN; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+                for (int j = 0; j < TN; ++j) acc[i][j] = fma((ACC)av[i], (ACC)bv[j], acc[i][j]);
         }
         if (kt + 1 < nk) {
             sstore(buf ^ 1);
@@ -97,7 +105,7 @@ k_gemm_simt(GemmBatch batch)
     }
 
     // ---- epilogue
-    const float alpha = batch.alpha, inv_alpha = 1.0f / batch.alpha;
+    const ACC alpha = (ACC)batch.alpha, inv_alpha = (ACC)1 / (ACC)batch.alpha;
     const int col = n0 + tx * TN;
     const bool colok = col < g.N; // N is a multiple of 32 and TN = 4: a thread's 4 columns are all in or all out
     float bias[TN] = {0.f, 0.f, 0.f, 0.f}, w4[TN] = {0.f, 0.f, 0.f, 0.f};
@@ -112,7 +120,7 @@ k_gemm_simt(GemmBatch batch)
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
         const int row = m0 + ty * TM + i;
-        float esum = 0.f;
+        ACC esum = (ACC)0;
         float4 out;
         float *o = reinterpret_cast<float *>(&out);
         float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -121,22 +129,22 @@ k_gemm_simt(GemmBatch batch)
         const float *pv = reinterpret_cast<const float *>(&prev);
 #pragma unroll
         for (int j = 0; j < TN; ++j) {
-            float v = acc[i][j];
-            if (EPI == EPI_CELU) v = celu_fwd(v + bias[j], alpha, inv_alpha);
+            ACC v = acc[i][j];
+            if (EPI == EPI_CELU) v = celu_fwd(v + (ACC)bias[j], alpha, inv_alpha);
             if (EPI == EPI_CELU_OUT) {
-                const float h = celu_fwd(v + bias[j], alpha, inv_alpha);
-                esum = fmaf(h, w4[j], esum);
-                v = w4[j] * celu_grad_from_h(h, inv_alpha);
+                const ACC h = celu_fwd(v + (ACC)bias[j], alpha, inv_alpha);
+                esum = fma(h, (ACC)w4[j], esum);
+                v = (ACC)w4[j] * celu_grad_from_h(h, inv_alpha);
             }
-            if (EPI == EPI_DCELU) v *= celu_grad_from_h(pv[j], inv_alpha);
-            if (EPI == EPI_ACCUM) v += pv[j];
-            o[j] = v;
+            if (EPI == EPI_DCELU) v *= celu_grad_from_h((ACC)pv[j], inv_alpha);
+            if (EPI == EPI_ACCUM) v += (ACC)pv[j];
+            o[j] = (float)v;
         }
         if (EPI == EPI_CELU_OUT) {
             // reduce the partial dot product over the 16 threads (tx) that share this row
 #pragma unroll
             for (int off = 8; off >= 1; off >>= 1) esum += __shfl_xor_sync(0xffffffffu, esum, off);
-            if (tx == 0 && row < g.M) atomicAdd(g.e_atom + row, esum);
+            if (tx == 0 && row < g.M) atomicAdd(g.e_atom + row, (float)esum);
         }
         if (row < g.M && colok) *reinterpret_cast<float4 *>(cp) = out;
     }
@@ -144,7 +152,19 @@ k_gemm_simt(GemmBatch batch)
 
 } // namespace
 
-void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b_in, int epi)
+template <typename ACC>
+static void launch_simt(cudaStream_t st, const GemmBatch &b, int epi, dim3 grid)
+{
+    switch (epi) {
+    case EPI_CELU: k_gemm_simt<EPI_CELU, ACC><<<grid, THREADS, 0, st>>>(b); break;
+    case EPI_CELU_OUT: k_gemm_simt<EPI_CELU_OUT, ACC><<<grid, THREADS, 0, st>>>(b); break;
+    case EPI_DCELU: k_gemm_simt<EPI_DCELU, ACC><<<grid, THREADS, 0, st>>>(b); break;
+    case EPI_STORE: k_gemm_simt<EPI_STORE, ACC><<<grid, THREADS, 0, st>>>(b); break;
+    case EPI_ACCUM: k_gemm_simt<EPI_ACCUM, ACC><<<grid, THREADS, 0, st>>>(b); break;
+    }
+}
+
+void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b_in, int epi, int fp64_acc)
 {
     GemmBatch b = b_in;
     int tiles = 0, nmax = 0;
@@ -156,12 +176,7 @@ void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b_in, int epi)
     b.tile_off[b.n_groups] = tiles;
     if (tiles == 0) return;
     dim3 grid(tiles, nnp_div_up(nmax, BN));
-    switch (epi) {
-    case EPI_CELU: k_gemm_simt<EPI_CELU><<<grid, THREADS, 0, c->stream>>>(b); break;
-    case EPI_CELU_OUT: k_gemm_simt<EPI_CELU_OUT><<<grid, THREADS, 0, c->stream>>>(b); break;
-    case EPI_DCELU: k_gemm_simt<EPI_DCELU><<<grid, THREADS, 0, c->stream>>>(b); break;
-    case EPI_STORE: k_gemm_simt<EPI_STORE><<<grid, THREADS, 0, c->stream>>>(b); break;
-    case EPI_ACCUM: k_gemm_simt<EPI_ACCUM><<<grid, THREADS, 0, c->stream>>>(b); break;
-    }
+    if (fp64_acc) launch_simt<double>(c->stream, b, epi, grid);
+    else launch_simt<float>(c->stream, b, epi, grid);
     c->launches += 1;
 }

@@ -61,16 +61,8 @@ struct TcBatch {
     int stages, stage_bytes, b_tile_bytes; // ring depth; 16 KiB + 2 * b_tile_bytes; nt_max * 128
     int acc_stride, a_slots;
     float alpha;
-#ifdef NNP_TC_TRACE
-    long long *trace; // [it][8] clock64 stamps of CTA 0
-#endif
 };
 
-#ifdef NNP_TC_TRACE
-#define TRACE(slot) do { if (blockIdx.x == 0 && batch.trace && it < 256) batch.trace[it * 8 + (slot)] = clock64(); } while (0)
-#else
-#define TRACE(slot) do { } while (0)
-#endif
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -270,7 +262,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     const int s = it % S;
                     const uint32_t ph = (it / S) & 1;
                     mbar_wait(bar_empty + 8 * s, ph ^ 1);
-                    TRACE(0);
                     const uint32_t stage = smem_base + s * stage_bytes;
                     // A -> full[s] (wakes the converters); B -> aready[s], the one barrier the MMA thread waits on
                     mbar_expect_tx(bar_full + 8 * s, A_TILE_BYTES);
@@ -295,14 +286,11 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 const int b = lt & 1;
                 const uint32_t acc = tmem_base + (uint32_t)(b * batch.acc_stride);
                 mbar_wait(bar_acce + 8 * b, ((lt >> 1) & 1) ^ 1); // epilogue has drained this accumulator buffer
-                TRACE(6);
                 tc_fence_after();
                 for (int kb = 0; kb < num_kb; ++kb, ++it) {
                     const int s = it % S;
                     const uint32_t ph = (it / S) & 1;
-                    TRACE(3);
                     mbar_wait(bar_aready + 8 * s, ph); // B tiles landed and A converted into TMEM
-                    TRACE(4);
                     tc_fence_after();
                     const uint32_t stage = smem_base + s * stage_bytes;
                     const uint64_t dhi = make_kmajor_sw128_desc(stage + A_TILE_BYTES);
@@ -325,7 +313,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                         if (kb + 1 == num_kb) tc_commit(bar_accf + 8 * b);
                     }
                     __syncwarp();
-                    TRACE(5);
                 }
             }
         }
@@ -350,7 +337,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     tc_fence_after();
                 }
                 mbar_wait(bar_full + 8 * s, ph);
-                if (threadIdx.x == 64 || threadIdx.x == 192) TRACE(1);
                 const uint32_t arow = smem_base + s * stage_bytes + row * 128;
                 uint32_t hi[32], lo[32];
 #pragma unroll
@@ -372,7 +358,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
                 mbar_arrive(bar_aready + 8 * s);
-                if (threadIdx.x == 64 || threadIdx.x == 192) TRACE(2);
             }
         }
     } else {
@@ -437,9 +422,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
             const int c_first = half * EPI_CW;
             if (c_first < g.NT) prefetch(c_first); // before the wait for the accumulator: hides behind the MMAs of this tile
             mbar_wait(bar_accf + 8 * b, (lt >> 1) & 1);
-#ifdef NNP_TC_TRACE
-            if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K) + 1; TRACE(7); }
-#endif
             tc_fence_after();
 
             for (int c0 = c_first; c0 < g.NT; c0 += 2 * EPI_CW) {
@@ -457,9 +439,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                 uint32_t acc[16];
                 tmem_ld16(lane_addr + (uint32_t)(b * batch.acc_stride) + c0, acc);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#ifdef NNP_TC_TRACE
-                if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 2; TRACE(7); }
-#endif
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const int col = 4 * q;
@@ -487,9 +466,6 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     }
                     asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + col * 4), "f"(o.x), "f"(o.y), "f"(o.z), "f"(o.w) : "memory");
                 }
-#ifdef NNP_TC_TRACE
-                if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 3; TRACE(7); }
-#endif
                 __syncwarp();
 #pragma unroll
                 for (int i = 0; i < 4; ++i) { // staging -> global, whole 64-byte row segments
@@ -502,16 +478,10 @@ k_gemm_tc(const __grid_constant__ TcBatch batch)
                     }
                 }
                 __syncwarp();
-#ifdef NNP_TC_TRACE
-                if (threadIdx.x == 320 && c0 == 0) { const int it = lt * (g.K / BLOCK_K) + 4; TRACE(7); }
-#endif
             }
             // the accumulator buffer may be overwritten by the MMAs of tile lt + 2
             tc_fence_before();
             mbar_arrive(bar_acce + 8 * b);
-#ifdef NNP_TC_TRACE
-            if (threadIdx.x == 320) { const int it = lt * (g.K / BLOCK_K); TRACE(7); }
-#endif
             // every epilogue warp (both chunk parities, each n-part of a wide layer) adds its share of the output-layer dot
             if (EPI == EPI_CELU_OUT && rowok) atomicAdd(g.e_atom + m, esum);
         }
@@ -585,9 +555,7 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     // a launch with a wider layer splits it into <= 128-column parts, and then the 48 KiB stages / 4-deep ring serve
     // all its groups better than 64 KiB stages / 3-deep (measured on the 98k water box: 0.363 -> 0.344 ms over the six GEMMs)
     int nt_cap = NT_MAX;
-    // fixed cost of a tile in the balance below, in 128-byte units (NNP_TC_FIXED overrides it for sweeps)
-    static int env_fixed = -1;
-    if (env_fixed < 0) { const char *e = getenv("NNP_TC_FIXED"); env_fixed = e ? atoi(e) : 3000; }
+    const int tile_fixed = 3000; // fixed cost of a tile in the balance below, in 128-byte units
     for (int i = 0; i < b.n_groups; ++i)
         if (b.g[i].N > NT_MAX) nt_cap = 128;
     for (int i = 0; i < b.n_groups; ++i) {
@@ -619,7 +587,7 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
         // ... plus a fixed 3000 per tile for the pipeline fill / accumulator hand-over (swept 0..20000 on the 98k water box with the
         // eight-warp epilogue: the six GEMMs take 0.323 ms at 1000, 0.314 at 3000, 0.313 at 4000, 0.329 at 8000; the layers
         // move in steps of ~4 us as the slowest CTA gains or loses a tile, which a dynamic tile queue would even out)
-        tb.tile_cost[i] = g.K / BLOCK_K * (TILE_M + 2 * NT) + ((epi == EPI_DCELU || epi == EPI_ACCUM) ? 8 : 4) * NT + env_fixed;
+        tb.tile_cost[i] = g.K / BLOCK_K * (TILE_M + 2 * NT) + ((epi == EPI_DCELU || epi == EPI_ACCUM) ? 8 : 4) * NT + tile_fixed;
         tb.cost_total += (long long)tb.tile_cost[i] * (tiles - tb.tile_off[i]);
     }
     tb.n_groups = b.n_groups;
@@ -633,13 +601,6 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     tb.acc_stride = nt_max <= 128 ? 128 : 192;
     tb.a_slots = (TMEM_COLS - 2 * tb.acc_stride) / 64;
     if (tb.a_slots > tb.stages) tb.a_slots = tb.stages;
-#ifdef NNP_TC_TRACE
-    static long long *d_trace = nullptr;
-    static int traced = 0;
-    if (!d_trace) { cudaMalloc(&d_trace, 256 * 8 * 8); }
-    tb.trace = (traced < 6) ? d_trace : nullptr;
-    if (tb.trace) cudaMemsetAsync(d_trace, 0, 256 * 8 * 8, c->stream);
-#endif
     const bool s3 = split3 != 0;
     switch (epi) {
     case EPI_CELU: launch<EPI_CELU>(c->stream, tb, tiles, s3); break;
@@ -651,19 +612,5 @@ int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3)
     default: c->err = "bad epilogue"; return NNP_EINVAL;
     }
     c->launches += 1;
-#ifdef NNP_TC_TRACE
-    if (tb.trace) {
-        static long long h[256 * 8];
-        cudaStreamSynchronize(c->stream);
-        cudaMemcpy(h, d_trace, sizeof(h), cudaMemcpyDeviceToHost);
-        fprintf(stderr, "TRACE launch %d epi %d tiles %d (cycles rel. to first TMA issue): it | P0 tma-issue | C1 full-seen | C2 aready | M3 pre-wait | M4 aready | M5 committed | M6 acc-free | E7 epi-done\n", traced, epi, tiles);
-        for (int it = 0; it < 40; ++it) {
-            if (!h[it * 8]) break;
-            fprintf(stderr, "  %3d | %7lld | %7lld | %7lld | %7lld | %7lld | %7lld | %7lld | %7lld\n", it, h[it * 8] - h[0], h[it * 8 + 1] - h[0], h[it * 8 + 2] - h[0],
-                    h[it * 8 + 3] - h[0], h[it * 8 + 4] - h[0], h[it * 8 + 5] - h[0], h[it * 8 + 6] ? h[it * 8 + 6] - h[0] : 0, h[it * 8 + 7] ? h[it * 8 + 7] - h[0] : 0);
-        }
-        ++traced;
-    }
-#endif
     return NNP_OK;
 }

@@ -77,6 +77,13 @@ __global__ void k_init_system(int n, const int *__restrict__ species, const floa
                               int *__restrict__ mol, int *__restrict__ counts, int S, int *__restrict__ bad)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (mol_offsets) { // offsets[0] = 0 <= offsets[1] <= ... <= offsets[n_mols] = n, checked by a grid-stride loop
+        for (int m = i; m <= n_mols; m += gridDim.x * blockDim.x) {
+            const int o = mol_offsets[m];
+            const bool ok = m == 0 ? o == 0 : (o >= mol_offsets[m - 1] && (m < n_mols || o == n));
+            if (!ok) atomicOr(bad, 2);
+        }
+    }
     if (i >= n) return;
     int s = species[i];
     if (s < 0 || s >= S) { atomicOr(bad, 1); s = 0; }
@@ -153,11 +160,26 @@ __global__ void k_set_rebuild_cond(cudaGraphConditionalHandle h, const int *__re
     cudaGraphSetConditional(h, *flag != 0 ? 1u : 0u);
 }
 
+// Every device buffer of the library comes from here: the caller's allocator (nnp_params.alloc, e.g. PyTorch's caching
+// allocator) or cudaMalloc.
 template <typename Tp>
 int dev_alloc(nnp_ctx *c, Tp **p, size_t count)
 {
-    CU(c, cudaMalloc((void **)p, sizeof(Tp) * (count ? count : 1)));
+    const size_t bytes = sizeof(Tp) * (count ? count : 1);
+    if (c->alloc_fn) {
+        *p = (Tp *)c->alloc_fn(bytes, c->alloc_user);
+        if (!*p) NNP_FAIL(c, NNP_ENOMEM, "nnp_params.alloc(%zu bytes) returned NULL", bytes);
+        if ((uintptr_t)*p & 255u) NNP_FAIL(c, NNP_EINVAL, "nnp_params.alloc returned a pointer that is not 256-byte aligned");
+        return NNP_OK;
+    }
+    CU(c, cudaMalloc((void **)p, bytes));
     return NNP_OK;
+}
+void dev_free(nnp_ctx *c, void *p)
+{
+    if (!p) return;
+    if (c->dealloc_fn) c->dealloc_fn(p, c->alloc_user);
+    else cudaFree(p);
 }
 
 LayerW &layer(nnp_ctx *c, int net, int s, int l) { return c->layers[((size_t)net * c->S + s) * NNP_NLAYERS + l]; }
@@ -191,7 +213,7 @@ int set_layout(nnp_ctx *c, unsigned mask)
     CU(c, cudaMemcpyAsync(c->d_fmap, fmap.data(), sizeof(int) * c->kpad_full, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream)); // fmap is a stack-lifetime host buffer
     float *base = c->d_l1c_blob;
-    const int narr = c->mm_mode ? 6 : 2;
+    const int narr = c->tc_mode ? 6 : 2;
     for (int net = 0; net < c->n_nets; ++net)
         for (int s = 0; s < S; ++s) {
             const int out = c->widths[s][1];
@@ -199,7 +221,7 @@ int set_layout(nnp_ctx *c, unsigned mask)
             Layer1C &L = l1c(c, net, s);
             L.W = base; L.Wt = base + cnt;
             L.W_hi = L.W_lo = L.Wt_hi = L.Wt_lo = nullptr;
-            if (c->mm_mode) { L.W_hi = base + 2 * cnt; L.W_lo = base + 3 * cnt; L.Wt_hi = base + 4 * cnt; L.Wt_lo = base + 5 * cnt; }
+            if (c->tc_mode) { L.W_hi = base + 2 * cnt; L.W_lo = base + 3 * cnt; L.Wt_hi = base + 4 * cnt; L.Wt_lo = base + 5 * cnt; }
             base += (size_t)narr * c->kpad_full * out;
             k_gather_l1<<<nnp_div_up((int)cnt, T), T, 0, c->stream>>>(a.kpad, out, c->d_fmap, layer(c, net, s, 0).W, L.W, L.Wt,
                                                                       L.W_hi, L.W_lo, L.Wt_hi, L.Wt_lo);
@@ -351,7 +373,7 @@ void make_batch(nnp_ctx *c, int net0, int n_batch, int op, GemmBatch &b)
 
 int run_gemm(nnp_ctx *c, const GemmBatch &b, int epi)
 {
-    if (c->mm_mode == NNP_MM_FP32_SIMT) { nnp_launch_gemm_simt(c, b, epi); return NNP_OK; }
+    if (!c->tc_mode) { nnp_launch_gemm_simt(c, b, epi, c->mm_mode == NNP_MM_FP64_SIMT); return NNP_OK; }
     return nnp_launch_gemm_tc(c, b, epi, c->mm_mode == NNP_MM_3XTF32_TC);
 }
 
@@ -366,7 +388,7 @@ int run_forces(nnp_ctx *c)
     GemmBatch b;
     // networks per grouped launch (tensor-core modes): as many as the group table holds
     const int np = c->aev.np > 0 ? c->aev.np : 1;
-    int nb = (c->mm_mode == NNP_MM_FP32_SIMT || c->n_nets == 1) ? 1 : NNP_MAX_GROUPS / np;
+    int nb = (!c->tc_mode || c->n_nets == 1) ? 1 : NNP_MAX_GROUPS / np;
     if (nb < 1) nb = 1;
     if (nb > c->n_nets) nb = c->n_nets;
     for (int net0 = 0; net0 < c->n_nets; net0 += nb)
@@ -434,8 +456,9 @@ int setup_grid(nnp_ctx *c, float skin)
     }
     const int nk = c->S * g.ncell + 1;
     if (nk > c->nkeys_cap) {
-        if (c->cell_start) cudaFree(c->cell_start);
-        if (c->cursor) cudaFree(c->cursor);
+        CU(c, cudaStreamSynchronize(c->stream)); // earlier builds may still read the old arrays
+        dev_free(c, c->cell_start);
+        dev_free(c, c->cursor);
         c->cell_start = c->cursor = nullptr;
         c->nkeys_cap = 0;
         int rc;
@@ -538,7 +561,7 @@ void nnp_destroy(nnp_ctx *c)
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags, c->aev_sched,
                     c->io_xyz, c->io_vel, c->io_species, c->d_res};
-    for (void *p : ptrs) if (p) cudaFree(p);
+    for (void *p : ptrs) dev_free(c, p);
     if (c->h_res) cudaFreeHost(c->h_res);
     for (auto &m : c->prof_marks) cudaEventDestroy(m.first);
     for (auto &e : c->prof_pool) cudaEventDestroy(e);
@@ -559,7 +582,8 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
         NNP_FAIL(none, NNP_EINVAL, "null parameter array");
     if (max_atoms < 1 || max_mols < 1 || p->n_nets < 1) NNP_FAIL(none, NNP_EINVAL, "max_atoms, max_mols, n_nets must be >= 1");
     if (!(p->rcr > 0.f) || !(p->rca > 0.f) || p->rca > p->rcr) NNP_FAIL(none, NNP_EINVAL, "need 0 < rca <= rcr");
-    if (p->mm_mode < 0 || p->mm_mode > 2) NNP_FAIL(none, NNP_EINVAL, "bad mm_mode");
+    if (p->mm_mode < 0 || p->mm_mode > 3) NNP_FAIL(none, NNP_EINVAL, "bad mm_mode");
+    if ((p->alloc == nullptr) != (p->dealloc == nullptr)) NNP_FAIL(none, NNP_EINVAL, "alloc and dealloc must be given together");
     const int S = p->n_species;
     const int aev_len = S * NNP_NSHF_R + S * (S + 1) / 2 * NNP_ANG_BLOCK;
     for (int s = 0; s < S; ++s) {
@@ -575,9 +599,10 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     if (cudaSetDevice(device) != cudaSuccess) NNP_FAIL(none, NNP_ECUDA, "cudaSetDevice(%d) failed", device);
     nnp_ctx *c = new nnp_ctx();
     // new T() value-initialises: every POD member starts at zero
-    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode; c->dense_aev = p->dense_aev != 0;
+    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode; c->tc_mode = p->mm_mode == NNP_MM_3XTF32_TC || p->mm_mode == NNP_MM_TF32_TC; c->dense_aev = p->dense_aev != 0;
     c->alpha = p->celu_alpha; c->accel_conv = p->accel_conv;
     c->stream = (cudaStream_t)cuda_stream; c->device = device;
+    c->alloc_fn = p->alloc; c->dealloc_fn = p->dealloc; c->alloc_user = p->alloc_user;
     { // the legacy / per-thread default streams cannot be captured: steps are then enqueued kernel by kernel
         const char *e = getenv("NNP_NO_GRAPH");
         c->no_graph = (e && e[0] == '1') || c->stream == nullptr || c->stream == cudaStreamLegacy || c->stream == cudaStreamPerThread;
@@ -614,14 +639,14 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     c->layers = new LayerW[(size_t)c->n_nets * S * NNP_NLAYERS];
     c->l1c = new Layer1C[(size_t)c->n_nets * S]();
     size_t total = 0, total_l1c = 0;
-    for (int s = 0; s < S; ++s) total_l1c += (size_t)c->n_nets * (c->mm_mode ? 6 : 2) * a.kpad * c->widths[s][1];
+    for (int s = 0; s < S; ++s) total_l1c += (size_t)c->n_nets * (c->tc_mode ? 6 : 2) * a.kpad * c->widths[s][1];
     for (int net = 0; net < c->n_nets; ++net)
         for (int s = 0; s < S; ++s)
             for (int l = 0; l < NNP_NLAYERS; ++l) {
                 LayerW &L = layer(c, net, s, l);
                 L.in = c->widths[s][l]; L.out = c->widths[s][l + 1];
                 L.in_pad = l == 0 ? a.kpad : L.in;
-                total += (c->mm_mode ? 6 : 2) * (size_t)L.in_pad * L.out + (size_t)((L.out + 3) / 4 * 4);
+                total += (c->tc_mode ? 6 : 2) * (size_t)L.in_pad * L.out + (size_t)((L.out + 3) / 4 * 4);
             }
     std::vector<float> blob(total, 0.f);
     std::vector<double> shift(S, 0.0);
@@ -646,7 +671,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
                     src += L.out;
                     if (l == NNP_NLAYERS - 1) shift[s] += (double)b[0] / c->n_nets;
                     L.W = (float *)(W - blob.data()); L.Wt = (float *)(Wt - blob.data()); L.b = (float *)(b - blob.data());
-                    if (c->mm_mode) { // tf32 hi / lo splits of both orientations (same rounding as the kernel's A split)
+                    if (c->tc_mode) { // tf32 hi / lo splits of both orientations (same rounding as the kernel's A split)
                         const size_t cnt = (size_t)L.in_pad * L.out;
                         float *dst[4] = {&blob[o], &blob[o + cnt], &blob[o + 2 * cnt], &blob[o + 3 * cnt]};
                         o += 4 * cnt;
@@ -683,7 +708,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     for (size_t q = 0; q < (size_t)c->n_nets * S * NNP_NLAYERS; ++q) { // offsets -> device pointers
         LayerW &L = c->layers[q];
         L.W = c->d_params_blob + (size_t)L.W; L.Wt = c->d_params_blob + (size_t)L.Wt; L.b = c->d_params_blob + (size_t)L.b;
-        if (c->mm_mode) {
+        if (c->tc_mode) {
             L.W_hi = c->d_params_blob + (size_t)L.W_hi; L.W_lo = c->d_params_blob + (size_t)L.W_lo;
             L.Wt_hi = c->d_params_blob + (size_t)L.Wt_hi; L.Wt_lo = c->d_params_blob + (size_t)L.Wt_lo;
         }
@@ -768,7 +793,11 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
         CU(c, cudaMemcpyAsync(h_counts, bins, sizeof(int) * NNP_MAX_SPECIES, cudaMemcpyDeviceToHost, c->stream));
         CU(c, cudaMemcpyAsync(&bad, c->flags + 3, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
         CU(c, cudaStreamSynchronize(c->stream));
-        if (bad) { c->have_system = 0; NNP_FAIL(c, NNP_EINVAL, "species index outside [0, n_species)"); }
+        if (bad) {
+            c->have_system = 0;
+            NNP_FAIL(c, NNP_EINVAL, (bad & 1) ? "species index outside [0, n_species)"
+                                              : "mol_offsets must be 0 = o[0] <= o[1] <= ... <= o[n_mols] = n_atoms");
+        }
     }
     c->bucket_off[0] = 0;
     for (int s = 0; s < NNP_MAX_SPECIES; ++s) c->bucket_off[s + 1] = c->bucket_off[s] + (s < c->S ? h_counts[s] : 0);
@@ -795,6 +824,9 @@ int nnp_build_neighbors(nnp_ctx *c, float skin)
     if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "nnp_set_system first");
     if (!(skin >= 0.f)) NNP_FAIL(c, NNP_EINVAL, "skin must be >= 0");
     CU(c, cudaSetDevice(c->device));
+    // A captured MD-step graph has the skin, the grid and the key-array pointers baked into its kernel arguments:
+    // it is re-captured by the next nnp_md_step.
+    drop_md_graph(c);
     c->skin = skin;
     int rc = setup_grid(c, skin);
     if (rc) return rc;

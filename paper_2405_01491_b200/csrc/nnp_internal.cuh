@@ -132,6 +132,7 @@ struct Layer1C {
 struct nnp_ctx {
     // model
     int S, n_nets, mm_mode, dense_aev;
+    int tc_mode;                    // mm_mode is one of the tcgen05 modes (weights carry tf32 hi / lo splits)
     int aev_len_full, kpad_full;    // 1008 / 1024 for 7 species
     unsigned present_mask;          // species mask the compact layer-1 copies were built for (0: none yet)
     Layer1C *l1c;                   // host array [n_nets][S]
@@ -151,6 +152,10 @@ struct nnp_ctx {
     float *d_e_shift;               // [S]
 
     cudaStream_t stream;
+    // device-memory hooks of nnp_params (nullptr: cudaMalloc / cudaFree)
+    void *(*alloc_fn)(size_t, void *);
+    void (*dealloc_fn)(void *, void *);
+    void *alloc_user;
     int device, max_atoms, max_mols;
     int64_t launches;
     std::string err;
@@ -218,7 +223,7 @@ void nnp_launch_aev_forward(nnp_ctx *c);
 void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets, double *d_virial /* [6] or nullptr */);
 void nnp_aev_tri_table(uint16_t *h_tri /* [NNP_TRI_LEN] */);
 // mlp_simt.cu / mlp_tc.cu
-void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi);
+void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi, int fp64_acc);
 int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3);
 // integrate.cu
 void nnp_launch_kick_drift(nnp_ctx *c);

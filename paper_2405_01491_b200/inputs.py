@@ -256,6 +256,19 @@ def molecule_batch(n_mols=8192, nmin=8, nmax=30, seed=SEED0 + 5):
     return species, xyz.astype(np.float32).astype(np.float64), offs
 
 
+def dense_box(density, L=12.0, dmin=1.2, seed=SEED0 + 6, n_species=7):
+    """Compressed mixed-species periodic box (not a workload of the paper: a stress case for the neighbour capacities):
+    `density` atoms / A^3 by random sequential addition with separation >= dmin, species iid uniform.
+    density 0.25 => ~45 neighbours inside 3.5 A and ~139 inside 5.1 A per atom (water: 18 / 56)."""
+    rng = np.random.default_rng(seed)
+    n = int(round(density * L ** 3))
+    xyz = _rsa_points(rng, n, L, dmin).astype(np.float32).astype(np.float64)
+    species = rng.integers(0, n_species, size=n).astype(np.int32)
+    species[:n_species] = np.arange(n_species)
+    L = float(np.float32(L))
+    return species, xyz, np.array([L, L, L])
+
+
 def replicate(species, xyz, box, k):
     """k x k x k periodic images of a box (extensivity pin)."""
     sh = np.array([[a, b, c] for a in range(k) for b in range(k) for c in range(k)], dtype=np.float64) * box

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
 
 NNP_OK, NNP_EINVAL, NNP_ENOMEM, NNP_ECUDA, NNP_ECAPACITY, NNP_ESTALE, NNP_EBOX = 0, -1, -2, -3, -4, -5, -6
-NNP_MM_FP32_SIMT, NNP_MM_3XTF32_TC, NNP_MM_TF32_TC = 0, 1, 2
+NNP_MM_FP32_SIMT, NNP_MM_3XTF32_TC, NNP_MM_TF32_TC, NNP_MM_FP64_SIMT = 0, 1, 2, 3
 STATUS_NAMES = {0: "NNP_OK", -1: "NNP_EINVAL", -2: "NNP_ENOMEM", -3: "NNP_ECUDA", -4: "NNP_ECAPACITY",
                 -5: "NNP_ESTALE", -6: "NNP_EBOX"}
 
@@ -32,6 +32,10 @@ class NnpError(RuntimeError):
         self.status = status
 
 
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)      # void *(*alloc)(size_t bytes, void *user)
+DEALLOC_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)          # void (*dealloc)(void *ptr, void *user)
+
+
 class nnp_params(C.Structure):
     _fields_ = [
         ("n_species", C.c_int), ("rcr", C.c_float), ("rca", C.c_float),
@@ -43,6 +47,7 @@ class nnp_params(C.Structure):
         ("self_energy", C.POINTER(C.c_float)), ("mass", C.POINTER(C.c_float)),
         ("accel_conv", C.c_float), ("mm_mode", C.c_int), ("cap_r", C.c_int), ("cap_a", C.c_int),
         ("dense_aev", C.c_int),
+        ("alloc", ALLOC_FN), ("dealloc", DEALLOC_FN), ("alloc_user", C.c_void_p),
     ]
 
 
@@ -107,8 +112,9 @@ def _check(ctx, rc):
 
 
 def make_params(consts, widths, params, mass, accel_conv, n_nets=1, self_energy=None, mm_mode=NNP_MM_FP32_SIMT,
-                cap_r=0, cap_a=0, dense_aev=0):
-    """Fills an nnp_params from numpy arrays; returns (struct, keepalive list)."""
+                cap_r=0, cap_a=0, dense_aev=0, alloc=None, dealloc=None):
+    """Fills an nnp_params from numpy arrays; returns (struct, keepalive list).  alloc / dealloc: Python callables
+    (bytes, user) -> device pointer and (ptr, user) -> None, passed to the library as its device-memory hooks."""
     f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
     keep = dict(shf_r=f32(consts["shf_r"]), shf_a=f32(consts["shf_a"]), shf_z=f32(consts["shf_z"]),
                 widths=np.ascontiguousarray(widths, dtype=np.int32), params=f32(params), mass=f32(mass),
@@ -129,6 +135,9 @@ def make_params(consts, widths, params, mass, accel_conv, n_nets=1, self_energy=
     p.mass = fp(keep["mass"])
     p.accel_conv, p.mm_mode, p.cap_r, p.cap_a = float(accel_conv), int(mm_mode), int(cap_r), int(cap_a)
     p.dense_aev = int(dense_aev)
+    if alloc is not None:
+        keep["alloc"], keep["dealloc"] = ALLOC_FN(alloc), DEALLOC_FN(dealloc)   # the thunks must outlive the context
+        p.alloc, p.dealloc = keep["alloc"], keep["dealloc"]
     return p, keep
 
 

@@ -40,6 +40,10 @@ def test_params_struct_matches_header_field_order():
         decl = decl.strip()
         if not decl:
             continue
+        fptr = re.search(r"\(\s*\*\s*([A-Za-z_0-9]+)\s*\)\s*\(", decl)     # function pointer: ret (*name)(args)
+        if fptr:
+            fields.append(fptr.group(1))
+            continue
         for part in decl.split(","):
             fields.append(re.findall(r"[A-Za-z_0-9]+", part)[-1])
     assert fields == [f[0] for f in nnp.nnp_params._fields_]
