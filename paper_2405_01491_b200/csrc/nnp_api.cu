@@ -391,29 +391,41 @@ int run_forces(nnp_ctx *c)
     int nb = (!c->tc_mode || c->n_nets == 1) ? 1 : NNP_MAX_GROUPS / np;
     if (nb < 1) nb = 1;
     if (nb > c->n_nets) nb = c->n_nets;
-    for (int net0 = 0; net0 < c->n_nets; net0 += nb)
-        for (int op = 0; op < 5; ++op) {
-            make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, op, b);
-            int rc = run_gemm(c, b, epi_of[op]);
-            if (rc != NNP_OK) return rc;
-            nnp_prof_mark(c, 3 + op);
-        }
-    if (nb > 1) {
-        // dE/dG sums over the networks: the groups of all batched networks add into the same rows with vector
-        // reductions in memory (the summation order over the networks is then not fixed, like the force scatter's)
-        CU(c, cudaMemsetAsync(c->dG, 0, sizeof(float) * (size_t)c->n * c->aev.kpad, c->stream));
-        for (int net0 = 0; net0 < c->n_nets; net0 += nb) {
-            make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, 5, b);
-            int rc = run_gemm(c, b, EPI_RED);
-            if (rc != NNP_OK) return rc;
-            nnp_prof_mark(c, 8);
-        }
+    // fused chain (mlp_fused.cu): 1 = all six GEMMs in one launch, 2 = the four middle ones (layer 1 / dE/dG stay launches)
+    const int fk = nnp_fused_kind(c);
+    if (fk == 1) {
+        if (c->n_nets > 1) CU(c, cudaMemsetAsync(c->dG, 0, sizeof(float) * (size_t)c->n * c->aev.kpad, c->stream));
+        nnp_launch_mlp_fused(c);
+        nnp_prof_mark(c, 3);
     } else {
-        for (int net = 0; net < c->n_nets; ++net) { // one network per launch, accumulated in place in network order
-            make_batch(c, net, 1, 5, b);
-            int rc = run_gemm(c, b, net > 0 ? EPI_ACCUM : EPI_STORE);
-            if (rc != NNP_OK) return rc;
-            nnp_prof_mark(c, 8);
+        for (int net0 = 0; net0 < c->n_nets; net0 += nb)
+            for (int op = 0; op < (fk == 2 ? 1 : 5); ++op) {
+                make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, op, b);
+                int rc = run_gemm(c, b, epi_of[op]);
+                if (rc != NNP_OK) return rc;
+                nnp_prof_mark(c, 3 + op);
+            }
+        if (fk == 2) {
+            nnp_launch_mlp_fused(c);
+            nnp_prof_mark(c, 4);
+        }
+        if (nb > 1) {
+            // dE/dG sums over the networks: the groups of all batched networks add into the same rows with vector
+            // reductions in memory (the summation order over the networks is then not fixed, like the force scatter's)
+            CU(c, cudaMemsetAsync(c->dG, 0, sizeof(float) * (size_t)c->n * c->aev.kpad, c->stream));
+            for (int net0 = 0; net0 < c->n_nets; net0 += nb) {
+                make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, 5, b);
+                int rc = run_gemm(c, b, EPI_RED);
+                if (rc != NNP_OK) return rc;
+                nnp_prof_mark(c, 8);
+            }
+        } else {
+            for (int net = 0; net < c->n_nets; ++net) { // one network per launch, accumulated in place in network order
+                make_batch(c, net, 1, 5, b);
+                int rc = run_gemm(c, b, net > 0 ? EPI_ACCUM : EPI_STORE);
+                if (rc != NNP_OK) return rc;
+                nnp_prof_mark(c, 8);
+            }
         }
     }
     nnp_launch_energy_reduce(c);
@@ -555,6 +567,7 @@ void nnp_destroy(nnp_ctx *c)
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     drop_md_graph(c);
+    nnp_fused_destroy(c);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     void *ptrs[] = {c->d_params_blob, c->d_l1c_blob, c->d_fmap, c->d_tri, c->d_inv_mass_conv, c->d_mass, c->d_e_shift, c->d_lgv_c2, c->d_virial, c->pos, c->pos_tmp, c->vel, c->vel_tmp,
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
@@ -606,6 +619,8 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     { // the legacy / per-thread default streams cannot be captured: steps are then enqueued kernel by kernel
         const char *e = getenv("NNP_NO_GRAPH");
         c->no_graph = (e && e[0] == '1') || c->stream == nullptr || c->stream == cudaStreamLegacy || c->stream == cudaStreamPerThread;
+        const char *f = getenv("NNP_NO_FUSED");
+        c->no_fused = f && f[0] == '1';
     }
     c->max_atoms = max_atoms; c->max_mols = max_mols;
     c->hmax[0] = c->hmax[1] = c->hmax[2] = 0;
@@ -805,7 +820,9 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
     for (int s = 0; s < c->S; ++s)
         if (h_counts[s] > 0) mask |= 1u << s;
     if (c->dense_aev || mask == 0) mask = (1u << c->S) - 1u;
-    return set_layout(c, mask);
+    int rc = set_layout(c, mask);
+    if (rc) return rc;
+    return nnp_fused_setup(c);
 }
 
 int nnp_set_positions(nnp_ctx *c, const float *d_xyz)

@@ -129,6 +129,8 @@ struct Layer1C {
     float *W, *Wt, *W_hi, *W_lo, *Wt_hi, *Wt_lo; // [kpad][out] / [out][kpad]
 };
 
+struct nnp_fused; // mlp_fused.cu: packed weight tiles, group table and tile ranges of the fused MLP kernel
+
 struct nnp_ctx {
     // model
     int S, n_nets, mm_mode, dense_aev;
@@ -213,6 +215,8 @@ struct nnp_ctx {
     cudaStream_t aux_stream;     // capture stream of the conditional body
     int64_t md_graph_launches;   // kernels per graph launch outside the conditional body
     int no_graph;                // NNP_NO_GRAPH=1: enqueue every step kernel by kernel
+    nnp_fused *fused;            // fused MLP chain (tensor-core modes), set up per loaded system
+    int no_fused;                // NNP_NO_FUSED=1: always the six-launch path
 };
 
 // ---- launches implemented across the .cu files --------------------------------------------------
@@ -225,6 +229,11 @@ void nnp_aev_tri_table(uint16_t *h_tri /* [NNP_TRI_LEN] */);
 // mlp_simt.cu / mlp_tc.cu
 void nnp_launch_gemm_simt(nnp_ctx *c, const GemmBatch &b, int epi, int fp64_acc);
 int nnp_launch_gemm_tc(nnp_ctx *c, const GemmBatch &b, int epi, int split3);
+// mlp_fused.cu
+int nnp_fused_setup(nnp_ctx *c);          // after the layout of a loaded system is known (nnp_set_system)
+int nnp_fused_kind(const nnp_ctx *c);     // 0: six launches, 1: whole chain fused, 2: the four middle GEMMs fused
+void nnp_launch_mlp_fused(nnp_ctx *c);
+void nnp_fused_destroy(nnp_ctx *c);
 // integrate.cu
 void nnp_launch_kick_drift(nnp_ctx *c);
 void nnp_launch_kick_ke(nnp_ctx *c, int count_step); // count_step: also advance the Langevin step counter flags[4]
