@@ -30,6 +30,7 @@ METRIC = "ANI-2x energy+force MD atom-steps/s (0.5 fs velocity Verlet, 98,304-at
 UNIT = "atom-steps/s"
 DT_FS, SKIN, T_KELVIN = 0.5, 0.5, 300.0
 N_WATERS = 32768
+MM_NAMES = ["fp32_simt", "3xtf32_tcgen05", "tf32_tcgen05", "fp64_simt", "3xf16_tcgen05_fused"]
 TRAJ_MAX = 1050   # longest stretch of one trajectory (steps): BASELINE.json's 1000-step run + the default warm-up
 BOX_L = 99.4
 
@@ -235,8 +236,8 @@ def run_eval_config(args):
         macs = sum(int(counts[s]) * (kpad * int(Wd[s, 1]) + int(Wd[s, 1]) * int(Wd[s, 2]) + int(Wd[s, 2]) * int(Wd[s, 3]) + int(Wd[s, 3]))
                    for s in range(7))
         ach = 2.0 * 2.0 * macs * n_nets / (mlp_ms * 1e-3) / 1e12           # forward + input gradient
-        peak = pk["bf16_sus"] * 0.5 if args.mm_mode in (1, 2) else fp32_peak
-        roof = {"kernel": "mlp_all_layers (6 grouped GEMM launches per network batch)", "bound": "tensor" if args.mm_mode in (1, 2) else "alu",
+        peak = pk["bf16_sus"] * 0.5 if args.mm_mode in (1, 2, 4) else fp32_peak
+        roof = {"kernel": "mlp_all_layers (6 grouped GEMM launches per network batch)", "bound": "tensor" if args.mm_mode in (1, 2, 4) else "alu",
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
                 "peak_source": "%s sustained bf16 cuBLAS x 0.5; fp32-equivalent flops counted once" % pk["source"]}
     elif dom in ("aev_forward", "aev_backward_scatter"):
@@ -258,7 +259,7 @@ def run_eval_config(args):
             "value": n * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": name, "atoms": n, "structures": n_mols, "n_nets": n_nets, "aev_active_columns": kact,
-                       "mm_mode": ["fp32_simt", "3xtf32_tcgen05", "tf32_tcgen05", "fp64_simt"][args.mm_mode],
+                       "mm_mode": MM_NAMES[args.mm_mode],
                        "us_per_evaluation": 1e3 * ms / K, "force_scale": args.force_scale,
                        "radial_terms": n_rad, "triplets": n_tri,
                        "launch_path": "kernel_by_kernel (nnp_build_neighbors + nnp_energy_forces per step)",
@@ -469,7 +470,7 @@ def run_ours(args):
         "config": {"workload": "water_%d_md (BASELINE configs[2])" % n if args.waters == N_WATERS else "water_%d_md" % n,
                    "atoms": n, "box_A": float(box[0]), "dt_fs": DT_FS, "skin_A": SKIN, "n_nets": 1,
                    "integrator": "langevin_baoab gamma=%g/fs" % args.langevin if args.langevin > 0 else "velocity_verlet",
-                   "mm_mode": ["fp32_simt", "3xtf32_tcgen05", "tf32_tcgen05"][args.mm_mode],
+                   "mm_mode": MM_NAMES[args.mm_mode],
                    "force_scale": args.force_scale, "ns_per_day": steps_per_s * DT_FS * 1e-6 * 86400,
                    "rebuilds_in_timed_region": n_rebuilds, "trajectory_restarts_in_timed_region": n_restarts,
                    "temperature_K_end": 2 * ek_end / (3 * n * inputs.KB), "temperature_K_start": 2 * ek_start / (3 * n * inputs.KB),

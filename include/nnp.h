@@ -48,14 +48,19 @@ typedef enum {
     NNP_ECUDA = -3,     /* CUDA runtime error (message in nnp_last_error) */
     NNP_ECAPACITY = -4, /* a neighbour row exceeded cap_r / cap_a: recreate with larger caps */
     NNP_ESTALE = -5,    /* energy/forces or MD requested without a neighbour list for the current system */
-    NNP_EBOX = -6       /* periodic box edge < 2*(cutoff+skin): minimum image not unique (reading C1) */
+    NNP_EBOX = -6,      /* periodic box edge < 2*(cutoff+skin): minimum image not unique (reading C1) */
+    NNP_ERANGE = -7     /* mm_mode 4: an activation left the range of the scaled fp16 split (|value| > 3750): the result
+                           of this evaluation is invalid; use mm_mode 1 for such a model */
 } nnp_status;
 
 /* How the MLP contractions are computed (Fig. 3: matmul precision decides energy conservation):
  * 0 fp32 FMA on the CUDA cores; 1 (default of the tests and the bench) 3xTF32 on tcgen05, fp32-grade; 2 plain TF32 on
  * tcgen05 (fails the parity bars, kept for the precision study); 3 fp32 operands with every product and sum in fp64
- * (DFMA on the CUDA cores) -- the fp64 leg of the precision study, slow. */
-enum { NNP_MM_FP32_SIMT = 0, NNP_MM_3XTF32_TC = 1, NNP_MM_TF32_TC = 2, NNP_MM_FP64_SIMT = 3 };
+ * (DFMA on the CUDA cores) -- the fp64 leg of the precision study, slow; 4 "3xF16": the hidden layers (and, when the
+ * system's active AEV columns are <= 256, all six GEMMs) as ONE fused tcgen05 kernel with every fp32 operand split into
+ * fp16 hi + fp16 lo (11 + 11 significant bits as in mode 1, power-of-two scaling against fp16's exponent range, fp32
+ * accumulation), fp32-grade; GEMMs outside the fused chain run as in mode 1.  Out-of-range activations -> NNP_ERANGE. */
+enum { NNP_MM_FP32_SIMT = 0, NNP_MM_3XTF32_TC = 1, NNP_MM_TF32_TC = 2, NNP_MM_FP64_SIMT = 3, NNP_MM_3XF16_TC = 4 };
 
 typedef struct {
     int n_species;            /* <= 7; ANI-2x: 7, index order H,C,N,O,S,F,Cl (reading B2) */

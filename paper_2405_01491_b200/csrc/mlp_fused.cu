@@ -1,34 +1,41 @@
-// Stage 3 + the MLP half of stage 4 as ONE persistent kernel (tensor-core modes): a CTA owns a 128-atom row tile and
-// takes it through the whole chain  G -> h1 -> h2 -> h3 (-> e_i, delta3) -> delta2 -> delta1 -> dE/dG  without leaving
-// the SM (ChemicalNet; forces by reverse mode, L65 / L176; the model of Fig. 2 is one fused executable,
-// L176).  SURVEY.md 8(f)-4 / 8(d) "intermediates": the unfused path (mlp_tc.cu, six launches) writes and re-reads every
-// activation through HBM (~0.8 GB per step on the 98k water box) and pays six launch / pipeline-fill costs.
+// Stage 3 + the MLP half of stage 4 as ONE persistent kernel (mm_mode NNP_MM_3XF16_TC): a CTA owns a 128-atom row tile
+// and takes it through the whole chain  G -> h1 -> h2 -> h3 (-> e_i, delta3) -> delta2 -> delta1 -> dE/dG  without
+// leaving the SM (ChemicalNet; forces by reverse mode, L65 / L176; the model of Fig. 2 is one fused
+// executable, L176).  SURVEY.md 8(f)-4 / 8(d) "intermediates": the unfused path (mlp_tc.cu, six launches) writes and
+// re-reads every activation through HBM (~0.8 GB per step on the 98k water box) and pays six launch / pipeline-fill costs.
 //
-// How a layer feeds the next one.  The accumulator of GEMM j lives in TMEM ([128 atoms] x [N_j columns], fp32).  When its
-// last MMA has completed, the epilogue warps drain it 16 columns at a time: bias + CELU (forward) or x CELU'(h) (reverse),
-// split into tf32 hi / lo, and write the two 128 x 16 blocks back into TMEM as an A-operand "slot" (tcgen05.st).  The MMA
-// thread multiplies each slot with the matching 16 rows of W_{j+1} as soon as it is ready (tcgen05.mma .ts form: A from
-// TMEM, B = weight tile in shared memory), so GEMM j+1 runs while the epilogue of GEMM j is still producing its operand.
-// Nothing but the weights is streamed: they are pre-packed at set-up into the exact 128-byte-swizzled K-major tile images
-// the MMA descriptors expect ([K block of 32][part][hi | lo][rows][32]), so one tile is one contiguous cp.async.bulk of
-// up to 32 KiB into a ring of shared-memory entries - no tensor map per weight matrix.
+// Arithmetic ("3xF16"): every fp32 operand x is split into hi = fp16(x) and lo = fp16(x - hi) (11 + 11 significant bits,
+// the same widths as the tf32 split of mlp_tc.cu) and A.B is accumulated in fp32 by tcgen05.mma kind::f16 as
+// A_lo.B_hi + A_hi.B_lo + A_hi.B_hi.  fp16 has the narrow exponent: weights are scaled per matrix by a power of two so
+// that max |w| lands in [2^13, 2^14), activations by 2^4; both scalings are undone exactly in the epilogue.  A value
+// above 60000 after scaling (|activation| > 3750) raises NNP_FLAG_RANGE -> NNP_ERANGE instead of silently saturating.
+//
+// How a layer feeds the next one - IN PLACE in tensor memory.  TMEM holds two 256-column regions.  The accumulator of
+// GEMM j ([128 atoms] x [N_j], fp32) lives in one of them.  When its last MMA has completed, sixteen epilogue warps drain
+// it 16 columns at a time: bias + CELU (forward) or x CELU'(h) (reverse), split into fp16 hi / lo - and the 16 fp32
+// columns just read are exactly the room their own hi (8 columns of packed pairs) and lo (8 columns) need as the A
+// operand of GEMM j+1, so the chunk is written back where it came from (tcgen05.st) and its mbarrier is armed.  The MMA
+// thread multiplies each chunk with the matching 16 rows of W_{j+1} as soon as it is ready (tcgen05.mma .ts form: A from
+// TMEM, B = weight tile in shared memory) into the OTHER region: no operand ring, no slot recycling, the epilogue never
+// waits for the tensor pipe.  Nothing but the weights is streamed: they are pre-packed at set-up into the exact
+// 128-byte-swizzled K-major fp16 tile images the MMA descriptors expect ([K block of 64][part][hi | lo][rows][64]), one
+// tile = one contiguous cp.async.bulk of up to 32 KiB into a ring of shared-memory entries.
 //   h1 and h2 are needed again by the reverse layers (CELU' = 1 + min(h,0)/alpha).  They do not fit on the SM next to the
-// weight ring (224 KiB per tile), so the forward epilogues also write them to the activation buffers in HBM and the reverse
-// epilogues of the same CTA read them back a few microseconds later (L2 hits; 1.8 KB per atom and direction).
-//
-// TMEM (512 columns): region X = [0, 256) and region Y = [256, 448) hold the accumulators of alternate GEMMs of the chain
-// (a GEMM with N > 128 is issued as two MMAs per K step, N = 128 at the region base and N - 128 at base + 128: both
-// destinations stay 128-column aligned); Z = [448, 512) holds two A slots of 32 columns (hi 16 | lo 16).
+// weight ring, so the forward epilogues also write them to the activation buffers and the reverse epilogues of the same
+// CTA read them back a few microseconds later (L2 hits; 1.8 KB per atom and direction).
 //
 // Chains (chosen per loaded system, nnp_fused_setup):
-//   full   (active AEV columns kpad <= 192, e.g. water: 128):  F1 F2 F3 B3 B2 B1, input G (TMA), output dE/dG
+//   full   (active AEV columns kpad <= 256, e.g. water: 128):  F1 F2 F3 B3 B2 B1, input G (TMA), output dE/dG
 //   middle (any kpad, e.g. 1024 for seven species):            F2 F3 B3 B2, input h1 (TMA), output delta1 in place;
-//          F1 and B1 (K or N = kpad) run as launches of the unfused kernel before / after.
-// Warp roles: 0 producer (TMA A tiles of the first GEMM + bulk weight copies), 1 MMA issue, 2-5 converters (first GEMM's
-// A operand: fp32 tile in shared memory -> tf32 hi / lo slots), 6-13 epilogue (two warps per TMEM lane quarter, alternate
-// 16-column chunks).
+//          F1 and B1 (K or N = kpad) run as 3xTF32 launches of the unfused kernel before / after.
+// Warp roles: 0 producer (TMA tiles of the chain's input + bulk weight copies), 1 MMA issue, 2-17 epilogue (four warps per
+// TMEM lane quarter, every fourth 16-column chunk each); the epilogue warps also convert the chain's input (fp32 tile in
+// shared memory -> fp16 hi / lo chunks in TMEM) at the start of a tile.  576 threads: 112 registers each, no spills - with
+// ~200 KiB of the SM's 228 KiB configured as shared memory, local-memory traffic would go to L2.
 #include <cuda.h>
+#include <cuda_fp16.h>
 
+#include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -42,52 +49,58 @@ namespace {
 #include "tc_ptx.cuh"
 
 constexpr int TILE_M = 128;
-constexpr int KB = 32;                 // K block: fp32 elements of one 128-byte swizzle row
-constexpr int CH = 16;                 // K chunk per A slot
+constexpr int KBH = 64;                // K block of the weight tiles: fp16 elements of one 128-byte swizzle row
+constexpr int KBF = 32;                // K block of the input tiles: fp32 elements of one 128-byte swizzle row
+constexpr int CH = 16;                 // K chunk: one tcgen05.mma kind::f16 K step, 16 accumulator columns
 constexpr int MAX_STAGES = 6;
-constexpr int NW = 5;                  // weight ring entries
+constexpr int NW = 4;                  // weight ring entries
 constexpr int W_ENTRY_BYTES = 32768;   // hi + lo tiles of up to 128 rows x 128 B
-constexpr int NA = 2;                  // ring of first-GEMM A tiles
-constexpr int A_TILE_BYTES = TILE_M * KB * 4;
-constexpr int EPI_WARPS = 8;
+constexpr int NA = 2;                  // ring of input tiles
+constexpr int A_TILE_BYTES = TILE_M * KBF * 4;
+constexpr int EPI_WARPS = 16;
+constexpr int EPI_SETS = EPI_WARPS / 4;
 constexpr int EPI_STG_LD = 20;
 constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;
 constexpr int BAR_BYTES = 512;
 constexpr int SMEM_BYTES = 1024 + NW * W_ENTRY_BYTES + NA * A_TILE_BYTES + BAR_BYTES + EPI_WARPS * EPI_STG_BYTES;
-constexpr int THREADS = 14 * 32;
-constexpr uint32_t COL_X = 0, COL_Y = 256, COL_Z = 448;
+constexpr int THREADS = (2 + EPI_WARPS) * 32;
+constexpr int REGION_COLS = 256;       // two accumulator / operand regions: columns [0, 256) and [256, 512)
+constexpr int MAX_CHUNKS = REGION_COLS / CH;
+constexpr int ACT_SHIFT = 4;           // activations enter the tensor core multiplied by 2^4
+constexpr float ACT_SCALE = 16.0f;
+constexpr float RANGE_LIMIT = 60000.0f;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
+static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 2) + 8 <= BAR_BYTES, "barrier area");
 
 enum FusedEpi {
-    FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> slots
-    FE_OUT = 1,     // h3 = celu(acc + bias); e_atom += h3 . w4; delta3 = w4 celu'(h3): hi/lo -> slots
-    FE_BWD = 2,     // delta = acc * celu'(stash): hi/lo -> slots
+    FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> operand
+    FE_OUT = 1,     // h3 = celu(acc + bias); e_atom += h3 . w4; delta3 = w4 celu'(h3): hi/lo -> operand
+    FE_BWD = 2,     // delta = acc * celu'(stash): hi/lo -> operand
     FE_BWD_ST = 3,  // delta = acc * celu'(out): stored over out (last GEMM of the middle chain)
     FE_ST = 4,      // out = acc
     FE_RED = 5      // out += acc (vector reductions in memory: ensembles add into the same rows)
 };
 
 struct FusedStage {
-    int K, N;            // K: columns of the A operand (multiple of 32); N: output columns (multiple of 32, <= 256 / 192)
+    int K, N;            // K: columns of the A operand (multiple of 32); N: output columns (multiple of 32, <= 256)
     int epi;
-    uint32_t w_off;      // byte offset of the packed weight tiles of this GEMM in the group's blob
-    const float *bias;   // [N] (forward GEMMs)
-    float *stash;        // rows of h: written by FE_FWD, read by FE_BWD (already offset to the group's first row)
+    uint32_t w_off;      // byte offset of the packed weight tiles of this GEMM in the blob
+    const float *bias;   // [N] forward GEMMs: bias * 2^ACT_SHIFT
+    float *stash;        // rows of 16 h: written by FE_FWD, read by FE_BWD (already offset to the group's first row)
     int ld_stash;
-    int pad_;
+    float c_acc;         // forward: acc -> 16 z;  FE_ST / FE_RED: acc -> true value
+    float gs, gc;        // reverse: out = acc * fma(min(h, 0), gs, gc)  (the scalings folded into CELU')
 };
 
 struct alignas(64) FusedGroup {
-    CUtensorMap mapA;    // A operand of the first GEMM: [M][K0] fp32, row pitch of the source buffer
+    CUtensorMap mapA;    // input of the chain: [M][K0] fp32, row pitch of the source buffer
     const uint8_t *wblob;
     const float *w4;
     float *e_atom;
     float *out;          // output rows of the last GEMM
     int ldo;
     int M, n_stages, tile0, n_tiles;
-    int chunks_per_tile; // sum_j K_j / 16
-    int y_first;         // accumulator region of GEMM j: (j & 1) ^ y_first ? Y : X
-    int pad_;
+    int pad_[3];
     FusedStage st[MAX_STAGES];
 };
 
@@ -96,6 +109,40 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
                  "r"(bytes), "r"(bar)
                  : "memory");
+}
+
+// D[tmem] (+)= A[tmem] . B[smem desc]^T, kind::f16 (fp16 operands, fp32 accumulate), A from tensor memory
+__device__ __forceinline__ void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+
+// 16 consecutive K values of one row -> the row's 16 operand columns: hi pairs (k, k+1) in columns 0..7, lo pairs in 8..15
+__device__ __forceinline__ void split16(const float (&x)[16], uint32_t (&v)[16])
+{
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const __half2 h = __floats2half2_rn(x[2 * q], x[2 * q + 1]);
+        const float2 hf = __half22float2(h);
+        const __half2 l = __floats2half2_rn(x[2 * q] - hf.x, x[2 * q + 1] - hf.y);
+        v[q] = *reinterpret_cast<const uint32_t *>(&h);
+        v[8 + q] = *reinterpret_cast<const uint32_t *>(&l);
+    }
 }
 
 __device__ __forceinline__ int find_group(const FusedGroup *__restrict__ groups, int n_groups, int t)
@@ -108,9 +155,144 @@ __device__ __forceinline__ int find_group(const FusedGroup *__restrict__ groups,
 // rows of the two MMAs of a GEMM with N columns: 128 + (N - 128), or N alone
 __device__ __forceinline__ int part_rows(int N, int p) { return p == 0 ? (N > 128 ? 128 : N) : N - 128; }
 
-template <bool SPLIT3>
+struct EpiArgs {
+    const FusedGroup *g;
+    const FusedStage *st;
+    int mrow0, lane, set;
+    uint32_t tm_acc;      // TMEM address of this warp's lane quarter at the accumulator's first column
+    uint32_t stg;         // this warp's staging chunk in shared memory
+    uint32_t bar_accf, accf_parity, bar_ready;
+    float alpha;
+    int site, aux;
+};
+
+// One accumulator through one epilogue warp: the 16-column chunks set, set + 4, ... of the warp's 32 rows.
+template <int EPI>
+__device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float &esum_out)
+{
+    float vmax = 0.f, esum = 0.f;
+    constexpr bool fwd = EPI == FE_FWD || EPI == FE_OUT;
+    constexpr bool rd_prev = EPI == FE_BWD || EPI == FE_BWD_ST;   // reads rows of h for CELU'
+    constexpr bool to_op = EPI == FE_FWD || EPI == FE_OUT || EPI == FE_BWD;
+    constexpr bool wr_rows = EPI == FE_FWD || EPI == FE_BWD_ST || EPI == FE_ST || EPI == FE_RED;
+    const FusedGroup &g = *ea.g;
+    const FusedStage &st = *ea.st;
+    const int N = st.N, M = g.M, mrow0 = ea.mrow0, lane = ea.lane;
+    const uint32_t stg = ea.stg;
+    const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
+    const int sub_r = (lane >> 3) + 4 * ((lane >> 2) & 1), sub_c = (lane & 3) * 4;
+    // rows read (h for CELU') and rows written (h stash, or the chain's output)
+    const float *rd_base = EPI == FE_BWD ? st.stash : g.out;
+    const int rd_ld = EPI == FE_BWD ? st.ld_stash : g.ldo;
+    float *wr_base = EPI == FE_FWD ? st.stash : g.out;
+    const int wr_ld = EPI == FE_FWD ? st.ld_stash : g.ldo;
+    const float c_acc = st.c_acc, gs = st.gs, gc = st.gc;
+    // everything the chunk loop needs sits in registers: the "memory" clobbers of the asm statements below would make the
+    // compiler re-read any field of ea / st / g it still reaches through a pointer, once per chunk
+    const float *bias = st.bias, *w4p = g.w4;
+    const uint32_t tm_acc = ea.tm_acc, bar_ready = ea.bar_ready;
+    const int c_first = ea.set * CH;
+    const float inv_alpha = 1.0f / ea.alpha;
+    const float a16 = ea.alpha * ACT_SCALE;                               // 16 h = max(16 z, 0) + 16 alpha (e - 1)
+    const float ce = 1.4426950408889634f / (ea.alpha * ACT_SCALE);       // e = 2^(min(16 z, 0) ce)
+    float4 pre[4];
+    auto prefetch = [&](int c0) {
+        const float *cb = rd_base + (size_t)mrow0 * rd_ld + c0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int r = i * 8 + sub_r;
+            pre[i] = mrow0 + r < M ? *reinterpret_cast<const float4 *>(cb + (size_t)r * rd_ld + sub_c) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    };
+    if (rd_prev && c_first < N) prefetch(c_first);
+    mbar_wait(ea.bar_accf, ea.accf_parity, ea.site, ea.aux);
+    tc_fence_after();
+    for (int c0 = c_first; c0 < N; c0 += EPI_SETS * CH) {
+        uint32_t a[16];
+        tmem_ld16(tm_acc + (uint32_t)c0, a);
+        if (rd_prev) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int r = i * 8 + sub_r;
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(pre[i].x), "f"(pre[i].y), "f"(pre[i].z), "f"(pre[i].w) : "memory");
+            }
+            __syncwarp();
+            if (c0 + EPI_SETS * CH < N) prefetch(c0 + EPI_SETS * CH);
+        }
+        float ov[16];
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f), w4v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (fwd) x4 = __ldg(reinterpret_cast<const float4 *>(bias + c0) + q);
+            if (EPI == FE_OUT) w4v = __ldg(reinterpret_cast<const float4 *>(w4p + c0) + q);
+            if (rd_prev) asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x4.x), "=f"(x4.y), "=f"(x4.z), "=f"(x4.w) : "r"(my_row + q * 16));
+            const float xq[4] = {x4.x, x4.y, x4.z, x4.w};
+            const float wq[4] = {w4v.x, w4v.y, w4v.z, w4v.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                float v = __uint_as_float(a[4 * q + e]);
+                if (fwd) {
+                    const float z = fmaf(v, c_acc, xq[e]);
+                    float ex;
+                    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(fminf(z, 0.f) * ce));
+                    v = fmaf(a16, ex, fmaxf(z, 0.f) - a16);                // 16 h
+                    if (EPI == FE_OUT) {
+                        esum = fmaf(v, wq[e], esum);
+                        v = wq[e] * fmaf(fminf(v, 0.f), inv_alpha, ACT_SCALE); // 16 w4 celu'(h3)
+                    }
+                } else if (rd_prev) {
+                    v *= fmaf(fminf(xq[e], 0.f), gs, gc);
+                } else {
+                    v *= c_acc;
+                }
+                ov[4 * q + e] = v;
+            }
+        }
+        if (to_op) {
+            uint32_t sl[16];
+#pragma unroll
+            for (int q = 0; q < 16; ++q) vmax = fmaxf(vmax, fabsf(ov[q]));
+            split16(ov, sl);
+            tmem_st16(tm_acc + (uint32_t)c0, sl); // hi / lo of the chunk go back into the accumulator's own columns
+        }
+        if (wr_rows) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + q * 16), "f"(ov[4 * q]), "f"(ov[4 * q + 1]), "f"(ov[4 * q + 2]), "f"(ov[4 * q + 3]) : "memory");
+        }
+        if (to_op) {
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            tc_fence_before();
+        }
+        __syncwarp();
+        if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * (c0 / CH));
+        if (wr_rows) {
+            float *cbase = wr_base + (size_t)mrow0 * wr_ld + c0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int r = i * 8 + sub_r;
+                if (mrow0 + r < M) {
+                    float4 v;
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
+                    if (EPI == FE_RED) atomicAdd(reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c), v);
+                    else *reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c) = v;
+                }
+            }
+            __syncwarp();
+        }
+    }
+    vmax_out = fmaxf(vmax_out, vmax);
+    esum_out = esum;
+}
+
+// Regions alternate along the chain AND across tiles: a running count rc of operand generations (the chain input is
+// generation rc, the accumulator of GEMM j generation rc + 1 + j, the next tile starts at rc + n_stages + 1) gives
+// generation q the region q & 1, so the input of tile t+1 goes where the last GEMM of tile t took its operand from while
+// the last accumulator of tile t is still being drained from the other one.
+
 __global__ void __launch_bounds__(THREADS, 1)
-k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__restrict__ cta_tiles, float alpha)
+k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__restrict__ cta_tiles, float alpha, int *__restrict__ flags)
 {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -119,10 +301,10 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     // barriers (8 B each)
     const uint32_t bar_wfull = bar_base, bar_wempty = bar_base + 8 * NW;
     const uint32_t bar_afull = bar_base + 16 * NW, bar_aempty = bar_afull + 8 * NA;
-    const uint32_t bar_sready = bar_aempty + 8 * NA, bar_sfree = bar_sready + 16;
-    const uint32_t bar_accf = bar_sfree + 16, bar_acce = bar_accf + 16;
-    const uint32_t bar_tdone = bar_acce + 16; // every MMA of a tile has completed: both A slots are free for the next tile
-    const uint32_t tmem_slot = bar_tdone + 8;
+    const uint32_t bar_ready = bar_aempty + 8 * NA;            // [2 regions][MAX_CHUNKS]: operand chunk written
+    const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_CHUNKS;  // [2 regions]: every MMA into the region has completed
+    const uint32_t bar_drained = bar_accf + 16;                // the last accumulator of a tile has been read
+    const uint32_t tmem_slot = bar_drained + 8;
     const uint32_t stg_base = bar_base + BAR_BYTES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -130,14 +312,11 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
 
     if (threadIdx.x == 0) {
         for (int e = 0; e < NW; ++e) { mbar_init(bar_wfull + 8 * e, 1); mbar_init(bar_wempty + 8 * e, 1); }
-        for (int e = 0; e < NA; ++e) { mbar_init(bar_afull + 8 * e, 1); mbar_init(bar_aempty + 8 * e, 128); }
-        for (int k = 0; k < 2; ++k) {
-            mbar_init(bar_sready + 8 * k, 128);
-            mbar_init(bar_sfree + 8 * k, 1);
-            mbar_init(bar_accf + 8 * k, 1);
-            mbar_init(bar_acce + 8 * k, EPI_WARPS * 32);
-        }
-        mbar_init(bar_tdone, 1);
+        for (int e = 0; e < NA; ++e) { mbar_init(bar_afull + 8 * e, 1); mbar_init(bar_aempty + 8 * e, 8); }
+        for (int k = 0; k < 2 * MAX_CHUNKS; ++k) mbar_init(bar_ready + 8 * k, 4);
+        mbar_init(bar_accf, 1);
+        mbar_init(bar_accf + 8, 1);
+        mbar_init(bar_drained, EPI_WARPS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -151,7 +330,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
     if (warp == 0) {
-        // ===== producer: everything the MMA thread consumes from shared memory, in its order of use
+        // ===== producer: everything that arrives in shared memory, in its order of use
         if (lane == 0) {
             uint32_t wi = 0, ai = 0;
             for (int t = t_beg; t < t_end; ++t) {
@@ -162,22 +341,21 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                     const int K = g.st[j].K, N = g.st[j].N;
                     const int parts = N > 128 ? 2 : 1;
                     const uint8_t *wsrc = g.wblob + g.st[j].w_off;
-                    for (int kb = 0; kb < K / KB; ++kb) {
-                        if (j == 0) {
-                            const uint32_t e = ai % NA;
-                            mbar_wait(bar_aempty + 8 * e, ((ai / NA) & 1) ^ 1, 150, (t - t_beg) * 100 + kb);
-                            mbar_expect_tx(bar_afull + 8 * e, A_TILE_BYTES);
-                            tma_load_2d(a_ring + e * A_TILE_BYTES, &g.mapA, kb * KB, m0, bar_afull + 8 * e);
-                            ++ai;
-                        }
+                    for (int kb = 0; kb < (K + KBH - 1) / KBH; ++kb) {
+                        if (j == 0)
+                            for (int h = 0; h < 2 && (2 * kb + h) * KBF < K; ++h, ++ai) {
+                                const uint32_t e = ai % NA;
+                                mbar_wait(bar_aempty + 8 * e, ((ai / NA) & 1) ^ 1, 150, (t - t_beg) * 100 + kb);
+                                mbar_expect_tx(bar_afull + 8 * e, A_TILE_BYTES);
+                                tma_load_2d(a_ring + e * A_TILE_BYTES, &g.mapA, (2 * kb + h) * KBF, m0, bar_afull + 8 * e);
+                            }
                         for (int p = 0; p < parts; ++p, ++wi) {
                             const uint32_t e = wi % NW;
-                            const uint32_t rows = (uint32_t)part_rows(N, p);
-                            const uint32_t bytes = (SPLIT3 ? 2u : 1u) * rows * 128u; // hi tile first, lo tile behind it
+                            const uint32_t bytes = 2u * (uint32_t)part_rows(N, p) * 128u; // hi tile, lo tile behind it
                             mbar_wait(bar_wempty + 8 * e, ((wi / NW) & 1) ^ 1, 100 + j, (t - t_beg) * 100 + kb);
                             mbar_expect_tx(bar_wfull + 8 * e, bytes);
                             bulk_load(w_ring + e * W_ENTRY_BYTES, wsrc, bytes, bar_wfull + 8 * e);
-                            wsrc += 2u * rows * 128u;
+                            wsrc += bytes;
                         }
                     }
                 }
@@ -185,129 +363,69 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         }
     } else if (warp == 1) {
         // ===== MMA issue (whole warp walks the loop, one elected lane issues)
-        uint32_t wi = 0, ci = 0, useX = 0, useY = 0;
+        uint32_t wi = 0, rc = 0, par0 = 0u, par1 = 0u; // parities of the chunk barriers, one bit per chunk and region
         for (int t = t_beg; t < t_end; ++t) {
             const int gi = find_group(groups, n_groups, t);
             const FusedGroup &g = groups[gi];
+            // the first GEMM of a tile writes the region the previous tile's last accumulator was drained from
+            if (t > t_beg) { mbar_wait(bar_drained, (uint32_t)(t - t_beg - 1) & 1, 200, t - t_beg); tc_fence_after(); }
             for (int j = 0; j < g.n_stages; ++j) {
                 const int K = g.st[j].K, N = g.st[j].N;
                 const int parts = N > 128 ? 2 : 1;
-                // regions alternate; the chain starts in the one that puts its widest GEMMs (N <= 256) into X
-                const int in_y = (j & 1) ^ g.y_first;
-                const uint32_t acc = tmem_base + (in_y ? COL_Y : COL_X);
-                uint32_t &use = in_y ? useY : useX;
-                mbar_wait(bar_acce + 8 * in_y, (use & 1) ^ 1, 200 + j, t - t_beg); // the epilogue has drained the previous accumulator of this region
-                tc_fence_after();
-                const uint32_t idesc0 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(part_rows(N, 0) >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
-                const uint32_t idesc1 = parts > 1 ? (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(part_rows(N, 1) >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24) : 0u;
-                for (int kb = 0; kb < K / KB; ++kb) {
+                const uint32_t ra = (rc + (uint32_t)j) & 1u, rd = ra ^ 1u;
+                const uint32_t a_base = tmem_base + ra * REGION_COLS, acc = tmem_base + rd * REGION_COLS;
+                const uint32_t idesc0 = (1u << 4) | ((uint32_t)(part_rows(N, 0) >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+                const uint32_t idesc1 = parts > 1 ? (1u << 4) | ((uint32_t)(part_rows(N, 1) >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24) : 0u;
+                const int nch_tot = K / CH;
+                for (int kb = 0; kb < (K + KBH - 1) / KBH; ++kb) {
                     const uint32_t e0 = wi % NW, e1 = (wi + 1) % NW;
                     mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - t_beg) * 100 + kb);
                     if (parts > 1) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - t_beg) * 100 + kb);
                     const uint32_t b0 = w_ring + e0 * W_ENTRY_BYTES, b1 = w_ring + e1 * W_ENTRY_BYTES;
                     const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + (uint32_t)part_rows(N, 0) * 128u);
                     const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + (uint32_t)(parts > 1 ? part_rows(N, 1) : 8) * 128u);
-#pragma unroll
-                    for (int h = 0; h < 2; ++h, ++ci) {
-                        const uint32_t k = ci & 1;
-                        mbar_wait(bar_sready + 8 * k, (ci >> 1) & 1, 240 + j, (t - t_beg) * 100 + 2 * kb + h);
+                    const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
+                    for (int h = 0; h < nh; ++h) {
+                        const int c = 4 * kb + h;
+                        mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + c), ((ra ? par1 : par0) >> c) & 1u, 240 + j, (t - t_beg) * 100 + c);
+                        if (ra) par1 ^= 1u << c; else par0 ^= 1u << c;
                         tc_fence_after();
-                        const uint32_t a_hi = tmem_base + COL_Z + 32u * k, a_lo = a_hi + 16;
                         if (elect_one()) {
-#pragma unroll
-                            for (int ks = 0; ks < 2; ++ks) {
-                                const uint64_t koff = (uint64_t)(((2 * h + ks) * 8 * 4) >> 4);
-                                const uint32_t first = (kb | h | ks) ? 1u : 0u;
-                                if (SPLIT3) {
-                                    mma_tf32_ts(acc, a_lo + 8 * ks, d0hi + koff, idesc0, first);
-                                    mma_tf32_ts(acc, a_hi + 8 * ks, d0lo + koff, idesc0, 1u);
-                                    mma_tf32_ts(acc, a_hi + 8 * ks, d0hi + koff, idesc0, 1u);
-                                    if (parts > 1) {
-                                        mma_tf32_ts(acc + 128, a_lo + 8 * ks, d1hi + koff, idesc1, first);
-                                        mma_tf32_ts(acc + 128, a_hi + 8 * ks, d1lo + koff, idesc1, 1u);
-                                        mma_tf32_ts(acc + 128, a_hi + 8 * ks, d1hi + koff, idesc1, 1u);
-                                    }
-                                } else {
-                                    mma_tf32_ts(acc, a_hi + 8 * ks, d0hi + koff, idesc0, first);
-                                    if (parts > 1) mma_tf32_ts(acc + 128, a_hi + 8 * ks, d1hi + koff, idesc1, first);
-                                }
+                            const uint32_t a_hi = a_base + (uint32_t)(CH * c), a_lo = a_hi + 8;
+                            const uint64_t koff = (uint64_t)(2 * h); // 16 fp16 = 32 B along the swizzled row
+                            const uint32_t acc_on = c ? 1u : 0u;
+                            mma_f16_ts(acc, a_lo, d0hi + koff, idesc0, acc_on);
+                            mma_f16_ts(acc, a_hi, d0lo + koff, idesc0, 1u);
+                            mma_f16_ts(acc, a_hi, d0hi + koff, idesc0, 1u);
+                            if (parts > 1) {
+                                mma_f16_ts(acc + 128, a_lo, d1hi + koff, idesc1, acc_on);
+                                mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
+                                mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
                             }
-                            tc_commit(bar_sfree + 8 * k);
-                            if (h == 1) {
+                            if (h + 1 == nh) {
                                 tc_commit(bar_wempty + 8 * e0);
                                 if (parts > 1) tc_commit(bar_wempty + 8 * e1);
-                                if (kb + 1 == K / KB) {
-                                    tc_commit(bar_accf + 8 * in_y);
-                                    if (j + 1 == g.n_stages) tc_commit(bar_tdone);
-                                }
+                                if (c + 1 == nch_tot) tc_commit(bar_accf + 8 * rd);
                             }
                         }
                         __syncwarp();
                     }
                     wi += parts;
                 }
-                ++use;
             }
-        }
-    } else if (warp < 6) {
-        // ===== converters: A operand of the first GEMM (fp32 rows from HBM through the TMA ring) -> hi / lo slots
-        const int quarter = warp & 3;
-        const int row = quarter * 32 + lane;
-        const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
-        uint32_t ai = 0, ci = 0;
-        for (int t = t_beg; t < t_end; ++t) {
-            const int gi = find_group(groups, n_groups, t);
-            const FusedGroup &g = groups[gi];
-            const int nkb = g.st[0].K / KB;
-            // The slot barriers count in parities: a converter that ran a whole tile ahead would take the completion of
-            // ANY earlier use of a slot for the one it waits for.  The epilogue warps are held back by the accumulator
-            // barriers; the converters wait here until the previous tile has consumed its last chunk.
-            if (t > t_beg) mbar_wait(bar_tdone, (uint32_t)(t - t_beg - 1) & 1, 320, t - t_beg);
-            for (int kb = 0; kb < nkb; ++kb, ++ai) {
-                const uint32_t e = ai % NA;
-                mbar_wait(bar_afull + 8 * e, (ai / NA) & 1, 300, (t - t_beg) * 100 + kb);
-                const uint32_t arow = a_ring + e * A_TILE_BYTES + row * 128;
-                float x[32];
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    const uint32_t addr = arow + (uint32_t)((c ^ (row & 7)) << 4);
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[4 * c]), "=f"(x[4 * c + 1]), "=f"(x[4 * c + 2]), "=f"(x[4 * c + 3]) : "r"(addr));
-                }
-                mbar_arrive(bar_aempty + 8 * e); // the tile is in registers
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const uint32_t c = ci + 2 * kb + h, k = c & 1;
-                    uint32_t v[32];
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) {
-                        const float xv = x[16 * h + q];
-                        const uint32_t hi = tf32_round(xv);
-                        v[q] = hi;
-                        v[16 + q] = SPLIT3 ? tf32_round(xv - __uint_as_float(hi)) : 0u;
-                    }
-                    mbar_wait(bar_sfree + 8 * k, ((c >> 1) & 1) ^ 1, 310, (t - t_beg) * 100 + 2 * kb + h);
-                    tc_fence_after();
-                    tmem_st32(lane_addr + COL_Z + 32u * k, v);
-                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-                    tc_fence_before();
-                    mbar_arrive(bar_sready + 8 * k);
-                }
-            }
-            ci += (uint32_t)g.chunks_per_tile;
+            rc += (uint32_t)g.n_stages + 1u;
         }
     } else {
-        // ===== epilogue: warps 6..13 -> TMEM lane quarters 2,3,0,1,2,3,0,1; set 0 (warps 6-9) takes the even 16-column
-        // chunks of an accumulator, set 1 the odd ones.  This thread owns accumulator row `row`.
-        const int ew = warp - 6;
+        // ===== epilogue: warps 2..17; warp -> TMEM lane quarter warp & 3; set s = (warp - 2) / 4 takes the 16-column chunks
+        // s, s + 4, ... of an accumulator (and of the chain's input).  Lane l owns row quarter * 32 + l of the tile.
+        const int ew = warp - 2;
         const int quarter = warp & 3;
         const int set = ew >> 2;
         const int row = quarter * 32 + lane;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
         const uint32_t stg = stg_base + (uint32_t)ew * EPI_STG_BYTES;
-        const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
-        const int sub_r = (lane >> 3) + 4 * ((lane >> 2) & 1), sub_c = (lane & 3) * 4;
-        const float inv_alpha = 1.0f / alpha;
-        uint32_t ci = 0, useX = 0, useY = 0;
+        uint32_t rc = 0, use0 = 0u, use1 = 0u, a_cnt = 0;
+        float vmax = 0.f;
         for (int t = t_beg; t < t_end; ++t) {
             const int gi = find_group(groups, n_groups, t);
             const FusedGroup &g = groups[gi];
@@ -315,122 +433,64 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
             const int mrow0 = m0 + quarter * 32;
             const int m = mrow0 + lane;
             const bool rowok = m < g.M;
-            uint32_t cj = ci + (uint32_t)(g.st[0].K / CH); // chunk index of the first slot this stage's epilogue produces
-            for (int j = 0; j < g.n_stages; ++j) {
-                const int N = g.st[j].N, epi = g.st[j].epi;
-                const int in_y = (j & 1) ^ g.y_first;
-                const uint32_t acc_col = in_y ? COL_Y : COL_X;
-                uint32_t &use = in_y ? useY : useX;
-                const bool fwd = epi == FE_FWD || epi == FE_OUT;
-                const bool rd_prev = epi == FE_BWD || epi == FE_BWD_ST;   // reads rows of h for CELU'
-                const bool to_slot = epi == FE_FWD || epi == FE_OUT || epi == FE_BWD;
-                const bool wr_rows = epi == FE_FWD || epi == FE_BWD_ST || epi == FE_ST || epi == FE_RED;
-                // rows read (h for CELU') and rows written (h stash, or the chain's output)
-                const float *rd_base = epi == FE_BWD ? g.st[j].stash : g.out;
-                const int rd_ld = epi == FE_BWD ? g.st[j].ld_stash : g.ldo;
-                float *wr_base = epi == FE_FWD ? g.st[j].stash : g.out;
-                const int wr_ld = epi == FE_FWD ? g.st[j].ld_stash : g.ldo;
-                const float *bias = g.st[j].bias, *w4 = g.w4;
-                float esum = 0.f;
-                float bias_l = 0.f, w4_l = 0.f;
-                float4 pre[4];
-                auto prefetch = [&](int c0) {
-                    if (fwd) bias_l = lane < CH ? bias[c0 + lane] : 0.f;
-                    if (epi == FE_OUT) w4_l = lane < CH ? w4[c0 + lane] : 0.f;
-                    if (rd_prev) {
-                        const float *cb = rd_base + (size_t)mrow0 * rd_ld + c0;
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const int r = i * 8 + sub_r;
-                            pre[i] = mrow0 + r < g.M ? *reinterpret_cast<const float4 *>(cb + (size_t)r * rd_ld + sub_c)
-                                                     : make_float4(0.f, 0.f, 0.f, 0.f);
-                        }
-                    }
-                };
-                const int c_first = set * CH;
-                if (c_first < N) prefetch(c_first);
-                mbar_wait(bar_accf + 8 * in_y, use & 1, 400 + j, t - t_beg);
-                tc_fence_after();
-                for (int c0 = c_first; c0 < N; c0 += 2 * CH) {
-                    const float bias_c = bias_l, w4_c = w4_l;
-                    if (rd_prev) {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const int r = i * 8 + sub_r;
-                            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(pre[i].x), "f"(pre[i].y), "f"(pre[i].z), "f"(pre[i].w) : "memory");
-                        }
-                        __syncwarp();
-                    }
-                    if (c0 + 2 * CH < N) prefetch(c0 + 2 * CH);
-                    uint32_t a[16];
-                    tmem_ld16(lane_addr + acc_col + (uint32_t)c0, a);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    uint32_t sl[32];
+            {
+                // chain input (fp32 rows through the TMA ring) -> fp16 hi / lo chunks.  Their region was the operand of the
+                // previous tile's last GEMM, which this warp has seen complete (accumulator barrier of that GEMM).
+                const int nch0 = g.st[0].K / CH;
+                const uint32_t r0 = rc & 1u;
+                for (int c = set; c < nch0; c += EPI_SETS) {
+                    const uint32_t ai = a_cnt + (uint32_t)(c >> 1), e = ai % NA;
+                    mbar_wait(bar_afull + 8 * e, (ai / NA) & 1, 300, (t - t_beg) * 100 + c);
+                    const uint32_t arow = a_ring + e * A_TILE_BYTES + row * 128;
+                    float x[16];
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
-                        float4 prev = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (rd_prev)
-                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(prev.x), "=f"(prev.y), "=f"(prev.z), "=f"(prev.w) : "r"(my_row + q * 16));
-                        const float pv[4] = {prev.x, prev.y, prev.z, prev.w};
-                        float ov[4], hv[4];
+                        const uint32_t addr = arow + (uint32_t)(((4 * (c & 1) + q) ^ (row & 7)) << 4);
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[4 * q]), "=f"(x[4 * q + 1]), "=f"(x[4 * q + 2]), "=f"(x[4 * q + 3]) : "r"(addr));
+                    }
+                    uint32_t v[16];
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            float v = __uint_as_float(a[4 * q + e]);
-                            float bv = 0.f, wv = 0.f;
-                            bv = __shfl_sync(0xffffffffu, bias_c, 4 * q + e);
-                            wv = __shfl_sync(0xffffffffu, w4_c, 4 * q + e);
-                            hv[e] = 0.f;
-                            if (epi == FE_FWD) { v = celu_fwd(v + bv, alpha, inv_alpha); hv[e] = v; }
-                            else if (epi == FE_OUT) {
-                                const float hh = celu_fwd(v + bv, alpha, inv_alpha);
-                                esum = fmaf(hh, wv, esum);
-                                v = wv * celu_grad_from_h(hh, inv_alpha);
-                            } else if (rd_prev) v *= celu_grad_from_h(pv[e], inv_alpha);
-                            ov[e] = v;
-                            const uint32_t hi = tf32_round(v);
-                            sl[4 * q + e] = hi;
-                            sl[16 + 4 * q + e] = SPLIT3 ? tf32_round(v - __uint_as_float(hi)) : 0u;
-                        }
-                        if (wr_rows) {
-                            if (rd_prev) __syncwarp(); // (same thread re-uses its own staged row: no hazard across lanes here)
-                            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + q * 16), "f"(epi == FE_FWD ? hv[0] : ov[0]), "f"(epi == FE_FWD ? hv[1] : ov[1]), "f"(epi == FE_FWD ? hv[2] : ov[2]), "f"(epi == FE_FWD ? hv[3] : ov[3]) : "memory");
-                        }
-                    }
-                    if (to_slot) {
-                        const uint32_t c = cj + (uint32_t)(c0 / CH), k = c & 1;
-                        mbar_wait(bar_sfree + 8 * k, ((c >> 1) & 1) ^ 1, 420 + j, (t - t_beg) * 1000 + c0);
-                        tc_fence_after();
-                        tmem_st32(lane_addr + COL_Z + 32u * k, sl);
-                        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-                        tc_fence_before();
-                        mbar_arrive(bar_sready + 8 * k);
-                    }
-                    if (wr_rows) {
-                        __syncwarp();
-                        float *cbase = wr_base + (size_t)mrow0 * wr_ld + c0;
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const int r = i * 8 + sub_r;
-                            if (mrow0 + r < g.M) {
-                                float4 v;
-                                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
-                                if (epi == FE_RED) atomicAdd(reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c), v);
-                                else *reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c) = v;
-                            }
-                        }
-                        __syncwarp();
-                    } else if (rd_prev) {
-                        __syncwarp(); // every lane has read its staged row before the next chunk overwrites the staging
-                    }
+                    for (int q = 0; q < 16; ++q) { x[q] *= ACT_SCALE; vmax = fmaxf(vmax, fabsf(x[q])); }
+                    split16(x, v);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_aempty + 8 * e); // this warp's half of the tile is in registers
+                    tmem_st16(lane_addr + r0 * REGION_COLS + (uint32_t)(CH * c), v);
+                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_CHUNKS + c));
                 }
-                tc_fence_before();
-                mbar_arrive(bar_acce + 8 * in_y);
-                ++use;
-                if (epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, esum);
-                if (to_slot) cj += (uint32_t)(N / CH);
+                a_cnt += (uint32_t)(g.st[0].K / KBF);
             }
-            ci = cj;
+            for (int j = 0; j < g.n_stages; ++j) {
+                const uint32_t rd = (rc + (uint32_t)j + 1u) & 1u;
+                EpiArgs ea;
+                ea.g = &g; ea.st = &g.st[j]; ea.mrow0 = mrow0; ea.lane = lane; ea.set = set;
+                ea.tm_acc = lane_addr + rd * REGION_COLS; ea.stg = stg;
+                ea.bar_accf = bar_accf + 8 * rd; ea.accf_parity = (rd ? use1 : use0) & 1u;
+                ea.bar_ready = bar_ready + 8 * (rd * MAX_CHUNKS);
+                ea.alpha = alpha; ea.site = 400 + j; ea.aux = t - t_beg;
+                if (rd) ++use1; else ++use0;
+                float esum = 0.f;
+                switch (g.st[j].epi) {
+                case FE_FWD: epi_stage<FE_FWD>(ea, vmax, esum); break;
+                case FE_OUT: epi_stage<FE_OUT>(ea, vmax, esum); break;
+                case FE_BWD: epi_stage<FE_BWD>(ea, vmax, esum); break;
+                case FE_BWD_ST: epi_stage<FE_BWD_ST>(ea, vmax, esum); break;
+                case FE_ST: epi_stage<FE_ST>(ea, vmax, esum); break;
+                default: epi_stage<FE_RED>(ea, vmax, esum); break;
+                }
+                if (j + 1 == g.n_stages) {
+                    // the tile's last accumulator has left tensor memory (for this warp): the next tile may overwrite it
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_drained);
+                }
+                if (g.st[j].epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, esum * (1.0f / ACT_SCALE));
+            }
+            rc += (uint32_t)g.n_stages + 1u;
         }
+        if (vmax > RANGE_LIMIT) atomicOr(&flags[0], NNP_FLAG_RANGE);
     }
     __syncthreads();
     if (warp == 1) {
@@ -439,29 +499,41 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     }
 }
 
-// Packs one weight matrix Bt [N][K] (K contiguous; the B operand of D = A . Bt^T) into the tile images the kernel copies
-// with one bulk load each: for every K block of 32 and part p (rows [0,128) / [128,N)): the tf32-hi tile then the tf32-lo
-// tile, rows of 128 B, 16-byte chunk c of row r stored at chunk position c ^ (r & 7) (128-byte swizzle).
-__global__ void k_pack_weights(const float *__restrict__ Bt, int N, int K, int ldb, uint8_t *__restrict__ dst)
+// Packs one weight matrix Bt [N][K] (K contiguous; the B operand of D = A . Bt^T), multiplied by `scale`, into the tile
+// images the kernel copies with one bulk load each: for every K block of 64 and part p (rows [0,128) / [128,N)): the
+// fp16-hi tile then the fp16-lo tile, rows of 128 B (zero beyond K), 16-byte chunk c of row r stored at chunk position
+// c ^ (r & 7) (128-byte swizzle).
+__global__ void k_pack_weights(const float *__restrict__ Bt, int N, int K, int ldb, float scale, uint8_t *__restrict__ dst)
 {
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x; // one 16-byte chunk of one row of one K block
-    const int nkb = K / KB;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x; // one 16-byte chunk (8 fp16) of one row of one K block
+    const int nkb = (K + KBH - 1) / KBH;
     if (idx >= N * nkb * 8) return;
     const int c = idx & 7, n = (idx >> 3) % N, kb = (idx >> 3) / N;
     const int p = n >= 128 ? 1 : 0, rows = p == 0 ? (N > 128 ? 128 : N) : N - 128, r = n - 128 * p;
     // K block kb: [part 0: hi rows0 x 128 | lo rows0 x 128][part 1: hi | lo]
     const size_t kb_bytes = (size_t)2 * N * 128;
     uint8_t *tile = dst + kb * kb_bytes + (p ? (size_t)2 * (N > 128 ? 128 : N) * 128 : 0);
-    const float4 v = *reinterpret_cast<const float4 *>(Bt + (size_t)n * ldb + kb * KB + 4 * c);
-    const float x[4] = {v.x, v.y, v.z, v.w};
     uint32_t hi[4], lo[4];
-    for (int e = 0; e < 4; ++e) {
-        hi[e] = (__float_as_uint(x[e]) + 0x1000u) & 0xffffe000u;
-        lo[e] = (__float_as_uint(x[e] - __uint_as_float(hi[e])) + 0x1000u) & 0xffffe000u;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int k = kb * KBH + 8 * c + 2 * q;
+        const float x0 = k < K ? Bt[(size_t)n * ldb + k] * scale : 0.f;
+        const float x1 = k + 1 < K ? Bt[(size_t)n * ldb + k + 1] * scale : 0.f;
+        const __half2 h = __floats2half2_rn(x0, x1);
+        const float2 hf = __half22float2(h);
+        const __half2 l = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+        hi[q] = *reinterpret_cast<const uint32_t *>(&h);
+        lo[q] = *reinterpret_cast<const uint32_t *>(&l);
     }
     const size_t off = (size_t)r * 128 + (size_t)((c ^ (r & 7)) << 4);
     *reinterpret_cast<uint4 *>(tile + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
     *reinterpret_cast<uint4 *>(tile + (size_t)rows * 128 + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+}
+
+__global__ void k_scale_copy(const float *__restrict__ src, int n, float scale, float *__restrict__ dst)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[i] * scale;
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -483,10 +555,25 @@ bool make_map_a(CUtensorMap *m, const float *base, int rows, int cols, int ld)
 {
     cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
     cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
-    cuuint32_t box[2] = {(cuuint32_t)KB, (cuuint32_t)TILE_M};
+    cuuint32_t box[2] = {(cuuint32_t)KBF, (cuuint32_t)TILE_M};
     cuuint32_t estr[2] = {1, 1};
     return g_encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// bytes of the packed tiles of one matrix Bt [N][K]
+size_t packed_bytes(int N, int K) { return (size_t)((K + KBH - 1) / KBH) * 2 * N * 128; }
+
+// power-of-two weight scale: max |w| 2^e in [2^13, 2^14)
+int weight_shift(float wmax)
+{
+    if (!(wmax > 0.f) || !isfinite(wmax)) return 0;
+    int e;
+    frexpf(wmax, &e); // wmax = f 2^e, f in [0.5, 1)
+    int sh = 14 - e;
+    if (sh > 40) sh = 40;
+    if (sh < -40) sh = -40;
+    return sh;
 }
 
 } // namespace
@@ -496,7 +583,8 @@ struct nnp_fused {
     int n_groups, n_tiles, grid;
     FusedGroup *d_groups;        // [n_nets * S]
     int *d_cta_tiles;            // [grid + 1]
-    uint8_t *d_wblob;            // packed weights of every (network, species): sized at first use for the full layout
+    uint8_t *d_wblob;            // packed weights of every (network, species): sized at first use for the largest layout
+    float *d_bias16;             // [n_nets * S][3][256] biases * 2^ACT_SHIFT
     size_t wblob_bytes;
     size_t w_off[64][MAX_STAGES + 1]; // per (network, species): byte offsets of F1 F2 F3 B3 B2 B1 in the blob
     unsigned packed_mask;        // species mask the layer-1 tiles were packed for (0: nothing packed yet)
@@ -511,7 +599,7 @@ void nnp_fused_destroy(nnp_ctx *c)
         if (!p) return;
         if (cc->dealloc_fn) cc->dealloc_fn(p, cc->alloc_user); else cudaFree(p);
     };
-    fr(c, f->d_groups); fr(c, f->d_cta_tiles); fr(c, f->d_wblob);
+    fr(c, f->d_groups); fr(c, f->d_cta_tiles); fr(c, f->d_wblob); fr(c, f->d_bias16);
     delete f;
     c->fused = nullptr;
 }
@@ -527,10 +615,10 @@ static void *fused_alloc(nnp_ctx *c, size_t bytes)
 // Decides whether (and which chain of) the fused kernel serves the loaded system, packs the weights (once per species
 // set: the layer-1 tiles depend on the active AEV columns) and builds the group table and the per-CTA tile ranges.
 // Called by nnp_set_system after the layout is known.  Returns NNP_OK also when the fused path is not applicable
-// (c->fused->kind = 0: the six-launch path runs).
+// (c->fused->kind = 0: the six-launch 3xTF32 path runs).
 int nnp_fused_setup(nnp_ctx *c)
 {
-    if (!c->tc_mode || c->no_fused) return NNP_OK;
+    if (c->mm_mode != NNP_MM_3XF16_TC || c->no_fused) return NNP_OK;
     if (!load_encode()) { c->err = "cuTensorMapEncodeTiled entry point not available"; return NNP_ECUDA; }
     const int S = c->S, nn = c->n_nets;
     if (nn * S > 64) return NNP_OK;
@@ -543,33 +631,38 @@ int nnp_fused_setup(nnp_ctx *c)
     nnp_fused *f = c->fused;
     f->kind = 0;
     const int kpad = c->aev.kpad;
-    // widths the TMEM layout can hold: X (256 columns): h1, h3; Y (192): h2 and, in the full chain, kpad
+    // widths a 256-column region holds; every accumulator must give all four epilogue sets a chunk
     for (int s = 0; s < S; ++s)
-        if (c->widths[s][1] > 256 || c->widths[s][2] > 192 || c->widths[s][3] > 256) return NNP_OK;
-    const int kind = kpad <= 192 ? 1 : 2;
+        for (int l = 1; l <= 3; ++l)
+            if (c->widths[s][l] > REGION_COLS || c->widths[s][l] < EPI_SETS * CH) return NNP_OK;
+    const int kind = kpad <= REGION_COLS ? 1 : 2;
+    const size_t k0max = c->kpad_full < REGION_COLS ? c->kpad_full : REGION_COLS; // layer-1 tiles exist for the full chain only
     // ---- packed weights: per (net, species) the six matrices in chain order; sized for the largest layout once
     if (!f->d_wblob) {
         size_t tot = 0;
         for (int net = 0; net < nn; ++net)
             for (int s = 0; s < S; ++s) {
-                const size_t k0 = c->kpad_full < 192 ? c->kpad_full : 192, h1 = c->widths[s][1], h2 = c->widths[s][2], h3 = c->widths[s][3];
-                tot += 8 * (2 * k0 * h1 + 2 * h1 * h2 + 2 * h2 * h3);
+                const int h1 = c->widths[s][1], h2 = c->widths[s][2], h3 = c->widths[s][3];
+                tot += packed_bytes(h1, (int)k0max) + packed_bytes((int)k0max, h1) + packed_bytes(h2, h1) + packed_bytes(h1, h2) +
+                       packed_bytes(h3, h2) + packed_bytes(h2, h3);
             }
         f->d_wblob = (uint8_t *)fused_alloc(c, tot);
         if (!f->d_wblob) { c->err = "fused MLP: weight tile allocation failed"; return NNP_ENOMEM; }
         f->wblob_bytes = tot;
         f->d_groups = (FusedGroup *)fused_alloc(c, sizeof(FusedGroup) * 64);
         f->d_cta_tiles = (int *)fused_alloc(c, sizeof(int) * (f->num_sms + 1));
-        if (!f->d_groups || !f->d_cta_tiles) { c->err = "fused MLP: table allocation failed"; return NNP_ENOMEM; }
+        f->d_bias16 = (float *)fused_alloc(c, sizeof(float) * (size_t)nn * S * 3 * REGION_COLS);
+        if (!f->d_groups || !f->d_cta_tiles || !f->d_bias16) { c->err = "fused MLP: table allocation failed"; return NNP_ENOMEM; }
         f->packed_mask = 0;
     }
-    auto pack = [&](const float *Bt, int N, int K, int ldb, uint8_t *dst) {
-        const int total = N * (K / KB) * 8;
-        k_pack_weights<<<nnp_div_up(total, 256), 256, 0, c->stream>>>(Bt, N, K, ldb, dst);
+    auto pack = [&](const float *Bt, int N, int K, int ldb, int shift, uint8_t *dst) {
+        const int total = N * ((K + KBH - 1) / KBH) * 8;
+        k_pack_weights<<<nnp_div_up(total, 256), 256, 0, c->stream>>>(Bt, N, K, ldb, ldexpf(1.0f, shift), dst);
         c->launches += 1;
     };
     const bool repack_l1 = f->packed_mask != c->present_mask;
     const bool first_pack = f->packed_mask == 0;
+    int wsh[64][3]; // weight shifts of layers 1..3 per (network, species)
     {
         size_t o = 0;
         for (int net = 0; net < nn; ++net)
@@ -578,24 +671,28 @@ int nnp_fused_setup(nnp_ctx *c)
                 const int h1 = c->widths[s][1], h2 = c->widths[s][2], h3 = c->widths[s][3];
                 const LayerW *L = &c->layers[((size_t)net * S + s) * NNP_NLAYERS];
                 const Layer1C &l1 = c->l1c[(size_t)net * S + s];
-                const size_t k0 = c->kpad_full < 192 ? c->kpad_full : 192; // layer-1 tiles exist for the full chain only
+                for (int l = 0; l < 3; ++l) wsh[q][l] = weight_shift(L[l].wmax);
                 // F1: B = W1^T [h1][kpad]; F2: W2^T [h2][h1]; F3: W3^T [h3][h2]; B3: W3 [h2][h3]; B2: W2 [h1][h2]; B1: W1 [kpad][h1]
-                f->w_off[q][0] = o; o += 8 * k0 * h1;
-                f->w_off[q][1] = o; o += 8 * (size_t)h1 * h2;
-                f->w_off[q][2] = o; o += 8 * (size_t)h2 * h3;
-                f->w_off[q][3] = o; o += 8 * (size_t)h2 * h3;
-                f->w_off[q][4] = o; o += 8 * (size_t)h1 * h2;
-                f->w_off[q][5] = o; o += 8 * k0 * h1;
+                f->w_off[q][0] = o; o += packed_bytes(h1, (int)k0max);
+                f->w_off[q][1] = o; o += packed_bytes(h2, h1);
+                f->w_off[q][2] = o; o += packed_bytes(h3, h2);
+                f->w_off[q][3] = o; o += packed_bytes(h2, h3);
+                f->w_off[q][4] = o; o += packed_bytes(h1, h2);
+                f->w_off[q][5] = o; o += packed_bytes((int)k0max, h1);
                 f->w_off[q][6] = o;
                 if (first_pack) {
-                    pack(L[1].Wt, h2, h1, h1, f->d_wblob + f->w_off[q][1]);
-                    pack(L[2].Wt, h3, h2, h2, f->d_wblob + f->w_off[q][2]);
-                    pack(L[2].W, h2, h3, h3, f->d_wblob + f->w_off[q][3]);
-                    pack(L[1].W, h1, h2, h2, f->d_wblob + f->w_off[q][4]);
+                    pack(L[1].Wt, h2, h1, h1, wsh[q][1], f->d_wblob + f->w_off[q][1]);
+                    pack(L[2].Wt, h3, h2, h2, wsh[q][2], f->d_wblob + f->w_off[q][2]);
+                    pack(L[2].W, h2, h3, h3, wsh[q][2], f->d_wblob + f->w_off[q][3]);
+                    pack(L[1].W, h1, h2, h2, wsh[q][1], f->d_wblob + f->w_off[q][4]);
+                    for (int l = 0; l < 3; ++l) {
+                        k_scale_copy<<<1, 256, 0, c->stream>>>(L[l].b, c->widths[s][l + 1], ACT_SCALE, f->d_bias16 + ((size_t)q * 3 + l) * REGION_COLS);
+                        c->launches += 1;
+                    }
                 }
                 if (repack_l1 && kind == 1) {
-                    pack(l1.Wt, h1, kpad, kpad, f->d_wblob + f->w_off[q][0]);
-                    pack(l1.W, kpad, h1, h1, f->d_wblob + f->w_off[q][5]);
+                    pack(l1.Wt, h1, kpad, kpad, wsh[q][0], f->d_wblob + f->w_off[q][0]);
+                    pack(l1.W, kpad, h1, h1, wsh[q][0], f->d_wblob + f->w_off[q][5]);
                 }
             }
     }
@@ -606,6 +703,7 @@ int nnp_fused_setup(nnp_ctx *c)
     std::vector<FusedGroup> groups;
     std::vector<long long> cost;
     int tiles = 0;
+    const float alpha = c->alpha;
     for (int net = 0; net < nn; ++net)
         for (int s = 0; s < S; ++s) {
             const int off = c->bucket_off[s], M = c->bucket_off[s + 1] - off;
@@ -615,6 +713,7 @@ int nnp_fused_setup(nnp_ctx *c)
             const LayerW *L = &c->layers[((size_t)net * S + s) * NNP_NLAYERS];
             float *H0 = c->H[0] + ((size_t)net * c->max_atoms + off) * c->hmax[0];
             float *H1 = c->H[1] + ((size_t)net * c->max_atoms + off) * c->hmax[1];
+            const float *b16 = f->d_bias16 + (size_t)q * 3 * REGION_COLS;
             FusedGroup g;
             memset(&g, 0, sizeof(g));
             g.wblob = f->d_wblob;
@@ -623,39 +722,46 @@ int nnp_fused_setup(nnp_ctx *c)
             g.M = M;
             g.tile0 = tiles;
             g.n_tiles = nnp_div_up(M, TILE_M);
-            auto stage = [&](int j, int K, int N, int epi, size_t w_off, const float *bias, float *stash, int ld) {
+            // acc = sum (16 a)(2^sh w): forward epilogues want 16 z = acc 2^-sh; reverse operand-producing epilogues
+            // 16 delta = acc 2^-sh celu'(h) with the stash holding 16 h; output epilogues the true value acc 2^-(sh + 4)
+            auto fwd = [&](int j, int K, int N, int epi, size_t w_off, const float *bias, float *stash, int ld, int sh) {
                 FusedStage &st = g.st[j];
                 st.K = K; st.N = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.bias = bias; st.stash = stash; st.ld_stash = ld;
+                st.c_acc = ldexpf(1.0f, -sh);
+            };
+            auto bwd = [&](int j, int K, int N, int epi, size_t w_off, float *stash, int ld, int sh) {
+                FusedStage &st = g.st[j];
+                st.K = K; st.N = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.stash = stash; st.ld_stash = ld;
+                const float s2 = ldexpf(1.0f, -sh);
+                if (epi == FE_BWD) { st.gs = s2 / (alpha * ACT_SCALE); st.gc = s2; }                       // stash = 16 h, out = 16 delta
+                else if (epi == FE_BWD_ST) { st.gs = s2 / ACT_SCALE / alpha; st.gc = s2 / ACT_SCALE; }     // out rows = true h, out = true delta
+                st.c_acc = s2 / ACT_SCALE;                                                                  // FE_ST / FE_RED
             };
             if (f->w_off[q][6] > 0xffffffffull) { c->err = "fused MLP: weight blob exceeds 4 GiB"; return NNP_EINVAL; }
             if (kind == 1) {
                 g.n_stages = 6;
                 if (!make_map_a(&g.mapA, c->G + (size_t)off * kpad, M, kpad, kpad)) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
-                stage(0, kpad, h1, FE_FWD, f->w_off[q][0], L[0].b, H0, c->hmax[0]);
-                stage(1, h1, h2, FE_FWD, f->w_off[q][1], L[1].b, H1, c->hmax[1]);
-                stage(2, h2, h3, FE_OUT, f->w_off[q][2], L[2].b, nullptr, 0);
-                stage(3, h3, h2, FE_BWD, f->w_off[q][3], nullptr, H1, c->hmax[1]);
-                stage(4, h2, h1, FE_BWD, f->w_off[q][4], nullptr, H0, c->hmax[0]);
-                stage(5, h1, kpad, nn > 1 ? FE_RED : FE_ST, f->w_off[q][5], nullptr, nullptr, 0);
+                fwd(0, kpad, h1, FE_FWD, f->w_off[q][0], b16, H0, c->hmax[0], wsh[q][0]);
+                fwd(1, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1]);
+                fwd(2, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2]);
+                bwd(3, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
+                bwd(4, h2, h1, FE_BWD, f->w_off[q][4], H0, c->hmax[0], wsh[q][1]);
+                bwd(5, h1, kpad, nn > 1 ? FE_RED : FE_ST, f->w_off[q][5], nullptr, 0, wsh[q][0]);
                 g.out = c->dG + (size_t)off * kpad;
                 g.ldo = kpad;
-                g.y_first = 0; // F1 X, F2 Y, F3 X, B3 Y, B2 X, B1 Y (kpad <= 192)
             } else {
                 g.n_stages = 4;
-                g.y_first = 1; // F2 Y, F3 X, B3 Y, B2 X (h1 <= 256)
                 if (!make_map_a(&g.mapA, H0, M, h1, c->hmax[0])) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
-                stage(0, h1, h2, FE_FWD, f->w_off[q][1], L[1].b, H1, c->hmax[1]);
-                stage(1, h2, h3, FE_OUT, f->w_off[q][2], L[2].b, nullptr, 0);
-                stage(2, h3, h2, FE_BWD, f->w_off[q][3], nullptr, H1, c->hmax[1]);
-                stage(3, h2, h1, FE_BWD_ST, f->w_off[q][4], nullptr, nullptr, 0);
+                fwd(0, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1]);
+                fwd(1, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2]);
+                bwd(2, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
+                bwd(3, h2, h1, FE_BWD_ST, f->w_off[q][4], nullptr, 0, wsh[q][1]);
                 g.out = H0;
                 g.ldo = c->hmax[0];
             }
             long long cst = 0;
-            for (int j = 0; j < g.n_stages; ++j) {
-                g.chunks_per_tile += g.st[j].K / CH;
-                cst += (long long)(g.st[j].K / 8) * 3 * (g.st[j].N / 2) + 1500; // MMA cycles + the hand-over bubble of a GEMM
-            }
+            for (int j = 0; j < g.n_stages; ++j)
+                cst += (long long)(g.st[j].K / CH) * 3 * (g.st[j].N / 2) + 1200; // MMA cycles + the hand-over bubble of a GEMM
             tiles += g.n_tiles;
             groups.push_back(g);
             cost.push_back(cst);
@@ -665,8 +771,6 @@ int nnp_fused_setup(nnp_ctx *c)
     if (tiles == 0) return NNP_OK;
     // contiguous tile ranges of equal cost
     int grid = tiles < f->num_sms ? tiles : f->num_sms;
-    const char *dbg = getenv("NNP_FUSED_DEBUG");
-    if (dbg && dbg[0] == '2') grid = (tiles + 1) / 2;
     std::vector<int> cta(grid + 1, tiles);
     {
         long long total = 0;
@@ -683,8 +787,6 @@ int nnp_fused_setup(nnp_ctx *c)
         for (int k = 1; k <= grid; ++k)
             if (cta[k] < cta[k - 1]) cta[k] = cta[k - 1];
     }
-    if (dbg && (dbg[0] == '1' || dbg[0] == '2'))
-        for (int k = 0; k <= grid; ++k) cta[k] = (int)((long long)tiles * k / grid);
     f->grid = grid;
     if (cudaMemcpyAsync(f->d_groups, groups.data(), sizeof(FusedGroup) * groups.size(), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(f->d_cta_tiles, cta.data(), sizeof(int) * (grid + 1), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
@@ -704,13 +806,9 @@ void nnp_launch_mlp_fused(nnp_ctx *c)
     nnp_fused *f = c->fused;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(k_mlp_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        cudaFuncSetAttribute(k_mlp_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaFuncSetAttribute(k_mlp_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         attr_set = true;
     }
-    if (c->mm_mode == NNP_MM_3XTF32_TC)
-        k_mlp_fused<true><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha);
-    else
-        k_mlp_fused<false><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha);
+    k_mlp_fused<<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
     c->launches += 1;
 }

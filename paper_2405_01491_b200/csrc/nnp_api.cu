@@ -306,6 +306,8 @@ int check_flags(nnp_ctx *c)
     if (h[0] & (NNP_FLAG_CAP_R | NNP_FLAG_CAP_A))
         NNP_FAIL(c, NNP_ECAPACITY, "neighbour capacity exceeded (%s): recreate with larger cap_r/cap_a",
                  (h[0] & NNP_FLAG_CAP_R) ? "radial" : "angular");
+    if (h[0] & NNP_FLAG_RANGE)
+        NNP_FAIL(c, NNP_ERANGE, "mm_mode 4: an activation exceeded the range of the scaled fp16 split; use mm_mode 1");
     return NNP_OK;
 }
 
@@ -374,7 +376,7 @@ void make_batch(nnp_ctx *c, int net0, int n_batch, int op, GemmBatch &b)
 int run_gemm(nnp_ctx *c, const GemmBatch &b, int epi)
 {
     if (!c->tc_mode) { nnp_launch_gemm_simt(c, b, epi, c->mm_mode == NNP_MM_FP64_SIMT); return NNP_OK; }
-    return nnp_launch_gemm_tc(c, b, epi, c->mm_mode == NNP_MM_3XTF32_TC);
+    return nnp_launch_gemm_tc(c, b, epi, c->split3);
 }
 
 // Stages 2-4 on the current lists: frc, e_mol.
@@ -595,7 +597,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
         NNP_FAIL(none, NNP_EINVAL, "null parameter array");
     if (max_atoms < 1 || max_mols < 1 || p->n_nets < 1) NNP_FAIL(none, NNP_EINVAL, "max_atoms, max_mols, n_nets must be >= 1");
     if (!(p->rcr > 0.f) || !(p->rca > 0.f) || p->rca > p->rcr) NNP_FAIL(none, NNP_EINVAL, "need 0 < rca <= rcr");
-    if (p->mm_mode < 0 || p->mm_mode > 3) NNP_FAIL(none, NNP_EINVAL, "bad mm_mode");
+    if (p->mm_mode < 0 || p->mm_mode > 4) NNP_FAIL(none, NNP_EINVAL, "bad mm_mode");
     if ((p->alloc == nullptr) != (p->dealloc == nullptr)) NNP_FAIL(none, NNP_EINVAL, "alloc and dealloc must be given together");
     const int S = p->n_species;
     const int aev_len = S * NNP_NSHF_R + S * (S + 1) / 2 * NNP_ANG_BLOCK;
@@ -612,7 +614,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     if (cudaSetDevice(device) != cudaSuccess) NNP_FAIL(none, NNP_ECUDA, "cudaSetDevice(%d) failed", device);
     nnp_ctx *c = new nnp_ctx();
     // new T() value-initialises: every POD member starts at zero
-    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode; c->tc_mode = p->mm_mode == NNP_MM_3XTF32_TC || p->mm_mode == NNP_MM_TF32_TC; c->dense_aev = p->dense_aev != 0;
+    c->S = S; c->n_nets = p->n_nets; c->mm_mode = p->mm_mode; c->tc_mode = p->mm_mode == NNP_MM_3XTF32_TC || p->mm_mode == NNP_MM_TF32_TC || p->mm_mode == NNP_MM_3XF16_TC; c->split3 = p->mm_mode != NNP_MM_TF32_TC; c->dense_aev = p->dense_aev != 0;
     c->alpha = p->celu_alpha; c->accel_conv = p->accel_conv;
     c->stream = (cudaStream_t)cuda_stream; c->device = device;
     c->alloc_fn = p->alloc; c->dealloc_fn = p->dealloc; c->alloc_user = p->alloc_user;
@@ -675,11 +677,13 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
                     float *W = &blob[o]; o += (size_t)L.in_pad * L.out;
                     float *Wt = &blob[o]; o += (size_t)L.in_pad * L.out;
                     float *b = &blob[o]; o += (size_t)((L.out + 3) / 4 * 4);
+                    L.wmax = 0.f;
                     for (int i = 0; i < L.in; ++i)
                         for (int j = 0; j < L.out; ++j) {
                             const float v = src[(size_t)i * L.out + j];
                             W[(size_t)i * L.out + j] = v;
                             Wt[(size_t)j * L.in_pad + i] = v;
+                            if (fabsf(v) > L.wmax) L.wmax = fabsf(v);
                         }
                     src += (size_t)L.in * L.out;
                     for (int j = 0; j < L.out; ++j) b[j] = src[j];
@@ -1107,6 +1111,8 @@ int nnp_md_step_host(nnp_ctx *c, float *h_xyz, float *h_vel, int n_steps, double
     if (f0 & (NNP_FLAG_CAP_R | NNP_FLAG_CAP_A))
         NNP_FAIL(c, NNP_ECAPACITY, "neighbour capacity exceeded (%s): recreate with larger cap_r/cap_a",
                  (f0 & NNP_FLAG_CAP_R) ? "radial" : "angular");
+    if (f0 & NNP_FLAG_RANGE)
+        NNP_FAIL(c, NNP_ERANGE, "mm_mode 4: an activation exceeded the range of the scaled fp16 split; use mm_mode 1");
     return NNP_OK;
 }
 

@@ -19,7 +19,7 @@
 #define NNP_TRI_LEN 2016 /* pairs (lo < hi) with hi < 64: decode table of the AEV kernels */
 
 // Device error flags latched by kernels, reported by synchronising calls.
-enum { NNP_FLAG_CAP_R = 1, NNP_FLAG_CAP_A = 2 };
+enum { NNP_FLAG_CAP_R = 1, NNP_FLAG_CAP_A = 2, NNP_FLAG_RANGE = 4 };
 
 // ---- periodic cell grid / molecule bins (stage 1) ------------------------------------------------
 struct GridInfo {
@@ -123,6 +123,7 @@ struct LayerW {
     float *b;  // device [out]
     float *W_hi, *W_lo, *Wt_hi, *Wt_lo; // tf32 splits (tensor-core modes only)
     int in, in_pad, out;
+    float wmax; // max |w| (scaling of the fp16 split, mlp_fused.cu)
 };
 // layer 1 restricted to the active columns of the loaded system (built by nnp_set_system)
 struct Layer1C {
@@ -135,6 +136,7 @@ struct nnp_ctx {
     // model
     int S, n_nets, mm_mode, dense_aev;
     int tc_mode;                    // mm_mode is one of the tcgen05 modes (weights carry tf32 hi / lo splits)
+    int split3;                     // unfused tcgen05 GEMMs run 3xTF32 (modes 1 and 4), else plain TF32
     int aev_len_full, kpad_full;    // 1008 / 1024 for 7 species
     unsigned present_mask;          // species mask the compact layer-1 copies were built for (0: none yet)
     Layer1C *l1c;                   // host array [n_nets][S]
@@ -215,7 +217,7 @@ struct nnp_ctx {
     cudaStream_t aux_stream;     // capture stream of the conditional body
     int64_t md_graph_launches;   // kernels per graph launch outside the conditional body
     int no_graph;                // NNP_NO_GRAPH=1: enqueue every step kernel by kernel
-    nnp_fused *fused;            // fused MLP chain (tensor-core modes), set up per loaded system
+    nnp_fused *fused;            // fused MLP chain (mm_mode 4), set up per loaded system
     int no_fused;                // NNP_NO_FUSED=1: always the six-launch path
 };
 

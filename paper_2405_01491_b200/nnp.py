@@ -13,8 +13,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
 
-NNP_OK, NNP_EINVAL, NNP_ENOMEM, NNP_ECUDA, NNP_ECAPACITY, NNP_ESTALE, NNP_EBOX = 0, -1, -2, -3, -4, -5, -6
-NNP_MM_FP32_SIMT, NNP_MM_3XTF32_TC, NNP_MM_TF32_TC, NNP_MM_FP64_SIMT = 0, 1, 2, 3
+NNP_OK, NNP_EINVAL, NNP_ENOMEM, NNP_ECUDA, NNP_ECAPACITY, NNP_ESTALE, NNP_EBOX, NNP_ERANGE = 0, -1, -2, -3, -4, -5, -6, -7
+NNP_MM_FP32_SIMT, NNP_MM_3XTF32_TC, NNP_MM_TF32_TC, NNP_MM_FP64_SIMT, NNP_MM_3XF16_TC = 0, 1, 2, 3, 4
 STATUS_NAMES = {0: "NNP_OK", -1: "NNP_EINVAL", -2: "NNP_ENOMEM", -3: "NNP_ECUDA", -4: "NNP_ECAPACITY",
                 -5: "NNP_ESTALE", -6: "NNP_EBOX"}
 
