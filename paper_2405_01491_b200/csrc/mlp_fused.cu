@@ -62,15 +62,18 @@ constexpr int EPI_SETS = EPI_WARPS / 4;
 constexpr int EPI_STG_LD = 20;
 constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;
 constexpr int BAR_BYTES = 512;
-constexpr int SMEM_BYTES = 1024 + NW * W_ENTRY_BYTES + NA * A_TILE_BYTES + BAR_BYTES + EPI_WARPS * EPI_STG_BYTES;
+constexpr int GCACHE = 8;               // group descriptors a CTA keeps in shared memory (its tile range spans at most that many)
+constexpr int GROUP_BYTES = 512;
+constexpr int SMEM_BYTES = 1024 + NW * W_ENTRY_BYTES + NA * A_TILE_BYTES + BAR_BYTES + EPI_WARPS * EPI_STG_BYTES + GCACHE * GROUP_BYTES;
 constexpr int THREADS = (2 + EPI_WARPS) * 32;
 constexpr int REGION_COLS = 256;       // two accumulator / operand regions: columns [0, 256) and [256, 512)
-constexpr int MAX_CHUNKS = REGION_COLS / CH;
+constexpr int GRP = 4 * CH;                // columns per operand group: one chunk of every epilogue set, one K block of weights
+constexpr int MAX_GRPS = REGION_COLS / GRP;
 constexpr int ACT_SHIFT = 4;           // activations enter the tensor core multiplied by 2^4
 constexpr float ACT_SCALE = 16.0f;
 constexpr float RANGE_LIMIT = 60000.0f;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
-static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 2) + 8 <= BAR_BYTES, "barrier area");
+static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_GRPS + 2 + 2) + 8 <= BAR_BYTES, "barrier area");
 
 enum FusedEpi {
     FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> operand
@@ -103,6 +106,8 @@ struct alignas(64) FusedGroup {
     int pad_[3];
     FusedStage st[MAX_STAGES];
 };
+
+static_assert(sizeof(FusedGroup) == GROUP_BYTES, "group descriptor size");
 
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
 {
@@ -155,30 +160,23 @@ __device__ __forceinline__ int find_group(const FusedGroup *__restrict__ groups,
 // rows of the two MMAs of a GEMM with N columns: 128 + (N - 128), or N alone
 __device__ __forceinline__ int part_rows(int N, int p) { return p == 0 ? (N > 128 ? 128 : N) : N - 128; }
 
-struct EpiArgs {
-    const FusedGroup *g;
-    const FusedStage *st;
-    int mrow0, lane, set;
-    uint32_t tm_acc;      // TMEM address of this warp's lane quarter at the accumulator's first column
-    uint32_t stg;         // this warp's staging chunk in shared memory
-    uint32_t bar_accf, accf_parity, bar_ready;
-    float alpha;
-    int site, aux;
-};
-
 // One accumulator through one epilogue warp: the 16-column chunks set, set + 4, ... of the warp's 32 rows.
+// Scalar arguments only (registers under the ABI; a struct would travel through local memory, i.e. L2 on this kernel):
+// lane_set = lane | set << 8, accf = accumulator barrier address | parity << 31; returns (max |operand value|, row's
+// partial energy sum).
 template <int EPI>
-__device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float &esum_out)
+__device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0, int lane_set, uint32_t tm_acc, uint32_t stg,
+                                         uint32_t accf, uint32_t bar_ready, float alpha, int aux)
 {
     float vmax = 0.f, esum = 0.f;
     constexpr bool fwd = EPI == FE_FWD || EPI == FE_OUT;
     constexpr bool rd_prev = EPI == FE_BWD || EPI == FE_BWD_ST;   // reads rows of h for CELU'
     constexpr bool to_op = EPI == FE_FWD || EPI == FE_OUT || EPI == FE_BWD;
     constexpr bool wr_rows = EPI == FE_FWD || EPI == FE_BWD_ST || EPI == FE_ST || EPI == FE_RED;
-    const FusedGroup &g = *ea.g;
-    const FusedStage &st = *ea.st;
-    const int N = st.N, M = g.M, mrow0 = ea.mrow0, lane = ea.lane;
-    const uint32_t stg = ea.stg;
+    const FusedGroup &g = *gp;
+    const FusedStage &st = g.st[j];
+    const int lane = lane_set & 31;
+    const int N = st.N, M = g.M;
     const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
     const int sub_r = (lane >> 3) + 4 * ((lane >> 2) & 1), sub_c = (lane & 3) * 4;
     // rows read (h for CELU') and rows written (h stash, or the chain's output)
@@ -188,13 +186,12 @@ __device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float
     const int wr_ld = EPI == FE_FWD ? st.ld_stash : g.ldo;
     const float c_acc = st.c_acc, gs = st.gs, gc = st.gc;
     // everything the chunk loop needs sits in registers: the "memory" clobbers of the asm statements below would make the
-    // compiler re-read any field of ea / st / g it still reaches through a pointer, once per chunk
+    // compiler re-read any field it still reaches through a pointer, once per chunk
     const float *bias = st.bias, *w4p = g.w4;
-    const uint32_t tm_acc = ea.tm_acc, bar_ready = ea.bar_ready;
-    const int c_first = ea.set * CH;
-    const float inv_alpha = 1.0f / ea.alpha;
-    const float a16 = ea.alpha * ACT_SCALE;                               // 16 h = max(16 z, 0) + 16 alpha (e - 1)
-    const float ce = 1.4426950408889634f / (ea.alpha * ACT_SCALE);       // e = 2^(min(16 z, 0) ce)
+    const int c_first = (lane_set >> 8) * CH;
+    const float inv_alpha = 1.0f / alpha;
+    const float a16 = alpha * ACT_SCALE;                               // 16 h = max(16 z, 0) + 16 alpha (e - 1)
+    const float ce = 1.4426950408889634f / (alpha * ACT_SCALE);       // e = 2^(min(16 z, 0) ce)
     float4 pre[4];
     auto prefetch = [&](int c0) {
         const float *cb = rd_base + (size_t)mrow0 * rd_ld + c0;
@@ -205,9 +202,13 @@ __device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float
         }
     };
     if (rd_prev && c_first < N) prefetch(c_first);
-    mbar_wait(ea.bar_accf, ea.accf_parity, ea.site, ea.aux);
+    mbar_wait(accf & 0x7fffffffu, accf >> 31, 400 + j, aux);
     tc_fence_after();
-    for (int c0 = c_first; c0 < N; c0 += EPI_SETS * CH) {
+    for (int c0 = c_first, grp = 0; grp * GRP < N; c0 += GRP, ++grp) {
+        if (c0 >= N) { // the accumulator's last group has no chunk for this set: arrive for it all the same
+            if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * grp);
+            break;
+        }
         uint32_t a[16];
         tmem_ld16(tm_acc + (uint32_t)c0, a);
         if (rd_prev) {
@@ -217,7 +218,7 @@ __device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float
                 asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4), "f"(pre[i].x), "f"(pre[i].y), "f"(pre[i].z), "f"(pre[i].w) : "memory");
             }
             __syncwarp();
-            if (c0 + EPI_SETS * CH < N) prefetch(c0 + EPI_SETS * CH);
+            if (c0 + GRP < N) prefetch(c0 + GRP);
         }
         float ov[16];
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -266,7 +267,7 @@ __device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float
             tc_fence_before();
         }
         __syncwarp();
-        if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * (c0 / CH));
+        if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * grp);
         if (wr_rows) {
             float *cbase = wr_base + (size_t)mrow0 * wr_ld + c0;
 #pragma unroll
@@ -282,8 +283,7 @@ __device__ __noinline__ void epi_stage(const EpiArgs &ea, float &vmax_out, float
             __syncwarp();
         }
     }
-    vmax_out = fmaxf(vmax_out, vmax);
-    esum_out = esum;
+    return make_float2(vmax, esum);
 }
 
 // Regions alternate along the chain AND across tiles: a running count rc of operand generations (the chain input is
@@ -301,19 +301,30 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     // barriers (8 B each)
     const uint32_t bar_wfull = bar_base, bar_wempty = bar_base + 8 * NW;
     const uint32_t bar_afull = bar_base + 16 * NW, bar_aempty = bar_afull + 8 * NA;
-    const uint32_t bar_ready = bar_aempty + 8 * NA;            // [2 regions][MAX_CHUNKS]: operand chunk written
-    const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_CHUNKS;  // [2 regions]: every MMA into the region has completed
+    const uint32_t bar_ready = bar_aempty + 8 * NA;            // [2 regions][MAX_GRPS]: operand group (64 columns) written
+    const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_GRPS;    // [2 regions]: every MMA into the region has completed
     const uint32_t bar_drained = bar_accf + 16;                // the last accumulator of a tile has been read
     const uint32_t tmem_slot = bar_drained + 8;
     const uint32_t stg_base = bar_base + BAR_BYTES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int t_beg = cta_tiles[blockIdx.x], t_end = cta_tiles[blockIdx.x + 1];
+    // The descriptors of the groups this CTA's tiles belong to go to shared memory once: with ~200 KiB of the SM carved
+    // out as shared memory the L1 holds next to nothing, and every field read from the table in global memory was an L2
+    // round trip on the critical path of a stage.  (The tensor map is used from its place in global memory.)
+    const FusedGroup *gsm = reinterpret_cast<const FusedGroup *>(smem_raw + (stg_base + EPI_WARPS * EPI_STG_BYTES - smem_u32(smem_raw)));
+    const int g_lo = t_beg < t_end ? find_group(groups, n_groups, t_beg) : 0;
+    const int n_gc = t_beg < t_end ? find_group(groups, n_groups, t_end - 1) - g_lo + 1 : 0;
+    {
+        const uint4 *src = reinterpret_cast<const uint4 *>(groups + g_lo);
+        uint4 *dst = reinterpret_cast<uint4 *>(const_cast<FusedGroup *>(gsm));
+        for (int k = threadIdx.x; k < n_gc * (GROUP_BYTES / 16); k += THREADS) dst[k] = src[k];
+    }
 
     if (threadIdx.x == 0) {
         for (int e = 0; e < NW; ++e) { mbar_init(bar_wfull + 8 * e, 1); mbar_init(bar_wempty + 8 * e, 1); }
         for (int e = 0; e < NA; ++e) { mbar_init(bar_afull + 8 * e, 1); mbar_init(bar_aempty + 8 * e, 8); }
-        for (int k = 0; k < 2 * MAX_CHUNKS; ++k) mbar_init(bar_ready + 8 * k, 4);
+        for (int k = 0; k < 2 * MAX_GRPS; ++k) mbar_init(bar_ready + 8 * k, EPI_WARPS);
         mbar_init(bar_accf, 1);
         mbar_init(bar_accf + 8, 1);
         mbar_init(bar_drained, EPI_WARPS);
@@ -334,8 +345,8 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         if (lane == 0) {
             uint32_t wi = 0, ai = 0;
             for (int t = t_beg; t < t_end; ++t) {
-                const int gi = find_group(groups, n_groups, t);
-                const FusedGroup &g = groups[gi];
+                const int gi = find_group(gsm, n_gc, t);
+                const FusedGroup &g = gsm[gi];
                 const int m0 = (t - g.tile0) * TILE_M;
                 for (int j = 0; j < g.n_stages; ++j) {
                     const int K = g.st[j].K, N = g.st[j].N;
@@ -347,7 +358,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                                 const uint32_t e = ai % NA;
                                 mbar_wait(bar_aempty + 8 * e, ((ai / NA) & 1) ^ 1, 150, (t - t_beg) * 100 + kb);
                                 mbar_expect_tx(bar_afull + 8 * e, A_TILE_BYTES);
-                                tma_load_2d(a_ring + e * A_TILE_BYTES, &g.mapA, (2 * kb + h) * KBF, m0, bar_afull + 8 * e);
+                                tma_load_2d(a_ring + e * A_TILE_BYTES, &groups[g_lo + gi].mapA, (2 * kb + h) * KBF, m0, bar_afull + 8 * e);
                             }
                         for (int p = 0; p < parts; ++p, ++wi) {
                             const uint32_t e = wi % NW;
@@ -362,38 +373,45 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issue (whole warp walks the loop, one elected lane issues)
-        uint32_t wi = 0, rc = 0, par0 = 0u, par1 = 0u; // parities of the chunk barriers, one bit per chunk and region
-        for (int t = t_beg; t < t_end; ++t) {
-            const int gi = find_group(groups, n_groups, t);
-            const FusedGroup &g = groups[gi];
+        // ===== MMA issue.  The whole warp walks the loop and one elected lane issues; every value an MMA takes is first made
+        // PROVABLY warp-uniform (uni(): a broadcast from lane 0) - the operands of tcgen05.mma live in uniform registers, and
+        // for values the compiler cannot prove uniform (anything loaded from memory) it wraps each MMA in an
+        // elect / R2UR.BROADCAST loop of a dozen dependent instructions (~150 cycles per MMA measured).
+        auto uni = [](uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); };
+        const uint32_t tb = uni(tmem_base), wr = uni(w_ring);
+        const int tu_beg = (int)uni((uint32_t)t_beg), tu_end = (int)uni((uint32_t)t_end);
+        uint32_t wi = 0, rc = 0, par0 = 0u, par1 = 0u; // parities of the group barriers, one bit per group and region
+        for (int t = tu_beg; t < tu_end; ++t) {
+            const int gi = (int)uni((uint32_t)find_group(gsm, n_gc, t));
+            const FusedGroup &g = gsm[gi];
+            const int n_stages = (int)uni((uint32_t)g.n_stages);
             // the first GEMM of a tile writes the region the previous tile's last accumulator was drained from
-            if (t > t_beg) { mbar_wait(bar_drained, (uint32_t)(t - t_beg - 1) & 1, 200, t - t_beg); tc_fence_after(); }
-            for (int j = 0; j < g.n_stages; ++j) {
-                const int K = g.st[j].K, N = g.st[j].N;
+            if (t > tu_beg) { mbar_wait(bar_drained, (uint32_t)(t - tu_beg - 1) & 1, 200, t - tu_beg); tc_fence_after(); }
+            for (int j = 0; j < n_stages; ++j) {
+                const int K = (int)uni((uint32_t)g.st[j].K), N = (int)uni((uint32_t)g.st[j].N);
                 const int parts = N > 128 ? 2 : 1;
                 const uint32_t ra = (rc + (uint32_t)j) & 1u, rd = ra ^ 1u;
-                const uint32_t a_base = tmem_base + ra * REGION_COLS, acc = tmem_base + rd * REGION_COLS;
-                const uint32_t idesc0 = (1u << 4) | ((uint32_t)(part_rows(N, 0) >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
-                const uint32_t idesc1 = parts > 1 ? (1u << 4) | ((uint32_t)(part_rows(N, 1) >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24) : 0u;
-                const int nch_tot = K / CH;
-                for (int kb = 0; kb < (K + KBH - 1) / KBH; ++kb) {
+                const uint32_t a_base = tb + ra * REGION_COLS, acc = tb + rd * REGION_COLS;
+                const uint32_t rows0 = (uint32_t)part_rows(N, 0), rows1 = parts > 1 ? (uint32_t)part_rows(N, 1) : 8u;
+                const uint32_t idesc0 = (1u << 4) | ((rows0 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+                const uint32_t idesc1 = (1u << 4) | ((rows1 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+                const int nch_tot = K / CH, nkb = (K + KBH - 1) / KBH;
+                for (int kb = 0; kb < nkb; ++kb) {
                     const uint32_t e0 = wi % NW, e1 = (wi + 1) % NW;
-                    mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - t_beg) * 100 + kb);
-                    if (parts > 1) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - t_beg) * 100 + kb);
-                    const uint32_t b0 = w_ring + e0 * W_ENTRY_BYTES, b1 = w_ring + e1 * W_ENTRY_BYTES;
-                    const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + (uint32_t)part_rows(N, 0) * 128u);
-                    const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + (uint32_t)(parts > 1 ? part_rows(N, 1) : 8) * 128u);
+                    mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - tu_beg) * 100 + kb);
+                    if (parts > 1) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - tu_beg) * 100 + kb);
+                    const uint32_t b0 = wr + e0 * W_ENTRY_BYTES, b1 = wr + e1 * W_ENTRY_BYTES;
+                    const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + rows0 * 128u);
+                    const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + rows1 * 128u);
                     const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
-                    for (int h = 0; h < nh; ++h) {
-                        const int c = 4 * kb + h;
-                        mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + c), ((ra ? par1 : par0) >> c) & 1u, 240 + j, (t - t_beg) * 100 + c);
-                        if (ra) par1 ^= 1u << c; else par0 ^= 1u << c;
-                        tc_fence_after();
-                        if (elect_one()) {
-                            const uint32_t a_hi = a_base + (uint32_t)(CH * c), a_lo = a_hi + 8;
+                    mbar_wait(bar_ready + 8 * (ra * MAX_GRPS + kb), ((ra ? par1 : par0) >> kb) & 1u, 240 + j, (t - tu_beg) * 100 + kb);
+                    if (ra) par1 ^= 1u << kb; else par0 ^= 1u << kb;
+                    tc_fence_after();
+                    if (elect_one()) {
+                        for (int h = 0; h < nh; ++h) {
+                            const uint32_t a_hi = a_base + (uint32_t)(CH * (4 * kb + h)), a_lo = a_hi + 8;
                             const uint64_t koff = (uint64_t)(2 * h); // 16 fp16 = 32 B along the swizzled row
-                            const uint32_t acc_on = c ? 1u : 0u;
+                            const uint32_t acc_on = (kb | h) ? 1u : 0u;
                             mma_f16_ts(acc, a_lo, d0hi + koff, idesc0, acc_on);
                             mma_f16_ts(acc, a_hi, d0lo + koff, idesc0, 1u);
                             mma_f16_ts(acc, a_hi, d0hi + koff, idesc0, 1u);
@@ -402,18 +420,16 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                                 mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
                                 mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
                             }
-                            if (h + 1 == nh) {
-                                tc_commit(bar_wempty + 8 * e0);
-                                if (parts > 1) tc_commit(bar_wempty + 8 * e1);
-                                if (c + 1 == nch_tot) tc_commit(bar_accf + 8 * rd);
-                            }
                         }
-                        __syncwarp();
+                        tc_commit(bar_wempty + 8 * e0);
+                        if (parts > 1) tc_commit(bar_wempty + 8 * e1);
+                        if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
                     }
+                    __syncwarp();
                     wi += parts;
                 }
             }
-            rc += (uint32_t)g.n_stages + 1u;
+            rc += (uint32_t)n_stages + 1u;
         }
     } else {
         // ===== epilogue: warps 2..17; warp -> TMEM lane quarter warp & 3; set s = (warp - 2) / 4 takes the 16-column chunks
@@ -427,8 +443,8 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         uint32_t rc = 0, use0 = 0u, use1 = 0u, a_cnt = 0;
         float vmax = 0.f;
         for (int t = t_beg; t < t_end; ++t) {
-            const int gi = find_group(groups, n_groups, t);
-            const FusedGroup &g = groups[gi];
+            const int gi = find_group(gsm, n_gc, t);
+            const FusedGroup &g = gsm[gi];
             const int m0 = (t - g.tile0) * TILE_M;
             const int mrow0 = m0 + quarter * 32;
             const int m = mrow0 + lane;
@@ -438,7 +454,11 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                 // previous tile's last GEMM, which this warp has seen complete (accumulator barrier of that GEMM).
                 const int nch0 = g.st[0].K / CH;
                 const uint32_t r0 = rc & 1u;
-                for (int c = set; c < nch0; c += EPI_SETS) {
+                for (int c = set, grp = 0; 4 * grp < nch0; c += EPI_SETS, ++grp) {
+                    if (c >= nch0) {
+                        if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_GRPS + grp));
+                        break;
+                    }
                     const uint32_t ai = a_cnt + (uint32_t)(c >> 1), e = ai % NA;
                     mbar_wait(bar_afull + 8 * e, (ai / NA) & 1, 300, (t - t_beg) * 100 + c);
                     const uint32_t arow = a_ring + e * A_TILE_BYTES + row * 128;
@@ -458,35 +478,35 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_CHUNKS + c));
+                    if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_GRPS + grp));
                 }
                 a_cnt += (uint32_t)(g.st[0].K / KBF);
             }
             for (int j = 0; j < g.n_stages; ++j) {
                 const uint32_t rd = (rc + (uint32_t)j + 1u) & 1u;
-                EpiArgs ea;
-                ea.g = &g; ea.st = &g.st[j]; ea.mrow0 = mrow0; ea.lane = lane; ea.set = set;
-                ea.tm_acc = lane_addr + rd * REGION_COLS; ea.stg = stg;
-                ea.bar_accf = bar_accf + 8 * rd; ea.accf_parity = (rd ? use1 : use0) & 1u;
-                ea.bar_ready = bar_ready + 8 * (rd * MAX_CHUNKS);
-                ea.alpha = alpha; ea.site = 400 + j; ea.aux = t - t_beg;
+                const uint32_t tm_acc = lane_addr + rd * REGION_COLS;
+                const uint32_t accf = (bar_accf + 8 * rd) | (((rd ? use1 : use0) & 1u) << 31);
+                const uint32_t brdy = bar_ready + 8 * (rd * MAX_GRPS);
+                const int lane_set = lane | (set << 8), aux = t - t_beg;
                 if (rd) ++use1; else ++use0;
-                float esum = 0.f;
-                switch (g.st[j].epi) {
-                case FE_FWD: epi_stage<FE_FWD>(ea, vmax, esum); break;
-                case FE_OUT: epi_stage<FE_OUT>(ea, vmax, esum); break;
-                case FE_BWD: epi_stage<FE_BWD>(ea, vmax, esum); break;
-                case FE_BWD_ST: epi_stage<FE_BWD_ST>(ea, vmax, esum); break;
-                case FE_ST: epi_stage<FE_ST>(ea, vmax, esum); break;
-                default: epi_stage<FE_RED>(ea, vmax, esum); break;
+                const int epi = g.st[j].epi;
+                float2 r;
+                switch (epi) {
+                case FE_FWD: r = epi_stage<FE_FWD>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
+                case FE_OUT: r = epi_stage<FE_OUT>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
+                case FE_BWD: r = epi_stage<FE_BWD>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
+                case FE_BWD_ST: r = epi_stage<FE_BWD_ST>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
+                case FE_ST: r = epi_stage<FE_ST>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
+                default: r = epi_stage<FE_RED>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
                 }
+                vmax = fmaxf(vmax, r.x);
+                if (epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, r.y * (1.0f / ACT_SCALE));
                 if (j + 1 == g.n_stages) {
                     // the tile's last accumulator has left tensor memory (for this warp): the next tile may overwrite it
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar_drained);
                 }
-                if (g.st[j].epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, esum * (1.0f / ACT_SCALE));
             }
             rc += (uint32_t)g.n_stages + 1u;
         }
@@ -788,6 +808,12 @@ int nnp_fused_setup(nnp_ctx *c)
             if (cta[k] < cta[k - 1]) cta[k] = cta[k - 1];
     }
     f->grid = grid;
+    for (int b = 0; b < grid; ++b) { // the kernel keeps the descriptors of a CTA's groups in shared memory
+        int span = 0;
+        for (size_t q = 0; q < groups.size(); ++q)
+            if (groups[q].tile0 < cta[b + 1] && groups[q].tile0 + groups[q].n_tiles > cta[b]) ++span;
+        if (span > GCACHE) return NNP_OK; // kind stays 0: the six-launch path
+    }
     if (cudaMemcpyAsync(f->d_groups, groups.data(), sizeof(FusedGroup) * groups.size(), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(f->d_cta_tiles, cta.data(), sizeof(int) * (grid + 1), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess) { // the host vectors go out of scope
