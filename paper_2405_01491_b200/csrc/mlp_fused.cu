@@ -63,17 +63,18 @@ constexpr int EPI_STG_LD = 20;
 constexpr int EPI_STG_BYTES = 32 * EPI_STG_LD * 4;
 constexpr int BAR_BYTES = 512;
 constexpr int GCACHE = 8;               // group descriptors a CTA keeps in shared memory (its tile range spans at most that many)
-constexpr int GROUP_BYTES = 512;
-constexpr int SMEM_BYTES = 1024 + NW * W_ENTRY_BYTES + NA * A_TILE_BYTES + BAR_BYTES + EPI_WARPS * EPI_STG_BYTES + GCACHE * GROUP_BYTES;
+constexpr int GROUP_BYTES = 576;
+constexpr int SB_BYTES = 4 * 256 * 4;     // biases of the three forward GEMMs (x 16) and w4 of the current group
+constexpr int SMEM_BYTES = 1024 + NW * W_ENTRY_BYTES + NA * A_TILE_BYTES + BAR_BYTES + EPI_WARPS * EPI_STG_BYTES + GCACHE * GROUP_BYTES + SB_BYTES;
 constexpr int THREADS = (2 + EPI_WARPS) * 32;
 constexpr int REGION_COLS = 256;       // two accumulator / operand regions: columns [0, 256) and [256, 512)
-constexpr int GRP = 4 * CH;                // columns per operand group: one chunk of every epilogue set, one K block of weights
-constexpr int MAX_GRPS = REGION_COLS / GRP;
+constexpr int GRP = 4 * CH;                // columns per round of the epilogue: one chunk of every set, one K block of weights
+constexpr int MAX_CHUNKS = REGION_COLS / CH;
 constexpr int ACT_SHIFT = 4;           // activations enter the tensor core multiplied by 2^4
 constexpr float ACT_SCALE = 16.0f;
 constexpr float RANGE_LIMIT = 60000.0f;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
-static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_GRPS + 2 + 2) + 8 <= BAR_BYTES, "barrier area");
+static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 2) + 8 <= BAR_BYTES, "barrier area");
 
 enum FusedEpi {
     FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> operand
@@ -91,6 +92,7 @@ struct FusedStage {
     const float *bias;   // [N] forward GEMMs: bias * 2^ACT_SHIFT
     float *stash;        // rows of 16 h: written by FE_FWD, read by FE_BWD (already offset to the group's first row)
     int ld_stash;
+    int brow;            // forward GEMMs: row of the shared-memory bias table
     float c_acc;         // forward: acc -> 16 z;  FE_ST / FE_RED: acc -> true value
     float gs, gc;        // reverse: out = acc * fma(min(h, 0), gs, gc)  (the scalings folded into CELU')
 };
@@ -103,7 +105,8 @@ struct alignas(64) FusedGroup {
     float *out;          // output rows of the last GEMM
     int ldo;
     int M, n_stages, tile0, n_tiles;
-    int pad_[3];
+    int h3;              // width of the last hidden layer (length of w4)
+    int pad_[14];
     FusedStage st[MAX_STAGES];
 };
 
@@ -161,12 +164,12 @@ __device__ __forceinline__ int find_group(const FusedGroup *__restrict__ groups,
 __device__ __forceinline__ int part_rows(int N, int p) { return p == 0 ? (N > 128 ? 128 : N) : N - 128; }
 
 // One accumulator through one epilogue warp: the 16-column chunks set, set + 4, ... of the warp's 32 rows.
-// Scalar arguments only (registers under the ABI; a struct would travel through local memory, i.e. L2 on this kernel):
 // lane_set = lane | set << 8, accf = accumulator barrier address | parity << 31; returns (max |operand value|, row's
-// partial energy sum).
+// partial energy sum).  Inlined once per GEMM of a chain (the kernel is specialised per chain, below): as functions called
+// from a loop over the stages, the caller's state went through local memory around every call - which on this kernel is L2.
 template <int EPI>
-__device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0, int lane_set, uint32_t tm_acc, uint32_t stg,
-                                         uint32_t accf, uint32_t bar_ready, float alpha, int aux)
+__device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0, int lane_set, uint32_t tm_acc, uint32_t stg,
+                                         uint32_t accf, uint32_t bar_ready, uint32_t sb, float alpha, int aux)
 {
     float vmax = 0.f, esum = 0.f;
     constexpr bool fwd = EPI == FE_FWD || EPI == FE_OUT;
@@ -187,7 +190,7 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
     const float c_acc = st.c_acc, gs = st.gs, gc = st.gc;
     // everything the chunk loop needs sits in registers: the "memory" clobbers of the asm statements below would make the
     // compiler re-read any field it still reaches through a pointer, once per chunk
-    const float *bias = st.bias, *w4p = g.w4;
+    const uint32_t sbias = sb + (uint32_t)st.brow * (REGION_COLS * 4), sw4 = sb + 3u * (REGION_COLS * 4);
     const int c_first = (lane_set >> 8) * CH;
     const float inv_alpha = 1.0f / alpha;
     const float a16 = alpha * ACT_SCALE;                               // 16 h = max(16 z, 0) + 16 alpha (e - 1)
@@ -204,11 +207,7 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
     if (rd_prev && c_first < N) prefetch(c_first);
     mbar_wait(accf & 0x7fffffffu, accf >> 31, 400 + j, aux);
     tc_fence_after();
-    for (int c0 = c_first, grp = 0; grp * GRP < N; c0 += GRP, ++grp) {
-        if (c0 >= N) { // the accumulator's last group has no chunk for this set: arrive for it all the same
-            if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * grp);
-            break;
-        }
+    for (int c0 = c_first; c0 < N; c0 += GRP) {
         uint32_t a[16];
         tmem_ld16(tm_acc + (uint32_t)c0, a);
         if (rd_prev) {
@@ -225,8 +224,8 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f), w4v = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (fwd) x4 = __ldg(reinterpret_cast<const float4 *>(bias + c0) + q);
-            if (EPI == FE_OUT) w4v = __ldg(reinterpret_cast<const float4 *>(w4p + c0) + q);
+            if (fwd) asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x4.x), "=f"(x4.y), "=f"(x4.z), "=f"(x4.w) : "r"(sbias + (uint32_t)(c0 + 4 * q) * 4));
+            if (EPI == FE_OUT) asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(w4v.x), "=f"(w4v.y), "=f"(w4v.z), "=f"(w4v.w) : "r"(sw4 + (uint32_t)(c0 + 4 * q) * 4));
             if (rd_prev) asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x4.x), "=f"(x4.y), "=f"(x4.z), "=f"(x4.w) : "r"(my_row + q * 16));
             const float xq[4] = {x4.x, x4.y, x4.z, x4.w};
             const float wq[4] = {w4v.x, w4v.y, w4v.z, w4v.w};
@@ -257,7 +256,11 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
             split16(ov, sl);
             tmem_st16(tm_acc + (uint32_t)c0, sl); // hi / lo of the chunk go back into the accumulator's own columns
         }
+#ifdef EXP_NO_STASH
+        if (wr_rows && EPI != FE_FWD) {
+#else
         if (wr_rows) {
+#endif
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + q * 16), "f"(ov[4 * q]), "f"(ov[4 * q + 1]), "f"(ov[4 * q + 2]), "f"(ov[4 * q + 3]) : "memory");
@@ -267,8 +270,12 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
             tc_fence_before();
         }
         __syncwarp();
-        if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * grp);
+        if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * (c0 / CH));
+#ifdef EXP_NO_STASH
+        if (wr_rows && EPI != FE_FWD) {
+#else
         if (wr_rows) {
+#endif
             float *cbase = wr_base + (size_t)mrow0 * wr_ld + c0;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
@@ -276,8 +283,12 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
                 if (mrow0 + r < M) {
                     float4 v;
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
+#ifndef EXP_NO_STG
                     if (EPI == FE_RED) atomicAdd(reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c), v);
                     else *reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c) = v;
+#else
+                    if (v.x == 123.456f) *reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c) = v;
+#endif
                 }
             }
             __syncwarp();
@@ -291,6 +302,17 @@ __device__ __noinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0,
 // generation q the region q & 1, so the input of tile t+1 goes where the last GEMM of tile t took its operand from while
 // the last accumulator of tile t is still being drained from the other one.
 
+// Chains (template parameter of the kernel): 0 full, one network (F1 F2 F3 B3 B2 B1 -> dE/dG stored); 1 full, ensemble
+// (dE/dG accumulated with reductions); 2 middle (F2 F3 B3 B2 -> delta1 in place).
+enum { CHAIN_FULL = 0, CHAIN_FULL_RED = 1, CHAIN_MIDDLE = 2 };
+__host__ __device__ constexpr int chain_len(int chain) { return chain == CHAIN_MIDDLE ? 4 : 6; }
+__host__ __device__ constexpr int chain_epi(int chain, int j)
+{
+    return chain == CHAIN_MIDDLE ? (j == 0 ? FE_FWD : j == 1 ? FE_OUT : j == 2 ? FE_BWD : FE_BWD_ST)
+                                 : (j < 2 ? FE_FWD : j == 2 ? FE_OUT : j < 5 ? FE_BWD : chain == CHAIN_FULL_RED ? FE_RED : FE_ST);
+}
+
+template <int CHAIN>
 __global__ void __launch_bounds__(THREADS, 1)
 k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__restrict__ cta_tiles, float alpha, int *__restrict__ flags)
 {
@@ -301,8 +323,8 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     // barriers (8 B each)
     const uint32_t bar_wfull = bar_base, bar_wempty = bar_base + 8 * NW;
     const uint32_t bar_afull = bar_base + 16 * NW, bar_aempty = bar_afull + 8 * NA;
-    const uint32_t bar_ready = bar_aempty + 8 * NA;            // [2 regions][MAX_GRPS]: operand group (64 columns) written
-    const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_GRPS;    // [2 regions]: every MMA into the region has completed
+    const uint32_t bar_ready = bar_aempty + 8 * NA;            // [2 regions][MAX_CHUNKS]: operand chunk written
+    const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_CHUNKS;  // [2 regions]: every MMA into the region has completed
     const uint32_t bar_drained = bar_accf + 16;                // the last accumulator of a tile has been read
     const uint32_t tmem_slot = bar_drained + 8;
     const uint32_t stg_base = bar_base + BAR_BYTES;
@@ -312,6 +334,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     // The descriptors of the groups this CTA's tiles belong to go to shared memory once: with ~200 KiB of the SM carved
     // out as shared memory the L1 holds next to nothing, and every field read from the table in global memory was an L2
     // round trip on the critical path of a stage.  (The tensor map is used from its place in global memory.)
+    const uint32_t sb_base = stg_base + EPI_WARPS * EPI_STG_BYTES + GCACHE * GROUP_BYTES;
     const FusedGroup *gsm = reinterpret_cast<const FusedGroup *>(smem_raw + (stg_base + EPI_WARPS * EPI_STG_BYTES - smem_u32(smem_raw)));
     const int g_lo = t_beg < t_end ? find_group(groups, n_groups, t_beg) : 0;
     const int n_gc = t_beg < t_end ? find_group(groups, n_groups, t_end - 1) - g_lo + 1 : 0;
@@ -324,7 +347,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     if (threadIdx.x == 0) {
         for (int e = 0; e < NW; ++e) { mbar_init(bar_wfull + 8 * e, 1); mbar_init(bar_wempty + 8 * e, 1); }
         for (int e = 0; e < NA; ++e) { mbar_init(bar_afull + 8 * e, 1); mbar_init(bar_aempty + 8 * e, 8); }
-        for (int k = 0; k < 2 * MAX_GRPS; ++k) mbar_init(bar_ready + 8 * k, EPI_WARPS);
+        for (int k = 0; k < 2 * MAX_CHUNKS; ++k) mbar_init(bar_ready + 8 * k, 4);
         mbar_init(bar_accf, 1);
         mbar_init(bar_accf + 8, 1);
         mbar_init(bar_drained, EPI_WARPS);
@@ -404,14 +427,15 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                     const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + rows0 * 128u);
                     const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + rows1 * 128u);
                     const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
-                    mbar_wait(bar_ready + 8 * (ra * MAX_GRPS + kb), ((ra ? par1 : par0) >> kb) & 1u, 240 + j, (t - tu_beg) * 100 + kb);
-                    if (ra) par1 ^= 1u << kb; else par0 ^= 1u << kb;
-                    tc_fence_after();
-                    if (elect_one()) {
-                        for (int h = 0; h < nh; ++h) {
-                            const uint32_t a_hi = a_base + (uint32_t)(CH * (4 * kb + h)), a_lo = a_hi + 8;
+                    for (int h = 0; h < nh; ++h) {
+                        const int c = 4 * kb + h;
+                        mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + c), ((ra ? par1 : par0) >> c) & 1u, 240 + j, (t - tu_beg) * 100 + c);
+                        if (ra) par1 ^= 1u << c; else par0 ^= 1u << c;
+                        tc_fence_after();
+                        if (elect_one()) {
+                            const uint32_t a_hi = a_base + (uint32_t)(CH * c), a_lo = a_hi + 8;
                             const uint64_t koff = (uint64_t)(2 * h); // 16 fp16 = 32 B along the swizzled row
-                            const uint32_t acc_on = (kb | h) ? 1u : 0u;
+                            const uint32_t acc_on = c ? 1u : 0u;
                             mma_f16_ts(acc, a_lo, d0hi + koff, idesc0, acc_on);
                             mma_f16_ts(acc, a_hi, d0lo + koff, idesc0, 1u);
                             mma_f16_ts(acc, a_hi, d0hi + koff, idesc0, 1u);
@@ -420,12 +444,14 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                                 mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
                                 mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
                             }
+                            if (h + 1 == nh) {
+                                tc_commit(bar_wempty + 8 * e0);
+                                if (parts > 1) tc_commit(bar_wempty + 8 * e1);
+                                if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
+                            }
                         }
-                        tc_commit(bar_wempty + 8 * e0);
-                        if (parts > 1) tc_commit(bar_wempty + 8 * e1);
-                        if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
+                        __syncwarp();
                     }
-                    __syncwarp();
                     wi += parts;
                 }
             }
@@ -441,10 +467,23 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
         const uint32_t stg = stg_base + (uint32_t)ew * EPI_STG_BYTES;
         uint32_t rc = 0, use0 = 0u, use1 = 0u, a_cnt = 0;
+        int cur_gi = -1;
         float vmax = 0.f;
         for (int t = t_beg; t < t_end; ++t) {
             const int gi = find_group(gsm, n_gc, t);
             const FusedGroup &g = gsm[gi];
+            if (gi != cur_gi) {
+                // biases (x 16) of the forward GEMMs and w4 of this group -> shared memory (a chunk reads them as broadcasts)
+                asm volatile("bar.sync 1, %0;" ::"n"(EPI_WARPS * 32) : "memory"); // nobody still reads the previous group's
+                float *sbp = reinterpret_cast<float *>(smem_raw + (sb_base - smem_u32(smem_raw)));
+                const int et = (int)threadIdx.x - 64;
+                for (int j = 0; j < g.n_stages; ++j)
+                    if (g.st[j].epi == FE_FWD || g.st[j].epi == FE_OUT)
+                        for (int k = et; k < g.st[j].N; k += EPI_WARPS * 32) sbp[g.st[j].brow * REGION_COLS + k] = g.st[j].bias[k];
+                for (int k = et; k < g.h3; k += EPI_WARPS * 32) sbp[3 * REGION_COLS + k] = g.w4[k];
+                asm volatile("bar.sync 1, %0;" ::"n"(EPI_WARPS * 32) : "memory");
+                cur_gi = gi;
+            }
             const int m0 = (t - g.tile0) * TILE_M;
             const int mrow0 = m0 + quarter * 32;
             const int m = mrow0 + lane;
@@ -454,11 +493,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                 // previous tile's last GEMM, which this warp has seen complete (accumulator barrier of that GEMM).
                 const int nch0 = g.st[0].K / CH;
                 const uint32_t r0 = rc & 1u;
-                for (int c = set, grp = 0; 4 * grp < nch0; c += EPI_SETS, ++grp) {
-                    if (c >= nch0) {
-                        if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_GRPS + grp));
-                        break;
-                    }
+                for (int c = set; c < nch0; c += EPI_SETS) {
                     const uint32_t ai = a_cnt + (uint32_t)(c >> 1), e = ai % NA;
                     mbar_wait(bar_afull + 8 * e, (ai / NA) & 1, 300, (t - t_beg) * 100 + c);
                     const uint32_t arow = a_ring + e * A_TILE_BYTES + row * 128;
@@ -478,36 +513,28 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_GRPS + grp));
+                    if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_CHUNKS + c));
                 }
                 a_cnt += (uint32_t)(g.st[0].K / KBF);
             }
-            for (int j = 0; j < g.n_stages; ++j) {
-                const uint32_t rd = (rc + (uint32_t)j + 1u) & 1u;
-                const uint32_t tm_acc = lane_addr + rd * REGION_COLS;
-                const uint32_t accf = (bar_accf + 8 * rd) | (((rd ? use1 : use0) & 1u) << 31);
-                const uint32_t brdy = bar_ready + 8 * (rd * MAX_GRPS);
-                const int lane_set = lane | (set << 8), aux = t - t_beg;
-                if (rd) ++use1; else ++use0;
-                const int epi = g.st[j].epi;
-                float2 r;
-                switch (epi) {
-                case FE_FWD: r = epi_stage<FE_FWD>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
-                case FE_OUT: r = epi_stage<FE_OUT>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
-                case FE_BWD: r = epi_stage<FE_BWD>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
-                case FE_BWD_ST: r = epi_stage<FE_BWD_ST>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
-                case FE_ST: r = epi_stage<FE_ST>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
-                default: r = epi_stage<FE_RED>(&g, j, mrow0, lane_set, tm_acc, stg, accf, brdy, alpha, aux); break;
-                }
-                vmax = fmaxf(vmax, r.x);
-                if (epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, r.y * (1.0f / ACT_SCALE));
-                if (j + 1 == g.n_stages) {
-                    // the tile's last accumulator has left tensor memory (for this warp): the next tile may overwrite it
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_drained);
-                }
-            }
+            const int lane_set = lane | (set << 8), aux = t - t_beg;
+#define NNP_FUSED_STAGE(J)                                                                                                    \
+    if (J < chain_len(CHAIN)) {                                                                                               \
+        constexpr int epi = chain_epi(CHAIN, J);                                                                              \
+        const uint32_t rd = (rc + (uint32_t)J + 1u) & 1u;                                                                     \
+        const uint32_t accf = (bar_accf + 8 * rd) | (((rd ? use1 : use0) & 1u) << 31);                                        \
+        if (rd) ++use1; else ++use0;                                                                                          \
+        const float2 r = epi_stage<epi>(&g, J, mrow0, lane_set, lane_addr + rd * REGION_COLS, stg, accf,                      \
+                                        bar_ready + 8 * (rd * MAX_CHUNKS), sb_base, alpha, aux);                              \
+        vmax = fmaxf(vmax, r.x);                                                                                              \
+        if (epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, r.y * (1.0f / ACT_SCALE));                                        \
+    }
+            NNP_FUSED_STAGE(0) NNP_FUSED_STAGE(1) NNP_FUSED_STAGE(2) NNP_FUSED_STAGE(3) NNP_FUSED_STAGE(4) NNP_FUSED_STAGE(5)
+#undef NNP_FUSED_STAGE
+            // the tile's last accumulator has left tensor memory (for this warp): the next tile may overwrite it
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_drained);
             rc += (uint32_t)g.n_stages + 1u;
         }
         if (vmax > RANGE_LIMIT) atomicOr(&flags[0], NNP_FLAG_RANGE);
@@ -740,14 +767,16 @@ int nnp_fused_setup(nnp_ctx *c)
             g.w4 = L[3].W;
             g.e_atom = c->e_atom + off;
             g.M = M;
+            g.h3 = h3;
             g.tile0 = tiles;
             g.n_tiles = nnp_div_up(M, TILE_M);
             // acc = sum (16 a)(2^sh w): forward epilogues want 16 z = acc 2^-sh; reverse operand-producing epilogues
             // 16 delta = acc 2^-sh celu'(h) with the stash holding 16 h; output epilogues the true value acc 2^-(sh + 4)
-            auto fwd = [&](int j, int K, int N, int epi, size_t w_off, const float *bias, float *stash, int ld, int sh) {
+            auto fwd = [&](int j, int K, int N, int epi, size_t w_off, const float *bias, float *stash, int ld, int sh, int brow) {
                 FusedStage &st = g.st[j];
                 st.K = K; st.N = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.bias = bias; st.stash = stash; st.ld_stash = ld;
                 st.c_acc = ldexpf(1.0f, -sh);
+                st.brow = brow;
             };
             auto bwd = [&](int j, int K, int N, int epi, size_t w_off, float *stash, int ld, int sh) {
                 FusedStage &st = g.st[j];
@@ -761,9 +790,9 @@ int nnp_fused_setup(nnp_ctx *c)
             if (kind == 1) {
                 g.n_stages = 6;
                 if (!make_map_a(&g.mapA, c->G + (size_t)off * kpad, M, kpad, kpad)) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
-                fwd(0, kpad, h1, FE_FWD, f->w_off[q][0], b16, H0, c->hmax[0], wsh[q][0]);
-                fwd(1, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1]);
-                fwd(2, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2]);
+                fwd(0, kpad, h1, FE_FWD, f->w_off[q][0], b16, H0, c->hmax[0], wsh[q][0], 0);
+                fwd(1, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1], 1);
+                fwd(2, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2], 2);
                 bwd(3, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
                 bwd(4, h2, h1, FE_BWD, f->w_off[q][4], H0, c->hmax[0], wsh[q][1]);
                 bwd(5, h1, kpad, nn > 1 ? FE_RED : FE_ST, f->w_off[q][5], nullptr, 0, wsh[q][0]);
@@ -772,8 +801,8 @@ int nnp_fused_setup(nnp_ctx *c)
             } else {
                 g.n_stages = 4;
                 if (!make_map_a(&g.mapA, H0, M, h1, c->hmax[0])) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
-                fwd(0, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1]);
-                fwd(1, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2]);
+                fwd(0, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1], 1);
+                fwd(1, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2], 2);
                 bwd(2, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
                 bwd(3, h2, h1, FE_BWD_ST, f->w_off[q][4], nullptr, 0, wsh[q][1]);
                 g.out = H0;
@@ -832,9 +861,16 @@ void nnp_launch_mlp_fused(nnp_ctx *c)
     nnp_fused *f = c->fused;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(k_mlp_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaFuncSetAttribute(k_mlp_fused<CHAIN_FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaFuncSetAttribute(k_mlp_fused<CHAIN_FULL_RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaFuncSetAttribute(k_mlp_fused<CHAIN_MIDDLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         attr_set = true;
     }
-    k_mlp_fused<<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
+    if (f->kind == 2)
+        k_mlp_fused<CHAIN_MIDDLE><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
+    else if (c->n_nets > 1)
+        k_mlp_fused<CHAIN_FULL_RED><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
+    else
+        k_mlp_fused<CHAIN_FULL><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
     c->launches += 1;
 }
