@@ -55,7 +55,7 @@ constexpr int CH = 16;                 // K chunk: one tcgen05.mma kind::f16 K s
 constexpr int MAX_STAGES = 6;
 constexpr int NW = 4;                  // weight ring entries
 constexpr int W_ENTRY_BYTES = 32768;   // hi + lo tiles of up to 128 rows x 128 B
-constexpr int NA = 2;                  // ring of input tiles
+constexpr int NA = 3;                  // ring of input tiles
 constexpr int A_TILE_BYTES = TILE_M * KBF * 4;
 constexpr int EPI_WARPS = 16;
 constexpr int EPI_SETS = EPI_WARPS / 4;
@@ -160,9 +160,6 @@ __device__ __forceinline__ int find_group(const FusedGroup *__restrict__ groups,
     return gi;
 }
 
-// rows of the two MMAs of a GEMM with N columns: 128 + (N - 128), or N alone
-__device__ __forceinline__ int part_rows(int N, int p) { return p == 0 ? (N > 128 ? 128 : N) : N - 128; }
-
 // One accumulator through one epilogue warp: the 16-column chunks set, set + 4, ... of the warp's 32 rows.
 // lane_set = lane | set << 8, accf = accumulator barrier address | parity << 31; returns (max |operand value|, row's
 // partial energy sum).  Inlined once per GEMM of a chain (the kernel is specialised per chain, below): as functions called
@@ -256,11 +253,7 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
             split16(ov, sl);
             tmem_st16(tm_acc + (uint32_t)c0, sl); // hi / lo of the chunk go back into the accumulator's own columns
         }
-#ifdef EXP_NO_STASH
-        if (wr_rows && EPI != FE_FWD) {
-#else
         if (wr_rows) {
-#endif
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(my_row + q * 16), "f"(ov[4 * q]), "f"(ov[4 * q + 1]), "f"(ov[4 * q + 2]), "f"(ov[4 * q + 3]) : "memory");
@@ -271,11 +264,7 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
         }
         __syncwarp();
         if (to_op && lane == 0) mbar_arrive(bar_ready + 8 * (c0 / CH));
-#ifdef EXP_NO_STASH
-        if (wr_rows && EPI != FE_FWD) {
-#else
         if (wr_rows) {
-#endif
             float *cbase = wr_base + (size_t)mrow0 * wr_ld + c0;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
@@ -283,12 +272,8 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
                 if (mrow0 + r < M) {
                     float4 v;
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(stg + (uint32_t)(r * EPI_STG_LD + sub_c) * 4));
-#ifndef EXP_NO_STG
                     if (EPI == FE_RED) atomicAdd(reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c), v);
                     else *reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c) = v;
-#else
-                    if (v.x == 123.456f) *reinterpret_cast<float4 *>(cbase + (size_t)r * wr_ld + sub_c) = v;
-#endif
                 }
             }
             __syncwarp();
@@ -296,6 +281,10 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
     }
     return make_float2(vmax, esum);
 }
+
+// rows of the two MMAs of a GEMM with N columns: 128 + (N - 128), or N alone (one MMA with N > 128 and its operand in
+// tensor memory ran at a quarter of the rate of two with N <= 128: measured, 370 against 2 x 64 cycles at N = 192)
+__device__ __forceinline__ int part_rows(int N, int p) { return p == 0 ? (N > 128 ? 128 : N) : N - 128; }
 
 // Regions alternate along the chain AND across tiles: a running count rc of operand generations (the chain input is
 // generation rc, the accumulator of GEMM j generation rc + 1 + j, the next tile starts at rc + n_stages + 1) gives
@@ -364,26 +353,39 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
     if (warp == 0) {
-        // ===== producer: everything that arrives in shared memory, in its order of use
+        // ===== producer: everything that arrives in shared memory.  Weights in their order of use; the first NA input tiles
+        // of the NEXT tile are requested while this tile is in its third GEMM (their ring entries are free by then), so that
+        // the conversion at the start of a tile never waits for a load queued behind the whole weight stream.
         if (lane == 0) {
             uint32_t wi = 0, ai = 0;
+            int pre = 0; // input tiles of tile t already requested
             for (int t = t_beg; t < t_end; ++t) {
                 const int gi = find_group(gsm, n_gc, t);
                 const FusedGroup &g = gsm[gi];
                 const int m0 = (t - g.tile0) * TILE_M;
-                for (int j = 0; j < g.n_stages; ++j) {
+                const int n_stages = g.n_stages;
+                auto load_a = [&](const FusedGroup &gg, int gidx, int row0, int k) {
+                    const uint32_t e = ai % NA;
+                    mbar_wait(bar_aempty + 8 * e, ((ai / NA) & 1) ^ 1, 150, k);
+                    mbar_expect_tx(bar_afull + 8 * e, A_TILE_BYTES);
+                    tma_load_2d(a_ring + e * A_TILE_BYTES, &groups[g_lo + gidx].mapA, k * KBF, row0, bar_afull + 8 * e);
+                    ++ai;
+                };
+                int a_next = pre; // next input tile (32 columns) of this tile to request
+                pre = 0;
+                for (int j = 0; j < n_stages; ++j) {
                     const int K = g.st[j].K, N = g.st[j].N;
-                    const int parts = N > 128 ? 2 : 1;
                     const uint8_t *wsrc = g.wblob + g.st[j].w_off;
+                    if (j == 2 && t + 1 < t_end) {
+                        const int gn = find_group(gsm, n_gc, t + 1);
+                        const FusedGroup &g2 = gsm[gn];
+                        const int nka = g2.st[0].K / KBF;
+                        for (; pre < NA && pre < nka; ++pre) load_a(g2, gn, (t + 1 - g2.tile0) * TILE_M, pre);
+                    }
                     for (int kb = 0; kb < (K + KBH - 1) / KBH; ++kb) {
                         if (j == 0)
-                            for (int h = 0; h < 2 && (2 * kb + h) * KBF < K; ++h, ++ai) {
-                                const uint32_t e = ai % NA;
-                                mbar_wait(bar_aempty + 8 * e, ((ai / NA) & 1) ^ 1, 150, (t - t_beg) * 100 + kb);
-                                mbar_expect_tx(bar_afull + 8 * e, A_TILE_BYTES);
-                                tma_load_2d(a_ring + e * A_TILE_BYTES, &groups[g_lo + gi].mapA, (2 * kb + h) * KBF, m0, bar_afull + 8 * e);
-                            }
-                        for (int p = 0; p < parts; ++p, ++wi) {
+                            for (; a_next < 2 * kb + 2 && a_next * KBF < K; ++a_next) load_a(g, gi, m0, a_next);
+                        for (int p = 0; p < (N > 128 ? 2 : 1); ++p, ++wi) {
                             const uint32_t e = wi % NW;
                             const uint32_t bytes = 2u * (uint32_t)part_rows(N, p) * 128u; // hi tile, lo tile behind it
                             mbar_wait(bar_wempty + 8 * e, ((wi / NW) & 1) ^ 1, 100 + j, (t - t_beg) * 100 + kb);
@@ -412,47 +414,54 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
             if (t > tu_beg) { mbar_wait(bar_drained, (uint32_t)(t - tu_beg - 1) & 1, 200, t - tu_beg); tc_fence_after(); }
             for (int j = 0; j < n_stages; ++j) {
                 const int K = (int)uni((uint32_t)g.st[j].K), N = (int)uni((uint32_t)g.st[j].N);
-                const int parts = N > 128 ? 2 : 1;
+                const bool wide = N > 128; // two MMAs per product term: columns [0, 128) and [128, N)
                 const uint32_t ra = (rc + (uint32_t)j) & 1u, rd = ra ^ 1u;
                 const uint32_t a_base = tb + ra * REGION_COLS, acc = tb + rd * REGION_COLS;
-                const uint32_t rows0 = (uint32_t)part_rows(N, 0), rows1 = parts > 1 ? (uint32_t)part_rows(N, 1) : 8u;
+                const uint32_t rows0 = (uint32_t)part_rows(N, 0), rows1 = wide ? (uint32_t)part_rows(N, 1) : 8u;
                 const uint32_t idesc0 = (1u << 4) | ((rows0 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
                 const uint32_t idesc1 = (1u << 4) | ((rows1 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
                 const int nch_tot = K / CH, nkb = (K + KBH - 1) / KBH;
                 for (int kb = 0; kb < nkb; ++kb) {
                     const uint32_t e0 = wi % NW, e1 = (wi + 1) % NW;
                     mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - tu_beg) * 100 + kb);
-                    if (parts > 1) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - tu_beg) * 100 + kb);
+                    if (wide) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - tu_beg) * 100 + kb);
                     const uint32_t b0 = wr + e0 * W_ENTRY_BYTES, b1 = wr + e1 * W_ENTRY_BYTES;
                     const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + rows0 * 128u);
                     const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + rows1 * 128u);
                     const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
-                    for (int h = 0; h < nh; ++h) {
-                        const int c = 4 * kb + h;
-                        mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + c), ((ra ? par1 : par0) >> c) & 1u, 240 + j, (t - tu_beg) * 100 + c);
-                        if (ra) par1 ^= 1u << c; else par0 ^= 1u << c;
+                    // one wait and one election per chunk (measured against the chunks of a K block in one batch, or the first
+                    // alone and the other three together: 0.203 against 0.214 ms for the chain)
+                    for (int h0 = 0; h0 < nh; ++h0) {
+                        const int h1 = h0 + 1;
+                        for (int h = h0; h < h1; ++h) {
+                            const int c = 4 * kb + h;
+                            mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + c), ((ra ? par1 : par0) >> c) & 1u, 240 + j, (t - tu_beg) * 100 + c);
+                            if (ra) par1 ^= 1u << c; else par0 ^= 1u << c;
+                        }
                         tc_fence_after();
                         if (elect_one()) {
-                            const uint32_t a_hi = a_base + (uint32_t)(CH * c), a_lo = a_hi + 8;
-                            const uint64_t koff = (uint64_t)(2 * h); // 16 fp16 = 32 B along the swizzled row
-                            const uint32_t acc_on = c ? 1u : 0u;
-                            mma_f16_ts(acc, a_lo, d0hi + koff, idesc0, acc_on);
-                            mma_f16_ts(acc, a_hi, d0lo + koff, idesc0, 1u);
-                            mma_f16_ts(acc, a_hi, d0hi + koff, idesc0, 1u);
-                            if (parts > 1) {
-                                mma_f16_ts(acc + 128, a_lo, d1hi + koff, idesc1, acc_on);
-                                mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
-                                mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
+                            for (int h = h0; h < h1; ++h) {
+                                const int c = 4 * kb + h;
+                                const uint32_t a_hi = a_base + (uint32_t)(CH * c), a_lo = a_hi + 8;
+                                const uint64_t koff = (uint64_t)(2 * h); // 16 fp16 = 32 B along the swizzled row
+                                mma_f16_ts(acc, a_lo, d0hi + koff, idesc0, c ? 1u : 0u);
+                                mma_f16_ts(acc, a_hi, d0lo + koff, idesc0, 1u);
+                                mma_f16_ts(acc, a_hi, d0hi + koff, idesc0, 1u);
+                                if (wide) {
+                                    mma_f16_ts(acc + 128, a_lo, d1hi + koff, idesc1, c ? 1u : 0u);
+                                    mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
+                                    mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
+                                }
                             }
-                            if (h + 1 == nh) {
+                            if (h1 == nh) {
                                 tc_commit(bar_wempty + 8 * e0);
-                                if (parts > 1) tc_commit(bar_wempty + 8 * e1);
+                                if (wide) tc_commit(bar_wempty + 8 * e1);
                                 if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
                             }
                         }
                         __syncwarp();
                     }
-                    wi += parts;
+                    wi += wide ? 2u : 1u;
                 }
             }
             rc += (uint32_t)n_stages + 1u;

@@ -33,11 +33,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int sit
     for (uint32_t it = 0; it < limit; ++it) {
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
-#ifdef EXP_HINT
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, 0x989680;\n\t"
-#else
             "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-#endif
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(done)
             : "r"(bar), "r"(parity)
