@@ -237,7 +237,8 @@ def run_eval_config(args):
                    for s in range(7))
         ach = 2.0 * 2.0 * macs * n_nets / (mlp_ms * 1e-3) / 1e12           # forward + input gradient
         peak = pk["bf16_sus"] * 0.5 if args.mm_mode in (1, 2, 4) else fp32_peak
-        roof = {"kernel": "mlp_all_layers (6 grouped GEMM launches per network batch)", "bound": "tensor" if args.mm_mode in (1, 2, 4) else "alu",
+        roof = {"kernel": "mlp_all_layers (mm_mode 4: fused chain [+ layer 1 / dE/dG launches]; else 6 grouped GEMM launches per network batch)",
+                "bound": "tensor" if args.mm_mode in (1, 2, 4) else "alu",
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
                 "peak_source": "%s sustained bf16 cuBLAS x 0.5; fp32-equivalent flops counted once" % pk["source"]}
     elif dom in ("aev_forward", "aev_backward_scatter"):
@@ -562,6 +563,15 @@ def _roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
                                 "mlp_bwd_l3": h3 * h2, "mlp_bwd_l2": h2 * h1, "mlp_bwd_l1_dEdG": h1 * kpad}[op]
         return tot
 
+    if stage == "mlp_fused_chain":
+        ops = (["mlp_fwd_l1", "mlp_bwd_l1_dEdG"] if kpad <= 256 else []) + ["mlp_fwd_l2", "mlp_fwd_l3_out", "mlp_bwd_l3", "mlp_bwd_l2"]
+        flops = 2.0 * sum(macs(op) for op in ops)
+        ach = flops / (ms * 1e-3) / 1e12 if ms else 0.0
+        peak = pk["bf16_sus"]
+        return {"kernel": "k_mlp_fused (%d GEMMs of the MLP chain in one launch, fp16 hi/lo split operands)" % len(ops), "bound": "tensor",
+                "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                "peak_source": "%s sustained bf16 cuBLAS %.1f TF/s (fp16 operands run at the bf16 rate); algorithmic fp32 flops counted "
+                               "once (the 3xF16 split issues 3 MMAs per product: a perfect kernel reads 1/3)" % (pk["source"], pk["bf16_sus"])}
     if stage.startswith("mlp"):
         flops = 2.0 * macs(stage)
         ach = flops / (ms * 1e-3) / 1e12 if ms else 0.0
@@ -595,7 +605,8 @@ def main():
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mm-mode", type=int, default=int(os.environ.get("NNP_MM_MODE", "1")))
+    ap.add_argument("--mm-mode", type=int, default=int(os.environ.get("NNP_MM_MODE", "4")),
+                    help="0 fp32 SIMT, 1 3xTF32 tcgen05 (six launches), 2 TF32, 3 fp64 SIMT, 4 3xF16 fused tcgen05 chain (default)")
     ap.add_argument("--waters", type=int, default=N_WATERS)
     ap.add_argument("--force-scale", type=float, default=None)
     ap.add_argument("--e2e-steps", type=int, default=200)

@@ -190,8 +190,10 @@ int nnp_md_step_host(nnp_ctx *ctx, float *h_xyz, float *h_vel, int n_steps, doub
  * nnp_profile_read synchronises and returns, per stage, the summed milliseconds and the number of samples:
  * 0 kick+drift, 1 neighbour build (all its kernels; near zero on steps without a rebuild), 2 AEV forward,
  * 3..5 MLP forward layers 1..3 (layer 3 includes the output layer), 6..8 MLP reverse layers 3..1 (8 = dE/dG),
- * 9 energy sum, 10 AEV reverse + force scatter, 11 kick + kinetic energy.  Arrays of NNP_N_STAGES entries. */
-#define NNP_N_STAGES 12
+ * 9 energy sum, 10 AEV reverse + force scatter, 11 kick + kinetic energy, 12 the fused MLP chain of mm_mode 4 (all six
+ * GEMMs, or the four middle ones when the active AEV columns exceed 256: layers 1 and dE/dG are then stages 3 and 8).
+ * Arrays of NNP_N_STAGES entries. */
+#define NNP_N_STAGES 13
 int nnp_profile(nnp_ctx *ctx, int stride);
 int nnp_profile_read(nnp_ctx *ctx, double *h_ms_sum, int64_t *h_samples);
 

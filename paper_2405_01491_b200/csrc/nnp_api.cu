@@ -398,7 +398,7 @@ int run_forces(nnp_ctx *c)
     if (fk == 1) {
         if (c->n_nets > 1) CU(c, cudaMemsetAsync(c->dG, 0, sizeof(float) * (size_t)c->n * c->aev.kpad, c->stream));
         nnp_launch_mlp_fused(c);
-        nnp_prof_mark(c, 3);
+        nnp_prof_mark(c, 12);
     } else {
         for (int net0 = 0; net0 < c->n_nets; net0 += nb)
             for (int op = 0; op < (fk == 2 ? 1 : 5); ++op) {
@@ -409,7 +409,7 @@ int run_forces(nnp_ctx *c)
             }
         if (fk == 2) {
             nnp_launch_mlp_fused(c);
-            nnp_prof_mark(c, 4);
+            nnp_prof_mark(c, 12);
         }
         if (nb > 1) {
             // dE/dG sums over the networks: the groups of all batched networks add into the same rows with vector

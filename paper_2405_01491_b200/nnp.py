@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
 NNP_OK, NNP_EINVAL, NNP_ENOMEM, NNP_ECUDA, NNP_ECAPACITY, NNP_ESTALE, NNP_EBOX, NNP_ERANGE = 0, -1, -2, -3, -4, -5, -6, -7
 NNP_MM_FP32_SIMT, NNP_MM_3XTF32_TC, NNP_MM_TF32_TC, NNP_MM_FP64_SIMT, NNP_MM_3XF16_TC = 0, 1, 2, 3, 4
 STATUS_NAMES = {0: "NNP_OK", -1: "NNP_EINVAL", -2: "NNP_ENOMEM", -3: "NNP_ECUDA", -4: "NNP_ECAPACITY",
-                -5: "NNP_ESTALE", -6: "NNP_EBOX"}
+                -5: "NNP_ESTALE", -6: "NNP_EBOX", -7: "NNP_ERANGE"}
 
 EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp_set_positions",
            "nnp_build_neighbors", "nnp_get_neighbors", "nnp_energy_forces", "nnp_get_aev",
@@ -215,9 +215,10 @@ def nnp_md_step_host(ctx, h_xyz, h_vel, n_steps, h_epot, h_ekin):
     return _check(ctx, lib().nnp_md_step_host(ctx, _ptr(h_xyz), _ptr(h_vel), int(n_steps), _ptr(h_epot), _ptr(h_ekin)))
 
 
-NNP_N_STAGES = 12
+NNP_N_STAGES = 13
 STAGE_NAMES = ["kick_drift", "neighbor_build", "aev_forward", "mlp_fwd_l1", "mlp_fwd_l2", "mlp_fwd_l3_out",
-               "mlp_bwd_l3", "mlp_bwd_l2", "mlp_bwd_l1_dEdG", "energy_sum", "aev_backward_scatter", "kick_ekin"]
+               "mlp_bwd_l3", "mlp_bwd_l2", "mlp_bwd_l1_dEdG", "energy_sum", "aev_backward_scatter", "kick_ekin",
+               "mlp_fused_chain"]
 
 
 def nnp_profile(ctx, stride):

@@ -21,7 +21,7 @@ def make_model(n_nets=1, seed=inputs.SEED0, widths=inputs.WIDTHS, scale=FORCE_SC
     return consts, widths, params, omodel
 
 
-MM_MODE = int(os.environ.get("NNP_MM_MODE", "1"))   # default: 3xTF32 tcgen05 (the mode bench.py reports)
+MM_MODE = int(os.environ.get("NNP_MM_MODE", "4"))   # default: the fused 3xF16 tcgen05 chain (the mode bench.py reports)
 
 
 def gpu_create(consts, widths, params, n_nets, max_atoms, max_mols=1, mm_mode=None, cap_r=0, cap_a=0, self_energy=None,

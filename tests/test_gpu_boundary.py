@@ -126,10 +126,12 @@ def test_matmul_modes_at_their_own_bars(model1):
     consts, widths, params, om = model1
     sp, xyz, box = inputs.water_box(343, seed=51)
     err = {m: _errors(m, consts, widths, params, om, sp, xyz, box)
-           for m in (nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_TF32_TC, nnp.NNP_MM_FP64_SIMT)}
+           for m in (nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_TF32_TC, nnp.NNP_MM_FP64_SIMT, nnp.NNP_MM_3XF16_TC)}
     print("mode: (|dE|/|E|, max|dF|)", err)
-    for m in (nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_FP64_SIMT):
+    for m in (nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_FP64_SIMT, nnp.NNP_MM_3XF16_TC):
         assert err[m][0] <= U.E_RTOL and err[m][1] <= U.F_ATOL, (m, err[m])
+    # the fp16 hi/lo split carries the same 11 + 11 bits as the tf32 split: the two fp32-grade tensor-core modes land together
+    assert err[nnp.NNP_MM_3XF16_TC][1] <= 3.0 * err[nnp.NNP_MM_3XTF32_TC][1] + 1e-5
     e2, f2 = err[nnp.NNP_MM_TF32_TC]
     assert e2 < 5e-3 and f2 < 0.3, (e2, f2)                       # its own, looser bar: the right order of magnitude
     assert f2 > U.F_ATOL                                           # ... and it does NOT meet the fp32 force bar

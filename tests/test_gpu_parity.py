@@ -159,16 +159,67 @@ def test_periodic_replica_batch(model1, n_waters, L, n_rep):
 
 
 # ---------------------------------------------------------------- the other matmul modes on an ensemble
-@pytest.mark.parametrize("mm_mode", [nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC], ids=["fp32_simt", "3xtf32_tc"])
+@pytest.mark.parametrize("mm_mode", [nnp.NNP_MM_FP32_SIMT, nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_3XF16_TC], ids=["fp32_simt", "3xtf32_tc", "3xf16_fused"])
 def test_ensemble_in_both_fp32_grade_modes(mm_mode):
-    """Three networks on a 216-water box: the fp32 SIMT path runs the networks one after the other, the tensor-core path
-    batches them into one grouped launch per layer (dE/dG summed by reductions in memory); both meet the bars."""
+    """Three networks on a 216-water box: the fp32 SIMT path runs the networks one after the other, the 3xTF32 path batches
+    them into one grouped launch per layer, the fused 3xF16 chain takes all of them in one launch (dE/dG summed by
+    reductions in memory in both tensor-core paths); all meet the bars."""
     consts, widths, params, om = U.make_model(3, seed=inputs.SEED0 + 21)
     sp, xyz, box = inputs.water_box(216, seed=inputs.SEED0 + 22)
     ctx = U.gpu_create(consts, widths, params, 3, len(sp), mm_mode=mm_mode)
     try:
         Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
         U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, want_e_atom=True))   # reading B8: E is a cancelling sum here
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+@pytest.mark.parametrize("mm_mode", [nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_3XF16_TC], ids=["3xtf32_six_launches", "3xf16_fused"])
+def test_both_tensor_core_modes_on_every_chain(mm_mode):
+    """The suite runs in ONE matmul mode (NNP_MM_MODE, default 4); this test takes the other fp32-grade tensor-core mode
+    through the same shapes: water (full fused chain / six launches, row tiles with a ragged tail), all seven species (middle
+    chain + layer-1 launches, buckets from 2 to ~1000 rows) and a molecule batch with two networks."""
+    consts, widths, params, om = U.make_model(1)
+    sp, xyz, box = inputs.water_box(1000, seed=3)
+    ctx = U.gpu_create(consts, widths, params, 1, 3600, mm_mode=mm_mode)
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, nbr_method=1))
+        sp, xyz, box = inputs.solvated_chain(n_solute=600, L=24.0, seed=5)
+        sp = sp.copy()
+        sp[:14] = np.arange(14) % 7
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, box, nbr_method=1))
+    finally:
+        nnp.nnp_destroy(ctx)
+    consts, widths, params, om = U.make_model(2, seed=inputs.SEED0 + 5)
+    sp, xyz, offs = inputs.molecule_batch(120, seed=12)
+    ctx = U.gpu_create(consts, widths, params, 2, len(sp), max_mols=120, mm_mode=mm_mode)
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, None, mol_offsets=offs)
+        U.assert_parity(Eg, Fg, orc.energy_forces(om, sp, xyz, None, offs, want_e_atom=True), mol_offsets=offs)
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+def test_fused_mode_reports_activations_out_of_fp16_range():
+    """mm_mode 4 scales activations by 16 into fp16 hi/lo operands: |value| > 3750 must come back as NNP_ERANGE, never as
+    a silently saturated energy.  A last layer 1e4 times the parity tests' makes delta3 = w4 celu'(h3) that large."""
+    consts, widths, params, om = U.make_model(1, scale=U.FORCE_SCALE * 1e4)
+    sp, xyz, box = inputs.water_box(64, 12.42)
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp), mm_mode=nnp.NNP_MM_3XF16_TC)
+    try:
+        with pytest.raises(nnp.NnpError) as ei:
+            U.gpu_energy_forces(ctx, sp, xyz, box)
+        assert ei.value.status == nnp.NNP_ERANGE
+    finally:
+        nnp.nnp_destroy(ctx)
+    # the same model through 3xTF32 (tf32 carries the fp32 exponent) evaluates fine
+    ctx = U.gpu_create(consts, widths, params, 1, len(sp), mm_mode=nnp.NNP_MM_3XTF32_TC)
+    try:
+        Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+        ref = orc.energy_forces(om, sp, xyz, box)
+        assert abs(Eg[0] - ref["E"][0]) <= U.E_RTOL * abs(ref["E"][0])
     finally:
         nnp.nnp_destroy(ctx)
 
