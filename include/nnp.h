@@ -151,7 +151,11 @@ int nnp_get_atomic_energies(nnp_ctx *ctx, float *d_e_atom);
 /* Stage 5.  nnp_md_init: velocities [n][3] (A/fs, original order), time step (fs), Verlet skin (A);
  * builds the lists and evaluates the initial forces.  nnp_md_step: n_steps of velocity Verlet
  * (v += dt/2 a; x += dt v; rebuild lists iff max_i |x_i - x_i(last build)| > skin/2, decided on the
- * device; forces; v += dt/2 a), no host synchronisation inside (reading C2). */
+ * device; forces; v += dt/2 a), no host synchronisation inside (reading C2).
+ * Batches (n_mols > 1: molecules, or replicas of one periodic cell - the ring-polymer beads of PAPER.md L309 get their
+ * potential energies and forces this way): every structure takes the same steps independently of the others; the rebuild
+ * test is one flag for the whole batch (any atom of any structure beyond skin/2 rebuilds all lists).  The bead-bead springs
+ * of a ring-polymer Hamiltonian are not part of this library. */
 int nnp_md_init(nnp_ctx *ctx, const float *d_vel, float dt_fs, float skin);
 int nnp_md_step(nnp_ctx *ctx, int n_steps);
 
@@ -164,8 +168,8 @@ int nnp_md_step(nnp_ctx *ctx, int n_steps);
  * gamma [1/fs] = 0 switches back to velocity Verlet.  kT in energy units.  nnp_md_init resets to velocity Verlet. */
 int nnp_md_set_langevin(nnp_ctx *ctx, float gamma, float kT, uint64_t seed);
 
-/* Copies out the current state in original order; any pointer may be NULL.  d_epot/d_ekin: fp64 scalars
- * (potential energy of the last force evaluation, kinetic energy after the last step, energy units);
+/* Copies out the current state in original order; any pointer may be NULL.  d_epot/d_ekin: fp64 [n_mols]
+ * (per structure: potential energy of the last force evaluation, kinetic energy after the last step, energy units);
  * d_n_rebuilds: list builds since nnp_md_init (the initial one included).  Asynchronous. */
 int nnp_get_state(nnp_ctx *ctx, float *d_xyz, float *d_vel, double *d_epot, double *d_ekin, int32_t *d_n_rebuilds);
 

@@ -81,10 +81,23 @@ __global__ void k_kick_drift_langevin(int n, float4 *__restrict__ pos, float4 *_
     if (__syncthreads_or(moved) && threadIdx.x == 0) flags[1] = 1;
 }
 
+// out[m] += v for the lanes with ok; the lanes of a warp that share a structure add once (the internal order keeps the
+// atoms of a structure together inside a species bucket, so a warp meets one or two structures)
+__device__ __forceinline__ void add_per_structure(bool ok, int m, double v, double *__restrict__ out)
+{
+    const unsigned peers = __match_any_sync(0xffffffffu, ok ? m : -1);
+    const int lane = threadIdx.x & 31;
+    const int leader = __ffs(peers) - 1;
+    double s = 0.0;
+    for (unsigned rest = peers; rest; rest &= rest - 1) s += __shfl_sync(peers, v, __ffs(rest) - 1);
+    if (ok && lane == leader) atomicAdd(&out[m], s);
+}
+
 // v += dt/2 a(F); kinetic energy sum_i m v^2 / (2 accel_conv) accumulated in fp64.
 __global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restrict__ frc, const int *__restrict__ spc,
                           const float *__restrict__ inv_mass_conv, const float *__restrict__ mass, float dt,
-                          float inv_accel_conv, double *__restrict__ ekin, int *__restrict__ step_ctr)
+                          float inv_accel_conv, const int *__restrict__ mol, int single, double *__restrict__ ekin,
+                          int *__restrict__ step_ctr)
 {
     if (step_ctr && blockIdx.x == 0 && threadIdx.x == 0) *step_ctr += 1; // Langevin step counter (read by the next drift kernel)
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -97,6 +110,10 @@ __global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restr
         v.x = fmaf(k, f.x, v.x); v.y = fmaf(k, f.y, v.y); v.z = fmaf(k, f.z, v.z);
         vel[i] = v;
         ke = 0.5f * mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z) * inv_accel_conv;
+    }
+    if (!single) { // one kinetic energy per structure (replica batches)
+        add_per_structure(i < n, i < n ? mol[i] : -1, (double)ke, ekin);
+        return;
     }
     __shared__ double part[T / 32];
     double d = (double)ke;
@@ -120,7 +137,7 @@ __global__ void k_energy_reduce(int n, const float *__restrict__ e_atom, const i
     double e = 0.0;
     if (i < n) e = (double)e_atom[i] * (double)inv_nets + (double)e_shift[spc[i]];
     if (!single) {
-        if (i < n) atomicAdd(&e_mol[mol[i]], e);
+        add_per_structure(i < n, i < n ? mol[i] : -1, e, e_mol);
         return;
     }
     __shared__ double part[T / 32];
@@ -219,9 +236,10 @@ void nnp_launch_kick_drift(nnp_ctx *c)
 
 void nnp_launch_kick_ke(nnp_ctx *c, int count_step)
 {
-    cudaMemsetAsync(c->ekin, 0, sizeof(double), c->stream);
+    cudaMemsetAsync(c->ekin, 0, sizeof(double) * c->n_mols, c->stream);
     k_kick_ke<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->vel, c->frc, c->spc, c->d_inv_mass_conv, c->d_mass,
-                                                       c->dt, 1.0f / c->accel_conv, c->ekin, count_step ? c->flags + 4 : nullptr);
+                                                       c->dt, 1.0f / c->accel_conv, c->mol, c->n_mols == 1, c->ekin,
+                                                       count_step ? c->flags + 4 : nullptr);
     c->launches += 1;
 }
 

@@ -765,7 +765,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     for (int l = 0; l < 3; ++l) TRY(dev_alloc(c, &c->H[l], N * c->hmax[l] * (size_t)c->n_nets));
     TRY(dev_alloc(c, &c->e_atom, N));
     TRY(dev_alloc(c, &c->e_mol, (size_t)max_mols));
-    TRY(dev_alloc(c, &c->ekin, 1));
+    TRY(dev_alloc(c, &c->ekin, (size_t)max_mols));
     TRY(dev_alloc(c, &c->flags, 16));
     TRY(dev_alloc(c, &c->io_xyz, 3 * N)); TRY(dev_alloc(c, &c->io_vel, 3 * N)); TRY(dev_alloc(c, &c->io_species, N));
     TRY(dev_alloc(c, &c->d_res, 8));
@@ -773,7 +773,7 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     TRYCU(cudaMemset(c->flags, 0, sizeof(int) * 16));
     TRY(dev_alloc(c, &c->aev_sched, 2 * NNP_AEV_SCHED_LEN));
     TRYCU(cudaMemset(c->aev_sched, 0, sizeof(int) * 2 * NNP_AEV_SCHED_LEN));
-    TRYCU(cudaMemset(c->ekin, 0, sizeof(double)));
+    TRYCU(cudaMemset(c->ekin, 0, sizeof(double) * (size_t)max_mols));
     TRYCU(cudaDeviceSynchronize());
 #undef TRY
 #undef TRYCU
@@ -946,7 +946,6 @@ int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
     if (!c) return NNP_EINVAL;
     if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "nnp_set_system first");
     if (!d_vel || !(dt_fs > 0.f) || !(skin > 0.f)) NNP_FAIL(c, NNP_EINVAL, "need velocities, dt > 0, skin > 0");
-    if (c->n_mols != 1) NNP_FAIL(c, NNP_EINVAL, "MD runs on one structure");
     if (c->n == 0) NNP_FAIL(c, NNP_EINVAL, "empty system");
     CU(c, cudaSetDevice(c->device));
     nnp_launch_permute_in3(c, d_vel, c->vel);
@@ -1022,8 +1021,8 @@ int nnp_get_state(nnp_ctx *c, float *d_xyz, float *d_vel, double *d_epot, double
         if (d_xyz) nnp_launch_unpermute3(c, c->pos, d_xyz);
         if (d_vel) nnp_launch_unpermute3(c, c->vel, d_vel);
     }
-    if (d_epot) CU(c, cudaMemcpyAsync(d_epot, c->e_mol, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
-    if (d_ekin) CU(c, cudaMemcpyAsync(d_ekin, c->ekin, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    if (d_epot) CU(c, cudaMemcpyAsync(d_epot, c->e_mol, sizeof(double) * c->n_mols, cudaMemcpyDeviceToDevice, c->stream));
+    if (d_ekin) CU(c, cudaMemcpyAsync(d_ekin, c->ekin, sizeof(double) * c->n_mols, cudaMemcpyDeviceToDevice, c->stream));
     if (d_n_rebuilds) CU(c, cudaMemcpyAsync(d_n_rebuilds, c->flags + 2, sizeof(int), cudaMemcpyDeviceToDevice, c->stream));
     return NNP_OK;
 }
@@ -1086,6 +1085,7 @@ int nnp_md_step_host(nnp_ctx *c, float *h_xyz, float *h_vel, int n_steps, double
     if (!c) return NNP_EINVAL;
     if (!c->md_ready) NNP_FAIL(c, NNP_ESTALE, "nnp_md_init first");
     if (!h_xyz || !h_vel) NNP_FAIL(c, NNP_EINVAL, "null argument");
+    if (c->n_mols != 1) NNP_FAIL(c, NNP_EINVAL, "nnp_md_step_host returns the energies of one structure: use nnp_md_step / nnp_get_state for a batch");
     CU(c, cudaSetDevice(c->device));
     const size_t bytes = sizeof(float) * 3 * (size_t)c->n;
     CU(c, cudaMemcpyAsync(c->io_xyz, h_xyz, bytes, cudaMemcpyHostToDevice, c->stream));

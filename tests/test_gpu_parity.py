@@ -335,6 +335,74 @@ def test_md_steps_against_oracle(model1, graph):
         nnp.nnp_destroy(ctx)
 
 
+@pytest.mark.parametrize("graph", [False, True], ids=["kernel_by_kernel", "cuda_graph"])
+def test_md_on_a_replica_batch(model1, graph):
+    """SURVEY 8(f)-4 / PAPER.md L309: the replicas of a ring polymer take their MD steps as ONE batch.  Four replicas of a
+    125-water cell (different positions and velocities) step together; each must follow the oracle's integrator run on that
+    replica alone, energies come back per replica, and after 40 steps (lists rebuilt by the shared displacement flag) the
+    oracle's E and F at the GPU's positions agree replica by replica."""
+    consts, widths, params, om = model1
+    n_rep = 4
+    sp1, x1, box = inputs.water_box(125, seed=inputs.SEED0 + 31)
+    n1 = len(sp1)
+    rng = np.random.default_rng(11)
+    reps = [(x1 + 0.03 * rng.standard_normal(x1.shape) * (r > 0)).astype(np.float32).astype(np.float64) for r in range(n_rep)]
+    vels = [inputs.maxwell_boltzmann(sp1, 300.0, seed=40 + r).astype(np.float32).astype(np.float64) for r in range(n_rep)]
+    sp, xyz, v = np.tile(sp1, n_rep), np.concatenate(reps), np.concatenate(vels)
+    offs = (np.arange(n_rep + 1) * n1).astype(np.int32)
+    n = len(sp)
+    dev = torch.device("cuda:0")
+    ctx = U.gpu_create(consts, widths, params, 1, n, max_mols=n_rep, stream=torch.cuda.Stream(device=dev) if graph else None)
+    try:
+        d_sp = torch.as_tensor(sp.astype(np.int32), device=dev)
+        d_x = torch.as_tensor(xyz.astype(np.float32), device=dev)
+        d_v = torch.as_tensor(v.astype(np.float32), device=dev)
+        d_o = torch.as_tensor(offs, device=dev)
+        torch.cuda.synchronize()
+        nnp.nnp_set_system(ctx, n, d_sp, d_x, box, n_rep, d_o)
+        nnp.nnp_md_init(ctx, d_v, 0.5, 0.5)
+        o_x, o_v = torch.zeros_like(d_x), torch.zeros_like(d_v)
+        o_ep = torch.zeros(n_rep, dtype=torch.float64, device=dev)
+        o_ek = torch.zeros(n_rep, dtype=torch.float64, device=dev)
+        o_nr = torch.zeros(1, dtype=torch.int32, device=dev)
+        torch.cuda.synchronize()
+
+        def state():
+            nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, o_nr)
+            nnp.nnp_sync(ctx)
+            return (o_x.cpu().numpy().astype(np.float64), o_v.cpu().numpy().astype(np.float64),
+                    o_ep.cpu().numpy(), o_ek.cpu().numpy(), int(o_nr.item()))
+
+        x0, v0, ep0, ek0, nr0 = state()
+        for r in range(n_rep):
+            ke = 0.5 * (inputs.MASS[sp1][:, None] * vels[r] ** 2).sum() / inputs.ACCEL_CONV
+            assert abs(ek0[r] - ke) <= 1e-5 * ke
+        nnp.nnp_md_step(ctx, 2)
+        x2, v2, ep2, ek2, nr2 = state()
+        for r in range(n_rep):
+            o = orc.md(om, sp1, reps[r], vels[r], inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 2)
+            sl = slice(offs[r], offs[r + 1])
+            assert np.abs(x2[sl] - o["xyz"]).max() < 4e-6 and np.abs(v2[sl] - o["vel"]).max() < 4e-6, r
+            assert abs(ep2[r] - o["epot"][2]) <= 2e-5 * abs(o["epot"][2]) and abs(ek2[r] - o["ekin"][2]) <= 1e-4 * o["ekin"][2], r
+        tot0 = ep2 + ek2
+        nnp.nnp_md_step(ctx, 38)
+        xs, vs, ep, ek, nr = state()
+        assert nr >= 2
+        tot = ep + ek
+        for r in range(n_rep):
+            sl = slice(offs[r], offs[r + 1])
+            ref = orc.energy_forces(om, sp1, xs[sl], box)
+            assert abs(ep[r] - ref["E"][0]) <= U.E_RTOL * abs(ref["E"][0]), r
+            assert abs(tot[r] - tot0[r]) < 1e-3 * abs(ek2[r]) + 1e-3 * abs(tot0[r]), r     # every replica conserves its own energy
+        # the host entry point returns the scalars of one structure only
+        h = np.zeros((n, 3), dtype=np.float32)
+        with pytest.raises(nnp.NnpError) as e:
+            nnp.nnp_md_step_host(ctx, h, h.copy(), 1, np.zeros(1), np.zeros(1))
+        assert e.value.status == nnp.NNP_EINVAL
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
 def test_host_entry_points_roundtrip(model1):
     consts, widths, params, om = model1
     sp, xyz, box = inputs.water_box(125, seed=10)
