@@ -158,6 +158,75 @@ int orc_neighbors_brute(int n, const double *xyz, const double *box, const int *
     return maxc > cap ? -maxc : maxc;
 }
 
+/* ---- NEXT-2 (second part; "optionally cell vectors", L49 shift vectors, L307
+ * "minimum image or all images"): a GENERAL cell (rows of cell[9] are the lattice vectors a, b, c; triclinic allowed) with
+ * ALL periodic images, written out as the definition: atom i sees every image x_j + s_0 a + s_1 b + s_2 c (s integer, the
+ * pair (j = i, s = 0) excluded) closer than rcut - including images of itself and several images of the same atom when the
+ * cell is smaller than 2 rcut.  A list entry is (j, s).  For cells wider than 2 rcut this is the minimum-image list. */
+static void disp_cell(const double *xi, const double *xj, const double *cell, const int *s, double d[3])
+{
+    for (int c = 0; c < 3; ++c)
+        d[c] = xj[c] - xi[c] + (double)s[0] * cell[c] + (double)s[1] * cell[3 + c] + (double)s[2] * cell[6 + c];
+}
+
+static void cross3(const double *a, const double *b, double *o)
+{
+    o[0] = a[1] * b[2] - a[2] * b[1]; o[1] = a[2] * b[0] - a[0] * b[2]; o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+/* Brute force over pairs and shifts, fp64 predicate r2 < rcut^2.  The shifts that can matter: a vector shorter than rcut
+ * has |fractional component c| <= rcut / w_c, w_c = volume / |area of the face spanned by the other two vectors| (the
+ * perpendicular width); every integer s_c with |frac_c(x_j - x_i) + s_c| <= rcut / w_c is tried.
+ * counts[n], list[n][cap], shifts[n][cap][3].  Returns max row length, or -(needed) if some row exceeds cap. */
+int orc_neighbors_cell(int n, const double *xyz, const double *cell, const int *mol_id, double rcut, int cap,
+                       int *counts, int *list, int *shifts)
+{
+    double rec[9], vol, reach[3]; /* rec rows: reciprocal vectors b x c, c x a, a x b (frac_c = rec_c . x / vol) */
+    cross3(cell + 3, cell + 6, rec); cross3(cell + 6, cell, rec + 3); cross3(cell, cell + 3, rec + 6);
+    vol = cell[0] * rec[0] + cell[1] * rec[1] + cell[2] * rec[2];
+    if (!(fabs(vol) > 0.0)) return -1000000000;
+    for (int c = 0; c < 3; ++c) {
+        double area = sqrt(rec[3 * c] * rec[3 * c] + rec[3 * c + 1] * rec[3 * c + 1] + rec[3 * c + 2] * rec[3 * c + 2]);
+        reach[c] = rcut * area / fabs(vol); /* rcut / w_c */
+    }
+    int maxc = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(max : maxc)
+    for (int i = 0; i < n; ++i) {
+        int cnt = 0;
+        for (int j = 0; j < n; ++j) {
+            if (mol_id && mol_id[i] != mol_id[j]) continue;
+            double f[3];
+            for (int c = 0; c < 3; ++c) {
+                double t = 0.0;
+                for (int q = 0; q < 3; ++q) t += rec[3 * c + q] * (xyz[3 * j + q] - xyz[3 * i + q]);
+                f[c] = t / vol;
+            }
+            int lo[3], hi[3];
+            for (int c = 0; c < 3; ++c) { lo[c] = (int)ceil(-reach[c] - f[c] - 1e-9); hi[c] = (int)floor(reach[c] - f[c] + 1e-9); }
+            for (int s0 = lo[0]; s0 <= hi[0]; ++s0)
+                for (int s1 = lo[1]; s1 <= hi[1]; ++s1)
+                    for (int s2 = lo[2]; s2 <= hi[2]; ++s2) {
+                        if (j == i && s0 == 0 && s1 == 0 && s2 == 0) continue;
+                        int sh[3] = {s0, s1, s2};
+                        double d[3];
+                        disp_cell(xyz + 3 * i, xyz + 3 * j, cell, sh, d);
+                        if ((d[0] * d[0] + d[1] * d[1] + d[2] * d[2]) < rcut * rcut) {
+                            if (cnt < cap) {
+                                list[(long)i * cap + cnt] = j;
+                                shifts[((long)i * cap + cnt) * 3] = s0;
+                                shifts[((long)i * cap + cnt) * 3 + 1] = s1;
+                                shifts[((long)i * cap + cnt) * 3 + 2] = s2;
+                            }
+                            ++cnt;
+                        }
+                    }
+        }
+        counts[i] = cnt;
+        if (cnt > maxc) maxc = cnt;
+    }
+    return maxc > cap ? -maxc : maxc;
+}
+
 /* Uniform grid for large periodic N (SURVEY 8(d) "Oracle timing"): bins of edge >= rcut, every atom
  * tests the atoms of all DISTINCT bins within +-1 in each dimension with the same predicate as the
  * brute force.  Independent of the CUDA cell list; pinned against orc_neighbors_brute in tests.
@@ -305,15 +374,23 @@ double orc_mlp(const orc_model *m, int net, int species, const double *G, double
 
 /* O2 + O3: AEV of atom i from its radial list (ids with r < rcr); angular neighbours are the subset
  * with r < rca (PAPER.md L51-55 GraphFilter / GraphAngularExtension). */
+/* displacement of list entry a (atom j) of centre i: minimum image in an orthorhombic box, or the entry's own image
+ * shift shf[3 a .. 3 a + 2] in a general cell (shf != NULL) */
+#define NBR_DISP(a_, j_, out_)                                                                  \
+    do {                                                                                         \
+        if (shf) disp_cell(xyz + 3 * i, xyz + 3 * (j_), cell, shf + 3 * (a_), out_);             \
+        else disp(xyz + 3 * i, xyz + 3 * (j_), box, out_);                                       \
+    } while (0)
+
 static void aev_atom(const orc_model *m, int i, const int *species, const double *xyz, const double *box,
-                     int nn, const int *nbr, double *G)
+                     const double *cell, const int *shf, int nn, const int *nbr, double *G)
 {
     const int S = m->n_species, nr = m->n_shf_r, na = m->n_shf_a, nz = m->n_shf_z;
     const int len = orc_aev_len(m), rad = S * nr;
     for (int q = 0; q < len; ++q) G[q] = 0.0;
     for (int a = 0; a < nn; ++a) {
         int j = nbr[a];
-        double d[3]; disp(xyz + 3 * i, xyz + 3 * j, box, d);
+        double d[3]; NBR_DISP(a, j, d);
         double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
         if (!(r < m->rcr)) continue;
         double f = orc_fc(r, m->rcr);
@@ -322,12 +399,12 @@ static void aev_atom(const orc_model *m, int i, const int *species, const double
     }
     for (int a = 0; a < nn; ++a) {
         int j = nbr[a];
-        double dj[3]; disp(xyz + 3 * i, xyz + 3 * j, box, dj);
+        double dj[3]; NBR_DISP(a, j, dj);
         double rj = sqrt(dj[0] * dj[0] + dj[1] * dj[1] + dj[2] * dj[2]);
         if (!(rj < m->rca)) continue;
         for (int b = a + 1; b < nn; ++b) { /* unordered pairs {j,k} */
             int k = nbr[b];
-            double dk[3]; disp(xyz + 3 * i, xyz + 3 * k, box, dk);
+            double dk[3]; NBR_DISP(b, k, dk);
             double rk = sqrt(dk[0] * dk[0] + dk[1] * dk[1] + dk[2] * dk[2]);
             if (!(rk < m->rca)) continue;
             double c = (dj[0] * dk[0] + dj[1] * dk[1] + dj[2] * dk[2]) / (rj * rk);
@@ -348,14 +425,14 @@ static void aev_atom(const orc_model *m, int i, const int *species, const double
 
 /* O6: given g = dE/dG_i, add -dE/dx to F for atom i and its neighbours. */
 static void aev_atom_backward(const orc_model *m, int i, const int *species, const double *xyz, const double *box,
-                              int nn, const int *nbr, const double *g, double *F, double *W /* NULL or [10]: strain derivative sum d_a dE/dd_b (9) and sum |d_a dE/dd_b| */)
+                              const double *cell, const int *shf, int nn, const int *nbr, const double *g, double *F, double *W /* NULL or [10]: strain derivative sum d_a dE/dd_b (9) and sum |d_a dE/dd_b| */)
 {
     const int S = m->n_species, nr = m->n_shf_r, na = m->n_shf_a, nz = m->n_shf_z;
     const int rad = S * nr;
     double Fi[3] = {0, 0, 0};
     for (int a = 0; a < nn; ++a) {
         int j = nbr[a];
-        double d[3]; disp(xyz + 3 * i, xyz + 3 * j, box, d);
+        double d[3]; NBR_DISP(a, j, d);
         double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
         if (!(r < m->rcr)) continue;
         double f = orc_fc(r, m->rcr), fp = dfc(r, m->rcr);
@@ -375,12 +452,12 @@ static void aev_atom_backward(const orc_model *m, int i, const int *species, con
     }
     for (int a = 0; a < nn; ++a) {
         int j = nbr[a];
-        double dj[3]; disp(xyz + 3 * i, xyz + 3 * j, box, dj);
+        double dj[3]; NBR_DISP(a, j, dj);
         double rj = sqrt(dj[0] * dj[0] + dj[1] * dj[1] + dj[2] * dj[2]);
         if (!(rj < m->rca)) continue;
         for (int b = a + 1; b < nn; ++b) {
             int k = nbr[b];
-            double dk[3]; disp(xyz + 3 * i, xyz + 3 * k, box, dk);
+            double dk[3]; NBR_DISP(b, k, dk);
             double rk = sqrt(dk[0] * dk[0] + dk[1] * dk[1] + dk[2] * dk[2]);
             if (!(rk < m->rca)) continue;
             double c = (dj[0] * dk[0] + dj[1] * dk[1] + dj[2] * dk[2]) / (rj * rk);
@@ -435,12 +512,13 @@ static void aev_atom_backward(const orc_model *m, int i, const int *species, con
  * cutoff in fp64.  Outputs (any may be NULL except E): E[n_mols] (O5), F[n][3] (O6), e_atom[n],
  * aev[n][len], dEdG[n][len].  mol_offsets NULL => one structure.  Returns 0, or <0 on failure. */
 static int energy_forces_impl(const orc_model *m, int n, const int *species, const double *xyz, const double *box,
+                              const double *cell /* NULL, or 9: general cell with all images (then box is ignored) */,
                               int n_mols, const int *mol_offsets, int nbr_method, double *E, double *F,
                               double *e_atom, double *aev, double *dEdG, double *virial)
 {
     const int len = orc_aev_len(m);
     const double *bx = NULL;
-    if (box && (box[0] > 0.0 || box[1] > 0.0 || box[2] > 0.0)) bx = box;
+    if (!cell && box && (box[0] > 0.0 || box[1] > 0.0 || box[2] > 0.0)) bx = box;
     int *mol_id = (int *)malloc(sizeof(int) * (n > 0 ? n : 1));
     if (mol_offsets) {
         for (int q = 0; q < n_mols; ++q)
@@ -454,13 +532,15 @@ static int energy_forces_impl(const orc_model *m, int n, const int *species, con
     if (n == 0) { free(mol_id); return 0; }
 
     int cap = 64, rc;
-    int *counts = (int *)malloc(sizeof(int) * n), *list = NULL;
+    int *counts = (int *)malloc(sizeof(int) * n), *list = NULL, *shifts = NULL;
     for (;;) {
         list = (int *)malloc(sizeof(int) * (size_t)n * cap);
-        if (nbr_method == 1 && bx) rc = orc_neighbors_grid(n, xyz, bx, m->rcr, 0, cap, counts, list);
+        if (cell) shifts = (int *)malloc(sizeof(int) * 3 * (size_t)n * cap);
+        if (cell) rc = orc_neighbors_cell(n, xyz, cell, mol_offsets ? mol_id : NULL, m->rcr, cap, counts, list, shifts);
+        else if (nbr_method == 1 && bx) rc = orc_neighbors_grid(n, xyz, bx, m->rcr, 0, cap, counts, list);
         else rc = orc_neighbors_brute(n, xyz, bx, mol_offsets ? mol_id : NULL, m->rcr, 0, cap, counts, list);
         if (rc >= 0) break;
-        free(list);
+        free(list); free(shifts); shifts = NULL;
         if (rc <= -1000000000) { free(counts); free(mol_id); return -1; }
         cap = -rc + 8;
     }
@@ -475,7 +555,7 @@ static int energy_forces_impl(const orc_model *m, int n, const int *species, con
         for (int i = 0; i < n; ++i) {
             int s = species[i];
             if (s < 0 || s >= m->n_species) { fail = 1; continue; }
-            aev_atom(m, i, species, xyz, bx, counts[i], list + (size_t)i * cap, G);
+            aev_atom(m, i, species, xyz, bx, cell, shifts ? shifts + 3 * (size_t)i * cap : NULL, counts[i], list + (size_t)i * cap, G);
             double e = 0.0;
             for (int q = 0; q < len; ++q) g[q] = 0.0;
             for (int net = 0; net < m->n_nets; ++net) { /* reading B5: mean over the ensemble */
@@ -490,7 +570,7 @@ static int energy_forces_impl(const orc_model *m, int n, const int *species, con
             if (dEdG) memcpy(dEdG + (size_t)i * len, g, sizeof(double) * len);
 #pragma omp atomic
             E[mol_id[i]] += e;
-            if (F) aev_atom_backward(m, i, species, xyz, bx, counts[i], list + (size_t)i * cap, g, F, virial ? Wt : NULL);
+            if (F) aev_atom_backward(m, i, species, xyz, bx, cell, shifts ? shifts + 3 * (size_t)i * cap : NULL, counts[i], list + (size_t)i * cap, g, F, virial ? Wt : NULL);
         }
         if (virial)
             for (int q = 0; q < 10; ++q) {
@@ -499,7 +579,7 @@ static int energy_forces_impl(const orc_model *m, int n, const int *species, con
             }
         free(G); free(g); free(gn);
     }
-    free(counts); free(list); free(mol_id);
+    free(counts); free(list); free(shifts); free(mol_id);
     return fail ? -2 : 0;
 }
 
@@ -507,7 +587,17 @@ int orc_energy_forces(const orc_model *m, int n, const int *species, const doubl
                       int n_mols, const int *mol_offsets, int nbr_method, double *E, double *F,
                       double *e_atom, double *aev, double *dEdG)
 {
-    return energy_forces_impl(m, n, species, xyz, box, n_mols, mol_offsets, nbr_method, E, F, e_atom, aev, dEdG, NULL);
+    return energy_forces_impl(m, n, species, xyz, box, NULL, n_mols, mol_offsets, nbr_method, E, F, e_atom, aev, dEdG, NULL);
+}
+
+/* The same in a general cell (rows a, b, c) with all periodic images; virial [10] as orc_energy_forces_virial or NULL
+ * (one structure). */
+int orc_energy_forces_cell(const orc_model *m, int n, const int *species, const double *xyz, const double *cell,
+                           int n_mols, const int *mol_offsets, double *E, double *F, double *e_atom, double *aev,
+                           double *virial)
+{
+    if (virial) for (int q = 0; q < 10; ++q) virial[q] = 0.0;
+    return energy_forces_impl(m, n, species, xyz, NULL, cell, n_mols, mol_offsets, 0, E, F, e_atom, aev, NULL, virial);
 }
 
 /* NEXT-2 (first part; "energy_and_forces_and_virial"): the energy depends on
@@ -521,7 +611,7 @@ int orc_energy_forces_virial(const orc_model *m, int n, const int *species, cons
                              int nbr_method, double *E, double *F, double *virial /*[10]*/)
 {
     for (int q = 0; q < 10; ++q) virial[q] = 0.0;
-    return energy_forces_impl(m, n, species, xyz, box, 1, NULL, nbr_method, E, F, NULL, NULL, NULL, virial);
+    return energy_forces_impl(m, n, species, xyz, box, NULL, 1, NULL, nbr_method, E, F, NULL, NULL, NULL, virial);
 }
 
 /* O7 rebuild rule (reading C2): max_i |x_i - xref_i| > skin/2 (strict). */
@@ -542,16 +632,16 @@ int orc_needs_rebuild(int n, const double *xyz, const double *xref, double skin)
  * n_rebuilds reports what an implementation using a Verlet skin must do (the initial build counts as 1).
  * F_io: forces at the input positions if have_forces, else computed here; holds the final forces on return.
  * epot/ekin: [n_steps+1] values at steps 0..n_steps (may be NULL). */
-int orc_md(const orc_model *m, int n, const int *species, double *xyz, double *vel, double *F_io, int have_forces,
-           const double *mass /*[S]*/, const double *box, double dt, double accel_conv, int n_steps, double skin,
-           int nbr_method, double *epot, double *ekin, int *n_rebuilds)
+static int md_impl(const orc_model *m, int n, const int *species, double *xyz, double *vel, double *F_io, int have_forces,
+                   const double *mass /*[S]*/, const double *box, const double *cell, double dt, double accel_conv, int n_steps,
+                   double skin, int nbr_method, double *epot, double *ekin, int *n_rebuilds)
 {
     double E;
     int rc = 0, nreb = 1;
     double *xref = (double *)malloc(sizeof(double) * 3 * (size_t)n);
     memcpy(xref, xyz, sizeof(double) * 3 * (size_t)n);
     if (!have_forces || epot) {
-        rc = orc_energy_forces(m, n, species, xyz, box, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL);
+        rc = energy_forces_impl(m, n, species, xyz, box, cell, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL, NULL);
         if (rc) { free(xref); return rc; }
     }
     for (int step = 0;; ++step) {
@@ -569,7 +659,7 @@ int orc_md(const orc_model *m, int n, const int *species, double *xyz, double *v
                 xyz[3 * i + c] += dt * vel[3 * i + c];
             }
         if (orc_needs_rebuild(n, xyz, xref, skin)) { memcpy(xref, xyz, sizeof(double) * 3 * (size_t)n); ++nreb; }
-        rc = orc_energy_forces(m, n, species, xyz, box, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL);
+        rc = energy_forces_impl(m, n, species, xyz, box, cell, 1, NULL, nbr_method, &E, F_io, NULL, NULL, NULL, NULL);
         if (rc) break;
         for (int i = 0; i < n; ++i)
             for (int c = 0; c < 3; ++c) vel[3 * i + c] += 0.5 * dt * accel_conv * F_io[3 * i + c] / mass[species[i]];
@@ -577,6 +667,22 @@ int orc_md(const orc_model *m, int n, const int *species, double *xyz, double *v
     if (n_rebuilds) *n_rebuilds = nreb;
     free(xref);
     return rc;
+}
+
+int orc_md(const orc_model *m, int n, const int *species, double *xyz, double *vel, double *F_io, int have_forces,
+           const double *mass /*[S]*/, const double *box, double dt, double accel_conv, int n_steps, double skin,
+           int nbr_method, double *epot, double *ekin, int *n_rebuilds)
+{
+    return md_impl(m, n, species, xyz, vel, F_io, have_forces, mass, box, NULL, dt, accel_conv, n_steps, skin, nbr_method, epot, ekin,
+                   n_rebuilds);
+}
+
+/* O7 in a general cell with all images (orc_energy_forces_cell). */
+int orc_md_cell(const orc_model *m, int n, const int *species, double *xyz, double *vel, double *F_io, int have_forces,
+                const double *mass /*[S]*/, const double *cell, double dt, double accel_conv, int n_steps, double skin,
+                double *epot, double *ekin, int *n_rebuilds)
+{
+    return md_impl(m, n, species, xyz, vel, F_io, have_forces, mass, NULL, cell, dt, accel_conv, n_steps, skin, 0, epot, ekin, n_rebuilds);
 }
 
 /* ---- NEXT-1: Langevin dynamics, BAOAB splitting.  PAPER.md L307: the MD engine offers

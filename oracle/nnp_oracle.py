@@ -68,6 +68,16 @@ def lib():
                              C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_double),
                              C.POINTER(C.c_double), C.c_double, C.c_double, C.c_int, C.c_double, C.c_int,
                              C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
+        L.orc_md_cell.argtypes = [C.POINTER(_Model), C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double),
+                                  C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_double),
+                                  C.POINTER(C.c_double), C.c_double, C.c_double, C.c_int, C.c_double,
+                                  C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int)]
+        L.orc_neighbors_cell.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int),
+                                         C.c_double, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.orc_energy_forces_cell.argtypes = [C.POINTER(_Model), C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double),
+                                             C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double),
+                                             C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                             C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -168,6 +178,70 @@ def energy_forces(model, species, xyz, box=None, mol_offsets=None, nbr_method=0,
     if rc != 0:
         raise RuntimeError("orc_energy_forces failed: %d" % rc)
     return {"E": E, "F": F, "e_atom": ea, "aev": aev, "dEdG": dg}
+
+
+def energy_forces_cell(model, species, xyz, cell, mol_offsets=None, want_forces=True, want_e_atom=False, want_aev=False,
+                       want_virial=False):
+    """O1-O6 in a general cell (rows of cell[3][3] = lattice vectors) with ALL periodic images.
+    Returns dict(E[n_mols], F[n,3], e_atom[n], aev[n,len], virial[3,3], virial_abs)."""
+    species = np.ascontiguousarray(species, dtype=np.int32)
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    n = xyz.shape[0]
+    cella = np.ascontiguousarray(cell, dtype=np.float64).reshape(9)
+    mo = None if mol_offsets is None else np.ascontiguousarray(mol_offsets, dtype=np.int32)
+    n_mols = 1 if mo is None else len(mo) - 1
+    E = np.zeros(n_mols)
+    F = np.zeros((n, 3)) if (want_forces or want_virial) else None
+    ea = np.zeros(n) if want_e_atom else None
+    aev = np.zeros((n, model.aev_len)) if want_aev else None
+    vir = np.zeros(10) if want_virial else None
+    rc = lib().orc_energy_forces_cell(C.byref(model.c), C.c_int(n), _ip(species), _dp(xyz), _dp(cella), C.c_int(n_mols),
+                                      _ip(mo), _dp(E), _dp(F), _dp(ea), _dp(aev), _dp(vir))
+    if rc != 0:
+        raise RuntimeError("orc_energy_forces_cell failed: %d" % rc)
+    out = {"E": E, "F": F, "e_atom": ea, "aev": aev}
+    if want_virial:
+        out["virial"], out["virial_abs"] = vir[:9].reshape(3, 3).copy(), float(vir[9])
+    return out
+
+
+def neighbors_cell(xyz, cell, rcut, mol_id=None):
+    """All-images lists in a general cell: per atom a sorted list of (j, s0, s1, s2)."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    n = xyz.shape[0]
+    cella = np.ascontiguousarray(cell, dtype=np.float64).reshape(9)
+    mid = None if mol_id is None else np.ascontiguousarray(mol_id, dtype=np.int32)
+    cap = 128
+    while True:
+        counts = np.zeros(n, dtype=np.int32)
+        lst = np.zeros((n, cap), dtype=np.int32)
+        shf = np.zeros((n, cap, 3), dtype=np.int32)
+        rc = lib().orc_neighbors_cell(n, _dp(xyz), _dp(cella), _ip(mid), float(rcut), cap, _ip(counts), _ip(lst), _ip(shf))
+        if rc >= 0:
+            break
+        if rc <= -1000000000:
+            raise RuntimeError("singular cell")
+        cap = -rc + 8
+    return [sorted((int(lst[i, k]), int(shf[i, k, 0]), int(shf[i, k, 1]), int(shf[i, k, 2])) for k in range(counts[i])) for i in range(n)]
+
+
+def md_cell(model, species, xyz, vel, mass, cell, dt, accel_conv, n_steps, skin=0.5):
+    """O7 velocity Verlet in a general cell with all images."""
+    species = np.ascontiguousarray(species, dtype=np.int32)
+    x = np.array(xyz, dtype=np.float64, order="C")
+    v = np.array(vel, dtype=np.float64, order="C")
+    n = x.shape[0]
+    F = np.zeros((n, 3))
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    cella = np.ascontiguousarray(cell, dtype=np.float64).reshape(9)
+    epot = np.zeros(n_steps + 1)
+    ekin = np.zeros(n_steps + 1)
+    nreb = C.c_int(0)
+    rc = lib().orc_md_cell(C.byref(model.c), n, _ip(species), _dp(x), _dp(v), _dp(F), 0, _dp(mass), _dp(cella), float(dt),
+                           float(accel_conv), int(n_steps), float(skin), _dp(epot), _dp(ekin), C.byref(nreb))
+    if rc != 0:
+        raise RuntimeError("orc_md_cell failed: %d" % rc)
+    return {"xyz": x, "vel": v, "F": F, "epot": epot, "ekin": ekin, "n_rebuilds": nreb.value}
 
 
 def needs_rebuild(xyz, xref, skin):

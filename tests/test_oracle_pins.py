@@ -686,3 +686,125 @@ def test_virial_of_a_dimer_by_hand(small_model, consts):
     V = r["virial"].copy()
     V[0, 0] = 0.0
     assert np.abs(V).max() < 1e-14
+
+
+# ---------------------------------------------------------------- NEXT-2, second part: general (triclinic) cells, all periodic images
+# SURVEY.md 8(f) item 2; PAPER.md L41 ("optionally cell vectors"), L49 (shift vectors), L307 (minimum image or all images).
+def _small_water(n_waters, L, seed):
+    return inputs.water_box(n_waters, L, seed=seed)
+
+
+def test_cell_path_equals_box_path_for_a_wide_orthorhombic_cell(small_model, water64):
+    """With every edge >= 2 R the all-images list IS the minimum-image list: the general-cell code must give the box code's
+    numbers (catches a wrong shift sign, a transposed cell, a self-pair left in)."""
+    sp, xyz, box = water64
+    a = orc.energy_forces(small_model, sp, xyz, box, want_e_atom=True, want_aev=True)
+    b = orc.energy_forces_cell(small_model, sp, xyz, np.diag(box), want_e_atom=True, want_aev=True, want_virial=True)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-10 * abs(a["E"][0])
+    assert np.abs(a["F"] - b["F"]).max() < 1e-10 and np.abs(a["aev"] - b["aev"]).max() < 1e-12
+    v = orc.energy_forces_virial(small_model, sp, xyz, box)
+    assert np.abs(v["virial"] - b["virial"]).max() < 1e-11 * v["virial_abs"]
+    # lists: every (j, 0-or-lattice shift) of the cell path is the box path's j, once
+    lc = orc.neighbors_cell(xyz, np.diag(box), 5.1)
+    lb = orc.neighbors(xyz, box, 5.1)
+    for i in range(len(sp)):
+        assert sorted(j for j, *_ in lc[i]) == sorted(lb[i])
+
+
+def test_lattice_equivalent_cells_give_the_same_answer(small_model):
+    """A lattice does not know which basis describes it: (a, b, c) -> (a, b + a, c + 2a - b) is unimodular, the cell becomes
+    strongly triclinic, every energy and force must stay (catches any place where the code assumes an orthogonal cell or
+    mixes up rows and columns of the cell matrix), for a wide cell and for one smaller than the cutoff."""
+    for n_w, L, seed in ((27, 9.31, 3), (4, 4.9, 4)):
+        sp, xyz, box = _small_water(n_w, L, seed)
+        h = np.diag(box).astype(float)
+        h2 = np.array([h[0], h[1] + h[0], h[2] + 2 * h[0] - h[1]])
+        a = orc.energy_forces_cell(small_model, sp, xyz, h, want_virial=True)
+        b = orc.energy_forces_cell(small_model, sp, xyz, h2, want_virial=True)
+        assert abs(a["E"][0] - b["E"][0]) < 1e-10 * abs(a["E"][0])
+        assert np.abs(a["F"] - b["F"]).max() < 1e-9
+        assert np.abs(a["virial"] - b["virial"]).max() < 1e-10 * a["virial_abs"]
+        # and the lists hold the same number of images per atom
+        la, lb = orc.neighbors_cell(xyz, h, 5.1), orc.neighbors_cell(xyz, h2, 5.1)
+        assert [len(r) for r in la] == [len(r) for r in lb]
+
+
+def test_small_cell_all_images_equals_its_supercell_by_minimum_image(small_model):
+    """All-images PBC in a cell below 2 R must equal the same crystal described by a supercell wide enough for the
+    minimum image, evaluated by the ORTHORHOMBIC BOX code (a different code path): E_super = copies x E_cell and every
+    image atom carries the force of its original.  L = 4.9 < R: atoms also see their own images."""
+    for n_w, L, m, seed in ((27, 9.31, 2, 3), (4, 4.9, 3, 4)):
+        sp, xyz, box = _small_water(n_w, L, seed)
+        cell = orc.energy_forces_cell(small_model, sp, xyz, np.diag(box))
+        shifts = np.array([[i, j, k] for i in range(m) for j in range(m) for k in range(m)], dtype=float) * np.asarray(box, dtype=float)
+        xs = np.concatenate([xyz + s for s in shifts])
+        sps = np.tile(sp, m ** 3)
+        sup = orc.energy_forces(small_model, sps, xs, np.asarray(box) * m)
+        assert abs(sup["E"][0] - m ** 3 * cell["E"][0]) < 1e-9 * abs(sup["E"][0])
+        n = len(sp)
+        for c in range(m ** 3):
+            assert np.abs(sup["F"][c * n:(c + 1) * n] - cell["F"]).max() < 1e-9
+    # the small cell really is in the regime the test is about: more images than atoms, self images included
+    lst = orc.neighbors_cell(xyz, np.diag(box), 5.1)
+    assert any(j == i for i, row in enumerate(lst) for j, *_ in row) and min(len(r) for r in lst) > len(sp)
+
+
+def test_all_images_list_against_explicit_images_and_kdtree():
+    """Lists of a skewed small cell against scipy's KD-tree over explicitly generated images (an independent search)."""
+    rng = np.random.default_rng(8)
+    h = np.array([[6.0, 0.0, 0.0], [2.2, 5.5, 0.0], [-1.3, 1.9, 6.4]])
+    xyz = rng.random((40, 3)) @ h + rng.integers(-2, 3, size=(40, 3)) @ h     # unwrapped coordinates
+    lst = orc.neighbors_cell(xyz, h, 5.1)
+    S = np.array([[i, j, k] for i in range(-7, 8) for j in range(-7, 8) for k in range(-7, 8)])
+    img = (xyz[None, :, :] + (S @ h)[:, None, :]).reshape(-1, 3)
+    tree = cKDTree(img)
+    for i in range(40):
+        near = tree.query_ball_point(xyz[i], 5.1 - 1e-12)
+        ref = sorted((q % 40, *S[q // 40]) for q in near if not (q % 40 == i and not S[q // 40].any()))
+        assert [tuple(int(v) for v in r) for r in ref] == lst[i]
+
+
+def test_triclinic_forces_and_sheared_virial_by_finite_differences(small_model):
+    """A genuinely triclinic small cell (a sheared, squeezed water cell - not a re-description of a cubic one): forces are
+    minus the energy gradient, and the FULL virial tensor, shear components included, is the derivative of the energy under
+    the homogeneous deformation x -> x (1 + eps), cell -> cell (1 + eps) (the first part of the row pinned
+    only the diagonal under PBC)."""
+    sp, xyz, box = _small_water(8, 6.2, 6)
+    D = np.array([[1.0, 0.0, 0.0], [0.23, 0.94, 0.0], [-0.17, 0.12, 1.05]])
+    x = xyz @ D
+    h = np.diag(box) @ D
+    r = orc.energy_forces_cell(small_model, sp, x, h, want_virial=True)
+    rng = np.random.default_rng(0)
+    for i in rng.choice(len(sp), 6, replace=False):
+        for c in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, c] += 1e-4
+            xm[i, c] -= 1e-4
+            g = (orc.energy_forces_cell(small_model, sp, xp, h, want_forces=False)["E"][0]
+                 - orc.energy_forces_cell(small_model, sp, xm, h, want_forces=False)["E"][0]) / 2e-4
+            assert abs(-g - r["F"][i, c]) < 2e-6 * max(1.0, np.abs(r["F"]).max())
+    e = 2e-5
+    for a in range(3):
+        for b in range(3):
+            eps = np.zeros((3, 3))
+            eps[a, b] = e
+            Ep = orc.energy_forces_cell(small_model, sp, x @ (np.eye(3) + eps), h @ (np.eye(3) + eps), want_forces=False)["E"][0]
+            Em = orc.energy_forces_cell(small_model, sp, x @ (np.eye(3) - eps), h @ (np.eye(3) - eps), want_forces=False)["E"][0]
+            assert abs((Ep - Em) / (2 * e) - r["virial"][a, b]) < 3e-7 * r["virial_abs"], (a, b)
+    assert np.abs(r["virial"] - r["virial"].T).max() < 1e-11 * r["virial_abs"]
+    assert np.abs(r["F"].sum(0)).max() < 1e-9
+
+
+def test_cell_rotation_covariance_and_md_reduces_to_box_md(small_model):
+    """Rotating cell and coordinates together leaves E and rotates F; orc_md_cell on a wide diagonal cell is orc_md."""
+    sp, xyz, box = _small_water(8, 6.2, 6)
+    h = np.diag(box) @ np.array([[1.0, 0.0, 0.0], [0.2, 1.0, 0.0], [0.1, -0.15, 1.0]])
+    R = rot(4)
+    a = orc.energy_forces_cell(small_model, sp, xyz, h)
+    b = orc.energy_forces_cell(small_model, sp, xyz @ R.T, h @ R.T)
+    assert abs(a["E"][0] - b["E"][0]) < 1e-10 * abs(a["E"][0]) and np.abs(a["F"] @ R.T - b["F"]).max() < 1e-9
+    sp, xyz, box = inputs.water_box(64, 12.42, seed=inputs.SEED0 + 1)
+    v = inputs.maxwell_boltzmann(sp, 300.0, seed=3)
+    m1 = orc.md(small_model, sp, xyz, v, inputs.MASS, box, 0.5, inputs.ACCEL_CONV, 3)
+    m2 = orc.md_cell(small_model, sp, xyz, v, inputs.MASS, np.diag(box), 0.5, inputs.ACCEL_CONV, 3)
+    assert np.abs(m1["xyz"] - m2["xyz"]).max() < 1e-12 and np.abs(m1["epot"] - m2["epot"]).max() < 1e-9
