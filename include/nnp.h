@@ -117,6 +117,20 @@ const char *nnp_last_error(const nnp_ctx *ctx); /* ctx may be NULL (create failu
 int nnp_set_system(nnp_ctx *ctx, int n_atoms, const int32_t *d_species, const float *d_xyz,
                    const float h_box[3], int n_mols, const int32_t *d_mol_offsets);
 
+/* The same with a GENERAL cell ("optionally cell vectors", L49, L307 "minimum image or
+ * all images"): h_cell[9] (host), rows = the lattice vectors a, b, c in Angstrom, any orientation, triclinic allowed; NULL or
+ * all zero = non-periodic.  Atoms interact with ALL periodic images inside the cutoffs:
+ *   - every perpendicular width of the cell >= 2 (rcr + 0.5 A): minimum image, found by rounding the displacement's
+ *     fractional coordinates (a diagonal cell takes exactly the orthorhombic path of nnp_set_system);
+ *   - a narrower cell (down to cells smaller than the cutoff, where an atom sees several images of the same neighbour and
+ *     of itself) is evaluated, exactly, as the smallest m0 x m1 x m2 supercell that reaches that width: the library holds
+ *     n_atoms * m0 m1 m2 internal atoms (this product must be <= max_atoms, else NNP_EBOX), returns energy / virial per
+ *     cell and the forces, AEVs, neighbour rows (an image of atom j is reported as j) of the caller's atoms.  One
+ *     structure only; energy / forces / virial only (nnp_md_init returns NNP_EINVAL: pass the supercell yourself).
+ * nnp_build_neighbors returns NNP_EBOX if a width of the (super)cell is below 2 (rcr + skin). */
+int nnp_set_system_cell(nnp_ctx *ctx, int n_atoms, const int32_t *d_species, const float *d_xyz, const float h_cell[9],
+                        int n_mols, const int32_t *d_mol_offsets);
+
 /* Replaces the coordinates of the loaded system ([n][3], original order); lists stay as they are (the
  * caller asserts no atom moved more than skin/2 since nnp_build_neighbors). */
 int nnp_set_positions(nnp_ctx *ctx, const float *d_xyz);
@@ -137,7 +151,7 @@ int nnp_get_neighbors(nnp_ctx *ctx, int which, int32_t *d_counts, int32_t *d_lis
 int nnp_energy_forces(nnp_ctx *ctx, double *d_energy, float *d_forces);
 
 /* Energy, forces and the virial of ONE structure (n_mols = 1; PAPER.md L262 energy_and_forces_and_virial, SURVEY.md
- * 8(f) item 2, orthorhombic cells): d_virial[9] fp64, row-major V_ab = dE/d eps_ab = sum over every displacement
+ * 8(f) item 2; any cell of nnp_set_system / nnp_set_system_cell): d_virial[9] fp64, row-major V_ab = dE/d eps_ab = sum over every displacement
  * vector d the energy is built from of d_a (dE/dd)_b -- the derivative of the energy under the homogeneous
  * deformation x -> (1 + eps) x, cell -> (1 + eps) cell; symmetric; stress = V / volume; without a cell
  * V_ab = -sum_i x_ia F_ib.  Accumulated in fp32 per lane and in fp64 across warps by the reverse AEV kernel.

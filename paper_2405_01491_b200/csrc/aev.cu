@@ -120,7 +120,15 @@ __device__ __forceinline__ float2 bc2(const float s) { return make_float2(s, s);
 __device__ __forceinline__ float3 min_image(const float4 a, const float4 b, const AevParams &P)
 {
     float dx = b.x - a.x, dy = b.y - a.y, dz = b.z - a.z;
-    if (P.periodic) {
+    if (P.tric) { // general cell: take off the lattice vector nearest in fractional coordinates (neighbor.cu r2_defined)
+        const float M = 12582912.0f;
+        const float k0 = (P.hinv[0] * dx + P.hinv[1] * dy + P.hinv[2] * dz + M) - M;
+        const float k1 = (P.hinv[3] * dx + P.hinv[4] * dy + P.hinv[5] * dz + M) - M;
+        const float k2 = (P.hinv[6] * dx + P.hinv[7] * dy + P.hinv[8] * dz + M) - M;
+        dx -= k0 * P.h[0] + k1 * P.h[3] + k2 * P.h[6];
+        dy -= k0 * P.h[1] + k1 * P.h[4] + k2 * P.h[7];
+        dz -= k0 * P.h[2] + k1 * P.h[5] + k2 * P.h[8];
+    } else if (P.periodic) {
         // round-to-nearest by the 1.5 * 2^23 trick: two FADDs on the FMA pipe instead of an FRND on the XU pipe
         // (|d / L| < 2^22 always); any consistent choice of image is fine here, list membership is decided in stage 1
         const float M = 12582912.0f;

@@ -131,11 +131,11 @@ __global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restr
 // E_mol += e_atom * inv_nets + e_shift[species]   (fp64 accumulation; block-reduced when there is one structure)
 __global__ void k_energy_reduce(int n, const float *__restrict__ e_atom, const int *__restrict__ spc,
                                 const int *__restrict__ mol, const float *__restrict__ e_shift, float inv_nets,
-                                int single, double *__restrict__ e_mol)
+                                double inv_rep, int single, double *__restrict__ e_mol)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     double e = 0.0;
-    if (i < n) e = (double)e_atom[i] * (double)inv_nets + (double)e_shift[spc[i]];
+    if (i < n) e = ((double)e_atom[i] * (double)inv_nets + (double)e_shift[spc[i]]) * inv_rep; // per cell of a replicated small cell
     if (!single) {
         add_per_structure(i < n, i < n ? mol[i] : -1, e, e_mol);
         return;
@@ -152,12 +152,14 @@ __global__ void k_energy_reduce(int n, const float *__restrict__ e_atom, const i
     }
 }
 
-__global__ void k_unpermute3(int n, const float4 *__restrict__ src, const int *__restrict__ orig, float *__restrict__ dst)
+// (n_user: the caller's atoms; internal atoms with orig >= n_user are the extra copies of a replicated small cell)
+__global__ void k_unpermute3(int n, const float4 *__restrict__ src, const int *__restrict__ orig, int n_user, float *__restrict__ dst)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float4 v = src[i];
     const int o = orig[i];
+    if (o >= n_user) return;
     dst[3 * o] = v.x; dst[3 * o + 1] = v.y; dst[3 * o + 2] = v.z;
 }
 
@@ -170,12 +172,13 @@ __global__ void k_permute_in3(int n, const float *__restrict__ src, const int *_
 }
 
 __global__ void k_unpermute3x2(int n, const float4 *__restrict__ srcA, const float4 *__restrict__ srcB,
-                               const int *__restrict__ orig, float *__restrict__ dstA, float *__restrict__ dstB)
+                               const int *__restrict__ orig, int n_user, float *__restrict__ dstA, float *__restrict__ dstB)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float4 a = srcA[i], b = srcB[i];
     const int o = orig[i];
+    if (o >= n_user) return;
     dstA[3 * o] = a.x; dstA[3 * o + 1] = a.y; dstA[3 * o + 2] = a.z;
     dstB[3 * o] = b.x; dstB[3 * o + 1] = b.y; dstB[3 * o + 2] = b.z;
 }
@@ -203,7 +206,7 @@ __global__ void k_pack_result(const double *__restrict__ e_mol, const double *__
 
 void nnp_launch_unpermute3x2(nnp_ctx *c, const float4 *srcA, float *dstA, const float4 *srcB, float *dstB)
 {
-    k_unpermute3x2<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, srcA, srcB, c->orig, dstA, dstB);
+    k_unpermute3x2<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, srcA, srcB, c->orig, c->n_user, dstA, dstB);
     c->launches += 1;
 }
 
@@ -247,13 +250,13 @@ void nnp_launch_energy_reduce(nnp_ctx *c)
 {
     cudaMemsetAsync(c->e_mol, 0, sizeof(double) * c->n_mols, c->stream);
     k_energy_reduce<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->e_atom, c->spc, c->mol, c->d_e_shift,
-                                                             1.0f / (float)c->n_nets, c->n_mols == 1, c->e_mol);
+                                                             1.0f / (float)c->n_nets, 1.0 / (double)c->rep, c->n_mols == 1, c->e_mol);
     c->launches += 1;
 }
 
 void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst)
 {
-    k_unpermute3<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, src, c->orig, dst);
+    k_unpermute3<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, src, c->orig, c->n_user, dst);
     c->launches += 1;
 }
 

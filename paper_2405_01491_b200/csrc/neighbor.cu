@@ -27,9 +27,23 @@ __device__ __forceinline__ int cell_coord_frac(float x, float L, float invL, flo
     return c;
 }
 
+// general cell: fractional coordinate c of x, wrapped into [0, 1)
+__device__ __forceinline__ float frac_wrapped(const float4 p, const GridInfo &g, int c)
+{
+    const float s = g.hinv[3 * c] * p.x + g.hinv[3 * c + 1] * p.y + g.hinv[3 * c + 2] * p.z;
+    const float w = s - floorf(s);
+    return w < 1.0f ? w : 0.0f;
+}
+
 __device__ __forceinline__ int cell_of(const float4 p, const GridInfo &g, int mol)
 {
     if (!g.periodic) return mol;
+    if (g.tric) { // bins cut in fractional coordinates (cell_scale = nc)
+        const int cx = min((int)(frac_wrapped(p, g, 0) * g.cell_scale[0]), g.nc[0] - 1);
+        const int cy = min((int)(frac_wrapped(p, g, 1) * g.cell_scale[1]), g.nc[1] - 1);
+        const int cz = min((int)(frac_wrapped(p, g, 2) * g.cell_scale[2]), g.nc[2] - 1);
+        return mol * g.ncell_box + (cz * g.nc[1] + cy) * g.nc[0] + cx;
+    }
     int cx = cell_coord(p.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0]);
     int cy = cell_coord(p.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1]);
     int cz = cell_coord(p.z, g.box[2], g.inv_box[2], g.cell_scale[2], g.nc[2]);
@@ -190,7 +204,16 @@ __global__ void k_copyback(int n, const float4 *__restrict__ pos_t, const float4
 __device__ __forceinline__ float r2_defined(const float4 a, const float4 b, const GridInfo &g)
 {
     float dx = __fsub_rn(b.x, a.x), dy = __fsub_rn(b.y, a.y), dz = __fsub_rn(b.z, a.z);
-    if (g.periodic) {
+    if (g.tric) {
+        // General cell: the lattice vector k_0 a + k_1 b + k_2 c nearest in fractional coordinates is taken
+        // off; exact minimum image for every |d| below half the smallest perpendicular width, which setup_grid enforces.
+        const float k0 = rintf(g.hinv[0] * dx + g.hinv[1] * dy + g.hinv[2] * dz);
+        const float k1 = rintf(g.hinv[3] * dx + g.hinv[4] * dy + g.hinv[5] * dz);
+        const float k2 = rintf(g.hinv[6] * dx + g.hinv[7] * dy + g.hinv[8] * dz);
+        dx -= k0 * g.h[0] + k1 * g.h[3] + k2 * g.h[6];
+        dy -= k0 * g.h[1] + k1 * g.h[4] + k2 * g.h[7];
+        dz -= k0 * g.h[2] + k1 * g.h[5] + k2 * g.h[8];
+    } else if (g.periodic) {
         dx = __fsub_rn(dx, __fmul_rn(g.box[0], rintf(__fmul_rn(dx, g.inv_box[0]))));
         dy = __fsub_rn(dy, __fmul_rn(g.box[1], rintf(__fmul_rn(dy, g.inv_box[1]))));
         dz = __fsub_rn(dz, __fmul_rn(g.box[2], rintf(__fmul_rn(dz, g.inv_box[2]))));
@@ -222,7 +245,25 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
     // range `lane` of the stencil: first / last cell (inside one species block) and whether it exists
     int c_first = 0, c_last = 0, nranges = 1;
     bool rng_ok = true; // false: no atom of this range can be inside the list radius
-    if (g.periodic) {
+    if (g.tric) { // general cell: the whole 3 x 3 x 3 stencil of fractional bins (every bin is at least the list radius wide)
+        const int cx = min((int)(frac_wrapped(pi, g, 0) * g.cell_scale[0]), g.nc[0] - 1);
+        const int cy = min((int)(frac_wrapped(pi, g, 1) * g.cell_scale[1]), g.nc[1] - 1);
+        const int cz = min((int)(frac_wrapped(pi, g, 2) * g.cell_scale[2]), g.nc[2] - 1);
+        const int nys = g.nc[1] >= 3 ? 3 : g.nc[1], nzs = g.nc[2] >= 3 ? 3 : g.nc[2];
+        const int nxs = (g.nc[0] > 3 && (cx == 0 || cx == g.nc[0] - 1)) ? 2 : 1;
+        nranges = nzs * nys * nxs;
+        const int ix = lane % nxs, t = lane / nxs, iy = t % nys, iz = t / nys;
+        const int y = nys == 3 ? (cy + iy + g.nc[1] - 1) % g.nc[1] : iy;
+        const int z = nzs == 3 ? (cz + iz + g.nc[2] - 1) % g.nc[2] : iz;
+        int xa, xb;
+        if (g.nc[0] <= 3) { xa = 0; xb = g.nc[0] - 1; }
+        else if (cx == 0) { xa = ix ? g.nc[0] - 1 : 0; xb = ix ? g.nc[0] - 1 : 1; }
+        else if (cx == g.nc[0] - 1) { xa = ix ? 0 : cx - 1; xb = ix ? 0 : cx; }
+        else { xa = cx - 1; xb = cx + 1; }
+        const int rowbase = mol[i] * g.ncell_box + (z * g.nc[1] + y) * g.nc[0];
+        c_first = rowbase + xa;
+        c_last = rowbase + xb;
+    } else if (g.periodic) {
         float fx, fy, fz;
         const int cx = cell_coord_frac(pi.x, g.box[0], g.inv_box[0], g.cell_scale[0], g.nc[0], fx);
         const int cy = cell_coord_frac(pi.y, g.box[1], g.inv_box[1], g.cell_scale[1], g.nc[1], fy);

@@ -71,12 +71,41 @@ namespace {
 
 constexpr int T = 256;
 
+void cross3f(const double *u, const double *v, double *o)
+{
+    o[0] = u[1] * v[2] - u[2] * v[1]; o[1] = u[2] * v[0] - u[0] * v[2]; o[2] = u[0] * v[1] - u[1] * v[0];
+}
+
+// Copy m = (m0, m1, m2) of a replicated small cell: shift m0 a + m1 b + m2 c of the caller's cell (rows of cu).
+struct RepInfo { int n_user, m[3]; float cu[9]; };
+__device__ __forceinline__ float3 rep_shift(const RepInfo &r, int copy)
+{
+    const int m0 = copy % r.m[0], m1 = (copy / r.m[0]) % r.m[1], m2 = copy / (r.m[0] * r.m[1]);
+    return make_float3((float)m0 * r.cu[0] + (float)m1 * r.cu[3] + (float)m2 * r.cu[6],
+                       (float)m0 * r.cu[1] + (float)m1 * r.cu[4] + (float)m2 * r.cu[7],
+                       (float)m0 * r.cu[2] + (float)m1 * r.cu[5] + (float)m2 * r.cu[8]);
+}
+
 __global__ void k_init_system(int n, const int *__restrict__ species, const float *__restrict__ xyz,
                               const int *__restrict__ mol_offsets, int n_mols, float4 *__restrict__ pos,
                               float4 *__restrict__ vel, int *__restrict__ spc, int *__restrict__ orig,
-                              int *__restrict__ mol, int *__restrict__ counts, int S, int *__restrict__ bad)
+                              int *__restrict__ mol, int *__restrict__ counts, int S, int *__restrict__ bad, RepInfo rep)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (rep.n_user < n) { // replicated cell (one structure): internal atom e = copy * n_user + a
+        if (i >= n) return;
+        const int a = i % rep.n_user;
+        const float3 sh = rep_shift(rep, i / rep.n_user);
+        int s = species[a];
+        if (s < 0 || s >= S) { atomicOr(bad, 1); s = 0; }
+        pos[i] = make_float4(xyz[3 * a] + sh.x, xyz[3 * a + 1] + sh.y, xyz[3 * a + 2] + sh.z, 0.f);
+        vel[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        spc[i] = s;
+        orig[i] = i;
+        mol[i] = 0;
+        atomicAdd(&counts[s], 1);
+        return;
+    }
     if (mol_offsets) { // offsets[0] = 0 <= offsets[1] <= ... <= offsets[n_mols] = n, checked by a grid-stride loop
         for (int m = i; m <= n_mols; m += gridDim.x * blockDim.x) {
             const int o = mol_offsets[m];
@@ -101,24 +130,38 @@ __global__ void k_init_system(int n, const int *__restrict__ species, const floa
     atomicAdd(&counts[s], 1);
 }
 
+__global__ void k_set_positions_rep(int n, const float *__restrict__ src, const int *__restrict__ orig, float4 *__restrict__ dst,
+                                    RepInfo rep)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int e = orig[i], a = e % rep.n_user;
+    const float3 sh = rep_shift(rep, e / rep.n_user);
+    dst[i] = make_float4(src[3 * a] + sh.x, src[3 * a + 1] + sh.y, src[3 * a + 2] + sh.z, 0.f);
+}
+
+// rows of the caller's atoms (copies 0 of a replicated cell); an image of atom j is reported as j
 __global__ void k_get_neighbors(int n, const int *__restrict__ nbr, const uint16_t *__restrict__ seg, int cap,
-                                const int *__restrict__ orig, int *__restrict__ counts, int *__restrict__ list, int stride)
+                                const int *__restrict__ orig, int n_user, int *__restrict__ counts, int *__restrict__ list,
+                                int stride)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int o = orig[i];
+    if (o >= n_user) return;
     const int cnt = seg[(size_t)i * NNP_MAX_SPECIES + NNP_MAX_SPECIES - 1];
     counts[o] = cnt;
-    for (int a = 0; a < cnt && a < stride; ++a) list[(size_t)o * stride + a] = orig[nbr[(size_t)i * cap + a]];
+    for (int a = 0; a < cnt && a < stride; ++a) list[(size_t)o * stride + a] = orig[nbr[(size_t)i * cap + a]] % n_user;
 }
 
 // Test hook: active columns of G -> the full aev_len layout (columns of absent species are zero).
 __global__ void k_get_aev(int n, int len_full, int len_c, int kpad, const float *__restrict__ G, const int *__restrict__ fmap,
-                          const int *__restrict__ orig, float *__restrict__ out)
+                          const int *__restrict__ orig, int n_user, float *__restrict__ out)
 {
     int i = blockIdx.x;
     if (i >= n) return;
     const int o = orig[i];
+    if (o >= n_user) return;
     for (int q = threadIdx.x; q < len_full; q += blockDim.x) out[(size_t)o * len_full + q] = 0.f;
     __syncthreads();
     for (int q = threadIdx.x; q < len_c; q += blockDim.x) out[(size_t)o * len_full + fmap[q]] = G[(size_t)i * kpad + q];
@@ -146,11 +189,11 @@ __global__ void k_gather_l1(int kpad, int out, const int *__restrict__ fmap, con
 }
 
 __global__ void k_get_e_atom(int n, const float *__restrict__ e_atom, const int *__restrict__ spc,
-                             const float *__restrict__ e_shift, float inv_nets, const int *__restrict__ orig,
+                             const float *__restrict__ e_shift, float inv_nets, const int *__restrict__ orig, int n_user,
                              float *__restrict__ out)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    if (i >= n || orig[i] >= n_user) return;
     out[orig[i]] = e_atom[i] * inv_nets + e_shift[spc[i]];
 }
 
@@ -447,16 +490,26 @@ int setup_grid(nnp_ctx *c, float skin)
     g.periodic = c->periodic;
     if (c->periodic) {
         long ncell = 1;
+        double h[9], rec[9];
+        for (int q = 0; q < 9; ++q) h[q] = c->cell[q];
+        cross3f(h + 3, h + 6, rec); cross3f(h + 6, h, rec + 3); cross3f(h, h + 3, rec + 6);
+        const double vol = h[0] * rec[0] + h[1] * rec[1] + h[2] * rec[2];
+        g.tric = c->tric;
+        for (int q = 0; q < 9; ++q) { g.h[q] = c->cell[q]; g.hinv[q] = (float)(rec[q] / vol); }
         for (int d = 0; d < 3; ++d) {
-            if (c->box[d] < 2.0f * rl)
-                NNP_FAIL(c, NNP_EBOX, "box edge %g < 2*(rcr+skin) = %g: minimum image not unique", c->box[d], 2.0f * rl);
-            int nc = (int)floorf(c->box[d] / (rl * 1.0001f));
+            // perpendicular width of the (super)cell along lattice direction d (= the edge of an orthorhombic box)
+            const float w = c->tric ? (float)(fabs(vol) / sqrt(rec[3 * d] * rec[3 * d] + rec[3 * d + 1] * rec[3 * d + 1] + rec[3 * d + 2] * rec[3 * d + 2]))
+                                    : c->box[d];
+            if (w < 2.0f * rl)
+                NNP_FAIL(c, NNP_EBOX, "cell width %g < 2*(rcr+skin) = %g: minimum image not unique%s", w, 2.0f * rl,
+                         c->rep > 1 ? " (the supercell of a small cell is sized for a skin of 0.5 A)" : "");
+            int nc = (int)floorf(w / (rl * 1.0001f));
             if (nc < 1) nc = 1;
             if (nc > 128) nc = 128;
             g.nc[d] = nc;
             g.box[d] = c->box[d];
             g.inv_box[d] = 1.0f / c->box[d];
-            g.cell_scale[d] = (float)nc / c->box[d];
+            g.cell_scale[d] = c->tric ? (float)nc : (float)nc / c->box[d];
             ncell *= nc;
         }
         // a periodic batch (replicas of one cell, e.g. the beads of a ring polymer): one bin set per replica
@@ -482,7 +535,9 @@ int setup_grid(nnp_ctx *c, float skin)
     }
     CU(c, cudaMemsetAsync(c->cursor, 0, sizeof(int) * nk, c->stream));
     c->aev.periodic = c->periodic;
+    c->aev.tric = g.tric;
     for (int d = 0; d < 3; ++d) { c->aev.box[d] = g.box[d]; c->aev.inv_box[d] = g.inv_box[d]; }
+    for (int q = 0; q < 9; ++q) { c->aev.h[q] = g.h[q]; c->aev.hinv[q] = g.hinv[q]; }
     return NNP_OK;
 }
 
@@ -781,21 +836,48 @@ int nnp_create(nnp_ctx **out, const nnp_params *p, int max_atoms, int max_mols, 
     return NNP_OK;
 }
 
-int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const float *d_xyz, const float h_box[3],
-                   int n_mols, const int32_t *d_mol_offsets)
+// cells narrower than this are replicated into the smallest supercell that reaches it (nnp_set_system_cell)
+static const float kPbcSkinReserve = 0.5f;
+
+static int set_system_impl(nnp_ctx *c, int n_atoms, const int32_t *d_species, const float *d_xyz, const float cell[9],
+                           int n_mols, const int32_t *d_mol_offsets)
 {
-    if (!c) return NNP_EINVAL;
-    static const float zero_box[3] = {0.f, 0.f, 0.f};
-    if (!h_box) h_box = zero_box;
     if (n_atoms > 0 && (!d_species || !d_xyz)) NNP_FAIL(c, NNP_EINVAL, "null argument");
     if (n_atoms < 0 || n_atoms > c->max_atoms) NNP_FAIL(c, NNP_EINVAL, "n_atoms %d outside [0, max_atoms=%d]", n_atoms, c->max_atoms);
     if (!d_mol_offsets) n_mols = 1;
     if (n_mols < 1 || n_mols > c->max_mols) NNP_FAIL(c, NNP_EINVAL, "n_mols %d outside [1, max_mols=%d]", n_mols, c->max_mols);
-    const int nper = (h_box[0] > 0.f) + (h_box[1] > 0.f) + (h_box[2] > 0.f);
-    if (nper != 0 && nper != 3) NNP_FAIL(c, NNP_EINVAL, "box must be all zero (non-periodic) or all positive");
+    bool any = false;
+    for (int q = 0; q < 9; ++q) any = any || cell[q] != 0.f;
+    int periodic = 0, tric = 0, m[3] = {1, 1, 1};
+    if (any) {
+        double h[9], rec[9];
+        for (int q = 0; q < 9; ++q) h[q] = cell[q];
+        cross3f(h + 3, h + 6, rec); cross3f(h + 6, h, rec + 3); cross3f(h, h + 3, rec + 6);
+        const double vol = h[0] * rec[0] + h[1] * rec[1] + h[2] * rec[2];
+        if (!(fabs(vol) > 1e-12)) NNP_FAIL(c, NNP_EINVAL, "cell vectors must be all zero (non-periodic) or span a volume");
+        periodic = 1;
+        tric = cell[1] != 0.f || cell[2] != 0.f || cell[3] != 0.f || cell[5] != 0.f || cell[6] != 0.f || cell[7] != 0.f;
+        if (!tric && (cell[0] <= 0.f || cell[4] <= 0.f || cell[8] <= 0.f)) NNP_FAIL(c, NNP_EINVAL, "box edges must be positive");
+        const double need = 2.0 * ((double)c->aev.rcr + (double)kPbcSkinReserve);
+        for (int d = 0; d < 3; ++d) {
+            const double w = fabs(vol) / sqrt(rec[3 * d] * rec[3 * d] + rec[3 * d + 1] * rec[3 * d + 1] + rec[3 * d + 2] * rec[3 * d + 2]);
+            if (w < need) m[d] = (int)ceil(need / w - 1e-9);
+        }
+    }
+    const long rep = (long)m[0] * m[1] * m[2];
+    if (rep > 1) {
+        if (n_mols != 1) NNP_FAIL(c, NNP_EBOX, "a batch of cells narrower than 2 (rcr + 0.5 A) is not supported");
+        if ((long)n_atoms * rep > c->max_atoms)
+            NNP_FAIL(c, NNP_EBOX, "cell narrower than 2 (rcr + 0.5 A): all periodic images are evaluated on a %d x %d x %d supercell, "
+                     "which needs max_atoms >= %ld", m[0], m[1], m[2], (long)n_atoms * rep);
+    }
     CU(c, cudaSetDevice(c->device));
-    c->n = n_atoms; c->n_mols = n_mols; c->periodic = nper == 3;
-    for (int d = 0; d < 3; ++d) c->box[d] = h_box[d];
+    c->n_user = n_atoms; c->rep = (int)rep; c->n = n_atoms * (int)rep; c->n_mols = n_mols; c->periodic = periodic; c->tric = tric;
+    for (int d = 0; d < 3; ++d) {
+        c->rep_m[d] = m[d];
+        for (int q = 0; q < 3; ++q) { c->cell_user[3 * d + q] = cell[3 * d + q]; c->cell[3 * d + q] = (float)m[d] * cell[3 * d + q]; }
+        c->box[d] = c->cell[4 * d];
+    }
     c->have_system = 1; c->have_lists = 0; c->have_forces = 0; c->md_ready = 0;
     drop_md_graph(c);
     int *bins = c->flags + 8; // [8..15] species histogram, [3] bad-species marker
@@ -804,9 +886,13 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
     if (n_atoms > 0) {
         if (d_mol_offsets)
             CU(c, cudaMemcpyAsync(c->mol_offsets, d_mol_offsets, sizeof(int) * (n_mols + 1), cudaMemcpyDeviceToDevice, c->stream));
-        k_init_system<<<nnp_div_up(n_atoms, T), T, 0, c->stream>>>(n_atoms, d_species, d_xyz, d_mol_offsets ? c->mol_offsets : nullptr,
-                                                                   n_mols, c->pos, c->vel, c->spc, c->orig, c->mol, bins, c->S,
-                                                                   c->flags + 3);
+        RepInfo ri;
+        ri.n_user = n_atoms;
+        for (int d = 0; d < 3; ++d) ri.m[d] = m[d];
+        for (int q = 0; q < 9; ++q) ri.cu[q] = cell[q];
+        k_init_system<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, d_species, d_xyz, d_mol_offsets ? c->mol_offsets : nullptr,
+                                                                n_mols, c->pos, c->vel, c->spc, c->orig, c->mol, bins, c->S,
+                                                                c->flags + 3, ri);
         c->launches += 1;
         int bad = 0;
         CU(c, cudaMemcpyAsync(h_counts, bins, sizeof(int) * NNP_MAX_SPECIES, cudaMemcpyDeviceToHost, c->stream));
@@ -829,12 +915,42 @@ int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const floa
     return nnp_fused_setup(c);
 }
 
+int nnp_set_system(nnp_ctx *c, int n_atoms, const int32_t *d_species, const float *d_xyz, const float h_box[3],
+                   int n_mols, const int32_t *d_mol_offsets)
+{
+    if (!c) return NNP_EINVAL;
+    float cell[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (h_box) {
+        const int nper = (h_box[0] > 0.f) + (h_box[1] > 0.f) + (h_box[2] > 0.f);
+        if (nper != 0 && nper != 3) NNP_FAIL(c, NNP_EINVAL, "box must be all zero (non-periodic) or all positive");
+        cell[0] = h_box[0]; cell[4] = h_box[1]; cell[8] = h_box[2];
+    }
+    return set_system_impl(c, n_atoms, d_species, d_xyz, cell, n_mols, d_mol_offsets);
+}
+
+int nnp_set_system_cell(nnp_ctx *c, int n_atoms, const int32_t *d_species, const float *d_xyz, const float h_cell[9],
+                        int n_mols, const int32_t *d_mol_offsets)
+{
+    if (!c) return NNP_EINVAL;
+    static const float zero[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    return set_system_impl(c, n_atoms, d_species, d_xyz, h_cell ? h_cell : zero, n_mols, d_mol_offsets);
+}
+
 int nnp_set_positions(nnp_ctx *c, const float *d_xyz)
 {
     if (!c) return NNP_EINVAL;
     if (!c->have_system || !d_xyz) NNP_FAIL(c, NNP_EINVAL, "no system loaded / null argument");
     if (c->n == 0) return NNP_OK;
-    nnp_launch_permute_in3(c, d_xyz, c->pos);
+    if (c->rep > 1) {
+        RepInfo rep;
+        rep.n_user = c->n_user;
+        for (int d = 0; d < 3; ++d) rep.m[d] = c->rep_m[d];
+        for (int q = 0; q < 9; ++q) rep.cu[q] = c->cell_user[q];
+        k_set_positions_rep<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, d_xyz, c->orig, c->pos, rep);
+        c->launches += 1;
+    } else {
+        nnp_launch_permute_in3(c, d_xyz, c->pos);
+    }
     c->have_forces = 0;
     return NNP_OK;
 }
@@ -865,7 +981,7 @@ int nnp_get_neighbors(nnp_ctx *c, int which, int32_t *d_counts, int32_t *d_list,
     if (!d_counts || !d_list || stride < 1 || (which != 0 && which != 1)) NNP_FAIL(c, NNP_EINVAL, "bad argument");
     if (c->n > 0) {
         k_get_neighbors<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, which ? c->nbr_a : c->nbr_r, which ? c->seg_a : c->seg_r,
-                                                                 which ? c->aev.cap_a : c->aev.cap_r, c->orig, d_counts, d_list, stride);
+                                                                 which ? c->aev.cap_a : c->aev.cap_r, c->orig, c->n_user, d_counts, d_list, stride);
         c->launches += 1;
     }
     return check_flags(c);
@@ -896,10 +1012,10 @@ int nnp_energy_forces(nnp_ctx *c, double *d_energy, float *d_forces)
 }
 
 // symmetric 3x3 from the six sums xx yy zz xy xz yz of the reverse AEV kernel
-__global__ void k_expand_virial(const double *__restrict__ v6, double *__restrict__ v9)
+__global__ void k_expand_virial(const double *__restrict__ v6, double scale, double *__restrict__ v9)
 {
     const int map[9] = {0, 3, 4, 3, 1, 5, 4, 5, 2};
-    if (threadIdx.x < 9) v9[threadIdx.x] = v6[map[threadIdx.x]];
+    if (threadIdx.x < 9) v9[threadIdx.x] = v6[map[threadIdx.x]] * scale;
 }
 
 int nnp_energy_forces_virial(nnp_ctx *c, double *d_energy, float *d_forces, double *d_virial)
@@ -913,7 +1029,7 @@ int nnp_energy_forces_virial(nnp_ctx *c, double *d_energy, float *d_forces, doub
     const int rc = energy_forces_impl(c, d_energy, d_forces);
     c->want_virial = 0;
     if (rc) return rc;
-    k_expand_virial<<<1, 32, 0, c->stream>>>(c->d_virial, d_virial);
+    k_expand_virial<<<1, 32, 0, c->stream>>>(c->d_virial, 1.0 / (double)c->rep, d_virial);
     c->launches += 1;
     CU(c, cudaGetLastError());
     return NNP_OK;
@@ -925,7 +1041,7 @@ int nnp_get_aev(nnp_ctx *c, float *d_aev)
     if (!c->have_lists || !d_aev) NNP_FAIL(c, NNP_ESTALE, "no neighbour list / null argument");
     if (c->n == 0) return NNP_OK;
     nnp_launch_aev_forward(c); // G may have been overwritten by dE/dG: recompute
-    k_get_aev<<<c->n, 128, 0, c->stream>>>(c->n, c->aev_len_full, c->aev.aev_len, c->aev.kpad, c->G, c->d_fmap, c->orig, d_aev);
+    k_get_aev<<<c->n, 128, 0, c->stream>>>(c->n, c->aev_len_full, c->aev.aev_len, c->aev.kpad, c->G, c->d_fmap, c->orig, c->n_user, d_aev);
     c->launches += 1;
     c->have_forces = 0;
     CU(c, cudaGetLastError());
@@ -936,7 +1052,7 @@ int nnp_get_atomic_energies(nnp_ctx *c, float *d_e_atom)
 {
     if (!c) return NNP_EINVAL;
     if (!c->have_forces || !d_e_atom) NNP_FAIL(c, NNP_ESTALE, "nnp_energy_forces first / null argument");
-    k_get_e_atom<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->e_atom, c->spc, c->d_e_shift, 1.0f / c->n_nets, c->orig, d_e_atom);
+    k_get_e_atom<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->e_atom, c->spc, c->d_e_shift, 1.0f / c->n_nets, c->orig, c->n_user, d_e_atom);
     c->launches += 1;
     return NNP_OK;
 }
@@ -947,6 +1063,7 @@ int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
     if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "nnp_set_system first");
     if (!d_vel || !(dt_fs > 0.f) || !(skin > 0.f)) NNP_FAIL(c, NNP_EINVAL, "need velocities, dt > 0, skin > 0");
     if (c->n == 0) NNP_FAIL(c, NNP_EINVAL, "empty system");
+    if (c->rep > 1) NNP_FAIL(c, NNP_EINVAL, "MD on a cell narrower than 2 (rcr + 0.5 A) is not supported: pass the supercell");
     CU(c, cudaSetDevice(c->device));
     nnp_launch_permute_in3(c, d_vel, c->vel);
     c->dt = dt_fs;

@@ -30,6 +30,10 @@ struct GridInfo {
     float box[3];
     float inv_box[3]; // 1.0f / box (IEEE division on the host)
     float cell_scale[3]; // nc / box
+    // general (triclinic) cell: rows of h are the lattice vectors, frac_c(x) = hinv[3c..3c+2] . x; bins are
+    // cut in fractional coordinates.  tric = 0: the orthorhombic arithmetic above (reading A3) is used unchanged.
+    int tric;
+    float h[9], hinv[9];
 };
 
 // ---- AEV constants (stage 2/4), passed to kernels by value --------------------------------------
@@ -68,6 +72,8 @@ struct AevParams {
     float lad_a[NNP_NSHF_A];
     int periodic;
     float box[3], inv_box[3];
+    int tric;                  // general cell: minimum image by rounding the fractional displacement (hinv), then h
+    float h[9], hinv[9];
     // Derived constants of the inner loops, computed once on the host (nnp_aev_derive): the kernels take them straight
     // from the parameter bank (the pairs as one 64-bit uniform-register operand of the packed f32x2 instructions)
     // instead of re-deriving them per loop trip under register pressure.
@@ -174,6 +180,12 @@ struct nnp_ctx {
     // system
     int n, n_mols, periodic, have_system, have_lists, have_forces, md_ready;
     float box[3];
+    // Cells narrower than 2 (rcr + skin) are evaluated as the smallest supercell wide enough for the minimum image: the
+    // caller's n_user atoms are copies 0 of n = n_user * rep internal atoms (internal "original" index e = copy * n_user +
+    // atom); every output is taken from copy 0 and extensive sums are divided by rep (all periodic images, exactly).
+    int n_user, rep, rep_m[3], tric;
+    float cell[9];                  // internal (super)cell, rows = lattice vectors; zero: non-periodic
+    float cell_user[9];
     int bucket_off[NNP_MAX_SPECIES + 1]; // species-major internal order: atoms of species s are [off[s], off[s+1])
     GridInfo grid;
     float skin, dt;

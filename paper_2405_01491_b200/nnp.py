@@ -18,7 +18,7 @@ NNP_MM_FP32_SIMT, NNP_MM_3XTF32_TC, NNP_MM_TF32_TC, NNP_MM_FP64_SIMT, NNP_MM_3XF
 STATUS_NAMES = {0: "NNP_OK", -1: "NNP_EINVAL", -2: "NNP_ENOMEM", -3: "NNP_ECUDA", -4: "NNP_ECAPACITY",
                 -5: "NNP_ESTALE", -6: "NNP_EBOX", -7: "NNP_ERANGE"}
 
-EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp_set_positions",
+EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp_set_system_cell", "nnp_set_positions",
            "nnp_build_neighbors", "nnp_get_neighbors", "nnp_energy_forces", "nnp_get_aev",
            "nnp_get_atomic_energies", "nnp_md_init", "nnp_md_step", "nnp_get_state", "nnp_sync",
            "nnp_energy_forces_host", "nnp_md_step_host", "nnp_profile", "nnp_profile_read", "nnp_launch_count",
@@ -68,6 +68,7 @@ def lib():
         L.nnp_last_error.argtypes = [vp]
         L.nnp_last_error.restype = C.c_char_p
         L.nnp_set_system.argtypes = [vp, C.c_int, ip, fp, C.POINTER(C.c_float), C.c_int, ip]
+        L.nnp_set_system_cell.argtypes = [vp, C.c_int, ip, fp, C.POINTER(C.c_float), C.c_int, ip]
         L.nnp_set_positions.argtypes = [vp, fp]
         L.nnp_build_neighbors.argtypes = [vp, C.c_float]
         L.nnp_get_neighbors.argtypes = [vp, C.c_int, ip, ip, C.c_int]
@@ -163,6 +164,14 @@ def nnp_set_system(ctx, n_atoms, d_species, d_xyz, box, n_mols=1, d_mol_offsets=
     b = (C.c_float * 3)(*[float(x) for x in (box if box is not None else (0, 0, 0))])
     return _check(ctx, lib().nnp_set_system(ctx, int(n_atoms), _ptr(d_species), _ptr(d_xyz), b, int(n_mols),
                                             _ptr(d_mol_offsets)))
+
+
+def nnp_set_system_cell(ctx, n_atoms, d_species, d_xyz, cell, n_mols=1, d_mol_offsets=None):
+    """cell: 3 x 3, rows = lattice vectors (None: non-periodic)."""
+    flat = [0.0] * 9 if cell is None else [float(x) for x in np.asarray(cell, dtype=np.float64).reshape(9)]
+    h = (C.c_float * 9)(*flat)
+    return _check(ctx, lib().nnp_set_system_cell(ctx, int(n_atoms), _ptr(d_species), _ptr(d_xyz), h, int(n_mols),
+                                                 _ptr(d_mol_offsets)))
 
 
 def nnp_set_positions(ctx, d_xyz):

@@ -54,6 +54,27 @@ def gpu_energy_forces(ctx, species, xyz, box, mol_offsets=None, skin=0.0):
     return d_E.cpu().numpy(), d_F.cpu().numpy()[:n].astype(np.float64)
 
 
+def gpu_energy_forces_cell(ctx, species, xyz, cell, skin=0.0, want_virial=False):
+    """One structure in a general cell (rows = lattice vectors) through nnp_set_system_cell."""
+    dev = torch.device("cuda:0")
+    n = len(species)
+    d_sp = torch.as_tensor(np.asarray(species, dtype=np.int32), device=dev)
+    d_x = torch.as_tensor(np.asarray(xyz, dtype=np.float32), device=dev).contiguous()
+    d_E = torch.zeros(1, dtype=torch.float64, device=dev)
+    d_F = torch.zeros((max(n, 1), 3), dtype=torch.float32, device=dev)
+    d_V = torch.zeros(9, dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+    nnp.nnp_set_system_cell(ctx, n, d_sp, d_x, cell)
+    nnp.nnp_build_neighbors(ctx, skin)
+    if want_virial:
+        nnp.nnp_energy_forces_virial(ctx, d_E, d_F, d_V)
+    else:
+        nnp.nnp_energy_forces(ctx, d_E, d_F)
+    nnp.nnp_sync(ctx)
+    out = (d_E.cpu().numpy(), d_F.cpu().numpy()[:n].astype(np.float64))
+    return out + (d_V.cpu().numpy().reshape(3, 3),) if want_virial else out
+
+
 def gpu_neighbors(ctx, which, n, stride=256):
     dev = torch.device("cuda:0")
     d_c = torch.zeros(max(n, 1), dtype=torch.int32, device=dev)

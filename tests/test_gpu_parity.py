@@ -743,3 +743,113 @@ def test_measured_peaks_are_plausible():
     for form in ("ss", "ts"):
         assert 300.0 < pk["tf32_tcgen05_%s_tflops" % form] < 1300.0, pk
         assert 16.0 <= pk["cycles_per_mma_m128n256k8_%s" % form] < 400.0, pk
+
+
+# ---------------------------------------------------------------- SURVEY 8(f)-2, second part: general cells, all periodic images
+def _lists_outside_guard_band(ctx, xyz, cell, n, skin, band=2e-4):
+    """fp64 all-images lists of the oracle against the rows of the caller's atoms (an image of j is reported as j): equal
+    as multisets once the pairs within `band` of the list radius - where fp32 and fp64 may disagree - are set aside."""
+    for which, rc in ((0, 5.1), (1, 3.5)):
+        rl = float(np.float32(rc) + np.float32(skin))
+        got = U.gpu_neighbors(ctx, which, n, stride=640)
+        inner = orc.neighbors_cell(xyz, cell, rl - band)
+        outer = orc.neighbors_cell(xyz, cell, rl + band)
+        for i in range(n):
+            g = sorted(int(j) for j in got[i])
+            lo, hi = sorted(j for j, *_ in inner[i]), sorted(j for j, *_ in outer[i])
+            assert len(lo) <= len(g) <= len(hi), (which, i, len(lo), len(g), len(hi))
+            from collections import Counter
+            cg, cl, ch = Counter(g), Counter(lo), Counter(hi)
+            assert all(cg[j] >= cl[j] for j in cl) and all(ch[j] >= cg[j] for j in cg), (which, i)
+
+
+VIRIAL_RTOL_CELL = 1e-5
+
+
+def test_triclinic_cell_against_oracle(model1):
+    """A sheared 343-water cell (perpendicular widths 20.8 / 19.6 / 22.7 A: minimum image, fractional-coordinate bins):
+    lists, energy, forces and the full virial against the oracle's all-images definition; unwrapped coordinates; then one
+    and ten MD steps against the oracle's integrator in the same cell."""
+    consts, widths, params, om = model1
+    sp, x0, box = inputs.water_box(343, seed=61)
+    D = np.array([[1.0, 0.0, 0.0], [0.21, 0.94, 0.0], [-0.13, 0.17, 1.05]])
+    cell = (np.diag(box) @ D).astype(np.float32).astype(np.float64)
+    rng = np.random.default_rng(1)
+    xyz = (x0 @ D + rng.integers(-2, 3, size=(len(sp), 3)) @ cell).astype(np.float32).astype(np.float64)
+    n = len(sp)
+    dev = torch.device("cuda:0")
+    ctx = U.gpu_create(consts, widths, params, 1, n)
+    try:
+        Eg, Fg, Vg = U.gpu_energy_forces_cell(ctx, sp, xyz, cell, skin=0.3, want_virial=True)
+        _lists_outside_guard_band(ctx, xyz, cell, n, 0.3)
+        ref = orc.energy_forces_cell(om, sp, xyz, cell, want_virial=True)
+        U.assert_parity(Eg, Fg, ref)
+        assert np.abs(Vg - ref["virial"]).max() <= VIRIAL_RTOL_CELL * ref["virial_abs"], (Vg, ref["virial"])
+        # MD in the triclinic cell
+        v = inputs.maxwell_boltzmann(sp, 300.0, seed=5).astype(np.float32).astype(np.float64)
+        d_v = torch.as_tensor(v.astype(np.float32), device=dev)
+        nnp.nnp_md_init(ctx, d_v, 0.5, 0.5)
+        o_x, o_v = torch.zeros((n, 3), device=dev), torch.zeros((n, 3), device=dev)
+        o_ep, o_ek = torch.zeros(1, dtype=torch.float64, device=dev), torch.zeros(1, dtype=torch.float64, device=dev)
+        nnp.nnp_md_step(ctx, 1)
+        nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, None)
+        nnp.nnp_sync(ctx)
+        o1 = orc.md_cell(om, sp, xyz, v, inputs.MASS, cell, 0.5, inputs.ACCEL_CONV, 1)
+        assert np.abs(o_x.cpu().numpy() - o1["xyz"]).max() < 1e-5 and np.abs(o_v.cpu().numpy() - o1["vel"]).max() < 2e-6
+        assert abs(float(o_ep.item()) - o1["epot"][1]) <= 2e-5 * abs(o1["epot"][1])
+        nnp.nnp_md_step(ctx, 30)
+        nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, None)
+        nnp.nnp_sync(ctx)
+        xs = o_x.cpu().numpy().astype(np.float64)
+        r2 = orc.energy_forces_cell(om, sp, xs, cell, want_forces=False)
+        assert abs(float(o_ep.item()) - r2["E"][0]) <= U.E_RTOL * abs(r2["E"][0])
+    finally:
+        nnp.nnp_destroy(ctx)
+
+
+@pytest.mark.parametrize("case", ["cubic_9.31", "cubic_4.9_below_the_cutoff", "triclinic_small"])
+def test_small_cells_see_all_periodic_images(model1, case):
+    """Cells narrower than 2 (rcr + skin), down to one smaller than the cutoff (atoms see their own images and several
+    images of one neighbour): energy per cell, forces, virial and the rows of the caller's atoms against the oracle's
+    explicit sum over images.  The library evaluates the smallest supercell that allows the minimum image."""
+    consts, widths, params, om = model1
+    if case == "cubic_9.31":
+        sp, xyz, box = inputs.water_box(27, 9.31, seed=3)
+        cell, copies = np.diag(box).astype(np.float64), 8
+    elif case == "cubic_4.9_below_the_cutoff":
+        sp, xyz, box = inputs.water_box(4, 4.9, seed=4)
+        cell, copies = np.diag(box).astype(np.float64), 27
+    else:
+        sp, x0, box = inputs.water_box(8, 6.2, seed=6)
+        D = np.array([[1.0, 0.0, 0.0], [0.23, 0.94, 0.0], [-0.17, 0.12, 1.05]])
+        cell = (np.diag(box) @ D).astype(np.float32).astype(np.float64)
+        xyz = (x0 @ D).astype(np.float32).astype(np.float64)
+        copies = 8
+    n = len(sp)
+    ctx = U.gpu_create(consts, widths, params, 1, n * copies, cap_r=320, cap_a=128)
+    try:
+        Eg, Fg, Vg = U.gpu_energy_forces_cell(ctx, sp, xyz, cell, want_virial=True)
+        ref = orc.energy_forces_cell(om, sp, xyz, cell, want_virial=True)
+        U.assert_parity(Eg, Fg, ref)
+        assert np.abs(Vg - ref["virial"]).max() <= VIRIAL_RTOL_CELL * ref["virial_abs"], (Vg, ref["virial"])
+        _lists_outside_guard_band(ctx, xyz, cell, n, 0.0)
+        # AEV rows of the caller's atoms
+        d_aev = torch.zeros((n, 1008), dtype=torch.float32, device="cuda")
+        nnp.nnp_get_aev(ctx, d_aev)
+        nnp.nnp_sync(ctx)
+        aev_ref = orc.energy_forces_cell(om, sp, xyz, cell, want_forces=False, want_aev=True)["aev"]
+        assert np.abs(d_aev.cpu().numpy() - aev_ref).max() < 2e-5 * max(1.0, np.abs(aev_ref).max())
+        # MD on a replicated cell is refused, loudly
+        with pytest.raises(nnp.NnpError) as e:
+            nnp.nnp_md_init(ctx, torch.zeros((n, 3), device="cuda"), 0.5, 0.5)
+        assert e.value.status == nnp.NNP_EINVAL
+    finally:
+        nnp.nnp_destroy(ctx)
+    # a context too small for the supercell says so
+    ctx = U.gpu_create(consts, widths, params, 1, n)
+    try:
+        with pytest.raises(nnp.NnpError) as e:
+            U.gpu_energy_forces_cell(ctx, sp, xyz, cell)
+        assert e.value.status == nnp.NNP_EBOX
+    finally:
+        nnp.nnp_destroy(ctx)
