@@ -117,10 +117,12 @@ __device__ __forceinline__ float2 add2(const float2 a, const float2 b)
 }
 __device__ __forceinline__ float2 bc2(const float s) { return make_float2(s, s); }
 
+// TRIC: general cell (a template parameter of the kernels: the orthorhombic kernels carry none of it)
+template <bool TRIC>
 __device__ __forceinline__ float3 min_image(const float4 a, const float4 b, const AevParams &P)
 {
     float dx = b.x - a.x, dy = b.y - a.y, dz = b.z - a.z;
-    if (P.tric) { // general cell: take off the lattice vector nearest in fractional coordinates (neighbor.cu r2_defined)
+    if (TRIC) { // take off the lattice vector nearest in fractional coordinates (neighbor.cu r2_defined)
         const float M = 12582912.0f;
         const float k0 = (P.hinv[0] * dx + P.hinv[1] * dy + P.hinv[2] * dz + M) - M;
         const float k1 = (P.hinv[3] * dx + P.hinv[4] * dy + P.hinv[5] * dz + M) - M;
@@ -328,7 +330,7 @@ __device__ __forceinline__ void load_centre(Centre &c, const AevParams &P, int i
 
 // Compacts the angular row entries with r < rca into shared memory in row order (= grouped by species); block lane
 // cs < np counts the hits in front of its species segment -> seg[].  Returns the count.
-template <bool BWD, class SM>
+template <bool BWD, bool TRIC, class SM>
 __device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const Centre &c, int i, int lane,
                                              const float4 *__restrict__ pos, const int *__restrict__ nbr_a,
                                              int *__restrict__ flags)
@@ -340,7 +342,7 @@ __device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const C
         float3 d = make_float3(0.f, 0.f, 0.f);
         float r2 = 1.f;
         if (j >= 0) {
-            d = min_image(c.pi, xj, P);
+            d = min_image<TRIC>(c.pi, xj, P);
             r2 = d.x * d.x + d.y * d.y + d.z * d.z;
             hit = r2 < P.rca2;
         }
@@ -387,7 +389,7 @@ __device__ __forceinline__ int stage_angular(SM &sm, const AevParams &P, const C
     return na;
 }
 
-template <bool LAD>
+template <bool LAD, bool TRIC>
 __global__ void __launch_bounds__(kWarps * 32, AEV_FWD_MINB)
 k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
               const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
@@ -428,7 +430,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 #pragma unroll
             for (int k = 0; k < NNP_NSHF_R / 2; ++k) acc[k] = make_float2(0.f, 0.f);
             auto term = [&](const float4 xj) {
-                const float3 d = min_image(c.pi, xj, P);
+                const float3 d = min_image<TRIC>(c.pi, xj, P);
                 const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
                 if (r2 < P.rcr2) {
                     const float r = r2 * rsq(r2);
@@ -502,7 +504,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
             sgr_n = seg_r[(size_t)i_next * NNP_MAX_SPECIES + lane];
             sga_n = seg_a[(size_t)i_next * NNP_MAX_SPECIES + lane];
         }
-        stage_angular<false>(sm, P, c, i, lane, pos, nbr_a, flags);
+        stage_angular<false, TRIC>(sm, P, c, i, lane, pos, nbr_a, flags);
         int n_b = 0;
         if (lane < nb_tot) {
             const int ns = sm.seg[bcs + 1] - sm.seg[bcs], nt = sm.seg[bct + 1] - sm.seg[bct];
@@ -610,7 +612,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 constexpr int kGsMax = 128;  // water: 128 active columns; 2 KiB per block keeps five blocks per SM
 // VIR: also accumulate the virial V_ab = sum_d d_a (dE/dd)_b over every displacement vector the energy is built from
 // (PAPER.md L262): six per-lane sums over all centres of the warp, reduced once at the end.
-template <bool GS, bool VIR>
+template <bool GS, bool VIR, bool TRIC>
 __global__ void __launch_bounds__(kWarps * 32, AEV_BWD_MINB)
 k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__restrict__ nbr_r,
                const uint16_t *__restrict__ seg_r, const int *__restrict__ nbr_a,
@@ -682,7 +684,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 gr[2 * k4 + 1] = make_float2(v.z * sc0, v.w * sc0);
             }
             auto term = [&](int j, const float4 xj) {
-                const float3 d = min_image(c.pi, xj, P);
+                const float3 d = min_image<TRIC>(c.pi, xj, P);
                 const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
                 if (r2 < P.rcr2) {
                     const float rinv = rsq(r2);
@@ -730,7 +732,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
             sgr_n = seg_r[(size_t)i_next * NNP_MAX_SPECIES + lane];
             sga_n = seg_a[(size_t)i_next * NNP_MAX_SPECIES + lane];
         }
-        const int na = stage_angular<true>(sm, P, c, i, lane, pos, nbr_a, flags);
+        const int na = stage_angular<true, TRIC>(sm, P, c, i, lane, pos, nbr_a, flags);
         const bool arena = na <= kMat; // warp-uniform
         if (arena) {
             if (lane < na) sm.ab[lane * kMatLd + lane] = make_float2(0.f, 0.f);
@@ -915,9 +917,10 @@ static int persistent_grid(nnp_ctx *c, int blocks_per_sm)
 
 void nnp_launch_aev_forward(nnp_ctx *c)
 {
-    if (!g_blocks_fwd) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_fwd, k_aev_forward<true>, kWarps * 32, 0);
+    if (!g_blocks_fwd) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&g_blocks_fwd, k_aev_forward<true, false>, kWarps * 32, 0);
     const int grid = persistent_grid(c, g_blocks_fwd);
-    auto kern = c->aev.ladder ? k_aev_forward<true> : k_aev_forward<false>;
+    auto kern = c->aev.tric ? (c->aev.ladder ? k_aev_forward<true, true> : k_aev_forward<false, true>)
+                            : (c->aev.ladder ? k_aev_forward<true, false> : k_aev_forward<false, false>);
     kern<<<grid, kWarps * 32, 0, c->stream>>>(c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a,
                                                                                   c->seg_a, c->d_tri, c->G, c->flags, c->aev_sched, g_sms);
     c->launches += 1;
@@ -928,8 +931,10 @@ void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets, double *d_virial)
     const int gs = c->aev.kpad <= kGsMax ? 1 : 0, vir = d_virial ? 1 : 0;
     const int smem = (int)sizeof(WarpSmemBwd) * kWarps + (gs ? kWarps * kGsMax * 4 : 0);
     static int blocks[2][2] = {{0, 0}, {0, 0}};
-    auto kern = gs ? (vir ? k_aev_backward<true, true> : k_aev_backward<true, false>)
-                   : (vir ? k_aev_backward<false, true> : k_aev_backward<false, false>);
+    auto kern = c->aev.tric ? (gs ? (vir ? k_aev_backward<true, true, true> : k_aev_backward<true, false, true>)
+                                  : (vir ? k_aev_backward<false, true, true> : k_aev_backward<false, false, true>))
+                            : (gs ? (vir ? k_aev_backward<true, true, false> : k_aev_backward<true, false, false>)
+                                  : (vir ? k_aev_backward<false, true, false> : k_aev_backward<false, false, false>));
     if (!blocks[gs][vir]) {
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks[gs][vir], kern, kWarps * 32, smem);
