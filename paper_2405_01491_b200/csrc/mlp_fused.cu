@@ -55,7 +55,7 @@ constexpr int CH = 16;                 // K chunk: one tcgen05.mma kind::f16 K s
 constexpr int MAX_STAGES = 6;
 constexpr int NW = 4;                  // weight ring entries
 constexpr int W_ENTRY_BYTES = 32768;   // hi + lo tiles of up to 128 rows x 128 B
-constexpr int NA = 3;                  // ring of input tiles
+constexpr int NA = 2;                  // ring of input tiles
 constexpr int A_TILE_BYTES = TILE_M * KBF * 4;
 constexpr int EPI_WARPS = 16;
 constexpr int EPI_SETS = EPI_WARPS / 4;
@@ -74,7 +74,8 @@ constexpr int ACT_SHIFT = 4;           // activations enter the tensor core mult
 constexpr float ACT_SCALE = 16.0f;
 constexpr float RANGE_LIMIT = 60000.0f;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
-static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 2) + 8 <= BAR_BYTES, "barrier area");
+static_assert(NA == 2, "input tile k lives in ring entry k & 1: one entry per pair of epilogue sets");
+static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 3) + 8 <= BAR_BYTES, "barrier area");
 
 enum FusedEpi {
     FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> operand
@@ -95,6 +96,7 @@ struct FusedStage {
     int brow;            // forward GEMMs: row of the shared-memory bias table
     float c_acc;         // forward: acc -> 16 z;  FE_ST / FE_RED: acc -> true value
     float gs, gc;        // reverse: out = acc * fma(min(h, 0), gs, gc)  (the scalings folded into CELU')
+    int n_total;         // output columns in all: > N for the last GEMM of a wide chain, which runs in passes of N columns
 };
 
 struct alignas(64) FusedGroup {
@@ -166,7 +168,7 @@ __device__ __forceinline__ int find_group(const FusedGroup *__restrict__ groups,
 // from a loop over the stages, the caller's state went through local memory around every call - which on this kernel is L2.
 template <int EPI>
 __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0, int lane_set, uint32_t tm_acc, uint32_t stg,
-                                         uint32_t accf, uint32_t bar_ready, uint32_t sb, float alpha, int aux)
+                                         uint32_t accf, uint32_t bar_ready, uint32_t sb, float alpha, int aux, int n_cols, int col_off)
 {
     float vmax = 0.f, esum = 0.f;
     constexpr bool fwd = EPI == FE_FWD || EPI == FE_OUT;
@@ -176,13 +178,13 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
     const FusedGroup &g = *gp;
     const FusedStage &st = g.st[j];
     const int lane = lane_set & 31;
-    const int N = st.N, M = g.M;
+    const int N = n_cols, M = g.M; // columns of this accumulator (a pass of the last GEMM of a wide chain: col_off onwards)
     const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
     const int sub_r = (lane >> 3) + 4 * ((lane >> 2) & 1), sub_c = (lane & 3) * 4;
     // rows read (h for CELU') and rows written (h stash, or the chain's output)
-    const float *rd_base = EPI == FE_BWD ? st.stash : g.out;
+    const float *rd_base = EPI == FE_BWD ? st.stash : g.out + col_off;
     const int rd_ld = EPI == FE_BWD ? st.ld_stash : g.ldo;
-    float *wr_base = EPI == FE_FWD ? st.stash : g.out;
+    float *wr_base = EPI == FE_FWD ? st.stash : g.out + col_off;
     const int wr_ld = EPI == FE_FWD ? st.ld_stash : g.ldo;
     const float c_acc = st.c_acc, gs = st.gs, gc = st.gc;
     // everything the chunk loop needs sits in registers: the "memory" clobbers of the asm statements below would make the
@@ -301,7 +303,9 @@ __host__ __device__ constexpr int chain_epi(int chain, int j)
                                  : (j < 2 ? FE_FWD : j == 2 ? FE_OUT : j < 5 ? FE_BWD : chain == CHAIN_FULL_RED ? FE_RED : FE_ST);
 }
 
-template <int CHAIN>
+// WIDE: the chain's input / output has more than 256 columns (first GEMM: operand passes, last GEMM: output passes); the
+// narrow kernels carry none of the pass logic.
+template <int CHAIN, bool WIDE>
 __global__ void __launch_bounds__(THREADS, 1)
 k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__restrict__ cta_tiles, float alpha, int *__restrict__ flags)
 {
@@ -314,8 +318,9 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     const uint32_t bar_afull = bar_base + 16 * NW, bar_aempty = bar_afull + 8 * NA;
     const uint32_t bar_ready = bar_aempty + 8 * NA;            // [2 regions][MAX_CHUNKS]: operand chunk written
     const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_CHUNKS;  // [2 regions]: every MMA into the region has completed
-    const uint32_t bar_drained = bar_accf + 16;                // the last accumulator of a tile has been read
-    const uint32_t tmem_slot = bar_drained + 8;
+    const uint32_t bar_drained = bar_accf + 16;                // an accumulator of the chain's last GEMM has been read
+    const uint32_t bar_pass = bar_drained + 8;                 // wide input: the MMAs of a pass of 16 chunks have completed
+    const uint32_t tmem_slot = bar_pass + 8;
     const uint32_t stg_base = bar_base + BAR_BYTES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -340,6 +345,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         mbar_init(bar_accf, 1);
         mbar_init(bar_accf + 8, 1);
         mbar_init(bar_drained, EPI_WARPS);
+        mbar_init(bar_pass, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -357,41 +363,51 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         // of the NEXT tile are requested while this tile is in its third GEMM (their ring entries are free by then), so that
         // the conversion at the start of a tile never waits for a load queued behind the whole weight stream.
         if (lane == 0) {
-            uint32_t wi = 0, ai = 0;
+            uint32_t wi = 0, aph0 = 0, aph1 = 0; // phases of the two input-ring entries requested so far
             int pre = 0; // input tiles of tile t already requested
             for (int t = t_beg; t < t_end; ++t) {
                 const int gi = find_group(gsm, n_gc, t);
                 const FusedGroup &g = gsm[gi];
                 const int m0 = (t - g.tile0) * TILE_M;
                 const int n_stages = g.n_stages;
+                // Input tile k of a row tile always goes to ring entry k & 1: even tiles (chunks 4i, 4i + 1) are read by the
+                // epilogue sets 0 and 1, odd tiles by sets 2 and 3, so every entry has ONE group of readers that takes each
+                // of its phases in turn.  (An mbarrier wait names a phase by its parity only: a reader that skipped a phase
+                // of an entry - with a ring of three the set pairs alternated on each entry - takes the phase before for its
+                // own and reads a tile that has not arrived; found as rare wrong energies and a hang on a wide chain.)
                 auto load_a = [&](const FusedGroup &gg, int gidx, int row0, int k) {
-                    const uint32_t e = ai % NA;
-                    mbar_wait(bar_aempty + 8 * e, ((ai / NA) & 1) ^ 1, 150, k);
+                    const uint32_t e = (uint32_t)k & 1u;
+                    uint32_t &ph = e ? aph1 : aph0;
+                    mbar_wait(bar_aempty + 8 * e, (ph & 1u) ^ 1u, 150, k);
                     mbar_expect_tx(bar_afull + 8 * e, A_TILE_BYTES);
                     tma_load_2d(a_ring + e * A_TILE_BYTES, &groups[g_lo + gidx].mapA, k * KBF, row0, bar_afull + 8 * e);
-                    ++ai;
+                    ++ph;
                 };
                 int a_next = pre; // next input tile (32 columns) of this tile to request
                 pre = 0;
                 for (int j = 0; j < n_stages; ++j) {
-                    const int K = g.st[j].K, N = g.st[j].N;
-                    const uint8_t *wsrc = g.wblob + g.st[j].w_off;
+                    const int K = g.st[j].K, Np = g.st[j].N;
+                    const int n_total = (WIDE && j + 1 == n_stages) ? g.st[j].n_total : Np;
+                    const uint8_t *wsrc = g.wblob + g.st[j].w_off; // the passes of a wide last GEMM are packed one after the other
                     if (j == 2 && t + 1 < t_end) {
                         const int gn = find_group(gsm, n_gc, t + 1);
                         const FusedGroup &g2 = gsm[gn];
                         const int nka = g2.st[0].K / KBF;
                         for (; pre < NA && pre < nka; ++pre) load_a(g2, gn, (t + 1 - g2.tile0) * TILE_M, pre);
                     }
-                    for (int kb = 0; kb < (K + KBH - 1) / KBH; ++kb) {
-                        if (j == 0)
-                            for (; a_next < 2 * kb + 2 && a_next * KBF < K; ++a_next) load_a(g, gi, m0, a_next);
-                        for (int p = 0; p < (N > 128 ? 2 : 1); ++p, ++wi) {
-                            const uint32_t e = wi % NW;
-                            const uint32_t bytes = 2u * (uint32_t)part_rows(N, p) * 128u; // hi tile, lo tile behind it
-                            mbar_wait(bar_wempty + 8 * e, ((wi / NW) & 1) ^ 1, 100 + j, (t - t_beg) * 100 + kb);
-                            mbar_expect_tx(bar_wfull + 8 * e, bytes);
-                            bulk_load(w_ring + e * W_ENTRY_BYTES, wsrc, bytes, bar_wfull + 8 * e);
-                            wsrc += bytes;
+                    for (int col = 0; col < n_total; col += Np) {
+                        const int N = n_total - col < Np ? n_total - col : Np;
+                        for (int kb = 0; kb < (K + KBH - 1) / KBH; ++kb) {
+                            if (j == 0)
+                                for (; a_next < 2 * kb + 2 && a_next * KBF < K; ++a_next) load_a(g, gi, m0, a_next);
+                            for (int p = 0; p < (N > 128 ? 2 : 1); ++p, ++wi) {
+                                const uint32_t e = wi % NW;
+                                const uint32_t bytes = 2u * (uint32_t)part_rows(N, p) * 128u; // hi tile, lo tile behind it
+                                mbar_wait(bar_wempty + 8 * e, ((wi / NW) & 1) ^ 1, 100 + j, (t - t_beg) * 100 + kb);
+                                mbar_expect_tx(bar_wfull + 8 * e, bytes);
+                                bulk_load(w_ring + e * W_ENTRY_BYTES, wsrc, bytes, bar_wfull + 8 * e);
+                                wsrc += bytes;
+                            }
                         }
                     }
                 }
@@ -405,44 +421,55 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         auto uni = [](uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); };
         const uint32_t tb = uni(tmem_base), wr = uni(w_ring);
         const int tu_beg = (int)uni((uint32_t)t_beg), tu_end = (int)uni((uint32_t)t_end);
-        uint32_t wi = 0, rc = 0, par0 = 0u, par1 = 0u; // parities of the group barriers, one bit per group and region
+        uint32_t wi = 0, rc = 0, par0 = 0u, par1 = 0u; // parities of the chunk barriers, one bit per chunk slot and region
+        uint32_t nd = 0;                               // phases of bar_drained consumed so far
+        bool pending_drain = false;                    // the last accumulator written has not been waited for yet
         for (int t = tu_beg; t < tu_end; ++t) {
             const int gi = (int)uni((uint32_t)find_group(gsm, n_gc, t));
             const FusedGroup &g = gsm[gi];
             const int n_stages = (int)uni((uint32_t)g.n_stages);
-            // the first GEMM of a tile writes the region the previous tile's last accumulator was drained from
-            if (t > tu_beg) { mbar_wait(bar_drained, (uint32_t)(t - tu_beg - 1) & 1, 200, t - tu_beg); tc_fence_after(); }
             for (int j = 0; j < n_stages; ++j) {
-                const int K = (int)uni((uint32_t)g.st[j].K), N = (int)uni((uint32_t)g.st[j].N);
-                const bool wide = N > 128; // two MMAs per product term: columns [0, 128) and [128, N)
+                const int K = (int)uni((uint32_t)g.st[j].K), Np = (int)uni((uint32_t)g.st[j].N);
+                const int n_total = (WIDE && j + 1 == n_stages) ? (int)uni((uint32_t)g.st[j].n_total) : Np;
                 const uint32_t ra = (rc + (uint32_t)j) & 1u, rd = ra ^ 1u;
                 const uint32_t a_base = tb + ra * REGION_COLS, acc = tb + rd * REGION_COLS;
-                const uint32_t rows0 = (uint32_t)part_rows(N, 0), rows1 = wide ? (uint32_t)part_rows(N, 1) : 8u;
-                const uint32_t idesc0 = (1u << 4) | ((rows0 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
-                const uint32_t idesc1 = (1u << 4) | ((rows1 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
                 const int nch_tot = K / CH, nkb = (K + KBH - 1) / KBH;
-                for (int kb = 0; kb < nkb; ++kb) {
-                    const uint32_t e0 = wi % NW, e1 = (wi + 1) % NW;
-                    mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - tu_beg) * 100 + kb);
-                    if (wide) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - tu_beg) * 100 + kb);
-                    const uint32_t b0 = wr + e0 * W_ENTRY_BYTES, b1 = wr + e1 * W_ENTRY_BYTES;
-                    const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + rows0 * 128u);
-                    const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + rows1 * 128u);
-                    const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
-                    // one wait and one election per chunk (measured against the chunks of a K block in one batch, or the first
-                    // alone and the other three together: 0.203 against 0.214 ms for the chain)
-                    for (int h0 = 0; h0 < nh; ++h0) {
-                        const int h1 = h0 + 1;
-                        for (int h = h0; h < h1; ++h) {
-                            const int c = 4 * kb + h;
-                            mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + c), ((ra ? par1 : par0) >> c) & 1u, 240 + j, (t - tu_beg) * 100 + c);
-                            if (ra) par1 ^= 1u << c; else par0 ^= 1u << c;
-                        }
+                // passes: only the last GEMM of a wide chain has more than one (its n_total output columns, Np at a time, from
+                // the same operand into the same region, which the epilogue must have drained in between)
+                int col = 0;
+                do { // (one pass, statically, in the narrow kernels)
+                    const int N = WIDE && n_total - col < Np ? n_total - col : Np;
+                    const bool wide = N > 128; // two MMAs per product term: columns [0, 128) and [128, N)
+                    const uint32_t rows0 = (uint32_t)part_rows(N, 0), rows1 = wide ? (uint32_t)part_rows(N, 1) : 8u;
+                    const uint32_t idesc0 = (1u << 4) | ((rows0 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+                    const uint32_t idesc1 = (1u << 4) | ((rows1 >> 3) << 17) | ((uint32_t)(TILE_M >> 4) << 24);
+                    // the first GEMM of a tile, and every further pass of the last one, write a region whose previous
+                    // accumulator (last GEMM of the previous tile / previous pass) the epilogue must have read
+                    if (pending_drain && (j == 0 || col > 0)) {
+                        mbar_wait(bar_drained, nd & 1u, 200, t - tu_beg);
+                        ++nd;
+                        pending_drain = false;
                         tc_fence_after();
-                        if (elect_one()) {
-                            for (int h = h0; h < h1; ++h) {
-                                const int c = 4 * kb + h;
-                                const uint32_t a_hi = a_base + (uint32_t)(CH * c), a_lo = a_hi + 8;
+                    }
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        const uint32_t e0 = wi % NW, e1 = (wi + 1) % NW;
+                        mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - tu_beg) * 100 + kb);
+                        if (wide) mbar_wait(bar_wfull + 8 * e1, ((wi + 1) / NW) & 1, 230 + j, (t - tu_beg) * 100 + kb);
+                        const uint32_t b0 = wr + e0 * W_ENTRY_BYTES, b1 = wr + e1 * W_ENTRY_BYTES;
+                        const uint64_t d0hi = make_kmajor_sw128_desc(b0), d0lo = make_kmajor_sw128_desc(b0 + rows0 * 128u);
+                        const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + rows1 * 128u);
+                        const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
+                        // one wait and one election per chunk (measured against the chunks of a K block in one batch, or the
+                        // first alone and the other three together: 0.203 against 0.214 ms for the chain)
+                        for (int h = 0; h < nh; ++h) {
+                            const int c = 4 * kb + h, slot = WIDE ? c % MAX_CHUNKS : c; // an operand wider than a region reuses its slots
+                            if (!WIDE || col == 0) { // (further passes multiply the operand that is already there)
+                                mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + slot), ((ra ? par1 : par0) >> slot) & 1u, 240 + j, (t - tu_beg) * 100 + c);
+                                if (ra) par1 ^= 1u << slot; else par0 ^= 1u << slot;
+                                tc_fence_after();
+                            }
+                            if (elect_one()) {
+                                const uint32_t a_hi = a_base + (uint32_t)(CH * slot), a_lo = a_hi + 8;
                                 const uint64_t koff = (uint64_t)(2 * h); // 16 fp16 = 32 B along the swizzled row
                                 mma_f16_ts(acc, a_lo, d0hi + koff, idesc0, c ? 1u : 0u);
                                 mma_f16_ts(acc, a_hi, d0lo + koff, idesc0, 1u);
@@ -452,17 +479,19 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                                     mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
                                     mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
                                 }
+                                if (WIDE && slot == MAX_CHUNKS - 1 && c + 1 < nch_tot) tc_commit(bar_pass); // the slots may be rewritten
+                                if (h + 1 == nh) {
+                                    tc_commit(bar_wempty + 8 * e0);
+                                    if (wide) tc_commit(bar_wempty + 8 * e1);
+                                    if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
+                                }
                             }
-                            if (h1 == nh) {
-                                tc_commit(bar_wempty + 8 * e0);
-                                if (wide) tc_commit(bar_wempty + 8 * e1);
-                                if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
-                            }
+                            __syncwarp();
                         }
-                        __syncwarp();
+                        wi += wide ? 2u : 1u;
                     }
-                    wi += wide ? 2u : 1u;
-                }
+                    if (j + 1 == n_stages) pending_drain = true;
+                } while (WIDE && (col += Np) < n_total);
             }
             rc += (uint32_t)n_stages + 1u;
         }
@@ -475,7 +504,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
         const int row = quarter * 32 + lane;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
         const uint32_t stg = stg_base + (uint32_t)ew * EPI_STG_BYTES;
-        uint32_t rc = 0, use0 = 0u, use1 = 0u, a_cnt = 0;
+        uint32_t rc = 0, use0 = 0u, use1 = 0u, a_ph = 0, pass_cnt = 0; // a_ph: phases of this set's input-ring entry taken so far
         int cur_gi = -1;
         float vmax = 0.f;
         for (int t = t_beg; t < t_end; ++t) {
@@ -502,48 +531,72 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                 // previous tile's last GEMM, which this warp has seen complete (accumulator barrier of that GEMM).
                 const int nch0 = g.st[0].K / CH;
                 const uint32_t r0 = rc & 1u;
-                for (int c = set; c < nch0; c += EPI_SETS) {
-                    const uint32_t ai = a_cnt + (uint32_t)(c >> 1), e = ai % NA;
-                    mbar_wait(bar_afull + 8 * e, (ai / NA) & 1, 300, (t - t_beg) * 100 + c);
-                    const uint32_t arow = a_ring + e * A_TILE_BYTES + row * 128;
-                    float x[16];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const uint32_t addr = arow + (uint32_t)(((4 * (c & 1) + q) ^ (row & 7)) << 4);
-                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[4 * q]), "=f"(x[4 * q + 1]), "=f"(x[4 * q + 2]), "=f"(x[4 * q + 3]) : "r"(addr));
+                for (int c_pass = 0, pass = 0; c_pass < (WIDE ? nch0 : 1); c_pass += MAX_CHUNKS, ++pass) {
+                    // an input wider than a region goes through it in passes of 16 chunks: a slot is written again once the
+                    // MMAs of the pass before have completed (bar_pass, committed by the MMA warp per pass).  Every warp
+                    // takes every phase of this barrier, with or without a chunk in the pass: an mbarrier wait names a
+                    // phase by its parity only, so a waiter that skipped one would take the phase before for its own.
+                    if (WIDE && pass > 0) {
+                        mbar_wait(bar_pass, (pass_cnt + (uint32_t)pass - 1u) & 1u, 330, (t - t_beg) * 100 + pass);
+                        tc_fence_after();
                     }
-                    uint32_t v[16];
+                    const int c_end = c_pass + MAX_CHUNKS < nch0 ? c_pass + MAX_CHUNKS : nch0;
+                    for (int c = c_pass + set; c < c_end; c += EPI_SETS) {
+                        const uint32_t e = (uint32_t)(set >> 1); // ring entry of this set's input tiles (producer: tile k -> k & 1)
+                        mbar_wait(bar_afull + 8 * e, a_ph & 1u, 300, (t - t_beg) * 100 + c);
+                        ++a_ph;
+                        const uint32_t arow = a_ring + e * A_TILE_BYTES + row * 128;
+                        float x[16];
 #pragma unroll
-                    for (int q = 0; q < 16; ++q) { x[q] *= ACT_SCALE; vmax = fmaxf(vmax, fabsf(x[q])); }
-                    split16(x, v);
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_aempty + 8 * e); // this warp's half of the tile is in registers
-                    tmem_st16(lane_addr + r0 * REGION_COLS + (uint32_t)(CH * c), v);
-                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_CHUNKS + c));
+                        for (int q = 0; q < 4; ++q) {
+                            const uint32_t addr = arow + (uint32_t)(((4 * (c & 1) + q) ^ (row & 7)) << 4);
+                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[4 * q]), "=f"(x[4 * q + 1]), "=f"(x[4 * q + 2]), "=f"(x[4 * q + 3]) : "r"(addr));
+                        }
+                        uint32_t v[16];
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) { x[q] *= ACT_SCALE; vmax = fmaxf(vmax, fabsf(x[q])); }
+                        split16(x, v);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_aempty + 8 * e); // this warp's half of the tile is in registers
+                        tmem_st16(lane_addr + r0 * REGION_COLS + (uint32_t)(CH * (WIDE ? c % MAX_CHUNKS : c)), v);
+                        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_ready + 8 * (r0 * MAX_CHUNKS + (WIDE ? c % MAX_CHUNKS : c)));
+                    }
                 }
-                a_cnt += (uint32_t)(g.st[0].K / KBF);
+                if (WIDE) pass_cnt += (uint32_t)((nch0 - 1) / MAX_CHUNKS);
             }
             const int lane_set = lane | (set << 8), aux = t - t_beg;
-#define NNP_FUSED_STAGE(J)                                                                                                    \
-    if (J < chain_len(CHAIN)) {                                                                                               \
-        constexpr int epi = chain_epi(CHAIN, J);                                                                              \
-        const uint32_t rd = (rc + (uint32_t)J + 1u) & 1u;                                                                     \
+#define NNP_FUSED_PASS(J, COL, NCOLS)                                                                                         \
+    {                                                                                                                         \
         const uint32_t accf = (bar_accf + 8 * rd) | (((rd ? use1 : use0) & 1u) << 31);                                        \
         if (rd) ++use1; else ++use0;                                                                                          \
-        const float2 r = epi_stage<epi>(&g, J, mrow0, lane_set, lane_addr + rd * REGION_COLS, stg, accf,                      \
-                                        bar_ready + 8 * (rd * MAX_CHUNKS), sb_base, alpha, aux);                              \
+        const float2 r = epi_stage<chain_epi(CHAIN, J)>(&g, J, mrow0, lane_set, lane_addr + rd * REGION_COLS, stg, accf,      \
+                                                        bar_ready + 8 * (rd * MAX_CHUNKS), sb_base, alpha, aux, NCOLS, COL);  \
         vmax = fmaxf(vmax, r.x);                                                                                              \
-        if (epi == FE_OUT && rowok) atomicAdd(g.e_atom + m, r.y * (1.0f / ACT_SCALE));                                        \
+        if (chain_epi(CHAIN, J) == FE_OUT && rowok) atomicAdd(g.e_atom + m, r.y * (1.0f / ACT_SCALE));                        \
+        if (J + 1 == chain_len(CHAIN)) { /* this accumulator has left tensor memory (for this warp): the next pass / tile    \
+                                            may overwrite it */                                                              \
+            tc_fence_before();                                                                                                \
+            __syncwarp();                                                                                                     \
+            if (lane == 0) mbar_arrive(bar_drained);                                                                          \
+        }                                                                                                                     \
+    }
+#define NNP_FUSED_STAGE(J)                                                                                                    \
+    if (J < chain_len(CHAIN)) {                                                                                               \
+        const uint32_t rd = (rc + (uint32_t)J + 1u) & 1u;                                                                     \
+        if (WIDE && J + 1 == chain_len(CHAIN)) { /* the last GEMM of a wide chain: passes of N of its n_total columns */      \
+            const int n_pass_cols = g.st[J].N, n_total = g.st[J].n_total;                                                     \
+            for (int col = 0; col < n_total; col += n_pass_cols)                                                              \
+                NNP_FUSED_PASS(J, col, n_total - col < n_pass_cols ? n_total - col : n_pass_cols)                             \
+        } else {                                                                                                              \
+            NNP_FUSED_PASS(J, 0, g.st[J].N)                                                                                   \
+        }                                                                                                                     \
     }
             NNP_FUSED_STAGE(0) NNP_FUSED_STAGE(1) NNP_FUSED_STAGE(2) NNP_FUSED_STAGE(3) NNP_FUSED_STAGE(4) NNP_FUSED_STAGE(5)
 #undef NNP_FUSED_STAGE
-            // the tile's last accumulator has left tensor memory (for this warp): the next tile may overwrite it
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_drained);
+#undef NNP_FUSED_PASS
             rc += (uint32_t)g.n_stages + 1u;
         }
         if (vmax > RANGE_LIMIT) atomicOr(&flags[0], NNP_FLAG_RANGE);
@@ -691,8 +744,11 @@ int nnp_fused_setup(nnp_ctx *c)
     for (int s = 0; s < S; ++s)
         for (int l = 1; l <= 3; ++l)
             if (c->widths[s][l] > REGION_COLS || c->widths[s][l] < EPI_SETS * CH) return NNP_OK;
-    const int kind = kpad <= REGION_COLS ? 1 : 2;
-    const size_t k0max = c->kpad_full < REGION_COLS ? c->kpad_full : REGION_COLS; // layer-1 tiles exist for the full chain only
+    // every system runs the full chain; NNP_FUSED_MIDDLE=1 keeps layer 1 / dE/dG of systems with more than 256 active columns
+    // as 3xTF32 launches around the four middle GEMMs (the form before the chain learnt to stream a wide layer)
+    const char *mid = getenv("NNP_FUSED_MIDDLE");
+    const int kind = (kpad > REGION_COLS && mid && mid[0] == '1') ? 2 : 1;
+    const size_t k0max = c->kpad_full;
     // ---- packed weights: per (net, species) the six matrices in chain order; sized for the largest layout once
     if (!f->d_wblob) {
         size_t tot = 0;
@@ -748,7 +804,12 @@ int nnp_fused_setup(nnp_ctx *c)
                 }
                 if (repack_l1 && kind == 1) {
                     pack(l1.Wt, h1, kpad, kpad, wsh[q][0], f->d_wblob + f->w_off[q][0]);
-                    pack(l1.W, kpad, h1, h1, wsh[q][0], f->d_wblob + f->w_off[q][5]);
+                    size_t ob = f->w_off[q][5]; // dE/dG: passes of <= 256 output columns, packed one after the other
+                    for (int col = 0; col < kpad; col += REGION_COLS) {
+                        const int nq = kpad - col < REGION_COLS ? kpad - col : REGION_COLS;
+                        pack(l1.W + (size_t)col * h1, nq, h1, h1, wsh[q][0], f->d_wblob + ob);
+                        ob += packed_bytes(nq, h1);
+                    }
                 }
             }
     }
@@ -786,10 +847,11 @@ int nnp_fused_setup(nnp_ctx *c)
                 st.K = K; st.N = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.bias = bias; st.stash = stash; st.ld_stash = ld;
                 st.c_acc = ldexpf(1.0f, -sh);
                 st.brow = brow;
+                st.n_total = N;
             };
             auto bwd = [&](int j, int K, int N, int epi, size_t w_off, float *stash, int ld, int sh) {
                 FusedStage &st = g.st[j];
-                st.K = K; st.N = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.stash = stash; st.ld_stash = ld;
+                st.K = K; st.N = N < REGION_COLS ? N : REGION_COLS; st.n_total = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.stash = stash; st.ld_stash = ld;
                 const float s2 = ldexpf(1.0f, -sh);
                 if (epi == FE_BWD) { st.gs = s2 / (alpha * ACT_SCALE); st.gc = s2; }                       // stash = 16 h, out = 16 delta
                 else if (epi == FE_BWD_ST) { st.gs = s2 / ACT_SCALE / alpha; st.gc = s2 / ACT_SCALE; }     // out rows = true h, out = true delta
@@ -819,7 +881,8 @@ int nnp_fused_setup(nnp_ctx *c)
             }
             long long cst = 0;
             for (int j = 0; j < g.n_stages; ++j)
-                cst += (long long)(g.st[j].K / CH) * 3 * (g.st[j].N / 2) + 1200; // MMA cycles + the hand-over bubble of a GEMM
+                cst += (long long)(g.st[j].K / CH) * 3 * (g.st[j].n_total / 2) + 1200LL * ((g.st[j].n_total + REGION_COLS - 1) / REGION_COLS) +
+                       (j + 1 == g.n_stages ? 25LL * g.st[j].n_total : 0); // MMA cycles + hand-over bubbles + a wide last GEMM's serial epilogues
             tiles += g.n_tiles;
             groups.push_back(g);
             cost.push_back(cst);
@@ -868,18 +931,16 @@ int nnp_fused_kind(const nnp_ctx *c) { return c->fused ? c->fused->kind : 0; }
 void nnp_launch_mlp_fused(nnp_ctx *c)
 {
     nnp_fused *f = c->fused;
+    typedef void (*Kern)(const FusedGroup *, int, const int *, float, int *);
+    static const Kern kerns[5] = {k_mlp_fused<CHAIN_FULL, false>, k_mlp_fused<CHAIN_FULL_RED, false>, k_mlp_fused<CHAIN_MIDDLE, false>,
+                                  k_mlp_fused<CHAIN_FULL, true>, k_mlp_fused<CHAIN_FULL_RED, true>};
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(k_mlp_fused<CHAIN_FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        cudaFuncSetAttribute(k_mlp_fused<CHAIN_FULL_RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        cudaFuncSetAttribute(k_mlp_fused<CHAIN_MIDDLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        for (int k = 0; k < 5; ++k) cudaFuncSetAttribute(kerns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         attr_set = true;
     }
-    if (f->kind == 2)
-        k_mlp_fused<CHAIN_MIDDLE><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
-    else if (c->n_nets > 1)
-        k_mlp_fused<CHAIN_FULL_RED><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
-    else
-        k_mlp_fused<CHAIN_FULL><<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
+    const int wide = f->kind == 1 && c->aev.kpad > REGION_COLS;
+    const Kern kern = f->kind == 2 ? kerns[2] : kerns[(c->n_nets > 1 ? 1 : 0) + (wide ? 3 : 0)];
+    kern<<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
     c->launches += 1;
 }
