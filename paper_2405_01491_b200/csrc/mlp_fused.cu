@@ -460,7 +460,8 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                         const uint64_t d1hi = make_kmajor_sw128_desc(b1), d1lo = make_kmajor_sw128_desc(b1 + rows1 * 128u);
                         const int nh = nch_tot - 4 * kb < 4 ? nch_tot - 4 * kb : 4;
                         // one wait and one election per chunk (measured against the chunks of a K block in one batch, or the
-                        // first alone and the other three together: 0.203 against 0.214 ms for the chain)
+                        // first alone and the other three together: 0.203 against 0.214 ms for the narrow chain; batching only
+                        // the first / last GEMM of a wide chain: config 5 7.35 -> 7.83 ms)
                         for (int h = 0; h < nh; ++h) {
                             const int c = 4 * kb + h, slot = WIDE ? c % MAX_CHUNKS : c; // an operand wider than a region reuses its slots
                             if (!WIDE || col == 0) { // (further passes multiply the operand that is already there)
