@@ -564,7 +564,7 @@ def _roofline_for(stage, ms, n, sp, mm_mode, pk, clocks, kpad):
         return tot
 
     if stage == "mlp_fused_chain":
-        ops = (["mlp_fwd_l1", "mlp_bwd_l1_dEdG"] if kpad <= 256 else []) + ["mlp_fwd_l2", "mlp_fwd_l3_out", "mlp_bwd_l3", "mlp_bwd_l2"]
+        ops = ["mlp_fwd_l1", "mlp_fwd_l2", "mlp_fwd_l3_out", "mlp_bwd_l3", "mlp_bwd_l2", "mlp_bwd_l1_dEdG"]
         flops = 2.0 * sum(macs(op) for op in ops)
         ach = flops / (ms * 1e-3) / 1e12 if ms else 0.0
         peak = pk["bf16_sus"]

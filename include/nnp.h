@@ -56,10 +56,11 @@ typedef enum {
 /* How the MLP contractions are computed (Fig. 3: matmul precision decides energy conservation):
  * 0 fp32 FMA on the CUDA cores; 1 (default of the tests and the bench) 3xTF32 on tcgen05, fp32-grade; 2 plain TF32 on
  * tcgen05 (fails the parity bars, kept for the precision study); 3 fp32 operands with every product and sum in fp64
- * (DFMA on the CUDA cores) -- the fp64 leg of the precision study, slow; 4 "3xF16": the hidden layers (and, when the
- * system's active AEV columns are <= 256, all six GEMMs) as ONE fused tcgen05 kernel with every fp32 operand split into
- * fp16 hi + fp16 lo (11 + 11 significant bits as in mode 1, power-of-two scaling against fp16's exponent range, fp32
- * accumulation), fp32-grade; GEMMs outside the fused chain run as in mode 1.  Out-of-range activations -> NNP_ERANGE. */
+ * (DFMA on the CUDA cores) -- the fp64 leg of the precision study, slow; 4 "3xF16": all six GEMMs of every network and
+ * species as ONE fused tcgen05 kernel with every fp32 operand split into fp16 hi + fp16 lo (11 + 11 significant bits as in
+ * mode 1, power-of-two scaling against fp16's exponent range, fp32 accumulation), fp32-grade; models the chain does not take
+ * (a hidden width outside [64, 256], more than 64 (network, species) pairs) run as in mode 1.  Out-of-range activations ->
+ * NNP_ERANGE. */
 enum { NNP_MM_FP32_SIMT = 0, NNP_MM_3XTF32_TC = 1, NNP_MM_TF32_TC = 2, NNP_MM_FP64_SIMT = 3, NNP_MM_3XF16_TC = 4 };
 
 typedef struct {
@@ -209,7 +210,7 @@ int nnp_md_step_host(nnp_ctx *ctx, float *h_xyz, float *h_vel, int n_steps, doub
  * 0 kick+drift, 1 neighbour build (all its kernels; near zero on steps without a rebuild), 2 AEV forward,
  * 3..5 MLP forward layers 1..3 (layer 3 includes the output layer), 6..8 MLP reverse layers 3..1 (8 = dE/dG),
  * 9 energy sum, 10 AEV reverse + force scatter, 11 kick + kinetic energy, 12 the fused MLP chain of mm_mode 4 (all six
- * GEMMs, or the four middle ones when the active AEV columns exceed 256: layers 1 and dE/dG are then stages 3 and 8).
+ * GEMMs in one launch; stages 3..8 stay zero then).
  * Arrays of NNP_N_STAGES entries. */
 #define NNP_N_STAGES 13
 int nnp_profile(nnp_ctx *ctx, int stride);

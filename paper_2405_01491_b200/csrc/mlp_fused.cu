@@ -24,10 +24,10 @@
 // weight ring, so the forward epilogues also write them to the activation buffers and the reverse epilogues of the same
 // CTA read them back a few microseconds later (L2 hits; 1.8 KB per atom and direction).
 //
-// Chains (chosen per loaded system, nnp_fused_setup):
-//   full   (active AEV columns kpad <= 256, e.g. water: 128):  F1 F2 F3 B3 B2 B1, input G (TMA), output dE/dG
-//   middle (any kpad, e.g. 1024 for seven species):            F2 F3 B3 B2, input h1 (TMA), output delta1 in place;
-//          F1 and B1 (K or N = kpad) run as 3xTF32 launches of the unfused kernel before / after.
+// One chain for every system: F1 F2 F3 B3 B2 B1, input G (TMA), output dE/dG.  With more than 256 active AEV columns (e.g.
+// 1024 for seven species) the first and the last GEMM are wider than a TMEM region: F1 takes its operand through the region in
+// passes of 16 chunks (a slot is rewritten once the MMAs of the pass before have completed), B1 writes its output in passes of
+// 256 columns into the same region, from the operand that stays in the other one (kernels with WIDE = true).
 // Warp roles: 0 producer (TMA tiles of the chain's input + bulk weight copies), 1 MMA issue, 2-17 epilogue (four warps per
 // TMEM lane quarter, every fourth 16-column chunk each); the epilogue warps also convert the chain's input (fp32 tile in
 // shared memory -> fp16 hi / lo chunks in TMEM) at the start of a tile.  576 threads: 112 registers each, no spills - with
@@ -81,9 +81,8 @@ enum FusedEpi {
     FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> operand
     FE_OUT = 1,     // h3 = celu(acc + bias); e_atom += h3 . w4; delta3 = w4 celu'(h3): hi/lo -> operand
     FE_BWD = 2,     // delta = acc * celu'(stash): hi/lo -> operand
-    FE_BWD_ST = 3,  // delta = acc * celu'(out): stored over out (last GEMM of the middle chain)
-    FE_ST = 4,      // out = acc
-    FE_RED = 5      // out += acc (vector reductions in memory: ensembles add into the same rows)
+    FE_ST = 3,      // out = acc
+    FE_RED = 4      // out += acc (vector reductions in memory: ensembles add into the same rows)
 };
 
 struct FusedStage {
@@ -172,9 +171,9 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
 {
     float vmax = 0.f, esum = 0.f;
     constexpr bool fwd = EPI == FE_FWD || EPI == FE_OUT;
-    constexpr bool rd_prev = EPI == FE_BWD || EPI == FE_BWD_ST;   // reads rows of h for CELU'
+    constexpr bool rd_prev = EPI == FE_BWD;                        // reads rows of h for CELU'
     constexpr bool to_op = EPI == FE_FWD || EPI == FE_OUT || EPI == FE_BWD;
-    constexpr bool wr_rows = EPI == FE_FWD || EPI == FE_BWD_ST || EPI == FE_ST || EPI == FE_RED;
+    constexpr bool wr_rows = EPI == FE_FWD || EPI == FE_ST || EPI == FE_RED;
     const FusedGroup &g = *gp;
     const FusedStage &st = g.st[j];
     const int lane = lane_set & 31;
@@ -182,8 +181,8 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
     const uint32_t my_row = stg + (uint32_t)lane * (EPI_STG_LD * 4);
     const int sub_r = (lane >> 3) + 4 * ((lane >> 2) & 1), sub_c = (lane & 3) * 4;
     // rows read (h for CELU') and rows written (h stash, or the chain's output)
-    const float *rd_base = EPI == FE_BWD ? st.stash : g.out + col_off;
-    const int rd_ld = EPI == FE_BWD ? st.ld_stash : g.ldo;
+    const float *rd_base = st.stash;
+    const int rd_ld = st.ld_stash;
     float *wr_base = EPI == FE_FWD ? st.stash : g.out + col_off;
     const int wr_ld = EPI == FE_FWD ? st.ld_stash : g.ldo;
     const float c_acc = st.c_acc, gs = st.gs, gc = st.gc;
@@ -293,14 +292,12 @@ __device__ __forceinline__ int part_rows(int N, int p) { return p == 0 ? (N > 12
 // generation q the region q & 1, so the input of tile t+1 goes where the last GEMM of tile t took its operand from while
 // the last accumulator of tile t is still being drained from the other one.
 
-// Chains (template parameter of the kernel): 0 full, one network (F1 F2 F3 B3 B2 B1 -> dE/dG stored); 1 full, ensemble
-// (dE/dG accumulated with reductions); 2 middle (F2 F3 B3 B2 -> delta1 in place).
-enum { CHAIN_FULL = 0, CHAIN_FULL_RED = 1, CHAIN_MIDDLE = 2 };
-__host__ __device__ constexpr int chain_len(int chain) { return chain == CHAIN_MIDDLE ? 4 : 6; }
+// Chains (template parameter of the kernel): 0 one network (dE/dG stored), 1 ensemble (dE/dG accumulated with reductions).
+enum { CHAIN_FULL = 0, CHAIN_FULL_RED = 1 };
+__host__ __device__ constexpr int chain_len(int) { return 6; }
 __host__ __device__ constexpr int chain_epi(int chain, int j)
 {
-    return chain == CHAIN_MIDDLE ? (j == 0 ? FE_FWD : j == 1 ? FE_OUT : j == 2 ? FE_BWD : FE_BWD_ST)
-                                 : (j < 2 ? FE_FWD : j == 2 ? FE_OUT : j < 5 ? FE_BWD : chain == CHAIN_FULL_RED ? FE_RED : FE_ST);
+    return j < 2 ? FE_FWD : j == 2 ? FE_OUT : j < 5 ? FE_BWD : chain == CHAIN_FULL_RED ? FE_RED : FE_ST;
 }
 
 // WIDE: the chain's input / output has more than 256 columns (first GEMM: operand passes, last GEMM: output passes); the
@@ -689,7 +686,7 @@ int weight_shift(float wmax)
 } // namespace
 
 struct nnp_fused {
-    int kind;                    // 0: not usable for the loaded system, 1: full chain, 2: middle chain
+    int kind;                    // 0: not usable for the loaded system (the six-launch path runs), 1: the fused chain
     int n_groups, n_tiles, grid;
     FusedGroup *d_groups;        // [n_nets * S]
     int *d_cta_tiles;            // [grid + 1]
@@ -745,10 +742,6 @@ int nnp_fused_setup(nnp_ctx *c)
     for (int s = 0; s < S; ++s)
         for (int l = 1; l <= 3; ++l)
             if (c->widths[s][l] > REGION_COLS || c->widths[s][l] < EPI_SETS * CH) return NNP_OK;
-    // every system runs the full chain; NNP_FUSED_MIDDLE=1 keeps layer 1 / dE/dG of systems with more than 256 active columns
-    // as 3xTF32 launches around the four middle GEMMs (the form before the chain learnt to stream a wide layer)
-    const char *mid = getenv("NNP_FUSED_MIDDLE");
-    const int kind = (kpad > REGION_COLS && mid && mid[0] == '1') ? 2 : 1;
     const size_t k0max = c->kpad_full;
     // ---- packed weights: per (net, species) the six matrices in chain order; sized for the largest layout once
     if (!f->d_wblob) {
@@ -803,7 +796,7 @@ int nnp_fused_setup(nnp_ctx *c)
                         c->launches += 1;
                     }
                 }
-                if (repack_l1 && kind == 1) {
+                if (repack_l1) {
                     pack(l1.Wt, h1, kpad, kpad, wsh[q][0], f->d_wblob + f->w_off[q][0]);
                     size_t ob = f->w_off[q][5]; // dE/dG: passes of <= 256 output columns, packed one after the other
                     for (int col = 0; col < kpad; col += REGION_COLS) {
@@ -814,8 +807,7 @@ int nnp_fused_setup(nnp_ctx *c)
                 }
             }
     }
-    if (kind == 1) f->packed_mask = c->present_mask;
-    else if (first_pack) f->packed_mask = 0x80000000u; // middle GEMMs packed, no layer-1 tiles
+    f->packed_mask = c->present_mask;
 
     // ---- groups (one per network and species present) and tiles
     std::vector<FusedGroup> groups;
@@ -855,31 +847,19 @@ int nnp_fused_setup(nnp_ctx *c)
                 st.K = K; st.N = N < REGION_COLS ? N : REGION_COLS; st.n_total = N; st.epi = epi; st.w_off = (uint32_t)w_off; st.stash = stash; st.ld_stash = ld;
                 const float s2 = ldexpf(1.0f, -sh);
                 if (epi == FE_BWD) { st.gs = s2 / (alpha * ACT_SCALE); st.gc = s2; }                       // stash = 16 h, out = 16 delta
-                else if (epi == FE_BWD_ST) { st.gs = s2 / ACT_SCALE / alpha; st.gc = s2 / ACT_SCALE; }     // out rows = true h, out = true delta
                 st.c_acc = s2 / ACT_SCALE;                                                                  // FE_ST / FE_RED
             };
             if (f->w_off[q][6] > 0xffffffffull) { c->err = "fused MLP: weight blob exceeds 4 GiB"; return NNP_EINVAL; }
-            if (kind == 1) {
-                g.n_stages = 6;
-                if (!make_map_a(&g.mapA, c->G + (size_t)off * kpad, M, kpad, kpad)) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
-                fwd(0, kpad, h1, FE_FWD, f->w_off[q][0], b16, H0, c->hmax[0], wsh[q][0], 0);
-                fwd(1, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1], 1);
-                fwd(2, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2], 2);
-                bwd(3, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
-                bwd(4, h2, h1, FE_BWD, f->w_off[q][4], H0, c->hmax[0], wsh[q][1]);
-                bwd(5, h1, kpad, nn > 1 ? FE_RED : FE_ST, f->w_off[q][5], nullptr, 0, wsh[q][0]);
-                g.out = c->dG + (size_t)off * kpad;
-                g.ldo = kpad;
-            } else {
-                g.n_stages = 4;
-                if (!make_map_a(&g.mapA, H0, M, h1, c->hmax[0])) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
-                fwd(0, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1], 1);
-                fwd(1, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2], 2);
-                bwd(2, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
-                bwd(3, h2, h1, FE_BWD_ST, f->w_off[q][4], nullptr, 0, wsh[q][1]);
-                g.out = H0;
-                g.ldo = c->hmax[0];
-            }
+            g.n_stages = 6;
+            if (!make_map_a(&g.mapA, c->G + (size_t)off * kpad, M, kpad, kpad)) { c->err = "cuTensorMapEncodeTiled failed"; return NNP_ECUDA; }
+            fwd(0, kpad, h1, FE_FWD, f->w_off[q][0], b16, H0, c->hmax[0], wsh[q][0], 0);
+            fwd(1, h1, h2, FE_FWD, f->w_off[q][1], b16 + REGION_COLS, H1, c->hmax[1], wsh[q][1], 1);
+            fwd(2, h2, h3, FE_OUT, f->w_off[q][2], b16 + 2 * REGION_COLS, nullptr, 0, wsh[q][2], 2);
+            bwd(3, h3, h2, FE_BWD, f->w_off[q][3], H1, c->hmax[1], wsh[q][2]);
+            bwd(4, h2, h1, FE_BWD, f->w_off[q][4], H0, c->hmax[0], wsh[q][1]);
+            bwd(5, h1, kpad, nn > 1 ? FE_RED : FE_ST, f->w_off[q][5], nullptr, 0, wsh[q][0]);
+            g.out = c->dG + (size_t)off * kpad;
+            g.ldo = kpad;
             long long cst = 0;
             for (int j = 0; j < g.n_stages; ++j)
                 cst += (long long)(g.st[j].K / CH) * 3 * (g.st[j].n_total / 2) + 1200LL * ((g.st[j].n_total + REGION_COLS - 1) / REGION_COLS) +
@@ -922,26 +902,25 @@ int nnp_fused_setup(nnp_ctx *c)
         c->err = std::string("fused MLP: table upload failed: ") + cudaGetErrorString(cudaGetLastError());
         return NNP_ECUDA;
     }
-    f->kind = kind;
+    f->kind = 1;
     return NNP_OK;
 }
 
 int nnp_fused_kind(const nnp_ctx *c) { return c->fused ? c->fused->kind : 0; }
 
-// Enqueues the fused chain.  kind 1: replaces all six GEMM launches; kind 2: replaces the four middle ones.
+// Enqueues the fused chain (all six GEMMs of every network and species in one launch).
 void nnp_launch_mlp_fused(nnp_ctx *c)
 {
     nnp_fused *f = c->fused;
     typedef void (*Kern)(const FusedGroup *, int, const int *, float, int *);
-    static const Kern kerns[5] = {k_mlp_fused<CHAIN_FULL, false>, k_mlp_fused<CHAIN_FULL_RED, false>, k_mlp_fused<CHAIN_MIDDLE, false>,
-                                  k_mlp_fused<CHAIN_FULL, true>, k_mlp_fused<CHAIN_FULL_RED, true>};
+    static const Kern kerns[4] = {k_mlp_fused<CHAIN_FULL, false>, k_mlp_fused<CHAIN_FULL_RED, false>, k_mlp_fused<CHAIN_FULL, true>,
+                                  k_mlp_fused<CHAIN_FULL_RED, true>};
     static bool attr_set = false;
     if (!attr_set) {
-        for (int k = 0; k < 5; ++k) cudaFuncSetAttribute(kerns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        for (int k = 0; k < 4; ++k) cudaFuncSetAttribute(kerns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         attr_set = true;
     }
-    const int wide = f->kind == 1 && c->aev.kpad > REGION_COLS;
-    const Kern kern = f->kind == 2 ? kerns[2] : kerns[(c->n_nets > 1 ? 1 : 0) + (wide ? 3 : 0)];
+    const Kern kern = kerns[(c->n_nets > 1 ? 1 : 0) + (c->aev.kpad > REGION_COLS ? 2 : 0)];
     kern<<<f->grid, THREADS, SMEM_BYTES, c->stream>>>(f->d_groups, f->n_groups, f->d_cta_tiles, c->alpha, c->flags);
     c->launches += 1;
 }

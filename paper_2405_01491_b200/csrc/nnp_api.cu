@@ -436,24 +436,20 @@ int run_forces(nnp_ctx *c)
     int nb = (!c->tc_mode || c->n_nets == 1) ? 1 : NNP_MAX_GROUPS / np;
     if (nb < 1) nb = 1;
     if (nb > c->n_nets) nb = c->n_nets;
-    // fused chain (mlp_fused.cu): 1 = all six GEMMs in one launch, 2 = the four middle ones (layer 1 / dE/dG stay launches)
-    const int fk = nnp_fused_kind(c);
-    if (fk == 1) {
+    // mm_mode 4: all six GEMMs of every network and species in one launch (mlp_fused.cu); nnp_fused_kind is 0 where the chain
+    // does not apply (hidden widths outside [64, 256], more than 64 (network, species) groups): six 3xTF32 launches then
+    if (nnp_fused_kind(c) == 1) {
         if (c->n_nets > 1) CU(c, cudaMemsetAsync(c->dG, 0, sizeof(float) * (size_t)c->n * c->aev.kpad, c->stream));
         nnp_launch_mlp_fused(c);
         nnp_prof_mark(c, 12);
     } else {
         for (int net0 = 0; net0 < c->n_nets; net0 += nb)
-            for (int op = 0; op < (fk == 2 ? 1 : 5); ++op) {
+            for (int op = 0; op < 5; ++op) {
                 make_batch(c, net0, nb < c->n_nets - net0 ? nb : c->n_nets - net0, op, b);
                 int rc = run_gemm(c, b, epi_of[op]);
                 if (rc != NNP_OK) return rc;
                 nnp_prof_mark(c, 3 + op);
             }
-        if (fk == 2) {
-            nnp_launch_mlp_fused(c);
-            nnp_prof_mark(c, 12);
-        }
         if (nb > 1) {
             // dE/dG sums over the networks: the groups of all batched networks add into the same rows with vector
             // reductions in memory (the summation order over the networks is then not fixed, like the force scatter's)

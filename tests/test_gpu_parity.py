@@ -177,8 +177,8 @@ def test_ensemble_in_both_fp32_grade_modes(mm_mode):
 @pytest.mark.parametrize("mm_mode", [nnp.NNP_MM_3XTF32_TC, nnp.NNP_MM_3XF16_TC], ids=["3xtf32_six_launches", "3xf16_fused"])
 def test_both_tensor_core_modes_on_every_chain(mm_mode):
     """The suite runs in ONE matmul mode (NNP_MM_MODE, default 4); this test takes the other fp32-grade tensor-core mode
-    through the same shapes: water (full fused chain / six launches, row tiles with a ragged tail), all seven species (middle
-    chain + layer-1 launches, buckets from 2 to ~1000 rows) and a molecule batch with two networks."""
+    through the same shapes: water (128 active AEV columns, row tiles with a ragged tail), all seven species (1024 columns: the
+    fused chain streams its first and last GEMM in passes; buckets from 2 to ~1000 rows) and a molecule batch with two networks."""
     consts, widths, params, om = U.make_model(1)
     sp, xyz, box = inputs.water_box(1000, seed=3)
     ctx = U.gpu_create(consts, widths, params, 1, 3600, mm_mode=mm_mode)
