@@ -695,6 +695,7 @@ struct nnp_fused {
     size_t wblob_bytes;
     size_t w_off[64][MAX_STAGES + 1]; // per (network, species): byte offsets of F1 F2 F3 B3 B2 B1 in the blob
     unsigned packed_mask;        // species mask the layer-1 tiles were packed for (0: nothing packed yet)
+    int last_off[NNP_MAX_SPECIES + 1], last_kpad; // bucket offsets / G pitch the tables were built for (last_kpad = 0: none)
     int num_sms;
 };
 
@@ -736,8 +737,14 @@ int nnp_fused_setup(nnp_ctx *c)
         if (c->fused->num_sms <= 0) c->fused->num_sms = 148;
     }
     nnp_fused *f = c->fused;
-    f->kind = 0;
     const int kpad = c->aev.kpad;
+    // same species counts and layout as the last system (e.g. one structure evaluated again and again through
+    // nnp_energy_forces_host): the packed weights, the group table and the tile ranges stand as they are
+    if (f->kind == 1 && f->last_kpad == kpad && f->packed_mask == c->present_mask &&
+        memcmp(f->last_off, c->bucket_off, sizeof(f->last_off)) == 0)
+        return NNP_OK;
+    f->kind = 0;
+    f->last_kpad = 0;
     // widths a 256-column region holds; every accumulator must give all four epilogue sets a chunk
     for (int s = 0; s < S; ++s)
         for (int l = 1; l <= 3; ++l)
@@ -903,6 +910,8 @@ int nnp_fused_setup(nnp_ctx *c)
         return NNP_ECUDA;
     }
     f->kind = 1;
+    f->last_kpad = kpad;
+    memcpy(f->last_off, c->bucket_off, sizeof(f->last_off));
     return NNP_OK;
 }
 
