@@ -248,3 +248,17 @@ def test_bad_mol_offsets_are_rejected(model1):
         U.gpu_energy_forces(ctx, sp, xyz, None, mol_offsets=[0, 2, 2, 6])      # an empty structure is fine
     finally:
         nnp.nnp_destroy(ctx)
+
+
+def test_repeatability_stress():
+    """The same structures evaluated again and again (water, 4 and 7 species, a molecule batch with an ensemble; default and
+    side stream): any repeat that deviates beyond the noise of the fp32 force scatter fails.  This is the test that found the
+    input-ring phase bug of the fused chain (rare wrong energies on seven-species systems)."""
+    import sys
+    from paper_2405_01491_b200 import repeatability
+    argv = sys.argv
+    sys.argv = ["repeatability", "--repeats", "20"]
+    try:
+        assert repeatability.main() == 0
+    finally:
+        sys.argv = argv
