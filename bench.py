@@ -479,9 +479,10 @@ def run_ours(args):
                    "aev_active_columns": kact,
                    "launch_path": "kernel_by_kernel" if os.environ.get("NNP_NO_GRAPH") == "1" else
                                   "cuda_graph (one graph launch per step, rebuild inside a conditional node)",
-                   "l2_policy": "inputs larger than L2: per step the kernels stream G (%d MB), the activations (%d MB) and "
-                                "the neighbour rows (%d MB); no flush needed" % (n * kpad * 4 // 2**20, n * 608 * 4 // 2**20,
-                                                                                   n * 224 * 4 // 2**20),
+                   "l2_policy": "inputs larger than L2: per step the kernels stream G (%d MB), the activations (%d MB%s) and "
+                                "the neighbour rows (%d MB); no flush needed"
+                                % (n * kpad * 4 // 2**20, n * (448 if args.mm_mode == 4 else 608) * 4 // 2**20,
+                                   ": only h1 and h2 leave the SM in mm_mode 4" if args.mm_mode == 4 else "", n * 224 * 4 // 2**20),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": world * n * Ke / (e2e_ms_max * 1e-3), "unit": UNIT, "steps": Ke,
