@@ -127,7 +127,8 @@ int nnp_set_system(nnp_ctx *ctx, int n_atoms, const int32_t *d_species, const fl
  *     of itself) is evaluated, exactly, as the smallest m0 x m1 x m2 supercell that reaches that width: the library holds
  *     n_atoms * m0 m1 m2 internal atoms (this product must be <= max_atoms, else NNP_EBOX), returns energy / virial per
  *     cell and the forces, AEVs, neighbour rows (an image of atom j is reported as j) of the caller's atoms.  One
- *     structure only; energy / forces / virial only (nnp_md_init returns NNP_EINVAL: pass the supercell yourself).
+ *     structure only.  In MD the copies are reset to their atom's state (+ the copy's lattice shift) after every drift
+ *     and before every kick, so the supercell stays exactly periodic in the caller's cell.
  * nnp_build_neighbors returns NNP_EBOX if a width of the (super)cell is below 2 (rcr + skin). */
 int nnp_set_system_cell(nnp_ctx *ctx, int n_atoms, const int32_t *d_species, const float *d_xyz, const float h_cell[9],
                         int n_mols, const int32_t *d_mol_offsets);

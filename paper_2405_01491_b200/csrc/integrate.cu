@@ -51,7 +51,7 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 __global__ void k_kick_drift_langevin(int n, float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ frc,
                                       const float4 *__restrict__ xref, const int *__restrict__ spc, const int *__restrict__ orig,
                                       const float *__restrict__ inv_mass_conv, const float *__restrict__ c2_s, float c1, float dt,
-                                      float half_skin2, uint32_t seed_lo, uint32_t seed_hi, int *__restrict__ flags)
+                                      float half_skin2, uint32_t seed_lo, uint32_t seed_hi, int *__restrict__ flags, int n_user)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
@@ -63,7 +63,7 @@ __global__ void k_kick_drift_langevin(int n, float4 *__restrict__ pos, float4 *_
         v.x = fmaf(k, f.x, v.x); v.y = fmaf(k, f.y, v.y); v.z = fmaf(k, f.z, v.z);
         x.x = fmaf(hdt, v.x, x.x); x.y = fmaf(hdt, v.y, x.y); x.z = fmaf(hdt, v.z, x.z);
         uint32_t rn[4];
-        philox4x32_10((uint32_t)orig[i], (uint32_t)flags[4], 0u, 0u, seed_lo, seed_hi, rn);
+        philox4x32_10((uint32_t)(orig[i] % n_user), (uint32_t)flags[4], 0u, 0u, seed_lo, seed_hi, rn); // (copies of a small cell: the atom's noise)
         float u[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) u[q] = ((float)(rn[q] >> 9) + 0.5f) * 1.1920928955078125e-07f; // 2^-23
@@ -96,7 +96,7 @@ __device__ __forceinline__ void add_per_structure(bool ok, int m, double v, doub
 // v += dt/2 a(F); kinetic energy sum_i m v^2 / (2 accel_conv) accumulated in fp64.
 __global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restrict__ frc, const int *__restrict__ spc,
                           const float *__restrict__ inv_mass_conv, const float *__restrict__ mass, float dt,
-                          float inv_accel_conv, const int *__restrict__ mol, int single, double *__restrict__ ekin,
+                          float inv_accel_conv, float inv_rep, const int *__restrict__ mol, int single, double *__restrict__ ekin,
                           int *__restrict__ step_ctr)
 {
     if (step_ctr && blockIdx.x == 0 && threadIdx.x == 0) *step_ctr += 1; // Langevin step counter (read by the next drift kernel)
@@ -109,7 +109,7 @@ __global__ void k_kick_ke(int n, float4 *__restrict__ vel, const float4 *__restr
         const float4 f = frc[i];
         v.x = fmaf(k, f.x, v.x); v.y = fmaf(k, f.y, v.y); v.z = fmaf(k, f.z, v.z);
         vel[i] = v;
-        ke = 0.5f * mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z) * inv_accel_conv;
+        ke = 0.5f * mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z) * inv_accel_conv * inv_rep;
     }
     if (!single) { // one kinetic energy per structure (replica batches)
         add_per_structure(i < n, i < n ? mol[i] : -1, (double)ke, ekin);
@@ -163,11 +163,11 @@ __global__ void k_unpermute3(int n, const float4 *__restrict__ src, const int *_
     dst[3 * o] = v.x; dst[3 * o + 1] = v.y; dst[3 * o + 2] = v.z;
 }
 
-__global__ void k_permute_in3(int n, const float *__restrict__ src, const int *__restrict__ orig, float4 *__restrict__ dst)
+__global__ void k_permute_in3(int n, const float *__restrict__ src, const int *__restrict__ orig, int n_user, float4 *__restrict__ dst)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int o = orig[i];
+    const int o = orig[i] % n_user; // (the copies of a replicated small cell take their atom's value)
     dst[i] = make_float4(src[3 * o], src[3 * o + 1], src[3 * o + 2], 0.f);
 }
 
@@ -184,11 +184,11 @@ __global__ void k_unpermute3x2(int n, const float4 *__restrict__ srcA, const flo
 }
 
 __global__ void k_permute_in3x2(int n, const float *__restrict__ srcA, const float *__restrict__ srcB,
-                                const int *__restrict__ orig, float4 *__restrict__ dstA, float4 *__restrict__ dstB)
+                                const int *__restrict__ orig, int n_user, float4 *__restrict__ dstA, float4 *__restrict__ dstB)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int o = orig[i];
+    const int o = orig[i] % n_user;
     dstA[i] = make_float4(srcA[3 * o], srcA[3 * o + 1], srcA[3 * o + 2], 0.f);
     dstB[i] = make_float4(srcB[3 * o], srcB[3 * o + 1], srcB[3 * o + 2], 0.f);
 }
@@ -202,7 +202,58 @@ __global__ void k_pack_result(const double *__restrict__ e_mol, const double *__
     }
 }
 
+// Replicated small cell (nnp_set_system_cell): the copies are kept bit-identical to copy 0 - a copy's position is its atom's
+// plus the copy's lattice shift, its velocity and force are its atom's.  (Left alone the copies drift apart by the rounding
+// of x + shift + dt v and by the summation order of the force scatter, and the supercell stops being periodic in the cell.)
+__global__ void k_stage_copy0(int n, const int *__restrict__ orig, int n_user, const float4 *__restrict__ a, const float4 *__restrict__ b,
+                              float4 *__restrict__ stage)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int e = orig[i];
+    if (e >= n_user) return;
+    stage[e] = a[i];
+    if (b) stage[n_user + e] = b[i];
+}
+
+struct RepCell { float cu[9]; };
+__global__ void k_spread_copy0(int n, const int *__restrict__ orig, int n_user, int m0, int m1, RepCell rc,
+                               const float4 *__restrict__ stage, float4 *__restrict__ a, float4 *__restrict__ b, int shift_a)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int e = orig[i];
+    if (e < n_user) return;
+    const int at = e % n_user, copy = e / n_user;
+    float4 v = stage[at];
+    if (shift_a) {
+        const float k0 = (float)(copy % m0), k1 = (float)((copy / m0) % m1), k2 = (float)(copy / (m0 * m1));
+        v.x += k0 * rc.cu[0] + k1 * rc.cu[3] + k2 * rc.cu[6];
+        v.y += k0 * rc.cu[1] + k1 * rc.cu[4] + k2 * rc.cu[7];
+        v.z += k0 * rc.cu[2] + k1 * rc.cu[5] + k2 * rc.cu[8];
+    }
+    a[i] = v;
+    if (b) b[i] = stage[n_user + at];
+}
+
 } // namespace
+
+int nnp_launch_sync_copies(nnp_ctx *c, int what)
+{
+    if (c->rep <= 1) return NNP_OK;
+    const int nb = nnp_div_up(c->n, T);
+    RepCell rcell;
+    for (int q = 0; q < 9; ++q) rcell.cu[q] = c->cell_user[q];
+    if (what == 0) {
+        k_stage_copy0<<<nb, T, 0, c->stream>>>(c->n, c->orig, c->n_user, c->pos, c->vel, c->rep_stage);
+        k_spread_copy0<<<nb, T, 0, c->stream>>>(c->n, c->orig, c->n_user, c->rep_m[0], c->rep_m[1], rcell, c->rep_stage, c->pos, c->vel, 1);
+    } else {
+        k_stage_copy0<<<nb, T, 0, c->stream>>>(c->n, c->orig, c->n_user, c->frc, nullptr, c->rep_stage);
+        k_spread_copy0<<<nb, T, 0, c->stream>>>(c->n, c->orig, c->n_user, c->rep_m[0], c->rep_m[1], rcell, c->rep_stage, c->frc, nullptr, 0);
+    }
+    c->launches += 2;
+    return NNP_OK;
+}
 
 void nnp_launch_unpermute3x2(nnp_ctx *c, const float4 *srcA, float *dstA, const float4 *srcB, float *dstB)
 {
@@ -212,7 +263,7 @@ void nnp_launch_unpermute3x2(nnp_ctx *c, const float4 *srcA, float *dstA, const 
 
 void nnp_launch_permute_in3x2(nnp_ctx *c, const float *srcA, float4 *dstA, const float *srcB, float4 *dstB)
 {
-    k_permute_in3x2<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, srcA, srcB, c->orig, dstA, dstB);
+    k_permute_in3x2<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, srcA, srcB, c->orig, c->n_user, dstA, dstB);
     c->launches += 1;
 }
 
@@ -228,20 +279,23 @@ void nnp_launch_kick_drift(nnp_ctx *c)
     if (c->lgv_gamma > 0.f) {
         k_kick_drift_langevin<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(
             c->n, c->pos, c->vel, c->frc, c->xref, c->spc, c->orig, c->d_inv_mass_conv, c->d_lgv_c2, c->lgv_c1, c->dt, hs * hs,
-            (uint32_t)c->lgv_seed, (uint32_t)(c->lgv_seed >> 32), c->flags);
+            (uint32_t)c->lgv_seed, (uint32_t)(c->lgv_seed >> 32), c->flags, c->n_user);
         c->launches += 1;
+        nnp_launch_sync_copies(c, 0);
         return;
     }
     k_kick_drift<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->pos, c->vel, c->frc, c->xref, c->spc,
                                                           c->d_inv_mass_conv, c->dt, hs * hs, c->flags);
     c->launches += 1;
+    nnp_launch_sync_copies(c, 0);
 }
 
 void nnp_launch_kick_ke(nnp_ctx *c, int count_step)
 {
+    nnp_launch_sync_copies(c, 1); // (replicated small cell: every copy is kicked with its atom's force)
     cudaMemsetAsync(c->ekin, 0, sizeof(double) * c->n_mols, c->stream);
     k_kick_ke<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, c->vel, c->frc, c->spc, c->d_inv_mass_conv, c->d_mass,
-                                                       c->dt, 1.0f / c->accel_conv, c->mol, c->n_mols == 1, c->ekin,
+                                                       c->dt, 1.0f / c->accel_conv, 1.0f / (float)c->rep, c->mol, c->n_mols == 1, c->ekin,
                                                        count_step ? c->flags + 4 : nullptr);
     c->launches += 1;
 }
@@ -262,6 +316,6 @@ void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst)
 
 void nnp_launch_permute_in3(nnp_ctx *c, const float *src, float4 *dst)
 {
-    k_permute_in3<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, src, c->orig, dst);
+    k_permute_in3<<<nnp_div_up(c->n, T), T, 0, c->stream>>>(c->n, src, c->orig, c->n_user, dst);
     c->launches += 1;
 }

@@ -626,7 +626,7 @@ void nnp_destroy(nnp_ctx *c)
                     c->frc, c->xref, c->spc, c->spc_tmp, c->orig, c->orig_tmp, c->mol, c->mol_tmp, c->mol_offsets, c->key,
                     c->order, c->cell_start, c->cursor, c->nbr_r, c->nbr_a, c->seg_r, c->seg_a, c->G,
                     c->dG == c->G ? nullptr : c->dG, c->H[0], c->H[1], c->H[2], c->e_atom, c->e_mol, c->ekin, c->flags, c->aev_sched,
-                    c->io_xyz, c->io_vel, c->io_species, c->d_res};
+                    c->io_xyz, c->io_vel, c->io_species, c->d_res, c->rep_stage};
     for (void *p : ptrs) dev_free(c, p);
     if (c->h_res) cudaFreeHost(c->h_res);
     for (auto &m : c->prof_marks) cudaEventDestroy(m.first);
@@ -1059,8 +1059,16 @@ int nnp_md_init(nnp_ctx *c, const float *d_vel, float dt_fs, float skin)
     if (!c->have_system) NNP_FAIL(c, NNP_ESTALE, "nnp_set_system first");
     if (!d_vel || !(dt_fs > 0.f) || !(skin > 0.f)) NNP_FAIL(c, NNP_EINVAL, "need velocities, dt > 0, skin > 0");
     if (c->n == 0) NNP_FAIL(c, NNP_EINVAL, "empty system");
-    if (c->rep > 1) NNP_FAIL(c, NNP_EINVAL, "MD on a cell narrower than 2 (rcr + 0.5 A) is not supported: pass the supercell");
     CU(c, cudaSetDevice(c->device));
+    if (c->rep > 1 && c->rep_stage_cap < 2 * c->n_user) { // a replicated small cell: staging for the state of copy 0
+        CU(c, cudaStreamSynchronize(c->stream));
+        dev_free(c, c->rep_stage);
+        c->rep_stage = nullptr;
+        c->rep_stage_cap = 0;
+        int rc0 = dev_alloc(c, &c->rep_stage, (size_t)2 * c->n_user);
+        if (rc0) return rc0;
+        c->rep_stage_cap = 2 * c->n_user;
+    }
     nnp_launch_permute_in3(c, d_vel, c->vel);
     c->dt = dt_fs;
     c->lgv_gamma = 0.f; // velocity Verlet until nnp_md_set_langevin
@@ -1204,6 +1212,7 @@ int nnp_md_step_host(nnp_ctx *c, float *h_xyz, float *h_vel, int n_steps, double
     CU(c, cudaMemcpyAsync(c->io_xyz, h_xyz, bytes, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->io_vel, h_vel, bytes, cudaMemcpyHostToDevice, c->stream));
     nnp_launch_permute_in3x2(c, c->io_xyz, c->pos, c->io_vel, c->vel);
+    nnp_launch_sync_copies(c, 0); // (a replicated small cell: the copies get their lattice shifts back)
     int rc = nnp_md_step(c, n_steps);
     if (rc) return rc;
     nnp_launch_unpermute3x2(c, c->pos, c->io_xyz, c->vel, c->io_vel);

@@ -200,6 +200,8 @@ struct nnp_ctx {
     float4 *pos, *pos_tmp; // xyz, w unused
     float4 *vel, *vel_tmp;
     float4 *frc;           // forces (fp32 atomics)
+    float4 *rep_stage;     // [3][n_user] replicated small cells in MD: state of copy 0 in caller order (allocated at need)
+    int rep_stage_cap;
     float4 *xref;          // positions at the last list build
     int *spc, *spc_tmp;    // species
     int *orig, *orig_tmp;  // internal -> original index
@@ -250,6 +252,7 @@ void nnp_launch_mlp_fused(nnp_ctx *c);
 void nnp_fused_destroy(nnp_ctx *c);
 // integrate.cu
 void nnp_launch_kick_drift(nnp_ctx *c);
+int nnp_launch_sync_copies(nnp_ctx *c, int what); // replicated small cell: copies := copy 0 (what 0: x + shift and v, 1: F)
 void nnp_launch_kick_ke(nnp_ctx *c, int count_step); // count_step: also advance the Langevin step counter flags[4]
 void nnp_launch_energy_reduce(nnp_ctx *c);
 void nnp_launch_unpermute3(nnp_ctx *c, const float4 *src, float *dst);

@@ -843,10 +843,24 @@ def test_small_cells_see_all_periodic_images(model1, case):
         nnp.nnp_sync(ctx)
         aev_ref = orc.energy_forces_cell(om, sp, xyz, cell, want_forces=False, want_aev=True)["aev"]
         assert np.abs(d_aev.cpu().numpy() - aev_ref).max() < 2e-5 * max(1.0, np.abs(aev_ref).max())
-        # MD on a replicated cell is refused, loudly
-        with pytest.raises(nnp.NnpError) as e:
-            nnp.nnp_md_init(ctx, torch.zeros((n, 3), device="cuda"), 0.5, 0.5)
-        assert e.value.status == nnp.NNP_EINVAL
+        # MD: every internal copy follows its atom; against the oracle's integrator in the small cell (all images)
+        v = inputs.maxwell_boltzmann(sp, 300.0, seed=8).astype(np.float32).astype(np.float64)
+        dev = torch.device("cuda:0")
+        nnp.nnp_md_init(ctx, torch.as_tensor(v.astype(np.float32), device=dev), 0.5, 0.3)
+        o_x, o_v = torch.zeros((n, 3), device=dev), torch.zeros((n, 3), device=dev)
+        o_ep, o_ek = torch.zeros(1, dtype=torch.float64, device=dev), torch.zeros(1, dtype=torch.float64, device=dev)
+        nnp.nnp_md_step(ctx, 3)
+        nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, None)
+        nnp.nnp_sync(ctx)
+        o3 = orc.md_cell(om, sp, xyz, v, inputs.MASS, cell, 0.5, inputs.ACCEL_CONV, 3)
+        assert np.abs(o_x.cpu().numpy() - o3["xyz"]).max() < 1e-5 and np.abs(o_v.cpu().numpy() - o3["vel"]).max() < 1e-5
+        assert abs(float(o_ep.item()) - o3["epot"][3]) <= 2e-5 * abs(o3["epot"][3])
+        assert abs(float(o_ek.item()) - o3["ekin"][3]) <= 1e-4 * o3["ekin"][3]
+        nnp.nnp_md_step(ctx, 40)
+        nnp.nnp_get_state(ctx, o_x, o_v, o_ep, o_ek, None)
+        nnp.nnp_sync(ctx)
+        r2 = orc.energy_forces_cell(om, sp, o_x.cpu().numpy().astype(np.float64), cell, want_forces=False)
+        assert abs(float(o_ep.item()) - r2["E"][0]) <= U.E_RTOL * abs(r2["E"][0])
     finally:
         nnp.nnp_destroy(ctx)
     # a context too small for the supercell says so
