@@ -236,11 +236,11 @@ def run_eval_config(args):
         macs = sum(int(counts[s]) * (kpad * int(Wd[s, 1]) + int(Wd[s, 1]) * int(Wd[s, 2]) + int(Wd[s, 2]) * int(Wd[s, 3]) + int(Wd[s, 3]))
                    for s in range(7))
         ach = 2.0 * 2.0 * macs * n_nets / (mlp_ms * 1e-3) / 1e12           # forward + input gradient
-        peak = pk["bf16_sus"] * 0.5 if args.mm_mode in (1, 2, 4) else fp32_peak
+        peak = pk["bf16_sus"] if args.mm_mode == 4 else pk["bf16_sus"] * 0.5 if args.mm_mode in (1, 2) else fp32_peak   # fp16 operands: the bf16 rate; tf32: half of it
         roof = {"kernel": "mlp_all_layers (mm_mode 4: fused chain [+ layer 1 / dE/dG launches]; else 6 grouped GEMM launches per network batch)",
                 "bound": "tensor" if args.mm_mode in (1, 2, 4) else "alu",
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
-                "peak_source": "%s sustained bf16 cuBLAS x 0.5; fp32-equivalent flops counted once" % pk["source"]}
+                "peak_source": "%s sustained bf16 cuBLAS%s; fp32-equivalent flops counted once (the split issues 3 MMAs per product)" % (pk["source"], "" if args.mm_mode == 4 else " x 0.5")}
     elif dom in ("aev_forward", "aev_backward_scatter"):
         flop = {"aev_forward": n_rad * 16 * 6 + n_tri * 150.0, "aev_backward_scatter": n_rad * 16 * 10 + n_tri * 330.0}[dom]
         ach = flop / (groups[dom] * 1e-3) / 1e12
