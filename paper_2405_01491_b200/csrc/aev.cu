@@ -675,13 +675,13 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
         // ---- radial: dE/dr_ij = sum_k g[s_j*16+k] * 1/4 e_k (-2 eta (r-ShfR_k) fc + fc')
         if (c.pr.I > 0) {
             float2 gr[NNP_NSHF_R / 2];
-            const float sc0 = 0.25f * inv_nets;
+            const float scr = 0.25f * inv_nets; // the 1/4 of the radial term and 1 / n_nets scale dE/dr once, not the 16 gradients
 #pragma unroll
             for (int k4 = 0; k4 < NNP_NSHF_R / 4; ++k4) {
                 float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (c.pr.r < c.pr.L) v = g4(c.pr.tag * NNP_NSHF_R + 4 * k4);
-                gr[2 * k4] = make_float2(v.x * sc0, v.y * sc0);
-                gr[2 * k4 + 1] = make_float2(v.z * sc0, v.w * sc0);
+                gr[2 * k4] = make_float2(v.x, v.y);
+                gr[2 * k4 + 1] = make_float2(v.z, v.w);
             }
             auto term = [&](int j, const float4 xj) {
                 const float3 d = min_image<TRIC>(c.pi, xj, P);
@@ -703,7 +703,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                         acc = fma2(mul2(gr[k], e), fma2(w, fc, dfc), acc);
                     }
                     const float dEdr = acc.x + acc.y;
-                    const float sc = dEdr * rinv;
+                    const float sc = dEdr * (rinv * scr);
                     const float vx = sc * d.x, vy = sc * d.y, vz = sc * d.z;
                     atomicAdd(&frc[j], make_float4(-vx, -vy, -vz, 0.f));
                     fi[0] += vx; fi[1] += vy; fi[2] += vz;
@@ -761,16 +761,16 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
             {
                 const int pb = wcs * (2 * P.np + 1 - wcs) / 2 + (wct - wcs);
                 const int gp = P.n_rad + pb * NNP_ANG_BLOCK;
-                const float sc0 = 2.0f * inv_nets; // the prefactor 2 of the angular term
 #pragma unroll
                 for (int q4 = 0; q4 < NNP_ANG_BLOCK / 4; ++q4) {
                     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (npairs > 0) v = g4(gp + 4 * q4);
-                    gw[2 * q4] = make_float2(v.x * sc0, v.y * sc0);
-                    gw[2 * q4 + 1] = make_float2(v.z * sc0, v.w * sc0);
+                    gw[2 * q4] = make_float2(v.x, v.y);
+                    gw[2 * q4 + 1] = make_float2(v.z, v.w);
                 }
             }
             const float2 zm12 = bc2(P.zm1), half2 = bc2(0.5f);
+            const float sc_ang = 2.0f * inv_nets;
             for (int q = pt.r; q < npairs; q += pt.L) {
                 int ia, ib;
                 decode_pair(q, same, nt, inv_nt, tri, ia, ib);
@@ -817,10 +817,10 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
                 const float2 T2 = fma2(Az[0], fz[0], mul2(Az[1], fz[1]));
                 const float2 D2 = fma2(Az[0], dfz[0], mul2(Az[1], dfz[1]));
                 const float2 R2 = fma2(Cz[0], fz[0], mul2(Cz[1], fz[1]));
-                const float T = T2.x + T2.y;
+                const float T = (T2.x + T2.y) * sc_ang; // (the prefactor 2 and 1 / n_nets scale the three sums, not the 32 gradients)
                 float dE_dcs = D2.x + D2.y;
                 const float dE_drb = R2.x + R2.y;
-                const float ff = fj.x * fk.x;
+                const float ff = (fj.x * fk.x) * sc_ang;
                 dE_dcs *= ff * (P.k_ang0 * sn_inv);
                 const float half_drb = P.half_drb_scale * dE_drb * ff;
                 const float dE_drj = fmaf(T * sm.dfc[ia], fk.x, half_drb);

@@ -28,10 +28,11 @@
 // 1024 for seven species) the first and the last GEMM are wider than a TMEM region: F1 takes its operand through the region in
 // passes of 16 chunks (a slot is rewritten once the MMAs of the pass before have completed), B1 writes its output in passes of
 // 256 columns into the same region, from the operand that stays in the other one (kernels with WIDE = true).
-// Warp roles: 0 producer (TMA tiles of the chain's input + bulk weight copies), 1 MMA issue, 2-17 epilogue (four warps per
-// TMEM lane quarter, every fourth 16-column chunk each); the epilogue warps also convert the chain's input (fp32 tile in
-// shared memory -> fp16 hi / lo chunks in TMEM) at the start of a tile.  576 threads: 112 registers each, no spills - with
-// ~200 KiB of the SM's 228 KiB configured as shared memory, local-memory traffic would go to L2.
+// Warp roles: 0 producer (TMA tiles of the chain's input + bulk weight copies), 1 and 18 MMA issue (even / odd chunks),
+// 2-17 epilogue (four warps per TMEM lane quarter, every fourth 16-column chunk each); the epilogue warps also convert the
+// chain's input (fp32 tile in shared memory -> fp16 hi / lo chunks in TMEM) at the start of a tile.  608 threads, at most
+// five warps per SM quadrant: 96 registers each - with ~200 KiB of the SM's 228 KiB configured as shared memory,
+// local-memory traffic would go to L2.
 #include <cuda.h>
 #include <cuda_fp16.h>
 
@@ -66,7 +67,8 @@ constexpr int GCACHE = 8;               // group descriptors a CTA keeps in shar
 constexpr int GROUP_BYTES = 576;
 constexpr int SB_BYTES = 4 * 256 * 4;     // biases of the three forward GEMMs (x 16) and w4 of the current group
 constexpr int SMEM_BYTES = 1024 + NW * W_ENTRY_BYTES + NA * A_TILE_BYTES + BAR_BYTES + EPI_WARPS * EPI_STG_BYTES + GCACHE * GROUP_BYTES + SB_BYTES;
-constexpr int THREADS = (2 + EPI_WARPS) * 32;
+constexpr int MMA2_WARP = 2 + EPI_WARPS;  // the second MMA-issuing warp (odd chunks)
+constexpr int THREADS = (3 + EPI_WARPS) * 32;
 constexpr int REGION_COLS = 256;       // two accumulator / operand regions: columns [0, 256) and [256, 512)
 constexpr int GRP = 4 * CH;                // columns per round of the epilogue: one chunk of every set, one K block of weights
 constexpr int MAX_CHUNKS = REGION_COLS / CH;
@@ -75,7 +77,7 @@ constexpr float ACT_SCALE = 16.0f;
 constexpr float RANGE_LIMIT = 60000.0f;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 static_assert(NA == 2, "input tile k lives in ring entry k & 1: one entry per pair of epilogue sets");
-static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 3) + 8 <= BAR_BYTES, "barrier area");
+static_assert(8 * (2 * NW + 2 * NA + 2 * MAX_CHUNKS + 2 + 4) + 8 <= BAR_BYTES, "barrier area");
 
 enum FusedEpi {
     FE_FWD = 0,     // h = celu(acc + bias): stash h, hi/lo -> operand
@@ -317,7 +319,8 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     const uint32_t bar_accf = bar_ready + 8 * 2 * MAX_CHUNKS;  // [2 regions]: every MMA into the region has completed
     const uint32_t bar_drained = bar_accf + 16;                // an accumulator of the chain's last GEMM has been read
     const uint32_t bar_pass = bar_drained + 8;                 // wide input: the MMAs of a pass of 16 chunks have completed
-    const uint32_t tmem_slot = bar_pass + 8;
+    const uint32_t bar_first = bar_pass + 8;                   // the MMAs of chunk 0 of a GEMM (they overwrite the accumulator) have completed
+    const uint32_t tmem_slot = bar_first + 8;
     const uint32_t stg_base = bar_base + BAR_BYTES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -336,13 +339,14 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
     }
 
     if (threadIdx.x == 0) {
-        for (int e = 0; e < NW; ++e) { mbar_init(bar_wfull + 8 * e, 1); mbar_init(bar_wempty + 8 * e, 1); }
+        for (int e = 0; e < NW; ++e) { mbar_init(bar_wfull + 8 * e, 1); mbar_init(bar_wempty + 8 * e, 2); } // (both MMA warps release an entry)
         for (int e = 0; e < NA; ++e) { mbar_init(bar_afull + 8 * e, 1); mbar_init(bar_aempty + 8 * e, 8); }
         for (int k = 0; k < 2 * MAX_CHUNKS; ++k) mbar_init(bar_ready + 8 * k, 4);
-        mbar_init(bar_accf, 1);
-        mbar_init(bar_accf + 8, 1);
+        mbar_init(bar_accf, 2);
+        mbar_init(bar_accf + 8, 2);
         mbar_init(bar_drained, EPI_WARPS);
-        mbar_init(bar_pass, 1);
+        mbar_init(bar_pass, 2);
+        mbar_init(bar_first, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -410,16 +414,21 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                 }
             }
         }
-    } else if (warp == 1) {
-        // ===== MMA issue.  The whole warp walks the loop and one elected lane issues; every value an MMA takes is first made
+    } else if (warp == 1 || warp == MMA2_WARP) {
+        // ===== MMA issue (two warps).  The whole warp walks the loop and one elected lane issues; every value an MMA takes is first made
         // PROVABLY warp-uniform (uni(): a broadcast from lane 0) - the operands of tcgen05.mma live in uniform registers, and
         // for values the compiler cannot prove uniform (anything loaded from memory) it wraps each MMA in an
         // elect / R2UR.BROADCAST loop of a dozen dependent instructions (~150 cycles per MMA measured).
         auto uni = [](uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); };
         const uint32_t tb = uni(tmem_base), wr = uni(w_ring);
         const int tu_beg = (int)uni((uint32_t)t_beg), tu_end = (int)uni((uint32_t)t_end);
+        // Two warps issue: this one (mw = 0) the even chunks of every GEMM, the second (mw = 1) the odd ones.  Waiting for a
+        // chunk, electing a lane and moving an MMA's operands into uniform registers costs ~500 cycles per chunk on one warp
+        // against 190-380 cycles of tensor work, and that warp paced the whole chain.  The MMAs of chunk 0 overwrite the
+        // accumulator: the second warp starts a GEMM only after they have COMPLETED (bar_first, committed by this warp).
+        const uint32_t mw = uni(warp == 1 ? 0u : 1u);
         uint32_t wi = 0, rc = 0, par0 = 0u, par1 = 0u; // parities of the chunk barriers, one bit per chunk slot and region
-        uint32_t nd = 0;                               // phases of bar_drained consumed so far
+        uint32_t nd = 0, nf = 0;                       // phases of bar_drained / bar_first consumed so far
         bool pending_drain = false;                    // the last accumulator written has not been waited for yet
         for (int t = tu_beg; t < tu_end; ++t) {
             const int gi = (int)uni((uint32_t)find_group(gsm, n_gc, t));
@@ -448,6 +457,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                         pending_drain = false;
                         tc_fence_after();
                     }
+                    bool first_pending = mw != 0u; // (second warp) chunk 0 of this GEMM / pass not known to be complete yet
                     for (int kb = 0; kb < nkb; ++kb) {
                         const uint32_t e0 = wi % NW, e1 = (wi + 1) % NW;
                         mbar_wait(bar_wfull + 8 * e0, (wi / NW) & 1, 220 + j, (t - tu_beg) * 100 + kb);
@@ -461,9 +471,16 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                         // the first / last GEMM of a wide chain: config 5 7.35 -> 7.83 ms)
                         for (int h = 0; h < nh; ++h) {
                             const int c = 4 * kb + h, slot = WIDE ? c % MAX_CHUNKS : c; // an operand wider than a region reuses its slots
+                            if ((uint32_t)(h & 1) != mw) continue;
                             if (!WIDE || col == 0) { // (further passes multiply the operand that is already there)
                                 mbar_wait(bar_ready + 8 * (ra * MAX_CHUNKS + slot), ((ra ? par1 : par0) >> slot) & 1u, 240 + j, (t - tu_beg) * 100 + c);
                                 if (ra) par1 ^= 1u << slot; else par0 ^= 1u << slot;
+                                tc_fence_after();
+                            }
+                            if (first_pending) {
+                                mbar_wait(bar_first, nf & 1u, 250 + j, (t - tu_beg) * 100 + c);
+                                ++nf;
+                                first_pending = false;
                                 tc_fence_after();
                             }
                             if (elect_one()) {
@@ -477,8 +494,10 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                                     mma_f16_ts(acc + 128, a_hi, d1lo + koff, idesc1, 1u);
                                     mma_f16_ts(acc + 128, a_hi, d1hi + koff, idesc1, 1u);
                                 }
-                                if (WIDE && slot == MAX_CHUNKS - 1 && c + 1 < nch_tot) tc_commit(bar_pass); // the slots may be rewritten
-                                if (h + 1 == nh) {
+                                if (c == 0) tc_commit(bar_first);
+                                // (each warp after its last slot of a pass of 16: the slots may be rewritten)
+                                if (WIDE && slot >= MAX_CHUNKS - 2 && (c | (MAX_CHUNKS - 1)) + 1 < nch_tot) tc_commit(bar_pass);
+                                if (h + 2 >= nh) { // this warp's last chunk of the K block
                                     tc_commit(bar_wempty + 8 * e0);
                                     if (wide) tc_commit(bar_wempty + 8 * e1);
                                     if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
@@ -486,7 +505,19 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                             }
                             __syncwarp();
                         }
+                        if ((uint32_t)nh <= mw) { // no chunk of this K block was this warp's: it releases the weights all the same
+                            if (elect_one()) {
+                                tc_commit(bar_wempty + 8 * e0);
+                                if (wide) tc_commit(bar_wempty + 8 * e1);
+                                if (kb + 1 == nkb) tc_commit(bar_accf + 8 * rd);
+                            }
+                            __syncwarp();
+                        }
                         wi += wide ? 2u : 1u;
+                    }
+                    if (first_pending) { // (a GEMM of a single chunk: the phase is taken all the same)
+                        mbar_wait(bar_first, nf & 1u, 260 + j, t - tu_beg);
+                        ++nf;
                     }
                     if (j + 1 == n_stages) pending_drain = true;
                 } while (WIDE && (col += Np) < n_total);
@@ -531,7 +562,7 @@ k_mlp_fused(const FusedGroup *__restrict__ groups, int n_groups, const int *__re
                 const uint32_t r0 = rc & 1u;
                 for (int c_pass = 0, pass = 0; c_pass < (WIDE ? nch0 : 1); c_pass += MAX_CHUNKS, ++pass) {
                     // an input wider than a region goes through it in passes of 16 chunks: a slot is written again once the
-                    // MMAs of the pass before have completed (bar_pass, committed by the MMA warp per pass).  Every warp
+                    // MMAs of the pass before have completed (bar_pass, committed by both MMA warps per pass).  Every warp
                     // takes every phase of this barrier, with or without a chunk in the pass: an mbarrier wait names a
                     // phase by its parity only, so a waiter that skipped one would take the phase before for its own.
                     if (WIDE && pass > 0) {
