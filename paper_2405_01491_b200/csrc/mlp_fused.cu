@@ -143,6 +143,34 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16
         : "memory");
 }
 
+// Packed fp32 pairs (FFMA2 / FMUL2 / FADD2): one issue slot for two columns of the epilogue arithmetic.
+__device__ __forceinline__ float2 f2_fma(const float2 a, const float2 b, const float2 c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<const unsigned long long *>(&a)), "l"(*reinterpret_cast<const unsigned long long *>(&b)),
+          "l"(*reinterpret_cast<const unsigned long long *>(&c)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 f2_mul(const float2 a, const float2 b)
+{
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<const unsigned long long *>(&a)), "l"(*reinterpret_cast<const unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 f2_add(const float2 a, const float2 b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<const unsigned long long *>(&a)), "l"(*reinterpret_cast<const unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&d);
+}
+__device__ __forceinline__ float2 f2_bc(const float s) { return make_float2(s, s); }
+
 // 16 consecutive K values of one row -> the row's 16 operand columns: hi pairs (k, k+1) in columns 0..7, lo pairs in 8..15
 __device__ __forceinline__ void split16(const float (&x)[16], uint32_t (&v)[16])
 {
@@ -150,7 +178,8 @@ __device__ __forceinline__ void split16(const float (&x)[16], uint32_t (&v)[16])
     for (int q = 0; q < 8; ++q) {
         const __half2 h = __floats2half2_rn(x[2 * q], x[2 * q + 1]);
         const float2 hf = __half22float2(h);
-        const __half2 l = __floats2half2_rn(x[2 * q] - hf.x, x[2 * q + 1] - hf.y);
+        const float2 lf = f2_fma(hf, f2_bc(-1.0f), make_float2(x[2 * q], x[2 * q + 1])); // x - hi, exact
+        const __half2 l = __floats2half2_rn(lf.x, lf.y);
         v[q] = *reinterpret_cast<const uint32_t *>(&h);
         v[8 + q] = *reinterpret_cast<const uint32_t *>(&l);
     }
@@ -171,7 +200,8 @@ template <int EPI>
 __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mrow0, int lane_set, uint32_t tm_acc, uint32_t stg,
                                          uint32_t accf, uint32_t bar_ready, uint32_t sb, float alpha, int aux, int n_cols, int col_off)
 {
-    float vmax = 0.f, esum = 0.f;
+    float vmax = 0.f;
+    float2 esum = make_float2(0.f, 0.f);
     constexpr bool fwd = EPI == FE_FWD || EPI == FE_OUT;
     constexpr bool rd_prev = EPI == FE_BWD;                        // reads rows of h for CELU'
     constexpr bool to_op = EPI == FE_FWD || EPI == FE_OUT || EPI == FE_BWD;
@@ -230,23 +260,28 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
             const float xq[4] = {x4.x, x4.y, x4.z, x4.w};
             const float wq[4] = {w4v.x, w4v.y, w4v.z, w4v.w};
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                float v = __uint_as_float(a[4 * q + e]);
+            for (int e = 0; e < 4; e += 2) { // two columns at a time: packed fp32 arithmetic, min / max and ex2 per column
+                float2 v = make_float2(__uint_as_float(a[4 * q + e]), __uint_as_float(a[4 * q + e + 1]));
+                const float2 x2 = make_float2(xq[e], xq[e + 1]);
                 if (fwd) {
-                    const float z = fmaf(v, c_acc, xq[e]);
-                    float ex;
-                    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(fminf(z, 0.f) * ce));
-                    v = fmaf(a16, ex, fmaxf(z, 0.f) - a16);                // 16 h
+                    const float2 z = f2_fma(v, f2_bc(c_acc), x2);
+                    const float2 t = f2_mul(make_float2(fminf(z.x, 0.f), fminf(z.y, 0.f)), f2_bc(ce));
+                    float2 ex;
+                    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex.x) : "f"(t.x));
+                    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex.y) : "f"(t.y));
+                    v = f2_fma(f2_bc(a16), ex, f2_add(make_float2(fmaxf(z.x, 0.f), fmaxf(z.y, 0.f)), f2_bc(-a16))); // 16 h
                     if (EPI == FE_OUT) {
-                        esum = fmaf(v, wq[e], esum);
-                        v = wq[e] * fmaf(fminf(v, 0.f), inv_alpha, ACT_SCALE); // 16 w4 celu'(h3)
+                        const float2 w2 = make_float2(wq[e], wq[e + 1]);
+                        esum = f2_fma(v, w2, esum);
+                        v = f2_mul(w2, f2_fma(make_float2(fminf(v.x, 0.f), fminf(v.y, 0.f)), f2_bc(inv_alpha), f2_bc(ACT_SCALE))); // 16 w4 celu'(h3)
                     }
                 } else if (rd_prev) {
-                    v *= fmaf(fminf(xq[e], 0.f), gs, gc);
+                    v = f2_mul(v, f2_fma(make_float2(fminf(x2.x, 0.f), fminf(x2.y, 0.f)), f2_bc(gs), f2_bc(gc)));
                 } else {
-                    v *= c_acc;
+                    v = f2_mul(v, f2_bc(c_acc));
                 }
-                ov[4 * q + e] = v;
+                ov[4 * q + e] = v.x;
+                ov[4 * q + e + 1] = v.y;
             }
         }
         if (to_op) {
@@ -282,7 +317,7 @@ __device__ __forceinline__ float2 epi_stage(const FusedGroup *gp, int j, int mro
             __syncwarp();
         }
     }
-    return make_float2(vmax, esum);
+    return make_float2(vmax, esum.x + esum.y);
 }
 
 // rows of the two MMAs of a GEMM with N columns: 128 + (N - 128), or N alone (one MMA with N > 128 and its operand in
@@ -898,10 +933,17 @@ int nnp_fused_setup(nnp_ctx *c)
             bwd(5, h1, kpad, nn > 1 ? FE_RED : FE_ST, f->w_off[q][5], nullptr, 0, wsh[q][0]);
             g.out = c->dG + (size_t)off * kpad;
             g.ldo = kpad;
-            long long cst = 0;
-            for (int j = 0; j < g.n_stages; ++j)
-                cst += (long long)(g.st[j].K / CH) * 3 * (g.st[j].n_total / 2) + 1200LL * ((g.st[j].n_total + REGION_COLS - 1) / REGION_COLS) +
-                       (j + 1 == g.n_stages ? 25LL * g.st[j].n_total : 0); // MMA cycles + hand-over bubbles + a wide last GEMM's serial epilogues
+            // Cost of a tile in cycles, for the split of the tiles over the CTAs.  Measured per CTA (clock64 around the tile
+            // loop, 98k-atom water box): a tile takes 3.1 k cycles per round of the epilogue (the sixteen warps drain 64
+            // accumulator columns per round) - 59.0 k for the H network (19 rounds), 49.7 k for O (16 rounds); a GEMM whose
+            // MMAs take longer than its rounds (the first of a wide chain) counts with those, and the conversion of the chain's
+            // input with 2 k cycles per 64 columns.  (The first model, MMA cycles + a constant per GEMM, made O tiles 0.78 of an
+            // H tile: CTAs with seven O tiles ran 349 k cycles against a mean of 290 k.)
+            long long cst = 2000LL * ((g.st[0].K + 63) / 64);
+            for (int j = 0; j < g.n_stages; ++j) {
+                const long long rounds = 3100LL * ((g.st[j].n_total + 63) / 64), mma = (long long)(g.st[j].K / CH) * 3 * (g.st[j].n_total / 2);
+                cst += rounds > mma ? rounds : mma;
+            }
             tiles += g.n_tiles;
             groups.push_back(g);
             cost.push_back(cst);
