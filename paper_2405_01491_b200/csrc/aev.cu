@@ -2,8 +2,8 @@
 // Definition: SURVEY.md 8(c) O2/O3/O6 (PAPER.md L61 cosine switch, L79 Gaussian radial basis, L443 angular form
 // (0.5+0.5cos(theta-theta_n))^zeta, L55 pairs of edges with a common centre, L65/L176 forces by reverse mode).
 //
-// Persistent warps, one centre atom per warp at a time (forward: handed out by a ticket counter, reverse: static
-// stride - CentreQueue below).  Neighbour rows are grouped by neighbour species (stage 1).  Arithmetic of the inner
+// One centre atom per warp at a time (forward: persistent warps, centres handed out by a ticket counter; reverse: two
+// consecutive centres per warp of a plain grid - CentreQueue below).  Neighbour rows are grouped by neighbour species (stage 1).  Arithmetic of the inner
 // loops is packed f32x2 (FFMA2 / FMUL2 / FADD2, one issue slot for two lanes of math); the forward kernel evaluates
 // uniformly spaced shift sets by a Gaussian ladder (AevParams::ladder).
 //   loads:   the species-segment table of the NEXT centre is fetched one centre ahead; for the current centre all
@@ -219,7 +219,18 @@ __device__ __forceinline__ void decode_pair(int q, bool same, int nt, float inv_
 #define AEV_FWD_SCHED 1
 #endif
 #ifndef AEV_BWD_SCHED
-#define AEV_BWD_SCHED 0
+#define AEV_BWD_SCHED 4
+#endif
+// MODE 4 (the reverse kernel): no queue and no persistent grid - a warp takes AEV_CPW consecutive centres and its block
+// ends; the hardware's block scheduler levels out the warps.  With the persistent static stride (MODE 0) the warps of the
+// 98k-atom water box finished between 217 and 288 us (mean 246 us: the cost of a centre varies with its pair count, and a warp
+// keeps its 33 centres whatever they cost); blocks of 4 warps x 2 centres: 0.2915 -> 0.282 ms (4 centres 0.283, 8 0.296,
+// one-warp blocks 0.283-0.287).  The ticket queues stay slower for this kernel (0.327 ms, re-measured), also as a hybrid
+// (static first, tickets for the last 8-25 %: 0.319-0.332 ms; with an empty ticket phase still 0.35 ms - every warp's centres
+// take 22 % longer although the loops compile to the same instructions), and MODE 4 is slower for the forward kernel
+// (0.191 against 0.185 ms with tickets).
+#ifndef AEV_CPW
+#define AEV_CPW 2
 #endif
 template <int MODE>
 struct CentreQueue {
@@ -227,6 +238,7 @@ struct CentreQueue {
     int n, nsm, s, lane;
     int beg, end;  // current range
     int pending;   // lane 0: ticket requested and not yet read
+    int cpw;           // MODE 4: consecutive centres per warp
 
     __device__ __forceinline__ void set_range(int r)
     {
@@ -234,9 +246,9 @@ struct CentreQueue {
         beg = (int)((long long)r * n / nsm);
         end = (int)((long long)(r + 1) * n / nsm);
     }
-    __device__ __forceinline__ void init(int *sched_, int n_, int nsm_, int lane_)
+    __device__ __forceinline__ void init(int *sched_, int n_, int nsm_, int lane_, int cpw_)
     {
-        sched = sched_; n = n_; lane = lane_; pending = 0;
+        sched = sched_; n = n_; lane = lane_; pending = 0; cpw = cpw_;
         nsm = MODE == 2 ? nsm_ : 1;
         unsigned smid = 0;
         if (MODE == 2) asm("mov.u32 %0, %%smid;" : "=r"(smid));
@@ -244,12 +256,17 @@ struct CentreQueue {
     }
     __device__ __forceinline__ void request()
     {
+        if (MODE == 4) return;
         if (MODE != 0 && lane == 0) pending = atomicAdd(sched + 32 + s, 1);
     }
     // cur: the centre being processed (MODE 0 only)
     __device__ __forceinline__ int receive(int cur)
     {
         if (MODE == 0) return cur < 0 ? (int)(blockIdx.x * kWarps + (threadIdx.x >> 5)) : cur + (int)(gridDim.x * kWarps);
+        if (MODE == 4) { // AEV_CPW consecutive centres per warp, one block after the other (the grid is not persistent)
+            if (cur < 0) return (int)(blockIdx.x * kWarps + (threadIdx.x >> 5)) * cpw;
+            return (cur + 1) % cpw ? cur + 1 : n;
+        }
         for (;;) {
             const int t = beg + __shfl_sync(kFull, pending, 0);
             if (t < end) return t;
@@ -275,7 +292,7 @@ struct CentreQueue {
     }
     __device__ __forceinline__ void release()
     {
-        if (MODE == 0) return;
+        if (MODE == 0 || MODE == 4) return;
         int last = 0;
         if (lane == 0) last = atomicAdd(sched, 1) == (int)(gridDim.x * kWarps) - 1;
         if (__shfl_sync(kFull, last, 0)) {
@@ -410,7 +427,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
     const float lad_r = LAD ? P.lad_r[lane & 15] : 1.0f, lad_a = LAD ? P.lad_a[lane >> 2] : 1.0f;
 
     CentreQueue<AEV_FWD_SCHED> queue;
-    queue.init(sched, n, nsm, lane);
+    queue.init(sched, n, nsm, lane, 1);
     queue.request();
     int i = queue.receive(-1);
     int sgr_l = 0, sga_l = 0;
@@ -639,11 +656,11 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     // (-2 eta / ka) w ra with w = ka (rb - s): P.half_drb_scale, P.dr_scale (AevParams, nnp_aev_derive)
     float (*fsm)[3] = reinterpret_cast<float (*)[3]>(sm.ab);
 
-    // Centres are assigned statically (AEV_BWD_SCHED 0: warp w takes w, w + W, ...): for this kernel the ticket queues
-    // measured slower (0.335 / 0.339 ms against 0.300 ms), see DESIGN.md section 6.
+    // Centres are assigned statically, AEV_CPW consecutive ones per warp of a non-persistent grid (AEV_BWD_SCHED 4, above);
+    // for this kernel the ticket queues measured slower, see DESIGN.md section 6.
     float vir[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     CentreQueue<AEV_BWD_SCHED> queue;
-    queue.init(sched, n, nsm, lane);
+    queue.init(sched, n, nsm, lane, AEV_CPW);
     queue.request();
     int i = queue.receive(-1);
     int sgr_l = 0, sga_l = 0;
@@ -939,7 +956,7 @@ void nnp_launch_aev_backward(nnp_ctx *c, float inv_nets, double *d_virial)
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks[gs][vir], kern, kWarps * 32, smem);
     }
-    const int grid = persistent_grid(c, blocks[gs][vir]);
+    const int grid = AEV_BWD_SCHED == 4 ? nnp_div_up(c->n, kWarps * AEV_CPW) : persistent_grid(c, blocks[gs][vir]);
     kern<<<grid, kWarps * 32, smem, c->stream>>>(
         c->n, c->aev, c->pos, c->nbr_r, c->seg_r, c->nbr_a, c->seg_a, c->d_tri, c->dG, inv_nets, c->frc, c->flags, c->aev_sched + NNP_AEV_SCHED_LEN, g_sms,
         d_virial);
