@@ -262,3 +262,38 @@ def test_repeatability_stress():
         assert repeatability.main() == 0
     finally:
         sys.argv = argv
+
+@pytest.mark.gpu
+def test_buckets_of_more_than_32_atoms_are_ordered_too(model1):
+    """The neighbour build orders every (species, cell) bucket by previous index: one warp ranks a bucket of up to 32 atoms,
+    lane 0 sorts larger ones serially.  A dense one-species box (54 atoms per cell) and a non-periodic cluster of 150 atoms
+    (its single "cell" is the structure) take that path; lists as exact rows, E and F against the oracle, and the same
+    result on a second evaluation after the atoms have been re-sorted once more."""
+    consts, widths, params, om = model1
+    cases = []
+    sp, xyz, box = inputs.dense_box(0.25, n_species=1)
+    cases.append((sp, xyz, box, 320, 128))
+    spw, xyzw, boxw = inputs.water_box(216)
+    centre = xyzw.mean(0)
+    keep = np.argsort(((xyzw - centre) ** 2).sum(1))[:150]
+    cases.append((spw[keep].astype(np.int32), xyzw[keep], None, 160, 64))
+    for sp, xyz, box, cap_r, cap_a in cases:
+        n = len(sp)
+        assert np.bincount(sp).max() > 32
+        ctx = U.gpu_create(consts, widths, params, 1, n, cap_r=cap_r, cap_a=cap_a)
+        try:
+            ref = orc.energy_forces(om, sp, xyz, box)
+            rms = np.sqrt((ref["F"] ** 2).sum(1).mean())
+            for rep in range(2):
+                Eg, Fg = U.gpu_energy_forces(ctx, sp, xyz, box)
+                assert abs(Eg[0] - ref["E"][0]) <= U.E_RTOL * abs(ref["E"][0])
+                assert np.abs(Fg - ref["F"]).max() <= U.F_ATOL * max(1.0, rms / 20.0)
+            for which, rc in ((0, 5.1), (1, 3.5)):
+                got = U.gpu_neighbors(ctx, which, n, stride=cap_r)
+                want = orc.neighbors(xyz, box, float(np.float32(rc)), fp32_pred=True)
+                assert all(np.array_equal(got[i], want[i]) for i in range(n))
+        finally:
+            nnp.nnp_destroy(ctx)
+
+
+
