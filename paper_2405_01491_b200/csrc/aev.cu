@@ -415,7 +415,11 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
 {
     __shared__ WarpSmem smem[kWarps];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    WarpSmem &sm = smem[wid];
+    // (as in the reverse kernel: an opaque base keeps the compiler from re-deriving it from %tid inside the centre loop -
+    // 36 of ~1480 instructions per centre, 0.1853 -> 0.1836 ms)
+    uint32_t sm_addr = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)wid * (uint32_t)sizeof(WarpSmem);
+    asm volatile("mov.b32 %0, %0;" : "+r"(sm_addr));
+    WarpSmem &sm = *reinterpret_cast<WarpSmem *>(__cvta_shared_to_generic(sm_addr));
     int bcs, bct;
     block_of_lane(P.np, lane, bcs, bct);
     const int nb_tot = P.np * (P.np + 1) / 2;
