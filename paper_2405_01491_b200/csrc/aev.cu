@@ -238,7 +238,6 @@ struct CentreQueue {
     int n, nsm, s, lane;
     int beg, end;  // current range
     int pending;   // lane 0: ticket requested and not yet read
-    int cpw;           // MODE 4: consecutive centres per warp
 
     __device__ __forceinline__ void set_range(int r)
     {
@@ -246,9 +245,9 @@ struct CentreQueue {
         beg = (int)((long long)r * n / nsm);
         end = (int)((long long)(r + 1) * n / nsm);
     }
-    __device__ __forceinline__ void init(int *sched_, int n_, int nsm_, int lane_, int cpw_)
+    __device__ __forceinline__ void init(int *sched_, int n_, int nsm_, int lane_)
     {
-        sched = sched_; n = n_; lane = lane_; pending = 0; cpw = cpw_;
+        sched = sched_; n = n_; lane = lane_; pending = 0;
         nsm = MODE == 2 ? nsm_ : 1;
         unsigned smid = 0;
         if (MODE == 2) asm("mov.u32 %0, %%smid;" : "=r"(smid));
@@ -264,8 +263,8 @@ struct CentreQueue {
     {
         if (MODE == 0) return cur < 0 ? (int)(blockIdx.x * kWarps + (threadIdx.x >> 5)) : cur + (int)(gridDim.x * kWarps);
         if (MODE == 4) { // AEV_CPW consecutive centres per warp, one block after the other (the grid is not persistent)
-            if (cur < 0) return (int)(blockIdx.x * kWarps + (threadIdx.x >> 5)) * cpw;
-            return (cur + 1) % cpw ? cur + 1 : n;
+            if (cur < 0) return (int)(blockIdx.x * kWarps + (threadIdx.x >> 5)) * AEV_CPW;
+            return (cur + 1) % AEV_CPW ? cur + 1 : n;
         }
         for (;;) {
             const int t = beg + __shfl_sync(kFull, pending, 0);
@@ -431,7 +430,7 @@ k_aev_forward(int n, AevParams P, const float4 *__restrict__ pos, const int *__r
     const float lad_r = LAD ? P.lad_r[lane & 15] : 1.0f, lad_a = LAD ? P.lad_a[lane >> 2] : 1.0f;
 
     CentreQueue<AEV_FWD_SCHED> queue;
-    queue.init(sched, n, nsm, lane, 1);
+    queue.init(sched, n, nsm, lane);
     queue.request();
     int i = queue.receive(-1);
     int sgr_l = 0, sga_l = 0;
@@ -664,7 +663,7 @@ k_aev_backward(int n, AevParams P, const float4 *__restrict__ pos, const int *__
     // for this kernel the ticket queues measured slower, see DESIGN.md section 6.
     float vir[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     CentreQueue<AEV_BWD_SCHED> queue;
-    queue.init(sched, n, nsm, lane, AEV_CPW);
+    queue.init(sched, n, nsm, lane);
     queue.request();
     int i = queue.receive(-1);
     int sgr_l = 0, sga_l = 0;
