@@ -4,6 +4,8 @@
 //   * every neighbour row, filled species by species, is automatically grouped by neighbour species
 //     (stage 2 needs that: its angular accumulators are per species pair).
 // List membership is the fp32 predicate of reading A3: fixed order, round-to-nearest, no FMA.
+#include <stdlib.h>
+
 #include "nnp_internal.cuh"
 
 namespace {
@@ -241,6 +243,17 @@ __device__ __forceinline__ float r2_defined(const float4 a, const float4 b, cons
     return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
 }
 
+// (the orthorhombic branch alone: the one-block-per-cell kernel never sees another cell type)
+__device__ __forceinline__ float r2_ortho(const float4 a, const float4 b, const GridInfo &g)
+{
+    float dx = __fsub_rn(b.x, a.x), dy = __fsub_rn(b.y, a.y), dz = __fsub_rn(b.z, a.z);
+    const float M = 12582912.0f;
+    dx = __fsub_rn(dx, __fmul_rn(g.box[0], __fsub_rn(__fadd_rn(__fmul_rn(dx, g.inv_box[0]), M), M)));
+    dy = __fsub_rn(dy, __fmul_rn(g.box[1], __fsub_rn(__fadd_rn(__fmul_rn(dy, g.inv_box[1]), M), M)));
+    dz = __fsub_rn(dz, __fmul_rn(g.box[2], __fsub_rn(__fadd_rn(__fmul_rn(dz, g.inv_box[2]), M), M)));
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+
 // One warp per atom.  Per species (rows must stay grouped by neighbour species, stage 2), the candidate cells
 // are <= 18 contiguous index ranges of the sorted order: the 3 x 3 (y,z) rows of the stencil, each one or two
 // x-ranges (x-adjacent cells are adjacent in the sort).  Lane r fetches the bounds of range r (one load round per
@@ -376,6 +389,162 @@ k_build_lists(int n, int S, unsigned present, const float4 *__restrict__ pos, co
     }
 }
 
+// The same lists, one block per cell (orthorhombic periodic boxes with at least three cells per dimension): the atoms of the
+// 27 stencil cells are staged ONCE in shared memory for all centres of the cell (SURVEY section 6 / north_star: "shared-
+// memory staging of neighbour tiles"), wrapped into the box and shifted by the periodic image under which the stencil cell is
+// seen from this one, so that a candidate costs a shared-memory load, three subtractions and a sum of squares instead of an
+// index-range decode, a global load and a minimum image (~40 against ~78 instructions per 32 candidates; all 27 cells instead
+// of the per-atom trimmed stencil: 1.4 times the candidates).  The wrapped and shifted difference is not the arithmetic of
+// reading A3, it only agrees with it to rounding: a candidate whose r^2 falls within `band` of a list radius is decided by
+// r2_defined() on the two original positions (a few per cent of the centres have one), so the rows are the defined ones.
+// band: the staged coordinates and the wrapped centre carry at most ~2 ulp of the largest |coordinate| involved each, so
+// |r2' - r2| <= 2 |d|_1 * 4 ulp(M) + rounding of the squares < 32 rl eps M with M = max |x| + 2 L (block maximum).
+// A pair whose cell-derived image differs from rint((xj - xi) / L) is at least 1.05 cell widths apart under both: rejected by both.
+constexpr int kTileWarps = 4;
+constexpr int kTileCap = 1024;   // candidates staged at a time (16 KiB); longer species segments come in windows
+constexpr int kTileCen = 128;    // centres of a cell handled at a time
+__global__ void __launch_bounds__(kTileWarps * 32)
+k_build_lists_tile(int n, int S, unsigned present, const float4 *__restrict__ pos, const int *__restrict__ cell_start, GridInfo g,
+                   float rl_r, float rl2_r, float rl2_a, int cap_r, int cap_a, int *__restrict__ nbr_r, int *__restrict__ nbr_a,
+                   uint16_t *__restrict__ seg_r, uint16_t *__restrict__ seg_a, int *__restrict__ flags, const int *cond)
+{
+    if (cond && *cond == 0) return;
+    __shared__ float4 cand[kTileCap + 32];            // wrapped + shifted position, w = index as bits (+ padding of the last trip)
+    __shared__ int s_rbeg[27], s_pref[28];            // stencil ranges of the current species: first atom, prefix of the lengths
+    __shared__ float s_sh[27][3];                     // their image shifts
+    __shared__ int s_cen[kTileCen], s_cnt_r[kTileCen], s_cnt_a[kTileCen];
+    __shared__ int s_cpref[NNP_MAX_SPECIES + 1];      // centres of the cell per species (prefix)
+    __shared__ unsigned s_mmax;
+    const unsigned kFull = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, wib = tid >> 5;
+    const int c = blockIdx.x, mol = c / g.ncell_box, cb = c - mol * g.ncell_box;
+    const int cx = cb % g.nc[0], cy = (cb / g.nc[0]) % g.nc[1], cz = cb / (g.nc[0] * g.nc[1]);
+    if (tid == 0) {
+        int acc = 0;
+        for (int s = 0; s < S; ++s) { s_cpref[s] = acc; acc += cell_start[s * g.ncell + c + 1] - cell_start[s * g.ncell + c]; }
+        for (int s = S; s <= NNP_MAX_SPECIES; ++s) s_cpref[s] = acc;
+        s_mmax = 0u;
+    }
+    __syncthreads();
+    const int ncen_all = s_cpref[S];
+    if (ncen_all == 0) return;
+    auto wrap = [&](float x, int d) { return x - g.box[d] * floorf(x * g.inv_box[d]); }; // as cell_coord(): may give exactly L
+    const unsigned lt = (1u << lane) - 1u;
+    // (an opaque copy of the staged array's address: the compiler re-derived it from the shared window in every trip)
+    uint32_t cand_a = (uint32_t)__cvta_generic_to_shared(cand);
+    asm volatile("mov.b32 %0, %0;" : "+r"(cand_a));
+    const float4 *cand_w = reinterpret_cast<const float4 *>(__cvta_shared_to_generic(cand_a));
+    for (int cen0 = 0; cen0 < ncen_all; cen0 += kTileCen) {
+        const int ncen = min(kTileCen, ncen_all - cen0);
+        for (int q = tid; q < ncen; q += kTileWarps * 32) {
+            const int f = cen0 + q; // f-th centre of the cell: species block s, atom cell_start[s][c] + (f - prefix)
+            int s = 0;
+            while (f >= s_cpref[s + 1]) ++s;
+            s_cen[q] = cell_start[s * g.ncell + c] + (f - s_cpref[s]);
+            s_cnt_r[q] = 0;
+            s_cnt_a[q] = 0;
+        }
+        __syncthreads();
+        for (int s = 0; s < S; ++s) {
+            for (int q = tid; q < ncen; q += kTileWarps * 32) { // where the segment of species s starts in the two rows
+                seg_r[(size_t)s_cen[q] * NNP_MAX_SPECIES + s] = (uint16_t)min(s_cnt_r[q], cap_r);
+                seg_a[(size_t)s_cen[q] * NNP_MAX_SPECIES + s] = (uint16_t)min(s_cnt_a[q], cap_a);
+            }
+            if (!(present >> s & 1u)) continue;
+            if (wib == 0) { // the 27 stencil cells of this cell for species s
+                int len = 0;
+                if (lane < 27) {
+                    const int dx = lane % 3 - 1, dy = (lane / 3) % 3 - 1, dz = lane / 9 - 1;
+                    int x = cx + dx, y = cy + dy, z = cz + dz;
+                    float sx = 0.f, sy = 0.f, sz = 0.f;
+                    if (x < 0) { x += g.nc[0]; sx = -g.box[0]; } else if (x >= g.nc[0]) { x -= g.nc[0]; sx = g.box[0]; }
+                    if (y < 0) { y += g.nc[1]; sy = -g.box[1]; } else if (y >= g.nc[1]) { y -= g.nc[1]; sy = g.box[1]; }
+                    if (z < 0) { z += g.nc[2]; sz = -g.box[2]; } else if (z >= g.nc[2]) { z -= g.nc[2]; sz = g.box[2]; }
+                    const int cc = s * g.ncell + mol * g.ncell_box + (z * g.nc[1] + y) * g.nc[0] + x;
+                    const int beg = cell_start[cc];
+                    len = cell_start[cc + 1] - beg;
+                    s_rbeg[lane] = beg;
+                    s_sh[lane][0] = sx; s_sh[lane][1] = sy; s_sh[lane][2] = sz;
+                }
+                int incl = len;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int y = __shfl_up_sync(kFull, incl, o);
+                    if (lane >= o) incl += y;
+                }
+                if (lane < 27) s_pref[lane + 1] = incl;
+                if (lane == 0) s_pref[0] = 0;
+            }
+            __syncthreads();
+            const int total = s_pref[27];
+            for (int w0 = 0; w0 < total; w0 += kTileCap) {
+                const int nw = min(kTileCap, total - w0);
+                float mloc = 0.f;
+                for (int v = tid; v < nw; v += kTileWarps * 32) {
+                    const int flat = w0 + v;
+                    int r = 0; // range of the flat index: s_pref[r] <= flat < s_pref[r + 1] (27 entries: five halvings)
+#pragma unroll
+                    for (int st = 16; st >= 1; st >>= 1)
+                        if (r + st <= 26 && s_pref[r + st] <= flat) r += st;
+                    const int j = s_rbeg[r] + (flat - s_pref[r]);
+                    const float4 p = pos[j];
+                    mloc = fmaxf(mloc, fmaxf(fabsf(p.x), fmaxf(fabsf(p.y), fabsf(p.z))));
+                    cand[v] = make_float4(wrap(p.x, 0) + s_sh[r][0], wrap(p.y, 1) + s_sh[r][1], wrap(p.z, 2) + s_sh[r][2], __int_as_float(j));
+                }
+                for (int v = nw + tid; v < ((nw + 31) & ~31); v += kTileWarps * 32) // pad the last trip: never a neighbour
+                    cand[v] = make_float4(3.0e18f, 3.0e18f, 3.0e18f, __int_as_float(-1));
+                const unsigned mw = __reduce_max_sync(kFull, __float_as_uint(mloc)); // (non-negative floats order as integers)
+                if (lane == 0) atomicMax(&s_mmax, mw);
+                __syncthreads();
+                for (int q = wib; q < ncen; q += kTileWarps) {
+                    const int i = s_cen[q];
+                    const float4 pi = pos[i];
+                    const float mi = fmaxf(fabsf(pi.x), fmaxf(fabsf(pi.y), fabsf(pi.z)));
+                    const float M = fmaxf(__uint_as_float(s_mmax), mi) + 2.0f * fmaxf(g.box[0], fmaxf(g.box[1], g.box[2]));
+                    const float band = 32.0f * rl_r * 1.1920929e-7f * M;
+                    const float wx = wrap(pi.x, 0), wy = wrap(pi.y, 1), wz = wrap(pi.z, 2);
+                    const int cnt_r0 = s_cnt_r[q], cnt_a0 = s_cnt_a[q];
+                    // this lane's next free slot in the two rows (a pointer that moves with the row, no index arithmetic per
+                    // store) and the slots left; rows that are full count on but store nothing
+                    int *dst_r = nbr_r + (size_t)i * cap_r + cnt_r0, *dst_a = nbr_a + (size_t)i * cap_a + cnt_a0;
+                    int left_r = cap_r - cnt_r0, left_a = cap_a - cnt_a0, cnt_r = cnt_r0, cnt_a = cnt_a0;
+                    const float4 *cv = cand_w + lane;
+                    const int ntrip = (nw + 31) >> 5;
+                    for (int t = 0; t < ntrip; ++t, cv += 32) {
+                        const float4 cj = *cv;
+                        const int j = __float_as_int(cj.w);
+                        const float dx = cj.x - wx, dy = cj.y - wy, dz = cj.z - wz;
+                        float r2 = dx * dx + dy * dy + dz * dz;
+                        if ((fabsf(r2 - rl2_r) <= band || fabsf(r2 - rl2_a) <= band) && j >= 0) r2 = r2_ortho(pi, pos[j], g);
+                        const bool hr = r2 < rl2_r && j != i, ha = r2 < rl2_a && j != i;
+                        const unsigned mr = __ballot_sync(kFull, hr);
+                        const unsigned ma = __ballot_sync(kFull, ha);
+                        const int o_r = __popc(mr & lt), o_a = __popc(ma & lt), n_r = __popc(mr), n_a = __popc(ma);
+                        if (hr && o_r < left_r) dst_r[o_r] = j;
+                        if (ha && o_a < left_a) dst_a[o_a] = j;
+                        dst_r += n_r; dst_a += n_a;
+                        left_r -= n_r; left_a -= n_a;
+                        cnt_r += n_r; cnt_a += n_a;
+                    }
+                    if (lane == 0) { s_cnt_r[q] = cnt_r; s_cnt_a[q] = cnt_a; }
+                }
+                __syncthreads();
+            }
+            __syncthreads(); // (a species without candidates: nobody reads the range table any more before it is rewritten)
+        }
+        for (int q = tid; q < ncen; q += kTileWarps * 32) { // entries S..7: the row length
+            const int i = s_cen[q], cr_ = s_cnt_r[q], ca_ = s_cnt_a[q];
+            for (int s = S; s < NNP_MAX_SPECIES; ++s) {
+                seg_r[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(cr_, cap_r);
+                seg_a[(size_t)i * NNP_MAX_SPECIES + s] = (uint16_t)min(ca_, cap_a);
+            }
+            if (cr_ > cap_r) atomicOr(&flags[0], NNP_FLAG_CAP_R);
+            if (ca_ > cap_a) atomicOr(&flags[0], NNP_FLAG_CAP_A);
+        }
+        __syncthreads();
+    }
+}
+
 __global__ void k_finish_build(int *flags, const int *cond)
 {
     if (cond && *cond == 0) return;
@@ -404,6 +573,13 @@ int nnp_launch_build(nnp_ctx *c, const int *cond)
     k_copyback<<<nb, T, 0, st>>>(n, c->pos_tmp, c->vel_tmp, c->spc_tmp, c->orig_tmp, c->mol_tmp, c->pos, c->vel,
                                  c->xref, c->spc, c->orig, c->mol, cond);
     const float rl_r = c->aev.rcr + c->skin, rl_a = c->aev.rca + c->skin;
+    // one block per cell where every dimension has three distinct stencil cells (NNP_LIST_TILE=0: the warp-per-atom kernel)
+    static const bool tile_on = !(getenv("NNP_LIST_TILE") && atoi(getenv("NNP_LIST_TILE")) == 0);
+    if (tile_on && c->grid.periodic && !c->grid.tric && c->grid.nc[0] >= 3 && c->grid.nc[1] >= 3 && c->grid.nc[2] >= 3)
+        k_build_lists_tile<<<c->grid.ncell, kTileWarps * 32, 0, st>>>(n, S, c->present_mask, c->pos, c->cell_start, c->grid, rl_r, rl_r * rl_r,
+                                                                      rl_a * rl_a, c->aev.cap_r, c->aev.cap_a, c->nbr_r, c->nbr_a, c->seg_r,
+                                                                      c->seg_a, c->flags, cond);
+    else
     k_build_lists<<<nnp_div_up(n, kWarpsPerBlock), kWarpsPerBlock * 32, 0, st>>>(
         n, S, c->present_mask, c->pos, c->mol, c->cell_start, c->grid, rl_r * rl_r, rl_a * rl_a, (rl_r + 0.01f) * (rl_r + 0.01f),
         c->aev.cap_r, c->aev.cap_a,
