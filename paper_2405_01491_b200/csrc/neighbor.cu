@@ -574,7 +574,8 @@ int nnp_launch_build(nnp_ctx *c, const int *cond)
                                  c->xref, c->spc, c->orig, c->mol, cond);
     const float rl_r = c->aev.rcr + c->skin, rl_a = c->aev.rca + c->skin;
     // one block per cell where every dimension has three distinct stencil cells (NNP_LIST_TILE=0: the warp-per-atom kernel)
-    static const bool tile_on = !(getenv("NNP_LIST_TILE") && atoi(getenv("NNP_LIST_TILE")) == 0);
+    const char *tile_env = getenv("NNP_LIST_TILE"); // (read per build: a test switches it)
+    const bool tile_on = !(tile_env && atoi(tile_env) == 0);
     if (tile_on && c->grid.periodic && !c->grid.tric && c->grid.nc[0] >= 3 && c->grid.nc[1] >= 3 && c->grid.nc[2] >= 3)
         k_build_lists_tile<<<c->grid.ncell, kTileWarps * 32, 0, st>>>(n, S, c->present_mask, c->pos, c->cell_start, c->grid, rl_r, rl_r * rl_r,
                                                                       rl_a * rl_a, c->aev.cap_r, c->aev.cap_a, c->nbr_r, c->nbr_a, c->seg_r,

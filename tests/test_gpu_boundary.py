@@ -295,5 +295,30 @@ def test_buckets_of_more_than_32_atoms_are_ordered_too(model1):
         finally:
             nnp.nnp_destroy(ctx)
 
+@pytest.mark.gpu
+def test_cell_tiled_list_build_gives_the_defined_rows(model1, monkeypatch):
+    """The one-block-per-cell list kernel tests wrapped, image-shifted coordinates and hands the candidates inside a guard
+    band of a list radius to the defined fp32 predicate.  4096 waters, every atom moved by up to +-3 box lengths per
+    dimension (unwrapped MD coordinates: the wrapped values then carry the rounding of the larger numbers): the rows of
+    both kernels equal the oracle's fp32-predicate rows, with and without a skin."""
+    consts, widths, params, om = model1
+    sp, xyz, box = inputs.water_box(4096)
+    rng = np.random.default_rng(11)
+    xyz = (xyz + rng.integers(-3, 4, size=xyz.shape) * box).astype(np.float32).astype(np.float64)
+    n = len(sp)
+    for skin in (0.0, 0.5):
+        want = [orc.neighbors(xyz, box, float(np.float32(rc) + np.float32(skin)), fp32_pred=True) for rc in (5.1, 3.5)]
+        for tile in ("1", "0"):
+            monkeypatch.setenv("NNP_LIST_TILE", tile)
+            ctx = U.gpu_create(consts, widths, params, 1, n)
+            try:
+                U.gpu_energy_forces(ctx, sp, xyz, box, skin=skin)
+                for which in (0, 1):
+                    got = U.gpu_neighbors(ctx, which, n, stride=160)
+                    bad = [i for i in range(n) if not np.array_equal(got[i], want[which][i])]
+                    assert not bad, (tile, skin, which, len(bad), bad[:5])
+            finally:
+                nnp.nnp_destroy(ctx)
+
 
 
