@@ -237,6 +237,27 @@ int nnp_aev_ladder(const nnp_ctx *ctx);
 #define NNP_N_PEAKS 13
 int nnp_measure_peaks(int device, double *h_out);
 
+/* Neighbour lists without any allocation (csrc/no_alloc.cu), for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it.  The cell-list build of stage 1 for ONE point
+ * set: for every atom i the set {j != i : r_ij < rcut} under the minimum image of an orthorhombic box, membership decided by
+ * the same fp32 predicate as nnp_build_neighbors (reading A3) - the rows equal those of nnp_get_neighbors for the
+ * same radius.  Needs no ctx, calls no cudaMalloc / cudaFree and no allocating library routine, does not synchronise: it
+ * enqueues one memset and four kernels on `cuda_stream` (a cudaStream_t, NULL = default stream) of the CURRENT device.
+ *   n_atoms   <= NNP_NO_ALLOC_MAX_ATOMS (else NNP_EINVAL, message in nnp_neighbors_no_alloc_error()); 0 is a no-op
+ *   d_xyz     device, [n_atoms][3] fp32, any image of the atoms (wrapped internally)
+ *   h_box     host, 3 edge lengths; NULL or all zero: not periodic (all pairs are tested).  NNP_EBOX if an edge < 2 rcut
+ *   d_counts  device, [n_atoms] int32: number of neighbours of atom i (the full count, also where it exceeds `stride`)
+ *   d_list    device, [n_atoms][stride] int32: the neighbours of atom i, unsorted; entries beyond min(count, stride) untouched
+ * All buffers are the caller's; nothing is retained.  The scratch memory (positions as float4, cell keys, the order by
+ * cell, the cell histogram and start table: ~450 KiB) is ONE array in the library image, held by every GPU that loads the
+ * library until the process exits, and shared by all calls: calls that overlap on one GPU (two streams, concurrent graph
+ * launches) race on it - serialise them.  The first call on a device looks up the array's device address
+ * (cudaGetSymbolAddress): make that call outside a stream capture. */
+#define NNP_NO_ALLOC_MAX_ATOMS 16384
+int nnp_neighbors_no_alloc(int n_atoms, const float *d_xyz, const float h_box[3], float rcut, int32_t *d_counts,
+                           int32_t *d_list, int stride, void *cuda_stream);
+const char *nnp_neighbors_no_alloc_error(void); /* message of the calling thread's last failed nnp_neighbors_no_alloc */
+
 #ifdef __cplusplus
 }
 #endif

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnnp_b200.so")
-SOURCES = ["nnp_api.cu", "neighbor.cu", "aev.cu", "mlp_simt.cu", "mlp_tc.cu", "mlp_fused.cu", "integrate.cu", "peaks.cu"]
+SOURCES = ["nnp_api.cu", "neighbor.cu", "aev.cu", "mlp_simt.cu", "mlp_tc.cu", "mlp_fused.cu", "integrate.cu", "peaks.cu", "no_alloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "--use_fast_math=false"]

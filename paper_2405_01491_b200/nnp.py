@@ -23,7 +23,7 @@ EXPORTS = ["nnp_create", "nnp_destroy", "nnp_last_error", "nnp_set_system", "nnp
            "nnp_get_atomic_energies", "nnp_md_init", "nnp_md_step", "nnp_get_state", "nnp_sync",
            "nnp_energy_forces_host", "nnp_md_step_host", "nnp_profile", "nnp_profile_read", "nnp_launch_count",
            "nnp_aev_len", "nnp_aev_active_columns", "nnp_aev_ladder", "nnp_md_set_langevin", "nnp_energy_forces_virial",
-           "nnp_measure_peaks"]
+           "nnp_measure_peaks", "nnp_neighbors_no_alloc", "nnp_neighbors_no_alloc_error"]
 
 
 class NnpError(RuntimeError):
@@ -91,6 +91,9 @@ def lib():
         L.nnp_md_set_langevin.argtypes = [vp, C.c_float, C.c_float, C.c_uint64]
         L.nnp_energy_forces_virial.argtypes = [vp, dp, fp, dp]
         L.nnp_measure_peaks.argtypes = [C.c_int, dp]
+        L.nnp_neighbors_no_alloc.argtypes = [C.c_int, fp, C.POINTER(C.c_float), C.c_float, ip, ip, C.c_int, vp]
+        L.nnp_neighbors_no_alloc_error.argtypes = []
+        L.nnp_neighbors_no_alloc_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -278,3 +281,21 @@ def nnp_measure_peaks(device=0):
     if rc != NNP_OK:
         raise RuntimeError("nnp_measure_peaks failed with status %d" % rc)
     return dict(zip(PEAK_NAMES, (float(v) for v in out)))
+
+
+NNP_NO_ALLOC_MAX_ATOMS = 16384
+
+
+def nnp_neighbors_no_alloc_error():
+    return (lib().nnp_neighbors_no_alloc_error() or b"").decode()
+
+
+def nnp_neighbors_no_alloc(n_atoms, d_xyz, box, rcut, d_counts, d_list, stride, stream=None):
+    """Neighbour lists of one point set with the scratch memory in the library's static device array (include/nnp.h):
+    no ctx, no allocation, no synchronisation.  box: 3 edge lengths or None (not periodic)."""
+    b = None if box is None else (C.c_float * 3)(*[float(x) for x in box])
+    rc = lib().nnp_neighbors_no_alloc(int(n_atoms), _ptr(d_xyz), b, float(rcut), _ptr(d_counts), _ptr(d_list), int(stride),
+                                      stream)
+    if rc != NNP_OK:
+        raise NnpError(rc, nnp_neighbors_no_alloc_error())
+    return rc
