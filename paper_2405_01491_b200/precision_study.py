@@ -9,11 +9,17 @@ bf16 ("default"), TF32 ("high"), fp32 ("highest") and fp64, and finds that only 
 on a seeded 216-water box with seeded random-init weights (the paper's trained ANI-2x weights are not available, so the
 comparison is qualitative: which modes conserve energy, not the paper's absolute numbers).
 
-  python -m paper_2405_01491_b200.precision_study [--steps 4000] [--dt 0.1] [--scale 66] [--waters 216]
+  python -m paper_2405_01491_b200.precision_study [--steps 3000] [--repeats 3] [--dt 0.1] [--scale 66] [--waters 216]
 
-Prints one markdown table row per mode: maximum |E_tot(t) - E_tot(0)|, the linear drift over the run, the shift of the
-initial total energy against the fp64 leg (Fig. 3's second criterion), all relative to the mean kinetic energy of the run
-(the quantity Fig. 3 plots against), and the final kinetic temperature.
+Prints one markdown table row per mode: maximum |E_tot(t) - E_tot(0)| (median and worst of the repeats), the linear drift over
+the run, the median change of E_tot per sampling interval, the shift of the initial total energy against the fp64 leg
+(Fig. 3's second criterion), all relative to the mean kinetic energy of the second half of the run (the quantity Fig. 3
+plots against), and the final kinetic temperature.
+The window is 0.3 ps by default on purpose.  The random-weight model is not a bound liquid: at 0.43 ps two hydrogens of the
+seeded box pass within 0.035 A of each other, and the integration error of that unphysical geometry (a transient of 1e-5 ..
+2e-4 <E_kin>, the same in every mode, fp64 included) then decides the maximum; repeats of one mode differ there by a factor
+of ten because the order of the force reductions differs from run to run and the trajectories have diverged by then.
+Before it the repeats of a mode agree to ~30 %.
 Needs a GPU and the built library; nothing here touches the oracle.
 """
 import argparse
@@ -52,7 +58,7 @@ def run_mode(mm_mode, args):
         t = np.arange(len(etot)) * args.every * args.dt
         ke = ekin[len(ekin) // 2:].mean()
         drift = np.polyfit(t, etot, 1)[0] * t[-1]
-        return dict(max_dev=np.abs(etot - etot[0]).max() / ke, drift=drift / ke,
+        return dict(max_dev=np.abs(etot - etot[0]).max() / ke, drift=drift / ke, step_med=np.median(np.abs(np.diff(etot))) / ke,
                     T_end=2 * ekin[-1] / (3 * n * inputs.KB), ke=ke, e0=etot[0])
     finally:
         nnp.nnp_destroy(ctx)
@@ -60,7 +66,8 @@ def run_mode(mm_mode, args):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--steps", type=int, default=4000)
+    ap.add_argument("--steps", type=int, default=3000)
+    ap.add_argument("--repeats", type=int, default=3)
     ap.add_argument("--every", type=int, default=20)
     ap.add_argument("--dt", type=float, default=0.1)
     ap.add_argument("--waters", type=int, default=216)
@@ -69,16 +76,18 @@ def main():
     from . import inputs
     if args.scale is None:
         args.scale = inputs.FORCE_SCALE_WATER
-    print("| matmul mode | max |dE_tot| / <E_kin> | drift over run / <E_kin> | E_tot(0) - E_tot(0)[fp64] / <E_kin> | T_end [K] |")
-    print("|---|---:|---:|---:|---:|")
+    print("| matmul mode | max |dE_tot| / <E_kin>: median (worst) of %d runs | drift over run / <E_kin> | median |dE_tot| per %d steps / <E_kin> "
+          "| E_tot(0) - E_tot(0)[fp64] / <E_kin> | T_end [K] |" % (args.repeats, args.every))
+    print("|---|---:|---:|---:|---:|---:|")
     ref = None
     for mode, name in ((3, "fp64-accumulate SIMT"), (0, "fp32 SIMT"), (1, "3xTF32 tcgen05"), (4, "3xF16 fused tcgen05 (default)"),
                        (2, "TF32 tcgen05")):
-        r = run_mode(mode, args)
+        rs = [run_mode(mode, args) for _ in range(args.repeats)]
+        med = lambda k: float(np.median([r[k] for r in rs]))  # noqa: E731
         if ref is None:
-            ref = r
-        print("| %s | %.2e | %+.2e | %+.2e | %.0f |" % (name, r["max_dev"], r["drift"], (r["e0"] - ref["e0"]) / ref["ke"], r["T_end"]),
-              flush=True)
+            ref = dict(e0=med("e0"), ke=med("ke"))
+        print("| %s | %.2e (%.2e) | %+.2e | %.2e | %+.2e | %.0f |" % (name, med("max_dev"), max(r["max_dev"] for r in rs), med("drift"),
+                                                                 med("step_med"), (med("e0") - ref["e0"]) / ref["ke"], med("T_end")), flush=True)
 
 
 if __name__ == "__main__":
